@@ -1,0 +1,135 @@
+/* mk.h — C ABI of libmk: the synthesis hot path of the iterative Neumann-series Marchenko method
+ * (arXiv 2106.04649) as hand-written sm_100a CUDA kernels.  One GPU, one context per reflection response.
+ *
+ * Citations: "PAPER.md:N" = /root/reference/PAPER.md line N; "§8" = SURVEY.md section 8; G1..G14 = the
+ * readings of the paper listed in DESIGN.md.
+ *
+ * What the library computes (notation of §8):
+ *   n = nshot = nrec (co-located fixed spread); time index j in [0, nt), negative times stored wrapped
+ *   (T f)[j] = f[(nt - j) % nt];  band B = {klo..khi} = {k : fmin <= k/(nt dt) <= fmax};  w[s] trapezoid weights
+ *   synthesis  (R N)[f][r][j] = P_B { dt * sum_s w[s] * sum_j' R[s][r][(j - j') % nt] * N[f][s][j'] }      eq. (1)
+ *   window     Theta[f][r][j] = ( |j+-| < h ),  h = clamp(floor(t_d/dt + 0.5) - eps, 0, nt/2)               PAPER.md:24, G2
+ *   one step   N_i = - Theta T R N_{i-1},   N_{-1} = T G_d
+ *   f1plus = N_{-1} + sum_{i odd} N_i ;  f1min = - sum_{i even} T N_i ;  p^- = sum_i R N_{i-1}
+ *   G^- = R f1plus - f1min ;  G^+ = T f1plus - R (T f1min) ;  G = p^- + T f1plus - f1min                    PAPER.md:24, 87-88, G3-G5
+ * The time convolution runs in the frequency domain: per bin k in B a complex contraction of
+ * R^[r][k][s] over source positions s against N^[s][k][f] — a streaming GEMV for few focal points, a batched
+ * complex GEMM for many.
+ *
+ * Conventions for every entry point
+ *   - returns int: MK_OK (0) or a negative MK_ERR_* code; never throws or aborts across the ABI;
+ *     mk_last_error(ctx) returns a NUL-terminated description of the last failure on that context.
+ *   - "d_" arguments are DEVICE pointers owned by the caller (allocated e.g. with PyTorch), 16-byte aligned;
+ *     "h_" arguments are HOST pointers owned by the caller (pinned memory makes the copies asynchronous).
+ *     The library never frees or retains caller buffers beyond the call (work is stream-ordered: a d_ buffer
+ *     may be reused once the context's stream has reached the end of the call).
+ *   - the library owns R^ (band-limited complex64 reflection response), its accumulators and workspaces.
+ *   - all work is enqueued on the context's stream (the legacy default stream until mk_set_stream).
+ *     d_-pointer calls do not synchronise the host; h_-pointer calls return after the results are in host memory.
+ *   - there is no CPU fallback: without a CUDA device mk_create fails with MK_ERR_CUDA.
+ */
+#ifndef MK_H_
+#define MK_H_
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct mk_ctx mk_ctx; /* opaque */
+
+enum {
+  MK_OK = 0,
+  MK_ERR_INVALID_ARG = -1, /* NULL pointer, non-positive size, nshot != nrec, nt not a power of two, ... */
+  MK_ERR_STATE = -2,       /* mk_run before every shot was loaded, mk_step before mk_begin, ... */
+  MK_ERR_OOM = -3,         /* device allocation failed */
+  MK_ERR_CUDA = -4         /* a CUDA call failed (sticky; text in mk_last_error) */
+};
+
+/* mk_set_option keys */
+enum {
+  MK_OPT_EPS_SAMPLES = 1, /* window margin eps in samples (default 8; BASELINE.json config 0; G2) */
+  MK_OPT_REGIME = 2,      /* contraction kernel: 0 auto (default), 1 streaming GEMV, 2 FP32-FFMA GEMM,
+                             3 tcgen05 3xTF32 GEMM (only where available; MK_ERR_INVALID_ARG otherwise) */
+  MK_OPT_TIMING = 3       /* 1: bracket every contraction launch with CUDA events on the context's stream */
+};
+
+/* mk_get_info keys (values returned as double) */
+enum {
+  MK_INFO_NB = 1,            /* number of bins in B */
+  MK_INFO_KLO = 2,           /* first bin of B */
+  MK_INFO_KHI = 3,           /* last bin of B */
+  MK_INFO_RHAT_BYTES = 4,    /* algorithmic bytes of R^: 8 * nrec * nb * nshot (unpadded) */
+  MK_INFO_RHAT_BYTES_PADDED = 5,
+  MK_INFO_LD_SHOT = 6,       /* padded shot dimension of R^ (multiple of 16 elements = 128 B) */
+  MK_INFO_SHOTS_LOADED = 7,
+  MK_INFO_SYN_LAUNCHES = 8,  /* contraction launches timed since the last MK_INFO_SYN_RESET (needs MK_OPT_TIMING) */
+  MK_INFO_SYN_MS_TOTAL = 9,  /* their summed device time in ms (synchronises the stream) */
+  MK_INFO_SYN_RESET = 10,    /* resets the two counters above; value returned is 0 */
+  MK_INFO_KERNEL_LAUNCHES = 11, /* total kernels this context has launched since creation */
+  MK_INFO_REGIME_USED = 12,  /* regime of the last contraction launch (1, 2 or 3) */
+  MK_INFO_DEVICE_BYTES = 13  /* device memory currently owned by the context */
+};
+
+/* Create a context for an nshot x nrec x nt reflection response sampled at dt (s) and dx (m), band fmin..fmax (Hz).
+ * Validates nshot == nrec > 0 (G10: co-located spread; the output index of one iteration is the integration
+ * index of the next), nt a power of two in [16, 65536], dt, dx > 0, 0 <= fmin <= fmax <= 1/(2 dt).
+ * Allocates R^ [nrec][nb][ld_shot] complex64 on the current CUDA device (BASELINE.json north_star (a)
+ * "the data layout is ordered as receivers, frequencies and shots").  *out receives the context. */
+int mk_create(mk_ctx** out, int nshot, int nrec, int nt, double dt, double dx, double fmin, double fmax);
+
+/* Frees everything the context owns.  NULL is accepted. */
+int mk_destroy(mk_ctx* ctx);
+
+/* cuda_stream: a cudaStream_t (e.g. torch.cuda.current_stream().cuda_stream); NULL = legacy default stream. */
+int mk_set_stream(mk_ctx* ctx, void* cuda_stream);
+
+int mk_set_option(mk_ctx* ctx, int key, double value);
+int mk_get_info(mk_ctx* ctx, int key, double* value);
+
+/* Ingest ("the whole reflection data being read, Fourier transformed and stored", 63-66; §8(a) a0).
+ * d_R_time: [nshots][nrec][nt] fp32 time-domain R(x_R = rec, x = shot, t) for shots shot0 .. shot0+nshots-1.
+ * Converted on the GPU, once, to band-limited complex64 with the quadrature weights folded in:
+ *   R^[r][k][s] = dt * w[s] * sum_j R[s][r][j] e^{-2 pi i k j / nt},  k in B  (shot index fastest, zero padded to ld_shot).
+ * May be called repeatedly with disjoint shot ranges (config 4: 61 calls of 64 shots). */
+int mk_load_R(mk_ctx* ctx, const float* d_R_time, int shot0, int nshots);
+/* Same from a HOST buffer: staged through an internal device buffer in bounded chunks; returns when done. */
+int mk_load_R_host(mk_ctx* ctx, const float* h_R_time, int shot0, int nshots);
+
+/* Outputs of a run; each pointer is [nfoc][nrec][nt] fp32 or NULL to skip that field.  G^- and G^+ cost one
+ * extra synthesis each ("estimating each component requires an extra synthesis"). */
+typedef struct mk_outputs {
+  float* N_last; /* N_{niter-1} */
+  float* f1plus;
+  float* f1min;
+  float* G;
+  float* Gplus;
+  float* Gminus;
+} mk_outputs;
+
+/* The whole scheme (Algorithm 1) for nfoc focal points:
+ * d_Gd [nfoc][nrec][nt] fp32 first arrivals G_d(x_R, x_F, t), d_td [nfoc][nrec] fp32 traveltimes in seconds.
+ * Equals mk_begin + niter x mk_step + mk_finish.  MK_ERR_STATE unless all nshot shots have been loaded. */
+int mk_run(mk_ctx* ctx, const float* d_Gd, const float* d_td, int nfoc, int niter, const mk_outputs* d_out);
+/* Same with HOST inputs and HOST outputs (copies in, runs, copies out, synchronises). */
+int mk_run_host(mk_ctx* ctx, const float* h_Gd, const float* h_td, int nfoc, int niter, const mk_outputs* h_out);
+
+/* Step access (same arithmetic; used by the parity tests to see every iterate). */
+int mk_begin(mk_ctx* ctx, const float* d_Gd, const float* d_td, int nfoc); /* a1: N_{-1} = f1plus = T G_d, f1min = p^- = 0 */
+int mk_step(mk_ctx* ctx, float* d_N_i /* optional [nfoc][nrec][nt] copy of the new iterate, or NULL */); /* a2..a6 */
+int mk_finish(mk_ctx* ctx, const mk_outputs* d_out); /* a7; may be called more than once with different fields */
+
+/* One bare synthesis without window (a6 + a2 + a3): d_S_out = R d_N_in, both [nfoc][nrec][nt] fp32.
+ * Does not disturb a run in progress.  This is the call the GB/s metric times. */
+int mk_synthesis(mk_ctx* ctx, const float* d_N_in, float* d_S_out, int nfoc);
+
+/* NEXT-1 (§8(f)): double-focusing image, image[f] = zero-time sample of sum_r w[r] (G^- conv f1plus)(x_F, x_F)
+ * (PAPER.md:24, 89).  d_image: [nfoc] fp32.  Requires a finished run. */
+int mk_image(mk_ctx* ctx, float* d_image);
+
+const char* mk_last_error(mk_ctx* ctx);
+const char* mk_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* MK_H_ */

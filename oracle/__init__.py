@@ -1,0 +1,142 @@
+"""ctypes front of the fp64 CPU oracle (oracle/marchenko_oracle.cpp) — TEST INFRASTRUCTURE ONLY.
+
+Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference leg may import this.
+Argument marshalling only; every number comes from the C++ file.  It imports nothing from the CUDA
+package (paper_2106_04649_b200.binding / csrc) and shares no code with it.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+import subprocess
+from pathlib import Path
+
+import numpy as np
+
+_HERE = Path(__file__).resolve().parent
+_SRC = _HERE / "marchenko_oracle.cpp"
+_LIB = _HERE / "libmarchenko_oracle.so"
+_lib = None
+
+
+def build(force: bool = False) -> Path:
+    """g++ -O2 -fopenmp; no fast-math, no FFT library, nothing but libstdc++/libgomp."""
+    if force or not _LIB.exists() or _LIB.stat().st_mtime < _SRC.stat().st_mtime:
+        cmd = ["g++", "-O3", "-mavx2", "-fopenmp", "-std=c++17", "-shared", "-fPIC",
+               "-ffp-contract=off", str(_SRC), "-o", str(_LIB)]
+        subprocess.check_call(cmd)
+    return _LIB
+
+
+_F32 = np.ctypeslib.ndpointer(dtype=np.float32, flags="C_CONTIGUOUS")
+_F64 = np.ctypeslib.ndpointer(dtype=np.float64, flags="C_CONTIGUOUS")
+_I32 = np.ctypeslib.ndpointer(dtype=np.int32, flags="C_CONTIGUOUS")
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        build()
+        L = C.CDLL(str(_LIB))
+        L.orc_num_threads.restype = C.c_int
+        L.orc_band.restype = C.c_int
+        L.orc_band.argtypes = [C.c_int, C.c_double, C.c_double, C.c_double, C.POINTER(C.c_int), C.POINTER(C.c_int)]
+        L.orc_weights.argtypes = [C.c_int, C.c_double, _F64]
+        L.orc_band_kernel.argtypes = [C.c_int, C.c_int, C.c_int, _F64]
+        L.orc_apply_band.argtypes = [C.c_int, _F64, _F64, _F64]
+        L.orc_window.argtypes = [C.c_int, C.c_int, C.c_double, C.c_int, _F32, _I32]
+        L.orc_theta.restype = C.c_int
+        L.orc_theta.argtypes = [C.c_int, C.c_int, C.c_int]
+        L.orc_synthesis.argtypes = [C.c_int, C.c_int, C.c_int, C.c_double, _F64, _F32, C.c_int, _F64, C.c_int,
+                                    C.c_int, _F64]
+        L.orc_marchenko.restype = C.c_int
+        L.orc_marchenko.argtypes = [C.c_int, C.c_int, C.c_double, C.c_double, C.c_double, C.c_double, C.c_int,
+                                    _F32, C.c_int, _F32, _F32, C.c_int] + [C.c_void_p] * 8
+        _lib = L
+    return _lib
+
+
+def num_threads() -> int:
+    return int(lib().orc_num_threads())
+
+
+def band(nt: int, dt: float, fmin: float, fmax: float):
+    """(klo, khi, nb) of the band B (reading G8)."""
+    lo, hi = C.c_int(), C.c_int()
+    nb = lib().orc_band(nt, dt, fmin, fmax, C.byref(lo), C.byref(hi))
+    return lo.value, hi.value, nb
+
+
+def weights(n: int, dx: float) -> np.ndarray:
+    w = np.empty(n, dtype=np.float64)
+    lib().orc_weights(n, dx, w)
+    return w
+
+
+def band_kernel(nt: int, klo: int, khi: int) -> np.ndarray:
+    b = np.empty(nt, dtype=np.float64)
+    lib().orc_band_kernel(nt, klo, khi, b)
+    return b
+
+
+def apply_band(b: np.ndarray, x: np.ndarray) -> np.ndarray:
+    x = np.ascontiguousarray(x, dtype=np.float64)
+    y = np.empty_like(x)
+    lib().orc_apply_band(len(x), np.ascontiguousarray(b, dtype=np.float64), x, y)
+    return y
+
+
+def window(td: np.ndarray, nt: int, dt: float, eps: int) -> np.ndarray:
+    """h[...] int32 window half-widths from fp32 traveltimes (O3)."""
+    td = np.ascontiguousarray(td, dtype=np.float32)
+    h = np.empty(td.shape, dtype=np.int32)
+    lib().orc_window(td.size, nt, dt, eps, td.reshape(-1), h.reshape(-1))
+    return h
+
+
+def theta(nt: int, h: int) -> np.ndarray:
+    L = lib()
+    return np.array([L.orc_theta(nt, int(h), j) for j in range(nt)], dtype=np.float64)
+
+
+def synthesis(R: np.ndarray, N: np.ndarray, dt: float, w: np.ndarray, klo: int, khi: int) -> np.ndarray:
+    """S[f][r][:] = P_B{dt sum_s w[s] R[s][r] (*) N[f][s]} (O5a).  R: [nshot][nrout][nt] fp32, N: [nfoc][nshot][nt]."""
+    R = np.ascontiguousarray(R, dtype=np.float32)
+    N = np.ascontiguousarray(N, dtype=np.float64)
+    nshot, nrout, nt = R.shape
+    nfoc = N.shape[0]
+    assert N.shape == (nfoc, nshot, nt)
+    S = np.empty((nfoc, nrout, nt), dtype=np.float64)
+    lib().orc_synthesis(nshot, nrout, nt, dt, np.ascontiguousarray(w, dtype=np.float64), R, nfoc, N, klo, khi, S)
+    return S
+
+
+def marchenko(R: np.ndarray, Gd: np.ndarray, td: np.ndarray, dt: float, dx: float, fmin: float, fmax: float,
+              niter: int, eps: int = 8, keep_iters: bool = True, want=("f1plus", "f1min", "f2", "pmin", "G", "Gplus",
+                                                                        "Gminus")):
+    """The whole scheme (O4..O6).  Returns a dict of float64 arrays [nfoc][n][nt] (+ 'N_iters' [niter][nfoc][n][nt])."""
+    R = np.ascontiguousarray(R, dtype=np.float32)
+    Gd = np.ascontiguousarray(Gd, dtype=np.float32)
+    td = np.ascontiguousarray(td, dtype=np.float32)
+    n, n2, nt = R.shape
+    assert n == n2
+    nfoc = Gd.shape[0]
+    assert Gd.shape == (nfoc, n, nt) and td.shape == (nfoc, n)
+    out = {}
+    names = ["f1plus", "f1min", "f2", "pmin", "G", "Gplus", "Gminus"]
+    ptrs = []
+    if keep_iters:
+        out["N_iters"] = np.empty((niter, nfoc, n, nt), dtype=np.float64)
+        ptrs.append(out["N_iters"].ctypes.data_as(C.c_void_p))
+    else:
+        ptrs.append(None)
+    for nm in names:
+        if nm in want:
+            out[nm] = np.empty((nfoc, n, nt), dtype=np.float64)
+            ptrs.append(out[nm].ctypes.data_as(C.c_void_p))
+        else:
+            ptrs.append(None)
+    rc = lib().orc_marchenko(n, nt, dt, dx, fmin, fmax, eps, R.reshape(-1), nfoc, Gd.reshape(-1), td.reshape(-1),
+                             niter, *ptrs)
+    assert rc == 0
+    return out
