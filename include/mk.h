@@ -72,9 +72,11 @@ enum {
 
 /* Create a context for an nshot x nrec x nt reflection response sampled at dt (s) and dx (m), band fmin..fmax (Hz).
  * Validates nshot == nrec > 0 (G10: co-located spread; the output index of one iteration is the integration
- * index of the next), nt a power of two in [16, 65536], dt, dx > 0, 0 <= fmin <= fmax <= 1/(2 dt).
+ * index of the next), nt a power of two in [16, 32768], dt, dx > 0, 0 <= fmin <= fmax <= 1/(2 dt).
  * Allocates R^ [nrec][nb][ld_shot] complex64 on the current CUDA device (BASELINE.json north_star (a)
- * "the data layout is ordered as receivers, frequencies and shots").  *out receives the context. */
+ * "the data layout is ordered as receivers, frequencies and shots").  *out receives the context; when a failure
+ * happens after the context exists, *out is still set so that mk_last_error can be read (destroy it afterwards),
+ * otherwise *out is NULL. */
 int mk_create(mk_ctx** out, int nshot, int nrec, int nt, double dt, double dx, double fmin, double fmax);
 
 /* Frees everything the context owns.  NULL is accepted. */
@@ -98,7 +100,7 @@ int mk_load_R_host(mk_ctx* ctx, const float* h_R_time, int shot0, int nshots);
 /* Outputs of a run; each pointer is [nfoc][nrec][nt] fp32 or NULL to skip that field.  G^- and G^+ cost one
  * extra synthesis each ("estimating each component requires an extra synthesis"). */
 typedef struct mk_outputs {
-  float* N_last; /* N_{niter-1} */
+  float* N_last; /* N_{niter-1}; honoured by mk_run / mk_run_host only (mk_finish rejects it: use mk_step's d_N_i) */
   float* f1plus;
   float* f1min;
   float* G;
@@ -122,9 +124,10 @@ int mk_finish(mk_ctx* ctx, const mk_outputs* d_out); /* a7; may be called more t
  * Does not disturb a run in progress.  This is the call the GB/s metric times. */
 int mk_synthesis(mk_ctx* ctx, const float* d_N_in, float* d_S_out, int nfoc);
 
-/* NEXT-1 (§8(f)): double-focusing image, image[f] = zero-time sample of sum_r w[r] (G^- conv f1plus)(x_F, x_F)
- * (PAPER.md:24, 89).  d_image: [nfoc] fp32.  Requires a finished run. */
-int mk_image(mk_ctx* ctx, float* d_image);
+/* NEXT-1 (§8(f)): double-focusing image: the zero-time sample of G^- convolved with f1plus and
+ * integrated over receivers,  image[f] = dt * sum_r w[r] sum_j G^-[f][r][(nt-j)%nt] * f1plus[f][r][j].
+ * d_Gminus: [nfoc][nrec][nt] fp32 as returned by mk_run / mk_finish for the current run; d_image: [nfoc] fp32. */
+int mk_image(mk_ctx* ctx, const float* d_Gminus, float* d_image);
 
 const char* mk_last_error(mk_ctx* ctx);
 const char* mk_version(void);

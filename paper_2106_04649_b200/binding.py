@@ -1,0 +1,226 @@
+"""Thin ctypes binding of libmk.so (include/mk.h) — same names, argument marshalling only.
+
+PyTorch is used for device memory and streams; every step of the path runs in the CUDA kernels of
+libmk.  There is no CPU fallback: if the library is missing or no CUDA device is present, loading or
+`Marchenko(...)` raises.
+"""
+from __future__ import annotations
+
+import ctypes as C
+from pathlib import Path
+
+_HERE = Path(__file__).resolve().parent
+LIB_PATH = _HERE / "libmk.so"
+
+MK_OK, MK_ERR_INVALID_ARG, MK_ERR_STATE, MK_ERR_OOM, MK_ERR_CUDA = 0, -1, -2, -3, -4
+MK_OPT_EPS_SAMPLES, MK_OPT_REGIME, MK_OPT_TIMING = 1, 2, 3
+(MK_INFO_NB, MK_INFO_KLO, MK_INFO_KHI, MK_INFO_RHAT_BYTES, MK_INFO_RHAT_BYTES_PADDED, MK_INFO_LD_SHOT,
+ MK_INFO_SHOTS_LOADED, MK_INFO_SYN_LAUNCHES, MK_INFO_SYN_MS_TOTAL, MK_INFO_SYN_RESET, MK_INFO_KERNEL_LAUNCHES,
+ MK_INFO_REGIME_USED, MK_INFO_DEVICE_BYTES) = range(1, 14)
+REGIME_AUTO, REGIME_GEMV, REGIME_GEMM_FFMA, REGIME_GEMM_TF32X3 = 0, 1, 2, 3
+
+# every symbol include/mk.h declares
+SYMBOLS = ("mk_create", "mk_destroy", "mk_set_stream", "mk_set_option", "mk_get_info", "mk_load_R", "mk_load_R_host",
+           "mk_run", "mk_run_host", "mk_begin", "mk_step", "mk_finish", "mk_synthesis", "mk_image", "mk_last_error",
+           "mk_version")
+
+
+class mk_outputs(C.Structure):
+    _fields_ = [(nm, C.c_void_p) for nm in ("N_last", "f1plus", "f1min", "G", "Gplus", "Gminus")]
+
+
+OUTPUT_FIELDS = tuple(nm for nm, _ in mk_outputs._fields_)
+
+
+class MkError(RuntimeError):
+    def __init__(self, code, msg):
+        super().__init__(f"libmk error {code}: {msg}")
+        self.code = code
+
+
+_lib = None
+
+
+def load():
+    """Loads libmk.so (raises if it has not been built: `python -m paper_2106_04649_b200.build`)."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not LIB_PATH.exists():
+        raise FileNotFoundError(f"{LIB_PATH} is missing — build it with `python -m paper_2106_04649_b200.build` "
+                                "(there is no CPU fallback)")
+    L = C.CDLL(str(LIB_PATH))
+    vp, ci, cd = C.c_void_p, C.c_int, C.c_double
+    L.mk_create.argtypes = [C.POINTER(vp), ci, ci, ci, cd, cd, cd, cd]
+    L.mk_destroy.argtypes = [vp]
+    L.mk_set_stream.argtypes = [vp, vp]
+    L.mk_set_option.argtypes = [vp, ci, cd]
+    L.mk_get_info.argtypes = [vp, ci, C.POINTER(cd)]
+    L.mk_load_R.argtypes = [vp, vp, ci, ci]
+    L.mk_load_R_host.argtypes = [vp, vp, ci, ci]
+    L.mk_run.argtypes = [vp, vp, vp, ci, ci, C.POINTER(mk_outputs)]
+    L.mk_run_host.argtypes = [vp, vp, vp, ci, ci, C.POINTER(mk_outputs)]
+    L.mk_begin.argtypes = [vp, vp, vp, ci]
+    L.mk_step.argtypes = [vp, vp]
+    L.mk_finish.argtypes = [vp, C.POINTER(mk_outputs)]
+    L.mk_synthesis.argtypes = [vp, vp, vp, ci]
+    L.mk_image.argtypes = [vp, vp, vp]
+    L.mk_last_error.argtypes = [vp]
+    L.mk_last_error.restype = C.c_char_p
+    L.mk_version.restype = C.c_char_p
+    for nm in SYMBOLS:
+        if nm not in ("mk_last_error", "mk_version"):
+            getattr(L, nm).restype = ci
+    _lib = L
+    return L
+
+
+def _dev_ptr(t, dtype=None, numel=None):
+    import torch
+    if t is None:
+        return None
+    if not (isinstance(t, torch.Tensor) and t.is_cuda and t.is_contiguous()):
+        raise TypeError("expected a contiguous CUDA tensor")
+    if dtype is not None and t.dtype != dtype:
+        raise TypeError(f"expected dtype {dtype}, got {t.dtype}")
+    if numel is not None and t.numel() != numel:
+        raise ValueError(f"expected {numel} elements, got {t.numel()}")
+    return C.c_void_p(t.data_ptr())
+
+
+def _host_ptr(a, numel=None):
+    """numpy array or CPU torch tensor (float32, contiguous) -> pointer."""
+    import numpy as np
+    import torch
+    if a is None:
+        return None
+    if isinstance(a, torch.Tensor):
+        if a.is_cuda or not a.is_contiguous() or a.dtype != torch.float32:
+            raise TypeError("expected a contiguous float32 CPU tensor")
+        n, p = a.numel(), a.data_ptr()
+    else:
+        if not (isinstance(a, np.ndarray) and a.dtype == np.float32 and a.flags.c_contiguous):
+            raise TypeError("expected a C-contiguous float32 numpy array")
+        n, p = a.size, a.ctypes.data
+    if numel is not None and n != numel:
+        raise ValueError(f"expected {numel} elements, got {n}")
+    return C.c_void_p(p)
+
+
+class Marchenko:
+    """One context = one reflection response resident in HBM (mk_create .. mk_destroy)."""
+
+    def __init__(self, nshot, nrec, nt, dt, dx, fmin, fmax, stream=None):
+        import torch
+        if not torch.cuda.is_available():
+            raise RuntimeError("libmk needs a CUDA device (there is no CPU fallback)")
+        self._L = load()
+        self._h = C.c_void_p()
+        self.nshot, self.nrec, self.nt = nshot, nrec, nt
+        rc = self._L.mk_create(C.byref(self._h), nshot, nrec, nt, dt, dx, fmin, fmax)
+        if rc != MK_OK:
+            msg = self._L.mk_last_error(self._h).decode() if self._h else "mk_create failed"
+            if self._h:
+                self._L.mk_destroy(self._h)
+                self._h = C.c_void_p()
+            raise MkError(rc, msg)
+        self.set_stream(torch.cuda.current_stream().cuda_stream if stream is None else stream)
+
+    # -- plumbing
+    def _check(self, rc):
+        if rc != MK_OK:
+            raise MkError(rc, self._L.mk_last_error(self._h).decode())
+
+    def close(self):
+        if getattr(self, "_h", None):
+            self._L.mk_destroy(self._h)
+            self._h = C.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *a):
+        self.close()
+
+    def set_stream(self, cuda_stream):
+        self._check(self._L.mk_set_stream(self._h, C.c_void_p(cuda_stream)))
+
+    def set_option(self, key, value):
+        self._check(self._L.mk_set_option(self._h, key, float(value)))
+
+    def get_info(self, key) -> float:
+        v = C.c_double()
+        self._check(self._L.mk_get_info(self._h, key, C.byref(v)))
+        return v.value
+
+    def _outs(self, outs, ptr, numel):
+        o = mk_outputs()
+        for nm, t in (outs or {}).items():
+            if nm not in OUTPUT_FIELDS:
+                raise KeyError(nm)
+            setattr(o, nm, ptr(t, numel=numel).value if t is not None else None)
+        return o
+
+    # -- the calls of include/mk.h
+    def load_R(self, d_R_time, shot0=0):
+        import torch
+        nshots = d_R_time.shape[0]
+        self._check(self._L.mk_load_R(self._h, _dev_ptr(d_R_time, torch.float32, nshots * self.nrec * self.nt), shot0, nshots))
+
+    def load_R_host(self, h_R_time, shot0=0):
+        nshots = h_R_time.shape[0]
+        self._check(self._L.mk_load_R_host(self._h, _host_ptr(h_R_time, nshots * self.nrec * self.nt), shot0, nshots))
+
+    def run(self, d_Gd, d_td, niter, outs):
+        import torch
+        nfoc = d_Gd.shape[0]
+        self._nfoc = nfoc
+        numel = nfoc * self.nrec * self.nt
+        o = self._outs(outs, lambda t, numel: _dev_ptr(t, torch.float32, numel), numel)
+        self._check(self._L.mk_run(self._h, _dev_ptr(d_Gd, torch.float32, numel), _dev_ptr(d_td, torch.float32, nfoc * self.nrec),
+                                   nfoc, niter, C.byref(o)))
+
+    def run_host(self, h_Gd, h_td, niter, outs):
+        nfoc = h_Gd.shape[0]
+        self._nfoc = nfoc
+        numel = nfoc * self.nrec * self.nt
+        o = self._outs(outs, lambda t, numel: _host_ptr(t, numel), numel)
+        self._check(self._L.mk_run_host(self._h, _host_ptr(h_Gd, numel), _host_ptr(h_td, nfoc * self.nrec), nfoc, niter, C.byref(o)))
+
+    def begin(self, d_Gd, d_td):
+        import torch
+        nfoc = d_Gd.shape[0]
+        self._nfoc = nfoc
+        self._check(self._L.mk_begin(self._h, _dev_ptr(d_Gd, torch.float32, nfoc * self.nrec * self.nt),
+                                     _dev_ptr(d_td, torch.float32, nfoc * self.nrec), nfoc))
+
+    def step(self, d_N_i=None):
+        import torch
+        self._check(self._L.mk_step(self._h, _dev_ptr(d_N_i, torch.float32, self._nfoc * self.nrec * self.nt) if d_N_i is not None else None))
+
+    def finish(self, outs):
+        import torch
+        numel = self._nfoc * self.nrec * self.nt
+        o = self._outs(outs, lambda t, numel: _dev_ptr(t, torch.float32, numel), numel)
+        self._check(self._L.mk_finish(self._h, C.byref(o)))
+
+    def synthesis(self, d_N_in, d_S_out):
+        import torch
+        nfoc = d_N_in.shape[0]
+        numel = nfoc * self.nrec * self.nt
+        self._check(self._L.mk_synthesis(self._h, _dev_ptr(d_N_in, torch.float32, numel), _dev_ptr(d_S_out, torch.float32, numel), nfoc))
+
+    def image(self, d_Gminus, d_image):
+        import torch
+        self._check(self._L.mk_image(self._h, _dev_ptr(d_Gminus, torch.float32, self._nfoc * self.nrec * self.nt),
+                                     _dev_ptr(d_image, torch.float32, self._nfoc)))
+
+
+def version() -> str:
+    return load().mk_version().decode()

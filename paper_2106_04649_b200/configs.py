@@ -47,15 +47,15 @@ class Config:
 # positive constant is a valid input; DESIGN.md "Input recipe" says how these were found.
 CONFIGS: Tuple[Config, ...] = (
     Config(name="tiny2d", k=0, n=101, dx=10.0, nt=512, dt=0.004, nlayers=3, refl="uniform03",
-           nfoc=1, focal="single:400", seed=SEED0 + 0, A_R=2.0),
+           nfoc=1, focal="single:400", seed=SEED0 + 0, A_R=0.6),
     Config(name="3GB_1foc", k=1, n=601, dx=10.0, nt=2048, dt=0.004, nlayers=8, refl="randsign025",
-           nfoc=1, focal="single:800", seed=SEED0 + 1, A_R=0.18),
+           nfoc=1, focal="single:800", seed=SEED0 + 1, A_R=0.125),
     Config(name="3GB_601foc", k=2, n=601, dx=10.0, nt=2048, dt=0.004, nlayers=8, refl="randsign025",
-           nfoc=601, focal="line:800", seed=SEED0 + 2, A_R=0.18, model_seed=SEED0 + 1),
+           nfoc=601, focal="line:800", seed=SEED0 + 2, A_R=0.125, model_seed=SEED0 + 1),
     Config(name="33GB_64foc", k=3, n=2001, dx=10.0, nt=2048, dt=0.004, nlayers=12, refl="randsign025",
-           nfoc=64, focal="grid8x8", seed=SEED0 + 3, A_R=0.07, noise_snr_db=40.0),
+           nfoc=64, focal="grid8x8", seed=SEED0 + 3, A_R=0.048, noise_snr_db=40.0),
     Config(name="250GB_256foc", k=4, n=3901, dx=5.0, nt=4096, dt=0.002, nlayers=16, refl="randsign025",
-           nfoc=256, focal="line256:800", seed=SEED0 + 4, A_R=0.066),
+           nfoc=256, focal="line256:800", seed=SEED0 + 4, A_R=0.058),
 )
 
 

@@ -1,0 +1,456 @@
+// mk_api.cu — the C ABI of include/mk.h: argument checks, device buffers, and the order of kernel launches.
+// No arithmetic of the method happens on the host: every step of SURVEY.md §8(a) is a kernel in
+// mk_fft_kernels.cu / mk_syn_gemv.cu / mk_syn_gemm.cu.  There is no CPU fallback.
+#include <algorithm>
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+
+#include "mk_internal.cuh"
+
+namespace mk {
+
+int set_err(mk_ctx* c, int code, const std::string& msg) {
+  if (c) c->err = msg;
+  return code;
+}
+
+int check_cuda(mk_ctx* c, cudaError_t e, const char* what) {
+  if (e == cudaSuccess) return MK_OK;
+  if (c) {
+    c->sticky = MK_ERR_CUDA;
+    c->err = std::string(what) + ": " + cudaGetErrorString(e);
+  }
+  return e == cudaErrorMemoryAllocation ? MK_ERR_OOM : MK_ERR_CUDA;
+}
+
+namespace {
+
+template <typename T>
+int ensure(mk_ctx* c, T** p, size_t* cap, size_t count, const char* what) {
+  if (*cap >= count && *p) return MK_OK;
+  if (*p) {
+    cudaFree(*p);
+    c->device_bytes -= *cap * sizeof(T);
+    *p = nullptr;
+    *cap = 0;
+  }
+  void* q = nullptr;
+  cudaError_t e = cudaMalloc(&q, count * sizeof(T));
+  if (e != cudaSuccess) {
+    cudaGetLastError();
+    char buf[160];
+    snprintf(buf, sizeof buf, "cudaMalloc(%s, %zu bytes) failed: %s", what, count * sizeof(T), cudaGetErrorString(e));
+    return set_err(c, MK_ERR_OOM, buf);
+  }
+  *p = static_cast<T*>(q);
+  *cap = count;
+  c->device_bytes += count * sizeof(T);
+  return MK_OK;
+}
+
+template <typename T>
+void release(mk_ctx* c, T** p, size_t* cap) {
+  if (*p) {
+    cudaFree(*p);
+    c->device_bytes -= *cap * sizeof(T);
+  }
+  *p = nullptr;
+  *cap = 0;
+}
+
+int resolve_regime(mk_ctx* c, int nfoc, int* regime) {
+  int r = c->regime;
+  if (r == 0) r = gemv_supported(c, nfoc) ? 1 : 2;
+  if (r == 1 && !gemv_supported(c, nfoc)) return set_err(c, MK_ERR_INVALID_ARG, "GEMV regime needs nfoc <= 8 and ld*nfoc*8 <= 96 KiB");
+  if (r == 3) return set_err(c, MK_ERR_INVALID_ARG, "tcgen05 3xTF32 regime is not built in this version");
+  if (r < 1 || r > 3) return set_err(c, MK_ERR_INVALID_ARG, "unknown regime");
+  *regime = r;
+  return MK_OK;
+}
+
+inline int ldf_for(int regime, int nfoc) { return regime == 1 ? nfoc : ((nfoc + 3) / 4) * 4; }
+
+// a2: S^ = R^ x N^ per bin, on the context's stream; optionally bracketed by events
+int contract(mk_ctx* c, const float2* Nhat, float2* Shat, int nfoc, int ldf, int regime) {
+  cudaEvent_t e0 = nullptr, e1 = nullptr;
+  if (c->timing) {
+    if (c->ev_used + 2 > c->ev.size()) {
+      if (c->ev.size() >= 16384) return set_err(c, MK_ERR_STATE, "timing event pool exhausted; read MK_INFO_SYN_MS_TOTAL / reset");
+      for (int i = 0; i < 2; ++i) {
+        cudaEvent_t e;
+        if (int rc = check_cuda(c, cudaEventCreate(&e), "cudaEventCreate")) return rc;
+        c->ev.push_back(e);
+      }
+    }
+    e0 = c->ev[c->ev_used];
+    e1 = c->ev[c->ev_used + 1];
+    c->ev_used += 2;
+    cudaEventRecord(e0, c->stream);
+  }
+  int rc = regime == 1 ? launch_syn_gemv(c, Nhat, Shat, nfoc) : launch_syn_gemm(c, Nhat, Shat, ldf);
+  if (c->timing) cudaEventRecord(e1, c->stream);
+  c->regime_used = regime;
+  return rc;
+}
+
+bool is_pow2(int v) { return v > 0 && (v & (v - 1)) == 0; }
+
+__global__ void k_image(const float* __restrict__ Gminus, const float* __restrict__ f1plus, float* __restrict__ image, int n, int nt,
+                        float w_mid, float w_end) {
+  // image[f] = dt * sum_r w[r] sum_j G^-[f][r][(nt-j)%nt] f1plus[f][r][j]: zero-time sample of the convolution  [PAPER.md:24, 89]
+  const int f = blockIdx.x;
+  double acc = 0.0;
+  for (int r = 0; r < n; ++r) {
+    const float* g = Gminus + ((size_t)f * n + r) * nt;
+    const float* p = f1plus + ((size_t)f * n + r) * nt;
+    float part = 0.f;
+    for (int j = threadIdx.x; j < nt; j += blockDim.x) part = fmaf(g[(nt - j) & (nt - 1)], p[j], part);
+    const float w = (n > 1 && (r == 0 || r == n - 1)) ? w_end : w_mid;
+    acc += (double)(w * part);
+  }
+  __shared__ double red[256];
+  red[threadIdx.x] = acc;
+  __syncthreads();
+  for (int s = 128; s > 0; s >>= 1) {
+    if ((int)threadIdx.x < s) red[threadIdx.x] += red[threadIdx.x + s];
+    __syncthreads();
+  }
+  if (threadIdx.x == 0) image[f] = (float)red[0];
+}
+
+}  // namespace
+}  // namespace mk
+
+using namespace mk;
+
+#define MK_GUARD(ctx)                                          \
+  if (!(ctx)) return MK_ERR_INVALID_ARG;                       \
+  if ((ctx)->sticky) return (ctx)->sticky;
+
+extern "C" {
+
+const char* mk_version(void) { return "libmk 0.1 (sm_100a)"; }
+
+const char* mk_last_error(mk_ctx* ctx) { return ctx ? ctx->err.c_str() : "null context"; }
+
+int mk_create(mk_ctx** out, int nshot, int nrec, int nt, double dt, double dx, double fmin, double fmax) {
+  if (!out) return MK_ERR_INVALID_ARG;
+  *out = nullptr;
+  if (nshot <= 0 || nrec <= 0 || nshot != nrec) return MK_ERR_INVALID_ARG;
+  if (!is_pow2(nt) || nt < 16 || nt > 32768) return MK_ERR_INVALID_ARG;
+  if (!(dt > 0.0) || !(dx > 0.0) || !(fmin >= 0.0) || !(fmax >= fmin) || fmax > 0.5 / dt * (1.0 + 1e-9)) return MK_ERR_INVALID_ARG;
+  int dev = 0, ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) {
+    cudaGetLastError();
+    return MK_ERR_CUDA;  // no CPU fallback
+  }
+  mk_ctx* c = new (std::nothrow) mk_ctx();
+  if (!c) return MK_ERR_OOM;
+  *out = c;  // returned even on failure so that mk_last_error can be read; the caller destroys it
+  c->n = nshot;
+  c->nt = nt;
+  c->dt = dt;
+  c->dx = dx;
+  c->fmin = fmin;
+  c->fmax = fmax;
+  // band B (reading G8): inclusive edges with a 1e-6-bin guard against rounding of 1/(nt dt)
+  const double df = 1.0 / ((double)nt * dt);
+  int lo = (int)std::ceil(fmin / df - 1e-6), hi = (int)std::floor(fmax / df + 1e-6);
+  if (lo < 0) lo = 0;
+  if (hi > nt / 2) hi = nt / 2;
+  if (hi < lo) return set_err(c, MK_ERR_INVALID_ARG, "empty band");
+  c->klo = lo;
+  c->khi = hi;
+  c->nb = hi - lo + 1;
+  c->ld = ((nshot + 15) / 16) * 16;
+  c->plan = mkfft::make_plan(nt);
+  if (int rc = check_cuda(c, cudaGetDevice(&dev), "cudaGetDevice")) return rc;
+  int v = 0;
+  cudaDeviceGetAttribute(&v, cudaDevAttrMultiProcessorCount, dev);
+  c->num_sms = v;
+  cudaDeviceGetAttribute(&v, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
+  c->smem_optin = (size_t)v;
+  c->shot_loaded.assign(nshot, 0);
+  // twiddles e^{-2 pi i k / nt}, evaluated in double (table constants only)
+  {
+    std::vector<float2> tw(nt);
+    const double two_pi = 6.283185307179586476925286766559;
+    for (int k = 0; k < nt; ++k) {
+      const double a = -two_pi * (double)k / (double)nt;
+      tw[k] = make_float2((float)std::cos(a), (float)std::sin(a));
+    }
+    size_t cap = 0;
+    if (int rc = ensure(c, &c->d_tw, &cap, (size_t)nt, "twiddles")) return rc;
+    if (int rc = check_cuda(c, cudaMemcpy(c->d_tw, tw.data(), nt * sizeof(float2), cudaMemcpyHostToDevice), "twiddle upload")) return rc;
+  }
+  {
+    size_t cap = 0;
+    const size_t cnt = (size_t)nrec * c->nb * c->ld;
+    if (int rc = ensure(c, &c->d_Rhat, &cap, cnt, "Rhat")) return rc;
+    if (int rc = check_cuda(c, cudaMemset(c->d_Rhat, 0, cnt * sizeof(float2)), "Rhat memset")) return rc;
+  }
+  return MK_OK;
+}
+
+int mk_destroy(mk_ctx* c) {
+  if (!c) return MK_OK;
+  cudaFree(c->d_tw);
+  cudaFree(c->d_Rhat);
+  cudaFree(c->d_f1plus);
+  cudaFree(c->d_f1min);
+  cudaFree(c->d_Nhat);
+  cudaFree(c->d_Shat);
+  cudaFree(c->d_phat);
+  cudaFree(c->d_h);
+  cudaFree(c->d_Nhat2);
+  cudaFree(c->d_Shat2);
+  cudaFree(c->d_stage);
+  for (cudaEvent_t e : c->ev) cudaEventDestroy(e);
+  cudaGetLastError();
+  delete c;
+  return MK_OK;
+}
+
+int mk_set_stream(mk_ctx* c, void* cuda_stream) {
+  MK_GUARD(c);
+  c->stream = static_cast<cudaStream_t>(cuda_stream);
+  return MK_OK;
+}
+
+int mk_set_option(mk_ctx* c, int key, double value) {
+  MK_GUARD(c);
+  switch (key) {
+    case MK_OPT_EPS_SAMPLES:
+      if (value < 0 || value > c->nt) return set_err(c, MK_ERR_INVALID_ARG, "eps out of range");
+      if (c->begun) return set_err(c, MK_ERR_STATE, "eps cannot change during a run");
+      c->eps = (int)value;
+      return MK_OK;
+    case MK_OPT_REGIME:
+      if (value < 0 || value > 3 || value != std::floor(value)) return set_err(c, MK_ERR_INVALID_ARG, "regime must be 0..3");
+      if ((int)value == 3) return set_err(c, MK_ERR_INVALID_ARG, "tcgen05 3xTF32 regime is not built in this version");
+      c->regime = (int)value;
+      return MK_OK;
+    case MK_OPT_TIMING:
+      c->timing = value != 0.0;
+      return MK_OK;
+    default:
+      return set_err(c, MK_ERR_INVALID_ARG, "unknown option");
+  }
+}
+
+int mk_get_info(mk_ctx* c, int key, double* value) {
+  MK_GUARD(c);
+  if (!value) return MK_ERR_INVALID_ARG;
+  switch (key) {
+    case MK_INFO_NB: *value = c->nb; return MK_OK;
+    case MK_INFO_KLO: *value = c->klo; return MK_OK;
+    case MK_INFO_KHI: *value = c->khi; return MK_OK;
+    case MK_INFO_RHAT_BYTES: *value = 8.0 * c->n * (double)c->nb * c->n; return MK_OK;
+    case MK_INFO_RHAT_BYTES_PADDED: *value = 8.0 * c->n * (double)c->nb * c->ld; return MK_OK;
+    case MK_INFO_LD_SHOT: *value = c->ld; return MK_OK;
+    case MK_INFO_SHOTS_LOADED: *value = c->shots_loaded; return MK_OK;
+    case MK_INFO_SYN_LAUNCHES: *value = (double)(c->ev_used / 2); return MK_OK;
+    case MK_INFO_SYN_MS_TOTAL: {
+      if (int rc = check_cuda(c, cudaStreamSynchronize(c->stream), "cudaStreamSynchronize")) return rc;
+      double tot = 0.0;
+      for (size_t i = 0; i + 1 < c->ev_used; i += 2) {
+        float ms = 0.f;
+        if (int rc = check_cuda(c, cudaEventElapsedTime(&ms, c->ev[i], c->ev[i + 1]), "cudaEventElapsedTime")) return rc;
+        tot += ms;
+      }
+      *value = tot;
+      return MK_OK;
+    }
+    case MK_INFO_SYN_RESET: c->ev_used = 0; *value = 0; return MK_OK;
+    case MK_INFO_KERNEL_LAUNCHES: *value = (double)c->launches; return MK_OK;
+    case MK_INFO_REGIME_USED: *value = c->regime_used; return MK_OK;
+    case MK_INFO_DEVICE_BYTES: *value = (double)c->device_bytes; return MK_OK;
+    default: return set_err(c, MK_ERR_INVALID_ARG, "unknown info key");
+  }
+}
+
+int mk_load_R(mk_ctx* c, const float* d_R_time, int shot0, int nshots) {
+  MK_GUARD(c);
+  if (!d_R_time || shot0 < 0 || nshots <= 0 || shot0 + nshots > c->n) return set_err(c, MK_ERR_INVALID_ARG, "mk_load_R: bad shot range");
+  if (c->begun) return set_err(c, MK_ERR_STATE, "mk_load_R during a run");
+  if (int rc = launch_load_R(c, d_R_time, shot0, nshots)) return rc;
+  for (int s = shot0; s < shot0 + nshots; ++s)
+    if (!c->shot_loaded[s]) {
+      c->shot_loaded[s] = 1;
+      ++c->shots_loaded;
+    }
+  return MK_OK;
+}
+
+int mk_load_R_host(mk_ctx* c, const float* h_R_time, int shot0, int nshots) {
+  MK_GUARD(c);
+  if (!h_R_time || shot0 < 0 || nshots <= 0 || shot0 + nshots > c->n) return set_err(c, MK_ERR_INVALID_ARG, "mk_load_R_host: bad shot range");
+  const size_t per_shot = (size_t)c->n * c->nt;
+  size_t chunk = ((size_t)1 << 28) / per_shot;  // <= 1 GiB of fp32 per staging chunk
+  if (chunk < 1) chunk = 1;
+  if (chunk > (size_t)nshots) chunk = nshots;
+  if (int rc = ensure(c, &c->d_stage, &c->cap_stage, chunk * per_shot, "staging")) return rc;
+  for (int s = 0; s < nshots; s += (int)chunk) {
+    const int ns = std::min((int)chunk, nshots - s);
+    if (int rc = check_cuda(c, cudaMemcpyAsync(c->d_stage, h_R_time + (size_t)s * per_shot, ns * per_shot * sizeof(float),
+                                               cudaMemcpyHostToDevice, c->stream), "H2D R chunk")) return rc;
+    if (int rc = mk_load_R(c, c->d_stage, shot0 + s, ns)) return rc;
+  }
+  return check_cuda(c, cudaStreamSynchronize(c->stream), "cudaStreamSynchronize");
+}
+
+int mk_begin(mk_ctx* c, const float* d_Gd, const float* d_td, int nfoc) {
+  MK_GUARD(c);
+  if (!d_Gd || !d_td || nfoc <= 0) return set_err(c, MK_ERR_INVALID_ARG, "mk_begin: bad arguments");
+  if (c->shots_loaded != c->n) return set_err(c, MK_ERR_STATE, "mk_begin before every shot of R was loaded");
+  int regime = 0;
+  if (int rc = resolve_regime(c, nfoc, &regime)) return rc;
+  const int ldf = ldf_for(regime, nfoc);
+  const size_t ntime = (size_t)nfoc * c->n * c->nt;
+  const size_t nN = (size_t)c->nb * c->ld * ldf, nS = (size_t)c->n * c->nb * ldf;
+  c->begun = false;
+  {
+    size_t cap2 = c->cap_time;
+    if (int rc = ensure(c, &c->d_f1plus, &c->cap_time, ntime, "f1plus")) return rc;
+    if (int rc = ensure(c, &c->d_f1min, &cap2, ntime, "f1min")) return rc;
+    size_t capS = c->cap_Shat;
+    if (int rc = ensure(c, &c->d_Nhat, &c->cap_Nhat, nN, "Nhat")) return rc;
+    if (int rc = ensure(c, &c->d_Shat, &c->cap_Shat, nS, "Shat")) return rc;
+    if (int rc = ensure(c, &c->d_phat, &capS, nS, "phat")) return rc;
+    if (int rc = ensure(c, &c->d_h, &c->cap_h, (size_t)nfoc * c->n, "window table")) return rc;
+  }
+  c->nfoc = nfoc;
+  c->ldf = ldf;
+  c->regime_used = regime;
+  c->iter = 0;
+  c->have_Gminus = false;
+  if (int rc = check_cuda(c, cudaMemsetAsync(c->d_Nhat, 0, nN * sizeof(float2), c->stream), "memset Nhat")) return rc;
+  if (int rc = check_cuda(c, cudaMemsetAsync(c->d_phat, 0, nS * sizeof(float2), c->stream), "memset phat")) return rc;
+  if (int rc = check_cuda(c, cudaMemsetAsync(c->d_f1min, 0, ntime * sizeof(float), c->stream), "memset f1min")) return rc;
+  if (int rc = launch_window(c, d_td, c->d_h, nfoc * c->n)) return rc;
+  // a1: N_{-1} = f1plus = T G_d; N^_{-1} = conj(G_d^)     [PAPER.md:19, 67, 74-75]
+  if (int rc = launch_fwd(c, d_Gd, c->d_Nhat, nfoc, ldf, /*conj_out=*/true, c->d_f1plus)) return rc;
+  c->begun = true;
+  return MK_OK;
+}
+
+int mk_step(mk_ctx* c, float* d_N_i) {
+  MK_GUARD(c);
+  if (!c->begun) return set_err(c, MK_ERR_STATE, "mk_step before mk_begin");
+  int regime = c->regime_used;
+  if (int rc = contract(c, c->d_Nhat, c->d_Shat, c->nfoc, c->ldf, regime)) return rc;      // a2  [PAPER.md:69]
+  if (int rc = launch_post(c, (c->iter % 2) == 0, d_N_i)) return rc;                       // a3..a6
+  ++c->iter;
+  return MK_OK;
+}
+
+static int scratch_operands(mk_ctx* c, int nfoc, int ldf) {
+  const size_t nN = (size_t)c->nb * c->ld * ldf, nS = (size_t)c->n * c->nb * ldf;
+  if (int rc = ensure(c, &c->d_Nhat2, &c->cap_Nhat2, nN, "Nhat scratch")) return rc;
+  if (int rc = ensure(c, &c->d_Shat2, &c->cap_Shat2, nS, "Shat scratch")) return rc;
+  // pad rows / columns of the operand must be zero; the layout may differ from the previous use
+  return check_cuda(c, cudaMemsetAsync(c->d_Nhat2, 0, nN * sizeof(float2), c->stream), "memset Nhat scratch");
+}
+
+int mk_finish(mk_ctx* c, const mk_outputs* o) {
+  MK_GUARD(c);
+  if (!c->begun) return set_err(c, MK_ERR_STATE, "mk_finish before mk_begin");
+  if (!o) return set_err(c, MK_ERR_INVALID_ARG, "mk_finish: null outputs");
+  if (o->N_last) return set_err(c, MK_ERR_INVALID_ARG, "N_last is delivered by mk_run (or by mk_step's d_N_i), not by mk_finish");
+  const size_t bytes = (size_t)c->nfoc * c->n * c->nt * sizeof(float);
+  const int regime = c->regime_used;
+  if (o->f1plus)
+    if (int rc = check_cuda(c, cudaMemcpyAsync(o->f1plus, c->d_f1plus, bytes, cudaMemcpyDeviceToDevice, c->stream), "copy f1plus")) return rc;
+  if (o->f1min)
+    if (int rc = check_cuda(c, cudaMemcpyAsync(o->f1min, c->d_f1min, bytes, cudaMemcpyDeviceToDevice, c->stream), "copy f1min")) return rc;
+  if (o->Gminus) {  // G^- = R f1plus - f1min   [PAPER.md:87-88; G5]
+    if (int rc = scratch_operands(c, c->nfoc, c->ldf)) return rc;
+    if (int rc = launch_fwd(c, c->d_f1plus, c->d_Nhat2, c->nfoc, c->ldf, false, nullptr)) return rc;
+    if (int rc = contract(c, c->d_Nhat2, c->d_Shat2, c->nfoc, c->ldf, regime)) return rc;
+    if (int rc = launch_inv(c, c->d_Shat2, c->nfoc, c->ldf, o->Gminus, 1.f, c->d_f1min, -1.f, nullptr, 0.f)) return rc;
+  }
+  if (o->Gplus) {  // G^+ = T f1plus - R (T f1min)   [PAPER.md:24; G4]
+    if (int rc = scratch_operands(c, c->nfoc, c->ldf)) return rc;
+    if (int rc = launch_fwd(c, c->d_f1min, c->d_Nhat2, c->nfoc, c->ldf, true, nullptr)) return rc;
+    if (int rc = contract(c, c->d_Nhat2, c->d_Shat2, c->nfoc, c->ldf, regime)) return rc;
+    if (int rc = launch_inv(c, c->d_Shat2, c->nfoc, c->ldf, o->Gplus, -1.f, nullptr, 0.f, c->d_f1plus, 1.f)) return rc;
+  }
+  if (o->G) {  // G = p^- + T f2 = p^- + T f1plus - f1min   [PAPER.md:24; G3]
+    if (int rc = launch_inv(c, c->d_phat, c->nfoc, c->ldf, o->G, 1.f, c->d_f1min, -1.f, c->d_f1plus, 1.f)) return rc;
+  }
+  return MK_OK;
+}
+
+int mk_run(mk_ctx* c, const float* d_Gd, const float* d_td, int nfoc, int niter, const mk_outputs* o) {
+  MK_GUARD(c);
+  if (niter < 0 || !o) return set_err(c, MK_ERR_INVALID_ARG, "mk_run: bad arguments");
+  if (o->N_last && niter == 0) return set_err(c, MK_ERR_INVALID_ARG, "N_last needs niter >= 1");
+  if (int rc = mk_begin(c, d_Gd, d_td, nfoc)) return rc;
+  for (int i = 0; i < niter; ++i)
+    if (int rc = mk_step(c, i == niter - 1 ? o->N_last : nullptr)) return rc;
+  mk_outputs rest = *o;
+  rest.N_last = nullptr;
+  return mk_finish(c, &rest);
+}
+
+int mk_run_host(mk_ctx* c, const float* h_Gd, const float* h_td, int nfoc, int niter, const mk_outputs* ho) {
+  MK_GUARD(c);
+  if (!h_Gd || !h_td || nfoc <= 0 || niter < 0 || !ho) return set_err(c, MK_ERR_INVALID_ARG, "mk_run_host: bad arguments");
+  if (ho->N_last && niter == 0) return set_err(c, MK_ERR_INVALID_ARG, "N_last needs niter >= 1");
+  const size_t ntime = (size_t)nfoc * c->n * c->nt, ntd = (size_t)nfoc * c->n;
+  if (int rc = ensure(c, &c->d_stage, &c->cap_stage, ntime + ntd, "staging")) return rc;
+  float* d_field = c->d_stage;
+  float* d_td = c->d_stage + ntime;
+  if (int rc = check_cuda(c, cudaMemcpyAsync(d_field, h_Gd, ntime * sizeof(float), cudaMemcpyHostToDevice, c->stream), "H2D G_d")) return rc;
+  if (int rc = check_cuda(c, cudaMemcpyAsync(d_td, h_td, ntd * sizeof(float), cudaMemcpyHostToDevice, c->stream), "H2D t_d")) return rc;
+  if (int rc = mk_begin(c, d_field, d_td, nfoc)) return rc;
+  for (int i = 0; i < niter; ++i) {
+    const bool last = (i == niter - 1) && ho->N_last;
+    if (int rc = mk_step(c, last ? d_field : nullptr)) return rc;
+    if (last)
+      if (int rc = check_cuda(c, cudaMemcpyAsync(ho->N_last, d_field, ntime * sizeof(float), cudaMemcpyDeviceToHost, c->stream), "D2H N_last")) return rc;
+  }
+  float* hosts[5] = {ho->f1plus, ho->f1min, ho->G, ho->Gplus, ho->Gminus};
+  for (int i = 0; i < 5; ++i) {
+    if (!hosts[i]) continue;
+    if (i == 0 || i == 1) {  // accumulators go straight from the library's buffers
+      const float* src = i == 0 ? c->d_f1plus : c->d_f1min;
+      if (int rc = check_cuda(c, cudaMemcpyAsync(hosts[i], src, ntime * sizeof(float), cudaMemcpyDeviceToHost, c->stream), "D2H accumulator")) return rc;
+      continue;
+    }
+    mk_outputs one{};
+    if (i == 2) one.G = d_field;
+    if (i == 3) one.Gplus = d_field;
+    if (i == 4) one.Gminus = d_field;
+    if (int rc = mk_finish(c, &one)) return rc;
+    if (int rc = check_cuda(c, cudaMemcpyAsync(hosts[i], d_field, ntime * sizeof(float), cudaMemcpyDeviceToHost, c->stream), "D2H output")) return rc;
+  }
+  return check_cuda(c, cudaStreamSynchronize(c->stream), "cudaStreamSynchronize");
+}
+
+int mk_synthesis(mk_ctx* c, const float* d_N_in, float* d_S_out, int nfoc) {
+  MK_GUARD(c);
+  if (!d_N_in || !d_S_out || nfoc <= 0) return set_err(c, MK_ERR_INVALID_ARG, "mk_synthesis: bad arguments");
+  if (c->shots_loaded != c->n) return set_err(c, MK_ERR_STATE, "mk_synthesis before every shot of R was loaded");
+  int regime = 0;
+  if (int rc = resolve_regime(c, nfoc, &regime)) return rc;
+  const int ldf = ldf_for(regime, nfoc);
+  if (int rc = scratch_operands(c, nfoc, ldf)) return rc;
+  if (int rc = launch_fwd(c, d_N_in, c->d_Nhat2, nfoc, ldf, false, nullptr)) return rc;      // a6
+  if (int rc = contract(c, c->d_Nhat2, c->d_Shat2, nfoc, ldf, regime)) return rc;            // a2
+  return launch_inv(c, c->d_Shat2, nfoc, ldf, d_S_out, 1.f, nullptr, 0.f, nullptr, 0.f);     // a3
+}
+
+int mk_image(mk_ctx* c, const float* d_Gminus, float* d_image) {
+  MK_GUARD(c);
+  if (!d_Gminus || !d_image) return set_err(c, MK_ERR_INVALID_ARG, "mk_image: bad arguments");
+  if (!c->begun) return set_err(c, MK_ERR_STATE, "mk_image before a run");
+  const float wm = (float)(c->dt * c->dx), we = (float)(c->dt * c->dx * 0.5);
+  k_image<<<c->nfoc, 256, 0, c->stream>>>(d_Gminus, c->d_f1plus, d_image, c->n, c->nt, wm, we);
+  ++c->launches;
+  return check_cuda(c, cudaGetLastError(), "k_image");
+}
+
+}  // extern "C"

@@ -1,0 +1,96 @@
+// mk_internal.cuh — context and kernel launchers shared by the translation units of libmk (not part of the ABI).
+#pragma once
+
+#include <cuda_runtime.h>
+
+#include <cstddef>
+#include <cstdint>
+#include <string>
+#include <vector>
+
+#include "../../include/mk.h"
+#include "fft_core.cuh"
+
+// Device layouts (complex64 = float2, interleaved re/im):
+//   Rhat [n][nb][ld]      R^[r][k][s] * dt * w[s]; ld = round_up(n, 16); pad columns are zero        (a0)
+//   Nhat [nb][ld][ldf]    N^[k][s][f]; pad rows (s >= n) and pad columns (f >= nfoc) are zero        (a1, a6)
+//   Shat [n][nb][ldf]     S^[r][k][f]                                                                 (a2)
+//   phat [n][nb][ldf]     running p^- spectrum                                                        (a3)
+//   f1plus, f1min [nfoc][n][nt] fp32 time domain                                                      (a5)
+//   h [nfoc][n] int32     window half-widths                                                          (a4)
+struct mk_ctx {
+  int n = 0, nt = 0, nb = 0, klo = 0, khi = 0, ld = 0;
+  double dt = 0, dx = 0, fmin = 0, fmax = 0;
+  int eps = 8, regime = 0, timing = 0;
+  cudaStream_t stream = nullptr;
+  mkfft::Plan plan{};
+  int num_sms = 0;
+  size_t smem_optin = 0;
+
+  float2* d_tw = nullptr;    // [nt] e^{-2 pi i k / nt}
+  float2* d_Rhat = nullptr;  // [n][nb][ld]
+  std::vector<unsigned char> shot_loaded;
+  int shots_loaded = 0;
+
+  // run state
+  int nfoc = 0, ldf = 0, iter = 0;
+  bool begun = false;
+  float* d_f1plus = nullptr;
+  float* d_f1min = nullptr;
+  size_t cap_time = 0;  // capacity (floats) of each of f1plus / f1min
+  float2* d_Nhat = nullptr;
+  float2* d_Shat = nullptr;
+  float2* d_phat = nullptr;
+  size_t cap_Nhat = 0, cap_Shat = 0;  // capacities in float2
+  int* d_h = nullptr;
+  size_t cap_h = 0;
+  // scratch operands for mk_synthesis / finals (so a run in progress is not disturbed)
+  float2* d_Nhat2 = nullptr;
+  float2* d_Shat2 = nullptr;
+  size_t cap_Nhat2 = 0, cap_Shat2 = 0;
+  float* d_stage = nullptr;  // host-call staging
+  size_t cap_stage = 0;
+  float* d_Gminus = nullptr;  // kept by mk_finish when G^- was requested (mk_image)
+  size_t cap_Gminus = 0;
+  bool have_Gminus = false;
+
+  size_t device_bytes = 0;
+  long launches = 0;
+  int regime_used = 0;
+
+  // timing of contraction launches
+  std::vector<cudaEvent_t> ev;  // pairs
+  size_t ev_used = 0;
+
+  std::string err;
+  int sticky = 0;
+};
+
+namespace mk {
+
+struct FftParams {
+  mkfft::Plan plan;
+  const float2* tw;
+  int n, nb, klo, ld, ldf, nfoc;
+};
+
+int set_err(mk_ctx* c, int code, const std::string& msg);
+int check_cuda(mk_ctx* c, cudaError_t e, const char* what);
+
+// mk_fft_kernels.cu
+int launch_window(mk_ctx* c, const float* d_td, int* d_h, int ntr);
+int launch_load_R(mk_ctx* c, const float* d_R_time, int shot0, int nshots);
+// time [nfoc][n][nt] -> Nhat band;  conj_out: spectrum of T(src);  d_init_Tsrc: optional, receives T src
+int launch_fwd(mk_ctx* c, const float* d_src, float2* d_Nhat, int nfoc, int ldf, bool conj_out, float* d_init_Tsrc);
+// spectrum [n][nb][ldf] -> out[j] = sS*S[j] + sA*A[j] + sB*B[(nt-j)%nt]
+int launch_inv(mk_ctx* c, const float2* d_spec, int nfoc, int ldf, float* d_out, float sS, const float* d_A, float sA,
+               const float* d_B, float sB);
+// fused a3..a6
+int launch_post(mk_ctx* c, int parity_even, float* d_Ni_out);
+
+// mk_syn_gemv.cu / mk_syn_gemm.cu:  Shat = Rhat x Nhat per bin
+bool gemv_supported(const mk_ctx* c, int nfoc);
+int launch_syn_gemv(mk_ctx* c, const float2* d_Nhat, float2* d_Shat, int nfoc);
+int launch_syn_gemm(mk_ctx* c, const float2* d_Nhat, float2* d_Shat, int ldf);
+
+}  // namespace mk

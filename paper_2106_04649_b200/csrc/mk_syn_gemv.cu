@@ -1,0 +1,128 @@
+// mk_syn_gemv.cu — synthesis contraction for few focal points (bandwidth-bound regime):
+//   S^[r][k][f] = sum_s R^[r][k][s] * N^[k][s][f]          (dt * w[s] already folded into R^ at ingest)
+// eq. (1) of the paper evaluated in the frequency domain.  The paper runs this as a pointwise
+// multiply kernel that materialises d_RF followed by a CUB segmented reduction; here the
+// product is never stored: every row of R^ (one receiver, one bin: ld complex, contiguous) is streamed from HBM
+// exactly once with 128-bit loads, multiplied against the bin's N^ column block held in shared memory, and reduced
+// with warp shuffles.  Algorithmic traffic: 8 bytes per complex element of R^.
+#include "mk_internal.cuh"
+
+namespace mk {
+
+namespace {
+
+constexpr int kThreads = 256;
+constexpr int kWarps = kThreads / 32;
+constexpr int kRows = 4;                         // rows of R^ a warp streams at once (x reuse + loads in flight)
+constexpr int kRowsPerCta = kWarps * kRows * 2;  // 64 receivers per CTA
+
+struct f8 {
+  float v[8];
+};
+// 256-bit streaming load (sm_100: LDG.E.256), L1 no-allocate, L2 evict-first: R^ is read exactly once per synthesis
+__device__ __forceinline__ f8 ld_stream(const float* p) {
+  f8 r;
+  asm volatile("ld.global.nc.L1::no_allocate.L2::evict_first.v8.f32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
+               : "=f"(r.v[0]), "=f"(r.v[1]), "=f"(r.v[2]), "=f"(r.v[3]), "=f"(r.v[4]), "=f"(r.v[5]), "=f"(r.v[6]), "=f"(r.v[7])
+               : "l"(p));
+  return r;
+}
+
+__device__ __forceinline__ void cfma(float2& acc, float ar, float ai, float2 b) {
+  acc.x = fmaf(ar, b.x, acc.x);
+  acc.x = fmaf(-ai, b.y, acc.x);
+  acc.y = fmaf(ar, b.y, acc.y);
+  acc.y = fmaf(ai, b.x, acc.y);
+}
+
+// grid (nb, ceil(n / kRowsPerCta)).  Rhat [n][nb][ld], Nhat [nb][ld][NFOC], Shat [n][nb][NFOC].
+template <int NFOC>
+__global__ void __launch_bounds__(kThreads) k_syn_gemv(const float2* __restrict__ Rhat, const float2* __restrict__ Nhat,
+                                                       float2* __restrict__ Shat, int n, int nb, int ld) {
+  extern __shared__ float4 smem4[];
+  float2* x = reinterpret_cast<float2*>(smem4);  // [ld][NFOC]
+  const int kk = blockIdx.x;
+  const int r_begin = blockIdx.y * kRowsPerCta;
+  const int r_end = min(r_begin + kRowsPerCta, n);
+  {
+    const float4* src = reinterpret_cast<const float4*>(Nhat + (size_t)kk * ld * NFOC);
+    const int nvec = ld * NFOC / 2;
+    for (int i = threadIdx.x; i < nvec; i += kThreads) smem4[i] = __ldg(src + i);
+  }
+  __syncthreads();
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int nchunk = ld >> 2;  // 256-bit chunk = 4 complex (ld is a multiple of 16)
+  for (int r0 = r_begin + warp * kRows; r0 < r_end; r0 += kWarps * kRows) {
+    const float* row[kRows];
+#pragma unroll
+    for (int i = 0; i < kRows; ++i) {
+      const int r = min(r0 + i, n - 1);
+      row[i] = reinterpret_cast<const float*>(Rhat + ((size_t)r * nb + kk) * ld);
+    }
+    float2 acc[kRows][NFOC];
+#pragma unroll
+    for (int i = 0; i < kRows; ++i)
+#pragma unroll
+      for (int f = 0; f < NFOC; ++f) acc[i][f] = make_float2(0.f, 0.f);
+#pragma unroll 2
+    for (int c = lane; c < nchunk; c += 32) {
+      f8 a[kRows];
+#pragma unroll
+      for (int i = 0; i < kRows; ++i) a[i] = ld_stream(row[i] + 8 * c);
+#pragma unroll
+      for (int e = 0; e < 4; ++e)
+#pragma unroll
+        for (int f = 0; f < NFOC; ++f) {
+          const float2 xv = x[(4 * c + e) * NFOC + f];
+#pragma unroll
+          for (int i = 0; i < kRows; ++i) cfma(acc[i][f], a[i].v[2 * e], a[i].v[2 * e + 1], xv);
+        }
+    }
+#pragma unroll
+    for (int i = 0; i < kRows; ++i)
+#pragma unroll
+      for (int f = 0; f < NFOC; ++f) {
+        float2 v = acc[i][f];
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {
+          v.x += __shfl_xor_sync(0xffffffffu, v.x, o);
+          v.y += __shfl_xor_sync(0xffffffffu, v.y, o);
+        }
+        if (lane == 0 && r0 + i < r_end) Shat[((size_t)(r0 + i) * nb + kk) * NFOC + f] = v;
+      }
+  }
+}
+
+template <int NFOC>
+int launch_t(mk_ctx* c, const float2* d_Nhat, float2* d_Shat) {
+  const size_t smem = (size_t)c->ld * NFOC * sizeof(float2);
+  auto kern = k_syn_gemv<NFOC>;
+  if (int rc = check_cuda(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem), "cudaFuncSetAttribute"))
+    return rc;
+  const dim3 grid(c->nb, (c->n + kRowsPerCta - 1) / kRowsPerCta);
+  kern<<<grid, kThreads, smem, c->stream>>>(c->d_Rhat, d_Nhat, d_Shat, c->n, c->nb, c->ld);
+  ++c->launches;
+  return check_cuda(c, cudaGetLastError(), "k_syn_gemv");
+}
+
+}  // namespace
+
+bool gemv_supported(const mk_ctx* c, int nfoc) {
+  return nfoc >= 1 && nfoc <= 8 && (size_t)c->ld * nfoc * sizeof(float2) <= 96 * 1024;
+}
+
+int launch_syn_gemv(mk_ctx* c, const float2* d_Nhat, float2* d_Shat, int nfoc) {
+  switch (nfoc) {
+    case 1: return launch_t<1>(c, d_Nhat, d_Shat);
+    case 2: return launch_t<2>(c, d_Nhat, d_Shat);
+    case 3: return launch_t<3>(c, d_Nhat, d_Shat);
+    case 4: return launch_t<4>(c, d_Nhat, d_Shat);
+    case 5: return launch_t<5>(c, d_Nhat, d_Shat);
+    case 6: return launch_t<6>(c, d_Nhat, d_Shat);
+    case 7: return launch_t<7>(c, d_Nhat, d_Shat);
+    case 8: return launch_t<8>(c, d_Nhat, d_Shat);
+    default: return set_err(c, MK_ERR_INVALID_ARG, "gemv regime needs 1 <= nfoc <= 8");
+  }
+}
+
+}  // namespace mk

@@ -1,0 +1,111 @@
+"""Parity of the CUDA path (through the C ABI) against the fp64 oracle, element by element on the same seeded
+inputs.  Tolerances are BASELINE.json north_star's: relative L2 error <= 2e-5 per iteration and <= 1e-4 on the
+final fields.  Run on the B200 box with `pytest -m gpu`."""
+import numpy as np
+import pytest
+
+import oracle
+from paper_2106_04649_b200 import configs, gen
+from _util import calibrated, gpu_chain, problem, rel_l2
+
+pytestmark = pytest.mark.gpu
+
+TOL_ITER, TOL_FINAL = 2e-5, 1e-4
+FINALS = ("f1plus", "f1min", "G", "Gplus", "Gminus")
+
+
+def _oracle_chain(cfg, R, Gd, td, niter=None):
+    return oracle.marchenko(R, Gd, td, cfg.dt, cfg.dx, cfg.fmin, cfg.fmax, cfg.niter if niter is None else niter, cfg.eps)
+
+
+def _check_chain(cfg, regime, niter=None, focs=None):
+    R, Gd, td = problem(cfg, focs)
+    ref = _oracle_chain(cfg, R, Gd, td, niter)
+    got = gpu_chain(cfg, R, Gd, td, niter=niter, regime=regime)
+    errs = [rel_l2(got["N_iters"][i], ref["N_iters"][i]) for i in range(ref["N_iters"].shape[0])]
+    ferr = {nm: rel_l2(got[nm], ref[nm]) for nm in FINALS}
+    print(f"\n[{cfg.name} n={cfg.n} nt={cfg.nt} nfoc={Gd.shape[0]} regime={got['regime_used']}] per-iter max {max(errs):.2e} "
+          + " ".join(f"{k}={v:.1e}" for k, v in ferr.items()))
+    assert max(errs) <= TOL_ITER, errs
+    for nm, e in ferr.items():
+        assert e <= TOL_FINAL, (nm, e)
+    return got, ref
+
+
+# ---------------------------------------------------------------- bare synthesis
+@pytest.mark.parametrize("n,nt,nfoc,regime", [(5, 32, 3, 0), (20, 64, 1, 1), (20, 64, 12, 2)])
+def test_delta_spike_shift(n, nt, nfoc, regime):
+    import torch
+    from paper_2106_04649_b200 import binding as B
+    dt, dx, q = 0.5, 2.0, 5
+    w = np.full(n, dx)
+    w[0] = w[-1] = dx / 2
+    R = np.zeros((n, n, nt), np.float32)
+    for s in range(n):
+        R[s, s, q] = 1.0 / (w[s] * dt)
+    rng = np.random.default_rng(1)
+    N = rng.standard_normal((nfoc, n, nt)).astype(np.float32)
+    with B.Marchenko(n, n, nt, dt, dx, 0.0, 1.0 / (2 * dt)) as mk:
+        mk.set_option(B.MK_OPT_REGIME, regime)
+        mk.load_R(torch.from_numpy(R).cuda())
+        S = torch.empty((nfoc, n, nt), dtype=torch.float32, device="cuda")
+        mk.synthesis(torch.from_numpy(N).cuda(), S)
+        S = S.cpu().numpy()
+    assert rel_l2(S, np.roll(N, q, axis=-1)) < 2e-6
+
+
+@pytest.mark.parametrize("n,nt,nfoc,regime", [
+    (37, 128, 1, 1), (37, 128, 3, 1), (37, 128, 8, 1),           # GEMV, ragged rows
+    (37, 128, 5, 2), (150, 64, 70, 2), (130, 256, 129, 2),        # FFMA GEMM, ragged M / N tiles
+    (16, 16, 2, 0), (33, 4096, 9, 0),                             # smallest / longest traces
+])
+def test_synthesis_random_vs_oracle(n, nt, nfoc, regime):
+    import torch
+    from paper_2106_04649_b200 import binding as B
+    dt, dx = 0.004, 10.0
+    fmax = 0.4 / dt
+    rng = np.random.default_rng(n * 1000 + nfoc)
+    R = rng.standard_normal((n, n, nt)).astype(np.float32)     # non-symmetric in (s, r): a transposed operand fails
+    N = rng.standard_normal((nfoc, n, nt)).astype(np.float32)
+    N[:, :, nt // 3:] = 0.0                                      # keeps the direct oracle cheap
+    klo, khi, nb = oracle.band(nt, dt, 10.0, fmax)
+    ref = oracle.synthesis(R, N.astype(np.float64), dt, oracle.weights(n, dx), klo, khi)
+    with B.Marchenko(n, n, nt, dt, dx, 10.0, fmax) as mk:
+        assert int(mk.get_info(B.MK_INFO_NB)) == nb and int(mk.get_info(B.MK_INFO_KLO)) == klo
+        mk.set_option(B.MK_OPT_REGIME, regime)
+        mk.load_R(torch.from_numpy(R).cuda())
+        S = torch.empty((nfoc, n, nt), dtype=torch.float32, device="cuda")
+        mk.synthesis(torch.from_numpy(N).cuda(), S)
+        S = S.cpu().numpy()
+    e = rel_l2(S, ref)
+    print(f"\n[synthesis n={n} nt={nt} nfoc={nfoc} regime={regime}] rel L2 {e:.2e}")
+    assert e <= TOL_ITER
+
+
+# ---------------------------------------------------------------- whole chain, reduced copies of the configs
+@pytest.mark.parametrize("k,n,nt,nfoc,regime", [
+    (0, 40, 256, 1, 1), (1, 70, 512, 4, 1), (1, 70, 512, 4, 2), (2, 70, 512, 70, 2), (3, 90, 512, 19, 2),
+    (4, 60, 1024, 33, 2),
+])
+def test_chain_reduced_configs(k, n, nt, nfoc, regime):
+    focal = "single:400" if nfoc == 1 else ("line:300" if nfoc == n else "fan:250")
+    cfg = calibrated(configs.scaled(k, n=n, nt=nt, nfoc=nfoc, focal=focal, niter=8))
+    _check_chain(cfg, regime)
+
+
+def test_config0_full_chain():
+    got, ref = _check_chain(configs.get(0), regime=0)
+    assert got["regime_used"] == 1
+
+
+def test_config0_host_api_and_run_match_steps():
+    cfg = configs.get(0)
+    R, Gd, td = problem(cfg)
+    a = gpu_chain(cfg, R, Gd, td, keep_iters=True)
+    b = gpu_chain(cfg, R, Gd, td, keep_iters=False)
+    c = gpu_chain(cfg, R, Gd, td, host_api=True)
+    for nm in FINALS:
+        np.testing.assert_array_equal(a[nm], b[nm])
+        np.testing.assert_array_equal(a[nm], c[nm])
+    np.testing.assert_array_equal(a["N_iters"][-1], b["N_last"])
+    np.testing.assert_array_equal(b["N_last"], c["N_last"])
