@@ -139,6 +139,7 @@ __global__ void __launch_bounds__(kThreads) k_fwd(const float* __restrict__ src,
       const int tl = idx / nt, j = idx - tl * nt;
       init_Tsrc[((size_t)(f0 + tl) * P.n + r) * nt + j] = zf[2 * tl * MP + mkfft::padj((nt - j) & (nt - 1))];
     }
+    __syncthreads();  // the in-place FFT below overwrites what this loop reads
   }
   fft_batch_fwd(smem, nf, MP, P.plan, P.tw);
   for (int idx = threadIdx.x; idx < P.nb * FT; idx += blockDim.x) {
