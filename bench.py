@@ -1,0 +1,337 @@
+#!/usr/bin/env python
+"""bench.py — one JSON line for the driver.
+
+A step = one pass of the whole hot path (mk_run = begin + niter Neumann steps + finals,
+niter + 2 = 18 syntheses) over one batch of seeded synthetic input of BASELINE.json config 1 (601 x 601 x 2048,
+one focal point, 16 iterations; the bandwidth-bound regime the metric is quoted on).  R^ (1.30 GB) is resident in
+HBM and far larger than the 126 MB L2, so no cache flush is needed between steps.
+
+  value      synthesis GB/s of R^ streamed  = syntheses * bytes(R^ unpadded) / device time   (inputs resident in HBM)
+  e2e        same metric through mk_run_host: pinned HOST G_d / t_d in, six HOST output fields out, copies timed
+  roofline   the streaming contraction kernel (k_syn_gemv): algorithmic bytes of R^ per launch / its CUDA-event time
+  cpu_baseline  the fp64 oracle timed on this box's host cores on a bounded sample (one full synthesis R N_0)
+
+`--impl reference` times the oracle itself (a deliberately slow, plain CPU program) on the same workload.
+`--workload K` benches another BASELINE.json config (2 = the 601-focal-point GEMM regime) for DESIGN.md's tables.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+from pathlib import Path
+
+import numpy as np
+
+ROOT = Path(__file__).resolve().parent
+sys.path.insert(0, str(ROOT))
+
+from paper_2106_04649_b200 import configs, gen, shard  # noqa: E402
+
+METRIC = "synthesis_GBps_of_R_streamed"
+UNIT = "GB/s"
+
+
+def dist_env():
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    return rank, world, local
+
+
+def measured_peaks():
+    p = ROOT / "MEASURED_PEAKS.json"
+    if p.exists():
+        d = json.loads(p.read_text())
+        return {"hbm_gbs": float(d["hbm_gbs"]), "bf16_tflops": float(d.get("bf16_tflops", 1590.0)),
+                "bf16_tflops_sustained": float(d.get("bf16_tflops_sustained", 1400.0)), "source": "measured"}
+    return {"hbm_gbs": 6650.0, "bf16_tflops": 1590.0, "bf16_tflops_sustained": 1400.0, "source": "fallback"}
+
+
+class ClockSampler(threading.Thread):
+    """Samples SM clock and throttle reasons DURING the timed region (pynvml; nvidia-smi would show the same)."""
+    REASONS = {0x4: "sw_power_cap", 0x8: "hw_slowdown", 0x20: "sw_thermal_slowdown", 0x40: "hw_thermal_slowdown",
+               0x80: "hw_power_brake_slowdown", 0x2: "applications_clocks_setting", 0x10: "sync_boost"}
+
+    def __init__(self, index, period=0.05):
+        super().__init__(daemon=True)
+        self.index, self.period = index, period
+        self.samples, self.reasons, self.power = [], set(), []
+        self.max_mhz = None
+        self._stop_evt = threading.Event()
+        self.ok = False
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = float(pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM))
+            self.ok = True
+        except Exception:
+            self.ok = False
+
+    def run(self):
+        if not self.ok:
+            return
+        nv = self.nv
+        while not self._stop_evt.is_set():
+            try:
+                self.samples.append(float(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM)))
+                try:
+                    mask = nv.nvmlDeviceGetCurrentClocksEventReasons(self.h)
+                except Exception:
+                    mask = nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h)
+                for bit, nm in self.REASONS.items():
+                    if mask & bit:
+                        self.reasons.add(nm)
+                self.power.append(nv.nvmlDeviceGetPowerUsage(self.h) / 1000.0)
+            except Exception:
+                pass
+            time.sleep(self.period)
+
+    def stop(self):
+        self._stop_evt.set()
+        self.join(timeout=2)
+        if not self.samples:
+            return {"sm_mhz": None, "sm_max_mhz": self.max_mhz, "reasons": [], "samples": 0}
+        return {"sm_mhz": float(np.median(self.samples)), "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons),
+                "samples": len(self.samples), "power_w_max": max(self.power) if self.power else None}
+
+
+def workload_arrays(cfg):
+    base = gen.base_traces(cfg)
+    R = gen.R_full(cfg, base)
+    Gd, td = gen.first_arrivals(cfg)
+    return R, Gd, td
+
+
+def nsyn_per_step(cfg):
+    return cfg.niter + 2        # niter Neumann steps + one extra synthesis each for G^- and G^+ 
+
+
+def rhat_bytes(cfg):
+    import math
+    df = 1.0 / (cfg.nt * cfg.dt)
+    klo = max(int(math.ceil(cfg.fmin / df - 1e-6)), 0)
+    khi = min(int(math.floor(cfg.fmax / df + 1e-6)), cfg.nt // 2)
+    return 8.0 * cfg.n * cfg.n * (khi - klo + 1), khi - klo + 1
+
+
+# ------------------------------------------------------------------------------------------------ oracle legs
+def oracle_sample(cfg, R, Gd, td, budget_s, full_first=True):
+    """Times the oracle (as it stands) on a bounded sample: one synthesis R N_0 over `nrec_s` receivers of the same
+    workload, N_0 being the first windowed iterate (computed by the oracle, untimed).  Returns (seconds, nrec_s)."""
+    import oracle
+    w = oracle.weights(cfg.n, cfg.dx)
+    klo, khi, _ = oracle.band(cfg.nt, cfg.dt, cfg.fmin, cfg.fmax)
+    f = [0] if Gd.shape[0] > 1 else slice(None)
+    N = np.roll(Gd[f][..., ::-1], 1, axis=-1).astype(np.float64)               # N_{-1} = T G_d
+    S = oracle.synthesis(R, N, cfg.dt, w, klo, khi)                              # untimed: sparse N_{-1}
+    h = oracle.window(td[f], cfg.nt, cfg.dt, cfg.eps)
+    j = np.arange(cfg.nt)
+    js = np.where(j < cfg.nt // 2, j, j - cfg.nt)
+    N0 = -(np.abs(js)[None, None, :] < h[..., None]).astype(np.float64) * np.roll(S[..., ::-1], 1, axis=-1)
+    # size the sample from a 4-receiver probe
+    probe = np.linspace(0, cfg.n - 1, 4).round().astype(int)
+    t0 = time.perf_counter()
+    oracle.synthesis(np.ascontiguousarray(R[:, probe]), N0, cfg.dt, w, klo, khi)
+    per_rec = (time.perf_counter() - t0) / 4 * max(1, min(4, oracle.num_threads())) / max(1, oracle.num_threads())
+    nrec_s = int(min(cfg.n, max(oracle.num_threads(), budget_s / max(per_rec, 1e-6))))
+    recs = np.linspace(0, cfg.n - 1, nrec_s).round().astype(int)
+    Rs = np.ascontiguousarray(R[:, recs])
+    t0 = time.perf_counter()
+    oracle.synthesis(Rs, N0, cfg.dt, w, klo, khi)
+    return time.perf_counter() - t0, nrec_s, N0, (w, klo, khi)
+
+
+def run_reference(args):
+    """--impl reference: the oracle is the reference arm.  Each step = one synthesis on a bounded receiver sample."""
+    rank, world, _ = dist_env()
+    if rank != 0:
+        return 0
+    import oracle
+    cfg = configs.get(args.workload)
+    R, Gd, td = workload_arrays(cfg) if cfg.nfoc == 1 else (gen.R_full(cfg), *gen.first_arrivals(cfg, focs=[cfg.nfoc // 2]))
+    nbytes, nb = rhat_bytes(cfg)
+    total_budget = 150.0
+    per_step = total_budget / (args.steps + args.warmup)
+    _, _, N0, (w, klo, khi) = oracle_sample(cfg, R, Gd, td, budget_s=per_step)
+    # pick the sample so that one step fits per_step seconds
+    probe = np.linspace(0, cfg.n - 1, 4).round().astype(int)
+    t0 = time.perf_counter()
+    oracle.synthesis(np.ascontiguousarray(R[:, probe]), N0, cfg.dt, w, klo, khi)
+    t_probe = time.perf_counter() - t0
+    nrec_s = int(min(cfg.n, max(1, 4 * per_step / max(t_probe, 1e-6))))
+    recs = np.linspace(0, cfg.n - 1, nrec_s).round().astype(int)
+    Rs = np.ascontiguousarray(R[:, recs])
+    for _ in range(args.warmup):
+        oracle.synthesis(Rs, N0, cfg.dt, w, klo, khi)
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        oracle.synthesis(Rs, N0, cfg.dt, w, klo, khi)
+    dt_s = time.perf_counter() - t0
+    val = (nbytes * nrec_s / cfg.n) * args.steps / dt_s / 1e9
+    sample = f"per step: one oracle synthesis R N_0 on {nrec_s} of {cfg.n} receivers x 1 focal point of config {cfg.k}"
+    line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": 1e3 * dt_s / args.steps, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": f"config{cfg.k}:{cfg.name}", "n": cfg.n, "nt": cfg.nt, "nfoc": 1, "nb": nb, "sample": sample},
+            "cpu_baseline": {"value": val, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle", "sample": sample},
+            "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}, "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+    return 0
+
+
+# ------------------------------------------------------------------------------------------------ our arm
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+    from paper_2106_04649_b200 import binding as B
+
+    rank, world, local = dist_env()
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device (there is no CPU fallback)")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    dev = torch.device("cuda", local)
+
+    cfg = shard.replica_config(configs.get(args.workload), rank, world)   # weak scaling: replicas, no collective
+    R, Gd, td = workload_arrays(cfg)
+    nbytes, nb = rhat_bytes(cfg)
+    nfoc, niter, nsyn = cfg.nfoc, cfg.niter, nsyn_per_step(cfg)
+    fields = ("N_last", "f1plus", "f1min", "G", "Gplus", "Gminus")
+
+    mk = B.Marchenko(cfg.n, cfg.n, cfg.nt, cfg.dt, cfg.dx, cfg.fmin, cfg.fmax)
+    mk.set_option(B.MK_OPT_EPS_SAMPLES, cfg.eps)
+    mk.set_option(B.MK_OPT_REGIME, args.regime)
+    mk.load_R_host(R)
+    dGd = torch.from_numpy(Gd).to(dev)
+    dtd = torch.from_numpy(td).to(dev)
+    douts = {nm: torch.empty((nfoc, cfg.n, cfg.nt), dtype=torch.float32, device=dev) for nm in fields}
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    # ---- device-timed region: inputs resident in HBM
+    for _ in range(args.warmup):
+        mk.run(dGd, dtd, niter, douts)
+    mk.set_option(B.MK_OPT_TIMING, 1)
+    mk.get_info(B.MK_INFO_SYN_RESET)
+    l0 = mk.get_info(B.MK_INFO_KERNEL_LAUNCHES)
+    barrier()
+    sampler = ClockSampler(local)
+    sampler.start()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(args.steps):
+        mk.run(dGd, dtd, niter, douts)
+    e1.record()
+    barrier()
+    clocks = sampler.stop()
+    ms_total = shard.max_over_ranks(e0.elapsed_time(e1), dist)
+    launches = int(mk.get_info(B.MK_INFO_KERNEL_LAUNCHES) - l0)
+    syn_n = mk.get_info(B.MK_INFO_SYN_LAUNCHES)
+    syn_ms = mk.get_info(B.MK_INFO_SYN_MS_TOTAL)
+    regime_used = int(mk.get_info(B.MK_INFO_REGIME_USED))
+    mk.set_option(B.MK_OPT_TIMING, 0)
+    value = world * nsyn * nbytes * args.steps / (ms_total * 1e-3) / 1e9
+
+    # ---- end-to-end through the public host API: pinned host inputs, host outputs, copies inside the timed region
+    hGd = torch.from_numpy(Gd).pin_memory()
+    htd = torch.from_numpy(td).pin_memory()
+    houts = {nm: torch.empty((nfoc, cfg.n, cfg.nt), dtype=torch.float32).pin_memory() for nm in fields}
+    e2e_steps = max(1, min(args.steps, args.e2e_steps))
+    for _ in range(min(3, args.warmup)):
+        mk.run_host(hGd, htd, niter, houts)
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(e2e_steps):
+        mk.run_host(hGd, htd, niter, houts)          # returns after the results are in host memory
+    torch.cuda.synchronize()
+    e2e_s = shard.max_over_ranks(time.perf_counter() - t0, dist)
+    barrier()
+    e2e_val = world * nsyn * nbytes * e2e_steps / e2e_s / 1e9
+    h2d = int(hGd.numel() * 4 + htd.numel() * 4)
+    d2h = int(sum(t.numel() * 4 for t in houts.values()))
+
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return 0
+
+    # ---- roofline of the dominant kernel (the contraction), from CUDA events recorded by the library on its stream
+    peaks = measured_peaks()
+    avg_ms = syn_ms / max(syn_n, 1)
+    traffic = None
+    tp = ROOT / "profiles" / "traffic.json"
+    if tp.exists():
+        traffic = json.loads(tp.read_text()).get(f"config{cfg.k}_regime{regime_used}")
+    if regime_used == 1:
+        ach = nbytes / (avg_ms * 1e-3) / 1e9
+        roof = {"bound": "hbm", "kernel": "k_syn_gemv", "achieved": ach, "peak": peaks["hbm_gbs"], "unit": "GB/s",
+                "frac": ach / peaks["hbm_gbs"], "traffic": traffic, "peak_source": peaks["source"] + " copy bandwidth (MEASURED_PEAKS.json)",
+                "frac_of_nominal_8TBps": ach / 8000.0, "launches_timed": int(syn_n), "avg_launch_ms": avg_ms,
+                "share_of_step": syn_ms / ms_total}
+    else:
+        flops = 8.0 * nfoc * cfg.n * cfg.n * nb
+        ach = flops / (avg_ms * 1e-3) / 1e12
+        sm_max = clocks.get("sm_max_mhz") or 1965.0
+        peak = 2 * 128 * 148 * sm_max * 1e6 / 1e12     # FFMA lanes x SMs x max clock
+        roof = {"bound": "alu", "kernel": "k_syn_gemm_ffma", "achieved": ach, "peak": peak, "unit": "TFLOP/s", "frac": ach / peak,
+                "traffic": traffic, "peak_source": "2 x 128 FFMA lanes x 148 SMs x clocks.max.sm (guide unit counts)",
+                "launches_timed": int(syn_n), "avg_launch_ms": avg_ms, "share_of_step": syn_ms / ms_total}
+
+    # ---- the oracle as it stands, on this box's host cores, bounded sample (rank 0, N = 1 only)
+    cpu = None
+    if world == 1 and not args.no_cpu_baseline:
+        import oracle
+        f = [0] if nfoc > 1 else None
+        t_s, nrec_s, _, _ = oracle_sample(cfg, R, Gd if f is None else Gd[f], td if f is None else td[f], budget_s=args.cpu_budget)
+        cpu = {"value": (nbytes * nrec_s / cfg.n) / t_s / 1e9, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle",
+               "sample": f"one oracle synthesis R N_0 (direct time-domain convolution, fp64) on {nrec_s} of {cfg.n} receivers x 1 focal "
+                         f"point of config {cfg.k}: {t_s:.2f} s"}
+
+    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": ms_total / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f32", "data": "synthetic",
+            "config": {"workload": f"config{cfg.k}:{cfg.name}", "n": cfg.n, "nt": cfg.nt, "nfoc": nfoc, "niter": niter, "nb": nb,
+                       "syntheses_per_step": nsyn, "rhat_bytes": nbytes, "regime": regime_used,
+                       "l2": "inputs_larger_than_L2 (R^ 1.30 GB vs 126 MB L2; no flush needed)",
+                       "parallelism": "1 GPU" if world == 1 else f"{world} independent replicas (no collective)"},
+            "focal_point_iterations_per_s": world * nfoc * niter * args.steps / (ms_total * 1e-3),
+            "clocks": clocks,
+            "e2e": {"value": e2e_val, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h, "steps": e2e_steps,
+                    "ms_per_step": 1e3 * e2e_s / e2e_steps, "api": "mk_run_host (pinned host G_d, t_d in; 6 host fields out)"},
+            "gpu_launches": launches, "roofline": roof, "cpu_baseline": cpu}
+    print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+    mk.close()
+    return 0
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=400)
+    ap.add_argument("--warmup", type=int, default=10)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", type=int, default=1, help="BASELINE.json config index (default 1)")
+    ap.add_argument("--regime", type=int, default=0)
+    ap.add_argument("--e2e-steps", type=int, default=50)
+    ap.add_argument("--cpu-budget", type=float, default=15.0, help="seconds of oracle work for cpu_baseline")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.warmup < 3 and args.impl == "ours":
+        args.warmup = 3
+    return run_reference(args) if args.impl == "reference" else run_ours(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())

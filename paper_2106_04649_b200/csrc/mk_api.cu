@@ -75,22 +75,24 @@ inline int ldf_for(int regime, int nfoc) { return regime == 1 ? nfoc : ((nfoc + 
 // a2: S^ = R^ x N^ per bin, on the context's stream; optionally bracketed by events
 int contract(mk_ctx* c, const float2* Nhat, float2* Shat, int nfoc, int ldf, int regime) {
   cudaEvent_t e0 = nullptr, e1 = nullptr;
-  if (c->timing) {
-    if (c->ev_used + 2 > c->ev.size()) {
-      if (c->ev.size() >= 16384) return set_err(c, MK_ERR_STATE, "timing event pool exhausted; read MK_INFO_SYN_MS_TOTAL / reset");
+  bool timed = c->timing != 0;
+  if (timed && c->ev_used + 2 > c->ev.size()) {
+    if (c->ev.size() >= 65536) timed = false;  // pool full: later launches go untimed (read / reset the counters)
+    else
       for (int i = 0; i < 2; ++i) {
         cudaEvent_t e;
         if (int rc = check_cuda(c, cudaEventCreate(&e), "cudaEventCreate")) return rc;
         c->ev.push_back(e);
       }
-    }
+  }
+  if (timed) {
     e0 = c->ev[c->ev_used];
     e1 = c->ev[c->ev_used + 1];
     c->ev_used += 2;
     cudaEventRecord(e0, c->stream);
   }
   int rc = regime == 1 ? launch_syn_gemv(c, Nhat, Shat, nfoc) : launch_syn_gemm(c, Nhat, Shat, ldf);
-  if (c->timing) cudaEventRecord(e1, c->stream);
+  if (timed) cudaEventRecord(e1, c->stream);
   c->regime_used = regime;
   return rc;
 }
