@@ -52,6 +52,11 @@ def lib():
         L.orc_marchenko.restype = C.c_int
         L.orc_marchenko.argtypes = [C.c_int, C.c_int, C.c_double, C.c_double, C.c_double, C.c_double, C.c_int,
                                     _F32, C.c_int, _F32, _F32, C.c_int] + [C.c_void_p] * 8
+        L.orc_step_subset.argtypes = [C.c_int, C.c_int, C.c_int, C.c_double, _F64, _F32, C.c_int, _F64, _I32, C.c_int,
+                                      C.c_int, C.c_int, _F64] + [C.c_void_p] * 5
+        L.orc_finals_subset.argtypes = [C.c_int, C.c_int, C.c_int, C.c_double, _F64, _F32, C.c_int, _F64, _F64, _F64,
+                                        _F64, _F64, _F64, C.c_int, C.c_int] + [C.c_void_p] * 3
+        L.orc_image.argtypes = [C.c_int, C.c_int, C.c_double, _F64, C.c_int, _F64, _F64, _F64]
         _lib = L
     return _lib
 
@@ -139,4 +144,64 @@ def marchenko(R: np.ndarray, Gd: np.ndarray, td: np.ndarray, dt: float, dx: floa
     rc = lib().orc_marchenko(n, nt, dt, dx, fmin, fmax, eps, R.reshape(-1), nfoc, Gd.reshape(-1), td.reshape(-1),
                              niter, *ptrs)
     assert rc == 0
+    return out
+
+
+def _opt(a):
+    return None if a is None else a.ctypes.data_as(C.c_void_p)
+
+
+class SubsetChain:
+    """The oracle restricted to a subset of output receivers (SURVEY.md §8(c) "single step"): every step takes the
+    previous iterate at EVERY source position (supplied by the caller) and advances the subset accumulators with
+    orc_step_subset; finals() is orc_finals_subset.  R_sub: [nshot][nrout][nt] fp32; td_sub: [nfoc][nrout] fp32."""
+
+    def __init__(self, R_sub, td_sub, Gd_sub, dt, dx, fmin, fmax, eps=8):
+        self.R = np.ascontiguousarray(R_sub, dtype=np.float32)
+        self.nshot, self.nrout, self.nt = self.R.shape
+        self.dt = float(dt)
+        self.w = weights(self.nshot, dx)
+        self.klo, self.khi, self.nb = band(self.nt, dt, fmin, fmax)
+        self.h = window(td_sub, self.nt, dt, eps)
+        self.nfoc = self.h.shape[0]
+        assert self.h.shape == (self.nfoc, self.nrout)
+        Gd_sub = np.ascontiguousarray(Gd_sub, dtype=np.float32)
+        assert Gd_sub.shape == (self.nfoc, self.nrout, self.nt)
+        # O4 on the subset: f1plus = f2 = T G_d; f1min = pmin = 0   [PAPER.md:19, 67, 74-75]
+        TG = np.roll(Gd_sub[..., ::-1], 1, axis=-1).astype(np.float64)
+        self.f1plus = TG.copy()
+        self.f2 = TG.copy()
+        self.f1min = np.zeros_like(TG)
+        self.pmin = np.zeros_like(TG)
+        self.it = 0
+
+    def step(self, N_prev_all):
+        """N_prev_all: [nfoc][nshot][nt]; returns the new iterate on the subset, float64 [nfoc][nrout][nt]."""
+        N_prev_all = np.ascontiguousarray(N_prev_all, dtype=np.float64)
+        assert N_prev_all.shape == (self.nfoc, self.nshot, self.nt)
+        Nn = np.empty((self.nfoc, self.nrout, self.nt), dtype=np.float64)
+        lib().orc_step_subset(self.nshot, self.nrout, self.nt, self.dt, self.w, self.R.reshape(-1), self.nfoc,
+                              N_prev_all.reshape(-1), self.h.reshape(-1), self.klo, self.khi, self.it, Nn.reshape(-1),
+                              None, _opt(self.pmin), _opt(self.f2), _opt(self.f1plus), _opt(self.f1min))
+        self.it += 1
+        return Nn
+
+    def finals(self, f1plus_all, f1min_all, want=("G", "Gplus", "Gminus")):
+        f1plus_all = np.ascontiguousarray(f1plus_all, dtype=np.float64)
+        f1min_all = np.ascontiguousarray(f1min_all, dtype=np.float64)
+        out = {nm: np.empty_like(self.f2) for nm in want}
+        lib().orc_finals_subset(self.nshot, self.nrout, self.nt, self.dt, self.w, self.R.reshape(-1), self.nfoc,
+                                f1plus_all.reshape(-1), f1min_all.reshape(-1), self.f1plus.reshape(-1),
+                                self.f1min.reshape(-1), self.f2.reshape(-1), self.pmin.reshape(-1), self.klo, self.khi,
+                                _opt(out.get("G")), _opt(out.get("Gplus")), _opt(out.get("Gminus")))
+        return out
+
+
+def image(Gminus, f1plus, dt, dx):
+    """image[f] = dt sum_r w[r] sum_j G^-[f][r][(nt-j)%nt] f1plus[f][r][j]  (NEXT-1)."""
+    Gminus = np.ascontiguousarray(Gminus, dtype=np.float64)
+    f1plus = np.ascontiguousarray(f1plus, dtype=np.float64)
+    nfoc, n, nt = Gminus.shape
+    out = np.empty(nfoc, dtype=np.float64)
+    lib().orc_image(n, nt, dt, weights(n, dx), nfoc, Gminus.reshape(-1), f1plus.reshape(-1), out)
     return out

@@ -177,10 +177,92 @@ void orc_synthesis(int nshot, int nrout, int nt, double dt, const double* w, con
   }
 }
 
+// O5 for a SUBSET of output receivers (one pass of the loop body), the "single step" of
+// N_prev [nfoc][nshot][nt] is the previous iterate at EVERY source position; R [nshot][nrout][nt]
+// holds the traces of the chosen output receivers for every shot; h [nfoc][nrout] their window half-widths.
+// Updates the subset accumulators pmin, f2, f1plus, f1min (each [nfoc][nrout][nt], any may be NULL) and writes the
+// new iterate N_new [nfoc][nrout][nt] and (optionally) the unwindowed synthesis S_out.
+void orc_step_subset(int nshot, int nrout, int nt, double dt, const double* w, const float* R, int nfoc,
+                     const double* N_prev, const int* h, int klo, int khi, int it, double* N_new, double* S_out,
+                     double* pmin, double* f2, double* f1plus, double* f1min) {
+  const size_t ntr = (size_t)nfoc * nrout, tot = ntr * nt;
+  std::vector<double> Sloc;
+  double* S = S_out;
+  if (!S) {
+    Sloc.resize(tot);
+    S = Sloc.data();
+  }
+  orc_synthesis(nshot, nrout, nt, dt, w, R, nfoc, N_prev, klo, khi, S);          // O5a [PAPER.md:69]
+  if (pmin)
+    for (size_t i = 0; i < tot; ++i) pmin[i] += S[i];                            // O5b [PAPER.md:79]
+  for (size_t i = 0; i < ntr; ++i)                                               // O5c [PAPER.md:71-72, 78, 80]
+    for (int j = 0; j < nt; ++j)
+      N_new[i * nt + j] = -(double)orc_theta(nt, h[i], j) * S[i * nt + wrapi((long)nt - j, nt)];
+  if (f2)
+    for (size_t i = 0; i < tot; ++i) f2[i] += N_new[i];                          // O5d [PAPER.md:81]
+  if (it % 2 == 0) {                                                             //     [PAPER.md:82-83]
+    if (f1min)
+      for (size_t i = 0; i < ntr; ++i)
+        for (int j = 0; j < nt; ++j) f1min[i * nt + j] -= N_new[i * nt + wrapi((long)nt - j, nt)];
+  } else {                                                                       //     [PAPER.md:84-85]
+    if (f1plus)
+      for (size_t i = 0; i < tot; ++i) f1plus[i] += N_new[i];
+  }
+}
+
+// O6 for a SUBSET of output receivers [PAPER.md:24, 87-88; readings G3, G4, G5].  f1plus_all / f1min_all
+// [nfoc][nshot][nt] are the operands of the two extra syntheses (every source position); f1plus / f1min / f2 / pmin
+// [nfoc][nrout][nt] are the same fields on the chosen receivers.  Outputs [nfoc][nrout][nt], any may be NULL.
+void orc_finals_subset(int nshot, int nrout, int nt, double dt, const double* w, const float* R, int nfoc,
+                       const double* f1plus_all, const double* f1min_all, const double* f1plus, const double* f1min,
+                       const double* f2, const double* pmin, int klo, int khi, double* G_out, double* Gplus_out,
+                       double* Gminus_out) {
+  const size_t ntr = (size_t)nfoc * nrout, tot = ntr * nt;
+  std::vector<double> S(tot), tmp(nt);
+  if (Gminus_out) {  // G- = R f1plus - f1min
+    orc_synthesis(nshot, nrout, nt, dt, w, R, nfoc, f1plus_all, klo, khi, S.data());
+    for (size_t i = 0; i < tot; ++i) Gminus_out[i] = S[i] - f1min[i];
+  }
+  if (Gplus_out) {  // G+ = T f1plus - R (T f1min)
+    const size_t ntr_all = (size_t)nfoc * nshot;
+    std::vector<double> Tf(ntr_all * nt);
+    for (size_t i = 0; i < ntr_all; ++i) time_reverse(f1min_all + i * nt, Tf.data() + i * nt, nt);
+    orc_synthesis(nshot, nrout, nt, dt, w, R, nfoc, Tf.data(), klo, khi, S.data());
+    for (size_t i = 0; i < ntr; ++i) {
+      time_reverse(f1plus + i * nt, tmp.data(), nt);
+      for (int j = 0; j < nt; ++j) Gplus_out[i * nt + j] = tmp[j] - S[i * nt + j];
+    }
+  }
+  if (G_out) {  // G = p- + T f2
+    for (size_t i = 0; i < ntr; ++i) {
+      time_reverse(f2 + i * nt, tmp.data(), nt);
+      for (int j = 0; j < nt; ++j) G_out[i * nt + j] = pmin[i * nt + j] + tmp[j];
+    }
+  }
+}
+
+// NEXT-1: double-focusing image, the zero-time sample of G^- convolved with f1plus and integrated
+// over receivers [PAPER.md:24 last sentences, 89]:  image[f] = dt sum_r w[r] sum_j G^-[f][r][(nt-j)%nt] f1plus[f][r][j].
+void orc_image(int n, int nt, double dt, const double* w, int nfoc, const double* Gminus, const double* f1plus,
+               double* image) {
+  for (int f = 0; f < nfoc; ++f) {
+    double acc = 0.0;
+    for (int r = 0; r < n; ++r) {
+      const double* g = Gminus + ((size_t)f * n + r) * nt;
+      const double* p = f1plus + ((size_t)f * n + r) * nt;
+      double part = 0.0;
+      for (int j = 0; j < nt; ++j) part += g[wrapi((long)nt - j, nt)] * p[j];
+      acc += w[r] * part;
+    }
+    image[f] = dt * acc;
+  }
+}
+
 // O4..O6: the whole scheme (Algorithm 1, accumulating "on the fly" as the paper says its
 // CPU version does).  Square geometry: R [n][n][nt] fp32, Gd [nfoc][n][nt] fp32, td [nfoc][n] fp32.
 // Outputs (double, each [nfoc][n][nt], any may be NULL): N_iters [niter][nfoc][n][nt] (every iterate N_i),
-// f1plus, f1min, f2, pmin, G, Gplus, Gminus.  Returns 0.
+// f1plus, f1min, f2, pmin, G, Gplus, Gminus.  Returns 0.  (The loop body and the finals are the subset routines
+// above with the subset = every receiver.)
 int orc_marchenko(int n, int nt, double dt, double dx, double fmin, double fmax, int eps, const float* R, int nfoc,
                   const float* Gd, const float* td, int niter, double* N_iters, double* f1plus_out,
                   double* f1min_out, double* f2_out, double* pmin_out, double* G_out, double* Gplus_out,
@@ -194,7 +276,7 @@ int orc_marchenko(int n, int nt, double dt, double dx, double fmin, double fmax,
   orc_window((int)ntr, nt, dt, eps, td, h.data());
 
   // O4: N_{-1} = f1plus = f2 = T G_d;  f1min = pmin = 0      [PAPER.md:19, 67, 74-75]
-  std::vector<double> N(tot), f1plus(tot), f2(tot), f1min(tot, 0.0), pmin(tot, 0.0), S(tot), tmp(nt);
+  std::vector<double> N(tot), Nn(tot), f1plus(tot), f2(tot), f1min(tot, 0.0), pmin(tot, 0.0);
   for (size_t i = 0; i < ntr; ++i)
     for (int j = 0; j < nt; ++j) N[i * nt + j] = (double)Gd[i * nt + wrapi((long)nt - j, nt)];
   f1plus = N;
@@ -202,41 +284,15 @@ int orc_marchenko(int n, int nt, double dt, double dx, double fmin, double fmax,
 
   // O5: niter passes, i = 0 .. niter-1                        [PAPER.md:68, 76; reading G6]
   for (int it = 0; it < niter; ++it) {
-    orc_synthesis(n, n, nt, dt, w.data(), R, nfoc, N.data(), klo, khi, S.data());  // O5a [PAPER.md:69]
-    for (size_t i = 0; i < tot; ++i) pmin[i] += S[i];                             // O5b [PAPER.md:79]
-    for (size_t i = 0; i < ntr; ++i)                                              // O5c [PAPER.md:71-72, 78, 80]
-      for (int j = 0; j < nt; ++j)
-        N[i * nt + j] = -(double)orc_theta(nt, h[i], j) * S[i * nt + wrapi((long)nt - j, nt)];
-    for (size_t i = 0; i < tot; ++i) f2[i] += N[i];                               // O5d [PAPER.md:81]
-    if (it % 2 == 0) {                                                            //     [PAPER.md:82-83]
-      for (size_t i = 0; i < ntr; ++i)
-        for (int j = 0; j < nt; ++j) f1min[i * nt + j] -= N[i * nt + wrapi((long)nt - j, nt)];
-    } else {                                                                      //     [PAPER.md:84-85]
-      for (size_t i = 0; i < tot; ++i) f1plus[i] += N[i];
-    }
+    orc_step_subset(n, n, nt, dt, w.data(), R, nfoc, N.data(), h.data(), klo, khi, it, Nn.data(), nullptr, pmin.data(),
+                    f2.data(), f1plus.data(), f1min.data());
+    N.swap(Nn);
     if (N_iters) std::memcpy(N_iters + (size_t)it * tot, N.data(), tot * sizeof(double));
   }
 
-  // O6: finals                                                [PAPER.md:24, 87-88; readings G3, G4, G5]
-  if (Gminus_out) {  // G- = R f1plus - f1min
-    orc_synthesis(n, n, nt, dt, w.data(), R, nfoc, f1plus.data(), klo, khi, S.data());
-    for (size_t i = 0; i < tot; ++i) Gminus_out[i] = S[i] - f1min[i];
-  }
-  if (Gplus_out) {  // G+ = T f1plus - R (T f1min)
-    std::vector<double> Tf(tot);
-    for (size_t i = 0; i < ntr; ++i) time_reverse(f1min.data() + i * nt, Tf.data() + i * nt, nt);
-    orc_synthesis(n, n, nt, dt, w.data(), R, nfoc, Tf.data(), klo, khi, S.data());
-    for (size_t i = 0; i < ntr; ++i) {
-      time_reverse(f1plus.data() + i * nt, tmp.data(), nt);
-      for (int j = 0; j < nt; ++j) Gplus_out[i * nt + j] = tmp[j] - S[i * nt + j];
-    }
-  }
-  if (G_out) {  // G = p- + T f2
-    for (size_t i = 0; i < ntr; ++i) {
-      time_reverse(f2.data() + i * nt, tmp.data(), nt);
-      for (int j = 0; j < nt; ++j) G_out[i * nt + j] = pmin[i * nt + j] + tmp[j];
-    }
-  }
+  // O6: finals
+  orc_finals_subset(n, n, nt, dt, w.data(), R, nfoc, f1plus.data(), f1min.data(), f1plus.data(), f1min.data(), f2.data(),
+                    pmin.data(), klo, khi, G_out, Gplus_out, Gminus_out);
   if (f1plus_out) std::memcpy(f1plus_out, f1plus.data(), tot * sizeof(double));
   if (f1min_out) std::memcpy(f1min_out, f1min.data(), tot * sizeof(double));
   if (f2_out) std::memcpy(f2_out, f2.data(), tot * sizeof(double));

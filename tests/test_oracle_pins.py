@@ -308,3 +308,47 @@ def test_geometric_series_closed_form_dense_matrices():
     for k in range(K):
         v = A @ v
         np.testing.assert_allclose(o["N_iters"][k].reshape(-1), v, atol=1e-12 * np.abs(b).max())
+
+
+def test_subset_chain_fed_with_full_iterates_equals_the_full_chain_restricted():
+    """Host logic of the "single step" parity harness: a proper receiver subset, fed at every step with the previous
+    iterate at every source position, reproduces the full chain on that subset (iterates, accumulators, finals)."""
+    n, nt, nfoc, dt, dx, eps, K = 7, 32, 2, 0.004, 10.0, 1, 5
+    fmin, fmax = 20.0, 100.0
+    R = (0.02 * rng.standard_normal((n, n, nt))).astype(np.float32)
+    Gd = rng.standard_normal((nfoc, n, nt)).astype(np.float32)
+    td = (dt * rng.uniform(5, 12, size=(nfoc, n))).astype(np.float32)
+    full = oracle.marchenko(R, Gd, td, dt, dx, fmin, fmax, niter=K, eps=eps)
+    recs = np.array([1, 4, 6])
+    sub = oracle.SubsetChain(R[:, recs], td[:, recs], Gd[:, recs], dt, dx, fmin, fmax, eps)
+    prev = T(Gd.astype(np.float64))
+    for it in range(K):
+        Nn = sub.step(prev)
+        np.testing.assert_array_equal(Nn, full["N_iters"][it][:, recs])
+        prev = full["N_iters"][it]
+    for nm in ("f1plus", "f1min", "f2", "pmin"):
+        np.testing.assert_array_equal(getattr(sub, nm), full[nm][:, recs])
+    fin = sub.finals(full["f1plus"], full["f1min"])
+    for nm in ("G", "Gplus", "Gminus"):
+        np.testing.assert_array_equal(fin[nm], full[nm][:, recs])
+
+
+def test_image_is_the_zero_lag_of_the_convolution():
+    """image[f] = dt sum_r w[r] (G^- (*) f1plus)[0]: brute force on a tiny case and numpy's FFT convolution theorem."""
+    nfoc, n, nt, dt, dx = 3, 5, 16, 0.004, 10.0
+    g = rng.standard_normal((nfoc, n, nt))
+    p = rng.standard_normal((nfoc, n, nt))
+    w = np.full(n, dx)
+    w[0] = w[-1] = dx / 2
+    brute = np.array([dt * sum(w[r] * sum(g[f, r, (0 - j) % nt] * p[f, r, j] for j in range(nt)) for r in range(n))
+                      for f in range(nfoc)])
+    lag0 = np.fft.irfft(np.fft.rfft(g) * np.fft.rfft(p), nt)[..., 0]
+    got = oracle.image(g, p, dt, dx)
+    np.testing.assert_allclose(got, brute, rtol=1e-13)
+    np.testing.assert_allclose(got, dt * (lag0 * w).sum(axis=1), rtol=1e-12)
+    # a pure delay pair: G^- = delta(t - a), f1plus = delta(t + a)  =>  image = dt * sum w
+    g[:] = 0.0
+    p[:] = 0.0
+    g[..., 3] = 1.0
+    p[..., nt - 3] = 1.0
+    np.testing.assert_allclose(oracle.image(g, p, dt, dx), dt * w.sum())

@@ -109,3 +109,25 @@ def test_config0_host_api_and_run_match_steps():
         np.testing.assert_array_equal(a[nm], c[nm])
     np.testing.assert_array_equal(a["N_iters"][-1], b["N_last"])
     np.testing.assert_array_equal(b["N_last"], c["N_last"])
+
+
+def test_image_matches_oracle():
+    """NEXT-1: double-focusing image of a small multi-focal run against the oracle's definition."""
+    import torch
+    from paper_2106_04649_b200 import binding as B
+    cfg = calibrated(configs.scaled(2, n=48, nt=256, nfoc=48, focal="line:300", niter=6))
+    R, Gd, td = problem(cfg)
+    ref = _oracle_chain(cfg, R, Gd, td)
+    img_ref = oracle.image(ref["Gminus"], ref["f1plus"], cfg.dt, cfg.dx)
+    dev = torch.device("cuda:0")
+    with B.Marchenko(cfg.n, cfg.n, cfg.nt, cfg.dt, cfg.dx, cfg.fmin, cfg.fmax) as mk:
+        mk.set_option(B.MK_OPT_EPS_SAMPLES, cfg.eps)
+        mk.load_R(torch.from_numpy(R).to(dev))
+        outs = {"Gminus": torch.empty((cfg.nfoc, cfg.n, cfg.nt), dtype=torch.float32, device=dev)}
+        mk.run(torch.from_numpy(Gd).to(dev), torch.from_numpy(td).to(dev), cfg.niter, outs)
+        img = torch.empty(cfg.nfoc, dtype=torch.float32, device=dev)
+        mk.image(outs["Gminus"], img)
+        img = img.cpu().numpy()
+    e = rel_l2(img, img_ref)
+    print(f"\n[image nfoc={cfg.nfoc}] rel L2 {e:.2e}")
+    assert e <= TOL_FINAL

@@ -1,0 +1,75 @@
+"""Multi-GPU host logic on CPU: world_size-2 `gloo` processes.  The path has no data-path
+collective (focal points are independent): ranks own disjoint focal slices, torch.distributed carries
+only the barrier and the max / sum over ranks that bench.py uses for its timing."""
+import os
+import socket
+
+import numpy as np
+import pytest
+
+from paper_2106_04649_b200 import configs, gen, shard
+
+
+def test_focal_slices_partition_every_count():
+    for nfoc in (1, 2, 7, 64, 256, 601):
+        for world in (1, 2, 3, 4, 8):
+            got = [i for r in range(world) for i in shard.focal_slice(nfoc, r, world)]
+            assert got == list(range(nfoc))
+            sizes = [len(shard.focal_slice(nfoc, r, world)) for r in range(world)]
+            assert max(sizes) - min(sizes) <= 1
+    with pytest.raises(ValueError):
+        shard.focal_slice(4, 2, 2)
+
+
+def test_replica_config_moves_the_focal_depth_only():
+    cfg = configs.get(1)
+    assert shard.replica_config(cfg, 0, 4) is cfg
+    c2 = shard.replica_config(cfg, 2, 4)
+    assert c2.focal == "single:850.0" and c2.n == cfg.n and c2.seed == cfg.seed and c2.A_R == cfg.A_R
+
+
+def _free_port():
+    s = socket.socket()
+    s.bind(("127.0.0.1", 0))
+    p = s.getsockname()[1]
+    s.close()
+    return p
+
+
+def _worker(rank, world, port, q):
+    import torch.distributed as dist
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), RANK=str(rank), WORLD_SIZE=str(world))
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    try:
+        cfg = configs.scaled(2, n=12, nt=64, nfoc=12, focal="line:300")
+        mine = list(shard.focal_slice(cfg.nfoc, rank, world))
+        gd, td = gen.first_arrivals(cfg, focs=mine)          # each rank generates only its own focal points
+        dist.barrier()
+        t_max = shard.max_over_ranks(10.0 + rank, dist)      # the max-over-ranks timing of bench.py
+        n_sum = shard.sum_over_ranks(float(len(mine)), dist)
+        q.put((rank, mine, float(gd.astype(np.float64).sum()), td.shape, t_max, n_sum))
+    finally:
+        dist.destroy_process_group()
+
+
+def test_world_size_2_gloo_focal_sharding():
+    import torch.multiprocessing as mp
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    port, world = _free_port(), 2
+    procs = [ctx.Process(target=_worker, args=(r, world, port, q)) for r in range(world)]
+    for p in procs:
+        p.start()
+    res = sorted(q.get(timeout=120) for _ in range(world))
+    for p in procs:
+        p.join(timeout=60)
+        assert p.exitcode == 0
+    cfg = configs.scaled(2, n=12, nt=64, nfoc=12, focal="line:300")
+    gd_all, td_all = gen.first_arrivals(cfg)
+    owned = []
+    for rank, mine, gsum, tshape, t_max, n_sum in res:
+        owned += mine
+        assert tshape == (len(mine), cfg.n)
+        assert gsum == float(gd_all[mine].astype(np.float64).sum())     # shards see the same bytes as the whole job
+        assert t_max == 11.0 and n_sum == float(cfg.nfoc)
+    assert owned == list(range(cfg.nfoc))
