@@ -129,6 +129,24 @@ MK_HD void dft_small(float2* a) {
   else dft2<INV>(a[0], a[1]);
 }
 
+// Twiddles w[m] = tw[m * tstep], m = 1 .. R-1.  Only the power-of-two multiples are read from the table (the table
+// lives in global memory / L1); the others are products of two table entries (one extra rounding, ~6e-8).
+template <int LGR>
+MK_HD void load_twiddles(float2* w, const float2* __restrict__ tw, int tstep) {
+  w[0] = make_float2(1.f, 0.f);
+  w[1] = tw[tstep];
+  if constexpr (LGR >= 2) {
+    w[2] = tw[2 * tstep];
+    w[3] = cmul(w[1], w[2]);
+  }
+  if constexpr (LGR >= 3) {
+    w[4] = tw[4 * tstep];
+    w[5] = cmul(w[4], w[1]);
+    w[6] = cmul(w[4], w[2]);
+    w[7] = cmul(w[4], w[3]);
+  }
+}
+
 // One butterfly (index t in [0, M >> LGR)) of forward pass with block length 2^lgL.  z: padded trace buffer,
 // tw[k] = e^{-2 pi i k / nt}, k in [0, nt).
 template <int LGR>
@@ -142,8 +160,10 @@ MK_HD void fwd_butterfly(float2* z, const float2* __restrict__ tw, int nt, int l
   for (int j = 0; j < R; ++j) a[j] = z[padi(base + (j << lgq))];
   dft_small<LGR, false>(a);
   const int tstep = i * (nt >> lgL);  // w_L^{i m} = tw[i m nt/L]
+  float2 w[R];
+  load_twiddles<LGR>(w, tw, tstep);
 #pragma unroll
-  for (int m = 1; m < R; ++m) a[m] = cmul(a[m], tw[tstep * m]);
+  for (int m = 1; m < R; ++m) a[m] = cmul(a[m], w[m]);
 #pragma unroll
   for (int m = 0; m < R; ++m) z[padi(base + (m << lgq))] = a[m];
 }
@@ -159,8 +179,10 @@ MK_HD void inv_butterfly(float2* z, const float2* __restrict__ tw, int nt, int l
 #pragma unroll
   for (int m = 0; m < R; ++m) a[m] = z[padi(base + (m << lgq))];
   const int tstep = i * (nt >> lgL);
+  float2 w[R];
+  load_twiddles<LGR>(w, tw, tstep);
 #pragma unroll
-  for (int m = 1; m < R; ++m) a[m] = cmulc(a[m], tw[tstep * m]);
+  for (int m = 1; m < R; ++m) a[m] = cmulc(a[m], w[m]);
   dft_small<LGR, true>(a);
 #pragma unroll
   for (int j = 0; j < R; ++j) z[padi(base + (j << lgq))] = a[j];

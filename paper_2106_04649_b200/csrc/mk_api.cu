@@ -64,16 +64,52 @@ int resolve_regime(mk_ctx* c, int nfoc, int* regime) {
   int r = c->regime;
   if (r == 0) r = gemv_supported(c, nfoc) ? 1 : 2;
   if (r == 1 && !gemv_supported(c, nfoc)) return set_err(c, MK_ERR_INVALID_ARG, "GEMV regime needs nfoc <= 8 and ld*nfoc*8 <= 96 KiB");
-  if (r == 3) return set_err(c, MK_ERR_INVALID_ARG, "tcgen05 3xTF32 regime is not built in this version");
   if (r < 1 || r > 3) return set_err(c, MK_ERR_INVALID_ARG, "unknown regime");
+  if (r == 3 && !tc_supported(c)) return set_err(c, MK_ERR_INVALID_ARG, "tcgen05 3xTF32 regime needs an sm_100 device");
   *regime = r;
   return MK_OK;
 }
 
 inline int ldf_for(int regime, int nfoc) { return regime == 1 ? nfoc : ((nfoc + 3) / 4) * 4; }
 
+inline int ldb_for(int nfoc) { return ((2 * nfoc + 31) / 32) * 32; }
+
+// the operand of slot 0 (the run) or 1 (scratch: mk_synthesis, finals) in the layout of `regime`
+OperandOut operand_out(mk_ctx* c, int slot, int regime, int ldf, int ldb) {
+  OperandOut O{};
+  O.ldf = ldf;
+  O.ldb = ldb;
+  if (regime == 3) {
+    O.bhi = slot ? c->d_Bhi2 : c->d_Bhi;
+    O.blo = slot ? c->d_Blo2 : c->d_Blo;
+  } else {
+    O.plain = slot ? c->d_Nhat2 : c->d_Nhat;
+  }
+  return O;
+}
+
+// allocate + zero the operand of a slot (pad rows / columns must be zero; the layout may differ from the last use)
+int prepare_operand(mk_ctx* c, int slot, int regime, int nfoc, int ldf, int ldb) {
+  if (regime == 3) {
+    const size_t cnt = (size_t)c->nb * 2 * c->ld * ldb;
+    float** hi = slot ? &c->d_Bhi2 : &c->d_Bhi;
+    float** lo = slot ? &c->d_Blo2 : &c->d_Blo;
+    size_t* cap = slot ? &c->cap_B2 : &c->cap_B;
+    size_t cap2 = *cap;
+    if (int rc = ensure(c, hi, cap, cnt, "B' hi plane")) return rc;
+    if (int rc = ensure(c, lo, &cap2, cnt, "B' lo plane")) return rc;
+    if (int rc = check_cuda(c, cudaMemsetAsync(*hi, 0, cnt * sizeof(float), c->stream), "memset B' hi")) return rc;
+    return check_cuda(c, cudaMemsetAsync(*lo, 0, cnt * sizeof(float), c->stream), "memset B' lo");
+  }
+  const size_t nN = (size_t)c->nb * c->ld * ldf;
+  float2** p = slot ? &c->d_Nhat2 : &c->d_Nhat;
+  size_t* cap = slot ? &c->cap_Nhat2 : &c->cap_Nhat;
+  if (int rc = ensure(c, p, cap, nN, "Nhat")) return rc;
+  return check_cuda(c, cudaMemsetAsync(*p, 0, nN * sizeof(float2), c->stream), "memset Nhat");
+}
+
 // a2: S^ = R^ x N^ per bin, on the context's stream; optionally bracketed by events
-int contract(mk_ctx* c, const float2* Nhat, float2* Shat, int nfoc, int ldf, int regime) {
+int contract(mk_ctx* c, int slot, float2* Shat, int nfoc, int ldf, int ldb, int regime) {
   cudaEvent_t e0 = nullptr, e1 = nullptr;
   bool timed = c->timing != 0;
   if (timed && c->ev_used + 2 > c->ev.size()) {
@@ -91,7 +127,10 @@ int contract(mk_ctx* c, const float2* Nhat, float2* Shat, int nfoc, int ldf, int
     c->ev_used += 2;
     cudaEventRecord(e0, c->stream);
   }
-  int rc = regime == 1 ? launch_syn_gemv(c, Nhat, Shat, nfoc) : launch_syn_gemm(c, Nhat, Shat, ldf);
+  int rc;
+  if (regime == 1) rc = launch_syn_gemv(c, slot ? c->d_Nhat2 : c->d_Nhat, Shat, nfoc);
+  else if (regime == 2) rc = launch_syn_gemm(c, slot ? c->d_Nhat2 : c->d_Nhat, Shat, ldf);
+  else rc = launch_syn_tc(c, slot, slot ? c->d_Bhi2 : c->d_Bhi, slot ? c->d_Blo2 : c->d_Blo, Shat, nfoc, ldf, ldb);
   if (timed) cudaEventRecord(e1, c->stream);
   c->regime_used = regime;
   return rc;
@@ -208,6 +247,10 @@ int mk_destroy(mk_ctx* c) {
   cudaFree(c->d_h);
   cudaFree(c->d_Nhat2);
   cudaFree(c->d_Shat2);
+  cudaFree(c->d_Bhi);
+  cudaFree(c->d_Blo);
+  cudaFree(c->d_Bhi2);
+  cudaFree(c->d_Blo2);
   cudaFree(c->d_stage);
   for (cudaEvent_t e : c->ev) cudaEventDestroy(e);
   cudaGetLastError();
@@ -231,7 +274,7 @@ int mk_set_option(mk_ctx* c, int key, double value) {
       return MK_OK;
     case MK_OPT_REGIME:
       if (value < 0 || value > 3 || value != std::floor(value)) return set_err(c, MK_ERR_INVALID_ARG, "regime must be 0..3");
-      if ((int)value == 3) return set_err(c, MK_ERR_INVALID_ARG, "tcgen05 3xTF32 regime is not built in this version");
+      if ((int)value == 3 && !tc_supported(c)) return set_err(c, MK_ERR_INVALID_ARG, "tcgen05 3xTF32 regime needs an sm_100 device");
       c->regime = (int)value;
       return MK_OK;
     case MK_OPT_TIMING:
@@ -309,31 +352,31 @@ int mk_begin(mk_ctx* c, const float* d_Gd, const float* d_td, int nfoc) {
   if (c->shots_loaded != c->n) return set_err(c, MK_ERR_STATE, "mk_begin before every shot of R was loaded");
   int regime = 0;
   if (int rc = resolve_regime(c, nfoc, &regime)) return rc;
-  const int ldf = ldf_for(regime, nfoc);
+  const int ldf = ldf_for(regime, nfoc), ldb = ldb_for(nfoc);
   const size_t ntime = (size_t)nfoc * c->n * c->nt;
-  const size_t nN = (size_t)c->nb * c->ld * ldf, nS = (size_t)c->n * c->nb * ldf;
+  const size_t nS = (size_t)c->n * c->nb * ldf;
   c->begun = false;
   {
     size_t cap2 = c->cap_time;
     if (int rc = ensure(c, &c->d_f1plus, &c->cap_time, ntime, "f1plus")) return rc;
     if (int rc = ensure(c, &c->d_f1min, &cap2, ntime, "f1min")) return rc;
     size_t capS = c->cap_Shat;
-    if (int rc = ensure(c, &c->d_Nhat, &c->cap_Nhat, nN, "Nhat")) return rc;
     if (int rc = ensure(c, &c->d_Shat, &c->cap_Shat, nS, "Shat")) return rc;
     if (int rc = ensure(c, &c->d_phat, &capS, nS, "phat")) return rc;
     if (int rc = ensure(c, &c->d_h, &c->cap_h, (size_t)nfoc * c->n, "window table")) return rc;
   }
   c->nfoc = nfoc;
   c->ldf = ldf;
+  c->ldb = ldb;
   c->regime_used = regime;
   c->iter = 0;
   c->have_Gminus = false;
-  if (int rc = check_cuda(c, cudaMemsetAsync(c->d_Nhat, 0, nN * sizeof(float2), c->stream), "memset Nhat")) return rc;
+  if (int rc = prepare_operand(c, 0, regime, nfoc, ldf, ldb)) return rc;
   if (int rc = check_cuda(c, cudaMemsetAsync(c->d_phat, 0, nS * sizeof(float2), c->stream), "memset phat")) return rc;
   if (int rc = check_cuda(c, cudaMemsetAsync(c->d_f1min, 0, ntime * sizeof(float), c->stream), "memset f1min")) return rc;
   if (int rc = launch_window(c, d_td, c->d_h, nfoc * c->n)) return rc;
   // a1: N_{-1} = f1plus = T G_d; N^_{-1} = conj(G_d^)     [PAPER.md:19, 67, 74-75]
-  if (int rc = launch_fwd(c, d_Gd, c->d_Nhat, nfoc, ldf, /*conj_out=*/true, c->d_f1plus)) return rc;
+  if (int rc = launch_fwd(c, d_Gd, operand_out(c, 0, regime, ldf, ldb), nfoc, /*conj_out=*/true, c->d_f1plus)) return rc;
   c->begun = true;
   return MK_OK;
 }
@@ -342,18 +385,16 @@ int mk_step(mk_ctx* c, float* d_N_i) {
   MK_GUARD(c);
   if (!c->begun) return set_err(c, MK_ERR_STATE, "mk_step before mk_begin");
   int regime = c->regime_used;
-  if (int rc = contract(c, c->d_Nhat, c->d_Shat, c->nfoc, c->ldf, regime)) return rc;      // a2  [PAPER.md:69]
-  if (int rc = launch_post(c, (c->iter % 2) == 0, d_N_i)) return rc;                       // a3..a6
+  if (int rc = contract(c, 0, c->d_Shat, c->nfoc, c->ldf, c->ldb, regime)) return rc;                               // a2  [PAPER.md:69]
+  if (int rc = launch_post(c, operand_out(c, 0, regime, c->ldf, c->ldb), (c->iter % 2) == 0, d_N_i)) return rc;     // a3..a6
   ++c->iter;
   return MK_OK;
 }
 
-static int scratch_operands(mk_ctx* c, int nfoc, int ldf) {
-  const size_t nN = (size_t)c->nb * c->ld * ldf, nS = (size_t)c->n * c->nb * ldf;
-  if (int rc = ensure(c, &c->d_Nhat2, &c->cap_Nhat2, nN, "Nhat scratch")) return rc;
+static int scratch_operands(mk_ctx* c, int regime, int nfoc, int ldf, int ldb) {
+  const size_t nS = (size_t)c->n * c->nb * ldf;
   if (int rc = ensure(c, &c->d_Shat2, &c->cap_Shat2, nS, "Shat scratch")) return rc;
-  // pad rows / columns of the operand must be zero; the layout may differ from the previous use
-  return check_cuda(c, cudaMemsetAsync(c->d_Nhat2, 0, nN * sizeof(float2), c->stream), "memset Nhat scratch");
+  return prepare_operand(c, 1, regime, nfoc, ldf, ldb);
 }
 
 int mk_finish(mk_ctx* c, const mk_outputs* o) {
@@ -368,15 +409,15 @@ int mk_finish(mk_ctx* c, const mk_outputs* o) {
   if (o->f1min)
     if (int rc = check_cuda(c, cudaMemcpyAsync(o->f1min, c->d_f1min, bytes, cudaMemcpyDeviceToDevice, c->stream), "copy f1min")) return rc;
   if (o->Gminus) {  // G^- = R f1plus - f1min   [PAPER.md:87-88; G5]
-    if (int rc = scratch_operands(c, c->nfoc, c->ldf)) return rc;
-    if (int rc = launch_fwd(c, c->d_f1plus, c->d_Nhat2, c->nfoc, c->ldf, false, nullptr)) return rc;
-    if (int rc = contract(c, c->d_Nhat2, c->d_Shat2, c->nfoc, c->ldf, regime)) return rc;
+    if (int rc = scratch_operands(c, regime, c->nfoc, c->ldf, c->ldb)) return rc;
+    if (int rc = launch_fwd(c, c->d_f1plus, operand_out(c, 1, regime, c->ldf, c->ldb), c->nfoc, false, nullptr)) return rc;
+    if (int rc = contract(c, 1, c->d_Shat2, c->nfoc, c->ldf, c->ldb, regime)) return rc;
     if (int rc = launch_inv(c, c->d_Shat2, c->nfoc, c->ldf, o->Gminus, 1.f, c->d_f1min, -1.f, nullptr, 0.f)) return rc;
   }
   if (o->Gplus) {  // G^+ = T f1plus - R (T f1min)   [PAPER.md:24; G4]
-    if (int rc = scratch_operands(c, c->nfoc, c->ldf)) return rc;
-    if (int rc = launch_fwd(c, c->d_f1min, c->d_Nhat2, c->nfoc, c->ldf, true, nullptr)) return rc;
-    if (int rc = contract(c, c->d_Nhat2, c->d_Shat2, c->nfoc, c->ldf, regime)) return rc;
+    if (int rc = scratch_operands(c, regime, c->nfoc, c->ldf, c->ldb)) return rc;
+    if (int rc = launch_fwd(c, c->d_f1min, operand_out(c, 1, regime, c->ldf, c->ldb), c->nfoc, true, nullptr)) return rc;
+    if (int rc = contract(c, 1, c->d_Shat2, c->nfoc, c->ldf, c->ldb, regime)) return rc;
     if (int rc = launch_inv(c, c->d_Shat2, c->nfoc, c->ldf, o->Gplus, -1.f, nullptr, 0.f, c->d_f1plus, 1.f)) return rc;
   }
   if (o->G) {  // G = p^- + T f2 = p^- + T f1plus - f1min   [PAPER.md:24; G3]
@@ -438,10 +479,10 @@ int mk_synthesis(mk_ctx* c, const float* d_N_in, float* d_S_out, int nfoc) {
   if (c->shots_loaded != c->n) return set_err(c, MK_ERR_STATE, "mk_synthesis before every shot of R was loaded");
   int regime = 0;
   if (int rc = resolve_regime(c, nfoc, &regime)) return rc;
-  const int ldf = ldf_for(regime, nfoc);
-  if (int rc = scratch_operands(c, nfoc, ldf)) return rc;
-  if (int rc = launch_fwd(c, d_N_in, c->d_Nhat2, nfoc, ldf, false, nullptr)) return rc;      // a6
-  if (int rc = contract(c, c->d_Nhat2, c->d_Shat2, nfoc, ldf, regime)) return rc;            // a2
+  const int ldf = ldf_for(regime, nfoc), ldb = ldb_for(nfoc);
+  if (int rc = scratch_operands(c, regime, nfoc, ldf, ldb)) return rc;
+  if (int rc = launch_fwd(c, d_N_in, operand_out(c, 1, regime, ldf, ldb), nfoc, false, nullptr)) return rc;   // a6
+  if (int rc = contract(c, 1, c->d_Shat2, nfoc, ldf, ldb, regime)) return rc;                                 // a2
   return launch_inv(c, c->d_Shat2, nfoc, ldf, d_S_out, 1.f, nullptr, 0.f, nullptr, 0.f);     // a3
 }
 

@@ -5,8 +5,13 @@
 //   k_inv      spectrum -> time field with a linear epilogue (finals, bare synthesis)          (a3, a7)
 //   k_post     p^ += S^; inverse rFFT; N_i = -Theta T S; f1min / f1plus accumulation; rFFT -> N^_i   (a3..a6 fused:
 //              one pass over N per iteration, BASELINE.json north_star (c))
-// One CTA owns one receiver r and FT consecutive focal points, so both the S^[r][k][f..] reads and the
-// N^[k][r][f..] writes are contiguous 8*FT-byte segments.  Traces live in padded shared memory (fft_core.cuh).
+//
+// Work decomposition.  One CTA (256 threads) owns one receiver r and FT consecutive focal points (FT a power of two
+// <= 8), so the S^[r][k][f..] reads and the N^[k][r][f..] writes are contiguous 8*FT-byte segments.  The traces live
+// in padded shared memory (fft_core.cuh).  Inside the CTA every trace belongs to a GROUP of 256/FT threads (one warp
+// when FT = 8): the FFT passes, the window and the accumulation of a trace synchronise only inside its group
+// (__syncwarp / a named barrier), so the groups drift apart and hide each other's latency; the CTA synchronises only
+// around the two phases whose thread mapping crosses traces (spectrum load, spectrum store).
 #include "mk_internal.cuh"
 
 namespace mk {
@@ -17,75 +22,182 @@ namespace {
 
 constexpr int kThreads = 256;
 
-__device__ __forceinline__ void fft_batch_fwd(float2* z, int ntr, int MP, const Plan& p, const float2* __restrict__ tw) {
+struct Group {
+  int tl;     // trace (local focal index) this thread works on
+  int lane;   // index inside the group
+  int size;   // threads per group = kThreads / FT
+};
+
+__device__ __forceinline__ Group my_group(int lgFT) {
+  Group g;
+  g.size = kThreads >> lgFT;
+  g.tl = threadIdx.x / g.size;
+  g.lane = threadIdx.x - g.tl * g.size;
+  return g;
+}
+
+__device__ __forceinline__ void group_sync(const Group& g) {
+  if (g.size == 32) __syncwarp();
+  else if (g.size == kThreads) __syncthreads();
+  else {  // FT = 2 or 4: named barriers 1..4 (immediate ids, so that only these are reserved)
+    switch (g.tl) {
+      case 0: asm volatile("bar.sync 1, %0;" ::"r"(g.size) : "memory"); break;
+      case 1: asm volatile("bar.sync 2, %0;" ::"r"(g.size) : "memory"); break;
+      case 2: asm volatile("bar.sync 3, %0;" ::"r"(g.size) : "memory"); break;
+      default: asm volatile("bar.sync 4, %0;" ::"r"(g.size) : "memory"); break;
+    }
+  }
+}
+
+// forward passes of ONE trace by its group (decimation in frequency; leaves Z digit-reversed)
+__device__ __forceinline__ void fft_fwd(float2* z, const Plan& p, const float2* __restrict__ tw, const Group& g) {
   for (int ps = 0; ps < p.npass; ++ps) {
-    const int lgr = p.lgr[ps], lgL = p.lgL[ps], lgB = p.logM - lgr;
-    const int total = ntr << lgB, mask = (1 << lgB) - 1;
+    const int lgr = p.lgr[ps], lgL = p.lgL[ps], nb = p.M >> lgr;
     if (lgr == 3) {
-      for (int b = threadIdx.x; b < total; b += blockDim.x) mkfft::fwd_butterfly<3>(z + (b >> lgB) * MP, tw, p.nt, lgL, b & mask);
+      for (int b = g.lane; b < nb; b += g.size) mkfft::fwd_butterfly<3>(z, tw, p.nt, lgL, b);
     } else if (lgr == 2) {
-      for (int b = threadIdx.x; b < total; b += blockDim.x) mkfft::fwd_butterfly<2>(z + (b >> lgB) * MP, tw, p.nt, lgL, b & mask);
+      for (int b = g.lane; b < nb; b += g.size) mkfft::fwd_butterfly<2>(z, tw, p.nt, lgL, b);
     } else {
-      for (int b = threadIdx.x; b < total; b += blockDim.x) mkfft::fwd_butterfly<1>(z + (b >> lgB) * MP, tw, p.nt, lgL, b & mask);
+      for (int b = g.lane; b < nb; b += g.size) mkfft::fwd_butterfly<1>(z, tw, p.nt, lgL, b);
     }
-    __syncthreads();
+    group_sync(g);
   }
 }
 
-__device__ __forceinline__ void fft_batch_inv(float2* z, int ntr, int MP, const Plan& p, const float2* __restrict__ tw) {
+__device__ __forceinline__ void fft_inv(float2* z, const Plan& p, const float2* __restrict__ tw, const Group& g) {
   for (int ps = p.npass - 1; ps >= 0; --ps) {
-    const int lgr = p.lgr[ps], lgL = p.lgL[ps], lgB = p.logM - lgr;
-    const int total = ntr << lgB, mask = (1 << lgB) - 1;
+    const int lgr = p.lgr[ps], lgL = p.lgL[ps], nb = p.M >> lgr;
     if (lgr == 3) {
-      for (int b = threadIdx.x; b < total; b += blockDim.x) mkfft::inv_butterfly<3>(z + (b >> lgB) * MP, tw, p.nt, lgL, b & mask);
+      for (int b = g.lane; b < nb; b += g.size) mkfft::inv_butterfly<3>(z, tw, p.nt, lgL, b);
     } else if (lgr == 2) {
-      for (int b = threadIdx.x; b < total; b += blockDim.x) mkfft::inv_butterfly<2>(z + (b >> lgB) * MP, tw, p.nt, lgL, b & mask);
+      for (int b = g.lane; b < nb; b += g.size) mkfft::inv_butterfly<2>(z, tw, p.nt, lgL, b);
     } else {
-      for (int b = threadIdx.x; b < total; b += blockDim.x) mkfft::inv_butterfly<1>(z + (b >> lgB) * MP, tw, p.nt, lgL, b & mask);
+      for (int b = g.lane; b < nb; b += g.size) mkfft::inv_butterfly<1>(z, tw, p.nt, lgL, b);
     }
-    __syncthreads();
+    group_sync(g);
   }
 }
 
-// copy `ntr` contiguous-time traces into the padded buffers; src_of(tl) = pointer to trace tl
-template <typename SrcOf>
-__device__ __forceinline__ void load_traces(float2* z, int ntr, int MP, int nt, SrcOf src_of) {
-  const int q = nt >> 2;  // float4 per trace
-  for (int idx = threadIdx.x; idx < ntr * q; idx += blockDim.x) {
-    const int tl = idx / q, j4 = idx - tl * q;
-    const float4 v = __ldg(reinterpret_cast<const float4*>(src_of(tl)) + j4);
-    float2* zt = z + tl * MP;
-    zt[mkfft::padi(2 * j4)] = make_float2(v.x, v.y);
-    zt[mkfft::padi(2 * j4 + 1)] = make_float2(v.z, v.w);
+// the group's trace: contiguous-time fp32 source -> padded buffer (float4 loads, 4 in flight per thread)
+__device__ __forceinline__ void load_trace(float2* z, const float* __restrict__ src, int nt, const Group& g) {
+  const float4* s4 = reinterpret_cast<const float4*>(src);
+  const int q = nt >> 2;
+  for (int j0 = g.lane; j0 < q; j0 += 4 * g.size) {
+    float4 v[4];
+#pragma unroll
+    for (int u = 0; u < 4; ++u) {
+      const int j4 = j0 + u * g.size;
+      if (j4 < q) v[u] = __ldg(s4 + j4);
+    }
+#pragma unroll
+    for (int u = 0; u < 4; ++u) {
+      const int j4 = j0 + u * g.size;
+      if (j4 < q) {
+        z[mkfft::padi(2 * j4)] = make_float2(v[u].x, v[u].y);
+        z[mkfft::padi(2 * j4 + 1)] = make_float2(v[u].z, v[u].w);
+      }
+    }
   }
 }
 
-// Build Z (digit-reversed, scaled) of `ntr` traces from a band-limited half spectrum.  spec_of(tl, kk) returns
-// X[klo + kk] of trace tl (with every side effect the caller wants, e.g. the p^ accumulation).
-template <bool CONJ, typename SpecOf>
-__device__ __forceinline__ void spectrum_to_Z(float2* z, int ntr, int ft, int MP, const Plan& p, const float2* __restrict__ tw,
-                                              int klo, int nb, SpecOf spec_of) {
-  const int M = p.M, half = M >> 1;
+__device__ __forceinline__ float4 read4(const float2* z, int j4) {  // samples 4 j4 .. 4 j4 + 3 of the padded trace
+  const float2 a = z[mkfft::padi(2 * j4)], b = z[mkfft::padi(2 * j4 + 1)];
+  return make_float4(a.x, a.y, b.x, b.y);
+}
+__device__ __forceinline__ void write4(float2* z, int j4, float4 v) {
+  z[mkfft::padi(2 * j4)] = make_float2(v.x, v.y);
+  z[mkfft::padi(2 * j4 + 1)] = make_float2(v.z, v.w);
+}
+// time-reversed samples: (T u)[4 j4 + e] = u[(nt - 4 j4 - e) % nt], e = 0..3
+__device__ __forceinline__ float4 read4_reversed(const float2* z, int j4, int nt) {
+  const float* zf = reinterpret_cast<const float*>(z);
+  const int j = 4 * j4;
+  return make_float4(zf[mkfft::padj((nt - j) & (nt - 1))], zf[mkfft::padj(nt - j - 1)], zf[mkfft::padj(nt - j - 2)],
+                     zf[mkfft::padj(nt - j - 3)]);
+}
+
+// Z (digit-reversed, scaled) of all FT traces from their band-limited half spectra.  CTA-wide: consecutive threads
+// take consecutive focal points of one bin.  load(tl, kk, aux) returns X[klo + kk] of trace tl (and may fetch a side
+// value into aux); commit(tl, kk, X, aux) runs afterwards.  Both are called exactly once per in-band (k, tl); the
+// loads of four items are issued before anything is consumed.
+template <bool CONJ, typename Load, typename Commit>
+__device__ __forceinline__ void spectrum_to_Z(float2* smem, int nf, int lgFT, int MP, const Plan& p,
+                                              const float2* __restrict__ tw, int klo, int nb, Load load, Commit commit) {
+  const int M = p.M, half = M >> 1, FT = 1 << lgFT;
   const float scale = 1.0f / (2.0f * (float)M);
-  for (int idx = threadIdx.x; idx < (half + 1) * ft; idx += blockDim.x) {
-    const int k = idx / ft, tl = idx - k * ft;
-    if (tl >= ntr) continue;
-    const int k2 = M - k;
-    float2 a = make_float2(0.f, 0.f), b = make_float2(0.f, 0.f);
-    if (k >= klo && k < klo + nb) a = spec_of(tl, k - klo);
-    if (k2 != k && k2 >= klo && k2 < klo + nb) b = spec_of(tl, k2 - klo);
-    if (k2 == k) b = a;
-    if (k == 0) {  // DC and Nyquist are real for a real trace (irfft convention)
-      a.y = 0.f;
-      b.y = 0.f;
+  const int total = (half + 1) << lgFT;
+  for (int i0 = threadIdx.x; i0 < total; i0 += 4 * kThreads) {
+    float2 a[4], b[4], xa[4], xb[4];
+#pragma unroll
+    for (int u = 0; u < 4; ++u) {
+      const int idx = i0 + u * kThreads;
+      a[u] = b[u] = xa[u] = xb[u] = make_float2(0.f, 0.f);
+      if (idx < total) {
+        const int k = idx >> lgFT, tl = idx & (FT - 1), k2 = M - k;
+        if (tl < nf) {
+          if (k >= klo && k < klo + nb) a[u] = load(tl, k - klo, xa[u]);
+          if (k2 != k && k2 >= klo && k2 < klo + nb) b[u] = load(tl, k2 - klo, xb[u]);
+        }
+      }
     }
-    if (CONJ) {
-      a.y = -a.y;
-      b.y = -b.y;
+#pragma unroll
+    for (int u = 0; u < 4; ++u) {
+      const int idx = i0 + u * kThreads;
+      if (idx >= total) continue;
+      const int k = idx >> lgFT, tl = idx & (FT - 1), k2 = M - k;
+      if (tl >= nf) continue;
+      if (k >= klo && k < klo + nb) commit(tl, k - klo, a[u], xa[u]);
+      if (k2 != k && k2 >= klo && k2 < klo + nb) commit(tl, k2 - klo, b[u], xb[u]);
+      float2 x = a[u], y = b[u];
+      if (k2 == k) y = x;
+      if (k == 0) {  // DC and Nyquist are real for a real trace (irfft convention)
+        x.y = 0.f;
+        y.y = 0.f;
+      }
+      if (CONJ) {
+        x.y = -x.y;
+        y.y = -y.y;
+      }
+      float2* zt = smem + tl * MP;
+      zt[mkfft::padi(mkfft::freq_pos(p, k))] = mkfft::irfft_pre(x, y, tw[k], scale);
+      if (k2 < M && k2 != k) zt[mkfft::padi(mkfft::freq_pos(p, k2))] = mkfft::irfft_pre(y, x, tw[k2], scale);
     }
-    float2* zt = z + tl * MP;
-    zt[mkfft::padi(mkfft::freq_pos(p, k))] = mkfft::irfft_pre(a, b, tw[k], scale);
-    if (k2 < M && k2 != k) zt[mkfft::padi(mkfft::freq_pos(p, k2))] = mkfft::irfft_pre(b, a, tw[k2], scale);
+  }
+}
+
+__device__ __forceinline__ float tf32_rna(float v) {
+  unsigned u;
+  asm("cvt.rna.tf32.f32 %0, %1;" : "=r"(u) : "f"(v));
+  return __uint_as_float(u);
+}
+
+// a6 store: X = N^[k][r][f] in the layout the contraction of the active regime reads
+__device__ __forceinline__ void store_operand(const OperandOut& O, int ld, int kk, int r, int f, float2 X) {
+  if (O.bhi == nullptr) {
+    O.plain[((size_t)kk * ld + r) * O.ldf + f] = X;
+    return;
+  }
+  // regime 3 (mk_syn_tc.cu): real operand B' [nb][2 ld][ldb], rows (2r, 2r+1) = (X, iX) as interleaved floats,
+  // split into a tf32 "hi" plane and a tf32 "lo" plane (3xTF32).
+  const float hx = tf32_rna(X.x), hy = tf32_rna(X.y);
+  const float lx = tf32_rna(X.x - hx), ly = tf32_rna(X.y - hy);
+  const size_t row0 = ((size_t)kk * 2 * ld + 2 * r) * O.ldb + 2 * f;
+  *reinterpret_cast<float2*>(O.bhi + row0) = make_float2(hx, hy);
+  *reinterpret_cast<float2*>(O.bhi + row0 + O.ldb) = make_float2(-hy, hx);
+  *reinterpret_cast<float2*>(O.blo + row0) = make_float2(lx, ly);
+  *reinterpret_cast<float2*>(O.blo + row0 + O.ldb) = make_float2(-ly, lx);
+}
+
+// band of the half spectra of all FT traces (held digit-reversed in smem) -> operand; CTA-wide mapping
+__device__ __forceinline__ void Z_to_operand(const float2* smem, int nf, int lgFT, int MP, const FftParams& P, int r, int f0,
+                                             bool conj_out, const OperandOut& O) {
+  const int FT = 1 << lgFT, total = P.nb << lgFT;
+  for (int idx = threadIdx.x; idx < total; idx += kThreads) {
+    const int kk = idx >> lgFT, tl = idx & (FT - 1);
+    if (tl >= nf) continue;
+    float2 X = mkfft::rfft_bin(smem + tl * MP, P.plan, P.tw, P.klo + kk);
+    if (conj_out) X.y = -X.y;  // spectrum of the time-reversed real trace
+    store_operand(O, P.ld, kk, r, f0 + tl, X);
   }
 }
 
@@ -103,17 +215,23 @@ __global__ void k_window(const float* __restrict__ td, int* __restrict__ h, int 
 // ------------------------------------------------------------------------------------------------ k_load_R
 // grid (ceil(nshots/ST), nrec); Rt: [nshots][nrec][nt]
 __global__ void __launch_bounds__(kThreads) k_load_R(const float* __restrict__ Rt, float2* __restrict__ Rhat, FftParams P,
-                                                     int shot0, int nshots, int ST, float scale_mid, float scale_end) {
+                                                     int shot0, int nshots, int lgST, float scale_mid, float scale_end) {
   extern __shared__ float2 smem[];
-  const int MP = mkfft::padded_len(P.plan.M);
+  const int MP = mkfft::padded_len(P.plan.M), ST = 1 << lgST;
   const int r = blockIdx.y, g0 = blockIdx.x * ST;
   const int ns = min(ST, nshots - g0);
+  const Group g = my_group(lgST);
   const size_t nt = P.plan.nt;
-  load_traces(smem, ns, MP, P.plan.nt, [&](int tl) { return Rt + ((size_t)(g0 + tl) * P.n + r) * nt; });
+  if (g.tl < ns) {
+    float2* z = smem + g.tl * MP;
+    load_trace(z, Rt + ((size_t)(g0 + g.tl) * P.n + r) * nt, P.plan.nt, g);
+    group_sync(g);
+    fft_fwd(z, P.plan, P.tw, g);
+  }
   __syncthreads();
-  fft_batch_fwd(smem, ns, MP, P.plan, P.tw);
-  for (int idx = threadIdx.x; idx < P.nb * ST; idx += blockDim.x) {
-    const int kk = idx / ST, tl = idx - kk * ST;
+  const int total = P.nb << lgST;
+  for (int idx = threadIdx.x; idx < total; idx += kThreads) {
+    const int kk = idx >> lgST, tl = idx & (ST - 1);
     if (tl >= ns) continue;
     const int s = shot0 + g0 + tl;
     const float sc = (P.n > 1 && (s == 0 || s == P.n - 1)) ? scale_end : scale_mid;
@@ -124,121 +242,146 @@ __global__ void __launch_bounds__(kThreads) k_load_R(const float* __restrict__ R
 
 // ------------------------------------------------------------------------------------------------ k_fwd
 // grid (ceil(nfoc/FT), n); src: [nfoc][n][nt]
-__global__ void __launch_bounds__(kThreads) k_fwd(const float* __restrict__ src, float2* __restrict__ Nhat, FftParams P, int FT,
+__global__ void __launch_bounds__(kThreads) k_fwd(const float* __restrict__ src, OperandOut O, FftParams P, int lgFT,
                                                   int conj_out, float* __restrict__ init_Tsrc) {
   extern __shared__ float2 smem[];
-  const int MP = mkfft::padded_len(P.plan.M);
+  const int MP = mkfft::padded_len(P.plan.M), FT = 1 << lgFT;
   const int r = blockIdx.y, f0 = blockIdx.x * FT;
   const int nf = min(FT, P.nfoc - f0);
   const int nt = P.plan.nt;
-  load_traces(smem, nf, MP, nt, [&](int tl) { return src + ((size_t)(f0 + tl) * P.n + r) * nt; });
-  __syncthreads();
-  if (init_Tsrc) {  // f1plus = N_{-1} = T G_d   [PAPER.md:19, 67, 74]
-    const float* zf = reinterpret_cast<const float*>(smem);
-    for (int idx = threadIdx.x; idx < nf * nt; idx += blockDim.x) {
-      const int tl = idx / nt, j = idx - tl * nt;
-      init_Tsrc[((size_t)(f0 + tl) * P.n + r) * nt + j] = zf[2 * tl * MP + mkfft::padj((nt - j) & (nt - 1))];
+  const Group g = my_group(lgFT);
+  if (g.tl < nf) {
+    float2* z = smem + g.tl * MP;
+    const size_t base = ((size_t)(f0 + g.tl) * P.n + r) * nt;
+    load_trace(z, src + base, nt, g);
+    group_sync(g);
+    if (init_Tsrc) {  // f1plus = N_{-1} = T G_d   [PAPER.md:19, 67, 74]
+      float4* dst = reinterpret_cast<float4*>(init_Tsrc + base);
+      for (int j4 = g.lane; j4 < (nt >> 2); j4 += g.size) dst[j4] = read4_reversed(z, j4, nt);
+      group_sync(g);  // the in-place FFT below overwrites what this loop reads
     }
-    __syncthreads();  // the in-place FFT below overwrites what this loop reads
+    fft_fwd(z, P.plan, P.tw, g);
   }
-  fft_batch_fwd(smem, nf, MP, P.plan, P.tw);
-  for (int idx = threadIdx.x; idx < P.nb * FT; idx += blockDim.x) {
-    const int kk = idx / FT, tl = idx - kk * FT;
-    if (tl >= nf) continue;
-    float2 X = mkfft::rfft_bin(smem + tl * MP, P.plan, P.tw, P.klo + kk);
-    if (conj_out) X.y = -X.y;  // spectrum of the time-reversed real trace
-    Nhat[((size_t)kk * P.ld + r) * P.ldf + f0 + tl] = X;
-  }
+  __syncthreads();
+  Z_to_operand(smem, nf, lgFT, MP, P, r, f0, conj_out != 0, O);
 }
 
 // ------------------------------------------------------------------------------------------------ k_inv
 // grid (ceil(nfoc/FT), n); spec: [n][nb][ldf]; out[j] = sS*S[j] + sA*A[j] + sB*B[(nt-j)%nt]
-__global__ void __launch_bounds__(kThreads) k_inv(const float2* __restrict__ spec, FftParams P, int FT, float* __restrict__ out,
+__global__ void __launch_bounds__(kThreads) k_inv(const float2* __restrict__ spec, FftParams P, int lgFT, float* __restrict__ out,
                                                   float sS, const float* __restrict__ A, float sA,
                                                   const float* __restrict__ B, float sB) {
   extern __shared__ float2 smem[];
-  const int MP = mkfft::padded_len(P.plan.M);
+  const int MP = mkfft::padded_len(P.plan.M), FT = 1 << lgFT;
   const int r = blockIdx.y, f0 = blockIdx.x * FT;
   const int nf = min(FT, P.nfoc - f0);
   const int nt = P.plan.nt;
   const float2* srow = spec + (size_t)r * P.nb * P.ldf + f0;
-  spectrum_to_Z<false>(smem, nf, FT, MP, P.plan, P.tw, P.klo, P.nb,
-                       [&](int tl, int kk) { return __ldg(srow + (size_t)kk * P.ldf + tl); });
+  spectrum_to_Z<false>(smem, nf, lgFT, MP, P.plan, P.tw, P.klo, P.nb,
+                       [&](int tl, int kk, float2&) { return __ldg(srow + (size_t)kk * P.ldf + tl); },
+                       [](int, int, float2, float2) {});
   __syncthreads();
-  fft_batch_inv(smem, nf, MP, P.plan, P.tw);
-  const float* zf = reinterpret_cast<const float*>(smem);
-  for (int idx = threadIdx.x; idx < nf * nt; idx += blockDim.x) {
-    const int tl = idx / nt, j = idx - tl * nt;
-    const size_t base = ((size_t)(f0 + tl) * P.n + r) * nt;
-    float v = sS * zf[2 * tl * MP + mkfft::padj(j)];
-    if (A) v += sA * A[base + j];
-    if (B) v += sB * B[base + ((nt - j) & (nt - 1))];
-    out[base + j] = v;
+  const Group g = my_group(lgFT);
+  if (g.tl >= nf) return;
+  float2* z = smem + g.tl * MP;
+  fft_inv(z, P.plan, P.tw, g);
+  const size_t base = ((size_t)(f0 + g.tl) * P.n + r) * nt;
+  const float4* A4 = A ? reinterpret_cast<const float4*>(A + base) : nullptr;
+  float4* o4 = reinterpret_cast<float4*>(out + base);
+  for (int j4 = g.lane; j4 < (nt >> 2); j4 += g.size) {
+    float4 v = read4(z, j4);
+    v = make_float4(sS * v.x, sS * v.y, sS * v.z, sS * v.w);
+    if (A4) {
+      const float4 a = __ldg(A4 + j4);
+      v.x += sA * a.x;
+      v.y += sA * a.y;
+      v.z += sA * a.z;
+      v.w += sA * a.w;
+    }
+    if (B) {
+      const int j = 4 * j4;
+      v.x += sB * __ldg(B + base + ((nt - j) & (nt - 1)));
+      v.y += sB * __ldg(B + base + (nt - j - 1));
+      v.z += sB * __ldg(B + base + (nt - j - 2));
+      v.w += sB * __ldg(B + base + (nt - j - 3));
+    }
+    o4[j4] = v;
   }
 }
 
 // ------------------------------------------------------------------------------------------------ k_post
-// grid (ceil(nfoc/FT), n).  Shat, phat: [n][nb][ldf]; Nhat: [nb][ld][ldf]; h: [nfoc][n]; f1plus/f1min: [nfoc][n][nt]
-__global__ void __launch_bounds__(kThreads) k_post(const float2* __restrict__ Shat, float2* __restrict__ phat, float2* __restrict__ Nhat,
+// grid (ceil(nfoc/FT), n).  Shat, phat: [n][nb][ldf]; operand out: see store_operand; h: [nfoc][n];
+// f1plus / f1min: [nfoc][n][nt]
+__global__ void __launch_bounds__(kThreads) k_post(const float2* __restrict__ Shat, float2* __restrict__ phat, OperandOut O,
                                                    const int* __restrict__ h, float* __restrict__ f1plus, float* __restrict__ f1min,
-                                                   FftParams P, int FT, int parity_even, float* __restrict__ Ni_out) {
+                                                   FftParams P, int lgFT, int parity_even, float* __restrict__ Ni_out) {
   extern __shared__ float2 smem[];
-  const int MP = mkfft::padded_len(P.plan.M);
+  const int MP = mkfft::padded_len(P.plan.M), FT = 1 << lgFT;
   const int r = blockIdx.y, f0 = blockIdx.x * FT;
   const int nf = min(FT, P.nfoc - f0);
   const int nt = P.plan.nt;
   const size_t rowoff = (size_t)r * P.nb * P.ldf + f0;
   // a3: p^ += S^ ; Z of conj(S^) so that the inverse transform yields u = T S directly  [PAPER.md:79, 71]
-  spectrum_to_Z<true>(smem, nf, FT, MP, P.plan, P.tw, P.klo, P.nb, [&](int tl, int kk) {
-    const size_t o = rowoff + (size_t)kk * P.ldf + tl;
-    const float2 s = __ldg(Shat + o);
-    float2 pv = phat[o];
-    pv.x += s.x;
-    pv.y += s.y;
-    phat[o] = pv;
-    return s;
-  });
+  spectrum_to_Z<true>(
+      smem, nf, lgFT, MP, P.plan, P.tw, P.klo, P.nb,
+      [&](int tl, int kk, float2& pv) {
+        const size_t o = rowoff + (size_t)kk * P.ldf + tl;
+        pv = phat[o];
+        return __ldg(Shat + o);
+      },
+      [&](int tl, int kk, float2 s, float2 pv) { phat[rowoff + (size_t)kk * P.ldf + tl] = make_float2(pv.x + s.x, pv.y + s.y); });
   __syncthreads();
-  fft_batch_inv(smem, nf, MP, P.plan, P.tw);
-  float* zf = reinterpret_cast<float*>(smem);
-  // a5: N_i = -Theta u.  i even: f1min -= T N_i  <=>  f1min[j] += Theta[j] u[(nt-j)%nt];  i odd: f1plus += N_i
-  //     [PAPER.md:82-85].  Only samples inside the window are touched.
-  for (int idx = threadIdx.x; idx < nf * nt; idx += blockDim.x) {
-    const int tl = idx / nt, j = idx - tl * nt;
-    const int hh = h[(size_t)(f0 + tl) * P.n + r];
-    if (j < hh || j > nt - hh) {
-      const size_t o = ((size_t)(f0 + tl) * P.n + r) * nt + j;
-      if (parity_even) f1min[o] += zf[2 * tl * MP + mkfft::padj((nt - j) & (nt - 1))];
-      else f1plus[o] -= zf[2 * tl * MP + mkfft::padj(j)];
+  const Group g = my_group(lgFT);
+  if (g.tl < nf) {
+    float2* z = smem + g.tl * MP;
+    fft_inv(z, P.plan, P.tw, g);  // z = u = T S
+    const int hh = __ldg(h + (size_t)(f0 + g.tl) * P.n + r);
+    const size_t base = ((size_t)(f0 + g.tl) * P.n + r) * nt;
+    const int q = nt >> 2;
+    // a5: N_i = -Theta u.  i even: f1min -= T N_i  <=>  f1min[j] += Theta[j] u[(nt-j)%nt];  i odd: f1plus += N_i
+    //     [PAPER.md:82-85].  Theta[j] = 1 iff j < h or j > nt - h; only chunks that meet the window touch HBM.
+    float4* acc4 = reinterpret_cast<float4*>((parity_even ? f1min : f1plus) + base);
+    for (int j4 = g.lane; j4 < q; j4 += g.size) {
+      const int j = 4 * j4;
+      if (!(j < hh || j + 3 > nt - hh)) continue;
+      const float4 u = parity_even ? read4_reversed(z, j4, nt) : read4(z, j4);
+      float4 a = acc4[j4];
+      const float sg = parity_even ? 1.f : -1.f;
+      if (j < hh || j > nt - hh) a.x += sg * u.x;
+      if (j + 1 < hh || j + 1 > nt - hh) a.y += sg * u.y;
+      if (j + 2 < hh || j + 2 > nt - hh) a.z += sg * u.z;
+      if (j + 3 < hh || j + 3 > nt - hh) a.w += sg * u.w;
+      acc4[j4] = a;
     }
+    group_sync(g);
+    // a4: N_i in place (hard 0/1 window, strict inequality; G2)
+    float4* ni4 = Ni_out ? reinterpret_cast<float4*>(Ni_out + base) : nullptr;
+    for (int j4 = g.lane; j4 < q; j4 += g.size) {
+      const int j = 4 * j4;
+      float4 v = make_float4(0.f, 0.f, 0.f, 0.f);
+      if (j < hh || j + 3 > nt - hh) {
+        const float4 u = read4(z, j4);
+        v.x = (j < hh || j > nt - hh) ? -u.x : 0.f;
+        v.y = (j + 1 < hh || j + 1 > nt - hh) ? -u.y : 0.f;
+        v.z = (j + 2 < hh || j + 2 > nt - hh) ? -u.z : 0.f;
+        v.w = (j + 3 < hh || j + 3 > nt - hh) ? -u.w : 0.f;
+      }
+      write4(z, j4, v);
+      if (ni4) ni4[j4] = v;
+    }
+    group_sync(g);
+    fft_fwd(z, P.plan, P.tw, g);  // a6
   }
   __syncthreads();
-  // a4: N_i in place (hard 0/1 window, strict inequality; G2)
-  for (int idx = threadIdx.x; idx < nf * nt; idx += blockDim.x) {
-    const int tl = idx / nt, j = idx - tl * nt;
-    const int hh = h[(size_t)(f0 + tl) * P.n + r];
-    const int a = 2 * tl * MP + mkfft::padj(j);
-    const float v = (j < hh || j > nt - hh) ? -zf[a] : 0.f;
-    zf[a] = v;
-    if (Ni_out) Ni_out[((size_t)(f0 + tl) * P.n + r) * nt + j] = v;
-  }
-  __syncthreads();
-  // a6: N^_i band
-  fft_batch_fwd(smem, nf, MP, P.plan, P.tw);
-  for (int idx = threadIdx.x; idx < P.nb * FT; idx += blockDim.x) {
-    const int kk = idx / FT, tl = idx - kk * FT;
-    if (tl >= nf) continue;
-    Nhat[((size_t)kk * P.ld + r) * P.ldf + f0 + tl] = mkfft::rfft_bin(smem + tl * MP, P.plan, P.tw, P.klo + kk);
-  }
+  Z_to_operand(smem, nf, lgFT, MP, P, r, f0, false, O);
 }
 
-int pick_ft(const mk_ctx* c, int nfoc, int cap) {
+int pick_lgft(const mk_ctx* c, int count) {
   const size_t per = (size_t)mkfft::padded_len(c->plan.M) * sizeof(float2);
-  int ft = (int)(72000 / per);
-  if (ft < 1) ft = 1;
-  if (ft > cap) ft = cap;
-  if (ft > nfoc) ft = nfoc;
-  return ft;
+  int lg = 3;                                           // FT <= 8
+  while (lg > 0 && ((size_t)1 << lg) * per > 72000) --lg;  // <= ~70 KB of traces per CTA: 3 CTAs per SM
+  while (lg > 0 && (1 << (lg - 1)) >= count) --lg;      // no more slots than traces
+  return lg;
 }
 
 FftParams make_params(const mk_ctx* c, int nfoc, int ldf) {
@@ -260,6 +403,8 @@ int set_smem(mk_ctx* c, K kernel, size_t bytes) {
   return check_cuda(c, cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes), "cudaFuncSetAttribute");
 }
 
+size_t trace_smem(const mk_ctx* c, int lgft) { return ((size_t)mkfft::padded_len(c->plan.M) << lgft) * sizeof(float2); }
+
 }  // namespace
 
 int launch_window(mk_ctx* c, const float* d_td, int* d_h, int ntr) {
@@ -269,44 +414,44 @@ int launch_window(mk_ctx* c, const float* d_td, int* d_h, int ntr) {
 }
 
 int launch_load_R(mk_ctx* c, const float* d_R_time, int shot0, int nshots) {
-  const int ST = pick_ft(c, nshots, 8);
-  const size_t smem = (size_t)ST * mkfft::padded_len(c->plan.M) * sizeof(float2);
+  const int lg = pick_lgft(c, nshots), ST = 1 << lg;
+  const size_t smem = trace_smem(c, lg);
   if (int rc = set_smem(c, k_load_R, smem)) return rc;
   const dim3 grid((nshots + ST - 1) / ST, c->n);
   const float sm = (float)(c->dt * c->dx), se = (float)(c->dt * c->dx * 0.5);
-  k_load_R<<<grid, kThreads, smem, c->stream>>>(d_R_time, c->d_Rhat, make_params(c, 0, 0), shot0, nshots, ST, sm, se);
+  k_load_R<<<grid, kThreads, smem, c->stream>>>(d_R_time, c->d_Rhat, make_params(c, 0, 0), shot0, nshots, lg, sm, se);
   ++c->launches;
   return check_cuda(c, cudaGetLastError(), "k_load_R");
 }
 
-int launch_fwd(mk_ctx* c, const float* d_src, float2* d_Nhat, int nfoc, int ldf, bool conj_out, float* d_init_Tsrc) {
-  const int FT = pick_ft(c, nfoc, 8);
-  const size_t smem = (size_t)FT * mkfft::padded_len(c->plan.M) * sizeof(float2);
+int launch_fwd(mk_ctx* c, const float* d_src, const OperandOut& O, int nfoc, bool conj_out, float* d_init_Tsrc) {
+  const int lg = pick_lgft(c, nfoc), FT = 1 << lg;
+  const size_t smem = trace_smem(c, lg);
   if (int rc = set_smem(c, k_fwd, smem)) return rc;
   const dim3 grid((nfoc + FT - 1) / FT, c->n);
-  k_fwd<<<grid, kThreads, smem, c->stream>>>(d_src, d_Nhat, make_params(c, nfoc, ldf), FT, conj_out ? 1 : 0, d_init_Tsrc);
+  k_fwd<<<grid, kThreads, smem, c->stream>>>(d_src, O, make_params(c, nfoc, O.ldf), lg, conj_out ? 1 : 0, d_init_Tsrc);
   ++c->launches;
   return check_cuda(c, cudaGetLastError(), "k_fwd");
 }
 
 int launch_inv(mk_ctx* c, const float2* d_spec, int nfoc, int ldf, float* d_out, float sS, const float* d_A, float sA,
                const float* d_B, float sB) {
-  const int FT = pick_ft(c, nfoc, 8);
-  const size_t smem = (size_t)FT * mkfft::padded_len(c->plan.M) * sizeof(float2);
+  const int lg = pick_lgft(c, nfoc), FT = 1 << lg;
+  const size_t smem = trace_smem(c, lg);
   if (int rc = set_smem(c, k_inv, smem)) return rc;
   const dim3 grid((nfoc + FT - 1) / FT, c->n);
-  k_inv<<<grid, kThreads, smem, c->stream>>>(d_spec, make_params(c, nfoc, ldf), FT, d_out, sS, d_A, sA, d_B, sB);
+  k_inv<<<grid, kThreads, smem, c->stream>>>(d_spec, make_params(c, nfoc, ldf), lg, d_out, sS, d_A, sA, d_B, sB);
   ++c->launches;
   return check_cuda(c, cudaGetLastError(), "k_inv");
 }
 
-int launch_post(mk_ctx* c, int parity_even, float* d_Ni_out) {
-  const int FT = pick_ft(c, c->nfoc, 8);
-  const size_t smem = (size_t)FT * mkfft::padded_len(c->plan.M) * sizeof(float2);
+int launch_post(mk_ctx* c, const OperandOut& O, int parity_even, float* d_Ni_out) {
+  const int lg = pick_lgft(c, c->nfoc), FT = 1 << lg;
+  const size_t smem = trace_smem(c, lg);
   if (int rc = set_smem(c, k_post, smem)) return rc;
   const dim3 grid((c->nfoc + FT - 1) / FT, c->n);
-  k_post<<<grid, kThreads, smem, c->stream>>>(c->d_Shat, c->d_phat, c->d_Nhat, c->d_h, c->d_f1plus, c->d_f1min,
-                                              make_params(c, c->nfoc, c->ldf), FT, parity_even, d_Ni_out);
+  k_post<<<grid, kThreads, smem, c->stream>>>(c->d_Shat, c->d_phat, O, c->d_h, c->d_f1plus, c->d_f1min,
+                                              make_params(c, c->nfoc, c->ldf), lg, parity_even, d_Ni_out);
   ++c->launches;
   return check_cuda(c, cudaGetLastError(), "k_post");
 }

@@ -14,6 +14,9 @@
 // Device layouts (complex64 = float2, interleaved re/im):
 //   Rhat [n][nb][ld]      R^[r][k][s] * dt * w[s]; ld = round_up(n, 16); pad columns are zero        (a0)
 //   Nhat [nb][ld][ldf]    N^[k][s][f]; pad rows (s >= n) and pad columns (f >= nfoc) are zero        (a1, a6)
+//   regime 3 keeps N^ instead as the REAL operand B' [nb][2 ld][ldb] fp32 of the equivalent real GEMM
+//   (rows 2s, 2s+1 = N^[k][s][.] and i N^[k][s][.] as interleaved re/im floats), split into two tf32 planes
+//   hi and lo (3xTF32); ldb = round_up(2 nfoc, 32); pad rows / columns are zero
 //   Shat [n][nb][ldf]     S^[r][k][f]                                                                 (a2)
 //   phat [n][nb][ldf]     running p^- spectrum                                                        (a3)
 //   f1plus, f1min [nfoc][n][nt] fp32 time domain                                                      (a5)
@@ -42,12 +45,26 @@ struct mk_ctx {
   float2* d_Shat = nullptr;
   float2* d_phat = nullptr;
   size_t cap_Nhat = 0, cap_Shat = 0;  // capacities in float2
+  float* d_Bhi = nullptr;             // regime 3 operand planes (see above)
+  float* d_Blo = nullptr;
+  size_t cap_B = 0;                   // capacity (floats) of each plane
+  int ldb = 0;
   int* d_h = nullptr;
   size_t cap_h = 0;
   // scratch operands for mk_synthesis / finals (so a run in progress is not disturbed)
   float2* d_Nhat2 = nullptr;
   float2* d_Shat2 = nullptr;
   size_t cap_Nhat2 = 0, cap_Shat2 = 0;
+  float* d_Bhi2 = nullptr;
+  float* d_Blo2 = nullptr;
+  size_t cap_B2 = 0;
+  // regime 3: cached TMA descriptors (CUtensorMap is 128 bytes, 64-byte aligned), built by mk_syn_tc.cu
+  alignas(64) unsigned char tmap_A[128];
+  alignas(64) unsigned char tmap_B[2][2][128];  // [main / scratch][hi / lo]
+  bool tmap_A_ok = false;
+  const void* tmap_B_key[2] = {nullptr, nullptr};
+  int tmap_B_ldb[2] = {0, 0};
+  void* encode_fn = nullptr;  // cuTensorMapEncodeTiled, resolved at run time through the CUDA runtime
   float* d_stage = nullptr;  // host-call staging
   size_t cap_stage = 0;
   float* d_Gminus = nullptr;  // kept by mk_finish when G^- was requested (mk_image)
@@ -74,6 +91,15 @@ struct FftParams {
   int n, nb, klo, ld, ldf, nfoc;
 };
 
+// where a forward transform stores N^ (a1, a6): the plain complex layout (regimes 1, 2) or the split real operand
+// of regime 3 (bhi != nullptr)
+struct OperandOut {
+  float2* plain;
+  float* bhi;
+  float* blo;
+  int ldf, ldb;
+};
+
 int set_err(mk_ctx* c, int code, const std::string& msg);
 int check_cuda(mk_ctx* c, cudaError_t e, const char* what);
 
@@ -81,16 +107,19 @@ int check_cuda(mk_ctx* c, cudaError_t e, const char* what);
 int launch_window(mk_ctx* c, const float* d_td, int* d_h, int ntr);
 int launch_load_R(mk_ctx* c, const float* d_R_time, int shot0, int nshots);
 // time [nfoc][n][nt] -> Nhat band;  conj_out: spectrum of T(src);  d_init_Tsrc: optional, receives T src
-int launch_fwd(mk_ctx* c, const float* d_src, float2* d_Nhat, int nfoc, int ldf, bool conj_out, float* d_init_Tsrc);
+int launch_fwd(mk_ctx* c, const float* d_src, const OperandOut& O, int nfoc, bool conj_out, float* d_init_Tsrc);
 // spectrum [n][nb][ldf] -> out[j] = sS*S[j] + sA*A[j] + sB*B[(nt-j)%nt]
 int launch_inv(mk_ctx* c, const float2* d_spec, int nfoc, int ldf, float* d_out, float sS, const float* d_A, float sA,
                const float* d_B, float sB);
 // fused a3..a6
-int launch_post(mk_ctx* c, int parity_even, float* d_Ni_out);
+int launch_post(mk_ctx* c, const OperandOut& O, int parity_even, float* d_Ni_out);
 
 // mk_syn_gemv.cu / mk_syn_gemm.cu:  Shat = Rhat x Nhat per bin
 bool gemv_supported(const mk_ctx* c, int nfoc);
 int launch_syn_gemv(mk_ctx* c, const float2* d_Nhat, float2* d_Shat, int nfoc);
 int launch_syn_gemm(mk_ctx* c, const float2* d_Nhat, float2* d_Shat, int ldf);
+// mk_syn_tc.cu: tcgen05 3xTF32 path.  slot: 0 = the run's operand, 1 = the scratch operand (descriptor cache)
+bool tc_supported(const mk_ctx* c);
+int launch_syn_tc(mk_ctx* c, int slot, const float* d_Bhi, const float* d_Blo, float2* d_Shat, int nfoc, int ldf, int ldb);
 
 }  // namespace mk

@@ -33,7 +33,7 @@ def _check_chain(cfg, regime, niter=None, focs=None):
 
 
 # ---------------------------------------------------------------- bare synthesis
-@pytest.mark.parametrize("n,nt,nfoc,regime", [(5, 32, 3, 0), (20, 64, 1, 1), (20, 64, 12, 2)])
+@pytest.mark.parametrize("n,nt,nfoc,regime", [(5, 32, 3, 0), (20, 64, 1, 1), (20, 64, 12, 2), (20, 64, 12, 3)])
 def test_delta_spike_shift(n, nt, nfoc, regime):
     import torch
     from paper_2106_04649_b200 import binding as B
@@ -57,6 +57,7 @@ def test_delta_spike_shift(n, nt, nfoc, regime):
 @pytest.mark.parametrize("n,nt,nfoc,regime", [
     (37, 128, 1, 1), (37, 128, 3, 1), (37, 128, 8, 1),           # GEMV, ragged rows
     (37, 128, 5, 2), (150, 64, 70, 2), (130, 256, 129, 2),        # FFMA GEMM, ragged M / N tiles
+    (37, 128, 5, 3), (150, 64, 70, 3), (130, 256, 129, 3), (260, 64, 140, 3),   # tcgen05 3xTF32, ragged M / N / K tiles
     (16, 16, 2, 0), (33, 4096, 9, 0),                             # smallest / longest traces
 ])
 def test_synthesis_random_vs_oracle(n, nt, nfoc, regime):
@@ -85,7 +86,7 @@ def test_synthesis_random_vs_oracle(n, nt, nfoc, regime):
 # ---------------------------------------------------------------- whole chain, reduced copies of the configs
 @pytest.mark.parametrize("k,n,nt,nfoc,regime", [
     (0, 40, 256, 1, 1), (1, 70, 512, 4, 1), (1, 70, 512, 4, 2), (2, 70, 512, 70, 2), (3, 90, 512, 19, 2),
-    (4, 60, 1024, 33, 2),
+    (4, 60, 1024, 33, 2), (2, 70, 512, 70, 3), (3, 90, 512, 19, 3), (4, 60, 1024, 33, 3),
 ])
 def test_chain_reduced_configs(k, n, nt, nfoc, regime):
     focal = "single:400" if nfoc == 1 else ("line:300" if nfoc == n else "fan:250")
