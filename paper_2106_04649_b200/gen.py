@@ -238,3 +238,96 @@ def subset_indices(cfg: Config, nrec: int = 32, nfoc: int = 16):
     recs = np.sort(rng.choice(cfg.n, size=min(nrec, cfg.n), replace=False))
     focs = np.sort(rng.choice(cfg.nfoc, size=min(nfoc, cfg.nfoc), replace=False))
     return recs, focs
+
+
+# ----------------------------------------------------------------------------------------------
+# device twin of R_block: configs 3 and 4 (33 GB / 250 GB of time-domain R) are produced chunk by chunk on the device
+# and handed to mk_load_R; nothing of that size is ever stored.  Same recipe, same counters: a gather of the same base
+# traces plus (config 3) the same Box-Muller normals.  Still no arithmetic of the method.
+# ----------------------------------------------------------------------------------------------
+def _i64(v: int) -> int:
+    """a uint64 constant as the int64 with the same bits (torch has no uint64 arithmetic)."""
+    v &= (1 << 64) - 1
+    return v - (1 << 64) if v >= (1 << 63) else v
+
+
+def _mix_torch(x):
+    """_mix on int64 tensors: wrapping multiply, logical right shifts by masking the sign extension."""
+    def lsr(z, k):
+        return (z >> k) & ((1 << (64 - k)) - 1)
+    z = x + _i64(int(_GOLD))
+    z = (z ^ lsr(z, 30)) * _i64(int(_M1))
+    z = (z ^ lsr(z, 27)) * _i64(int(_M2))
+    return z ^ lsr(z, 31)
+
+
+def _uniforms_torch(seed: int, stream: int, idx):
+    import torch
+    z = _mix_torch(idx * _i64(int(_GOLD)) + _i64(int(_key(seed, stream))))
+    top53 = (z >> 11) & ((1 << 53) - 1)
+    return top53.to(torch.float64) * (1.0 / 9007199254740992.0)
+
+
+class DeviceR:
+    """R_block on a torch device.  `take(shots)` returns the fp32 chunk [len(shots)][n][nt] (receivers = all)."""
+
+    def __init__(self, cfg: Config, device, base: np.ndarray | None = None):
+        import torch
+        self.cfg, self.device = cfg, device
+        base = base_traces(cfg) if base is None else base
+        self.base = torch.from_numpy(base).to(device)
+        self.sigma = None
+        if cfg.noise_snr_db is not None:
+            self.sigma = torch.from_numpy(_noise_sigma(cfg, base)).to(device)          # fp64 [n]
+
+    def take(self, shots, recs=None):
+        import torch
+        cfg = self.cfg
+        shots = torch.as_tensor(np.asarray(shots, dtype=np.int64), device=self.device)
+        recs = torch.arange(cfg.n, device=self.device) if recs is None else torch.as_tensor(np.asarray(recs, dtype=np.int64),
+                                                                                          device=self.device)
+        off = (shots[:, None] - recs[None, :]).abs()
+        blk = self.base[off]                                                           # gather (copy)
+        if self.sigma is not None:
+            half, pairs = cfg.nt // 2, cfg.nt // 4
+            trace_id = shots[:, None] * cfg.n + recs[None, :]
+            ctr = trace_id[:, :, None] * half + 2 * torch.arange(pairs, device=self.device, dtype=torch.int64)[None, None, :]
+            u1 = 1.0 - _uniforms_torch(cfg.seed, _S_NOISE, ctr)
+            u2 = _uniforms_torch(cfg.seed, _S_NOISE, ctr + 1)
+            rad = torch.sqrt(-2.0 * torch.log(u1))
+            ang = 2.0 * math.pi * u2
+            z = torch.empty(trace_id.shape + (half,), dtype=torch.float64, device=self.device)
+            z[..., 0::2] = rad * torch.cos(ang)
+            z[..., 1::2] = rad * torch.sin(ang)
+            blk[:, :, :half] = (blk[:, :, :half].to(torch.float64) + self.sigma[off][:, :, None] * z).to(torch.float32)
+        return blk
+
+
+def first_arrivals_torch(cfg: Config, device, focs=None, chunk: int = 8):
+    """first_arrivals with the wavelet evaluated on `device` (config 4: 256 x 3901 x 4096 samples).  t_d is the
+    host function's, bit for bit; G_d may differ from the numpy one in the last fp32 bit (exp), so whoever needs
+    the same bytes on both sides takes them from this tensor."""
+    import torch
+    xf, zf = focal_points(cfg)
+    if focs is not None:
+        focs = np.asarray(focs, dtype=np.int64)
+        xf, zf = xf[focs], zf[focs]
+    r = np.arange(cfg.n)
+    v0 = layer_model(cfg).v[0]
+    td = np.sqrt(zf[:, None] ** 2 + (r[None, :] * cfg.dx - xf[:, None]) ** 2) / v0
+    frac = td / cfg.dt + 0.5
+    tie = np.abs(frac - np.round(frac)) < 1e-3
+    td32 = np.where(tie, td + 0.01 * cfg.dt, td).astype(np.float32)
+    tmax = (cfg.nt // 2) * cfg.dt
+    d_td = torch.from_numpy(td32).to(device)
+    t = torch.arange(cfg.nt, device=device, dtype=torch.float64) * cfg.dt
+    gd = torch.empty((len(xf), cfg.n, cfg.nt), dtype=torch.float32, device=device)
+    for f0 in range(0, len(xf), chunk):
+        tdc = d_td[f0:f0 + chunk].to(torch.float64)
+        u = t[None, None, :] - tdc[:, :, None]
+        a = (math.pi * cfg.fpeak) ** 2 * u * u
+        w = (1.0 - 2.0 * a) * torch.exp(-a)
+        w = torch.where(u.abs() <= cfg.half_support, w, torch.zeros_like(w))
+        live = (tdc + cfg.half_support <= tmax)
+        gd[f0:f0 + chunk] = (w * live[:, :, None]).to(torch.float32)
+    return gd, d_td

@@ -46,3 +46,42 @@ def test_first_arrivals():
     assert r == 50 and abs(np.argmax(gd[0, r]) * cfg.dt - td[0, r]) <= cfg.dt
     frac = td.astype(np.float64) / cfg.dt + 0.5
     assert np.all(np.abs(frac - np.round(frac)) > 1e-4)           # no half-sample ties (G2c)
+
+
+def test_device_twin_matches_numpy_generator():
+    """gen.DeviceR (configs 3 / 4 are generated chunk by chunk on the device) == gen.R_block on a CPU torch device:
+    bit-exact without noise; with noise the normals go through torch's log / cos / sin instead of numpy's, so allow
+    one fp32 ulp of the trace peak."""
+    import torch
+    from paper_2106_04649_b200 import configs, gen
+    for k, exact in ((4, True), (3, False)):
+        cfg = configs.scaled(k, n=23, nt=128, nfoc=1, focal="single:300")
+        base = gen.base_traces(cfg)
+        shots, recs = np.array([0, 5, 22, 7]), np.array([3, 22, 0, 11, 12])
+        ref = gen.R_block(cfg, base, shots, recs)
+        got = gen.DeviceR(cfg, torch.device("cpu"), base).take(shots, recs).numpy()
+        assert got.shape == ref.shape and got.dtype == np.float32
+        if exact:
+            np.testing.assert_array_equal(got, ref)
+        else:
+            assert np.abs(ref).max() > 0 and not np.array_equal(ref, gen.R_block(replace_noise(cfg), base, shots, recs))
+            np.testing.assert_allclose(got, ref, rtol=0, atol=2e-7 * np.abs(ref).max())
+        full = gen.DeviceR(cfg, torch.device("cpu"), base).take(np.arange(cfg.n)).numpy()
+        np.testing.assert_allclose(full, gen.R_full(cfg, base), rtol=0, atol=0 if exact else 2e-7 * np.abs(ref).max())
+
+
+def replace_noise(cfg):
+    from dataclasses import replace
+    return replace(cfg, noise_snr_db=None)
+
+
+def test_first_arrivals_device_twin():
+    import torch
+    from paper_2106_04649_b200 import configs, gen
+    cfg = configs.scaled(3, n=41, nt=256, nfoc=5, focal="fan:250")
+    gd, td = gen.first_arrivals(cfg)
+    gdt, tdt = gen.first_arrivals_torch(cfg, torch.device("cpu"), chunk=2)
+    np.testing.assert_array_equal(tdt.numpy(), td)
+    np.testing.assert_allclose(gdt.numpy(), gd, rtol=0, atol=2e-7)
+    gdt2, tdt2 = gen.first_arrivals_torch(cfg, torch.device("cpu"), focs=[1, 4])
+    np.testing.assert_array_equal(gdt2.numpy(), gdt.numpy()[[1, 4]])

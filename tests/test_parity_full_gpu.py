@@ -1,0 +1,134 @@
+"""Parity at BASELINE.json's FULL sizes, in the launch configuration bench.py times (regime chosen by the library).
+
+Config 1 (601 x 601 x 2048, one focal point): the whole chain, every receiver, oracle feeding itself.
+Configs 2-4: SURVEY.md section 8(c) "single step" — the oracle takes the GPU's N_{i-1} at every source position of a
+seeded subset of focal points (gen.subset_indices, seed_k + 1000) and computes its own N_i on a seeded subset of
+receivers; the 2e-5 per-iteration bound is checked on that, and the 1e-4 bound on f1+/-, G, G+/- accumulated by the
+oracle from its own single-step iterates plus two single-step finals.  Subset: 32 receivers x 16 focal points
+(north_star) for configs 2 and 3; config 4 defaults to 8 x 4 so that the suite stays within minutes
+(MK_PARITY_SUBSET=32x16 gives the full subset there as well; MK_PARITY_SKIP=4 leaves a config out).
+
+R of configs 3 and 4 (33 GB / 250 GB in the time domain) is produced on the device in 64-shot chunks by the generator's
+device twin and handed to mk_load_R chunk by chunk; the oracle's receiver columns are taken from the very same chunks,
+so both sides see the same bytes.  Nothing here reads /root/reference.
+"""
+import os
+import time
+
+import numpy as np
+import pytest
+
+import oracle
+from paper_2106_04649_b200 import configs, gen
+from _util import gpu_chain, problem, rel_l2
+
+pytestmark = pytest.mark.gpu
+
+TOL_ITER, TOL_FINAL = 2e-5, 1e-4
+REGIME = int(os.environ.get("MK_PARITY_REGIME", "0"))      # 0 = the library's own choice (what bench.py times)
+SKIP = {int(x) for x in os.environ.get("MK_PARITY_SKIP", "").split(",") if x.strip()}
+
+
+def _subset_shape(k):
+    env = os.environ.get("MK_PARITY_SUBSET")
+    if env:
+        a, b = env.lower().split("x")
+        return int(a), int(b)
+    return (8, 4) if k == 4 else (32, 16)
+
+
+def test_config1_full_chain_all_receivers():
+    if 1 in SKIP:
+        pytest.skip("MK_PARITY_SKIP")
+    cfg = configs.get(1)
+    R, Gd, td = problem(cfg)
+    t0 = time.time()
+    ref = oracle.marchenko(R, Gd, td, cfg.dt, cfg.dx, cfg.fmin, cfg.fmax, cfg.niter, cfg.eps)
+    t_or = time.time() - t0
+    got = gpu_chain(cfg, R, Gd, td)                       # regime 0 = automatic: the streaming GEMV
+    assert got["regime_used"] == 1
+    errs = [rel_l2(got["N_iters"][i], ref["N_iters"][i]) for i in range(cfg.niter)]
+    fin = {nm: rel_l2(got[nm], ref[nm]) for nm in ("f1plus", "f1min", "G", "Gplus", "Gminus")}
+    print(f"\n[config 1 full chain, oracle {t_or:.0f} s on {oracle.num_threads()} threads] per-iteration max {max(errs):.2e}; "
+          + " ".join(f"{k}={v:.1e}" for k, v in fin.items()))
+    # the series must still be alive at the last iterate, or the per-iteration bound would be vacuous
+    assert np.linalg.norm(ref["N_iters"][-1]) > 1e-7 * np.linalg.norm(ref["N_iters"][0])
+    assert max(errs) <= TOL_ITER, errs
+    assert max(fin.values()) <= TOL_FINAL, fin
+
+
+@pytest.mark.parametrize("k", [2, 3, 4])
+def test_full_size_single_steps_on_seeded_subset(k):
+    if k in SKIP:
+        pytest.skip("MK_PARITY_SKIP")
+    import torch
+    from paper_2106_04649_b200 import binding as B
+    cfg = configs.get(k)
+    n, nt, nfoc, niter = cfg.n, cfg.nt, cfg.nfoc, cfg.niter
+    dev = torch.device("cuda:0")
+    free, _ = torch.cuda.mem_get_info()
+    klo, khi, nb = oracle.band(nt, cfg.dt, cfg.fmin, cfg.fmax)
+    # R^ + three time fields (f1plus, f1min, one in/out buffer) + operands (regime 3: 4x a complex N^ per slot, two slots,
+    # plus S^, p^, scratch S^) + the 64-shot chunk
+    need = 8.0 * n * nb * (n + 16) + 4.0 * nfoc * n * nt * 3.1 + 8.0 * n * nb * nfoc * 11 + 6e9
+    if free < need:
+        pytest.skip(f"config {k} needs about {need / 1e9:.0f} GB of device memory, {free / 1e9:.0f} GB free")
+    nrec_s, nfoc_s = _subset_shape(k)
+    recs, focs = gen.subset_indices(cfg, nrec_s, nfoc_s)
+    recs_t = torch.as_tensor(recs, device=dev)
+    focs_t = torch.as_tensor(focs, device=dev)
+    T = lambda a: np.roll(a[..., ::-1], 1, axis=-1)
+
+    t0 = time.time()
+    gR = gen.DeviceR(cfg, dev)
+    R_sub = np.empty((n, len(recs), nt), np.float32)
+    with B.Marchenko(n, n, nt, cfg.dt, cfg.dx, cfg.fmin, cfg.fmax) as mk:
+        mk.set_option(B.MK_OPT_EPS_SAMPLES, cfg.eps)
+        mk.set_option(B.MK_OPT_REGIME, REGIME)
+        for s0 in range(0, n, 64):                                    # BASELINE.json config 4: 64-shot chunks
+            s1 = min(s0 + 64, n)
+            chunk = gR.take(np.arange(s0, s1))
+            mk.load_R(chunk, s0)
+            R_sub[s0:s1] = chunk[:, recs_t].cpu().numpy()
+            del chunk
+        del gR
+        t_load = time.time() - t0
+        dGd, dtd = gen.first_arrivals_torch(cfg, dev)
+        Gd_f = dGd[focs_t].cpu().numpy()                               # [nfoc_s][n][nt]: same bytes as the GPU's input
+        td = dtd.cpu().numpy()
+        sub = oracle.SubsetChain(R_sub, td[focs][:, recs], Gd_f[:, recs], cfg.dt, cfg.dx, cfg.fmin, cfg.fmax, cfg.eps)
+        mk.begin(dGd, dtd)
+        torch.cuda.synchronize()
+        del dGd
+        torch.cuda.empty_cache()
+        buf = torch.empty((nfoc, n, nt), dtype=torch.float32, device=dev)
+        prev = T(Gd_f.astype(np.float64))                              # N_{-1} = T G_d at every source position
+        errs, norms, t_or = [], [], 0.0
+        for it in range(niter):
+            mk.step(buf)
+            cur = buf[focs_t].cpu().numpy()
+            t1 = time.time()
+            Nn = sub.step(prev)                                        # the oracle's N_i from the GPU's N_{i-1}
+            t_or += time.time() - t1
+            errs.append(rel_l2(cur[:, recs], Nn))
+            norms.append(float(np.linalg.norm(Nn)))
+            prev = cur.astype(np.float64)
+        regime = int(mk.get_info(B.MK_INFO_REGIME_USED))
+        fin_err = {}
+        acc = {}
+        for nm in ("f1plus", "f1min"):
+            mk.finish({nm: buf})
+            acc[nm] = buf[focs_t].cpu().numpy().astype(np.float64)
+            fin_err[nm] = rel_l2(acc[nm][:, recs], getattr(sub, nm))
+        t1 = time.time()
+        fin = sub.finals(acc["f1plus"], acc["f1min"])
+        t_or += time.time() - t1
+        for nm in ("G", "Gplus", "Gminus"):
+            mk.finish({nm: buf})
+            fin_err[nm] = rel_l2(buf[focs_t][:, recs_t].cpu().numpy(), fin[nm])
+    print(f"\n[config {k} full size n={n} nt={nt} nfoc={nfoc} regime={regime}; subset {len(recs)} rec x {len(focs)} foc; "
+          f"ingest {t_load:.0f} s, oracle {t_or:.0f} s on {oracle.num_threads()} threads] per-iteration max {max(errs):.2e}; "
+          + " ".join(f"{a}={b:.1e}" for a, b in fin_err.items()))
+    assert norms[-1] > 1e-7 * norms[0] > 0, norms                    # the series is alive: the bound is not vacuous
+    assert max(errs) <= TOL_ITER, errs
+    assert max(fin_err.values()) <= TOL_FINAL, fin_err
