@@ -188,6 +188,41 @@ MK_HD void inv_butterfly(float2* z, const float2* __restrict__ tw, int nt, int l
   for (int j = 0; j < R; ++j) z[padi(base + (j << lgq))] = a[j];
 }
 
+// ---- 32-point DFT held entirely in registers (the building block of the register-resident path, mk_fft_fast.cu):
+// 32 = 4 x 8, natural order in and out; every index below is a compile-time constant after unrolling, so the
+// twiddles are immediates and the final reordering is a renaming of registers.
+MK_HD float w32_cos(int m) {
+  constexpr float t[32] = {1.f, 0.980785251f, 0.923879504f, 0.831469595f, 0.707106769f, 0.555570245f, 0.382683426f, 0.195090324f,
+                           0.f, -0.195090324f, -0.382683426f, -0.555570245f, -0.707106769f, -0.831469595f, -0.923879504f, -0.980785251f,
+                           -1.f, -0.980785251f, -0.923879504f, -0.831469595f, -0.707106769f, -0.555570245f, -0.382683426f, -0.195090324f,
+                           0.f, 0.195090324f, 0.382683426f, 0.555570245f, 0.707106769f, 0.831469595f, 0.923879504f, 0.980785251f};
+  return t[m & 31];
+}
+MK_HD float w32_sin(int m) { return w32_cos(m - 8); }  // sin(x) = cos(x - pi/2)
+
+template <bool INV>
+MK_HD void fft32(float2 (&a)[32]) {
+  // input n = 8 n1 + n2, output k = k1 + 4 k2
+#pragma unroll
+  for (int n2 = 0; n2 < 8; ++n2) dft4<INV>(a[n2], a[8 + n2], a[16 + n2], a[24 + n2]);  // a[8 k1 + n2] = Y[k1][n2]
+#pragma unroll
+  for (int k1 = 1; k1 < 4; ++k1)
+#pragma unroll
+    for (int n2 = 1; n2 < 8; ++n2) {
+      const float2 w = make_float2(w32_cos(k1 * n2), -w32_sin(k1 * n2));  // e^{-2 pi i k1 n2 / 32}
+      a[8 * k1 + n2] = INV ? cmulc(a[8 * k1 + n2], w) : cmul(a[8 * k1 + n2], w);
+    }
+#pragma unroll
+  for (int k1 = 0; k1 < 4; ++k1) dft8<INV>(&a[8 * k1]);  // a[8 k1 + k2] = X[k1 + 4 k2]
+  float2 b[32];
+#pragma unroll
+  for (int k1 = 0; k1 < 4; ++k1)
+#pragma unroll
+    for (int k2 = 0; k2 < 8; ++k2) b[k1 + 4 * k2] = a[8 * k1 + k2];
+#pragma unroll
+  for (int i = 0; i < 32; ++i) a[i] = b[i];
+}
+
 // ---- real <-> half-spectrum split steps
 // Forward: X[k] (0 <= k <= M) of the real trace from the digit-reversed Z held in z.
 MK_HD float2 rfft_bin(const float2* z, const Plan& p, const float2* __restrict__ tw, int k) {

@@ -7,7 +7,7 @@
 #include <cstring>
 #include <new>
 
-#include "mk_internal.cuh"
+#include "mk_fft_common.cuh"
 
 namespace mk {
 
@@ -226,6 +226,18 @@ int mk_create(mk_ctx** out, int nshot, int nrec, int nt, double dt, double dx, d
     if (int rc = ensure(c, &c->d_tw, &cap, (size_t)nt, "twiddles")) return rc;
     if (int rc = check_cuda(c, cudaMemcpy(c->d_tw, tw.data(), nt * sizeof(float2), cudaMemcpyHostToDevice), "twiddle upload")) return rc;
   }
+  {  // middle twiddles of the register-resident path: W_1024^{k1 t}, table constants evaluated in double
+    std::vector<float2> tw(1024);
+    const double two_pi = 6.283185307179586476925286766559;
+    for (int k1 = 0; k1 < 32; ++k1)
+      for (int t = 0; t < 32; ++t) {
+        const double a = -two_pi * (double)(k1 * t) / 1024.0;
+        tw[k1 * 32 + t] = make_float2((float)std::cos(a), (float)std::sin(a));
+      }
+    size_t cap = 0;
+    if (int rc = ensure(c, &c->d_tw1k, &cap, (size_t)1024, "twiddles 1k")) return rc;
+    if (int rc = check_cuda(c, cudaMemcpy(c->d_tw1k, tw.data(), 1024 * sizeof(float2), cudaMemcpyHostToDevice), "twiddle upload")) return rc;
+  }
   {
     size_t cap = 0;
     const size_t cnt = (size_t)nrec * c->nb * c->ld;
@@ -238,6 +250,7 @@ int mk_create(mk_ctx** out, int nshot, int nrec, int nt, double dt, double dx, d
 int mk_destroy(mk_ctx* c) {
   if (!c) return MK_OK;
   cudaFree(c->d_tw);
+  cudaFree(c->d_tw1k);
   cudaFree(c->d_Rhat);
   cudaFree(c->d_f1plus);
   cudaFree(c->d_f1min);
@@ -279,6 +292,12 @@ int mk_set_option(mk_ctx* c, int key, double value) {
       return MK_OK;
     case MK_OPT_TIMING:
       c->timing = value != 0.0;
+      return MK_OK;
+    case MK_OPT_FFT_PATH:
+      if (value < 0 || value > 2 || value != std::floor(value)) return set_err(c, MK_ERR_INVALID_ARG, "fft path must be 0..2");
+      if ((int)value == 2 && c->nt != 2048 && c->nt != 4096)
+        return set_err(c, MK_ERR_INVALID_ARG, "the register-resident transform path needs nt = 2048 or 4096");
+      c->fft_path = (int)value;
       return MK_OK;
     default:
       return set_err(c, MK_ERR_INVALID_ARG, "unknown option");

@@ -1,0 +1,477 @@
+// mk_fft_fast.cu — register-resident transform kernels for nt = 2048 and nt = 4096 (every BASELINE.json config but
+// the tiny one): the same four per-trace kernels as mk_fft_kernels.cu, built on
+// a 1024-point complex FFT that ONE WARP runs with 32 values per thread:
+//
+//   four-step FFT, 1024 = 32 x 32:  a 32-point DFT in registers (fft_core.cuh fft32), the middle twiddles W_1024^{k1 t}
+//   from a 32 x 32 table, ONE transposition through shared memory (rows padded to 33, conflict-free both ways), and a
+//   second 32-point DFT in registers.  Input: lane t holds x[t + 32 q], q = 0..31; output: lane t holds X[t + 32 q].
+//   The transform of the time-domain result therefore starts straight from the registers the window left.
+//
+// A real trace of nt samples is M = nt/2 complex numbers z[m] = x[2m] + i x[2m+1] (fft_core.cuh).  nt = 2048: M = 1024,
+// one warp per trace.  nt = 4096: M = 2048 = 2 x 1024, two warps per trace (HF = 2): warp h owns the samples
+// z[2 n' + h]; the radix-2 step that joins the two halves is folded into the shared-memory phases that exist anyway
+// (decimation in frequency on the way in: A_h[k] = (Z[k] + (-1)^h Z[k + 1024]) W_2048^{-h k}; decimation in time on
+// the way out: Z[k] = F_0[k mod 1024] +- W_2048^{k mod 1024} F_1[k mod 1024]).
+//
+// One CTA = one receiver r and FT consecutive focal points (the S^[r][k][f..] reads and N^[k][r][f..] writes are
+// contiguous 8 FT-byte segments); its phases:
+//   P1 (CTA-wide, focal point fastest)  half spectra from HBM -> Z in shared memory (p^ += S^ on the way)
+//   P2 (per warp)  inverse transform, registers <- time samples
+//   P3 (per warp)  window, accumulation into f1min / f1plus straight from registers (coalesced float2 rows)
+//   P4 (per warp)  forward transform, Z -> shared memory
+//   P5 (CTA-wide)  band of the half spectrum -> operand of the next contraction
+// Compared with the generic kernels this is ~8 shared-memory accesses per complex element and pass instead of ~21,
+// no digit-reversal arithmetic, and warp-level synchronisation only inside P2..P4.
+#include "mk_fft_common.cuh"
+
+namespace mk {
+
+namespace {
+
+using mkfft::cadd;
+using mkfft::cmul;
+using mkfft::cmulc;
+using mkfft::csub;
+
+constexpr int SUB = 32 * 33;  // float2 per 1024-point block: 32 rows of 32 + 1 pad
+
+template <int HF>
+struct Geo {
+  static constexpr int M = 1024 * HF;      // complex length of a trace
+  static constexpr int TS = HF * SUB + 2;  // float2 between traces in shared memory (== 2 mod 16: P1 / P5 conflict-free)
+};
+
+struct FastParams {
+  const float2* tw;    // [nt]      e^{-2 pi i k / nt}
+  const float2* tw1k;  // [32][32]  e^{-2 pi i k1 t / 1024}
+  int nt, n, nb, klo, ld, ldf, nfoc;
+};
+
+// natural index k (0 <= k < M) of Z -> float2 offset inside the trace's shared-memory block
+__device__ __forceinline__ int zaddr(int k) { return (k >> 10) * SUB + ((k & 1023) >> 5) * 33 + (k & 31); }
+
+// all warps of one trace (HF = 1: the warp itself)
+template <int HF>
+__device__ __forceinline__ void trace_sync(int tl) {
+  if (HF == 1) __syncwarp();
+  else asm volatile("bar.sync %0, %1;" ::"r"(tl + 1), "r"(32 * HF) : "memory");
+}
+
+// 1024-point complex FFT by one warp.  In: lane t holds a[q] = x[t + 32 q].  Out: lane t holds a[q] = X[t + 32 q].
+// scratch: 1056 float2 owned by this warp (contents destroyed).  INV: e^{+...}, no scaling.
+template <bool INV>
+__device__ __forceinline__ void warp_fft1024(float2 (&a)[32], float2* scratch, const float2* __restrict__ tw1k, int t) {
+  mkfft::fft32<INV>(a);  // a[k1] = Y[k1][n2 = t]
+#pragma unroll
+  for (int k1 = 1; k1 < 32; ++k1) {
+    const float2 w = __ldg(tw1k + k1 * 32 + t);
+    a[k1] = INV ? cmulc(a[k1], w) : cmul(a[k1], w);
+  }
+  __syncwarp();  // every lane is done reading the scratch block
+#pragma unroll
+  for (int k1 = 0; k1 < 32; ++k1) scratch[k1 * 33 + t] = a[k1];
+  __syncwarp();
+#pragma unroll
+  for (int n2 = 0; n2 < 32; ++n2) a[n2] = scratch[t * 33 + n2];
+  mkfft::fft32<INV>(a);  // a[k2] = X[k1 = t + 32 k2]
+}
+
+// P2 load: this warp's input of the inverse transform from the natural-order Z in shared memory
+template <int HF>
+__device__ __forceinline__ void load_Z(float2 (&a)[32], const float2* zt, int hf, int t, const float2* __restrict__ tw) {
+  if (HF == 1) {
+#pragma unroll
+    for (int n1 = 0; n1 < 32; ++n1) a[n1] = zt[n1 * 33 + t];
+  } else {
+#pragma unroll
+    for (int n1 = 0; n1 < 32; ++n1) {
+      const float2 z0 = zt[n1 * 33 + t], z1 = zt[SUB + n1 * 33 + t];
+      if (hf == 0) a[n1] = cadd(z0, z1);
+      else a[n1] = cmulc(csub(z0, z1), __ldg(tw + 2 * (32 * n1 + t)));  // e^{+2 pi i k / 2048} = conj tw[2k], nt = 4096
+    }
+  }
+}
+
+// P4 store: this warp's forward result -> natural-order blocks in shared memory (HF = 2: the odd half pre-twiddled)
+template <int HF>
+__device__ __forceinline__ void store_Z(const float2 (&a)[32], float2* zt, int hf, int t, const float2* __restrict__ tw) {
+  __syncwarp();
+#pragma unroll
+  for (int k2 = 0; k2 < 32; ++k2) {
+    float2 v = a[k2];
+    if (HF == 2 && hf == 1) v = cmul(v, __ldg(tw + 2 * (t + 32 * k2)));
+    zt[hf * SUB + k2 * 33 + t] = v;
+  }
+}
+
+template <int HF>
+__device__ __forceinline__ float2 Zval(const float2* zt, int k) {  // Z[k], 0 <= k < M, after store_Z
+  if (HF == 1) return zt[zaddr(k)];
+  const int kp = k & 1023, ad = (kp >> 5) * 33 + (kp & 31);
+  const float2 e = zt[ad], o = zt[SUB + ad];
+  return k < 1024 ? cadd(e, o) : csub(e, o);
+}
+
+// X[k] (0 <= k <= M) of the real trace from its Z (same arithmetic as mkfft::rfft_bin)
+template <int HF>
+__device__ __forceinline__ float2 rfft_bin_fast(const float2* zt, const float2* __restrict__ tw, int k) {
+  constexpr int M = Geo<HF>::M;
+  const float2 a = Zval<HF>(zt, k & (M - 1));
+  const float2 b = Zval<HF>(zt, (M - k) & (M - 1));
+  const float er = 0.5f * (a.x + b.x), ei = 0.5f * (a.y - b.y);
+  const float orr = 0.5f * (a.y + b.y), oi = -0.5f * (a.x - b.x);
+  const float2 w = __ldg(tw + k);
+  return make_float2(er + w.x * orr - w.y * oi, ei + w.x * oi + w.y * orr);
+}
+
+// P1.  Z (natural order, scaled by 1/nt) of all FT traces from their band-limited half spectra.  CTA-wide: consecutive
+// threads take consecutive focal points of one bin.  load(tl, kk, aux) returns X[klo + kk] of trace tl (and may fetch
+// a side value into aux); commit(tl, kk, X, aux) runs afterwards.  Both are called exactly once per in-band (k, tl);
+// the loads of four items are issued before anything is consumed.  CONJ: transform conj(X) instead (time reversal).
+template <int HF, typename Load, typename Commit>
+__device__ __forceinline__ void spectrum_in(float2* smem, int nf, int lgFT, bool conj_in, const FastParams& P, Load load,
+                                            Commit commit) {
+  constexpr int M = Geo<HF>::M, half = M >> 1, TS = Geo<HF>::TS;
+  const int FT = 1 << lgFT, nthr = blockDim.x;
+  const float scale = 1.0f / (2.0f * (float)M);
+  const int total = (half + 1) << lgFT;
+  const int klo = P.klo, khi1 = P.klo + P.nb;
+  for (int i0 = threadIdx.x; i0 < total; i0 += 4 * nthr) {
+    float2 a[4], b[4], xa[4], xb[4];
+#pragma unroll
+    for (int u = 0; u < 4; ++u) {
+      const int idx = i0 + u * nthr;
+      a[u] = b[u] = xa[u] = xb[u] = make_float2(0.f, 0.f);
+      if (idx < total) {
+        const int k = idx >> lgFT, tl = idx & (FT - 1), k2 = M - k;
+        if (tl < nf) {
+          if (k >= klo && k < khi1) a[u] = load(tl, k - klo, xa[u]);
+          if (k2 != k && k2 >= klo && k2 < khi1) b[u] = load(tl, k2 - klo, xb[u]);
+        }
+      }
+    }
+#pragma unroll
+    for (int u = 0; u < 4; ++u) {
+      const int idx = i0 + u * nthr;
+      if (idx >= total) continue;
+      const int k = idx >> lgFT, tl = idx & (FT - 1), k2 = M - k;
+      if (tl >= nf) continue;
+      if (k >= klo && k < khi1) commit(tl, k - klo, a[u], xa[u]);
+      if (k2 != k && k2 >= klo && k2 < khi1) commit(tl, k2 - klo, b[u], xb[u]);
+      float2 x = a[u], y = b[u];
+      if (k2 == k) y = x;
+      if (k == 0) {  // DC and Nyquist are real for a real trace (irfft convention)
+        x.y = 0.f;
+        y.y = 0.f;
+      }
+      if (conj_in) {
+        x.y = -x.y;
+        y.y = -y.y;
+      }
+      float2* zt = smem + tl * TS;
+      zt[zaddr(k)] = mkfft::irfft_pre(x, y, __ldg(P.tw + k), scale);
+      if (k2 < M && k2 != k) zt[zaddr(k2)] = mkfft::irfft_pre(y, x, __ldg(P.tw + k2), scale);
+    }
+  }
+}
+
+// P5.  emit(tl, kk, X[klo + kk]) for every in-band bin of every trace; CTA-wide, trace index fastest
+template <int HF, typename Emit>
+__device__ __forceinline__ void band_out(const float2* smem, int nf, int lgFT, const FastParams& P, Emit emit) {
+  constexpr int TS = Geo<HF>::TS;
+  const int FT = 1 << lgFT, total = P.nb << lgFT;
+  for (int idx = threadIdx.x; idx < total; idx += blockDim.x) {
+    const int kk = idx >> lgFT, tl = idx & (FT - 1);
+    if (tl >= nf) continue;
+    emit(tl, kk, rfft_bin_fast<HF>(smem + tl * TS, P.tw, P.klo + kk));
+  }
+}
+
+// float offset inside a trace of the sample pair held in register q of lane t of warp hf
+template <int HF>
+__device__ __forceinline__ int sample_j(int q, int t, int hf) { return 2 * (HF * (t + 32 * q) + hf); }
+
+struct Who {
+  int tl, hf, t;
+};
+template <int HF>
+__device__ __forceinline__ Who who() {
+  const int w = threadIdx.x >> 5;
+  return Who{w / HF, w % HF, (int)(threadIdx.x & 31)};
+}
+
+// P3 load of a whole trace: lane t, register q <- samples (j, j+1), j = sample_j(q)
+template <int HF>
+__device__ __forceinline__ void load_time(float2 (&a)[32], const float* __restrict__ src, const Who& me) {
+#pragma unroll
+  for (int q = 0; q < 32; ++q) a[q] = __ldg(reinterpret_cast<const float2*>(src + sample_j<HF>(q, me.t, me.hf)));
+}
+
+// ------------------------------------------------------------------------------------------------ k_load_R_fast
+// grid (ceil(nshots / ST), nrec); Rt: [nshots][nrec][nt]                                        (a0)
+template <int HF>
+__global__ void __launch_bounds__(256 * HF, 2 / HF)
+k_load_R_fast(const float* __restrict__ Rt, float2* __restrict__ Rhat, FastParams P, int shot0, int nshots, int lgST,
+              float scale_mid, float scale_end) {
+  extern __shared__ float2 smem[];
+  constexpr int TS = Geo<HF>::TS;
+  const int ST = 1 << lgST, r = blockIdx.y, g0 = blockIdx.x * ST;
+  const int ns = min(ST, nshots - g0);
+  const Who me = who<HF>();
+  if (me.tl < ns) {
+    float2 a[32];
+    load_time<HF>(a, Rt + ((size_t)(g0 + me.tl) * P.n + r) * P.nt, me);
+    float2* zt = smem + me.tl * TS;
+    warp_fft1024<false>(a, zt + me.hf * SUB, P.tw1k, me.t);
+    store_Z<HF>(a, zt, me.hf, me.t, P.tw);
+  }
+  __syncthreads();
+  band_out<HF>(smem, ns, lgST, P, [&](int tl, int kk, float2 X) {
+    const int s = shot0 + g0 + tl;
+    const float sc = (P.n > 1 && (s == 0 || s == P.n - 1)) ? scale_end : scale_mid;
+    Rhat[((size_t)r * P.nb + kk) * P.ld + s] = make_float2(sc * X.x, sc * X.y);
+  });
+}
+
+// ------------------------------------------------------------------------------------------------ k_fwd_fast
+// grid (ceil(nfoc / FT), n); src: [nfoc][n][nt]                                                        (a1, a6)
+template <int HF>
+__global__ void __launch_bounds__(256 * HF, 2 / HF)
+k_fwd_fast(const float* __restrict__ src, OperandOut O, FastParams P, int lgFT, int conj_out, float* __restrict__ init_Tsrc) {
+  extern __shared__ float2 smem[];
+  constexpr int TS = Geo<HF>::TS;
+  const int FT = 1 << lgFT, r = blockIdx.y, f0 = blockIdx.x * FT;
+  const int nf = min(FT, P.nfoc - f0), nt = P.nt;
+  const Who me = who<HF>();
+  if (me.tl < nf) {
+    float2 a[32];
+    const size_t base = ((size_t)(f0 + me.tl) * P.n + r) * nt;
+    load_time<HF>(a, src + base, me);
+    if (init_Tsrc) {  // f1plus = N_{-1} = T G_d   [PAPER.md:19, 67, 74]
+      float* dst = init_Tsrc + base;
+#pragma unroll
+      for (int q = 0; q < 32; ++q) {
+        const int j = sample_j<HF>(q, me.t, me.hf);
+        dst[(nt - j) & (nt - 1)] = a[q].x;
+        dst[nt - j - 1] = a[q].y;
+      }
+    }
+    float2* zt = smem + me.tl * TS;
+    warp_fft1024<false>(a, zt + me.hf * SUB, P.tw1k, me.t);
+    store_Z<HF>(a, zt, me.hf, me.t, P.tw);
+  }
+  __syncthreads();
+  band_out<HF>(smem, nf, lgFT, P, [&](int tl, int kk, float2 X) {
+    if (conj_out) X.y = -X.y;  // spectrum of the time-reversed real trace
+    store_operand(O, P.ld, kk, r, f0 + tl, X);
+  });
+}
+
+// ------------------------------------------------------------------------------------------------ k_inv_fast
+// grid (ceil(nfoc / FT), n); spec: [n][nb][ldf]; out[j] = sS*S[j] + sA*A[j] + sB*B[(nt-j)%nt]              (a3, a7)
+template <int HF>
+__global__ void __launch_bounds__(256 * HF, 2 / HF)
+k_inv_fast(const float2* __restrict__ spec, FastParams P, int lgFT, float* __restrict__ out, float sS,
+           const float* __restrict__ A, float sA, const float* __restrict__ B, float sB) {
+  extern __shared__ float2 smem[];
+  constexpr int TS = Geo<HF>::TS;
+  const int FT = 1 << lgFT, r = blockIdx.y, f0 = blockIdx.x * FT;
+  const int nf = min(FT, P.nfoc - f0), nt = P.nt;
+  const float2* srow = spec + (size_t)r * P.nb * P.ldf + f0;
+  spectrum_in<HF>(
+      smem, nf, lgFT, false, P, [&](int tl, int kk, float2&) { return __ldg(srow + (size_t)kk * P.ldf + tl); },
+      [](int, int, float2, float2) {});
+  __syncthreads();
+  const Who me = who<HF>();
+  if (me.tl >= nf) return;
+  float2* zt = smem + me.tl * TS;
+  float2 a[32];
+  load_Z<HF>(a, zt, me.hf, me.t, P.tw);
+  trace_sync<HF>(me.tl);
+  warp_fft1024<true>(a, zt + me.hf * SUB, P.tw1k, me.t);
+  const size_t base = ((size_t)(f0 + me.tl) * P.n + r) * nt;
+#pragma unroll
+  for (int q = 0; q < 32; ++q) {
+    const int j = sample_j<HF>(q, me.t, me.hf);
+    float2 v = make_float2(sS * a[q].x, sS * a[q].y);
+    if (A) {
+      const float2 av = __ldg(reinterpret_cast<const float2*>(A + base + j));
+      v.x += sA * av.x;
+      v.y += sA * av.y;
+    }
+    if (B) {
+      v.x += sB * __ldg(B + base + ((nt - j) & (nt - 1)));
+      v.y += sB * __ldg(B + base + (nt - j - 1));
+    }
+    *reinterpret_cast<float2*>(out + base + j) = v;
+  }
+}
+
+// ------------------------------------------------------------------------------------------------ k_post_fast
+// grid (ceil(nfoc / FT), n).  Shat, phat: [n][nb][ldf]; operand out: see store_operand; h: [nfoc][n];
+// f1plus / f1min: [nfoc][n][nt].  One Neumann step after the contraction (a3..a6):
+//   i even:  v = S (plain inverse transform);   w = Theta v;  f1min += w;   N_i = -T w  =>  N^_i = -conj(FFT w)
+//   i odd:   u = T S (inverse of conj S^);      w = Theta u;  f1plus -= w;  N_i = -w    =>  N^_i = -FFT w
+// (Theta is symmetric in +-t, so Theta T = T Theta; w is real, so FFT(T w) = conj FFT(w).)  Every global access of
+// the time fields is a natural-order float2 row; only the optional N_i copy of an even step is written reversed.
+template <int HF>
+__global__ void __launch_bounds__(256 * HF, 2 / HF)
+k_post_fast(const float2* __restrict__ Shat, float2* __restrict__ phat, OperandOut O, const int* __restrict__ h,
+            float* __restrict__ f1plus, float* __restrict__ f1min, FastParams P, int lgFT, int parity_even,
+            float* __restrict__ Ni_out) {
+  extern __shared__ float2 smem[];
+  constexpr int TS = Geo<HF>::TS;
+  const int FT = 1 << lgFT, r = blockIdx.y, f0 = blockIdx.x * FT;
+  const int nf = min(FT, P.nfoc - f0), nt = P.nt;
+  const size_t rowoff = (size_t)r * P.nb * P.ldf + f0;
+  // a3: p^ += S^   [PAPER.md:79]
+  spectrum_in<HF>(
+      smem, nf, lgFT, parity_even == 0, P,
+      [&](int tl, int kk, float2& pv) {
+        const size_t o = rowoff + (size_t)kk * P.ldf + tl;
+        pv = phat[o];
+        return __ldg(Shat + o);
+      },
+      [&](int tl, int kk, float2 s, float2 pv) { phat[rowoff + (size_t)kk * P.ldf + tl] = make_float2(pv.x + s.x, pv.y + s.y); });
+  __syncthreads();
+  const Who me = who<HF>();
+  if (me.tl < nf) {
+    float2* zt = smem + me.tl * TS;
+    float2 a[32];
+    load_Z<HF>(a, zt, me.hf, me.t, P.tw);
+    trace_sync<HF>(me.tl);
+    warp_fft1024<true>(a, zt + me.hf * SUB, P.tw1k, me.t);
+    const int hh = __ldg(h + (size_t)(f0 + me.tl) * P.n + r);
+    const size_t base = ((size_t)(f0 + me.tl) * P.n + r) * nt;
+    float* acc = (parity_even ? f1min : f1plus) + base;
+    const float sg = parity_even ? 1.f : -1.f;
+    // a4 + a5.  Theta[j] = 1 iff j < h or j > nt - h (hard 0/1 window, strict inequality; G2).  A register row q of
+    // the warp covers samples [jlo, jlo + 64 HF - 2 HF + 1]; rows that miss the window touch no memory.
+#pragma unroll
+    for (int q0 = 0; q0 < 32; q0 += 8) {
+      float2 c[8];
+#pragma unroll
+      for (int u = 0; u < 8; ++u) {
+        const int q = q0 + u;
+        const int jlo = sample_j<HF>(q, 0, me.hf), jhi = sample_j<HF>(q, 31, me.hf) + 1;
+        c[u] = make_float2(0.f, 0.f);
+        if (jlo < hh || jhi > nt - hh) c[u] = *reinterpret_cast<const float2*>(acc + sample_j<HF>(q, me.t, me.hf));
+      }
+#pragma unroll
+      for (int u = 0; u < 8; ++u) {
+        const int q = q0 + u;
+        const int jlo = sample_j<HF>(q, 0, me.hf), jhi = sample_j<HF>(q, 31, me.hf) + 1;
+        if (jlo < hh || jhi > nt - hh) {
+          const int j = sample_j<HF>(q, me.t, me.hf);
+          const float wx = (j < hh || j > nt - hh) ? a[q].x : 0.f;
+          const float wy = (j + 1 < hh || j + 1 > nt - hh) ? a[q].y : 0.f;
+          a[q] = make_float2(wx, wy);
+          *reinterpret_cast<float2*>(acc + j) = make_float2(c[u].x + sg * wx, c[u].y + sg * wy);
+        } else {
+          a[q] = make_float2(0.f, 0.f);
+        }
+      }
+    }
+    if (Ni_out) {  // test / N_last copy of the new iterate
+      float* ni = Ni_out + base;
+#pragma unroll
+      for (int q = 0; q < 32; ++q) {
+        const int j = sample_j<HF>(q, me.t, me.hf);
+        if (parity_even) {  // N_i[j'] = -w[(nt - j') % nt]
+          ni[(nt - j) & (nt - 1)] = -a[q].x;
+          ni[nt - j - 1] = -a[q].y;
+        } else {
+          *reinterpret_cast<float2*>(ni + j) = make_float2(-a[q].x, -a[q].y);
+        }
+      }
+    }
+    warp_fft1024<false>(a, zt + me.hf * SUB, P.tw1k, me.t);  // a6
+    store_Z<HF>(a, zt, me.hf, me.t, P.tw);
+  }
+  __syncthreads();
+  band_out<HF>(smem, nf, lgFT, P, [&](int tl, int kk, float2 X) {
+    store_operand(O, P.ld, kk, r, f0 + tl, parity_even ? make_float2(-X.x, X.y) : make_float2(-X.x, -X.y));
+  });
+}
+
+// ------------------------------------------------------------------------------------------------ host side
+FastParams make_fast(const mk_ctx* c, int nfoc, int ldf) {
+  FastParams P;
+  P.tw = c->d_tw;
+  P.tw1k = c->d_tw1k;
+  P.nt = c->nt;
+  P.n = c->n;
+  P.nb = c->nb;
+  P.klo = c->klo;
+  P.ld = c->ld;
+  P.ldf = ldf;
+  P.nfoc = nfoc;
+  return P;
+}
+
+struct Shape {
+  int lg, threads;
+  size_t smem;
+};
+// FT <= 8 traces per CTA (no more slots than traces); at least 256 threads so that P1 / P5 have loads in flight
+Shape shape_for(const mk_ctx* c, int count) {
+  const int HF = c->nt / 2048;
+  int lg = 3;
+  while (lg > 0 && (1 << (lg - 1)) >= count) --lg;
+  Shape s;
+  s.lg = lg;
+  s.threads = std::max(32 * HF << lg, 256);
+  s.smem = ((size_t)(HF * SUB + 2) << lg) * sizeof(float2);
+  return s;
+}
+
+template <typename K>
+int set_smem(mk_ctx* c, K kernel, size_t bytes) {
+  return check_cuda(c, cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes), "cudaFuncSetAttribute");
+}
+
+}  // namespace
+
+bool fast_fft_ok(const mk_ctx* c) { return (c->nt == 2048 || c->nt == 4096) && c->fft_path != 1 && c->d_tw1k != nullptr; }
+
+#define MK_FAST_LAUNCH(KERN, GRID, SH, ...)                                          \
+  do {                                                                               \
+    if (c->nt == 2048) {                                                             \
+      if (int rc = set_smem(c, KERN<1>, (SH).smem)) return rc;                       \
+      KERN<1><<<GRID, (SH).threads, (SH).smem, c->stream>>>(__VA_ARGS__);            \
+    } else {                                                                         \
+      if (int rc = set_smem(c, KERN<2>, (SH).smem)) return rc;                       \
+      KERN<2><<<GRID, (SH).threads, (SH).smem, c->stream>>>(__VA_ARGS__);            \
+    }                                                                                \
+    ++c->launches;                                                                   \
+    return check_cuda(c, cudaGetLastError(), #KERN);                                 \
+  } while (0)
+
+int launch_load_R_fast(mk_ctx* c, const float* d_R_time, int shot0, int nshots) {
+  const Shape sh = shape_for(c, nshots);
+  const dim3 grid((nshots + (1 << sh.lg) - 1) >> sh.lg, c->n);
+  const float sm = (float)(c->dt * c->dx), se = (float)(c->dt * c->dx * 0.5);
+  MK_FAST_LAUNCH(k_load_R_fast, grid, sh, d_R_time, c->d_Rhat, make_fast(c, 0, 0), shot0, nshots, sh.lg, sm, se);
+}
+
+int launch_fwd_fast(mk_ctx* c, const float* d_src, const OperandOut& O, int nfoc, bool conj_out, float* d_init_Tsrc) {
+  const Shape sh = shape_for(c, nfoc);
+  const dim3 grid((nfoc + (1 << sh.lg) - 1) >> sh.lg, c->n);
+  MK_FAST_LAUNCH(k_fwd_fast, grid, sh, d_src, O, make_fast(c, nfoc, O.ldf), sh.lg, conj_out ? 1 : 0, d_init_Tsrc);
+}
+
+int launch_inv_fast(mk_ctx* c, const float2* d_spec, int nfoc, int ldf, float* d_out, float sS, const float* d_A, float sA,
+                    const float* d_B, float sB) {
+  const Shape sh = shape_for(c, nfoc);
+  const dim3 grid((nfoc + (1 << sh.lg) - 1) >> sh.lg, c->n);
+  MK_FAST_LAUNCH(k_inv_fast, grid, sh, d_spec, make_fast(c, nfoc, ldf), sh.lg, d_out, sS, d_A, sA, d_B, sB);
+}
+
+int launch_post_fast(mk_ctx* c, const OperandOut& O, int parity_even, float* d_Ni_out) {
+  const Shape sh = shape_for(c, c->nfoc);
+  const dim3 grid((c->nfoc + (1 << sh.lg) - 1) >> sh.lg, c->n);
+  MK_FAST_LAUNCH(k_post_fast, grid, sh, c->d_Shat, c->d_phat, O, c->d_h, c->d_f1plus, c->d_f1min, make_fast(c, c->nfoc, c->ldf),
+                 sh.lg, parity_even, d_Ni_out);
+}
+
+}  // namespace mk

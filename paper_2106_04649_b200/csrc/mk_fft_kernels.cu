@@ -12,7 +12,7 @@
 // when FT = 8): the FFT passes, the window and the accumulation of a trace synchronise only inside its group
 // (__syncwarp / a named barrier), so the groups drift apart and hide each other's latency; the CTA synchronises only
 // around the two phases whose thread mapping crosses traces (spectrum load, spectrum store).
-#include "mk_internal.cuh"
+#include "mk_fft_common.cuh"
 
 namespace mk {
 
@@ -163,29 +163,6 @@ __device__ __forceinline__ void spectrum_to_Z(float2* smem, int nf, int lgFT, in
       if (k2 < M && k2 != k) zt[mkfft::padi(mkfft::freq_pos(p, k2))] = mkfft::irfft_pre(y, x, tw[k2], scale);
     }
   }
-}
-
-__device__ __forceinline__ float tf32_rna(float v) {
-  unsigned u;
-  asm("cvt.rna.tf32.f32 %0, %1;" : "=r"(u) : "f"(v));
-  return __uint_as_float(u);
-}
-
-// a6 store: X = N^[k][r][f] in the layout the contraction of the active regime reads
-__device__ __forceinline__ void store_operand(const OperandOut& O, int ld, int kk, int r, int f, float2 X) {
-  if (O.bhi == nullptr) {
-    O.plain[((size_t)kk * ld + r) * O.ldf + f] = X;
-    return;
-  }
-  // regime 3 (mk_syn_tc.cu): real operand B' [nb][2 ld][ldb], rows (2r, 2r+1) = (X, iX) as interleaved floats,
-  // split into a tf32 "hi" plane and a tf32 "lo" plane (3xTF32).
-  const float hx = tf32_rna(X.x), hy = tf32_rna(X.y);
-  const float lx = tf32_rna(X.x - hx), ly = tf32_rna(X.y - hy);
-  const size_t row0 = ((size_t)kk * 2 * ld + 2 * r) * O.ldb + 2 * f;
-  *reinterpret_cast<float2*>(O.bhi + row0) = make_float2(hx, hy);
-  *reinterpret_cast<float2*>(O.bhi + row0 + O.ldb) = make_float2(-hy, hx);
-  *reinterpret_cast<float2*>(O.blo + row0) = make_float2(lx, ly);
-  *reinterpret_cast<float2*>(O.blo + row0 + O.ldb) = make_float2(-ly, lx);
 }
 
 // band of the half spectra of all FT traces (held digit-reversed in smem) -> operand; CTA-wide mapping
@@ -414,6 +391,7 @@ int launch_window(mk_ctx* c, const float* d_td, int* d_h, int ntr) {
 }
 
 int launch_load_R(mk_ctx* c, const float* d_R_time, int shot0, int nshots) {
+  if (fast_fft_ok(c)) return launch_load_R_fast(c, d_R_time, shot0, nshots);
   const int lg = pick_lgft(c, nshots), ST = 1 << lg;
   const size_t smem = trace_smem(c, lg);
   if (int rc = set_smem(c, k_load_R, smem)) return rc;
@@ -425,6 +403,7 @@ int launch_load_R(mk_ctx* c, const float* d_R_time, int shot0, int nshots) {
 }
 
 int launch_fwd(mk_ctx* c, const float* d_src, const OperandOut& O, int nfoc, bool conj_out, float* d_init_Tsrc) {
+  if (fast_fft_ok(c)) return launch_fwd_fast(c, d_src, O, nfoc, conj_out, d_init_Tsrc);
   const int lg = pick_lgft(c, nfoc), FT = 1 << lg;
   const size_t smem = trace_smem(c, lg);
   if (int rc = set_smem(c, k_fwd, smem)) return rc;
@@ -436,6 +415,7 @@ int launch_fwd(mk_ctx* c, const float* d_src, const OperandOut& O, int nfoc, boo
 
 int launch_inv(mk_ctx* c, const float2* d_spec, int nfoc, int ldf, float* d_out, float sS, const float* d_A, float sA,
                const float* d_B, float sB) {
+  if (fast_fft_ok(c)) return launch_inv_fast(c, d_spec, nfoc, ldf, d_out, sS, d_A, sA, d_B, sB);
   const int lg = pick_lgft(c, nfoc), FT = 1 << lg;
   const size_t smem = trace_smem(c, lg);
   if (int rc = set_smem(c, k_inv, smem)) return rc;
@@ -446,6 +426,7 @@ int launch_inv(mk_ctx* c, const float2* d_spec, int nfoc, int ldf, float* d_out,
 }
 
 int launch_post(mk_ctx* c, const OperandOut& O, int parity_even, float* d_Ni_out) {
+  if (fast_fft_ok(c)) return launch_post_fast(c, O, parity_even, d_Ni_out);
   const int lg = pick_lgft(c, c->nfoc), FT = 1 << lg;
   const size_t smem = trace_smem(c, lg);
   if (int rc = set_smem(c, k_post, smem)) return rc;

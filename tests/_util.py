@@ -21,7 +21,8 @@ def problem(cfg, focs=None):
     return R, Gd, td
 
 
-def gpu_chain(cfg, R, Gd, td, niter=None, regime=0, keep_iters=True, host_api=False, outputs=("f1plus", "f1min", "G", "Gplus", "Gminus")):
+def gpu_chain(cfg, R, Gd, td, niter=None, regime=0, keep_iters=True, host_api=False, outputs=("f1plus", "f1min", "G", "Gplus", "Gminus"),
+              fft_path=0):
     """Runs the CUDA path through the C ABI; returns numpy arrays like oracle.marchenko does."""
     import torch
     from paper_2106_04649_b200 import binding as B
@@ -32,6 +33,7 @@ def gpu_chain(cfg, R, Gd, td, niter=None, regime=0, keep_iters=True, host_api=Fa
     with B.Marchenko(cfg.n, cfg.n, cfg.nt, cfg.dt, cfg.dx, cfg.fmin, cfg.fmax) as mk:
         mk.set_option(B.MK_OPT_EPS_SAMPLES, cfg.eps)
         mk.set_option(B.MK_OPT_REGIME, regime)
+        mk.set_option(B.MK_OPT_FFT_PATH, fft_path)
         if host_api:
             mk.load_R_host(np.ascontiguousarray(R))
             houts = {nm: np.empty((nfoc, cfg.n, cfg.nt), np.float32) for nm in outputs + ("N_last",)}

@@ -33,7 +33,8 @@ def _check_chain(cfg, regime, niter=None, focs=None):
 
 
 # ---------------------------------------------------------------- bare synthesis
-@pytest.mark.parametrize("n,nt,nfoc,regime", [(5, 32, 3, 0), (20, 64, 1, 1), (20, 64, 12, 2), (20, 64, 12, 3)])
+@pytest.mark.parametrize("n,nt,nfoc,regime", [(5, 32, 3, 0), (20, 64, 1, 1), (20, 64, 12, 2), (20, 64, 12, 3),
+                                               (6, 2048, 3, 0), (6, 4096, 2, 0), (5, 4096, 9, 0)])   # register-resident transforms, all-pass band
 def test_delta_spike_shift(n, nt, nfoc, regime):
     import torch
     from paper_2106_04649_b200 import binding as B
@@ -59,6 +60,7 @@ def test_delta_spike_shift(n, nt, nfoc, regime):
     (37, 128, 5, 2), (150, 64, 70, 2), (130, 256, 129, 2),        # FFMA GEMM, ragged M / N tiles
     (37, 128, 5, 3), (150, 64, 70, 3), (130, 256, 129, 3), (260, 64, 140, 3),   # tcgen05 3xTF32, ragged M / N / K tiles
     (16, 16, 2, 0), (33, 4096, 9, 0),                             # smallest / longest traces
+    (24, 2048, 11, 0), (24, 2048, 1, 1), (20, 2048, 3, 1), (20, 4096, 1, 1), (18, 4096, 16, 3),   # register-resident transforms
 ])
 def test_synthesis_random_vs_oracle(n, nt, nfoc, regime):
     import torch
@@ -87,11 +89,24 @@ def test_synthesis_random_vs_oracle(n, nt, nfoc, regime):
 @pytest.mark.parametrize("k,n,nt,nfoc,regime", [
     (0, 40, 256, 1, 1), (1, 70, 512, 4, 1), (1, 70, 512, 4, 2), (2, 70, 512, 70, 2), (3, 90, 512, 19, 2),
     (4, 60, 1024, 33, 2), (2, 70, 512, 70, 3), (3, 90, 512, 19, 3), (4, 60, 1024, 33, 3),
+    # nt = 2048 / 4096: the register-resident transform kernels (mk_fft_fast.cu), ragged focal groups
+    (1, 30, 2048, 1, 1), (2, 30, 2048, 30, 2), (3, 26, 2048, 11, 3), (4, 24, 4096, 11, 2), (4, 24, 4096, 5, 1),
 ])
 def test_chain_reduced_configs(k, n, nt, nfoc, regime):
     focal = "single:400" if nfoc == 1 else ("line:300" if nfoc == n else "fan:250")
     cfg = calibrated(configs.scaled(k, n=n, nt=nt, nfoc=nfoc, focal=focal, niter=8))
     _check_chain(cfg, regime)
+
+
+def test_transform_paths_agree():
+    """MK_OPT_FFT_PATH: the generic shared-memory kernels and the register-resident ones are two implementations of
+    the same steps; both must meet the oracle (checked above) and therefore agree with each other to rounding."""
+    cfg = calibrated(configs.scaled(3, n=26, nt=2048, nfoc=11, focal="fan:250", niter=6))
+    R, Gd, td = problem(cfg)
+    a = gpu_chain(cfg, R, Gd, td, regime=2, fft_path=1)
+    b = gpu_chain(cfg, R, Gd, td, regime=2, fft_path=2)
+    for nm in FINALS + ("N_iters",):
+        assert rel_l2(a[nm], b[nm]) <= 5e-6, nm
 
 
 def test_config0_full_chain():
