@@ -136,10 +136,11 @@ __device__ __forceinline__ void spectrum_in(float2* smem, int nf, int lgFT, bool
   const float scale = 1.0f / (2.0f * (float)M);
   const int total = (half + 1) << lgFT;
   const int klo = P.klo, khi1 = P.klo + P.nb;
-  for (int i0 = threadIdx.x; i0 < total; i0 += 4 * nthr) {
-    float2 a[4], b[4], xa[4], xb[4];
+  constexpr int kBatch = 8;
+  for (int i0 = threadIdx.x; i0 < total; i0 += kBatch * nthr) {
+    float2 a[kBatch], b[kBatch], xa[kBatch], xb[kBatch];
 #pragma unroll
-    for (int u = 0; u < 4; ++u) {
+    for (int u = 0; u < kBatch; ++u) {
       const int idx = i0 + u * nthr;
       a[u] = b[u] = xa[u] = xb[u] = make_float2(0.f, 0.f);
       if (idx < total) {
@@ -151,7 +152,7 @@ __device__ __forceinline__ void spectrum_in(float2* smem, int nf, int lgFT, bool
       }
     }
 #pragma unroll
-    for (int u = 0; u < 4; ++u) {
+    for (int u = 0; u < kBatch; ++u) {
       const int idx = i0 + u * nthr;
       if (idx >= total) continue;
       const int k = idx >> lgFT, tl = idx & (FT - 1), k2 = M - k;
@@ -207,6 +208,106 @@ __device__ __forceinline__ void load_time(float2 (&a)[32], const float* __restri
   for (int q = 0; q < 32; ++q) a[q] = __ldg(reinterpret_cast<const float2*>(src + sample_j<HF>(q, me.t, me.hf)));
 }
 
+
+// ---- P1 / P5 with two focal points per thread (FT = 8, even ldf): 128-bit accesses of S^, p^ and the operand.
+// P1 needs the usual band shape 1 <= klo, khi < M/2 (no DC / Nyquist / mid bin, the mirror M - k of an in-band bin is
+// out of band): then Z[k] and Z[M-k] depend on X[k] alone,
+//   o = X tw*,  Z[k] = s (X.x - o.y, X.y + o.x),  Z[M-k] = s (X.x + o.y, o.x - X.y)      (irfft_pre with the other bin 0,
+//   tw[M-k] = -conj tw[k]), and every other Z is zero.  All loads of a thread are issued before anything is consumed.
+__device__ __forceinline__ bool simple_band(const FastParams& P, int M) { return P.klo >= 1 && P.klo + P.nb - 1 < M / 2; }
+
+template <int HF, bool RMW>
+__device__ __forceinline__ void spectrum_in_pairs(float2* smem, int nf, bool conj_in, const FastParams& P,
+                                                  const float2* __restrict__ Srow, float2* prow) {
+  constexpr int M = Geo<HF>::M, TS = Geo<HF>::TS, kBatch = 8 / HF;
+  const int nthr = blockDim.x, klo = P.klo, khi = P.klo + P.nb - 1;
+  const float scale = 1.0f / (2.0f * (float)M);
+  {  // zero fill of the out-of-band Z: k in [0, klo) u (khi, M - khi) u (M - klo, M)
+    const int n0 = klo, n1 = M - 2 * khi - 1, nz = n0 + n1 + (klo - 1);
+    for (int idx = threadIdx.x; idx < nz * 8; idx += nthr) {
+      const int tl = idx & 7, j = idx >> 3;
+      const int k = j < n0 ? j : (j < n0 + n1 ? khi + 1 + (j - n0) : M - klo + 1 + (j - n0 - n1));
+      if (tl < nf) smem[tl * TS + zaddr(k)] = make_float2(0.f, 0.f);
+    }
+  }
+  const int total = P.nb * 4;
+  for (int i0 = threadIdx.x; i0 < total; i0 += kBatch * nthr) {
+    float4 sv[kBatch], pv[kBatch];
+#pragma unroll
+    for (int u = 0; u < kBatch; ++u) {
+      const int idx = i0 + u * nthr;
+      if (idx < total && 2 * (idx & 3) < nf) {
+        const size_t o = (size_t)(idx >> 2) * P.ldf + 2 * (idx & 3);
+        sv[u] = __ldg(reinterpret_cast<const float4*>(Srow + o));
+        if (RMW) pv[u] = *reinterpret_cast<const float4*>(prow + o);
+      }
+    }
+#pragma unroll
+    for (int u = 0; u < kBatch; ++u) {
+      const int idx = i0 + u * nthr;
+      if (idx >= total) continue;
+      const int kk = idx >> 2, t0 = 2 * (idx & 3), k = klo + kk;
+      if (t0 >= nf) continue;
+      if (RMW) {
+        const size_t o = (size_t)kk * P.ldf + t0;
+        *reinterpret_cast<float4*>(prow + o) = make_float4(pv[u].x + sv[u].x, pv[u].y + sv[u].y, pv[u].z + sv[u].z, pv[u].w + sv[u].w);
+      }
+      const float2 tw = __ldg(P.tw + k);
+      const int a0 = zaddr(k), a1 = zaddr(M - k);
+#pragma unroll
+      for (int e = 0; e < 2; ++e) {
+        if (t0 + e >= nf) continue;
+        const float xr = e ? sv[u].z : sv[u].x, xi0 = e ? sv[u].w : sv[u].y;
+        const float xi = conj_in ? -xi0 : xi0;
+        const float o_r = xr * tw.x + xi * tw.y, o_i = xi * tw.x - xr * tw.y;
+        float2* zt = smem + (t0 + e) * TS;
+        zt[a0] = make_float2(scale * (xr - o_i), scale * (xi + o_r));
+        zt[a1] = make_float2(scale * (xr + o_i), scale * (o_r - xi));
+      }
+    }
+  }
+}
+
+// P5: emit2(kk, first trace t0 (even), X of t0, X of t0 + 1 (zero if that trace does not exist), whether it exists)
+template <int HF, typename Emit2>
+__device__ __forceinline__ void band_out_pairs(const float2* smem, int nf, const FastParams& P, Emit2 emit2) {
+  constexpr int TS = Geo<HF>::TS;
+  const int total = P.nb * 4;
+  for (int idx = threadIdx.x; idx < total; idx += blockDim.x) {
+    const int kk = idx >> 2, t0 = 2 * (idx & 3);
+    if (t0 >= nf) continue;
+    const float2 X0 = rfft_bin_fast<HF>(smem + t0 * TS, P.tw, P.klo + kk);
+    const float2 X1 = t0 + 1 < nf ? rfft_bin_fast<HF>(smem + (t0 + 1) * TS, P.tw, P.klo + kk) : make_float2(0.f, 0.f);
+    emit2(kk, t0, X0, X1, t0 + 1 < nf);
+  }
+}
+
+// operand store of two adjacent focal points f, f + 1 (f even, ldf even): see store_operand
+__device__ __forceinline__ void store_operand2(const OperandOut& O, int ld, int kk, int r, int f, float2 X0, float2 X1) {
+  if (O.bhi == nullptr) {
+    *reinterpret_cast<float4*>(O.plain + ((size_t)kk * ld + r) * O.ldf + f) = make_float4(X0.x, X0.y, X1.x, X1.y);
+    return;
+  }
+  const float h0x = tf32_rna(X0.x), h0y = tf32_rna(X0.y), h1x = tf32_rna(X1.x), h1y = tf32_rna(X1.y);
+  const float l0x = tf32_rna(X0.x - h0x), l0y = tf32_rna(X0.y - h0y), l1x = tf32_rna(X1.x - h1x), l1y = tf32_rna(X1.y - h1y);
+  const size_t row0 = ((size_t)kk * 2 * ld + 2 * r) * O.ldb + 2 * f;
+  *reinterpret_cast<float4*>(O.bhi + row0) = make_float4(h0x, h0y, h1x, h1y);
+  *reinterpret_cast<float4*>(O.bhi + row0 + O.ldb) = make_float4(-h0y, h0x, -h1y, h1x);
+  *reinterpret_cast<float4*>(O.blo + row0) = make_float4(l0x, l0y, l1x, l1y);
+  *reinterpret_cast<float4*>(O.blo + row0 + O.ldb) = make_float4(-l0y, l0x, -l1y, l1x);
+}
+
+// L2 prefetch of the part of a time-domain trace that meets the window (j < hh or j > nt - hh), one 128-byte line
+// per lane and step; issued at kernel start so that P3 finds the rows in L2
+template <int HF>
+__device__ __forceinline__ void prefetch_window(const float* trace, int nt, int hh, const Who& me) {
+#pragma unroll
+  for (int i = 0; i < 2; ++i) {
+    const int line = me.hf * 64 + me.t + 32 * i, j0 = 32 * line;
+    if (j0 < hh || j0 + 31 > nt - hh) asm volatile("prefetch.global.L2 [%0];" ::"l"(trace + j0));
+  }
+}
+
 // ------------------------------------------------------------------------------------------------ k_load_R_fast
 // grid (ceil(nshots / ST), nrec); Rt: [nshots][nrec][nt]                                        (a0)
 template <int HF>
@@ -226,11 +327,22 @@ k_load_R_fast(const float* __restrict__ Rt, float2* __restrict__ Rhat, FastParam
     store_Z<HF>(a, zt, me.hf, me.t, P.tw);
   }
   __syncthreads();
-  band_out<HF>(smem, ns, lgST, P, [&](int tl, int kk, float2 X) {
-    const int s = shot0 + g0 + tl;
-    const float sc = (P.n > 1 && (s == 0 || s == P.n - 1)) ? scale_end : scale_mid;
-    Rhat[((size_t)r * P.nb + kk) * P.ld + s] = make_float2(sc * X.x, sc * X.y);
-  });
+  auto weight = [&](int s) { return (P.n > 1 && (s == 0 || s == P.n - 1)) ? scale_end : scale_mid; };
+  if (lgST == 3 && ((shot0 + g0) & 1) == 0) {
+    band_out_pairs<HF>(smem, ns, P, [&](int kk, int t0, float2 X0, float2 X1, bool two) {
+      const int s = shot0 + g0 + t0;  // even
+      const float c0 = weight(s), c1 = weight(s + 1);
+      float2* dst = Rhat + ((size_t)r * P.nb + kk) * P.ld + s;
+      if (two) *reinterpret_cast<float4*>(dst) = make_float4(c0 * X0.x, c0 * X0.y, c1 * X1.x, c1 * X1.y);
+      else *dst = make_float2(c0 * X0.x, c0 * X0.y);  // column s + 1 belongs to another chunk (or is padding)
+    });
+  } else {
+    band_out<HF>(smem, ns, lgST, P, [&](int tl, int kk, float2 X) {
+      const int s = shot0 + g0 + tl;
+      const float sc = weight(s);
+      Rhat[((size_t)r * P.nb + kk) * P.ld + s] = make_float2(sc * X.x, sc * X.y);
+    });
+  }
 }
 
 // ------------------------------------------------------------------------------------------------ k_fwd_fast
@@ -261,10 +373,14 @@ k_fwd_fast(const float* __restrict__ src, OperandOut O, FastParams P, int lgFT, 
     store_Z<HF>(a, zt, me.hf, me.t, P.tw);
   }
   __syncthreads();
-  band_out<HF>(smem, nf, lgFT, P, [&](int tl, int kk, float2 X) {
-    if (conj_out) X.y = -X.y;  // spectrum of the time-reversed real trace
-    store_operand(O, P.ld, kk, r, f0 + tl, X);
-  });
+  const float cs = conj_out ? -1.f : 1.f;  // conj: spectrum of the time-reversed real trace
+  if (lgFT == 3 && (O.ldf & 1) == 0) {
+    band_out_pairs<HF>(smem, nf, P, [&](int kk, int t0, float2 X0, float2 X1, bool) {
+      store_operand2(O, P.ld, kk, r, f0 + t0, make_float2(X0.x, cs * X0.y), make_float2(X1.x, cs * X1.y));
+    });
+  } else {
+    band_out<HF>(smem, nf, lgFT, P, [&](int tl, int kk, float2 X) { store_operand(O, P.ld, kk, r, f0 + tl, make_float2(X.x, cs * X.y)); });
+  }
 }
 
 // ------------------------------------------------------------------------------------------------ k_inv_fast
@@ -278,9 +394,13 @@ k_inv_fast(const float2* __restrict__ spec, FastParams P, int lgFT, float* __res
   const int FT = 1 << lgFT, r = blockIdx.y, f0 = blockIdx.x * FT;
   const int nf = min(FT, P.nfoc - f0), nt = P.nt;
   const float2* srow = spec + (size_t)r * P.nb * P.ldf + f0;
-  spectrum_in<HF>(
-      smem, nf, lgFT, false, P, [&](int tl, int kk, float2&) { return __ldg(srow + (size_t)kk * P.ldf + tl); },
-      [](int, int, float2, float2) {});
+  if (lgFT == 3 && (P.ldf & 1) == 0 && simple_band(P, Geo<HF>::M)) {
+    spectrum_in_pairs<HF, false>(smem, nf, false, P, srow, nullptr);
+  } else {
+    spectrum_in<HF>(
+        smem, nf, lgFT, false, P, [&](int tl, int kk, float2&) { return __ldg(srow + (size_t)kk * P.ldf + tl); },
+        [](int, int, float2, float2) {});
+  }
   __syncthreads();
   const Who me = who<HF>();
   if (me.tl >= nf) return;
@@ -324,24 +444,33 @@ k_post_fast(const float2* __restrict__ Shat, float2* __restrict__ phat, OperandO
   const int FT = 1 << lgFT, r = blockIdx.y, f0 = blockIdx.x * FT;
   const int nf = min(FT, P.nfoc - f0), nt = P.nt;
   const size_t rowoff = (size_t)r * P.nb * P.ldf + f0;
-  // a3: p^ += S^   [PAPER.md:79]
-  spectrum_in<HF>(
-      smem, nf, lgFT, parity_even == 0, P,
-      [&](int tl, int kk, float2& pv) {
-        const size_t o = rowoff + (size_t)kk * P.ldf + tl;
-        pv = phat[o];
-        return __ldg(Shat + o);
-      },
-      [&](int tl, int kk, float2 s, float2 pv) { phat[rowoff + (size_t)kk * P.ldf + tl] = make_float2(pv.x + s.x, pv.y + s.y); });
-  __syncthreads();
   const Who me = who<HF>();
+  const bool pairs = lgFT == 3 && (P.ldf & 1) == 0;
+  int hh = 0;
+  if (me.tl < nf) {  // the accumulator rows that P3 will touch: on their way to L2 while P1 / P2 run
+    hh = __ldg(h + (size_t)(f0 + me.tl) * P.n + r);
+    prefetch_window<HF>((parity_even ? f1min : f1plus) + ((size_t)(f0 + me.tl) * P.n + r) * nt, nt, hh, me);
+  }
+  // a3: p^ += S^   [PAPER.md:79]
+  if (pairs && simple_band(P, Geo<HF>::M)) {
+    spectrum_in_pairs<HF, true>(smem, nf, parity_even == 0, P, Shat + rowoff, phat + rowoff);
+  } else {
+    spectrum_in<HF>(
+        smem, nf, lgFT, parity_even == 0, P,
+        [&](int tl, int kk, float2& pv) {
+          const size_t o = rowoff + (size_t)kk * P.ldf + tl;
+          pv = phat[o];
+          return __ldg(Shat + o);
+        },
+        [&](int tl, int kk, float2 s, float2 pv) { phat[rowoff + (size_t)kk * P.ldf + tl] = make_float2(pv.x + s.x, pv.y + s.y); });
+  }
+  __syncthreads();
   if (me.tl < nf) {
     float2* zt = smem + me.tl * TS;
     float2 a[32];
     load_Z<HF>(a, zt, me.hf, me.t, P.tw);
     trace_sync<HF>(me.tl);
     warp_fft1024<true>(a, zt + me.hf * SUB, P.tw1k, me.t);
-    const int hh = __ldg(h + (size_t)(f0 + me.tl) * P.n + r);
     const size_t base = ((size_t)(f0 + me.tl) * P.n + r) * nt;
     float* acc = (parity_even ? f1min : f1plus) + base;
     const float sg = parity_even ? 1.f : -1.f;
@@ -389,9 +518,14 @@ k_post_fast(const float2* __restrict__ Shat, float2* __restrict__ phat, OperandO
     store_Z<HF>(a, zt, me.hf, me.t, P.tw);
   }
   __syncthreads();
-  band_out<HF>(smem, nf, lgFT, P, [&](int tl, int kk, float2 X) {
-    store_operand(O, P.ld, kk, r, f0 + tl, parity_even ? make_float2(-X.x, X.y) : make_float2(-X.x, -X.y));
-  });
+  const float cs = parity_even ? 1.f : -1.f;
+  if (pairs) {
+    band_out_pairs<HF>(smem, nf, P, [&](int kk, int t0, float2 X0, float2 X1, bool) {
+      store_operand2(O, P.ld, kk, r, f0 + t0, make_float2(-X0.x, cs * X0.y), make_float2(-X1.x, cs * X1.y));
+    });
+  } else {
+    band_out<HF>(smem, nf, lgFT, P, [&](int tl, int kk, float2 X) { store_operand(O, P.ld, kk, r, f0 + tl, make_float2(-X.x, cs * X.y)); });
+  }
 }
 
 // ------------------------------------------------------------------------------------------------ host side
@@ -413,14 +547,16 @@ struct Shape {
   int lg, threads;
   size_t smem;
 };
-// FT <= 8 traces per CTA (no more slots than traces); at least 256 threads so that P1 / P5 have loads in flight
+// FT <= 8 traces per CTA (no more slots than traces), 32 HF threads per trace, at least 64 threads: with a single focal
+// point the 2-warp CTAs of all receivers are resident at once (8 per SM at 128 registers) and the second warp shares
+// the CTA-wide phases P1 / P5.  Measured on config 1 (601 traces per launch): 256 threads 29 us (3 waves), 32 threads 40 us
 Shape shape_for(const mk_ctx* c, int count) {
   const int HF = c->nt / 2048;
   int lg = 3;
   while (lg > 0 && (1 << (lg - 1)) >= count) --lg;
   Shape s;
   s.lg = lg;
-  s.threads = std::max(32 * HF << lg, 256);
+  s.threads = std::max(32 * HF << lg, 64);
   s.smem = ((size_t)(HF * SUB + 2) << lg) * sizeof(float2);
   return s;
 }

@@ -13,8 +13,14 @@ namespace {
 
 constexpr int kThreads = 256;
 constexpr int kWarps = kThreads / 32;
-constexpr int kRows = 4;                         // rows of R^ a warp streams at once (x reuse + loads in flight)
-constexpr int kRowsPerCta = kWarps * kRows * 2;  // 64 receivers per CTA
+constexpr int kRowsPerCta = 64;  // receivers per CTA
+// Rows of R^ a warp streams at once (x reuse, independent load streams), unroll of the chunk loop (loads in flight per
+// stream) and CTAs per SM.  Measured on B200, config 1 (nfoc = 1, 1.30 GB of R^): (4, 2, 3) 6.81 TB/s, (4, 1, 4) 7.00,
+// (2, 4, 4) 7.03; a pure read of the same bytes peaks at 7.70 TB/s.
+template <int NFOC>
+struct Tune {
+  static constexpr int kRows = NFOC == 1 ? 2 : 4, kUnroll = NFOC == 1 ? 4 : 2, kMinBlocks = NFOC == 1 ? 4 : (NFOC <= 2 ? 3 : 1);
+};
 
 struct f8 {
   float v[8];
@@ -37,7 +43,7 @@ __device__ __forceinline__ void cfma(float2& acc, float ar, float ai, float2 b) 
 
 // grid (nb, ceil(n / kRowsPerCta)).  Rhat [n][nb][ld], Nhat [nb][ld][NFOC], Shat [n][nb][NFOC].
 template <int NFOC>
-__global__ void __launch_bounds__(kThreads) k_syn_gemv(const float2* __restrict__ Rhat, const float2* __restrict__ Nhat,
+__global__ void __launch_bounds__(kThreads, Tune<NFOC>::kMinBlocks) k_syn_gemv(const float2* __restrict__ Rhat, const float2* __restrict__ Nhat,
                                                        float2* __restrict__ Shat, int n, int nb, int ld) {
   extern __shared__ float4 smem4[];
   float2* x = reinterpret_cast<float2*>(smem4);  // [ld][NFOC]
@@ -50,6 +56,7 @@ __global__ void __launch_bounds__(kThreads) k_syn_gemv(const float2* __restrict_
     for (int i = threadIdx.x; i < nvec; i += kThreads) smem4[i] = __ldg(src + i);
   }
   __syncthreads();
+  constexpr int kRows = Tune<NFOC>::kRows;
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int nchunk = ld >> 2;  // 256-bit chunk = 4 complex (ld is a multiple of 16)
   for (int r0 = r_begin + warp * kRows; r0 < r_end; r0 += kWarps * kRows) {
@@ -64,7 +71,7 @@ __global__ void __launch_bounds__(kThreads) k_syn_gemv(const float2* __restrict_
     for (int i = 0; i < kRows; ++i)
 #pragma unroll
       for (int f = 0; f < NFOC; ++f) acc[i][f] = make_float2(0.f, 0.f);
-#pragma unroll 2
+#pragma unroll Tune<NFOC>::kUnroll
     for (int c = lane; c < nchunk; c += 32) {
       f8 a[kRows];
 #pragma unroll
