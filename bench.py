@@ -279,13 +279,26 @@ def run_ours(args):
                 "frac_of_nominal_8TBps": ach / 8000.0, "launches_timed": int(syn_n), "avg_launch_ms": avg_ms,
                 "share_of_step": syn_ms / ms_total}
     else:
-        flops = 8.0 * nfoc * cfg.n * cfg.n * nb
+        flops = 8.0 * nfoc * cfg.n * cfg.n * nb        # algorithmic: one complex MAC (8 flops) per element of R^ and focal point
         ach = flops / (avg_ms * 1e-3) / 1e12
         sm_max = clocks.get("sm_max_mhz") or 1965.0
-        peak = 2 * 128 * 148 * sm_max * 1e6 / 1e12     # FFMA lanes x SMs x max clock
-        roof = {"bound": "alu", "kernel": "k_syn_gemm_ffma", "achieved": ach, "peak": peak, "unit": "TFLOP/s", "frac": ach / peak,
-                "traffic": traffic, "peak_source": "2 x 128 FFMA lanes x 148 SMs x clocks.max.sm (guide unit counts)",
-                "launches_timed": int(syn_n), "avg_launch_ms": avg_ms, "share_of_step": syn_ms / ms_total}
+        ffma_peak = 2 * 128 * 148 * sm_max * 1e6 / 1e12     # FFMA lanes x SMs x max clock
+        if regime_used == 2:
+            roof = {"bound": "alu", "kernel": "k_syn_gemm_ffma", "achieved": ach, "peak": ffma_peak, "unit": "TFLOP/s",
+                    "frac": ach / ffma_peak, "traffic": traffic,
+                    "peak_source": "2 x 128 FFMA lanes x 148 SMs x clocks.max.sm (guide unit counts)",
+                    "launches_timed": int(syn_n), "avg_launch_ms": avg_ms, "share_of_step": syn_ms / ms_total}
+        else:
+            # 3xTF32: every algorithmic flop costs three tf32 tensor flops.  Peak for this dtype = measured bf16 peak
+            # (sustained figure: the kernel is timed inside a long step) x 1/2 (nominal tf32 : bf16), / 3 for the split.
+            tf32_peak = 0.5 * peaks["bf16_tflops_sustained"]
+            roof = {"bound": "tensor", "kernel": "k_syn_gemm_tf32x3", "achieved": ach, "peak": tf32_peak / 3.0, "unit": "TFLOP/s",
+                    "frac": ach / (tf32_peak / 3.0), "traffic": traffic,
+                    "peak_source": peaks["source"] + " bf16 sustained x 0.5 (nominal tf32:bf16) / 3 (3xTF32 split); "
+                                   "achieved counts algorithmic fp32 flops (8 per complex MAC)",
+                    "tensor_tflops_issued": 3.0 * ach, "tf32_peak": tf32_peak,
+                    "frac_of_fp32_ffma_roofline": ach / ffma_peak,
+                    "launches_timed": int(syn_n), "avg_launch_ms": avg_ms, "share_of_step": syn_ms / ms_total}
 
     # ---- the oracle as it stands, on this box's host cores, bounded sample (rank 0, N = 1 only)
     cpu = None

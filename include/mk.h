@@ -48,8 +48,9 @@ enum {
 /* mk_set_option keys */
 enum {
   MK_OPT_EPS_SAMPLES = 1, /* window margin eps in samples (default 8; BASELINE.json config 0; G2) */
-  MK_OPT_REGIME = 2,      /* contraction kernel: 0 auto (default), 1 streaming GEMV, 2 FP32-FFMA GEMM,
-                             3 tcgen05 3xTF32 GEMM (only where available; MK_ERR_INVALID_ARG otherwise) */
+  MK_OPT_REGIME = 2,      /* contraction kernel: 0 auto (default: 1 for nfoc <= 8, else 3), 1 streaming GEMV,
+                             2 FP32-FFMA GEMM, 3 tcgen05 3xTF32 GEMM with chunked fp32 accumulation (sm_100 only;
+                             MK_ERR_INVALID_ARG otherwise) */
   MK_OPT_TIMING = 3,      /* 1: bracket every contraction launch with CUDA events on the context's stream */
   MK_OPT_FFT_PATH = 4     /* transform kernels: 0 auto (default), 1 generic shared-memory passes (any nt),
                              2 register-resident path (nt = 2048 or 4096 only; MK_ERR_INVALID_ARG otherwise) */

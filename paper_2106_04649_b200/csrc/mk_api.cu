@@ -62,7 +62,7 @@ void release(mk_ctx* c, T** p, size_t* cap) {
 
 int resolve_regime(mk_ctx* c, int nfoc, int* regime) {
   int r = c->regime;
-  if (r == 0) r = gemv_supported(c, nfoc) ? 1 : 2;
+  if (r == 0) r = gemv_supported(c, nfoc) ? 1 : (tc_supported(c) ? 3 : 2);
   if (r == 1 && !gemv_supported(c, nfoc)) return set_err(c, MK_ERR_INVALID_ARG, "GEMV regime needs nfoc <= 8 and ld*nfoc*8 <= 96 KiB");
   if (r < 1 || r > 3) return set_err(c, MK_ERR_INVALID_ARG, "unknown regime");
   if (r == 3 && !tc_supported(c)) return set_err(c, MK_ERR_INVALID_ARG, "tcgen05 3xTF32 regime needs an sm_100 device");

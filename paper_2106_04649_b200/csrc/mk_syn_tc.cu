@@ -12,13 +12,22 @@
 // shared-memory tile); every k'-chunk issues  Alo*Bhi + Ahi*Blo + Ahi*Bhi  into one fp32 accumulator in TMEM.  The dropped
 // term Alo*Blo is O(2^-20) relative.
 //
-// Kernel: persistent, one CTA per SM, warp-specialised —
-//   warp 0     TMA producer: A' tile [128 rows][16 floats] (SWIZZLE_64B, K-major) and the two B' tiles
-//              [16 k'][256 floats] (SWIZZLE_128B with 32-byte atoms, MN-major) per stage, 4 stages, mbarrier full/empty ring
-//   warp 1     tcgen05.mma issuer (one thread): kind::tf32, M = 128, N <= 256, K = 8; accumulators double-buffered in
-//              TMEM (2 x 256 columns); tcgen05.commit releases the stage / publishes the accumulator
-//   warps 2-5  split warps: Alo tile of the stage
-//   warps 6-9  epilogue: tcgen05.ld 32x32b -> registers -> 128-bit global stores of S^
+// Accumulation.  The tensor core adds into its fp32 accumulator with TRUNCATION, not round-to-nearest: measured on B200
+// with one accumulator over the whole K extent the relative error of S^ grows linearly with the number of MMA steps
+// (about 2e-8 per step: 6.8e-7 at n = 32, 2.9e-5 at n = 2048, against 1.2e-6 for the FFMA kernel), which breaks the
+// 2e-5 per-iteration tolerance from n ~ 600 on.  So K is cut into CHUNKS of kChunkKb k'-blocks (24 MMA steps): every
+// chunk starts a fresh TMEM accumulator, and the epilogue warps add the finished chunk into fp32 registers
+// (round-to-nearest) while the tensor core works on the next chunk in the other TMEM buffer.  The error is then that
+// of one chunk (~5e-7), independent of n.
+//
+// Kernel: persistent, one CTA per SM, warp-specialised, 384 threads —
+//   warp 0      TMA producer: A' tile [128 rows][16 floats] (SWIZZLE_64B, K-major) and the two B' tiles
+//               [16 k'][256 floats] (SWIZZLE_128B with 32-byte atoms, MN-major) per stage, 4 stages, mbarrier full/empty ring
+//   warp 1      tcgen05.mma issuer (one thread): kind::tf32, M = 128, N <= 256, K = 8; chunk accumulators double-buffered
+//               in TMEM (2 x 256 columns); tcgen05.commit releases the stage / publishes the chunk
+//   warps 2-3   split warps: Alo tile of the stage
+//   warps 4-11  epilogue: warp w owns TMEM lanes 32 (w % 4) .. +31 and the column half (w - 4) / 4; per chunk
+//               tcgen05.ld 32x32b -> += 128 running sums in registers; per tile 128-bit global stores of S^
 #include <cuda.h>
 
 #include "mk_internal.cuh"
@@ -32,7 +41,9 @@ constexpr int BN = 256;        // real columns (2 per focal point) per tile = TM
 constexpr int BK = 16;         // k' (floats of the interleaved shot dimension) per stage: 64-byte rows of A'
 constexpr int UK = 8;          // k' per tcgen05.mma (kind::tf32)
 constexpr int STAGES = 4;
-constexpr int kThreads = 320;  // 10 warps
+constexpr int kThreads = 384;  // 12 warps
+constexpr int kChunkKb = 4;    // k'-blocks per accumulation chunk (24 MMA steps)
+constexpr int kSplitThreads = 64, kEpiWarps = 8;
 constexpr uint32_t A_BYTES = BM * BK * 4;   // 8 KB
 constexpr uint32_t B_BYTES = BK * BN * 4;   // 16 KB
 constexpr uint32_t STAGE_BYTES = 2 * A_BYTES + 2 * B_BYTES;  // A raw, A lo, B hi, B lo = 48 KB
@@ -82,43 +93,23 @@ __device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::
 __device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
 
 __device__ __forceinline__ void umma_tf32(uint32_t tmem_d, uint64_t adesc, uint64_t bdesc, uint32_t idesc, uint32_t accumulate) {
-#if defined(TC_VARIANT) && TC_VARIANT == 1
-  const uint32_t z = 0;
-  asm volatile(
-      "{\n\t.reg .pred p;\n\t"
-      "setp.ne.b32 p, %4, 0;\n\t"
-      "tcgen05.mma.cta_group::1.kind::tf32 [%0], %1, %2, %3, {%5, %5, %5, %5}, p;\n\t}" ::"r"(tmem_d),
-      "l"(adesc), "l"(bdesc), "r"(idesc), "r"(accumulate), "r"(z)
-      : "memory");
-#elif defined(TC_VARIANT) && TC_VARIANT == 3
-  asm volatile(
-      "{\n\t.reg .pred p;\n\t"
-      "setp.ne.b32 p, %4, 0;\n\t"
-      "tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n\t}" ::"r"(tmem_d),
-      "l"(adesc), "l"(bdesc), "r"((idesc & ~((7u << 7) | (7u << 10))) | (1u << 7) | (1u << 10)), "r"(accumulate)
-      : "memory");
-#else
   asm volatile(
       "{\n\t.reg .pred p;\n\t"
       "setp.ne.b32 p, %4, 0;\n\t"
       "tcgen05.mma.cta_group::1.kind::tf32 [%0], %1, %2, %3, p;\n\t}" ::"r"(tmem_d),
       "l"(adesc), "l"(bdesc), "r"(idesc), "r"(accumulate)
       : "memory");
-#endif
 }
 __device__ __forceinline__ void umma_commit(uint64_t* bar) {  // arrives on `bar` when every MMA issued so far is done
   asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(smem_u32(bar)) : "memory");
 }
 
-__device__ __forceinline__ void tmem_ld32(uint32_t taddr, uint32_t* v) {
+__device__ __forceinline__ void tmem_ld16(uint32_t taddr, uint32_t* v) {
   asm volatile(
-      "tcgen05.ld.sync.aligned.32x32b.x32.b32 "
-      "{%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, "
-      "%16, %17, %18, %19, %20, %21, %22, %23, %24, %25, %26, %27, %28, %29, %30, %31}, [%32];"
+      "tcgen05.ld.sync.aligned.32x32b.x16.b32 "
+      "{%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15}, [%16];"
       : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]), "=r"(v[8]), "=r"(v[9]),
-        "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15]), "=r"(v[16]), "=r"(v[17]), "=r"(v[18]),
-        "=r"(v[19]), "=r"(v[20]), "=r"(v[21]), "=r"(v[22]), "=r"(v[23]), "=r"(v[24]), "=r"(v[25]), "=r"(v[26]), "=r"(v[27]),
-        "=r"(v[28]), "=r"(v[29]), "=r"(v[30]), "=r"(v[31])
+        "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15])
       : "r"(taddr)
       : "memory");
 }
@@ -133,17 +124,8 @@ constexpr uint32_t LAYOUT_SW128_BASE32B = 1, LAYOUT_SW64 = 4;
 // instruction descriptor, kind::tf32: D fp32, A tf32 K-major, B tf32 MN-major, M = 128, N = n
 __device__ __forceinline__ uint32_t instr_desc(uint32_t n) {
   return (1u << 4) /*D = f32*/ | (2u << 7) /*A = tf32*/ | (2u << 10) /*B = tf32*/ | (0u << 15) /*A K-major*/ |
-#if defined(TC_VARIANT) && TC_VARIANT == 2
-         (0u << 16) |
-#else
-         (1u << 16) /*B MN-major*/ |
-#endif
- ((n >> 3) << 17) | ((uint32_t)(BM >> 4) << 24);
+         (1u << 16) /*B MN-major*/ | ((n >> 3) << 17) | ((uint32_t)(BM >> 4) << 24);
 }
-
-#ifdef TC_DEBUG
-__device__ float* g_dbg = nullptr;  // bring-up only: stage 0 of the first tile (A raw 2048 floats, B hi 4096 floats)
-#endif
 
 struct TcParams {
   int n, nb, ld;        // receivers, bins, padded shots
@@ -161,8 +143,8 @@ k_syn_gemm_tf32x3(const __grid_constant__ CUtensorMap tmA, const __grid_constant
   uint64_t* full = bars;                   // [STAGES] TMA landed
   uint64_t* empty = bars + STAGES;         // [STAGES] MMAs of the stage retired
   uint64_t* split = bars + 2 * STAGES;     // [STAGES] Alo written
-  uint64_t* acc_full = bars + 3 * STAGES;  // [2]
-  uint64_t* acc_empty = acc_full + 2;      // [2]
+  uint64_t* acc_full = bars + 3 * STAGES;  // [2] chunk accumulator complete
+  uint64_t* acc_empty = acc_full + 2;      // [2] chunk accumulator drained
   uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(acc_empty + 2);
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -173,11 +155,11 @@ k_syn_gemm_tf32x3(const __grid_constant__ CUtensorMap tmA, const __grid_constant
     for (int s = 0; s < STAGES; ++s) {
       mbar_init(full + s, 1);
       mbar_init(empty + s, 1);
-      mbar_init(split + s, 4);
+      mbar_init(split + s, kSplitThreads / 32);
     }
     for (int b = 0; b < 2; ++b) {
       mbar_init(acc_full + b, 1);
-      mbar_init(acc_empty + b, 4);
+      mbar_init(acc_empty + b, kEpiWarps);
     }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
@@ -189,18 +171,6 @@ k_syn_gemm_tf32x3(const __grid_constant__ CUtensorMap tmA, const __grid_constant
   __syncthreads();
   tc_fence_after();
   const uint32_t tmem_base = *tmem_slot;
-#ifdef TC_DEBUG2
-  if (warp >= 6) {  // bring-up: preset accumulator 0, columns 0..31, to 1.0 and accumulate from the first MMA on
-    const uint32_t one = __float_as_uint(1.0f);
-    const uint32_t ta = tmem_base + ((uint32_t)((warp & 3) * 32) << 16);
-    asm volatile("tcgen05.st.sync.aligned.32x32b.x4.b32 [%0], {%1, %1, %1, %1};" ::"r"(ta), "r"(one) : "memory");
-    asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
-  }
-  tc_fence_before();
-  __syncthreads();
-  tc_fence_after();
-  if (threadIdx.x == 0 && blockIdx.x == 0) printf("tmem_base = 0x%x\n", tmem_base);
-#endif
 
   if (warp == 0) {
     // ------------------------------------------------------------------------------------ TMA producer
@@ -222,50 +192,49 @@ k_syn_gemm_tf32x3(const __grid_constant__ CUtensorMap tmA, const __grid_constant
   } else if (warp == 1) {
     // ------------------------------------------------------------------------------------ MMA issuer
     if (lane == 0) {
-      uint32_t it = 0, tile_it = 0;
-      for (int t = blockIdx.x; t < ntiles; t += gridDim.x, ++tile_it) {
+      uint32_t it = 0, chunk_it = 0;
+      for (int t = blockIdx.x; t < ntiles; t += gridDim.x) {
         const int rem = t % per_bin, ni = rem % P.ntl;
         int nmma = P.ncols - ni * BN;
         nmma = nmma > BN ? BN : ((nmma + 15) / 16) * 16;
         const uint32_t idesc = instr_desc((uint32_t)nmma);
-        const int b = tile_it & 1;
-        mbar_wait(acc_empty + b, ((tile_it >> 1) & 1) ^ 1);
-        tc_fence_after();
-        const uint32_t d = tmem_base + (uint32_t)b * BN;
-        for (int kb = 0; kb < KB; ++kb, ++it) {
-          const int s = it % STAGES;
-          const uint32_t ph = (it / STAGES) & 1;
-          mbar_wait(full + s, ph);
-          mbar_wait(split + s, ph);
+        for (int kb0 = 0; kb0 < KB; kb0 += kChunkKb, ++chunk_it) {
+          const int b = chunk_it & 1;
+          mbar_wait(acc_empty + b, ((chunk_it >> 1) & 1) ^ 1);
           tc_fence_after();
-          const uint32_t a_raw = smem_u32(smem + (size_t)s * STAGE_BYTES), a_lo = a_raw + A_BYTES;
-          const uint32_t b_hi = a_raw + 2 * A_BYTES, b_lo = b_hi + B_BYTES;
+          const uint32_t d = tmem_base + (uint32_t)b * BN;
+          const int kb1 = min(kb0 + kChunkKb, KB);
+          for (int kb = kb0; kb < kb1; ++kb, ++it) {
+            const int s = it % STAGES;
+            const uint32_t ph = (it / STAGES) & 1;
+            mbar_wait(full + s, ph);
+            mbar_wait(split + s, ph);
+            tc_fence_after();
+            const uint32_t a_raw = smem_u32(smem + (size_t)s * STAGE_BYTES), a_lo = a_raw + A_BYTES;
+            const uint32_t b_hi = a_raw + 2 * A_BYTES, b_lo = b_hi + B_BYTES;
 #pragma unroll
-          for (int j = 0; j < BK / UK; ++j) {
-            // A: K-major, 64-byte rows, SWIZZLE_64B: 8-row groups 512 B apart; a k'-chunk is 32 B further along the row
-            const uint64_t da_raw = smem_desc(a_raw + j * 32, 16, 512, LAYOUT_SW64);
-            const uint64_t da_lo = smem_desc(a_lo + j * 32, 16, 512, LAYOUT_SW64);
-            // B: MN-major tf32 must use the 128-byte swizzle with 32-byte atoms (the only MN-major layout the tensor
-            //    core takes for 32-bit operands): [8 blocks of 32 columns][16 k' rows][128 B]; LBO = 2048 (next column
-            //    block), SBO = 512 (next group of 4 k' rows); a k'-chunk of 8 rows is 1024 B further
-            const uint64_t db_hi = smem_desc(b_hi + j * 1024, 2048, 512, LAYOUT_SW128_BASE32B);
-            const uint64_t db_lo = smem_desc(b_lo + j * 1024, 2048, 512, LAYOUT_SW128_BASE32B);
-#ifdef TC_DEBUG2
-            umma_tf32(d, da_lo, db_hi, idesc, 1);
-#else
-            umma_tf32(d, da_lo, db_hi, idesc, (kb | j) != 0);  // small terms first
-#endif
-            umma_tf32(d, da_raw, db_lo, idesc, 1);
-            umma_tf32(d, da_raw, db_hi, idesc, 1);
+            for (int j = 0; j < BK / UK; ++j) {
+              // A: K-major, 64-byte rows, SWIZZLE_64B: 8-row groups 512 B apart; a k'-chunk is 32 B further along the row
+              const uint64_t da_raw = smem_desc(a_raw + j * 32, 16, 512, LAYOUT_SW64);
+              const uint64_t da_lo = smem_desc(a_lo + j * 32, 16, 512, LAYOUT_SW64);
+              // B: MN-major tf32 must use the 128-byte swizzle with 32-byte atoms (the only MN-major layout the tensor
+              //    core takes for 32-bit operands): [8 blocks of 32 columns][16 k' rows][128 B]; LBO = 2048 (next column
+              //    block), SBO = 512 (next group of 4 k' rows); a k'-chunk of 8 rows is 1024 B further
+              const uint64_t db_hi = smem_desc(b_hi + j * 1024, 2048, 512, LAYOUT_SW128_BASE32B);
+              const uint64_t db_lo = smem_desc(b_lo + j * 1024, 2048, 512, LAYOUT_SW128_BASE32B);
+              umma_tf32(d, da_lo, db_hi, idesc, (kb != kb0) || (j != 0));  // small terms first; a chunk starts from zero
+              umma_tf32(d, da_raw, db_lo, idesc, 1);
+              umma_tf32(d, da_raw, db_hi, idesc, 1);
+            }
+            umma_commit(empty + s);
           }
-          umma_commit(empty + s);
+          umma_commit(acc_full + b);
         }
-        umma_commit(acc_full + b);
       }
     }
-  } else if (warp < 6) {
+  } else if (warp < 4) {
     // ------------------------------------------------------------------------------------ split warps: Alo = A - tf32_trunc(A)
-    const int tid = threadIdx.x - 64;  // 0..127
+    const int tid = threadIdx.x - 64;  // 0..63
     uint32_t it = 0;
     for (int t = blockIdx.x; t < ntiles; t += gridDim.x) {
       for (int kb = 0; kb < KB; ++kb, ++it) {
@@ -273,23 +242,17 @@ k_syn_gemm_tf32x3(const __grid_constant__ CUtensorMap tmA, const __grid_constant
         mbar_wait(full + s, (it / STAGES) & 1);
         const float4* src = reinterpret_cast<const float4*>(smem + (size_t)s * STAGE_BYTES);
         float4* dst = reinterpret_cast<float4*>(smem + (size_t)s * STAGE_BYTES + A_BYTES);
-#ifdef TC_DEBUG
-        if (it == 0 && blockIdx.x == 0 && g_dbg) {
-          const float* a = reinterpret_cast<const float*>(smem);
-          for (int i = tid; i < 2048; i += 128) g_dbg[i] = a[i];
-          const float* bh = reinterpret_cast<const float*>(smem + 2 * A_BYTES);
-          for (int i = tid; i < 4096; i += 128) g_dbg[2048 + i] = bh[i];
-        }
-#endif
+        float4 v[(A_BYTES / 16) / kSplitThreads];
 #pragma unroll
-        for (int i = 0; i < (int)(A_BYTES / 16) / 128; ++i) {
-          const float4 v = src[tid + i * 128];
+        for (int i = 0; i < (int)(A_BYTES / 16) / kSplitThreads; ++i) v[i] = src[tid + i * kSplitThreads];
+#pragma unroll
+        for (int i = 0; i < (int)(A_BYTES / 16) / kSplitThreads; ++i) {
           float4 l;
-          l.x = v.x - __uint_as_float(__float_as_uint(v.x) & 0xffffe000u);
-          l.y = v.y - __uint_as_float(__float_as_uint(v.y) & 0xffffe000u);
-          l.z = v.z - __uint_as_float(__float_as_uint(v.z) & 0xffffe000u);
-          l.w = v.w - __uint_as_float(__float_as_uint(v.w) & 0xffffe000u);
-          dst[tid + i * 128] = l;
+          l.x = v[i].x - __uint_as_float(__float_as_uint(v[i].x) & 0xffffe000u);
+          l.y = v[i].y - __uint_as_float(__float_as_uint(v[i].y) & 0xffffe000u);
+          l.z = v[i].z - __uint_as_float(__float_as_uint(v[i].z) & 0xffffe000u);
+          l.w = v[i].w - __uint_as_float(__float_as_uint(v[i].w) & 0xffffe000u);
+          dst[tid + i * kSplitThreads] = l;
         }
         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");  // generic-proxy writes -> visible to the tensor core
         __syncwarp();
@@ -297,45 +260,43 @@ k_syn_gemm_tf32x3(const __grid_constant__ CUtensorMap tmA, const __grid_constant
       }
     }
   } else {
-    // ------------------------------------------------------------------------------------ epilogue
-    const int quad = warp & 3;  // TMEM lanes 32 quad .. 32 quad + 31 are the ones this warp may read
-    uint32_t tile_it = 0;
-    for (int t = blockIdx.x; t < ntiles; t += gridDim.x, ++tile_it) {
+    // ------------------------------------------------------------------------------------ epilogue: chunk sums in registers
+    const int quad = warp & 3;        // TMEM lanes 32 quad .. 32 quad + 31 are the ones this warp may read
+    const int half = (warp - 4) >> 2; // columns 128 half .. 128 half + 127 of the tile
+    uint32_t chunk_it = 0;
+    for (int t = blockIdx.x; t < ntiles; t += gridDim.x) {
       const int kk = t / per_bin, rem = t - kk * per_bin, mi = rem / P.ntl, ni = rem - mi * P.ntl;
-      const int b = tile_it & 1;
-      mbar_wait(acc_full + b, (tile_it >> 1) & 1);
-      tc_fence_after();
-#ifdef TC_DEBUG2
-      if (tile_it == 0 && blockIdx.x == 0 && g_dbg) {
-        for (int c = 0; c < 2; ++c) {
-          uint32_t v[32];
-          tmem_ld32(tmem_base + ((uint32_t)(quad * 32) << 16) + (uint32_t)(c * 32), v);
-          asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
-          for (int q = 0; q < 32; ++q) g_dbg[6144 + (quad * 32 + lane) * 64 + c * 32 + q] = __uint_as_float(v[q]);
-        }
-      }
-#endif
-      const int r = mi * BM + quad * 32 + lane;
-      float* dst = Shat + (size_t)r * P.s_row + (size_t)kk * P.ncols + ni * BN;
-      const int cols = P.ncols - ni * BN;  // valid columns of this tile (may exceed BN)
-#pragma unroll 1
-      for (int c = 0; c < BN / 32; ++c) {
-        if (c * 32 >= cols) break;
-        uint32_t v[32];
-        tmem_ld32(tmem_base + ((uint32_t)(quad * 32) << 16) + (uint32_t)(b * BN + c * 32), v);
-        asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
-        if (r < P.n) {
+      const int cols = P.ncols - ni * BN - half * (BN / 2);  // valid columns of this warp's half (may exceed BN / 2, may be <= 0)
+      float sum[BN / 2];
 #pragma unroll
-          for (int q = 0; q < 8; ++q)
-            if (c * 32 + q * 4 < cols)
-              *reinterpret_cast<float4*>(dst + c * 32 + q * 4) =
-                  make_float4(__uint_as_float(v[4 * q]), __uint_as_float(v[4 * q + 1]), __uint_as_float(v[4 * q + 2]),
-                              __uint_as_float(v[4 * q + 3]));
+      for (int i = 0; i < BN / 2; ++i) sum[i] = 0.f;
+      for (int kb0 = 0; kb0 < KB; kb0 += kChunkKb, ++chunk_it) {
+        const int b = chunk_it & 1;
+        mbar_wait(acc_full + b, (chunk_it >> 1) & 1);
+        tc_fence_after();
+        const uint32_t ta = tmem_base + ((uint32_t)(quad * 32) << 16) + (uint32_t)(b * BN + half * (BN / 2));
+#pragma unroll
+        for (int c = 0; c < BN / 32; ++c) {
+          if (c * 16 < cols) {  // warp-uniform; columns past the MMA's N hold stale data
+            uint32_t v[16];
+            tmem_ld16(ta + (uint32_t)(c * 16), v);
+            asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+#pragma unroll
+            for (int q = 0; q < 16; ++q) sum[c * 16 + q] += __uint_as_float(v[q]);
+          }
         }
+        tc_fence_before();
+        __syncwarp();
+        if (lane == 0) mbar_arrive(acc_empty + b);
       }
-      tc_fence_before();
-      __syncwarp();
-      if (lane == 0) mbar_arrive(acc_empty + b);
+      const int r = mi * BM + quad * 32 + lane;
+      if (r < P.n) {
+        float* dst = Shat + (size_t)r * P.s_row + (size_t)kk * P.ncols + ni * BN + half * (BN / 2);
+#pragma unroll
+        for (int q = 0; q < BN / 8; ++q)
+          if (q * 4 < cols)
+            *reinterpret_cast<float4*>(dst + q * 4) = make_float4(sum[4 * q], sum[4 * q + 1], sum[4 * q + 2], sum[4 * q + 3]);
+      }
     }
   }
 
