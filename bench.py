@@ -200,18 +200,34 @@ def run_ours(args):
     dev = torch.device("cuda", local)
 
     cfg = shard.replica_config(configs.get(args.workload), rank, world)   # weak scaling: replicas, no collective
-    R, Gd, td = workload_arrays(cfg)
     nbytes, nb = rhat_bytes(cfg)
     nfoc, niter, nsyn = cfg.nfoc, cfg.niter, nsyn_per_step(cfg)
     fields = ("N_last", "f1plus", "f1min", "G", "Gplus", "Gminus")
+    big = cfg.k >= 3            # 33 GB / 250 GB of time-domain R: generated on the device in 64-shot chunks, never on the host
 
     mk = B.Marchenko(cfg.n, cfg.n, cfg.nt, cfg.dt, cfg.dx, cfg.fmin, cfg.fmax)
     mk.set_option(B.MK_OPT_EPS_SAMPLES, cfg.eps)
     mk.set_option(B.MK_OPT_REGIME, args.regime)
-    mk.load_R_host(R)
-    dGd = torch.from_numpy(Gd).to(dev)
-    dtd = torch.from_numpy(td).to(dev)
-    douts = {nm: torch.empty((nfoc, cfg.n, cfg.nt), dtype=torch.float32, device=dev) for nm in fields}
+    if big:
+        gR = gen.DeviceR(cfg, dev)
+        for s0 in range(0, cfg.n, 64):
+            mk.load_R(gR.take(np.arange(s0, min(s0 + 64, cfg.n))), s0)
+        torch.cuda.synchronize()
+        del gR
+        torch.cuda.empty_cache()
+        dGd, dtd = gen.first_arrivals_torch(cfg, dev)
+        R = Gd = td = None
+        # 180 GB of HBM do not hold six distinct output fields of config 4 next to R^ and the accumulators: the six
+        # outputs are written one after the other into ONE buffer there (same kernels, same traffic)
+        shared = torch.empty((nfoc, cfg.n, cfg.nt), dtype=torch.float32, device=dev) if cfg.k == 4 else None
+        douts = {nm: (shared if shared is not None else torch.empty((nfoc, cfg.n, cfg.nt), dtype=torch.float32, device=dev))
+                 for nm in fields}
+    else:
+        R, Gd, td = workload_arrays(cfg)
+        mk.load_R_host(R)
+        dGd = torch.from_numpy(Gd).to(dev)
+        dtd = torch.from_numpy(td).to(dev)
+        douts = {nm: torch.empty((nfoc, cfg.n, cfg.nt), dtype=torch.float32, device=dev) for nm in fields}
 
     def barrier():
         if world > 1:
@@ -243,22 +259,25 @@ def run_ours(args):
     value = world * nsyn * nbytes * args.steps / (ms_total * 1e-3) / 1e9
 
     # ---- end-to-end through the public host API: pinned host inputs, host outputs, copies inside the timed region
-    hGd = torch.from_numpy(Gd).pin_memory()
-    htd = torch.from_numpy(td).pin_memory()
-    houts = {nm: torch.empty((nfoc, cfg.n, cfg.nt), dtype=torch.float32).pin_memory() for nm in fields}
-    e2e_steps = max(1, min(args.steps, args.e2e_steps))
-    for _ in range(min(3, args.warmup)):
-        mk.run_host(hGd, htd, niter, houts)
-    barrier()
-    t0 = time.perf_counter()
-    for _ in range(e2e_steps):
-        mk.run_host(hGd, htd, niter, houts)          # returns after the results are in host memory
-    torch.cuda.synchronize()
-    e2e_s = shard.max_over_ranks(time.perf_counter() - t0, dist)
-    barrier()
-    e2e_val = world * nsyn * nbytes * e2e_steps / e2e_s / 1e9
-    h2d = int(hGd.numel() * 4 + htd.numel() * 4)
-    d2h = int(sum(t.numel() * 4 for t in houts.values()))
+    e2e = None
+    if not big:
+        hGd = torch.from_numpy(Gd).pin_memory()
+        htd = torch.from_numpy(td).pin_memory()
+        houts = {nm: torch.empty((nfoc, cfg.n, cfg.nt), dtype=torch.float32).pin_memory() for nm in fields}
+        e2e_steps = max(1, min(args.steps, args.e2e_steps))
+        for _ in range(min(3, args.warmup)):
+            mk.run_host(hGd, htd, niter, houts)
+        barrier()
+        t0 = time.perf_counter()
+        for _ in range(e2e_steps):
+            mk.run_host(hGd, htd, niter, houts)          # returns after the results are in host memory
+        torch.cuda.synchronize()
+        e2e_s = shard.max_over_ranks(time.perf_counter() - t0, dist)
+        barrier()
+        e2e = {"value": world * nsyn * nbytes * e2e_steps / e2e_s / 1e9, "unit": UNIT,
+               "h2d_bytes_per_step": int(hGd.numel() * 4 + htd.numel() * 4),
+               "d2h_bytes_per_step": int(sum(t.numel() * 4 for t in houts.values())), "steps": e2e_steps,
+               "ms_per_step": 1e3 * e2e_s / e2e_steps, "api": "mk_run_host (pinned host G_d, t_d in; 6 host fields out)"}
 
     if rank != 0:
         if world > 1:
@@ -302,7 +321,7 @@ def run_ours(args):
 
     # ---- the oracle as it stands, on this box's host cores, bounded sample (rank 0, N = 1 only)
     cpu = None
-    if world == 1 and not args.no_cpu_baseline:
+    if world == 1 and not args.no_cpu_baseline and not big:
         import oracle
         f = [0] if nfoc > 1 else None
         t_s, nrec_s, _, _ = oracle_sample(cfg, R, Gd if f is None else Gd[f], td if f is None else td[f], budget_s=args.cpu_budget)
@@ -315,12 +334,12 @@ def run_ours(args):
             "dtype": "f32", "data": "synthetic",
             "config": {"workload": f"config{cfg.k}:{cfg.name}", "n": cfg.n, "nt": cfg.nt, "nfoc": nfoc, "niter": niter, "nb": nb,
                        "syntheses_per_step": nsyn, "rhat_bytes": nbytes, "regime": regime_used,
-                       "l2": "inputs_larger_than_L2 (R^ 1.30 GB vs 126 MB L2; no flush needed)",
+                       "l2": f"inputs_larger_than_L2 (R^ {nbytes / 1e9:.2f} GB vs 126 MB L2; no flush needed)",
+                       "input_source": "device generator, 64-shot chunks (no e2e / cpu_baseline legs)" if big else "host arrays",
                        "parallelism": "1 GPU" if world == 1 else f"{world} independent replicas (no collective)"},
             "focal_point_iterations_per_s": world * nfoc * niter * args.steps / (ms_total * 1e-3),
             "clocks": clocks,
-            "e2e": {"value": e2e_val, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h, "steps": e2e_steps,
-                    "ms_per_step": 1e3 * e2e_s / e2e_steps, "api": "mk_run_host (pinned host G_d, t_d in; 6 host fields out)"},
+            "e2e": e2e,
             "gpu_launches": launches, "roofline": roof, "cpu_baseline": cpu}
     print(json.dumps(line), flush=True)
     if world > 1:

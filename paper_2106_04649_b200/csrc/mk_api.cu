@@ -88,24 +88,37 @@ OperandOut operand_out(mk_ctx* c, int slot, int regime, int ldf, int ldb) {
   return O;
 }
 
-// allocate + zero the operand of a slot (pad rows / columns must be zero; the layout may differ from the last use)
+// allocate the operand of a slot; zero it when the buffer is new or its layout changed.  Pad rows / columns must be
+// zero and no kernel ever writes a non-zero there (the forward transforms store rows r < n, columns f < nfoc, and zeros
+// into the odd pad column of a pair), so an operand that keeps its layout needs no second memset.
 int prepare_operand(mk_ctx* c, int slot, int regime, int nfoc, int ldf, int ldb) {
+  const long long key = ((long long)regime << 56) ^ ((long long)nfoc << 32) ^ ((long long)ldf << 16) ^ (long long)ldb;
   if (regime == 3) {
     const size_t cnt = (size_t)c->nb * 2 * c->ld * ldb;
     float** hi = slot ? &c->d_Bhi2 : &c->d_Bhi;
     float** lo = slot ? &c->d_Blo2 : &c->d_Blo;
     size_t* cap = slot ? &c->cap_B2 : &c->cap_B;
+    const float* before = *hi;
     size_t cap2 = *cap;
     if (int rc = ensure(c, hi, cap, cnt, "B' hi plane")) return rc;
     if (int rc = ensure(c, lo, &cap2, cnt, "B' lo plane")) return rc;
+    if (*hi == before && c->operand_key[slot] == key) return MK_OK;
+    c->operand_key[slot] = 0;
     if (int rc = check_cuda(c, cudaMemsetAsync(*hi, 0, cnt * sizeof(float), c->stream), "memset B' hi")) return rc;
-    return check_cuda(c, cudaMemsetAsync(*lo, 0, cnt * sizeof(float), c->stream), "memset B' lo");
+    if (int rc = check_cuda(c, cudaMemsetAsync(*lo, 0, cnt * sizeof(float), c->stream), "memset B' lo")) return rc;
+    c->operand_key[slot] = key;
+    return MK_OK;
   }
   const size_t nN = (size_t)c->nb * c->ld * ldf;
   float2** p = slot ? &c->d_Nhat2 : &c->d_Nhat;
   size_t* cap = slot ? &c->cap_Nhat2 : &c->cap_Nhat;
+  const float2* before = *p;
   if (int rc = ensure(c, p, cap, nN, "Nhat")) return rc;
-  return check_cuda(c, cudaMemsetAsync(*p, 0, nN * sizeof(float2), c->stream), "memset Nhat");
+  if (*p == before && c->operand_key[slot] == key) return MK_OK;
+  c->operand_key[slot] = 0;
+  if (int rc = check_cuda(c, cudaMemsetAsync(*p, 0, nN * sizeof(float2), c->stream), "memset Nhat")) return rc;
+  c->operand_key[slot] = key;
+  return MK_OK;
 }
 
 // a2: S^ = R^ x N^ per bin, on the context's stream; optionally bracketed by events

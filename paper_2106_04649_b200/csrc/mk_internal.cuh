@@ -60,6 +60,7 @@ struct mk_ctx {
   float* d_Bhi2 = nullptr;
   float* d_Blo2 = nullptr;
   size_t cap_B2 = 0;
+  long long operand_key[2] = {0, 0};  // layout the slot's operand was last zeroed for (0 = not zeroed)
   // regime 3: cached TMA descriptors (CUtensorMap is 128 bytes, 64-byte aligned), built by mk_syn_tc.cu
   alignas(64) unsigned char tmap_A[128];
   alignas(64) unsigned char tmap_B[2][2][128];  // [main / scratch][hi / lo]
