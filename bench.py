@@ -199,15 +199,29 @@ def run_ours(args):
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     dev = torch.device("cuda", local)
 
-    cfg = shard.replica_config(configs.get(args.workload), rank, world)   # weak scaling: replicas, no collective
+    rows_mode = args.parallel == "rows"
+    # weak scaling: replicas, no collective;  --parallel rows: ONE job, R^ split by receiver rows over the ranks
+    cfg = configs.get(args.workload) if rows_mode else shard.replica_config(configs.get(args.workload), rank, world)
+    my_rows = shard.row_slice(cfg.n, rank, world) if rows_mode else range(cfg.n)
     nbytes, nb = rhat_bytes(cfg)
     nfoc, niter, nsyn = cfg.nfoc, cfg.niter, nsyn_per_step(cfg)
     fields = ("N_last", "f1plus", "f1min", "G", "Gplus", "Gminus")
     big = cfg.k >= 3            # 33 GB / 250 GB of time-domain R: generated on the device in 64-shot chunks, never on the host
 
-    mk = B.Marchenko(cfg.n, cfg.n, cfg.nt, cfg.dt, cfg.dx, cfg.fmin, cfg.fmax)
+    mk = B.Marchenko(cfg.n, cfg.n, cfg.nt, cfg.dt, cfg.dx, cfg.fmin, cfg.fmax, rows=(my_rows.start, len(my_rows)))
     mk.set_option(B.MK_OPT_EPS_SAMPLES, cfg.eps)
     mk.set_option(B.MK_OPT_REGIME, args.regime)
+    if rows_mode:
+        if world > 1:
+            exchange = shard.distributed_exchange(mk, dist)
+        else:
+            exchange = mk.operand_exchanged                 # one rank owns every row: nothing to move
+
+        def run_step():
+            shard.run_row_sharded(mk, dGd, dtd, niter, douts, exchange)
+    else:
+        def run_step():
+            mk.run(dGd, dtd, niter, douts)
     if big:
         gR = gen.DeviceR(cfg, dev)
         for s0 in range(0, cfg.n, 64):
@@ -236,7 +250,7 @@ def run_ours(args):
 
     # ---- device-timed region: inputs resident in HBM
     for _ in range(args.warmup):
-        mk.run(dGd, dtd, niter, douts)
+        run_step()
     mk.set_option(B.MK_OPT_TIMING, 1)
     mk.get_info(B.MK_INFO_SYN_RESET)
     l0 = mk.get_info(B.MK_INFO_KERNEL_LAUNCHES)
@@ -246,7 +260,7 @@ def run_ours(args):
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     e0.record()
     for _ in range(args.steps):
-        mk.run(dGd, dtd, niter, douts)
+        run_step()
     e1.record()
     barrier()
     clocks = sampler.stop()
@@ -256,11 +270,12 @@ def run_ours(args):
     syn_ms = mk.get_info(B.MK_INFO_SYN_MS_TOTAL)
     regime_used = int(mk.get_info(B.MK_INFO_REGIME_USED))
     mk.set_option(B.MK_OPT_TIMING, 0)
-    value = world * nsyn * nbytes * args.steps / (ms_total * 1e-3) / 1e9
+    jobs = 1 if rows_mode else world        # rows: the ranks share ONE job (strong scaling)
+    value = jobs * nsyn * nbytes * args.steps / (ms_total * 1e-3) / 1e9
 
     # ---- end-to-end through the public host API: pinned host inputs, host outputs, copies inside the timed region
     e2e = None
-    if not big:
+    if not big and not rows_mode:
         hGd = torch.from_numpy(Gd).pin_memory()
         htd = torch.from_numpy(td).pin_memory()
         houts = {nm: torch.empty((nfoc, cfg.n, cfg.nt), dtype=torch.float32).pin_memory() for nm in fields}
@@ -291,14 +306,15 @@ def run_ours(args):
     tp = ROOT / "profiles" / "traffic.json"
     if tp.exists():
         traffic = json.loads(tp.read_text()).get(f"config{cfg.k}_regime{regime_used}")
+    share = len(my_rows) / cfg.n            # rows mode: this rank's launches contract its own rows of R^ only
     if regime_used == 1:
-        ach = nbytes / (avg_ms * 1e-3) / 1e9
+        ach = share * nbytes / (avg_ms * 1e-3) / 1e9
         roof = {"bound": "hbm", "kernel": "k_syn_gemv", "achieved": ach, "peak": peaks["hbm_gbs"], "unit": "GB/s",
                 "frac": ach / peaks["hbm_gbs"], "traffic": traffic, "peak_source": peaks["source"] + " copy bandwidth (MEASURED_PEAKS.json)",
                 "frac_of_nominal_8TBps": ach / 8000.0, "launches_timed": int(syn_n), "avg_launch_ms": avg_ms,
                 "share_of_step": syn_ms / ms_total}
     else:
-        flops = 8.0 * nfoc * cfg.n * cfg.n * nb        # algorithmic: one complex MAC (8 flops) per element of R^ and focal point
+        flops = share * 8.0 * nfoc * cfg.n * cfg.n * nb        # algorithmic: one complex MAC (8 flops) per element of R^ and focal point
         ach = flops / (avg_ms * 1e-3) / 1e12
         sm_max = clocks.get("sm_max_mhz") or 1965.0
         ffma_peak = 2 * 128 * 148 * sm_max * 1e6 / 1e12     # FFMA lanes x SMs x max clock
@@ -330,14 +346,16 @@ def run_ours(args):
                          f"point of config {cfg.k}: {t_s:.2f} s"}
 
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
-            "ms_per_step": ms_total / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "ms_per_step": ms_total / args.steps, "higher_is_better": True, "scaling": "strong" if rows_mode else "weak", "vs_baseline": None,
             "dtype": "f32", "data": "synthetic",
             "config": {"workload": f"config{cfg.k}:{cfg.name}", "n": cfg.n, "nt": cfg.nt, "nfoc": nfoc, "niter": niter, "nb": nb,
                        "syntheses_per_step": nsyn, "rhat_bytes": nbytes, "regime": regime_used,
                        "l2": f"inputs_larger_than_L2 (R^ {nbytes / 1e9:.2f} GB vs 126 MB L2; no flush needed)",
                        "input_source": "device generator, 64-shot chunks (no e2e / cpu_baseline legs)" if big else "host arrays",
-                       "parallelism": "1 GPU" if world == 1 else f"{world} independent replicas (no collective)"},
-            "focal_point_iterations_per_s": world * nfoc * niter * args.steps / (ms_total * 1e-3),
+                       "parallelism": "1 GPU" if world == 1 and not rows_mode else
+                                      (f"{world} ranks, receiver rows sharded, all-gather of the operand rows per synthesis" if rows_mode
+                                       else f"{world} independent replicas (no collective)")},
+            "focal_point_iterations_per_s": jobs * nfoc * niter * args.steps / (ms_total * 1e-3),
             "clocks": clocks,
             "e2e": e2e,
             "gpu_launches": launches, "roofline": roof, "cpu_baseline": cpu}
@@ -356,6 +374,9 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", type=int, default=1, help="BASELINE.json config index (default 1)")
     ap.add_argument("--regime", type=int, default=0)
+    ap.add_argument("--parallel", default="replicas", choices=["replicas", "rows"],
+                    help="N > 1: independent replicas (default, weak scaling) or receiver-row sharding with one all-gather of the "
+                         "operand rows per synthesis (strong scaling; SURVEY.md section 8(e) / NEXT-3)")
     ap.add_argument("--e2e-steps", type=int, default=50)
     ap.add_argument("--cpu-budget", type=float, default=15.0, help="seconds of oracle work for cpu_baseline")
     ap.add_argument("--no-cpu-baseline", action="store_true")

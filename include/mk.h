@@ -132,6 +132,39 @@ int mk_synthesis(mk_ctx* ctx, const float* d_N_in, float* d_S_out, int nfoc);
  * d_Gminus: [nfoc][nrec][nt] fp32 as returned by mk_run / mk_finish for the current run; d_image: [nfoc] fp32. */
 int mk_image(mk_ctx* ctx, const float* d_Gminus, float* d_image);
 
+/* ---- NEXT-3: receiver-row sharding across GPUs ------------------------------------------
+ * The B200 equivalent of the paper's multi-GPU scheme (every output trace depends on one
+ * (receiver, focal point) pair): rank g owns the receiver rows row0 .. row0+nrows-1 of R^ (read-only,
+ * never moves) and computes a2..a6 for those rows; the ONE exchange step per synthesis is an all-gather of the rows
+ * of the operand N^ the ranks have just produced.  The library computes; the caller moves the rows (NCCL all-gather
+ * or peer copies) between the calls, in this order:
+ *   mk_create_sharded; mk_load_R (same full chunks on every rank: the library keeps its rows only);
+ *   mk_begin; [exchange slot 0]; niter x { mk_step; [exchange slot 0] };
+ *   for G^-, G^+: mk_finish_prepare(field); [exchange slot 1]; mk_finish_complete(field, out);  mk_finish for f1+-, G.
+ * "[exchange slot s]" = read mk_operand(ctx, s, &v), make every rank's rows of every plane identical on all ranks,
+ * then call mk_operand_exchanged(ctx, s).  A contraction on an operand whose rows were not exchanged fails with
+ * MK_ERR_STATE instead of computing on stale rows.  Time-domain fields keep their full [nfoc][nrec][nt] shape; a
+ * rank reads and writes only its own receiver rows of them (the other rows of its outputs are zero or untouched).
+ * mk_run, mk_run_host, mk_synthesis and the G^-/G^+ fields of mk_finish need the whole operand at once and return
+ * MK_ERR_STATE on a sharded context. */
+int mk_create_sharded(mk_ctx** out, int nshot, int nrec, int nt, double dt, double dx, double fmin, double fmax,
+                      int row0, int nrows);
+
+/* Where the operand of slot 0 (the run) or 1 (finals) lives.  plane[p] (p < nplanes) is a device array
+ * [nb][rows_per_bin][row_floats] fp32; receiver r occupies rows rows_per_rec * r .. rows_per_rec * (r + 1) - 1 of
+ * every bin.  (Regimes 1, 2: one plane, complex N^[k][s][f] as interleaved floats; regime 3: the tf32 hi / lo planes
+ * of the real operand, two rows per receiver.)  Valid after mk_begin (slot 0) / mk_finish_prepare (slot 1). */
+typedef struct mk_operand_view {
+  float* plane[2];
+  int nplanes, nb, rows_per_bin, rows_per_rec, row_floats, row0, nrows;
+} mk_operand_view;
+int mk_operand(mk_ctx* ctx, int slot, mk_operand_view* out);
+int mk_operand_exchanged(mk_ctx* ctx, int slot);
+
+enum { MK_FIELD_GMINUS = 1, MK_FIELD_GPLUS = 2 };
+int mk_finish_prepare(mk_ctx* ctx, int field);                   /* forward transform of f1plus / T f1min -> slot 1 */
+int mk_finish_complete(mk_ctx* ctx, int field, float* d_out);    /* contraction + inverse transform + epilogue      */
+
 const char* mk_last_error(mk_ctx* ctx);
 const char* mk_version(void);
 

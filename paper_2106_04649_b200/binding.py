@@ -22,7 +22,8 @@ REGIME_AUTO, REGIME_GEMV, REGIME_GEMM_FFMA, REGIME_GEMM_TF32X3 = 0, 1, 2, 3
 # every symbol include/mk.h declares
 SYMBOLS = ("mk_create", "mk_destroy", "mk_set_stream", "mk_set_option", "mk_get_info", "mk_load_R", "mk_load_R_host",
            "mk_run", "mk_run_host", "mk_begin", "mk_step", "mk_finish", "mk_synthesis", "mk_image", "mk_last_error",
-           "mk_version")
+           "mk_version", "mk_create_sharded", "mk_operand", "mk_operand_exchanged", "mk_finish_prepare", "mk_finish_complete")
+MK_FIELD_GMINUS, MK_FIELD_GPLUS = 1, 2
 
 
 class mk_outputs(C.Structure):
@@ -30,6 +31,11 @@ class mk_outputs(C.Structure):
 
 
 OUTPUT_FIELDS = tuple(nm for nm, _ in mk_outputs._fields_)
+
+
+class mk_operand_view(C.Structure):
+    _fields_ = [("plane", C.c_void_p * 2)] + [(nm, C.c_int) for nm in ("nplanes", "nb", "rows_per_bin", "rows_per_rec", "row_floats",
+                                                                         "row0", "nrows")]
 
 
 class MkError(RuntimeError):
@@ -65,6 +71,11 @@ def load():
     L.mk_finish.argtypes = [vp, C.POINTER(mk_outputs)]
     L.mk_synthesis.argtypes = [vp, vp, vp, ci]
     L.mk_image.argtypes = [vp, vp, vp]
+    L.mk_create_sharded.argtypes = [C.POINTER(vp), ci, ci, ci, cd, cd, cd, cd, ci, ci]
+    L.mk_operand.argtypes = [vp, ci, C.POINTER(mk_operand_view)]
+    L.mk_operand_exchanged.argtypes = [vp, ci]
+    L.mk_finish_prepare.argtypes = [vp, ci]
+    L.mk_finish_complete.argtypes = [vp, ci, vp]
     L.mk_last_error.argtypes = [vp]
     L.mk_last_error.restype = C.c_char_p
     L.mk_version.restype = C.c_char_p
@@ -110,14 +121,16 @@ def _host_ptr(a, numel=None):
 class Marchenko:
     """One context = one reflection response resident in HBM (mk_create .. mk_destroy)."""
 
-    def __init__(self, nshot, nrec, nt, dt, dx, fmin, fmax, stream=None):
+    def __init__(self, nshot, nrec, nt, dt, dx, fmin, fmax, stream=None, rows=None):
+        """rows = (row0, nrows): a row-sharded context that owns these receiver rows of R^ (mk_create_sharded)."""
         import torch
         if not torch.cuda.is_available():
             raise RuntimeError("libmk needs a CUDA device (there is no CPU fallback)")
         self._L = load()
         self._h = C.c_void_p()
         self.nshot, self.nrec, self.nt = nshot, nrec, nt
-        rc = self._L.mk_create(C.byref(self._h), nshot, nrec, nt, dt, dx, fmin, fmax)
+        self.rows = (0, nrec) if rows is None else (int(rows[0]), int(rows[1]))
+        rc = self._L.mk_create_sharded(C.byref(self._h), nshot, nrec, nt, dt, dx, fmin, fmax, self.rows[0], self.rows[1])
         if rc != MK_OK:
             msg = self._L.mk_last_error(self._h).decode() if self._h else "mk_create failed"
             if self._h:
@@ -215,6 +228,30 @@ class Marchenko:
         nfoc = d_N_in.shape[0]
         numel = nfoc * self.nrec * self.nt
         self._check(self._L.mk_synthesis(self._h, _dev_ptr(d_N_in, torch.float32, numel), _dev_ptr(d_S_out, torch.float32, numel), nfoc))
+
+    # -- row sharding
+    def operand(self, slot):
+        """Torch views (no copy) of the operand planes of `slot`, each [nb][rows_per_bin][row_floats] fp32, and the view struct."""
+        import torch
+        v = mk_operand_view()
+        self._check(self._L.mk_operand(self._h, slot, C.byref(v)))
+        planes = []
+        for p in range(v.nplanes):
+            shape = (v.nb, v.rows_per_bin, v.row_floats)
+            holder = type("_DevArray", (), {"__cuda_array_interface__": {"shape": shape, "typestr": "<f4", "data": (int(v.plane[p]), False),
+                                                                        "version": 3, "strides": None}})()
+            planes.append(torch.as_tensor(holder, device="cuda"))
+        return planes, v
+
+    def operand_exchanged(self, slot):
+        self._check(self._L.mk_operand_exchanged(self._h, slot))
+
+    def finish_prepare(self, field):
+        self._check(self._L.mk_finish_prepare(self._h, field))
+
+    def finish_complete(self, field, d_out):
+        import torch
+        self._check(self._L.mk_finish_complete(self._h, field, _dev_ptr(d_out, torch.float32, self._nfoc * self.nrec * self.nt)))
 
     def image(self, d_Gminus, d_image):
         import torch

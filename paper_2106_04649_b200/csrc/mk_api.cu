@@ -123,6 +123,8 @@ int prepare_operand(mk_ctx* c, int slot, int regime, int nfoc, int ldf, int ldb)
 
 // a2: S^ = R^ x N^ per bin, on the context's stream; optionally bracketed by events
 int contract(mk_ctx* c, int slot, float2* Shat, int nfoc, int ldf, int ldb, int regime) {
+  if (c->operand_stale[slot])
+    return set_err(c, MK_ERR_STATE, "row-sharded context: the operand rows were not exchanged (mk_operand / mk_operand_exchanged)");
   cudaEvent_t e0 = nullptr, e1 = nullptr;
   bool timed = c->timing != 0;
   if (timed && c->ev_used + 2 > c->ev.size()) {
@@ -190,9 +192,15 @@ const char* mk_version(void) { return "libmk 0.1 (sm_100a)"; }
 const char* mk_last_error(mk_ctx* ctx) { return ctx ? ctx->err.c_str() : "null context"; }
 
 int mk_create(mk_ctx** out, int nshot, int nrec, int nt, double dt, double dx, double fmin, double fmax) {
+  return mk_create_sharded(out, nshot, nrec, nt, dt, dx, fmin, fmax, 0, nrec);
+}
+
+int mk_create_sharded(mk_ctx** out, int nshot, int nrec, int nt, double dt, double dx, double fmin, double fmax, int row0,
+                      int nrows) {
   if (!out) return MK_ERR_INVALID_ARG;
   *out = nullptr;
   if (nshot <= 0 || nrec <= 0 || nshot != nrec) return MK_ERR_INVALID_ARG;
+  if (row0 < 0 || nrows <= 0 || row0 + nrows > nrec) return MK_ERR_INVALID_ARG;
   if (!is_pow2(nt) || nt < 16 || nt > 32768) return MK_ERR_INVALID_ARG;
   if (!(dt > 0.0) || !(dx > 0.0) || !(fmin >= 0.0) || !(fmax >= fmin) || fmax > 0.5 / dt * (1.0 + 1e-9)) return MK_ERR_INVALID_ARG;
   int dev = 0, ndev = 0;
@@ -204,6 +212,8 @@ int mk_create(mk_ctx** out, int nshot, int nrec, int nt, double dt, double dx, d
   if (!c) return MK_ERR_OOM;
   *out = c;  // returned even on failure so that mk_last_error can be read; the caller destroys it
   c->n = nshot;
+  c->r0 = row0;
+  c->nrow = nrows;
   c->nt = nt;
   c->dt = dt;
   c->dx = dx;
@@ -253,7 +263,7 @@ int mk_create(mk_ctx** out, int nshot, int nrec, int nt, double dt, double dx, d
   }
   {
     size_t cap = 0;
-    const size_t cnt = (size_t)nrec * c->nb * c->ld;
+    const size_t cnt = (size_t)nrows * c->nb * c->ld;  // the rows this context owns
     if (int rc = ensure(c, &c->d_Rhat, &cap, cnt, "Rhat")) return rc;
     if (int rc = check_cuda(c, cudaMemset(c->d_Rhat, 0, cnt * sizeof(float2)), "Rhat memset")) return rc;
   }
@@ -324,8 +334,8 @@ int mk_get_info(mk_ctx* c, int key, double* value) {
     case MK_INFO_NB: *value = c->nb; return MK_OK;
     case MK_INFO_KLO: *value = c->klo; return MK_OK;
     case MK_INFO_KHI: *value = c->khi; return MK_OK;
-    case MK_INFO_RHAT_BYTES: *value = 8.0 * c->n * (double)c->nb * c->n; return MK_OK;
-    case MK_INFO_RHAT_BYTES_PADDED: *value = 8.0 * c->n * (double)c->nb * c->ld; return MK_OK;
+    case MK_INFO_RHAT_BYTES: *value = 8.0 * c->nrow * (double)c->nb * c->n; return MK_OK;
+    case MK_INFO_RHAT_BYTES_PADDED: *value = 8.0 * c->nrow * (double)c->nb * c->ld; return MK_OK;
     case MK_INFO_LD_SHOT: *value = c->ld; return MK_OK;
     case MK_INFO_SHOTS_LOADED: *value = c->shots_loaded; return MK_OK;
     case MK_INFO_SYN_LAUNCHES: *value = (double)(c->ev_used / 2); return MK_OK;
@@ -408,7 +418,11 @@ int mk_begin(mk_ctx* c, const float* d_Gd, const float* d_td, int nfoc) {
   if (int rc = check_cuda(c, cudaMemsetAsync(c->d_f1min, 0, ntime * sizeof(float), c->stream), "memset f1min")) return rc;
   if (int rc = launch_window(c, d_td, c->d_h, nfoc * c->n)) return rc;
   // a1: N_{-1} = f1plus = T G_d; N^_{-1} = conj(G_d^)     [PAPER.md:19, 67, 74-75]
+  const bool sharded = c->nrow != c->n;
+  if (sharded)  // the rows of other ranks stay zero in this rank's fields
+    if (int rc = check_cuda(c, cudaMemsetAsync(c->d_f1plus, 0, ntime * sizeof(float), c->stream), "memset f1plus")) return rc;
   if (int rc = launch_fwd(c, d_Gd, operand_out(c, 0, regime, ldf, ldb), nfoc, /*conj_out=*/true, c->d_f1plus)) return rc;
+  c->operand_stale[0] = sharded;
   c->begun = true;
   return MK_OK;
 }
@@ -419,6 +433,7 @@ int mk_step(mk_ctx* c, float* d_N_i) {
   int regime = c->regime_used;
   if (int rc = contract(c, 0, c->d_Shat, c->nfoc, c->ldf, c->ldb, regime)) return rc;                               // a2  [PAPER.md:69]
   if (int rc = launch_post(c, operand_out(c, 0, regime, c->ldf, c->ldb), (c->iter % 2) == 0, d_N_i)) return rc;     // a3..a6
+  c->operand_stale[0] = c->nrow != c->n;
   ++c->iter;
   return MK_OK;
 }
@@ -440,17 +455,15 @@ int mk_finish(mk_ctx* c, const mk_outputs* o) {
     if (int rc = check_cuda(c, cudaMemcpyAsync(o->f1plus, c->d_f1plus, bytes, cudaMemcpyDeviceToDevice, c->stream), "copy f1plus")) return rc;
   if (o->f1min)
     if (int rc = check_cuda(c, cudaMemcpyAsync(o->f1min, c->d_f1min, bytes, cudaMemcpyDeviceToDevice, c->stream), "copy f1min")) return rc;
-  if (o->Gminus) {  // G^- = R f1plus - f1min   [PAPER.md:87-88; G5]
-    if (int rc = scratch_operands(c, regime, c->nfoc, c->ldf, c->ldb)) return rc;
-    if (int rc = launch_fwd(c, c->d_f1plus, operand_out(c, 1, regime, c->ldf, c->ldb), c->nfoc, false, nullptr)) return rc;
-    if (int rc = contract(c, 1, c->d_Shat2, c->nfoc, c->ldf, c->ldb, regime)) return rc;
-    if (int rc = launch_inv(c, c->d_Shat2, c->nfoc, c->ldf, o->Gminus, 1.f, c->d_f1min, -1.f, nullptr, 0.f)) return rc;
+  if ((o->Gminus || o->Gplus) && c->nrow != c->n)
+    return set_err(c, MK_ERR_STATE, "row-sharded context: G^- / G^+ need mk_finish_prepare, an exchange of slot 1, mk_finish_complete");
+  if (o->Gminus) {
+    if (int rc = mk_finish_prepare(c, MK_FIELD_GMINUS)) return rc;
+    if (int rc = mk_finish_complete(c, MK_FIELD_GMINUS, o->Gminus)) return rc;
   }
-  if (o->Gplus) {  // G^+ = T f1plus - R (T f1min)   [PAPER.md:24; G4]
-    if (int rc = scratch_operands(c, regime, c->nfoc, c->ldf, c->ldb)) return rc;
-    if (int rc = launch_fwd(c, c->d_f1min, operand_out(c, 1, regime, c->ldf, c->ldb), c->nfoc, true, nullptr)) return rc;
-    if (int rc = contract(c, 1, c->d_Shat2, c->nfoc, c->ldf, c->ldb, regime)) return rc;
-    if (int rc = launch_inv(c, c->d_Shat2, c->nfoc, c->ldf, o->Gplus, -1.f, nullptr, 0.f, c->d_f1plus, 1.f)) return rc;
+  if (o->Gplus) {
+    if (int rc = mk_finish_prepare(c, MK_FIELD_GPLUS)) return rc;
+    if (int rc = mk_finish_complete(c, MK_FIELD_GPLUS, o->Gplus)) return rc;
   }
   if (o->G) {  // G = p^- + T f2 = p^- + T f1plus - f1min   [PAPER.md:24; G3]
     if (int rc = launch_inv(c, c->d_phat, c->nfoc, c->ldf, o->G, 1.f, c->d_f1min, -1.f, c->d_f1plus, 1.f)) return rc;
@@ -458,8 +471,68 @@ int mk_finish(mk_ctx* c, const mk_outputs* o) {
   return MK_OK;
 }
 
+int mk_finish_prepare(mk_ctx* c, int field) {
+  MK_GUARD(c);
+  if (!c->begun) return set_err(c, MK_ERR_STATE, "mk_finish_prepare before mk_begin");
+  if (field != MK_FIELD_GMINUS && field != MK_FIELD_GPLUS) return set_err(c, MK_ERR_INVALID_ARG, "mk_finish_prepare: unknown field");
+  const int regime = c->regime_used;
+  if (int rc = scratch_operands(c, regime, c->nfoc, c->ldf, c->ldb)) return rc;
+  // G^- = R f1plus - f1min [PAPER.md:87-88; G5]: operand = spectrum of f1plus;  G^+ = T f1plus - R (T f1min) [PAPER.md:24; G4]:
+  // operand = spectrum of T f1min = conj of the spectrum of f1min
+  const bool minus = field == MK_FIELD_GMINUS;
+  if (int rc = launch_fwd(c, minus ? c->d_f1plus : c->d_f1min, operand_out(c, 1, regime, c->ldf, c->ldb), c->nfoc, !minus, nullptr)) return rc;
+  c->operand_stale[1] = c->nrow != c->n;
+  c->prepared_field = field;
+  return MK_OK;
+}
+
+int mk_finish_complete(mk_ctx* c, int field, float* d_out) {
+  MK_GUARD(c);
+  if (!d_out) return set_err(c, MK_ERR_INVALID_ARG, "mk_finish_complete: null output");
+  if (!c->begun || c->prepared_field != field || field == 0) return set_err(c, MK_ERR_STATE, "mk_finish_complete without the matching mk_finish_prepare");
+  const int regime = c->regime_used;
+  if (int rc = contract(c, 1, c->d_Shat2, c->nfoc, c->ldf, c->ldb, regime)) return rc;
+  c->prepared_field = 0;
+  if (field == MK_FIELD_GMINUS) return launch_inv(c, c->d_Shat2, c->nfoc, c->ldf, d_out, 1.f, c->d_f1min, -1.f, nullptr, 0.f);
+  return launch_inv(c, c->d_Shat2, c->nfoc, c->ldf, d_out, -1.f, nullptr, 0.f, c->d_f1plus, 1.f);
+}
+
+int mk_operand(mk_ctx* c, int slot, mk_operand_view* v) {
+  MK_GUARD(c);
+  if (!v || slot < 0 || slot > 1) return set_err(c, MK_ERR_INVALID_ARG, "mk_operand: bad arguments");
+  if (!c->begun) return set_err(c, MK_ERR_STATE, "mk_operand before mk_begin");
+  std::memset(v, 0, sizeof *v);
+  v->nb = c->nb;
+  v->row0 = c->r0;
+  v->nrows = c->nrow;
+  if (c->regime_used == 3) {
+    v->nplanes = 2;
+    v->plane[0] = slot ? c->d_Bhi2 : c->d_Bhi;
+    v->plane[1] = slot ? c->d_Blo2 : c->d_Blo;
+    v->rows_per_bin = 2 * c->ld;
+    v->rows_per_rec = 2;
+    v->row_floats = c->ldb;
+  } else {
+    v->nplanes = 1;
+    v->plane[0] = reinterpret_cast<float*>(slot ? c->d_Nhat2 : c->d_Nhat);
+    v->rows_per_bin = c->ld;
+    v->rows_per_rec = 1;
+    v->row_floats = 2 * c->ldf;
+  }
+  if (!v->plane[0]) return set_err(c, MK_ERR_STATE, "mk_operand: this slot has no operand yet");
+  return MK_OK;
+}
+
+int mk_operand_exchanged(mk_ctx* c, int slot) {
+  MK_GUARD(c);
+  if (slot < 0 || slot > 1) return set_err(c, MK_ERR_INVALID_ARG, "mk_operand_exchanged: bad slot");
+  c->operand_stale[slot] = false;
+  return MK_OK;
+}
+
 int mk_run(mk_ctx* c, const float* d_Gd, const float* d_td, int nfoc, int niter, const mk_outputs* o) {
   MK_GUARD(c);
+  if (c->nrow != c->n) return set_err(c, MK_ERR_STATE, "row-sharded context: drive mk_begin / mk_step / mk_finish_* with the exchanges in between");
   if (niter < 0 || !o) return set_err(c, MK_ERR_INVALID_ARG, "mk_run: bad arguments");
   if (o->N_last && niter == 0) return set_err(c, MK_ERR_INVALID_ARG, "N_last needs niter >= 1");
   if (int rc = mk_begin(c, d_Gd, d_td, nfoc)) return rc;
@@ -472,6 +545,7 @@ int mk_run(mk_ctx* c, const float* d_Gd, const float* d_td, int nfoc, int niter,
 
 int mk_run_host(mk_ctx* c, const float* h_Gd, const float* h_td, int nfoc, int niter, const mk_outputs* ho) {
   MK_GUARD(c);
+  if (c->nrow != c->n) return set_err(c, MK_ERR_STATE, "row-sharded context: mk_run_host is not available");
   if (!h_Gd || !h_td || nfoc <= 0 || niter < 0 || !ho) return set_err(c, MK_ERR_INVALID_ARG, "mk_run_host: bad arguments");
   if (ho->N_last && niter == 0) return set_err(c, MK_ERR_INVALID_ARG, "N_last needs niter >= 1");
   const size_t ntime = (size_t)nfoc * c->n * c->nt, ntd = (size_t)nfoc * c->n;
@@ -507,6 +581,7 @@ int mk_run_host(mk_ctx* c, const float* h_Gd, const float* h_td, int nfoc, int n
 
 int mk_synthesis(mk_ctx* c, const float* d_N_in, float* d_S_out, int nfoc) {
   MK_GUARD(c);
+  if (c->nrow != c->n) return set_err(c, MK_ERR_STATE, "row-sharded context: mk_synthesis is not available");
   if (!d_N_in || !d_S_out || nfoc <= 0) return set_err(c, MK_ERR_INVALID_ARG, "mk_synthesis: bad arguments");
   if (c->shots_loaded != c->n) return set_err(c, MK_ERR_STATE, "mk_synthesis before every shot of R was loaded");
   int regime = 0;

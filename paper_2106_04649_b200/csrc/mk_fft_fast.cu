@@ -45,6 +45,7 @@ struct FastParams {
   const float2* tw;    // [nt]      e^{-2 pi i k / nt}
   const float2* tw1k;  // [32][32]  e^{-2 pi i k1 t / 1024}
   int nt, n, nb, klo, ld, ldf, nfoc;
+  int r0;  // first receiver row of this context (row sharding): grid row b handles receiver r0 + b
 };
 
 // natural index k (0 <= k < M) of Z -> float2 offset inside the trace's shared-memory block
@@ -53,8 +54,16 @@ __device__ __forceinline__ int zaddr(int k) { return (k >> 10) * SUB + ((k & 102
 // all warps of one trace (HF = 1: the warp itself)
 template <int HF>
 __device__ __forceinline__ void trace_sync(int tl) {
-  if (HF == 1) __syncwarp();
-  else asm volatile("bar.sync %0, %1;" ::"r"(tl + 1), "r"(32 * HF) : "memory");
+  if (HF == 1) {
+    __syncwarp();
+  } else {  // named barriers 1..4 (immediate ids, so that only these are reserved); FT <= 4 when HF = 2
+    switch (tl) {
+      case 0: asm volatile("bar.sync 1, %0;" ::"n"(32 * HF) : "memory"); break;
+      case 1: asm volatile("bar.sync 2, %0;" ::"n"(32 * HF) : "memory"); break;
+      case 2: asm volatile("bar.sync 3, %0;" ::"n"(32 * HF) : "memory"); break;
+      default: asm volatile("bar.sync 4, %0;" ::"n"(32 * HF) : "memory"); break;
+    }
+  }
 }
 
 // 1024-point complex FFT by one warp.  In: lane t holds a[q] = x[t + 32 q].  Out: lane t holds a[q] = X[t + 32 q].
@@ -209,7 +218,7 @@ __device__ __forceinline__ void load_time(float2 (&a)[32], const float* __restri
 }
 
 
-// ---- P1 / P5 with two focal points per thread (FT = 8, even ldf): 128-bit accesses of S^, p^ and the operand.
+// ---- P1 / P5 with two focal points per thread (FT = 4 or 8, even ldf): 128-bit accesses of S^, p^ and the operand.
 // P1 needs the usual band shape 1 <= klo, khi < M/2 (no DC / Nyquist / mid bin, the mirror M - k of an in-band bin is
 // out of band): then Z[k] and Z[M-k] depend on X[k] alone,
 //   o = X tw*,  Z[k] = s (X.x - o.y, X.y + o.x),  Z[M-k] = s (X.x + o.y, o.x - X.y)      (irfft_pre with the other bin 0,
@@ -217,27 +226,28 @@ __device__ __forceinline__ void load_time(float2 (&a)[32], const float* __restri
 __device__ __forceinline__ bool simple_band(const FastParams& P, int M) { return P.klo >= 1 && P.klo + P.nb - 1 < M / 2; }
 
 template <int HF, bool RMW>
-__device__ __forceinline__ void spectrum_in_pairs(float2* smem, int nf, bool conj_in, const FastParams& P,
+__device__ __forceinline__ void spectrum_in_pairs(float2* smem, int nf, int lgFT, bool conj_in, const FastParams& P,
                                                   const float2* __restrict__ Srow, float2* prow) {
   constexpr int M = Geo<HF>::M, TS = Geo<HF>::TS, kBatch = 8 / HF;
   const int nthr = blockDim.x, klo = P.klo, khi = P.klo + P.nb - 1;
   const float scale = 1.0f / (2.0f * (float)M);
   {  // zero fill of the out-of-band Z: k in [0, klo) u (khi, M - khi) u (M - klo, M)
     const int n0 = klo, n1 = M - 2 * khi - 1, nz = n0 + n1 + (klo - 1);
-    for (int idx = threadIdx.x; idx < nz * 8; idx += nthr) {
-      const int tl = idx & 7, j = idx >> 3;
+    for (int idx = threadIdx.x; idx < (nz << lgFT); idx += nthr) {
+      const int tl = idx & ((1 << lgFT) - 1), j = idx >> lgFT;
       const int k = j < n0 ? j : (j < n0 + n1 ? khi + 1 + (j - n0) : M - klo + 1 + (j - n0 - n1));
       if (tl < nf) smem[tl * TS + zaddr(k)] = make_float2(0.f, 0.f);
     }
   }
-  const int total = P.nb * 4;
+  const int lgP = lgFT - 1, pm = (1 << lgP) - 1;  // focal-point pairs per bin
+  const int total = P.nb << lgP;
   for (int i0 = threadIdx.x; i0 < total; i0 += kBatch * nthr) {
     float4 sv[kBatch], pv[kBatch];
 #pragma unroll
     for (int u = 0; u < kBatch; ++u) {
       const int idx = i0 + u * nthr;
-      if (idx < total && 2 * (idx & 3) < nf) {
-        const size_t o = (size_t)(idx >> 2) * P.ldf + 2 * (idx & 3);
+      if (idx < total && 2 * (idx & pm) < nf) {
+        const size_t o = (size_t)(idx >> lgP) * P.ldf + 2 * (idx & pm);
         sv[u] = __ldg(reinterpret_cast<const float4*>(Srow + o));
         if (RMW) pv[u] = *reinterpret_cast<const float4*>(prow + o);
       }
@@ -246,7 +256,7 @@ __device__ __forceinline__ void spectrum_in_pairs(float2* smem, int nf, bool con
     for (int u = 0; u < kBatch; ++u) {
       const int idx = i0 + u * nthr;
       if (idx >= total) continue;
-      const int kk = idx >> 2, t0 = 2 * (idx & 3), k = klo + kk;
+      const int kk = idx >> lgP, t0 = 2 * (idx & pm), k = klo + kk;
       if (t0 >= nf) continue;
       if (RMW) {
         const size_t o = (size_t)kk * P.ldf + t0;
@@ -270,11 +280,11 @@ __device__ __forceinline__ void spectrum_in_pairs(float2* smem, int nf, bool con
 
 // P5: emit2(kk, first trace t0 (even), X of t0, X of t0 + 1 (zero if that trace does not exist), whether it exists)
 template <int HF, typename Emit2>
-__device__ __forceinline__ void band_out_pairs(const float2* smem, int nf, const FastParams& P, Emit2 emit2) {
+__device__ __forceinline__ void band_out_pairs(const float2* smem, int nf, int lgFT, const FastParams& P, Emit2 emit2) {
   constexpr int TS = Geo<HF>::TS;
-  const int total = P.nb * 4;
+  const int lgP = lgFT - 1, total = P.nb << lgP;
   for (int idx = threadIdx.x; idx < total; idx += blockDim.x) {
-    const int kk = idx >> 2, t0 = 2 * (idx & 3);
+    const int kk = idx >> lgP, t0 = 2 * (idx & ((1 << lgP) - 1));
     if (t0 >= nf) continue;
     const float2 X0 = rfft_bin_fast<HF>(smem + t0 * TS, P.tw, P.klo + kk);
     const float2 X1 = t0 + 1 < nf ? rfft_bin_fast<HF>(smem + (t0 + 1) * TS, P.tw, P.klo + kk) : make_float2(0.f, 0.f);
@@ -311,12 +321,12 @@ __device__ __forceinline__ void prefetch_window(const float* trace, int nt, int 
 // ------------------------------------------------------------------------------------------------ k_load_R_fast
 // grid (ceil(nshots / ST), nrec); Rt: [nshots][nrec][nt]                                        (a0)
 template <int HF>
-__global__ void __launch_bounds__(256 * HF, 2 / HF)
+__global__ void __launch_bounds__(256, 2)
 k_load_R_fast(const float* __restrict__ Rt, float2* __restrict__ Rhat, FastParams P, int shot0, int nshots, int lgST,
               float scale_mid, float scale_end) {
   extern __shared__ float2 smem[];
   constexpr int TS = Geo<HF>::TS;
-  const int ST = 1 << lgST, r = blockIdx.y, g0 = blockIdx.x * ST;
+  const int ST = 1 << lgST, r = P.r0 + blockIdx.y, g0 = blockIdx.x * ST;
   const int ns = min(ST, nshots - g0);
   const Who me = who<HF>();
   if (me.tl < ns) {
@@ -328,11 +338,11 @@ k_load_R_fast(const float* __restrict__ Rt, float2* __restrict__ Rhat, FastParam
   }
   __syncthreads();
   auto weight = [&](int s) { return (P.n > 1 && (s == 0 || s == P.n - 1)) ? scale_end : scale_mid; };
-  if (lgST == 3 && ((shot0 + g0) & 1) == 0) {
-    band_out_pairs<HF>(smem, ns, P, [&](int kk, int t0, float2 X0, float2 X1, bool two) {
+  if (lgST >= 2 && ((shot0 + g0) & 1) == 0) {
+    band_out_pairs<HF>(smem, ns, lgST, P, [&](int kk, int t0, float2 X0, float2 X1, bool two) {
       const int s = shot0 + g0 + t0;  // even
       const float c0 = weight(s), c1 = weight(s + 1);
-      float2* dst = Rhat + ((size_t)r * P.nb + kk) * P.ld + s;
+      float2* dst = Rhat + ((size_t)(r - P.r0) * P.nb + kk) * P.ld + s;
       if (two) *reinterpret_cast<float4*>(dst) = make_float4(c0 * X0.x, c0 * X0.y, c1 * X1.x, c1 * X1.y);
       else *dst = make_float2(c0 * X0.x, c0 * X0.y);  // column s + 1 belongs to another chunk (or is padding)
     });
@@ -340,7 +350,7 @@ k_load_R_fast(const float* __restrict__ Rt, float2* __restrict__ Rhat, FastParam
     band_out<HF>(smem, ns, lgST, P, [&](int tl, int kk, float2 X) {
       const int s = shot0 + g0 + tl;
       const float sc = weight(s);
-      Rhat[((size_t)r * P.nb + kk) * P.ld + s] = make_float2(sc * X.x, sc * X.y);
+      Rhat[((size_t)(r - P.r0) * P.nb + kk) * P.ld + s] = make_float2(sc * X.x, sc * X.y);
     });
   }
 }
@@ -348,11 +358,11 @@ k_load_R_fast(const float* __restrict__ Rt, float2* __restrict__ Rhat, FastParam
 // ------------------------------------------------------------------------------------------------ k_fwd_fast
 // grid (ceil(nfoc / FT), n); src: [nfoc][n][nt]                                                        (a1, a6)
 template <int HF>
-__global__ void __launch_bounds__(256 * HF, 2 / HF)
+__global__ void __launch_bounds__(256, 2)
 k_fwd_fast(const float* __restrict__ src, OperandOut O, FastParams P, int lgFT, int conj_out, float* __restrict__ init_Tsrc) {
   extern __shared__ float2 smem[];
   constexpr int TS = Geo<HF>::TS;
-  const int FT = 1 << lgFT, r = blockIdx.y, f0 = blockIdx.x * FT;
+  const int FT = 1 << lgFT, r = P.r0 + blockIdx.y, f0 = blockIdx.x * FT;
   const int nf = min(FT, P.nfoc - f0), nt = P.nt;
   const Who me = who<HF>();
   if (me.tl < nf) {
@@ -374,8 +384,8 @@ k_fwd_fast(const float* __restrict__ src, OperandOut O, FastParams P, int lgFT, 
   }
   __syncthreads();
   const float cs = conj_out ? -1.f : 1.f;  // conj: spectrum of the time-reversed real trace
-  if (lgFT == 3 && (O.ldf & 1) == 0) {
-    band_out_pairs<HF>(smem, nf, P, [&](int kk, int t0, float2 X0, float2 X1, bool) {
+  if (lgFT >= 2 && (O.ldf & 1) == 0) {
+    band_out_pairs<HF>(smem, nf, lgFT, P, [&](int kk, int t0, float2 X0, float2 X1, bool) {
       store_operand2(O, P.ld, kk, r, f0 + t0, make_float2(X0.x, cs * X0.y), make_float2(X1.x, cs * X1.y));
     });
   } else {
@@ -386,16 +396,16 @@ k_fwd_fast(const float* __restrict__ src, OperandOut O, FastParams P, int lgFT, 
 // ------------------------------------------------------------------------------------------------ k_inv_fast
 // grid (ceil(nfoc / FT), n); spec: [n][nb][ldf]; out[j] = sS*S[j] + sA*A[j] + sB*B[(nt-j)%nt]              (a3, a7)
 template <int HF>
-__global__ void __launch_bounds__(256 * HF, 2 / HF)
+__global__ void __launch_bounds__(256, 2)
 k_inv_fast(const float2* __restrict__ spec, FastParams P, int lgFT, float* __restrict__ out, float sS,
            const float* __restrict__ A, float sA, const float* __restrict__ B, float sB) {
   extern __shared__ float2 smem[];
   constexpr int TS = Geo<HF>::TS;
-  const int FT = 1 << lgFT, r = blockIdx.y, f0 = blockIdx.x * FT;
+  const int FT = 1 << lgFT, r = P.r0 + blockIdx.y, f0 = blockIdx.x * FT;
   const int nf = min(FT, P.nfoc - f0), nt = P.nt;
   const float2* srow = spec + (size_t)r * P.nb * P.ldf + f0;
-  if (lgFT == 3 && (P.ldf & 1) == 0 && simple_band(P, Geo<HF>::M)) {
-    spectrum_in_pairs<HF, false>(smem, nf, false, P, srow, nullptr);
+  if (lgFT >= 2 && (P.ldf & 1) == 0 && simple_band(P, Geo<HF>::M)) {
+    spectrum_in_pairs<HF, false>(smem, nf, lgFT, false, P, srow, nullptr);
   } else {
     spectrum_in<HF>(
         smem, nf, lgFT, false, P, [&](int tl, int kk, float2&) { return __ldg(srow + (size_t)kk * P.ldf + tl); },
@@ -435,17 +445,17 @@ k_inv_fast(const float2* __restrict__ spec, FastParams P, int lgFT, float* __res
 // (Theta is symmetric in +-t, so Theta T = T Theta; w is real, so FFT(T w) = conj FFT(w).)  Every global access of
 // the time fields is a natural-order float2 row; only the optional N_i copy of an even step is written reversed.
 template <int HF>
-__global__ void __launch_bounds__(256 * HF, 2 / HF)
+__global__ void __launch_bounds__(256, 2)
 k_post_fast(const float2* __restrict__ Shat, float2* __restrict__ phat, OperandOut O, const int* __restrict__ h,
             float* __restrict__ f1plus, float* __restrict__ f1min, FastParams P, int lgFT, int parity_even,
             float* __restrict__ Ni_out) {
   extern __shared__ float2 smem[];
   constexpr int TS = Geo<HF>::TS;
-  const int FT = 1 << lgFT, r = blockIdx.y, f0 = blockIdx.x * FT;
+  const int FT = 1 << lgFT, r = P.r0 + blockIdx.y, f0 = blockIdx.x * FT;
   const int nf = min(FT, P.nfoc - f0), nt = P.nt;
   const size_t rowoff = (size_t)r * P.nb * P.ldf + f0;
   const Who me = who<HF>();
-  const bool pairs = lgFT == 3 && (P.ldf & 1) == 0;
+  const bool pairs = lgFT >= 2 && (P.ldf & 1) == 0;
   int hh = 0;
   if (me.tl < nf) {  // the accumulator rows that P3 will touch: on their way to L2 while P1 / P2 run
     hh = __ldg(h + (size_t)(f0 + me.tl) * P.n + r);
@@ -453,7 +463,7 @@ k_post_fast(const float2* __restrict__ Shat, float2* __restrict__ phat, OperandO
   }
   // a3: p^ += S^   [PAPER.md:79]
   if (pairs && simple_band(P, Geo<HF>::M)) {
-    spectrum_in_pairs<HF, true>(smem, nf, parity_even == 0, P, Shat + rowoff, phat + rowoff);
+    spectrum_in_pairs<HF, true>(smem, nf, lgFT, parity_even == 0, P, Shat + rowoff, phat + rowoff);
   } else {
     spectrum_in<HF>(
         smem, nf, lgFT, parity_even == 0, P,
@@ -520,7 +530,7 @@ k_post_fast(const float2* __restrict__ Shat, float2* __restrict__ phat, OperandO
   __syncthreads();
   const float cs = parity_even ? 1.f : -1.f;
   if (pairs) {
-    band_out_pairs<HF>(smem, nf, P, [&](int kk, int t0, float2 X0, float2 X1, bool) {
+    band_out_pairs<HF>(smem, nf, lgFT, P, [&](int kk, int t0, float2 X0, float2 X1, bool) {
       store_operand2(O, P.ld, kk, r, f0 + t0, make_float2(-X0.x, cs * X0.y), make_float2(-X1.x, cs * X1.y));
     });
   } else {
@@ -540,6 +550,7 @@ FastParams make_fast(const mk_ctx* c, int nfoc, int ldf) {
   P.ld = c->ld;
   P.ldf = ldf;
   P.nfoc = nfoc;
+  P.r0 = c->r0;
   return P;
 }
 
@@ -552,7 +563,7 @@ struct Shape {
 // the CTA-wide phases P1 / P5.  Measured on config 1 (601 traces per launch): 256 threads 29 us (3 waves), 32 threads 40 us
 Shape shape_for(const mk_ctx* c, int count) {
   const int HF = c->nt / 2048;
-  int lg = 3;
+  int lg = HF == 1 ? 3 : 2;  // 256 threads and <= 68 KB of traces per CTA: two CTAs per SM overlap each other's memory phases
   while (lg > 0 && (1 << (lg - 1)) >= count) --lg;
   Shape s;
   s.lg = lg;
@@ -585,27 +596,27 @@ bool fast_fft_ok(const mk_ctx* c) { return (c->nt == 2048 || c->nt == 4096) && c
 
 int launch_load_R_fast(mk_ctx* c, const float* d_R_time, int shot0, int nshots) {
   const Shape sh = shape_for(c, nshots);
-  const dim3 grid((nshots + (1 << sh.lg) - 1) >> sh.lg, c->n);
+  const dim3 grid((nshots + (1 << sh.lg) - 1) >> sh.lg, c->nrow);
   const float sm = (float)(c->dt * c->dx), se = (float)(c->dt * c->dx * 0.5);
   MK_FAST_LAUNCH(k_load_R_fast, grid, sh, d_R_time, c->d_Rhat, make_fast(c, 0, 0), shot0, nshots, sh.lg, sm, se);
 }
 
 int launch_fwd_fast(mk_ctx* c, const float* d_src, const OperandOut& O, int nfoc, bool conj_out, float* d_init_Tsrc) {
   const Shape sh = shape_for(c, nfoc);
-  const dim3 grid((nfoc + (1 << sh.lg) - 1) >> sh.lg, c->n);
+  const dim3 grid((nfoc + (1 << sh.lg) - 1) >> sh.lg, c->nrow);
   MK_FAST_LAUNCH(k_fwd_fast, grid, sh, d_src, O, make_fast(c, nfoc, O.ldf), sh.lg, conj_out ? 1 : 0, d_init_Tsrc);
 }
 
 int launch_inv_fast(mk_ctx* c, const float2* d_spec, int nfoc, int ldf, float* d_out, float sS, const float* d_A, float sA,
                     const float* d_B, float sB) {
   const Shape sh = shape_for(c, nfoc);
-  const dim3 grid((nfoc + (1 << sh.lg) - 1) >> sh.lg, c->n);
+  const dim3 grid((nfoc + (1 << sh.lg) - 1) >> sh.lg, c->nrow);
   MK_FAST_LAUNCH(k_inv_fast, grid, sh, d_spec, make_fast(c, nfoc, ldf), sh.lg, d_out, sS, d_A, sA, d_B, sB);
 }
 
 int launch_post_fast(mk_ctx* c, const OperandOut& O, int parity_even, float* d_Ni_out) {
   const Shape sh = shape_for(c, c->nfoc);
-  const dim3 grid((c->nfoc + (1 << sh.lg) - 1) >> sh.lg, c->n);
+  const dim3 grid((c->nfoc + (1 << sh.lg) - 1) >> sh.lg, c->nrow);
   MK_FAST_LAUNCH(k_post_fast, grid, sh, c->d_Shat, c->d_phat, O, c->d_h, c->d_f1plus, c->d_f1min, make_fast(c, c->nfoc, c->ldf),
                  sh.lg, parity_even, d_Ni_out);
 }

@@ -195,7 +195,7 @@ __global__ void __launch_bounds__(kThreads) k_load_R(const float* __restrict__ R
                                                      int shot0, int nshots, int lgST, float scale_mid, float scale_end) {
   extern __shared__ float2 smem[];
   const int MP = mkfft::padded_len(P.plan.M), ST = 1 << lgST;
-  const int r = blockIdx.y, g0 = blockIdx.x * ST;
+  const int r = P.r0 + blockIdx.y, g0 = blockIdx.x * ST;
   const int ns = min(ST, nshots - g0);
   const Group g = my_group(lgST);
   const size_t nt = P.plan.nt;
@@ -213,7 +213,7 @@ __global__ void __launch_bounds__(kThreads) k_load_R(const float* __restrict__ R
     const int s = shot0 + g0 + tl;
     const float sc = (P.n > 1 && (s == 0 || s == P.n - 1)) ? scale_end : scale_mid;
     const float2 X = mkfft::rfft_bin(smem + tl * MP, P.plan, P.tw, P.klo + kk);
-    Rhat[((size_t)r * P.nb + kk) * P.ld + s] = make_float2(sc * X.x, sc * X.y);
+    Rhat[((size_t)(r - P.r0) * P.nb + kk) * P.ld + s] = make_float2(sc * X.x, sc * X.y);
   }
 }
 
@@ -223,7 +223,7 @@ __global__ void __launch_bounds__(kThreads) k_fwd(const float* __restrict__ src,
                                                   int conj_out, float* __restrict__ init_Tsrc) {
   extern __shared__ float2 smem[];
   const int MP = mkfft::padded_len(P.plan.M), FT = 1 << lgFT;
-  const int r = blockIdx.y, f0 = blockIdx.x * FT;
+  const int r = P.r0 + blockIdx.y, f0 = blockIdx.x * FT;
   const int nf = min(FT, P.nfoc - f0);
   const int nt = P.plan.nt;
   const Group g = my_group(lgFT);
@@ -250,7 +250,7 @@ __global__ void __launch_bounds__(kThreads) k_inv(const float2* __restrict__ spe
                                                   const float* __restrict__ B, float sB) {
   extern __shared__ float2 smem[];
   const int MP = mkfft::padded_len(P.plan.M), FT = 1 << lgFT;
-  const int r = blockIdx.y, f0 = blockIdx.x * FT;
+  const int r = P.r0 + blockIdx.y, f0 = blockIdx.x * FT;
   const int nf = min(FT, P.nfoc - f0);
   const int nt = P.plan.nt;
   const float2* srow = spec + (size_t)r * P.nb * P.ldf + f0;
@@ -294,7 +294,7 @@ __global__ void __launch_bounds__(kThreads) k_post(const float2* __restrict__ Sh
                                                    FftParams P, int lgFT, int parity_even, float* __restrict__ Ni_out) {
   extern __shared__ float2 smem[];
   const int MP = mkfft::padded_len(P.plan.M), FT = 1 << lgFT;
-  const int r = blockIdx.y, f0 = blockIdx.x * FT;
+  const int r = P.r0 + blockIdx.y, f0 = blockIdx.x * FT;
   const int nf = min(FT, P.nfoc - f0);
   const int nt = P.plan.nt;
   const size_t rowoff = (size_t)r * P.nb * P.ldf + f0;
@@ -371,6 +371,7 @@ FftParams make_params(const mk_ctx* c, int nfoc, int ldf) {
   P.ld = c->ld;
   P.ldf = ldf;
   P.nfoc = nfoc;
+  P.r0 = c->r0;
   return P;
 }
 
@@ -395,7 +396,7 @@ int launch_load_R(mk_ctx* c, const float* d_R_time, int shot0, int nshots) {
   const int lg = pick_lgft(c, nshots), ST = 1 << lg;
   const size_t smem = trace_smem(c, lg);
   if (int rc = set_smem(c, k_load_R, smem)) return rc;
-  const dim3 grid((nshots + ST - 1) / ST, c->n);
+  const dim3 grid((nshots + ST - 1) / ST, c->nrow);
   const float sm = (float)(c->dt * c->dx), se = (float)(c->dt * c->dx * 0.5);
   k_load_R<<<grid, kThreads, smem, c->stream>>>(d_R_time, c->d_Rhat, make_params(c, 0, 0), shot0, nshots, lg, sm, se);
   ++c->launches;
@@ -407,7 +408,7 @@ int launch_fwd(mk_ctx* c, const float* d_src, const OperandOut& O, int nfoc, boo
   const int lg = pick_lgft(c, nfoc), FT = 1 << lg;
   const size_t smem = trace_smem(c, lg);
   if (int rc = set_smem(c, k_fwd, smem)) return rc;
-  const dim3 grid((nfoc + FT - 1) / FT, c->n);
+  const dim3 grid((nfoc + FT - 1) / FT, c->nrow);
   k_fwd<<<grid, kThreads, smem, c->stream>>>(d_src, O, make_params(c, nfoc, O.ldf), lg, conj_out ? 1 : 0, d_init_Tsrc);
   ++c->launches;
   return check_cuda(c, cudaGetLastError(), "k_fwd");
@@ -419,7 +420,7 @@ int launch_inv(mk_ctx* c, const float2* d_spec, int nfoc, int ldf, float* d_out,
   const int lg = pick_lgft(c, nfoc), FT = 1 << lg;
   const size_t smem = trace_smem(c, lg);
   if (int rc = set_smem(c, k_inv, smem)) return rc;
-  const dim3 grid((nfoc + FT - 1) / FT, c->n);
+  const dim3 grid((nfoc + FT - 1) / FT, c->nrow);
   k_inv<<<grid, kThreads, smem, c->stream>>>(d_spec, make_params(c, nfoc, ldf), lg, d_out, sS, d_A, sA, d_B, sB);
   ++c->launches;
   return check_cuda(c, cudaGetLastError(), "k_inv");
@@ -430,7 +431,7 @@ int launch_post(mk_ctx* c, const OperandOut& O, int parity_even, float* d_Ni_out
   const int lg = pick_lgft(c, c->nfoc), FT = 1 << lg;
   const size_t smem = trace_smem(c, lg);
   if (int rc = set_smem(c, k_post, smem)) return rc;
-  const dim3 grid((c->nfoc + FT - 1) / FT, c->n);
+  const dim3 grid((c->nfoc + FT - 1) / FT, c->nrow);
   k_post<<<grid, kThreads, smem, c->stream>>>(c->d_Shat, c->d_phat, O, c->d_h, c->d_f1plus, c->d_f1min,
                                               make_params(c, c->nfoc, c->ldf), lg, parity_even, d_Ni_out);
   ++c->launches;

@@ -23,6 +23,9 @@
 //   h [nfoc][n] int32     window half-widths                                                          (a4)
 struct mk_ctx {
   int n = 0, nt = 0, nb = 0, klo = 0, khi = 0, ld = 0;
+  int r0 = 0, nrow = 0;  // receiver rows this context owns (row sharding; nrow == n: everything)
+  bool operand_stale[2] = {false, false};  // sharded: rows produced locally but not yet exchanged
+  int prepared_field = 0;                  // mk_finish_prepare
   double dt = 0, dx = 0, fmin = 0, fmax = 0;
   int eps = 8, regime = 0, timing = 0;
   cudaStream_t stream = nullptr;
@@ -92,6 +95,7 @@ struct FftParams {
   mkfft::Plan plan;
   const float2* tw;
   int n, nb, klo, ld, ldf, nfoc;
+  int r0;  // first receiver row of this context (grid row b handles receiver r0 + b; R^ is stored from row r0 on)
 };
 
 // where a forward transform stores N^ (a1, a6): the plain complex layout (regimes 1, 2) or the split real operand

@@ -106,8 +106,9 @@ int launch_t(mk_ctx* c, const float2* d_Nhat, float2* d_Shat) {
   auto kern = k_syn_gemv<NFOC>;
   if (int rc = check_cuda(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem), "cudaFuncSetAttribute"))
     return rc;
-  const dim3 grid(c->nb, (c->n + kRowsPerCta - 1) / kRowsPerCta);
-  kern<<<grid, kThreads, smem, c->stream>>>(c->d_Rhat, d_Nhat, d_Shat, c->n, c->nb, c->ld);
+  // row sharding: R^ holds the rows r0 .. r0 + nrow - 1; S^ is indexed by the global receiver
+  const dim3 grid(c->nb, (c->nrow + kRowsPerCta - 1) / kRowsPerCta);
+  kern<<<grid, kThreads, smem, c->stream>>>(c->d_Rhat, d_Nhat, d_Shat + (size_t)c->r0 * c->nb * NFOC, c->nrow, c->nb, c->ld);
   ++c->launches;
   return check_cuda(c, cudaGetLastError(), "k_syn_gemv");
 }

@@ -352,7 +352,7 @@ int launch_syn_tc(mk_ctx* c, int slot, const float* d_Bhi, const float* d_Blo, f
   if (int rc = get_encode(c, &enc)) return rc;
   if (!c->tmap_A_ok) {
     // A' = R^ as fp32 [n][nb][2 ld]: dims (k', bin, r); box = 16 floats x 1 bin x 128 receivers; rows r >= n read as zero
-    const cuuint64_t dims[3] = {(cuuint64_t)2 * c->ld, (cuuint64_t)c->nb, (cuuint64_t)c->n};
+    const cuuint64_t dims[3] = {(cuuint64_t)2 * c->ld, (cuuint64_t)c->nb, (cuuint64_t)c->nrow};  // local rows of R^
     const cuuint64_t str[2] = {(cuuint64_t)2 * c->ld * 4, (cuuint64_t)c->nb * 2 * c->ld * 4};
     const cuuint32_t box[3] = {BK, 1, BM};
     if (int rc = encode3(c, enc, c->tmap_A, c->d_Rhat, dims, str, box, CU_TENSOR_MAP_SWIZZLE_64B, "A")) return rc;
@@ -370,11 +370,11 @@ int launch_syn_tc(mk_ctx* c, int slot, const float* d_Bhi, const float* d_Blo, f
     c->tmap_B_ldb[slot] = ldb;
   }
   TcParams P;
-  P.n = c->n;
+  P.n = c->nrow;  // row sharding: local rows; S^ is offset to the first one below
   P.nb = c->nb;
   P.ld = c->ld;
   P.ncols = 2 * ldf;
-  P.mt = (c->n + BM - 1) / BM;
+  P.mt = (c->nrow + BM - 1) / BM;
   P.ntl = (P.ncols + BN - 1) / BN;
   P.s_row = (size_t)c->nb * 2 * ldf;
   if (int rc = check_cuda(c, cudaFuncSetAttribute(k_syn_gemm_tf32x3, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemBytes),
@@ -385,7 +385,7 @@ int launch_syn_tc(mk_ctx* c, int slot, const float* d_Bhi, const float* d_Blo, f
   k_syn_gemm_tf32x3<<<grid, kThreads, kSmemBytes, c->stream>>>(*reinterpret_cast<const CUtensorMap*>(c->tmap_A),
                                                                *reinterpret_cast<const CUtensorMap*>(c->tmap_B[slot][0]),
                                                                *reinterpret_cast<const CUtensorMap*>(c->tmap_B[slot][1]),
-                                                               reinterpret_cast<float*>(d_Shat), P);
+                                                               reinterpret_cast<float*>(d_Shat + (size_t)c->r0 * c->nb * ldf), P);
   ++c->launches;
   return check_cuda(c, cudaGetLastError(), "k_syn_gemm_tf32x3");
 }

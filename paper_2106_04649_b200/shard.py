@@ -2,7 +2,11 @@
 runs on one GPU").  Focal points are independent of one another (each trace of N_i depends on a single focal
 point), so with N GPUs the job shards over focal points with R^ replicated and NO data-path
 collective; when a workload has a single focal point (config 1) the ranks are independent replicas, each with its
-own focal point.  torch.distributed is used only for the barrier and the max-over-ranks timing."""
+own focal point.  torch.distributed is used only for the barrier and the max-over-ranks timing.
+
+The second half of this module is the receiver-row sharding of section 8(e) / NEXT-3: R^ split by rows over the ranks,
+one all-gather of the freshly produced operand rows per synthesis (for an R^ that does not fit one GPU, or to cut the
+time of one focal batch)."""
 from __future__ import annotations
 
 from dataclasses import replace
@@ -50,3 +54,78 @@ def sum_over_ranks(value: float, dist=None) -> float:
     t = torch.tensor([float(value)], dtype=torch.float64, device=dev)
     dist.all_reduce(t, op=dist.ReduceOp.SUM)
     return float(t.item())
+
+
+# ---------------------------------------------------------------------------------------------------------------------
+# Receiver-row sharding (SURVEY.md section 8(e) "B200 equivalent", section 8(f) NEXT-3; include/mk.h mk_create_sharded).
+# Rank g owns a contiguous block of receiver rows of R^ and computes a2..a6 for them; the one exchange step per
+# synthesis is an all-gather of the operand rows just produced.  The kernels are the library's; what follows only moves
+# rows between ranks (NCCL all-gather under torch.distributed, or plain copies between contexts of one process).
+def row_slice(n: int, rank: int, world: int) -> range:
+    """Contiguous, balanced block of receiver rows owned by `rank` (sizes differ by at most 1)."""
+    return focal_slice(n, rank, world)
+
+
+def allgather_operand_rows(planes, rows_per_rec: int, n: int, rank: int, world: int, dist) -> None:
+    """In place: after the call every plane ([nb][rows_per_bin][row_floats], rows of receiver r at rows_per_rec * r ..)
+    holds the rows of every rank.  Works on CPU tensors (gloo) and CUDA tensors (nccl) alike."""
+    import torch
+    nmax = max(len(row_slice(n, g, world)) for g in range(world)) * rows_per_rec
+    mine = row_slice(n, rank, world)
+    for plane in planes:
+        nb, _, rf = plane.shape
+        send = torch.zeros((nb, nmax, rf), dtype=plane.dtype, device=plane.device)
+        send[:, :rows_per_rec * len(mine)] = plane[:, rows_per_rec * mine.start:rows_per_rec * mine.stop]
+        recv = [torch.empty_like(send) for _ in range(world)]
+        dist.all_gather(recv, send)
+        for g in range(world):
+            if g == rank:
+                continue
+            rg = row_slice(n, g, world)
+            plane[:, rows_per_rec * rg.start:rows_per_rec * rg.stop] = recv[g][:, :rows_per_rec * len(rg)]
+
+
+def exchange_in_process(mks, slot: int) -> None:
+    """The same exchange between row-sharded contexts that live in ONE process (single-GPU verification of the sharded
+    path: the contexts are stepped in lock-step by the caller, nothing waits on anything)."""
+    views = [mk.operand(slot) for mk in mks]
+    for src, (sp, sv) in enumerate(views):
+        lo, hi = sv.rows_per_rec * sv.row0, sv.rows_per_rec * (sv.row0 + sv.nrows)
+        for dst, (dp, _) in enumerate(views):
+            if dst != src:
+                for a, b in zip(dp, sp):
+                    a[:, lo:hi] = b[:, lo:hi]
+    for mk in mks:
+        mk.operand_exchanged(slot)
+
+
+def run_row_sharded(mk, d_Gd, d_td, niter: int, outs: dict, exchange, on_iterate=None) -> None:
+    """Algorithm 1 on a row-sharded context: the library's calls with `exchange(slot)` between them (include/mk.h).
+    `exchange` must make the operand rows of `slot` identical on all ranks and then call mk.operand_exchanged(slot);
+    `outs` maps field names to [nfoc][nrec][nt] device tensors (only this rank's receiver rows are meaningful)."""
+    from . import binding as B
+    mk.begin(d_Gd, d_td)
+    exchange(0)
+    for i in range(niter):
+        last = outs.get("N_last") if i == niter - 1 else None
+        mk.step(last)
+        if on_iterate is not None:
+            on_iterate(i)
+        exchange(0)
+    plain = {k: v for k, v in outs.items() if k in ("f1plus", "f1min", "G") and v is not None}
+    if plain:
+        mk.finish(plain)
+    for name, field in (("Gminus", B.MK_FIELD_GMINUS), ("Gplus", B.MK_FIELD_GPLUS)):
+        if outs.get(name) is not None:
+            mk.finish_prepare(field)
+            exchange(1)
+            mk.finish_complete(field, outs[name])
+
+
+def distributed_exchange(mk, dist):
+    """exchange(slot) for run_row_sharded under torch.distributed (one process per GPU, backend nccl)."""
+    def exchange(slot):
+        planes, v = mk.operand(slot)
+        allgather_operand_rows(planes, v.rows_per_rec, mk.nrec, dist.get_rank(), dist.get_world_size(), dist)
+        mk.operand_exchanged(slot)
+    return exchange

@@ -147,3 +147,67 @@ def test_image_matches_oracle():
     e = rel_l2(img, img_ref)
     print(f"\n[image nfoc={cfg.nfoc}] rel L2 {e:.2e}")
     assert e <= TOL_FINAL
+
+
+# ---------------------------------------------------------------- receiver-row sharding (section 8(e), NEXT-3)
+@pytest.mark.parametrize("k,n,nt,nfoc,regime,world", [(1, 37, 512, 3, 1, 2), (3, 45, 512, 19, 2, 3), (3, 150, 2048, 19, 3, 3)])
+def test_row_sharded_contexts_reproduce_the_single_context(k, n, nt, nfoc, regime, world):
+    """`world` row-sharded contexts in one process, stepped in lock-step with the operand rows copied between them
+    (shard.exchange_in_process — what the NCCL all-gather does across GPUs): every rank's receiver rows of every iterate
+    and every final field must equal the unsharded run, which the tests above hold against the oracle."""
+    import torch
+    from paper_2106_04649_b200 import binding as B, shard
+    focal = "single:400" if nfoc == 1 else "fan:250"
+    cfg = calibrated(configs.scaled(k, n=n, nt=nt, nfoc=nfoc, focal=focal, niter=6))
+    R, Gd, td = problem(cfg)
+    whole = gpu_chain(cfg, R, Gd, td, regime=regime)
+    dev = torch.device("cuda:0")
+    dR, dGd, dtd = (torch.from_numpy(np.ascontiguousarray(a)).to(dev) for a in (R, Gd, td))
+    mks = []
+    try:
+        for g in range(world):
+            rows = shard.row_slice(n, g, world)
+            mk = B.Marchenko(n, n, nt, cfg.dt, cfg.dx, cfg.fmin, cfg.fmax, rows=(rows.start, len(rows)))
+            mk.set_option(B.MK_OPT_EPS_SAMPLES, cfg.eps)
+            mk.set_option(B.MK_OPT_REGIME, regime)
+            mk.load_R(dR)                                   # same full chunk on every rank; the library keeps its rows
+            mks.append(mk)
+        # a contraction on rows that were not exchanged must fail loudly
+        mks[0].begin(dGd, dtd)
+        with pytest.raises(B.MkError):
+            mks[0].step()
+        with pytest.raises(B.MkError):
+            mks[0].run(dGd, dtd, 1, {})
+        for mk in mks:
+            mk.begin(dGd, dtd)
+        shard.exchange_in_process(mks, 0)
+        its = [[] for _ in mks]
+        bufs = [torch.zeros((nfoc, n, nt), dtype=torch.float32, device=dev) for _ in mks]
+        for _ in range(cfg.niter):
+            for g, mk in enumerate(mks):
+                mk.step(bufs[g])
+                its[g].append(bufs[g].cpu().numpy().copy())
+            shard.exchange_in_process(mks, 0)
+        outs = [{nm: torch.zeros((nfoc, n, nt), dtype=torch.float32, device=dev) for nm in FINALS} for _ in mks]
+        for g, mk in enumerate(mks):
+            mk.finish({nm: outs[g][nm] for nm in ("f1plus", "f1min", "G")})
+        for name, field in (("Gminus", B.MK_FIELD_GMINUS), ("Gplus", B.MK_FIELD_GPLUS)):
+            for mk in mks:
+                mk.finish_prepare(field)
+            shard.exchange_in_process(mks, 1)
+            for g, mk in enumerate(mks):
+                mk.finish_complete(field, outs[g][name])
+        torch.cuda.synchronize()
+        worst = 0.0
+        for g in range(world):
+            rows = shard.row_slice(n, g, world)
+            sl = slice(rows.start, rows.stop)
+            for i in range(cfg.niter):
+                worst = max(worst, rel_l2(its[g][i][:, sl], whole["N_iters"][i][:, sl]))
+            for nm in FINALS:
+                worst = max(worst, rel_l2(outs[g][nm].cpu().numpy()[:, sl], whole[nm][:, sl]))
+        print(f"\n[row-sharded {world} x, n={n} nt={nt} nfoc={nfoc} regime={regime}] worst deviation from the single context {worst:.1e}")
+        assert worst <= 1e-6
+    finally:
+        for mk in mks:
+            mk.close()

@@ -73,3 +73,60 @@ def test_world_size_2_gloo_focal_sharding():
         assert gsum == float(gd_all[mine].astype(np.float64).sum())     # shards see the same bytes as the whole job
         assert t_max == 11.0 and n_sum == float(cfg.nfoc)
     assert owned == list(range(cfg.nfoc))
+
+
+# ---------------------------------------------------------------- receiver-row sharding (section 8(e), NEXT-3)
+def _row_worker(rank, world, port, q, n, nb, rpr, rf, nplanes):
+    import torch
+    import torch.distributed as dist
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), RANK=str(rank), WORLD_SIZE=str(world))
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    try:
+        ld = ((n + 15) // 16) * 16
+        full = [_row_truth(p, nb, rpr * ld, rf) for p in range(nplanes)]
+        mine = shard.row_slice(n, rank, world)
+        planes = []
+        for p in range(nplanes):                      # a rank starts with its own rows only (the rest is stale: -1)
+            t = torch.full((nb, rpr * ld, rf), -1.0)
+            t[:, rpr * mine.start:rpr * mine.stop] = full[p][:, rpr * mine.start:rpr * mine.stop]
+            t[:, rpr * n:] = 0.0                      # pad rows are zero and must stay zero
+            planes.append(t)
+        shard.allgather_operand_rows(planes, rpr, n, rank, world, dist)
+        ok = all(bool(torch.equal(planes[p][:, :rpr * n], full[p][:, :rpr * n])) and float(planes[p][:, rpr * n:].abs().max()) == 0.0
+                 for p in range(nplanes))
+        q.put((rank, ok))
+    finally:
+        dist.destroy_process_group()
+
+
+def _row_truth(p, nb, rows, rf):
+    import torch
+    g = torch.Generator().manual_seed(1234 + p)
+    return torch.randn((nb, rows, rf), generator=g)
+
+
+def test_row_slices_partition():
+    for n in (1, 5, 37, 601, 3901):
+        for world in (1, 2, 3, 8):
+            if world > n:
+                continue
+            got = [i for r in range(world) for i in shard.row_slice(n, r, world)]
+            assert got == list(range(n))
+
+
+@pytest.mark.parametrize("world,n,rpr,nplanes", [(2, 37, 1, 1), (3, 37, 2, 2)])
+def test_gloo_allgather_of_operand_rows(world, n, rpr, nplanes):
+    """The exchange step of the row-sharded path on CPU tensors: uneven row blocks, one- and two-plane operands
+    (regimes 1/2 and the two-rows-per-receiver split operand of regime 3), pad rows untouched."""
+    import torch.multiprocessing as mp
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    port = _free_port()
+    procs = [ctx.Process(target=_row_worker, args=(r, world, port, q, n, 5, rpr, 12, nplanes)) for r in range(world)]
+    for p in procs:
+        p.start()
+    res = sorted(q.get(timeout=120) for _ in range(world))
+    for p in procs:
+        p.join(timeout=60)
+        assert p.exitcode == 0
+    assert res == [(r, True) for r in range(world)]
