@@ -51,6 +51,22 @@ def test_outputs_struct_layout_matches_header():
     assert C.sizeof(binding.mk_outputs) == 6 * C.sizeof(C.c_void_p)
 
 
+def test_operand_view_struct_layout_matches_header():
+    from paper_2106_04649_b200 import binding
+    m = re.search(r"typedef struct mk_operand_view \{(.*?)\} mk_operand_view;", HEADER, flags=re.S)
+    ints = [x.strip() for x in re.search(r"int ([^;]+);", m.group(1)).group(1).split(",")]
+    assert "float* plane[2];" in m.group(1)
+    assert [nm for nm, _ in binding.mk_operand_view._fields_] == ["plane"] + ints
+    assert C.sizeof(binding.mk_operand_view) == 2 * C.sizeof(C.c_void_p) + 4 * len(ints) + (4 * len(ints)) % 8
+
+
+def test_sharded_create_rejects_bad_row_ranges(lib):
+    h = C.c_void_p()
+    for row0, nrows in ((-1, 4), (0, 0), (8, 4), (0, 11)):
+        assert lib.mk_create_sharded(C.byref(h), 10, 10, 64, 0.004, 10.0, 5.0, 60.0, row0, nrows) == -1
+        assert not h
+
+
 def test_invalid_arguments_are_rejected_before_touching_the_device(lib):
     h = C.c_void_p()
     assert lib.mk_create(C.byref(h), 10, 11, 64, 0.004, 10.0, 5.0, 60.0) == -1      # nshot != nrec (G10)
