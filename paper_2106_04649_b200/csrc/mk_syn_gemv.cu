@@ -16,10 +16,14 @@ constexpr int kWarps = kThreads / 32;
 constexpr int kRowsPerCta = 64;  // receivers per CTA
 // Rows of R^ a warp streams at once (x reuse, independent load streams), unroll of the chunk loop (loads in flight per
 // stream) and CTAs per SM.  Measured on B200, config 1 (nfoc = 1, 1.30 GB of R^): (4, 2, 3) 6.81 TB/s, (4, 1, 4) 7.00,
-// (2, 4, 4) 7.03; a pure read of the same bytes peaks at 7.70 TB/s.
+// (2, 4, 4) 7.03; a pure read of the same bytes peaks at 7.70 TB/s.  Larger NFOC: registers decide (accumulators =
+// rows x NFOC complex), the x reads from shared memory are 2 NFOC / rows bytes per byte of R^.
 template <int NFOC>
 struct Tune {
-  static constexpr int kRows = NFOC == 1 ? 2 : 4, kUnroll = NFOC == 1 ? 4 : 2, kMinBlocks = NFOC == 1 ? 4 : (NFOC <= 2 ? 3 : 1);
+  // measured per NFOC on config 1's R^ (us per launch): 188, 209, 211, 248, 270, 305, 360, 383 for NFOC = 1..8
+  static constexpr int kRows = NFOC == 1 ? 2 : (NFOC == 2 ? 4 : (NFOC <= 6 ? 2 : 4));
+  static constexpr int kUnroll = NFOC == 1 ? 4 : (NFOC <= 4 ? 2 : 1);
+  static constexpr int kMinBlocks = NFOC == 1 ? 4 : (NFOC <= 4 ? 3 : 2);
 };
 
 struct f8 {
@@ -46,19 +50,29 @@ template <int NFOC>
 __global__ void __launch_bounds__(kThreads, Tune<NFOC>::kMinBlocks) k_syn_gemv(const float2* __restrict__ Rhat, const float2* __restrict__ Nhat,
                                                        float2* __restrict__ Shat, int n, int nb, int ld) {
   extern __shared__ float4 smem4[];
-  float2* x = reinterpret_cast<float2*>(smem4);  // [ld][NFOC]
+  // N^ bin column in shared memory.  A lane always reads the four shots 4c .. 4c+3 of its 256-bit chunk c, so the natural
+  // [shot][focal] order puts the lanes 32 NFOC bytes apart: for NFOC = 4, 8 every lane of a warp hits the same banks
+  // (measured: 436 / 778 us against 210 us at NFOC = 3).  NFOC >= 4 therefore keeps x as [focal][e][chunk]: the lanes of
+  // one load are consecutive.
+  float2* x = reinterpret_cast<float2*>(smem4);
   const int kk = blockIdx.x;
   const int r_begin = blockIdx.y * kRowsPerCta;
   const int r_end = min(r_begin + kRowsPerCta, n);
-  {
+  const int nchunk = ld >> 2;  // 256-bit chunk = 4 complex (ld is a multiple of 16)
+  constexpr bool kTransposed = NFOC >= 4;
+  if (!kTransposed) {
     const float4* src = reinterpret_cast<const float4*>(Nhat + (size_t)kk * ld * NFOC);
-    const int nvec = ld * NFOC / 2;
-    for (int i = threadIdx.x; i < nvec; i += kThreads) smem4[i] = __ldg(src + i);
+    for (int i = threadIdx.x; i < ld * NFOC / 2; i += kThreads) smem4[i] = __ldg(src + i);
+  } else {
+    const float2* src = Nhat + (size_t)kk * ld * NFOC;
+    for (int i = threadIdx.x; i < ld * NFOC; i += kThreads) {
+      const int s = i / NFOC, f = i - s * NFOC;
+      x[(f * 4 + (s & 3)) * nchunk + (s >> 2)] = __ldg(src + i);
+    }
   }
   __syncthreads();
   constexpr int kRows = Tune<NFOC>::kRows;
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  const int nchunk = ld >> 2;  // 256-bit chunk = 4 complex (ld is a multiple of 16)
   for (int r0 = r_begin + warp * kRows; r0 < r_end; r0 += kWarps * kRows) {
     const float* row[kRows];
 #pragma unroll
@@ -80,7 +94,7 @@ __global__ void __launch_bounds__(kThreads, Tune<NFOC>::kMinBlocks) k_syn_gemv(c
       for (int e = 0; e < 4; ++e)
 #pragma unroll
         for (int f = 0; f < NFOC; ++f) {
-          const float2 xv = x[(4 * c + e) * NFOC + f];
+          const float2 xv = kTransposed ? x[(f * 4 + e) * nchunk + c] : x[(4 * c + e) * NFOC + f];
 #pragma unroll
           for (int i = 0; i < kRows; ++i) cfma(acc[i][f], a[i].v[2 * e], a[i].v[2 * e + 1], xv);
         }

@@ -30,6 +30,8 @@
 //               tcgen05.ld 32x32b -> += 128 running sums in registers; per tile 128-bit global stores of S^
 #include <cuda.h>
 
+#include <algorithm>
+
 #include "mk_internal.cuh"
 
 namespace mk {
@@ -40,15 +42,16 @@ constexpr int BM = 128;        // rows (receivers) per tile = TMEM lanes
 constexpr int BN = 256;        // real columns (2 per focal point) per tile = TMEM columns per accumulator
 constexpr int BK = 16;         // k' (floats of the interleaved shot dimension) per stage: 64-byte rows of A'
 constexpr int UK = 8;          // k' per tcgen05.mma (kind::tf32)
-constexpr int STAGES = 4;
+constexpr int kMaxStages = 12;  // the ring has as many stages as fit (4 at N = 256, 11 for a single column block)
 constexpr int kThreads = 384;  // 12 warps
 constexpr int kChunkKb = 4;    // k'-blocks per accumulation chunk (24 MMA steps)
 constexpr int kSplitThreads = 64, kEpiWarps = 8;
 constexpr uint32_t A_BYTES = BM * BK * 4;   // 8 KB
-constexpr uint32_t B_BYTES = BK * BN * 4;   // 16 KB
-constexpr uint32_t STAGE_BYTES = 2 * A_BYTES + 2 * B_BYTES;  // A raw, A lo, B hi, B lo = 48 KB
-constexpr uint32_t TX_BYTES = A_BYTES + 2 * B_BYTES;
-constexpr size_t kSmemBytes = (size_t)STAGES * STAGE_BYTES + 1024 /*alignment slack*/ + 256 /*barriers*/;
+constexpr uint32_t BLK_BYTES = BK * 32 * 4;  // one 32-column block of a B' tile: 2 KB
+// A stage = A raw, A lo (8 KB each), B hi, B lo (nblk column blocks each, nblk = min(8, ceil(columns / 32))): narrow
+// focal batches move and hold only the columns they have, and get a deeper ring for it (HBM-bound regime)
+__host__ __device__ constexpr uint32_t stage_bytes(int nblk) { return 2 * A_BYTES + 2 * (uint32_t)nblk * BLK_BYTES; }
+constexpr size_t kSmemExtra = 1024 /*alignment slack*/ + 512 /*barriers*/;
 constexpr uint32_t kTmemCols = 512;
 
 // ---------------------------------------------------------------------------------------------- PTX wrappers
@@ -131,6 +134,7 @@ struct TcParams {
   int n, nb, ld;        // receivers, bins, padded shots
   int ncols;            // 2 * ldf: valid real columns of S^
   int mt, ntl;          // tiles along M and N
+  int nblk, stages;     // column blocks per B' tile, stages of the ring
   size_t s_row;         // floats between consecutive receivers of S^: nb * 2 ldf
 };
 
@@ -139,11 +143,13 @@ k_syn_gemm_tf32x3(const __grid_constant__ CUtensorMap tmA, const __grid_constant
                   const __grid_constant__ CUtensorMap tmBlo, float* __restrict__ Shat, TcParams P) {
   extern __shared__ uint8_t smem_raw[];
   uint8_t* smem = reinterpret_cast<uint8_t*>(((uintptr_t)smem_raw + 1023) & ~(uintptr_t)1023);
+  const int STAGES = P.stages;
+  const uint32_t STAGE_BYTES = stage_bytes(P.nblk), B_BYTES = (uint32_t)P.nblk * BLK_BYTES, TX_BYTES = A_BYTES + 2 * B_BYTES;
   uint64_t* bars = reinterpret_cast<uint64_t*>(smem + (size_t)STAGES * STAGE_BYTES);
-  uint64_t* full = bars;                   // [STAGES] TMA landed
-  uint64_t* empty = bars + STAGES;         // [STAGES] MMAs of the stage retired
-  uint64_t* split = bars + 2 * STAGES;     // [STAGES] Alo written
-  uint64_t* acc_full = bars + 3 * STAGES;  // [2] chunk accumulator complete
+  uint64_t* full = bars;                      // [kMaxStages] TMA landed
+  uint64_t* empty = bars + kMaxStages;        // [kMaxStages] MMAs of the stage retired
+  uint64_t* split = bars + 2 * kMaxStages;    // [kMaxStages] Alo written
+  uint64_t* acc_full = bars + 3 * kMaxStages; // [2] chunk accumulator complete
   uint64_t* acc_empty = acc_full + 2;      // [2] chunk accumulator drained
   uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(acc_empty + 2);
 
@@ -175,24 +181,29 @@ k_syn_gemm_tf32x3(const __grid_constant__ CUtensorMap tmA, const __grid_constant
   if (warp == 0) {
     // ------------------------------------------------------------------------------------ TMA producer
     if (lane == 0) {
-      uint32_t it = 0;
+      int s = 0;
+      uint32_t ph = 0;  // ring position and its phase, kept incrementally (the ring length is a run-time value)
       for (int t = blockIdx.x; t < ntiles; t += gridDim.x) {
         const int kk = t / per_bin, rem = t - kk * per_bin, mi = rem / P.ntl, ni = rem - mi * P.ntl;
-        for (int kb = 0; kb < KB; ++kb, ++it) {
-          const int s = it % STAGES;
-          mbar_wait(empty + s, ((it / STAGES) & 1) ^ 1);
+        for (int kb = 0; kb < KB; ++kb) {
+          mbar_wait(empty + s, ph ^ 1);
           uint8_t* st = smem + (size_t)s * STAGE_BYTES;
           mbar_expect_tx(full + s, TX_BYTES);
           tma_load_3d(&tmA, full + s, st, kb * BK, kk, mi * BM);
           tma_load_3d(&tmBhi, full + s, st + 2 * A_BYTES, 0, kk * 2 * P.ld + kb * BK, ni * (BN / 32));
           tma_load_3d(&tmBlo, full + s, st + 2 * A_BYTES + B_BYTES, 0, kk * 2 * P.ld + kb * BK, ni * (BN / 32));
+          if (++s == STAGES) {
+            s = 0;
+            ph ^= 1;
+          }
         }
       }
     }
   } else if (warp == 1) {
     // ------------------------------------------------------------------------------------ MMA issuer
     if (lane == 0) {
-      uint32_t it = 0, chunk_it = 0;
+      uint32_t chunk_it = 0, ph = 0;
+      int s = 0;
       for (int t = blockIdx.x; t < ntiles; t += gridDim.x) {
         const int rem = t % per_bin, ni = rem % P.ntl;
         int nmma = P.ncols - ni * BN;
@@ -204,9 +215,7 @@ k_syn_gemm_tf32x3(const __grid_constant__ CUtensorMap tmA, const __grid_constant
           tc_fence_after();
           const uint32_t d = tmem_base + (uint32_t)b * BN;
           const int kb1 = min(kb0 + kChunkKb, KB);
-          for (int kb = kb0; kb < kb1; ++kb, ++it) {
-            const int s = it % STAGES;
-            const uint32_t ph = (it / STAGES) & 1;
+          for (int kb = kb0; kb < kb1; ++kb) {
             mbar_wait(full + s, ph);
             mbar_wait(split + s, ph);
             tc_fence_after();
@@ -227,6 +236,10 @@ k_syn_gemm_tf32x3(const __grid_constant__ CUtensorMap tmA, const __grid_constant
               umma_tf32(d, da_raw, db_hi, idesc, 1);
             }
             umma_commit(empty + s);
+            if (++s == STAGES) {
+              s = 0;
+              ph ^= 1;
+            }
           }
           umma_commit(acc_full + b);
         }
@@ -235,11 +248,11 @@ k_syn_gemm_tf32x3(const __grid_constant__ CUtensorMap tmA, const __grid_constant
   } else if (warp < 4) {
     // ------------------------------------------------------------------------------------ split warps: Alo = A - tf32_trunc(A)
     const int tid = threadIdx.x - 64;  // 0..63
-    uint32_t it = 0;
+    int s = 0;
+    uint32_t ph = 0;
     for (int t = blockIdx.x; t < ntiles; t += gridDim.x) {
-      for (int kb = 0; kb < KB; ++kb, ++it) {
-        const int s = it % STAGES;
-        mbar_wait(full + s, (it / STAGES) & 1);
+      for (int kb = 0; kb < KB; ++kb) {
+        mbar_wait(full + s, ph);
         const float4* src = reinterpret_cast<const float4*>(smem + (size_t)s * STAGE_BYTES);
         float4* dst = reinterpret_cast<float4*>(smem + (size_t)s * STAGE_BYTES + A_BYTES);
         float4 v[(A_BYTES / 16) / kSplitThreads];
@@ -257,6 +270,10 @@ k_syn_gemm_tf32x3(const __grid_constant__ CUtensorMap tmA, const __grid_constant
         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");  // generic-proxy writes -> visible to the tensor core
         __syncwarp();
         if (lane == 0) mbar_arrive(split + s);
+        if (++s == STAGES) {
+          s = 0;
+          ph ^= 1;
+        }
       }
     }
   } else {
@@ -343,7 +360,7 @@ bool tc_supported(const mk_ctx* c) {
   int dev = 0, major = 0;
   if (cudaGetDevice(&dev) != cudaSuccess) return false;
   cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev);
-  return major == 10 && c->smem_optin >= kSmemBytes;
+  return major == 10 && c->smem_optin >= 2 * stage_bytes(1) + kSmemExtra;
 }
 
 int launch_syn_tc(mk_ctx* c, int slot, const float* d_Bhi, const float* d_Blo, float2* d_Shat, int nfoc, int ldf, int ldb) {
@@ -358,12 +375,13 @@ int launch_syn_tc(mk_ctx* c, int slot, const float* d_Bhi, const float* d_Blo, f
     if (int rc = encode3(c, enc, c->tmap_A, c->d_Rhat, dims, str, box, CU_TENSOR_MAP_SWIZZLE_64B, "A")) return rc;
     c->tmap_A_ok = true;
   }
+  const int nblk = std::min(BN / 32, (2 * ldf + 31) / 32);
   if (c->tmap_B_key[slot] != d_Bhi || c->tmap_B_ldb[slot] != ldb) {
     // B' plane [nb * 2 ld rows][ldb] seen as (column in block, row, column block): box = 32 x 16 x 8 lands in shared
     // memory as [8 column blocks][16 rows][128 B], the MN-major SWIZZLE_128B_BASE32B operand layout
     const cuuint64_t dims[3] = {32, (cuuint64_t)c->nb * 2 * c->ld, (cuuint64_t)ldb / 32};
     const cuuint64_t str[2] = {(cuuint64_t)ldb * 4, 128};
-    const cuuint32_t box[3] = {32, BK, BN / 32};
+    const cuuint32_t box[3] = {32, BK, (cuuint32_t)nblk};  // ldb is a function of nfoc, so is nblk: one cache key
     if (int rc = encode3(c, enc, c->tmap_B[slot][0], d_Bhi, dims, str, box, CU_TENSOR_MAP_SWIZZLE_128B_ATOM_32B, "B hi")) return rc;
     if (int rc = encode3(c, enc, c->tmap_B[slot][1], d_Blo, dims, str, box, CU_TENSOR_MAP_SWIZZLE_128B_ATOM_32B, "B lo")) return rc;
     c->tmap_B_key[slot] = d_Bhi;
@@ -377,6 +395,10 @@ int launch_syn_tc(mk_ctx* c, int slot, const float* d_Bhi, const float* d_Blo, f
   P.mt = (c->nrow + BM - 1) / BM;
   P.ntl = (P.ncols + BN - 1) / BN;
   P.s_row = (size_t)c->nb * 2 * ldf;
+  P.nblk = nblk;
+  P.stages = (int)std::min<size_t>(kMaxStages, (c->smem_optin - kSmemExtra) / stage_bytes(nblk));
+  if (P.stages < 2) return set_err(c, MK_ERR_INVALID_ARG, "not enough shared memory for the tcgen05 contraction");
+  const size_t kSmemBytes = (size_t)P.stages * stage_bytes(nblk) + kSmemExtra;
   if (int rc = check_cuda(c, cudaFuncSetAttribute(k_syn_gemm_tf32x3, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemBytes),
                           "cudaFuncSetAttribute"))
     return rc;
