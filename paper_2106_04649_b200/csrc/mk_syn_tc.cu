@@ -161,7 +161,7 @@ k_syn_gemm_tf32x3(const __grid_constant__ CUtensorMap tmA, const __grid_constant
     for (int s = 0; s < STAGES; ++s) {
       mbar_init(full + s, 1);
       mbar_init(empty + s, 1);
-      mbar_init(split + s, kSplitThreads / 32);
+      mbar_init(split + s, 1);
     }
     for (int b = 0; b < 2; ++b) {
       mbar_init(acc_full + b, 1);
@@ -247,29 +247,37 @@ k_syn_gemm_tf32x3(const __grid_constant__ CUtensorMap tmA, const __grid_constant
     }
   } else if (warp < 4) {
     // ------------------------------------------------------------------------------------ split warps: Alo = A - tf32_trunc(A)
-    const int tid = threadIdx.x - 64;  // 0..63
+    // The two warps take ALTERNATE stages (a whole A tile each): the generic -> async proxy fence that must follow the
+    // stores costs several hundred cycles, and this way two of them are in flight.
+    const int sw = warp - 2;  // 0, 1
     int s = 0;
-    uint32_t ph = 0;
+    uint32_t ph = 0, cnt = 0;
     for (int t = blockIdx.x; t < ntiles; t += gridDim.x) {
-      for (int kb = 0; kb < KB; ++kb) {
-        mbar_wait(full + s, ph);
-        const float4* src = reinterpret_cast<const float4*>(smem + (size_t)s * STAGE_BYTES);
-        float4* dst = reinterpret_cast<float4*>(smem + (size_t)s * STAGE_BYTES + A_BYTES);
-        float4 v[(A_BYTES / 16) / kSplitThreads];
+      for (int kb = 0; kb < KB; ++kb, ++cnt) {
+        if ((int)(cnt & 1) == sw) {
+          mbar_wait(full + s, ph);
+          const float4* src = reinterpret_cast<const float4*>(smem + (size_t)s * STAGE_BYTES);
+          float4* dst = reinterpret_cast<float4*>(smem + (size_t)s * STAGE_BYTES + A_BYTES);
+          constexpr int kPer = (int)(A_BYTES / 16) / 32;  // 16 float4 per lane
 #pragma unroll
-        for (int i = 0; i < (int)(A_BYTES / 16) / kSplitThreads; ++i) v[i] = src[tid + i * kSplitThreads];
+          for (int h = 0; h < 2; ++h) {
+            float4 v[kPer / 2];
 #pragma unroll
-        for (int i = 0; i < (int)(A_BYTES / 16) / kSplitThreads; ++i) {
-          float4 l;
-          l.x = v[i].x - __uint_as_float(__float_as_uint(v[i].x) & 0xffffe000u);
-          l.y = v[i].y - __uint_as_float(__float_as_uint(v[i].y) & 0xffffe000u);
-          l.z = v[i].z - __uint_as_float(__float_as_uint(v[i].z) & 0xffffe000u);
-          l.w = v[i].w - __uint_as_float(__float_as_uint(v[i].w) & 0xffffe000u);
-          dst[tid + i * kSplitThreads] = l;
+            for (int i = 0; i < kPer / 2; ++i) v[i] = src[lane + (h * (kPer / 2) + i) * 32];
+#pragma unroll
+            for (int i = 0; i < kPer / 2; ++i) {
+              float4 l;
+              l.x = v[i].x - __uint_as_float(__float_as_uint(v[i].x) & 0xffffe000u);
+              l.y = v[i].y - __uint_as_float(__float_as_uint(v[i].y) & 0xffffe000u);
+              l.z = v[i].z - __uint_as_float(__float_as_uint(v[i].z) & 0xffffe000u);
+              l.w = v[i].w - __uint_as_float(__float_as_uint(v[i].w) & 0xffffe000u);
+              dst[lane + (h * (kPer / 2) + i) * 32] = l;
+            }
+          }
+          asm volatile("fence.proxy.async.shared::cta;" ::: "memory");  // generic-proxy writes -> visible to the tensor core
+          __syncwarp();
+          if (lane == 0) mbar_arrive(split + s);
         }
-        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");  // generic-proxy writes -> visible to the tensor core
-        __syncwarp();
-        if (lane == 0) mbar_arrive(split + s);
         if (++s == STAGES) {
           s = 0;
           ph ^= 1;
