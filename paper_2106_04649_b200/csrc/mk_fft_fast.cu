@@ -188,12 +188,20 @@ __device__ __forceinline__ void spectrum_in(float2* smem, int nf, int lgFT, bool
 // P5.  emit(tl, kk, X[klo + kk]) for every in-band bin of every trace; CTA-wide, trace index fastest
 template <int HF, typename Emit>
 __device__ __forceinline__ void band_out(const float2* smem, int nf, int lgFT, const FastParams& P, Emit emit) {
-  constexpr int TS = Geo<HF>::TS;
-  const int FT = 1 << lgFT, total = P.nb << lgFT;
-  for (int idx = threadIdx.x; idx < total; idx += blockDim.x) {
-    const int kk = idx >> lgFT, tl = idx & (FT - 1);
-    if (tl >= nf) continue;
-    emit(tl, kk, rfft_bin_fast<HF>(smem + tl * TS, P.tw, P.klo + kk));
+  constexpr int TS = Geo<HF>::TS, kBatch = 4;
+  const int FT = 1 << lgFT, total = P.nb << lgFT, nthr = blockDim.x;
+  for (int i0 = threadIdx.x; i0 < total; i0 += kBatch * nthr) {
+    float2 X[kBatch];
+#pragma unroll
+    for (int u = 0; u < kBatch; ++u) {  // shared-memory and twiddle loads of the whole batch first
+      const int idx = i0 + u * nthr;
+      if (idx < total && (idx & (FT - 1)) < nf) X[u] = rfft_bin_fast<HF>(smem + (idx & (FT - 1)) * TS, P.tw, P.klo + (idx >> lgFT));
+    }
+#pragma unroll
+    for (int u = 0; u < kBatch; ++u) {
+      const int idx = i0 + u * nthr;
+      if (idx < total && (idx & (FT - 1)) < nf) emit(idx & (FT - 1), idx >> lgFT, X[u]);
+    }
   }
 }
 
@@ -274,6 +282,50 @@ __device__ __forceinline__ void spectrum_in_pairs(float2* smem, int nf, int lgFT
         zt[a0] = make_float2(scale * (xr - o_i), scale * (xi + o_r));
         zt[a1] = make_float2(scale * (xr + o_i), scale * (o_r - xi));
       }
+    }
+  }
+}
+
+
+// The same for any FT with one focal point per thread (single-focal runs: FT = 1, S^ contiguous in the bin index)
+template <int HF, bool RMW>
+__device__ __forceinline__ void spectrum_in_singles(float2* smem, int nf, int lgFT, bool conj_in, const FastParams& P,
+                                                    const float2* __restrict__ Srow, float2* prow) {
+  constexpr int M = Geo<HF>::M, TS = Geo<HF>::TS, kBatch = 8;
+  const int nthr = blockDim.x, klo = P.klo, khi = P.klo + P.nb - 1, fm = (1 << lgFT) - 1;
+  const float scale = 1.0f / (2.0f * (float)M);
+  {
+    const int n0 = klo, n1 = M - 2 * khi - 1, nz = n0 + n1 + (klo - 1);
+    for (int idx = threadIdx.x; idx < (nz << lgFT); idx += nthr) {
+      const int tl = idx & fm, j = idx >> lgFT;
+      const int k = j < n0 ? j : (j < n0 + n1 ? khi + 1 + (j - n0) : M - klo + 1 + (j - n0 - n1));
+      if (tl < nf) smem[tl * TS + zaddr(k)] = make_float2(0.f, 0.f);
+    }
+  }
+  const int total = P.nb << lgFT;
+  for (int i0 = threadIdx.x; i0 < total; i0 += kBatch * nthr) {
+    float2 sv[kBatch], pv[kBatch], tw[kBatch];
+#pragma unroll
+    for (int u = 0; u < kBatch; ++u) {
+      const int idx = i0 + u * nthr;
+      if (idx < total && (idx & fm) < nf) {
+        const size_t o = (size_t)(idx >> lgFT) * P.ldf + (idx & fm);
+        sv[u] = __ldg(Srow + o);
+        if (RMW) pv[u] = prow[o];
+        tw[u] = __ldg(P.tw + klo + (idx >> lgFT));
+      }
+    }
+#pragma unroll
+    for (int u = 0; u < kBatch; ++u) {
+      const int idx = i0 + u * nthr;
+      if (idx >= total || (idx & fm) >= nf) continue;
+      const int kk = idx >> lgFT, tl = idx & fm, k = klo + kk;
+      if (RMW) prow[(size_t)kk * P.ldf + tl] = make_float2(pv[u].x + sv[u].x, pv[u].y + sv[u].y);
+      const float xr = sv[u].x, xi = conj_in ? -sv[u].y : sv[u].y;
+      const float o_r = xr * tw[u].x + xi * tw[u].y, o_i = xi * tw[u].x - xr * tw[u].y;
+      float2* zt = smem + tl * TS;
+      zt[zaddr(k)] = make_float2(scale * (xr - o_i), scale * (xi + o_r));
+      zt[zaddr(M - k)] = make_float2(scale * (xr + o_i), scale * (o_r - xi));
     }
   }
 }
@@ -406,6 +458,8 @@ k_inv_fast(const float2* __restrict__ spec, FastParams P, int lgFT, float* __res
   const float2* srow = spec + (size_t)r * P.nb * P.ldf + f0;
   if (lgFT >= 2 && (P.ldf & 1) == 0 && simple_band(P, Geo<HF>::M)) {
     spectrum_in_pairs<HF, false>(smem, nf, lgFT, false, P, srow, nullptr);
+  } else if (simple_band(P, Geo<HF>::M)) {
+    spectrum_in_singles<HF, false>(smem, nf, lgFT, false, P, srow, nullptr);
   } else {
     spectrum_in<HF>(
         smem, nf, lgFT, false, P, [&](int tl, int kk, float2&) { return __ldg(srow + (size_t)kk * P.ldf + tl); },
@@ -464,6 +518,8 @@ k_post_fast(const float2* __restrict__ Shat, float2* __restrict__ phat, OperandO
   // a3: p^ += S^   [PAPER.md:79]
   if (pairs && simple_band(P, Geo<HF>::M)) {
     spectrum_in_pairs<HF, true>(smem, nf, lgFT, parity_even == 0, P, Shat + rowoff, phat + rowoff);
+  } else if (simple_band(P, Geo<HF>::M)) {
+    spectrum_in_singles<HF, true>(smem, nf, lgFT, parity_even == 0, P, Shat + rowoff, phat + rowoff);
   } else {
     spectrum_in<HF>(
         smem, nf, lgFT, parity_even == 0, P,
