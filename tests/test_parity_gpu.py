@@ -211,3 +211,46 @@ def test_row_sharded_contexts_reproduce_the_single_context(k, n, nt, nfoc, regim
     finally:
         for mk in mks:
             mk.close()
+
+
+# ---------------------------------------------------------------- error behaviour and degenerate runs through the C ABI
+def test_error_paths_and_degenerate_runs():
+    import torch
+    from paper_2106_04649_b200 import binding as B
+    n, nt, dt, dx = 12, 64, 0.004, 10.0
+    dev = torch.device("cuda:0")
+    rng = np.random.default_rng(5)
+    R = torch.from_numpy(rng.standard_normal((n, n, nt)).astype(np.float32)).to(dev)
+    Gd = torch.from_numpy(rng.standard_normal((2, n, nt)).astype(np.float32)).to(dev)
+    td = torch.full((2, n), 0.05, dtype=torch.float32, device=dev)
+    outs = {nm: torch.empty((2, n, nt), dtype=torch.float32, device=dev) for nm in ("f1plus", "f1min", "G")}
+    with B.Marchenko(n, n, nt, dt, dx, 10.0, 100.0) as mk:
+        mk.load_R(R[:5].contiguous(), 0)
+        with pytest.raises(B.MkError) as e:                      # a run before every shot is loaded is an error, not a silent zero
+            mk.run(Gd, td, 2, outs)
+        assert e.value.code == B.MK_ERR_STATE
+        with pytest.raises(B.MkError):
+            mk.load_R(R[:5].contiguous(), 9)                     # shot range past the end
+        with pytest.raises(B.MkError):
+            mk.step()                                            # step before begin
+        mk.load_R(R[5:].contiguous(), 5)
+        with pytest.raises(B.MkError):
+            mk.set_option(B.MK_OPT_FFT_PATH, 2)                  # register-resident transforms need nt = 2048 / 4096
+        mk.set_option(B.MK_OPT_REGIME, 1)
+        Gd9 = torch.zeros((9, n, nt), dtype=torch.float32, device=dev)
+        with pytest.raises(B.MkError):
+            mk.begin(Gd9, torch.zeros((9, n), dtype=torch.float32, device=dev))   # the streaming GEMV takes at most 8 focal points
+        mk.set_option(B.MK_OPT_REGIME, 0)
+        with pytest.raises(B.MkError):
+            mk.run(Gd, td, 0, {"N_last": outs["G"]})             # N_last of a run without iterations
+        # niter = 0: f1plus = N_{-1} = T G_d, f1min = 0, G = p^- + T f2 = G_d   [PAPER.md:19, 67, 74-75]
+        mk.run(Gd, td, 0, outs)
+        torch.cuda.synchronize()
+        g = Gd.cpu().numpy()
+        np.testing.assert_array_equal(outs["f1plus"].cpu().numpy(), np.roll(g[..., ::-1], 1, axis=-1))
+        assert float(outs["f1min"].abs().max()) == 0.0
+        assert rel_l2(outs["G"].cpu().numpy(), g) < 1e-6
+        # the context stays usable after errors
+        mk.run(Gd, td, 1, outs)
+        torch.cuda.synchronize()
+        assert np.isfinite(outs["G"].cpu().numpy()).all()
