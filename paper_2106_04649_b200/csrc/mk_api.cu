@@ -288,6 +288,8 @@ int mk_destroy(mk_ctx* c) {
   cudaFree(c->d_Bhi2);
   cudaFree(c->d_Blo2);
   cudaFree(c->d_stage);
+  if (c->copy_stream) cudaStreamDestroy(c->copy_stream);
+  if (c->copy_ev) cudaEventDestroy(c->copy_ev);
   for (cudaEvent_t e : c->ev) cudaEventDestroy(e);
   cudaGetLastError();
   delete c;
@@ -549,33 +551,53 @@ int mk_run_host(mk_ctx* c, const float* h_Gd, const float* h_td, int nfoc, int n
   if (!h_Gd || !h_td || nfoc <= 0 || niter < 0 || !ho) return set_err(c, MK_ERR_INVALID_ARG, "mk_run_host: bad arguments");
   if (ho->N_last && niter == 0) return set_err(c, MK_ERR_INVALID_ARG, "N_last needs niter >= 1");
   const size_t ntime = (size_t)nfoc * c->n * c->nt, ntd = (size_t)nfoc * c->n;
-  if (int rc = ensure(c, &c->d_stage, &c->cap_stage, ntime + ntd, "staging")) return rc;
+  // Small runs get one staging field per output, and the device -> host copies go to a second stream so that they
+  // overlap the finals' syntheses; big ones (> 256 MiB per field) share one staging field and stay on one stream.
+  const bool overlap = ntime * sizeof(float) <= ((size_t)256 << 20);
+  const int nstage = overlap ? 4 : 1;
+  if (int rc = ensure(c, &c->d_stage, &c->cap_stage, nstage * ntime + ntd, "staging")) return rc;
   float* d_field = c->d_stage;
-  float* d_td = c->d_stage + ntime;
+  float* d_td = c->d_stage + nstage * ntime;
+  if (overlap && !c->copy_stream) {
+    if (int rc = check_cuda(c, cudaStreamCreateWithFlags(&c->copy_stream, cudaStreamNonBlocking), "cudaStreamCreate")) return rc;
+    if (int rc = check_cuda(c, cudaEventCreateWithFlags(&c->copy_ev, cudaEventDisableTiming), "cudaEventCreate")) return rc;
+  }
+  cudaStream_t cs = overlap ? c->copy_stream : c->stream;
+  // everything enqueued on the main stream so far may be copied out on the copy stream
+  auto hand_over = [&]() -> int {
+    if (!overlap) return MK_OK;
+    if (int rc = check_cuda(c, cudaEventRecord(c->copy_ev, c->stream), "cudaEventRecord")) return rc;
+    return check_cuda(c, cudaStreamWaitEvent(cs, c->copy_ev, 0), "cudaStreamWaitEvent");
+  };
   if (int rc = check_cuda(c, cudaMemcpyAsync(d_field, h_Gd, ntime * sizeof(float), cudaMemcpyHostToDevice, c->stream), "H2D G_d")) return rc;
   if (int rc = check_cuda(c, cudaMemcpyAsync(d_td, h_td, ntd * sizeof(float), cudaMemcpyHostToDevice, c->stream), "H2D t_d")) return rc;
   if (int rc = mk_begin(c, d_field, d_td, nfoc)) return rc;
   for (int i = 0; i < niter; ++i) {
     const bool last = (i == niter - 1) && ho->N_last;
     if (int rc = mk_step(c, last ? d_field : nullptr)) return rc;
-    if (last)
-      if (int rc = check_cuda(c, cudaMemcpyAsync(ho->N_last, d_field, ntime * sizeof(float), cudaMemcpyDeviceToHost, c->stream), "D2H N_last")) return rc;
   }
+  if (int rc = hand_over()) return rc;
+  if (ho->N_last)
+    if (int rc = check_cuda(c, cudaMemcpyAsync(ho->N_last, d_field, ntime * sizeof(float), cudaMemcpyDeviceToHost, cs), "D2H N_last")) return rc;
   float* hosts[5] = {ho->f1plus, ho->f1min, ho->G, ho->Gplus, ho->Gminus};
   for (int i = 0; i < 5; ++i) {
     if (!hosts[i]) continue;
-    if (i == 0 || i == 1) {  // accumulators go straight from the library's buffers
+    if (i == 0 || i == 1) {  // accumulators go straight from the library's buffers (the finals only read them)
       const float* src = i == 0 ? c->d_f1plus : c->d_f1min;
-      if (int rc = check_cuda(c, cudaMemcpyAsync(hosts[i], src, ntime * sizeof(float), cudaMemcpyDeviceToHost, c->stream), "D2H accumulator")) return rc;
+      if (int rc = check_cuda(c, cudaMemcpyAsync(hosts[i], src, ntime * sizeof(float), cudaMemcpyDeviceToHost, cs), "D2H accumulator")) return rc;
       continue;
     }
+    float* d_out = overlap ? d_field + (size_t)(i - 1) * ntime : d_field;  // fields 1..3 of the staging area; field 0 holds N_last
     mk_outputs one{};
-    if (i == 2) one.G = d_field;
-    if (i == 3) one.Gplus = d_field;
-    if (i == 4) one.Gminus = d_field;
+    if (i == 2) one.G = d_out;
+    if (i == 3) one.Gplus = d_out;
+    if (i == 4) one.Gminus = d_out;
     if (int rc = mk_finish(c, &one)) return rc;
-    if (int rc = check_cuda(c, cudaMemcpyAsync(hosts[i], d_field, ntime * sizeof(float), cudaMemcpyDeviceToHost, c->stream), "D2H output")) return rc;
+    if (int rc = hand_over()) return rc;
+    if (int rc = check_cuda(c, cudaMemcpyAsync(hosts[i], d_out, ntime * sizeof(float), cudaMemcpyDeviceToHost, cs), "D2H output")) return rc;
   }
+  if (overlap)
+    if (int rc = check_cuda(c, cudaStreamSynchronize(cs), "cudaStreamSynchronize")) return rc;
   return check_cuda(c, cudaStreamSynchronize(c->stream), "cudaStreamSynchronize");
 }
 

@@ -72,6 +72,8 @@ struct mk_ctx {
   int tmap_B_ldb[2] = {0, 0};
   void* encode_fn = nullptr;  // cuTensorMapEncodeTiled, resolved at run time through the CUDA runtime
   float* d_stage = nullptr;  // host-call staging
+  cudaStream_t copy_stream = nullptr;  // mk_run_host: device -> host copies overlapping the finals
+  cudaEvent_t copy_ev = nullptr;
   size_t cap_stage = 0;
   float* d_Gminus = nullptr;  // kept by mk_finish when G^- was requested (mk_image)
   size_t cap_Gminus = 0;
