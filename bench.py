@@ -199,7 +199,7 @@ def run_ours(args):
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     dev = torch.device("cuda", local)
 
-    rows_mode = args.parallel == "rows"
+    rows_mode = args.parallel in ("rows", "rows_fused")
     # weak scaling: replicas, no collective;  --parallel rows: ONE job, R^ split by receiver rows over the ranks
     cfg = configs.get(args.workload) if rows_mode else shard.replica_config(configs.get(args.workload), rank, world)
     my_rows = shard.row_slice(cfg.n, rank, world) if rows_mode else range(cfg.n)
@@ -211,7 +211,19 @@ def run_ours(args):
     mk = B.Marchenko(cfg.n, cfg.n, cfg.nt, cfg.dt, cfg.dx, cfg.fmin, cfg.fmax, rows=(my_rows.start, len(my_rows)))
     mk.set_option(B.MK_OPT_EPS_SAMPLES, cfg.eps)
     mk.set_option(B.MK_OPT_REGIME, args.regime)
-    if rows_mode:
+    ipc_ptrs = []
+    if args.parallel == "rows_fused":
+        if world > 1:
+            ipc_ptrs = shard.attach_ipc(mk, cfg.nfoc, dist)
+
+        def fused_barrier():
+            torch.cuda.synchronize()
+            if world > 1:
+                dist.barrier()
+
+        def run_step():
+            shard.run_row_sharded_fused(mk, dGd, dtd, niter, douts, fused_barrier)
+    elif rows_mode:
         if world > 1:
             exchange = shard.distributed_exchange(mk, dist)
         else:
@@ -294,6 +306,9 @@ def run_ours(args):
                "d2h_bytes_per_step": int(sum(t.numel() * 4 for t in houts.values())), "steps": e2e_steps,
                "ms_per_step": 1e3 * e2e_s / e2e_steps, "api": "mk_run_host (pinned host G_d, t_d in; 6 host fields out)"}
 
+    for ptr in ipc_ptrs:            # peers' operand mappings: closed on every rank before any context goes away
+        B.ipc_close(ptr)
+    barrier()
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
@@ -353,7 +368,9 @@ def run_ours(args):
                        "l2": f"inputs_larger_than_L2 (R^ {nbytes / 1e9:.2f} GB vs 126 MB L2; no flush needed)",
                        "input_source": "device generator, 64-shot chunks (no e2e / cpu_baseline legs)" if big else "host arrays",
                        "parallelism": "1 GPU" if world == 1 and not rows_mode else
-                                      (f"{world} ranks, receiver rows sharded, all-gather of the operand rows per synthesis" if rows_mode
+                                      (f"{world} ranks, receiver rows sharded, " + ("operand rows stored into the peers' operands by the producing kernels"
+                                                                                if args.parallel == "rows_fused" else
+                                                                                "all-gather of the operand rows per synthesis") if rows_mode
                                        else f"{world} independent replicas (no collective)")},
             "focal_point_iterations_per_s": jobs * nfoc * niter * args.steps / (ms_total * 1e-3),
             "clocks": clocks,
@@ -374,9 +391,10 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", type=int, default=1, help="BASELINE.json config index (default 1)")
     ap.add_argument("--regime", type=int, default=0)
-    ap.add_argument("--parallel", default="replicas", choices=["replicas", "rows"],
+    ap.add_argument("--parallel", default="replicas", choices=["replicas", "rows", "rows_fused"],
                     help="N > 1: independent replicas (default, weak scaling) or receiver-row sharding with one all-gather of the "
-                         "operand rows per synthesis (strong scaling; SURVEY.md section 8(e) / NEXT-3)")
+                         "operand rows per synthesis (strong scaling; SURVEY.md section 8(e) / NEXT-3); rows_fused: the same with the "
+                         "all-gather fused into the producing kernels as peer stores over CUDA IPC mappings (two barriers per synthesis)")
     ap.add_argument("--e2e-steps", type=int, default=50)
     ap.add_argument("--cpu-budget", type=float, default=15.0, help="seconds of oracle work for cpu_baseline")
     ap.add_argument("--no-cpu-baseline", action="store_true")

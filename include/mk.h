@@ -122,6 +122,11 @@ int mk_run_host(mk_ctx* ctx, const float* h_Gd, const float* h_td, int nfoc, int
 int mk_begin(mk_ctx* ctx, const float* d_Gd, const float* d_td, int nfoc); /* a1: N_{-1} = f1plus = T G_d, f1min = p^- = 0 */
 int mk_step(mk_ctx* ctx, float* d_N_i /* optional [nfoc][nrec][nt] copy of the new iterate, or NULL */); /* a2..a6 */
 int mk_finish(mk_ctx* ctx, const mk_outputs* d_out); /* a7; may be called more than once with different fields */
+/* mk_step in its two halves: the contraction a2 (reads the operand) and the fused pass a3..a6 (writes the operand of the
+ * next step).  With peers attached (mk_operand_attach) the second half stores into the peers' operands too, so every rank
+ * must have finished its contraction before any rank runs mk_step_post: put the cross-rank barrier between the two. */
+int mk_step_contract(mk_ctx* ctx);
+int mk_step_post(mk_ctx* ctx, float* d_N_i);
 
 /* One bare synthesis without window (a6 + a2 + a3): d_S_out = R d_N_in, both [nfoc][nrec][nt] fp32.
  * Does not disturb a run in progress.  This is the call the GB/s metric times. */
@@ -160,6 +165,25 @@ typedef struct mk_operand_view {
 } mk_operand_view;
 int mk_operand(mk_ctx* ctx, int slot, mk_operand_view* out);
 int mk_operand_exchanged(mk_ctx* ctx, int slot);
+
+/* The exchange fused into the producing kernels (section 8(e): "fused as peer stores from the FFT kernel's epilogue").
+ * mk_operand_reserve allocates and zeroes the operands of both slots for runs with nfoc focal points, so that their
+ * addresses exist before mk_begin; mk_operand_attach then registers, for one slot, the same slot's operand of up to 7
+ * other ranks (views of identical layout, device pointers valid in this process: other contexts of the process, or
+ * peer GPU memory mapped through CUDA IPC / peer access).  From then on every kernel of this context that produces
+ * operand rows (mk_begin, mk_step, mk_finish_prepare) stores them into its own operand AND, at the same offsets, into
+ * every attached one, so no copy is needed afterwards: the caller only has to make sure that all ranks have finished
+ * producing (a barrier across the ranks' streams) before it calls mk_operand_exchanged and the next contraction.
+ * npeers = 0 detaches.  The attachment is dropped when the operand layout changes (another nfoc or regime). */
+int mk_operand_reserve(mk_ctx* ctx, int nfoc);
+int mk_operand_attach(mk_ctx* ctx, int slot, int npeers, const mk_operand_view* peers);
+
+/* Plumbing for one process per GPU: CUDA IPC handles of operand planes (each plane is one device allocation), to be
+ * exchanged between the ranks by any host channel (torch.distributed all_gather_object) and opened by the peers.
+ * handle: 64 bytes.  A pointer opened here must be closed before the exporting context is destroyed. */
+int mk_ipc_export(const void* d_ptr, unsigned char handle[64]);
+int mk_ipc_open(const unsigned char handle[64], void** d_ptr);
+int mk_ipc_close(void* d_ptr);
 
 enum { MK_FIELD_GMINUS = 1, MK_FIELD_GPLUS = 2 };
 int mk_finish_prepare(mk_ctx* ctx, int field);                   /* forward transform of f1plus / T f1min -> slot 1 */

@@ -22,7 +22,8 @@ REGIME_AUTO, REGIME_GEMV, REGIME_GEMM_FFMA, REGIME_GEMM_TF32X3 = 0, 1, 2, 3
 # every symbol include/mk.h declares
 SYMBOLS = ("mk_create", "mk_destroy", "mk_set_stream", "mk_set_option", "mk_get_info", "mk_load_R", "mk_load_R_host",
            "mk_run", "mk_run_host", "mk_begin", "mk_step", "mk_finish", "mk_synthesis", "mk_image", "mk_last_error",
-           "mk_version", "mk_create_sharded", "mk_operand", "mk_operand_exchanged", "mk_finish_prepare", "mk_finish_complete")
+           "mk_version", "mk_create_sharded", "mk_operand", "mk_operand_exchanged", "mk_finish_prepare", "mk_finish_complete",
+           "mk_operand_reserve", "mk_operand_attach", "mk_step_contract", "mk_step_post", "mk_ipc_export", "mk_ipc_open", "mk_ipc_close")
 MK_FIELD_GMINUS, MK_FIELD_GPLUS = 1, 2
 
 
@@ -68,6 +69,8 @@ def load():
     L.mk_run_host.argtypes = [vp, vp, vp, ci, ci, C.POINTER(mk_outputs)]
     L.mk_begin.argtypes = [vp, vp, vp, ci]
     L.mk_step.argtypes = [vp, vp]
+    L.mk_step_contract.argtypes = [vp]
+    L.mk_step_post.argtypes = [vp, vp]
     L.mk_finish.argtypes = [vp, C.POINTER(mk_outputs)]
     L.mk_synthesis.argtypes = [vp, vp, vp, ci]
     L.mk_image.argtypes = [vp, vp, vp]
@@ -75,6 +78,11 @@ def load():
     L.mk_operand.argtypes = [vp, ci, C.POINTER(mk_operand_view)]
     L.mk_operand_exchanged.argtypes = [vp, ci]
     L.mk_finish_prepare.argtypes = [vp, ci]
+    L.mk_operand_reserve.argtypes = [vp, ci]
+    L.mk_operand_attach.argtypes = [vp, ci, ci, C.POINTER(mk_operand_view)]
+    L.mk_ipc_export.argtypes = [vp, C.c_char_p]
+    L.mk_ipc_open.argtypes = [C.c_char_p, C.POINTER(vp)]
+    L.mk_ipc_close.argtypes = [vp]
     L.mk_finish_complete.argtypes = [vp, ci, vp]
     L.mk_last_error.argtypes = [vp]
     L.mk_last_error.restype = C.c_char_p
@@ -217,6 +225,13 @@ class Marchenko:
         import torch
         self._check(self._L.mk_step(self._h, _dev_ptr(d_N_i, torch.float32, self._nfoc * self.nrec * self.nt) if d_N_i is not None else None))
 
+    def step_contract(self):
+        self._check(self._L.mk_step_contract(self._h))
+
+    def step_post(self, d_N_i=None):
+        import torch
+        self._check(self._L.mk_step_post(self._h, _dev_ptr(d_N_i, torch.float32, self._nfoc * self.nrec * self.nt) if d_N_i is not None else None))
+
     def finish(self, outs):
         import torch
         numel = self._nfoc * self.nrec * self.nt
@@ -243,6 +258,20 @@ class Marchenko:
             planes.append(torch.as_tensor(holder, device="cuda"))
         return planes, v
 
+    def operand_reserve(self, nfoc):
+        self._nfoc = nfoc
+        self._check(self._L.mk_operand_reserve(self._h, nfoc))
+
+    def operand_view(self, slot):
+        v = mk_operand_view()
+        self._check(self._L.mk_operand(self._h, slot, C.byref(v)))
+        return v
+
+    def operand_attach(self, slot, views):
+        """views: mk_operand_view structs of the peers' operands of the same slot (pointers valid in this process)."""
+        arr = (mk_operand_view * max(len(views), 1))(*views)
+        self._check(self._L.mk_operand_attach(self._h, slot, len(views), arr))
+
     def operand_exchanged(self, slot):
         self._check(self._L.mk_operand_exchanged(self._h, slot))
 
@@ -257,6 +286,26 @@ class Marchenko:
         import torch
         self._check(self._L.mk_image(self._h, _dev_ptr(d_Gminus, torch.float32, self._nfoc * self.nrec * self.nt),
                                      _dev_ptr(d_image, torch.float32, self._nfoc)))
+
+
+def ipc_export(ptr: int) -> bytes:
+    buf = C.create_string_buffer(64)
+    rc = load().mk_ipc_export(C.c_void_p(ptr), buf)
+    if rc != MK_OK:
+        raise MkError(rc, "cudaIpcGetMemHandle failed")
+    return buf.raw
+
+
+def ipc_open(handle: bytes) -> int:
+    p = C.c_void_p()
+    rc = load().mk_ipc_open(C.c_char_p(handle), C.byref(p))
+    if rc != MK_OK:
+        raise MkError(rc, "cudaIpcOpenMemHandle failed")
+    return p.value
+
+
+def ipc_close(ptr: int) -> None:
+    load().mk_ipc_close(C.c_void_p(ptr))
 
 
 def version() -> str:

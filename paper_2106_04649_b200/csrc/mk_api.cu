@@ -85,6 +85,13 @@ OperandOut operand_out(mk_ctx* c, int slot, int regime, int ldf, int ldb) {
   } else {
     O.plain = slot ? c->d_Nhat2 : c->d_Nhat;
   }
+  if (c->npeer[slot] > 0 && c->peer_key[slot] == c->operand_key[slot] && c->operand_key[slot] != 0) {
+    O.npeer = c->npeer[slot];
+    for (int p = 0; p < O.npeer; ++p) {
+      O.peer[p][0] = c->peer_plane[slot][p][0];
+      O.peer[p][1] = c->peer_plane[slot][p][1];
+    }
+  }
   return O;
 }
 
@@ -122,6 +129,13 @@ int prepare_operand(mk_ctx* c, int slot, int regime, int nfoc, int ldf, int ldb)
 }
 
 // a2: S^ = R^ x N^ per bin, on the context's stream; optionally bracketed by events
+// peers attached for another operand layout would silently receive nothing: refuse to produce rows then
+int check_peers(mk_ctx* c, int slot) {
+  if (c->npeer[slot] > 0 && c->peer_key[slot] != c->operand_key[slot])
+    return set_err(c, MK_ERR_STATE, "the operand layout changed since mk_operand_attach: reserve and attach again");
+  return MK_OK;
+}
+
 int contract(mk_ctx* c, int slot, float2* Shat, int nfoc, int ldf, int ldb, int regime) {
   if (c->operand_stale[slot])
     return set_err(c, MK_ERR_STATE, "row-sharded context: the operand rows were not exchanged (mk_operand / mk_operand_exchanged)");
@@ -414,12 +428,14 @@ int mk_begin(mk_ctx* c, const float* d_Gd, const float* d_td, int nfoc) {
   c->ldb = ldb;
   c->regime_used = regime;
   c->iter = 0;
+  c->contracted = false;
   c->have_Gminus = false;
   if (int rc = prepare_operand(c, 0, regime, nfoc, ldf, ldb)) return rc;
   if (int rc = check_cuda(c, cudaMemsetAsync(c->d_phat, 0, nS * sizeof(float2), c->stream), "memset phat")) return rc;
   if (int rc = check_cuda(c, cudaMemsetAsync(c->d_f1min, 0, ntime * sizeof(float), c->stream), "memset f1min")) return rc;
   if (int rc = launch_window(c, d_td, c->d_h, nfoc * c->n)) return rc;
   // a1: N_{-1} = f1plus = T G_d; N^_{-1} = conj(G_d^)     [PAPER.md:19, 67, 74-75]
+  if (int rc = check_peers(c, 0)) return rc;
   const bool sharded = c->nrow != c->n;
   if (sharded)  // the rows of other ranks stay zero in this rank's fields
     if (int rc = check_cuda(c, cudaMemsetAsync(c->d_f1plus, 0, ntime * sizeof(float), c->stream), "memset f1plus")) return rc;
@@ -429,15 +445,30 @@ int mk_begin(mk_ctx* c, const float* d_Gd, const float* d_td, int nfoc) {
   return MK_OK;
 }
 
-int mk_step(mk_ctx* c, float* d_N_i) {
+int mk_step_contract(mk_ctx* c) {
   MK_GUARD(c);
   if (!c->begun) return set_err(c, MK_ERR_STATE, "mk_step before mk_begin");
-  int regime = c->regime_used;
-  if (int rc = contract(c, 0, c->d_Shat, c->nfoc, c->ldf, c->ldb, regime)) return rc;                               // a2  [PAPER.md:69]
+  if (c->contracted) return set_err(c, MK_ERR_STATE, "mk_step_contract twice without mk_step_post");
+  if (int rc = contract(c, 0, c->d_Shat, c->nfoc, c->ldf, c->ldb, c->regime_used)) return rc;                       // a2  [PAPER.md:69]
+  c->contracted = true;
+  return MK_OK;
+}
+
+int mk_step_post(mk_ctx* c, float* d_N_i) {
+  MK_GUARD(c);
+  if (!c->begun || !c->contracted) return set_err(c, MK_ERR_STATE, "mk_step_post without mk_step_contract");
+  const int regime = c->regime_used;
+  if (int rc = check_peers(c, 0)) return rc;
   if (int rc = launch_post(c, operand_out(c, 0, regime, c->ldf, c->ldb), (c->iter % 2) == 0, d_N_i)) return rc;     // a3..a6
   c->operand_stale[0] = c->nrow != c->n;
+  c->contracted = false;
   ++c->iter;
   return MK_OK;
+}
+
+int mk_step(mk_ctx* c, float* d_N_i) {
+  if (int rc = mk_step_contract(c)) return rc;
+  return mk_step_post(c, d_N_i);
 }
 
 static int scratch_operands(mk_ctx* c, int regime, int nfoc, int ldf, int ldb) {
@@ -452,7 +483,6 @@ int mk_finish(mk_ctx* c, const mk_outputs* o) {
   if (!o) return set_err(c, MK_ERR_INVALID_ARG, "mk_finish: null outputs");
   if (o->N_last) return set_err(c, MK_ERR_INVALID_ARG, "N_last is delivered by mk_run (or by mk_step's d_N_i), not by mk_finish");
   const size_t bytes = (size_t)c->nfoc * c->n * c->nt * sizeof(float);
-  const int regime = c->regime_used;
   if (o->f1plus)
     if (int rc = check_cuda(c, cudaMemcpyAsync(o->f1plus, c->d_f1plus, bytes, cudaMemcpyDeviceToDevice, c->stream), "copy f1plus")) return rc;
   if (o->f1min)
@@ -481,6 +511,7 @@ int mk_finish_prepare(mk_ctx* c, int field) {
   if (int rc = scratch_operands(c, regime, c->nfoc, c->ldf, c->ldb)) return rc;
   // G^- = R f1plus - f1min [PAPER.md:87-88; G5]: operand = spectrum of f1plus;  G^+ = T f1plus - R (T f1min) [PAPER.md:24; G4]:
   // operand = spectrum of T f1min = conj of the spectrum of f1min
+  if (int rc = check_peers(c, 1)) return rc;
   const bool minus = field == MK_FIELD_GMINUS;
   if (int rc = launch_fwd(c, minus ? c->d_f1plus : c->d_f1min, operand_out(c, 1, regime, c->ldf, c->ldb), c->nfoc, !minus, nullptr)) return rc;
   c->operand_stale[1] = c->nrow != c->n;
@@ -502,7 +533,7 @@ int mk_finish_complete(mk_ctx* c, int field, float* d_out) {
 int mk_operand(mk_ctx* c, int slot, mk_operand_view* v) {
   MK_GUARD(c);
   if (!v || slot < 0 || slot > 1) return set_err(c, MK_ERR_INVALID_ARG, "mk_operand: bad arguments");
-  if (!c->begun) return set_err(c, MK_ERR_STATE, "mk_operand before mk_begin");
+  if (!c->begun && !c->reserved) return set_err(c, MK_ERR_STATE, "mk_operand before mk_begin / mk_operand_reserve");
   std::memset(v, 0, sizeof *v);
   v->nb = c->nb;
   v->row0 = c->r0;
@@ -529,6 +560,77 @@ int mk_operand_exchanged(mk_ctx* c, int slot) {
   MK_GUARD(c);
   if (slot < 0 || slot > 1) return set_err(c, MK_ERR_INVALID_ARG, "mk_operand_exchanged: bad slot");
   c->operand_stale[slot] = false;
+  return MK_OK;
+}
+
+int mk_ipc_export(const void* d_ptr, unsigned char handle[64]) {
+  static_assert(sizeof(cudaIpcMemHandle_t) == 64, "CUDA IPC handle size");
+  if (!d_ptr || !handle) return MK_ERR_INVALID_ARG;
+  cudaIpcMemHandle_t h;
+  if (cudaIpcGetMemHandle(&h, const_cast<void*>(d_ptr)) != cudaSuccess) {
+    cudaGetLastError();
+    return MK_ERR_CUDA;
+  }
+  std::memcpy(handle, &h, 64);
+  return MK_OK;
+}
+
+int mk_ipc_open(const unsigned char handle[64], void** d_ptr) {
+  if (!handle || !d_ptr) return MK_ERR_INVALID_ARG;
+  cudaIpcMemHandle_t h;
+  std::memcpy(&h, handle, 64);
+  if (cudaIpcOpenMemHandle(d_ptr, h, cudaIpcMemLazyEnablePeerAccess) != cudaSuccess) {
+    cudaGetLastError();
+    *d_ptr = nullptr;
+    return MK_ERR_CUDA;
+  }
+  return MK_OK;
+}
+
+int mk_ipc_close(void* d_ptr) {
+  if (!d_ptr) return MK_OK;
+  if (cudaIpcCloseMemHandle(d_ptr) != cudaSuccess) {
+    cudaGetLastError();
+    return MK_ERR_CUDA;
+  }
+  return MK_OK;
+}
+
+int mk_operand_reserve(mk_ctx* c, int nfoc) {
+  MK_GUARD(c);
+  if (nfoc <= 0) return set_err(c, MK_ERR_INVALID_ARG, "mk_operand_reserve: bad nfoc");
+  if (c->begun && nfoc != c->nfoc) c->begun = false;  // a run with another batch size is over
+  int regime = 0;
+  if (int rc = resolve_regime(c, nfoc, &regime)) return rc;
+  const int ldf = ldf_for(regime, nfoc), ldb = ldb_for(nfoc);
+  if (int rc = prepare_operand(c, 0, regime, nfoc, ldf, ldb)) return rc;
+  if (int rc = prepare_operand(c, 1, regime, nfoc, ldf, ldb)) return rc;
+  c->nfoc = nfoc;
+  c->ldf = ldf;
+  c->ldb = ldb;
+  c->regime_used = regime;
+  c->reserved = true;
+  return MK_OK;
+}
+
+int mk_operand_attach(mk_ctx* c, int slot, int npeers, const mk_operand_view* peers) {
+  MK_GUARD(c);
+  if (slot < 0 || slot > 1 || npeers < 0 || npeers > kMaxPeers || (npeers > 0 && !peers))
+    return set_err(c, MK_ERR_INVALID_ARG, "mk_operand_attach: bad arguments");
+  c->npeer[slot] = 0;
+  if (npeers == 0) return MK_OK;
+  mk_operand_view mine;
+  if (int rc = mk_operand(c, slot, &mine)) return rc;
+  for (int p = 0; p < npeers; ++p) {
+    const mk_operand_view& v = peers[p];
+    if (v.nplanes != mine.nplanes || v.nb != mine.nb || v.rows_per_bin != mine.rows_per_bin || v.rows_per_rec != mine.rows_per_rec ||
+        v.row_floats != mine.row_floats || !v.plane[0] || (v.nplanes == 2 && !v.plane[1]))
+      return set_err(c, MK_ERR_INVALID_ARG, "mk_operand_attach: a peer's operand has another layout");
+    c->peer_plane[slot][p][0] = v.plane[0];
+    c->peer_plane[slot][p][1] = v.plane[1];
+  }
+  c->npeer[slot] = npeers;
+  c->peer_key[slot] = c->operand_key[slot];
   return MK_OK;
 }
 

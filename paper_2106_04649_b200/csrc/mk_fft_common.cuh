@@ -12,21 +12,29 @@ __device__ __forceinline__ float tf32_rna(float v) {
   return __uint_as_float(u);
 }
 
-// a6 store: X = N^[k][r][f] in the layout the contraction of the active regime reads
-__device__ __forceinline__ void store_operand(const OperandOut& O, int ld, int kk, int r, int f, float2 X) {
-  if (O.bhi == nullptr) {
-    O.plain[((size_t)kk * ld + r) * O.ldf + f] = X;
-    return;
-  }
+// a6 store: X = N^[k][r][f] in the layout the contraction of the active regime reads, into this rank's operand and,
+// when peers are attached (row sharding), into theirs
+__device__ __forceinline__ void store_split_rows(float* hi, float* lo, size_t row0, int ldb, float2 X) {
   // regime 3 (mk_syn_tc.cu): real operand B' [nb][2 ld][ldb], rows (2r, 2r+1) = (X, iX) as interleaved floats,
   // split into a tf32 "hi" plane and a tf32 "lo" plane (3xTF32).
   const float hx = tf32_rna(X.x), hy = tf32_rna(X.y);
   const float lx = tf32_rna(X.x - hx), ly = tf32_rna(X.y - hy);
+  *reinterpret_cast<float2*>(hi + row0) = make_float2(hx, hy);
+  *reinterpret_cast<float2*>(hi + row0 + ldb) = make_float2(-hy, hx);
+  *reinterpret_cast<float2*>(lo + row0) = make_float2(lx, ly);
+  *reinterpret_cast<float2*>(lo + row0 + ldb) = make_float2(-ly, lx);
+}
+
+__device__ __forceinline__ void store_operand(const OperandOut& O, int ld, int kk, int r, int f, float2 X) {
+  if (O.bhi == nullptr) {
+    const size_t idx = ((size_t)kk * ld + r) * O.ldf + f;
+    O.plain[idx] = X;
+    for (int p = 0; p < O.npeer; ++p) reinterpret_cast<float2*>(O.peer[p][0])[idx] = X;
+    return;
+  }
   const size_t row0 = ((size_t)kk * 2 * ld + 2 * r) * O.ldb + 2 * f;
-  *reinterpret_cast<float2*>(O.bhi + row0) = make_float2(hx, hy);
-  *reinterpret_cast<float2*>(O.bhi + row0 + O.ldb) = make_float2(-hy, hx);
-  *reinterpret_cast<float2*>(O.blo + row0) = make_float2(lx, ly);
-  *reinterpret_cast<float2*>(O.blo + row0 + O.ldb) = make_float2(-ly, lx);
+  store_split_rows(O.bhi, O.blo, row0, O.ldb, X);
+  for (int p = 0; p < O.npeer; ++p) store_split_rows(O.peer[p][0], O.peer[p][1], row0, O.ldb, X);
 }
 
 // mk_fft_fast.cu: true when the register-resident path handles this context's nt (and it is not switched off)

@@ -43,6 +43,8 @@ struct mk_ctx {
   // run state
   int nfoc = 0, ldf = 0, iter = 0;
   bool begun = false;
+  bool contracted = false;  // mk_step_contract done, mk_step_post pending
+  bool reserved = false;  // mk_operand_reserve: operands of c->nfoc exist
   float* d_f1plus = nullptr;
   float* d_f1min = nullptr;
   size_t cap_time = 0;  // capacity (floats) of each of f1plus / f1min
@@ -63,7 +65,10 @@ struct mk_ctx {
   float* d_Bhi2 = nullptr;
   float* d_Blo2 = nullptr;
   size_t cap_B2 = 0;
-  long long operand_key[2] = {0, 0};  // layout the slot's operand was last zeroed for (0 = not zeroed)
+  long long operand_key[2] = {0, 0};
+  int npeer[2] = {0, 0};               // mk_operand_attach
+  float* peer_plane[2][7][2] = {};     // [slot][peer][plane]
+  long long peer_key[2] = {0, 0};      // operand layout the peers were attached for  // layout the slot's operand was last zeroed for (0 = not zeroed)
   // regime 3: cached TMA descriptors (CUtensorMap is 128 bytes, 64-byte aligned), built by mk_syn_tc.cu
   alignas(64) unsigned char tmap_A[128];
   alignas(64) unsigned char tmap_B[2][2][128];  // [main / scratch][hi / lo]
@@ -102,11 +107,17 @@ struct FftParams {
 
 // where a forward transform stores N^ (a1, a6): the plain complex layout (regimes 1, 2) or the split real operand
 // of regime 3 (bhi != nullptr)
+constexpr int kMaxPeers = 7;  // other ranks of a row-sharded run whose operand receives this rank's rows directly
+
 struct OperandOut {
   float2* plain;
   float* bhi;
   float* blo;
   int ldf, ldb;
+  // row sharding with attached peers (mk_operand_attach): every store of this rank's rows goes to the same offset of
+  // each peer's operand as well — the all-gather fused into the producing kernel as peer stores over NVLink
+  int npeer;
+  float* peer[kMaxPeers][2];  // [p][0] = plain (as floats) or hi plane, [p][1] = lo plane
 };
 
 int set_err(mk_ctx* c, int code, const std::string& msg);

@@ -45,7 +45,7 @@ constexpr int UK = 8;          // k' per tcgen05.mma (kind::tf32)
 constexpr int kMaxStages = 12;  // the ring has as many stages as fit (4 at N = 256, 11 for a single column block)
 constexpr int kThreads = 384;  // 12 warps
 constexpr int kChunkKb = 4;    // k'-blocks per accumulation chunk (24 MMA steps)
-constexpr int kSplitThreads = 64, kEpiWarps = 8;
+constexpr int kEpiWarps = 8;
 constexpr uint32_t A_BYTES = BM * BK * 4;   // 8 KB
 constexpr uint32_t BLK_BYTES = BK * 32 * 4;  // one 32-column block of a B' tile: 2 KB
 // A stage = A raw, A lo (8 KB each), B hi, B lo (nblk column blocks each, nblk = min(8, ceil(columns / 32))): narrow

@@ -129,3 +129,75 @@ def distributed_exchange(mk, dist):
         allgather_operand_rows(planes, v.rows_per_rec, mk.nrec, dist.get_rank(), dist.get_world_size(), dist)
         mk.operand_exchanged(slot)
     return exchange
+
+
+# ---- the same exchange FUSED into the producing kernels: peer stores (include/mk.h mk_operand_attach) ----------------
+def attach_in_process(mks, nfoc: int) -> None:
+    """Row-sharded contexts of ONE process: every context's operand-producing kernels store their rows into all the
+    others' operands as well."""
+    for mk in mks:
+        mk.operand_reserve(nfoc)
+    for slot in (0, 1):
+        views = [mk.operand_view(slot) for mk in mks]
+        for i, mk in enumerate(mks):
+            mk.operand_attach(slot, [v for j, v in enumerate(views) if j != i])
+
+
+def attach_ipc(mk, nfoc: int, dist):
+    """One process per GPU (or several processes on one GPU): exchange CUDA IPC handles of the operand planes through
+    torch.distributed and attach every other rank's operand.  Returns the opened pointers (close them with
+    binding.ipc_close before the contexts are destroyed)."""
+    from . import binding as B
+    mk.operand_reserve(nfoc)
+    rank, world = dist.get_rank(), dist.get_world_size()
+    mine = {slot: mk.operand_view(slot) for slot in (0, 1)}
+    handles = {slot: [B.ipc_export(int(v.plane[p])) for p in range(v.nplanes)] for slot, v in mine.items()}
+    everyone = [None] * world
+    dist.all_gather_object(everyone, handles)
+    opened = []
+    for slot in (0, 1):
+        views = []
+        for g in range(world):
+            if g == rank:
+                continue
+            v = B.mk_operand_view()
+            for name, _ in B.mk_operand_view._fields_:
+                if name != "plane":
+                    setattr(v, name, getattr(mine[slot], name))
+            for p, h in enumerate(everyone[g][slot]):
+                ptr = B.ipc_open(h)
+                opened.append(ptr)
+                v.plane[p] = ptr
+            views.append(v)
+        mk.operand_attach(slot, views)
+    return opened
+
+
+def run_row_sharded_fused(mk, d_Gd, d_td, niter: int, outs: dict, barrier, on_iterate=None) -> None:
+    """Algorithm 1 on a row-sharded context whose peers are attached: no copies, two barriers per synthesis.
+    `barrier()` must return only when every rank's stream has finished the work enqueued so far (e.g.
+    torch.cuda.synchronize(); dist.barrier()): once before a rank may overwrite operand rows that others read
+    (contractions done), once before anyone reads the new rows (stores done)."""
+    from . import binding as B
+    barrier()                                      # nobody still reads the operands of a previous run
+    mk.begin(d_Gd, d_td)
+    barrier()
+    mk.operand_exchanged(0)
+    for i in range(niter):
+        mk.step_contract()
+        barrier()                                  # every rank has read the operand: it may be overwritten
+        mk.step_post(outs.get("N_last") if i == niter - 1 else None)
+        if on_iterate is not None:
+            on_iterate(i)
+        barrier()                                  # every rank's rows have landed everywhere
+        mk.operand_exchanged(0)
+    plain = {k: v for k, v in outs.items() if k in ("f1plus", "f1min", "G") and v is not None}
+    if plain:
+        mk.finish(plain)
+    for name, field in (("Gminus", B.MK_FIELD_GMINUS), ("Gplus", B.MK_FIELD_GPLUS)):
+        if outs.get(name) is not None:
+            barrier()                              # slot 1 of the previous field has been consumed everywhere
+            mk.finish_prepare(field)
+            barrier()
+            mk.operand_exchanged(1)
+            mk.finish_complete(field, outs[name])

@@ -254,3 +254,70 @@ def test_error_paths_and_degenerate_runs():
         mk.run(Gd, td, 1, outs)
         torch.cuda.synchronize()
         assert np.isfinite(outs["G"].cpu().numpy()).all()
+
+
+@pytest.mark.parametrize("k,n,nt,nfoc,regime,world", [(1, 37, 512, 3, 1, 2), (3, 45, 512, 19, 2, 3), (3, 150, 2048, 19, 3, 3)])
+def test_row_sharded_with_fused_peer_stores(k, n, nt, nfoc, regime, world):
+    """The exchange fused into the producing kernels (mk_operand_attach): no copies between the contexts, every rank's
+    k_fwd / k_post stores its rows into all the others' operands; lock-step order contract -> post, as the barriers of
+    shard.run_row_sharded_fused enforce across processes."""
+    import torch
+    from paper_2106_04649_b200 import binding as B, shard
+    cfg = calibrated(configs.scaled(k, n=n, nt=nt, nfoc=nfoc, focal="fan:250", niter=5))
+    R, Gd, td = problem(cfg)
+    whole = gpu_chain(cfg, R, Gd, td, regime=regime)
+    dev = torch.device("cuda:0")
+    dR, dGd, dtd = (torch.from_numpy(np.ascontiguousarray(a)).to(dev) for a in (R, Gd, td))
+    mks = []
+    try:
+        for g in range(world):
+            rows = shard.row_slice(n, g, world)
+            mk = B.Marchenko(n, n, nt, cfg.dt, cfg.dx, cfg.fmin, cfg.fmax, rows=(rows.start, len(rows)))
+            mk.set_option(B.MK_OPT_EPS_SAMPLES, cfg.eps)
+            mk.set_option(B.MK_OPT_REGIME, regime)
+            mk.load_R(dR)
+            mks.append(mk)
+        shard.attach_in_process(mks, nfoc)
+        for mk in mks:
+            mk.begin(dGd, dtd)
+        for mk in mks:
+            mk.operand_exchanged(0)
+        bufs = [torch.zeros((nfoc, n, nt), dtype=torch.float32, device=dev) for _ in mks]
+        its = [[] for _ in mks]
+        for _ in range(cfg.niter):
+            for mk in mks:
+                mk.step_contract()
+            for g, mk in enumerate(mks):
+                mk.step_post(bufs[g])
+                its[g].append(bufs[g].cpu().numpy().copy())
+            for mk in mks:
+                mk.operand_exchanged(0)
+        outs = [{nm: torch.zeros((nfoc, n, nt), dtype=torch.float32, device=dev) for nm in FINALS} for _ in mks]
+        for g, mk in enumerate(mks):
+            mk.finish({nm: outs[g][nm] for nm in ("f1plus", "f1min", "G")})
+        for name, field in (("Gminus", B.MK_FIELD_GMINUS), ("Gplus", B.MK_FIELD_GPLUS)):
+            for mk in mks:
+                mk.finish_prepare(field)
+            for mk in mks:
+                mk.operand_exchanged(1)
+            for g, mk in enumerate(mks):
+                mk.finish_complete(field, outs[g][name])
+        torch.cuda.synchronize()
+        worst = 0.0
+        for g in range(world):
+            rows = shard.row_slice(n, g, world)
+            sl = slice(rows.start, rows.stop)
+            for i in range(cfg.niter):
+                worst = max(worst, rel_l2(its[g][i][:, sl], whole["N_iters"][i][:, sl]))
+            for nm in FINALS:
+                worst = max(worst, rel_l2(outs[g][nm].cpu().numpy()[:, sl], whole[nm][:, sl]))
+        print(f"\n[fused peer stores, {world} x, n={n} nt={nt} nfoc={nfoc} regime={regime}] worst deviation {worst:.1e}")
+        assert worst <= 1e-6
+        # a new batch size drops the attachment loudly instead of exchanging nothing
+        mks[0].operand_reserve(nfoc + 1)
+        Gd2 = torch.zeros((nfoc + 1, n, nt), dtype=torch.float32, device=dev)
+        with pytest.raises(B.MkError):
+            mks[0].begin(Gd2, torch.zeros((nfoc + 1, n), dtype=torch.float32, device=dev))
+    finally:
+        for mk in mks:
+            mk.close()
