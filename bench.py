@@ -243,11 +243,13 @@ def run_ours(args):
         torch.cuda.empty_cache()
         dGd, dtd = gen.first_arrivals_torch(cfg, dev)
         R = Gd = td = None
-        # 180 GB of HBM do not hold six distinct output fields of config 4 next to R^ and the accumulators: the six
-        # outputs are written one after the other into ONE buffer there (same kernels, same traffic)
-        shared = torch.empty((nfoc, cfg.n, cfg.nt), dtype=torch.float32, device=dev) if cfg.k == 4 else None
-        douts = {nm: (shared if shared is not None else torch.empty((nfoc, cfg.n, cfg.nt), dtype=torch.float32, device=dev))
-                 for nm in fields}
+        # 180 GB of HBM do not hold six distinct output fields of config 4 next to R^ and the operands: f1plus and f1min
+        # (the accumulators of the run) get their own fields, the other four outputs are written one after the other
+        # into ONE shared field there (same kernels, same traffic)
+        def field():
+            return torch.empty((nfoc, cfg.n, cfg.nt), dtype=torch.float32, device=dev)
+        shared = field() if cfg.k == 4 else None
+        douts = {nm: (field() if (shared is None or nm in ("f1plus", "f1min")) else shared) for nm in fields}
     else:
         R, Gd, td = workload_arrays(cfg)
         mk.load_R_host(R)

@@ -113,7 +113,10 @@ typedef struct mk_outputs {
 
 /* The whole scheme (Algorithm 1) for nfoc focal points:
  * d_Gd [nfoc][nrec][nt] fp32 first arrivals G_d(x_R, x_F, t), d_td [nfoc][nrec] fp32 traveltimes in seconds.
- * Equals mk_begin + niter x mk_step + mk_finish.  MK_ERR_STATE unless all nshot shots have been loaded. */
+ * Equals mk_begin + niter x mk_step + mk_finish.  MK_ERR_STATE unless all nshot shots have been loaded.
+ * When d_out->f1plus / f1min are given, the series is accumulated in those fields directly (no copy at the end, no
+ * library-owned twin): they must not alias each other or d_Gd, and until the next mk_begin / mk_run the context reads
+ * them again for mk_finish and mk_image, so they must stay allocated and unmodified for those calls. */
 int mk_run(mk_ctx* ctx, const float* d_Gd, const float* d_td, int nfoc, int niter, const mk_outputs* d_out);
 /* Same with HOST inputs and HOST outputs (copies in, runs, copies out, synchronises). */
 int mk_run_host(mk_ctx* ctx, const float* h_Gd, const float* h_td, int nfoc, int niter, const mk_outputs* h_out);

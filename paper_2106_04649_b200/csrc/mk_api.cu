@@ -404,7 +404,9 @@ int mk_load_R_host(mk_ctx* c, const float* h_R_time, int shot0, int nshots) {
   return check_cuda(c, cudaStreamSynchronize(c->stream), "cudaStreamSynchronize");
 }
 
-int mk_begin(mk_ctx* c, const float* d_Gd, const float* d_td, int nfoc) {
+// a1.  ext_plus / ext_min: caller-owned [nfoc][nrec][nt] buffers to accumulate f1plus / f1min in (mk_run hands its output
+// fields in, which saves the copies at the end and the library's own fields), or NULL for the library's own.
+static int begin_impl(mk_ctx* c, const float* d_Gd, const float* d_td, int nfoc, float* ext_plus, float* ext_min) {
   MK_GUARD(c);
   if (!d_Gd || !d_td || nfoc <= 0) return set_err(c, MK_ERR_INVALID_ARG, "mk_begin: bad arguments");
   if (c->shots_loaded != c->n) return set_err(c, MK_ERR_STATE, "mk_begin before every shot of R was loaded");
@@ -415,9 +417,12 @@ int mk_begin(mk_ctx* c, const float* d_Gd, const float* d_td, int nfoc) {
   const size_t nS = (size_t)c->n * c->nb * ldf;
   c->begun = false;
   {
-    size_t cap2 = c->cap_time;
-    if (int rc = ensure(c, &c->d_f1plus, &c->cap_time, ntime, "f1plus")) return rc;
-    if (int rc = ensure(c, &c->d_f1min, &cap2, ntime, "f1min")) return rc;
+    if (!ext_plus)
+      if (int rc = ensure(c, &c->d_f1plus, &c->cap_time, ntime, "f1plus")) return rc;
+    if (!ext_min)
+      if (int rc = ensure(c, &c->d_f1min, &c->cap_time_min, ntime, "f1min")) return rc;
+    c->acc_plus = ext_plus ? ext_plus : c->d_f1plus;
+    c->acc_min = ext_min ? ext_min : c->d_f1min;
     size_t capS = c->cap_Shat;
     if (int rc = ensure(c, &c->d_Shat, &c->cap_Shat, nS, "Shat")) return rc;
     if (int rc = ensure(c, &c->d_phat, &capS, nS, "phat")) return rc;
@@ -432,18 +437,20 @@ int mk_begin(mk_ctx* c, const float* d_Gd, const float* d_td, int nfoc) {
   c->have_Gminus = false;
   if (int rc = prepare_operand(c, 0, regime, nfoc, ldf, ldb)) return rc;
   if (int rc = check_cuda(c, cudaMemsetAsync(c->d_phat, 0, nS * sizeof(float2), c->stream), "memset phat")) return rc;
-  if (int rc = check_cuda(c, cudaMemsetAsync(c->d_f1min, 0, ntime * sizeof(float), c->stream), "memset f1min")) return rc;
+  if (int rc = check_cuda(c, cudaMemsetAsync(c->acc_min, 0, ntime * sizeof(float), c->stream), "memset f1min")) return rc;
   if (int rc = launch_window(c, d_td, c->d_h, nfoc * c->n)) return rc;
   // a1: N_{-1} = f1plus = T G_d; N^_{-1} = conj(G_d^)     [PAPER.md:19, 67, 74-75]
   if (int rc = check_peers(c, 0)) return rc;
   const bool sharded = c->nrow != c->n;
   if (sharded)  // the rows of other ranks stay zero in this rank's fields
-    if (int rc = check_cuda(c, cudaMemsetAsync(c->d_f1plus, 0, ntime * sizeof(float), c->stream), "memset f1plus")) return rc;
-  if (int rc = launch_fwd(c, d_Gd, operand_out(c, 0, regime, ldf, ldb), nfoc, /*conj_out=*/true, c->d_f1plus)) return rc;
+    if (int rc = check_cuda(c, cudaMemsetAsync(c->acc_plus, 0, ntime * sizeof(float), c->stream), "memset f1plus")) return rc;
+  if (int rc = launch_fwd(c, d_Gd, operand_out(c, 0, regime, ldf, ldb), nfoc, /*conj_out=*/true, c->acc_plus)) return rc;
   c->operand_stale[0] = sharded;
   c->begun = true;
   return MK_OK;
 }
+
+int mk_begin(mk_ctx* c, const float* d_Gd, const float* d_td, int nfoc) { return begin_impl(c, d_Gd, d_td, nfoc, nullptr, nullptr); }
 
 int mk_step_contract(mk_ctx* c) {
   MK_GUARD(c);
@@ -483,10 +490,10 @@ int mk_finish(mk_ctx* c, const mk_outputs* o) {
   if (!o) return set_err(c, MK_ERR_INVALID_ARG, "mk_finish: null outputs");
   if (o->N_last) return set_err(c, MK_ERR_INVALID_ARG, "N_last is delivered by mk_run (or by mk_step's d_N_i), not by mk_finish");
   const size_t bytes = (size_t)c->nfoc * c->n * c->nt * sizeof(float);
-  if (o->f1plus)
-    if (int rc = check_cuda(c, cudaMemcpyAsync(o->f1plus, c->d_f1plus, bytes, cudaMemcpyDeviceToDevice, c->stream), "copy f1plus")) return rc;
-  if (o->f1min)
-    if (int rc = check_cuda(c, cudaMemcpyAsync(o->f1min, c->d_f1min, bytes, cudaMemcpyDeviceToDevice, c->stream), "copy f1min")) return rc;
+  if (o->f1plus && o->f1plus != c->acc_plus)  // mk_run accumulates in the caller's field directly
+    if (int rc = check_cuda(c, cudaMemcpyAsync(o->f1plus, c->acc_plus, bytes, cudaMemcpyDeviceToDevice, c->stream), "copy f1plus")) return rc;
+  if (o->f1min && o->f1min != c->acc_min)
+    if (int rc = check_cuda(c, cudaMemcpyAsync(o->f1min, c->acc_min, bytes, cudaMemcpyDeviceToDevice, c->stream), "copy f1min")) return rc;
   if ((o->Gminus || o->Gplus) && c->nrow != c->n)
     return set_err(c, MK_ERR_STATE, "row-sharded context: G^- / G^+ need mk_finish_prepare, an exchange of slot 1, mk_finish_complete");
   if (o->Gminus) {
@@ -498,7 +505,7 @@ int mk_finish(mk_ctx* c, const mk_outputs* o) {
     if (int rc = mk_finish_complete(c, MK_FIELD_GPLUS, o->Gplus)) return rc;
   }
   if (o->G) {  // G = p^- + T f2 = p^- + T f1plus - f1min   [PAPER.md:24; G3]
-    if (int rc = launch_inv(c, c->d_phat, c->nfoc, c->ldf, o->G, 1.f, c->d_f1min, -1.f, c->d_f1plus, 1.f)) return rc;
+    if (int rc = launch_inv(c, c->d_phat, c->nfoc, c->ldf, o->G, 1.f, c->acc_min, -1.f, c->acc_plus, 1.f)) return rc;
   }
   return MK_OK;
 }
@@ -513,7 +520,7 @@ int mk_finish_prepare(mk_ctx* c, int field) {
   // operand = spectrum of T f1min = conj of the spectrum of f1min
   if (int rc = check_peers(c, 1)) return rc;
   const bool minus = field == MK_FIELD_GMINUS;
-  if (int rc = launch_fwd(c, minus ? c->d_f1plus : c->d_f1min, operand_out(c, 1, regime, c->ldf, c->ldb), c->nfoc, !minus, nullptr)) return rc;
+  if (int rc = launch_fwd(c, minus ? c->acc_plus : c->acc_min, operand_out(c, 1, regime, c->ldf, c->ldb), c->nfoc, !minus, nullptr)) return rc;
   c->operand_stale[1] = c->nrow != c->n;
   c->prepared_field = field;
   return MK_OK;
@@ -526,8 +533,8 @@ int mk_finish_complete(mk_ctx* c, int field, float* d_out) {
   const int regime = c->regime_used;
   if (int rc = contract(c, 1, c->d_Shat2, c->nfoc, c->ldf, c->ldb, regime)) return rc;
   c->prepared_field = 0;
-  if (field == MK_FIELD_GMINUS) return launch_inv(c, c->d_Shat2, c->nfoc, c->ldf, d_out, 1.f, c->d_f1min, -1.f, nullptr, 0.f);
-  return launch_inv(c, c->d_Shat2, c->nfoc, c->ldf, d_out, -1.f, nullptr, 0.f, c->d_f1plus, 1.f);
+  if (field == MK_FIELD_GMINUS) return launch_inv(c, c->d_Shat2, c->nfoc, c->ldf, d_out, 1.f, c->acc_min, -1.f, nullptr, 0.f);
+  return launch_inv(c, c->d_Shat2, c->nfoc, c->ldf, d_out, -1.f, nullptr, 0.f, c->acc_plus, 1.f);
 }
 
 int mk_operand(mk_ctx* c, int slot, mk_operand_view* v) {
@@ -639,7 +646,9 @@ int mk_run(mk_ctx* c, const float* d_Gd, const float* d_td, int nfoc, int niter,
   if (c->nrow != c->n) return set_err(c, MK_ERR_STATE, "row-sharded context: drive mk_begin / mk_step / mk_finish_* with the exchanges in between");
   if (niter < 0 || !o) return set_err(c, MK_ERR_INVALID_ARG, "mk_run: bad arguments");
   if (o->N_last && niter == 0) return set_err(c, MK_ERR_INVALID_ARG, "N_last needs niter >= 1");
-  if (int rc = mk_begin(c, d_Gd, d_td, nfoc)) return rc;
+  if ((o->f1plus && (o->f1plus == o->f1min || (const float*)o->f1plus == d_Gd)) || (o->f1min && (const float*)o->f1min == d_Gd))
+    return set_err(c, MK_ERR_INVALID_ARG, "mk_run: f1plus / f1min must not alias each other or G_d");
+  if (int rc = begin_impl(c, d_Gd, d_td, nfoc, o->f1plus, o->f1min)) return rc;  // accumulate in the caller's fields
   for (int i = 0; i < niter; ++i)
     if (int rc = mk_step(c, i == niter - 1 ? o->N_last : nullptr)) return rc;
   mk_outputs rest = *o;
@@ -685,7 +694,7 @@ int mk_run_host(mk_ctx* c, const float* h_Gd, const float* h_td, int nfoc, int n
   for (int i = 0; i < 5; ++i) {
     if (!hosts[i]) continue;
     if (i == 0 || i == 1) {  // accumulators go straight from the library's buffers (the finals only read them)
-      const float* src = i == 0 ? c->d_f1plus : c->d_f1min;
+      const float* src = i == 0 ? c->acc_plus : c->acc_min;
       if (int rc = check_cuda(c, cudaMemcpyAsync(hosts[i], src, ntime * sizeof(float), cudaMemcpyDeviceToHost, cs), "D2H accumulator")) return rc;
       continue;
     }
@@ -722,7 +731,7 @@ int mk_image(mk_ctx* c, const float* d_Gminus, float* d_image) {
   if (!d_Gminus || !d_image) return set_err(c, MK_ERR_INVALID_ARG, "mk_image: bad arguments");
   if (!c->begun) return set_err(c, MK_ERR_STATE, "mk_image before a run");
   const float wm = (float)(c->dt * c->dx), we = (float)(c->dt * c->dx * 0.5);
-  k_image<<<c->nfoc, 256, 0, c->stream>>>(d_Gminus, c->d_f1plus, d_image, c->n, c->nt, wm, we);
+  k_image<<<c->nfoc, 256, 0, c->stream>>>(d_Gminus, c->acc_plus, d_image, c->n, c->nt, wm, we);
   ++c->launches;
   return check_cuda(c, cudaGetLastError(), "k_image");
 }

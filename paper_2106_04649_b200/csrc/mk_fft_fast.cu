@@ -681,7 +681,7 @@ int launch_inv_fast(mk_ctx* c, const float2* d_spec, int nfoc, int ldf, float* d
 int launch_post_fast(mk_ctx* c, const OperandOut& O, int parity_even, float* d_Ni_out) {
   const Shape sh = shape_for(c, c->nfoc);
   const dim3 grid((c->nfoc + (1 << sh.lg) - 1) >> sh.lg, c->nrow);
-  MK_FAST_LAUNCH(k_post_fast, grid, sh, c->d_Shat, c->d_phat, O, c->d_h, c->d_f1plus, c->d_f1min, make_fast(c, c->nfoc, c->ldf),
+  MK_FAST_LAUNCH(k_post_fast, grid, sh, c->d_Shat, c->d_phat, O, c->d_h, c->acc_plus, c->acc_min, make_fast(c, c->nfoc, c->ldf),
                  sh.lg, parity_even, d_Ni_out);
 }
 

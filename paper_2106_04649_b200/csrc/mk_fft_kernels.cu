@@ -432,7 +432,7 @@ int launch_post(mk_ctx* c, const OperandOut& O, int parity_even, float* d_Ni_out
   const size_t smem = trace_smem(c, lg);
   if (int rc = set_smem(c, k_post, smem)) return rc;
   const dim3 grid((c->nfoc + FT - 1) / FT, c->nrow);
-  k_post<<<grid, kThreads, smem, c->stream>>>(c->d_Shat, c->d_phat, O, c->d_h, c->d_f1plus, c->d_f1min,
+  k_post<<<grid, kThreads, smem, c->stream>>>(c->d_Shat, c->d_phat, O, c->d_h, c->acc_plus, c->acc_min,
                                               make_params(c, c->nfoc, c->ldf), lg, parity_even, d_Ni_out);
   ++c->launches;
   return check_cuda(c, cudaGetLastError(), "k_post");

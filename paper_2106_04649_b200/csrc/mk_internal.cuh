@@ -47,7 +47,9 @@ struct mk_ctx {
   bool reserved = false;  // mk_operand_reserve: operands of c->nfoc exist
   float* d_f1plus = nullptr;
   float* d_f1min = nullptr;
-  size_t cap_time = 0;  // capacity (floats) of each of f1plus / f1min
+  size_t cap_time = 0, cap_time_min = 0;  // capacities (floats) of d_f1plus / d_f1min
+  float* acc_plus = nullptr;  // the accumulators of the current run: the library's own fields, or (mk_run) the caller's
+  float* acc_min = nullptr;   // f1plus / f1min output fields
   float2* d_Nhat = nullptr;
   float2* d_Shat = nullptr;
   float2* d_phat = nullptr;
