@@ -50,7 +50,9 @@ constexpr uint32_t A_BYTES = BM * BK * 4;   // 8 KB
 constexpr uint32_t BLK_BYTES = BK * 32 * 4;  // one 32-column block of a B' tile: 2 KB
 // A stage = A raw, A lo (8 KB each), B hi, B lo (nblk column blocks each, nblk = min(8, ceil(columns / 32))): narrow
 // focal batches move and hold only the columns they have, and get a deeper ring for it (HBM-bound regime)
-__host__ __device__ constexpr uint32_t stage_bytes(int nblk) { return 2 * A_BYTES + 2 * (uint32_t)nblk * BLK_BYTES; }
+// mp = M tiles (of 128 receivers) that share the stage's B' tile: 2 when the focal batch fits 128 columns, so that a
+// stage feeds as many MMA cycles as a 256-column one with 32 KB instead of 2 x 24 KB of loads (the kernel is feed-bound)
+__host__ __device__ constexpr uint32_t stage_bytes(int nblk, int mp) { return 2 * (uint32_t)mp * A_BYTES + 2 * (uint32_t)nblk * BLK_BYTES; }
 constexpr size_t kSmemExtra = 1024 /*alignment slack*/ + 512 /*barriers*/;
 constexpr uint32_t kTmemCols = 512;
 
@@ -135,6 +137,7 @@ struct TcParams {
   int ncols;            // 2 * ldf: valid real columns of S^
   int mt, ntl;          // tiles along M and N
   int nblk, stages;     // column blocks per B' tile, stages of the ring
+  int mp;               // M tiles per CTA tile (1, or 2 when ncols <= 128: accumulator m lives in columns 128 m .. of the buffer)
   size_t s_row;         // floats between consecutive receivers of S^: nb * 2 ldf
 };
 
@@ -144,7 +147,9 @@ k_syn_gemm_tf32x3(const __grid_constant__ CUtensorMap tmA, const __grid_constant
   extern __shared__ uint8_t smem_raw[];
   uint8_t* smem = reinterpret_cast<uint8_t*>(((uintptr_t)smem_raw + 1023) & ~(uintptr_t)1023);
   const int STAGES = P.stages;
-  const uint32_t STAGE_BYTES = stage_bytes(P.nblk), B_BYTES = (uint32_t)P.nblk * BLK_BYTES, TX_BYTES = A_BYTES + 2 * B_BYTES;
+  const int MP = P.mp;
+  const uint32_t STAGE_BYTES = stage_bytes(P.nblk, MP), B_BYTES = (uint32_t)P.nblk * BLK_BYTES, AREG = (uint32_t)MP * A_BYTES;
+  const uint32_t TX_BYTES = AREG + 2 * B_BYTES;
   uint64_t* bars = reinterpret_cast<uint64_t*>(smem + (size_t)STAGES * STAGE_BYTES);
   uint64_t* full = bars;                      // [kMaxStages] TMA landed
   uint64_t* empty = bars + kMaxStages;        // [kMaxStages] MMAs of the stage retired
@@ -189,9 +194,10 @@ k_syn_gemm_tf32x3(const __grid_constant__ CUtensorMap tmA, const __grid_constant
           mbar_wait(empty + s, ph ^ 1);
           uint8_t* st = smem + (size_t)s * STAGE_BYTES;
           mbar_expect_tx(full + s, TX_BYTES);
-          tma_load_3d(&tmA, full + s, st, kb * BK, kk, mi * BM);
-          tma_load_3d(&tmBhi, full + s, st + 2 * A_BYTES, 0, kk * 2 * P.ld + kb * BK, ni * (BN / 32));
-          tma_load_3d(&tmBlo, full + s, st + 2 * A_BYTES + B_BYTES, 0, kk * 2 * P.ld + kb * BK, ni * (BN / 32));
+          for (int m = 0; m < MP; ++m)  // rows past the last receiver arrive as zeros (and still count their bytes)
+            tma_load_3d(&tmA, full + s, st + m * A_BYTES, kb * BK, kk, (mi * MP + m) * BM);
+          tma_load_3d(&tmBhi, full + s, st + 2 * AREG, 0, kk * 2 * P.ld + kb * BK, ni * (BN / 32));
+          tma_load_3d(&tmBlo, full + s, st + 2 * AREG + B_BYTES, 0, kk * 2 * P.ld + kb * BK, ni * (BN / 32));
           if (++s == STAGES) {
             s = 0;
             ph ^= 1;
@@ -219,13 +225,15 @@ k_syn_gemm_tf32x3(const __grid_constant__ CUtensorMap tmA, const __grid_constant
             mbar_wait(full + s, ph);
             mbar_wait(split + s, ph);
             tc_fence_after();
-            const uint32_t a_raw = smem_u32(smem + (size_t)s * STAGE_BYTES), a_lo = a_raw + A_BYTES;
-            const uint32_t b_hi = a_raw + 2 * A_BYTES, b_lo = b_hi + B_BYTES;
+            const uint32_t a_raw = smem_u32(smem + (size_t)s * STAGE_BYTES), a_lo = a_raw + AREG;
+            const uint32_t b_hi = a_raw + 2 * AREG, b_lo = b_hi + B_BYTES;
 #pragma unroll
             for (int j = 0; j < BK / UK; ++j) {
               // A: K-major, 64-byte rows, SWIZZLE_64B: 8-row groups 512 B apart; a k'-chunk is 32 B further along the row
               const uint64_t da_raw = smem_desc(a_raw + j * 32, 16, 512, LAYOUT_SW64);
               const uint64_t da_lo = smem_desc(a_lo + j * 32, 16, 512, LAYOUT_SW64);
+              const uint64_t da_raw1 = smem_desc(a_raw + A_BYTES + j * 32, 16, 512, LAYOUT_SW64);  // second M tile (MP = 2)
+              const uint64_t da_lo1 = smem_desc(a_lo + A_BYTES + j * 32, 16, 512, LAYOUT_SW64);
               // B: MN-major tf32 must use the 128-byte swizzle with 32-byte atoms (the only MN-major layout the tensor
               //    core takes for 32-bit operands): [8 blocks of 32 columns][16 k' rows][128 B]; LBO = 2048 (next column
               //    block), SBO = 512 (next group of 4 k' rows); a k'-chunk of 8 rows is 1024 B further
@@ -234,6 +242,11 @@ k_syn_gemm_tf32x3(const __grid_constant__ CUtensorMap tmA, const __grid_constant
               umma_tf32(d, da_lo, db_hi, idesc, (kb != kb0) || (j != 0));  // small terms first; a chunk starts from zero
               umma_tf32(d, da_raw, db_lo, idesc, 1);
               umma_tf32(d, da_raw, db_hi, idesc, 1);
+              if (MP == 2) {
+                umma_tf32(d + BN / 2, da_lo1, db_hi, idesc, (kb != kb0) || (j != 0));
+                umma_tf32(d + BN / 2, da_raw1, db_lo, idesc, 1);
+                umma_tf32(d + BN / 2, da_raw1, db_hi, idesc, 1);
+              }
             }
             umma_commit(empty + s);
             if (++s == STAGES) {
@@ -257,10 +270,9 @@ k_syn_gemm_tf32x3(const __grid_constant__ CUtensorMap tmA, const __grid_constant
         if ((int)(cnt & 1) == sw) {
           mbar_wait(full + s, ph);
           const float4* src = reinterpret_cast<const float4*>(smem + (size_t)s * STAGE_BYTES);
-          float4* dst = reinterpret_cast<float4*>(smem + (size_t)s * STAGE_BYTES + A_BYTES);
-          constexpr int kPer = (int)(A_BYTES / 16) / 32;  // 16 float4 per lane
-#pragma unroll
-          for (int h = 0; h < 2; ++h) {
+          float4* dst = reinterpret_cast<float4*>(smem + (size_t)s * STAGE_BYTES + AREG);
+          constexpr int kPer = (int)(A_BYTES / 16) / 32;  // 16 float4 per lane and M tile
+          for (int h = 0; h < 2 * MP; ++h) {
             float4 v[kPer / 2];
 #pragma unroll
             for (int i = 0; i < kPer / 2; ++i) v[i] = src[lane + (h * (kPer / 2) + i) * 32];
@@ -291,7 +303,8 @@ k_syn_gemm_tf32x3(const __grid_constant__ CUtensorMap tmA, const __grid_constant
     uint32_t chunk_it = 0;
     for (int t = blockIdx.x; t < ntiles; t += gridDim.x) {
       const int kk = t / per_bin, rem = t - kk * per_bin, mi = rem / P.ntl, ni = rem - mi * P.ntl;
-      const int cols = P.ncols - ni * BN - half * (BN / 2);  // valid columns of this warp's half (may exceed BN / 2, may be <= 0)
+      // MP = 1: this warp's half of the 256 columns; MP = 2: the whole (<= 128-column) tile of M tile `half`
+      const int cols = MP == 2 ? P.ncols : P.ncols - ni * BN - half * (BN / 2);  // valid columns (may exceed BN / 2, may be <= 0)
       float sum[BN / 2];
 #pragma unroll
       for (int i = 0; i < BN / 2; ++i) sum[i] = 0.f;
@@ -314,9 +327,9 @@ k_syn_gemm_tf32x3(const __grid_constant__ CUtensorMap tmA, const __grid_constant
         __syncwarp();
         if (lane == 0) mbar_arrive(acc_empty + b);
       }
-      const int r = mi * BM + quad * 32 + lane;
+      const int r = (MP == 2 ? mi * 2 + half : mi) * BM + quad * 32 + lane;
       if (r < P.n) {
-        float* dst = Shat + (size_t)r * P.s_row + (size_t)kk * P.ncols + ni * BN + half * (BN / 2);
+        float* dst = Shat + (size_t)r * P.s_row + (size_t)kk * P.ncols + (MP == 2 ? 0 : ni * BN + half * (BN / 2));
 #pragma unroll
         for (int q = 0; q < BN / 8; ++q)
           if (q * 4 < cols)
@@ -368,7 +381,7 @@ bool tc_supported(const mk_ctx* c) {
   int dev = 0, major = 0;
   if (cudaGetDevice(&dev) != cudaSuccess) return false;
   cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev);
-  return major == 10 && c->smem_optin >= 2 * stage_bytes(1) + kSmemExtra;
+  return major == 10 && c->smem_optin >= 2 * stage_bytes(1, 1) + kSmemExtra;
 }
 
 int launch_syn_tc(mk_ctx* c, int slot, const float* d_Bhi, const float* d_Blo, float2* d_Shat, int nfoc, int ldf, int ldb) {
@@ -400,13 +413,15 @@ int launch_syn_tc(mk_ctx* c, int slot, const float* d_Bhi, const float* d_Blo, f
   P.nb = c->nb;
   P.ld = c->ld;
   P.ncols = 2 * ldf;
-  P.mt = (c->nrow + BM - 1) / BM;
+  const int mtiles = (c->nrow + BM - 1) / BM;
+  P.mp = (2 * ldf <= BN / 2 && mtiles >= 2) ? 2 : 1;
+  P.mt = (mtiles + P.mp - 1) / P.mp;
   P.ntl = (P.ncols + BN - 1) / BN;
   P.s_row = (size_t)c->nb * 2 * ldf;
   P.nblk = nblk;
-  P.stages = (int)std::min<size_t>(kMaxStages, (c->smem_optin - kSmemExtra) / stage_bytes(nblk));
+  P.stages = (int)std::min<size_t>(kMaxStages, (c->smem_optin - kSmemExtra) / stage_bytes(nblk, P.mp));
   if (P.stages < 2) return set_err(c, MK_ERR_INVALID_ARG, "not enough shared memory for the tcgen05 contraction");
-  const size_t kSmemBytes = (size_t)P.stages * stage_bytes(nblk) + kSmemExtra;
+  const size_t kSmemBytes = (size_t)P.stages * stage_bytes(nblk, P.mp) + kSmemExtra;
   if (int rc = check_cuda(c, cudaFuncSetAttribute(k_syn_gemm_tf32x3, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemBytes),
                           "cudaFuncSetAttribute"))
     return rc;
