@@ -121,7 +121,7 @@ def rhat_bytes(cfg):
 
 
 # ------------------------------------------------------------------------------------------------ oracle legs
-def oracle_sample(cfg, R, Gd, td, budget_s, full_first=True):
+def oracle_sample(cfg, R, Gd, td, budget_s, full_first=True, repeat=True):
     """Times the oracle (as it stands) on a bounded sample: one synthesis R N_0 over `nrec_s` receivers of the same
     workload, N_0 being the first windowed iterate (computed by the oracle, untimed).  Returns (seconds, nrec_s)."""
     import oracle
@@ -142,9 +142,15 @@ def oracle_sample(cfg, R, Gd, td, budget_s, full_first=True):
     nrec_s = int(min(cfg.n, max(oracle.num_threads(), budget_s / max(per_rec, 1e-6))))
     recs = np.linspace(0, cfg.n - 1, nrec_s).round().astype(int)
     Rs = np.ascontiguousarray(R[:, recs])
-    t0 = time.perf_counter()
-    oracle.synthesis(Rs, N0, cfg.dt, w, klo, khi)
-    return time.perf_counter() - t0, nrec_s, N0, (w, klo, khi)
+    # when the whole problem is cheaper than the budget, repeat it: about `budget_s` seconds of CPU work in all
+    reps, t_total = 0, 0.0
+    while reps == 0 or (repeat and nrec_s == cfg.n and t_total < 0.8 * budget_s and reps < 64):
+        t0 = time.perf_counter()
+        oracle.synthesis(Rs, N0, cfg.dt, w, klo, khi)
+        t_total += time.perf_counter() - t0
+        reps += 1
+    oracle_sample.reps = reps
+    return t_total / reps, nrec_s, N0, (w, klo, khi)
 
 
 def run_reference(args):
@@ -158,7 +164,7 @@ def run_reference(args):
     nbytes, nb = rhat_bytes(cfg)
     total_budget = 150.0
     per_step = total_budget / (args.steps + args.warmup)
-    _, _, N0, (w, klo, khi) = oracle_sample(cfg, R, Gd, td, budget_s=per_step)
+    _, _, N0, (w, klo, khi) = oracle_sample(cfg, R, Gd, td, budget_s=per_step, repeat=False)
     # pick the sample so that one step fits per_step seconds
     probe = np.linspace(0, cfg.n - 1, 4).round().astype(int)
     t0 = time.perf_counter()
@@ -360,7 +366,7 @@ def run_ours(args):
         t_s, nrec_s, _, _ = oracle_sample(cfg, R, Gd if f is None else Gd[f], td if f is None else td[f], budget_s=args.cpu_budget)
         cpu = {"value": (nbytes * nrec_s / cfg.n) / t_s / 1e9, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle",
                "sample": f"one oracle synthesis R N_0 (direct time-domain convolution, fp64) on {nrec_s} of {cfg.n} receivers x 1 focal "
-                         f"point of config {cfg.k}: {t_s:.2f} s"}
+                         f"point of config {cfg.k}: {t_s:.2f} s per synthesis, {getattr(oracle_sample, 'reps', 1)} repetitions"}
 
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": ms_total / args.steps, "higher_is_better": True, "scaling": "strong" if rows_mode else "weak", "vs_baseline": None,
