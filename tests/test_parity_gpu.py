@@ -59,6 +59,7 @@ def test_delta_spike_shift(n, nt, nfoc, regime):
     (37, 128, 1, 1), (37, 128, 3, 1), (37, 128, 8, 1),           # GEMV, ragged rows
     (37, 128, 5, 2), (150, 64, 70, 2), (130, 256, 129, 2),        # FFMA GEMM, ragged M / N tiles
     (37, 128, 5, 3), (150, 64, 70, 3), (130, 256, 129, 3), (260, 64, 140, 3),   # tcgen05 3xTF32, ragged M / N / K tiles
+    (300, 64, 20, 3), (257, 64, 64, 3),                           # two M tiles per B' tile, odd tile count / one-row last tile
     (16, 16, 2, 0), (33, 4096, 9, 0),                             # smallest / longest traces
     (24, 2048, 11, 0), (24, 2048, 1, 1), (20, 2048, 3, 1), (20, 4096, 1, 1), (18, 4096, 16, 3),   # register-resident transforms
 ])
