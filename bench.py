@@ -6,7 +6,8 @@ niter + 2 = 18 syntheses) over one batch of seeded synthetic input of BASELINE.j
 one focal point, 16 iterations; the bandwidth-bound regime the metric is quoted on).  R^ (1.30 GB) is resident in
 HBM and far larger than the 126 MB L2, so no cache flush is needed between steps.
 
-  value      synthesis GB/s of R^ streamed  = syntheses * bytes(R^ unpadded) / device time   (inputs resident in HBM)
+  value      synthesis GB/s of R^ streamed  = syntheses * bytes(R^ unpadded) / device time   (inputs resident in HBM;
+             algorithmic bytes: with 1, 2 or 4 focal points the two final syntheses share one pass over R^)
   e2e        same metric through mk_run_host: pinned HOST G_d / t_d in, six HOST output fields out, copies timed
   roofline   the streaming contraction kernel (k_syn_gemv): algorithmic bytes of R^ per launch / its CUDA-event time
   cpu_baseline  the fp64 oracle timed on this box's host cores on a bounded sample (one full synthesis R N_0)
@@ -372,7 +373,11 @@ def run_ours(args):
             "ms_per_step": ms_total / args.steps, "higher_is_better": True, "scaling": "strong" if rows_mode else "weak", "vs_baseline": None,
             "dtype": "f32", "data": "synthetic",
             "config": {"workload": f"config{cfg.k}:{cfg.name}", "n": cfg.n, "nt": cfg.nt, "nfoc": nfoc, "niter": niter, "nb": nb,
-                       "syntheses_per_step": nsyn, "rhat_bytes": nbytes, "regime": regime_used,
+                       "syntheses_per_step": nsyn, "contraction_launches_per_step": syn_n / max(args.steps, 1),
+                       "note": ("value counts the niter + 2 syntheses of Algorithm 1 (algorithmic bytes: one R^ per synthesis); with "
+                                "1, 2 or 4 focal points the two syntheses of the finals share ONE pass over R^ (2 nfoc right-hand sides)"
+                                if syn_n / max(args.steps, 1) < nsyn else "one pass over R^ per synthesis"),
+                       "rhat_bytes": nbytes, "regime": regime_used,
                        "l2": f"inputs_larger_than_L2 (R^ {nbytes / 1e9:.2f} GB vs 126 MB L2; no flush needed)",
                        "input_source": "device generator, 64-shot chunks (no e2e / cpu_baseline legs)" if big else "host arrays",
                        "parallelism": "1 GPU" if world == 1 and not rows_mode else

@@ -52,6 +52,8 @@ enum {
                              2 FP32-FFMA GEMM, 3 tcgen05 3xTF32 GEMM with chunked fp32 accumulation (sm_100 only;
                              MK_ERR_INVALID_ARG otherwise) */
   MK_OPT_TIMING = 3,      /* 1: bracket every contraction launch with CUDA events on the context's stream */
+  MK_OPT_FUSED_FINALS = 5, /* 1 (default): with 1, 2 or 4 focal points mk_finish / mk_run compute the extra syntheses of G^- and
+                             G^+ in ONE pass over R^ (2 nfoc right-hand sides, streaming GEMV); 0: one pass each */
   MK_OPT_FFT_PATH = 4     /* transform kernels: 0 auto (default), 1 generic shared-memory passes (any nt),
                              2 register-resident path (nt = 2048 or 4096 only; MK_ERR_INVALID_ARG otherwise) */
 };

@@ -332,6 +332,9 @@ int mk_set_option(mk_ctx* c, int key, double value) {
     case MK_OPT_TIMING:
       c->timing = value != 0.0;
       return MK_OK;
+    case MK_OPT_FUSED_FINALS:
+      c->fused_finals = value != 0.0;
+      return MK_OK;
     case MK_OPT_FFT_PATH:
       if (value < 0 || value > 2 || value != std::floor(value)) return set_err(c, MK_ERR_INVALID_ARG, "fft path must be 0..2");
       if ((int)value == 2 && c->nt != 2048 && c->nt != 4096)
@@ -496,11 +499,27 @@ int mk_finish(mk_ctx* c, const mk_outputs* o) {
     if (int rc = check_cuda(c, cudaMemcpyAsync(o->f1min, c->acc_min, bytes, cudaMemcpyDeviceToDevice, c->stream), "copy f1min")) return rc;
   if ((o->Gminus || o->Gplus) && c->nrow != c->n)
     return set_err(c, MK_ERR_STATE, "row-sharded context: G^- / G^+ need mk_finish_prepare, an exchange of slot 1, mk_finish_complete");
-  if (o->Gminus) {
+  // Few focal points: the two extra syntheses of the finals ("estimating each component requires an extra
+  // synthesis") are ONE pass over R^ with 2 nfoc right-hand sides — columns [0, nfoc) = spectrum of f1plus (G^-),
+  // [nfoc, 2 nfoc) = spectrum of T f1min (G^+) — in the bandwidth-bound regime that costs little more than one.
+  const bool fuse = o->Gminus && o->Gplus && c->fused_finals && c->regime_used == 1 && (c->nfoc == 1 || c->nfoc == 2 || c->nfoc == 4) &&
+                    gemv_supported(c, 2 * c->nfoc);
+  if (fuse) {
+    const int nf = c->nfoc, ldf2 = 2 * nf, ldb2 = ldb_for(ldf2);
+    if (int rc = ensure(c, &c->d_Shat2, &c->cap_Shat2, (size_t)c->n * c->nb * ldf2, "Shat scratch")) return rc;
+    if (int rc = prepare_operand(c, 1, 1, ldf2, ldf2, ldb2)) return rc;
+    OperandOut O = operand_out(c, 1, 1, ldf2, ldb2);
+    if (int rc = launch_fwd(c, c->acc_plus, O, nf, false, nullptr)) return rc;
+    O.plain += nf;
+    if (int rc = launch_fwd(c, c->acc_min, O, nf, true, nullptr)) return rc;
+    if (int rc = contract(c, 1, c->d_Shat2, ldf2, ldf2, ldb2, 1)) return rc;
+    if (int rc = launch_inv(c, c->d_Shat2, nf, ldf2, o->Gminus, 1.f, c->acc_min, -1.f, nullptr, 0.f)) return rc;       // [PAPER.md:87-88]
+    if (int rc = launch_inv(c, c->d_Shat2 + nf, nf, ldf2, o->Gplus, -1.f, nullptr, 0.f, c->acc_plus, 1.f)) return rc;   // [G4]
+  } else if (o->Gminus) {
     if (int rc = mk_finish_prepare(c, MK_FIELD_GMINUS)) return rc;
     if (int rc = mk_finish_complete(c, MK_FIELD_GMINUS, o->Gminus)) return rc;
   }
-  if (o->Gplus) {
+  if (!fuse && o->Gplus) {
     if (int rc = mk_finish_prepare(c, MK_FIELD_GPLUS)) return rc;
     if (int rc = mk_finish_complete(c, MK_FIELD_GPLUS, o->Gplus)) return rc;
   }
@@ -703,9 +722,15 @@ int mk_run_host(mk_ctx* c, const float* h_Gd, const float* h_td, int nfoc, int n
     if (i == 2) one.G = d_out;
     if (i == 3) one.Gplus = d_out;
     if (i == 4) one.Gminus = d_out;
+    const bool both = overlap && i == 3 && hosts[4];  // G^+ and G^- in one call: they may share one pass over R^
+    if (both) one.Gminus = d_field + (size_t)3 * ntime;
     if (int rc = mk_finish(c, &one)) return rc;
     if (int rc = hand_over()) return rc;
     if (int rc = check_cuda(c, cudaMemcpyAsync(hosts[i], d_out, ntime * sizeof(float), cudaMemcpyDeviceToHost, cs), "D2H output")) return rc;
+    if (both) {
+      if (int rc = check_cuda(c, cudaMemcpyAsync(hosts[4], one.Gminus, ntime * sizeof(float), cudaMemcpyDeviceToHost, cs), "D2H output")) return rc;
+      break;
+    }
   }
   if (overlap)
     if (int rc = check_cuda(c, cudaStreamSynchronize(cs), "cudaStreamSynchronize")) return rc;

@@ -35,6 +35,7 @@ struct mk_ctx {
 
   float2* d_tw = nullptr;    // [nt] e^{-2 pi i k / nt}
   float2* d_tw1k = nullptr;  // [32][32] e^{-2 pi i k1 t / 1024}: middle twiddles of the register-resident path
+  bool fused_finals = true;  // MK_OPT_FUSED_FINALS
   int fft_path = 0;          // MK_OPT_FFT_PATH: 0 auto, 1 generic shared-memory passes, 2 register-resident
   float2* d_Rhat = nullptr;  // [n][nb][ld]
   std::vector<unsigned char> shot_loaded;

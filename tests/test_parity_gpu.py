@@ -322,3 +322,30 @@ def test_row_sharded_with_fused_peer_stores(k, n, nt, nfoc, regime, world):
     finally:
         for mk in mks:
             mk.close()
+
+
+@pytest.mark.parametrize("nfoc", [1, 2, 4])
+def test_fused_finals_match_separate_finals(nfoc):
+    """MK_OPT_FUSED_FINALS: with 1, 2 or 4 focal points G^- and G^+ come from ONE pass over R^ (2 nfoc right-hand sides);
+    the separate path is the one the chain tests hold against the oracle."""
+    cfg = calibrated(configs.scaled(1, n=70, nt=2048 if nfoc == 4 else 512, nfoc=nfoc, focal="single:400" if nfoc == 1 else "fan:250", niter=4))
+    R, Gd, td = problem(cfg)
+    ref = _oracle_chain(cfg, R, Gd, td)
+    import torch
+    from paper_2106_04649_b200 import binding as B
+    dev = torch.device("cuda:0")
+    res = {}
+    for fused in (0, 1):
+        with B.Marchenko(cfg.n, cfg.n, cfg.nt, cfg.dt, cfg.dx, cfg.fmin, cfg.fmax) as mk:
+            mk.set_option(B.MK_OPT_EPS_SAMPLES, cfg.eps)
+            mk.set_option(B.MK_OPT_FUSED_FINALS, fused)
+            mk.load_R(torch.from_numpy(R).to(dev))
+            outs = {nm: torch.empty((nfoc, cfg.n, cfg.nt), dtype=torch.float32, device=dev) for nm in FINALS}
+            mk.set_option(B.MK_OPT_TIMING, 1)
+            mk.run(torch.from_numpy(Gd).to(dev), torch.from_numpy(td).to(dev), cfg.niter, outs)
+            torch.cuda.synchronize()
+            assert int(mk.get_info(B.MK_INFO_SYN_LAUNCHES)) == cfg.niter + (1 if fused else 2)
+            res[fused] = {nm: t.cpu().numpy() for nm, t in outs.items()}
+    for nm in FINALS:
+        assert rel_l2(res[1][nm], ref[nm]) <= TOL_FINAL, nm
+        assert rel_l2(res[1][nm], res[0][nm]) <= 2e-6, nm
