@@ -129,12 +129,8 @@ def oracle_sample(cfg, R, Gd, td, budget_s, full_first=True, repeat=True):
     w = oracle.weights(cfg.n, cfg.dx)
     klo, khi, _ = oracle.band(cfg.nt, cfg.dt, cfg.fmin, cfg.fmax)
     f = [0] if Gd.shape[0] > 1 else slice(None)
-    N = np.roll(Gd[f][..., ::-1], 1, axis=-1).astype(np.float64)               # N_{-1} = T G_d
-    S = oracle.synthesis(R, N, cfg.dt, w, klo, khi)                              # untimed: sparse N_{-1}
-    h = oracle.window(td[f], cfg.nt, cfg.dt, cfg.eps)
-    j = np.arange(cfg.nt)
-    js = np.where(j < cfg.nt // 2, j, j - cfg.nt)
-    N0 = -(np.abs(js)[None, None, :] < h[..., None]).astype(np.float64) * np.roll(S[..., ::-1], 1, axis=-1)
+    # N_0 = the oracle's own first iterate (untimed; N_{-1} = T G_d is sparse, so this pass is cheap)
+    N0 = oracle.marchenko(R, Gd[f], td[f], cfg.dt, cfg.dx, cfg.fmin, cfg.fmax, 1, cfg.eps, want=())["N_iters"][0]
     # size the sample from a 4-receiver probe
     probe = np.linspace(0, cfg.n - 1, 4).round().astype(int)
     t0 = time.perf_counter()

@@ -27,6 +27,14 @@
  *   - all work is enqueued on the context's stream (the legacy default stream until mk_set_stream).
  *     d_-pointer calls do not synchronise the host; h_-pointer calls return after the results are in host memory.
  *   - there is no CPU fallback: without a CUDA device mk_create fails with MK_ERR_CUDA.
+ *   - a context lives on the CUDA device that was current in mk_create; every entry point makes that device current
+ *     again (cudaSetDevice) before it does anything, so the caller may switch devices between calls.
+ *   - run state: mk_begin / mk_run start a run; mk_step, mk_finish*, mk_image, mk_operand need one.  Calls that change
+ *     what the run was started from — mk_load_R (another R^), MK_OPT_EPS_SAMPLES with a new value (another window),
+ *     mk_operand_reserve with another nfoc / regime (another operand layout) — END the run: afterwards the calls that
+ *     need a run return MK_ERR_STATE until the next mk_begin / mk_run.  Between mk_step_contract and mk_step_post they
+ *     are refused with MK_ERR_STATE.  MK_OPT_REGIME only affects runs started afterwards (a run keeps its regime);
+ *     mk_synthesis picks its own regime from its own nfoc and never disturbs the run in progress.
  */
 #ifndef MK_H_
 #define MK_H_
@@ -97,7 +105,8 @@ int mk_get_info(mk_ctx* ctx, int key, double* value);
  * d_R_time: [nshots][nrec][nt] fp32 time-domain R(x_R = rec, x = shot, t) for shots shot0 .. shot0+nshots-1.
  * Converted on the GPU, once, to band-limited complex64 with the quadrature weights folded in:
  *   R^[r][k][s] = dt * w[s] * sum_j R[s][r][j] e^{-2 pi i k j / nt},  k in B  (shot index fastest, zero padded to ld_shot).
- * May be called repeatedly with disjoint shot ranges (config 4: 61 calls of 64 shots). */
+ * May be called repeatedly with disjoint shot ranges (config 4: 61 calls of 64 shots), and again later to replace
+ * shots (it ends a run in progress, see "run state" above). */
 int mk_load_R(mk_ctx* ctx, const float* d_R_time, int shot0, int nshots);
 /* Same from a HOST buffer: staged through an internal device buffer in bounded chunks; returns when done. */
 int mk_load_R_host(mk_ctx* ctx, const float* h_R_time, int shot0, int nshots);
@@ -117,8 +126,11 @@ typedef struct mk_outputs {
  * d_Gd [nfoc][nrec][nt] fp32 first arrivals G_d(x_R, x_F, t), d_td [nfoc][nrec] fp32 traveltimes in seconds.
  * Equals mk_begin + niter x mk_step + mk_finish.  MK_ERR_STATE unless all nshot shots have been loaded.
  * When d_out->f1plus / f1min are given, the series is accumulated in those fields directly (no copy at the end, no
- * library-owned twin): they must not alias each other or d_Gd, and until the next mk_begin / mk_run the context reads
- * them again for mk_finish and mk_image, so they must stay allocated and unmodified for those calls. */
+ * library-owned twin): they must not overlap each other or d_Gd, and until the next mk_begin / mk_run the context reads
+ * them again for mk_finish and mk_image, so they must stay allocated and unmodified for those calls.  N_last, G, Gplus
+ * and Gminus are written while f1plus / f1min are still read: they must not overlap those two (MK_ERR_INVALID_ARG);
+ * they MAY share one buffer among themselves (each is complete before the next is written; the last one written wins:
+ * order N_last, Gminus, Gplus, G). */
 int mk_run(mk_ctx* ctx, const float* d_Gd, const float* d_td, int nfoc, int niter, const mk_outputs* d_out);
 /* Same with HOST inputs and HOST outputs (copies in, runs, copies out, synchronises). */
 int mk_run_host(mk_ctx* ctx, const float* h_Gd, const float* h_td, int nfoc, int niter, const mk_outputs* h_out);

@@ -52,6 +52,7 @@ def lib():
         L.orc_marchenko.restype = C.c_int
         L.orc_marchenko.argtypes = [C.c_int, C.c_int, C.c_double, C.c_double, C.c_double, C.c_double, C.c_int,
                                     _F32, C.c_int, _F32, _F32, C.c_int] + [C.c_void_p] * 8
+        L.orc_init_subset.argtypes = [C.c_int, C.c_int, _F32] + [C.c_void_p] * 5
         L.orc_step_subset.argtypes = [C.c_int, C.c_int, C.c_int, C.c_double, _F64, _F32, C.c_int, _F64, _I32, C.c_int,
                                       C.c_int, C.c_int, _F64] + [C.c_void_p] * 5
         L.orc_finals_subset.argtypes = [C.c_int, C.c_int, C.c_int, C.c_double, _F64, _F32, C.c_int, _F64, _F64, _F64,
@@ -167,12 +168,11 @@ class SubsetChain:
         assert self.h.shape == (self.nfoc, self.nrout)
         Gd_sub = np.ascontiguousarray(Gd_sub, dtype=np.float32)
         assert Gd_sub.shape == (self.nfoc, self.nrout, self.nt)
-        # O4 on the subset: f1plus = f2 = T G_d; f1min = pmin = 0   [PAPER.md:19, 67, 74-75]
-        TG = np.roll(Gd_sub[..., ::-1], 1, axis=-1).astype(np.float64)
-        self.f1plus = TG.copy()
-        self.f2 = TG.copy()
-        self.f1min = np.zeros_like(TG)
-        self.pmin = np.zeros_like(TG)
+        # O4 on the subset (orc_init_subset): f1plus = f2 = T G_d; f1min = pmin = 0   [PAPER.md:19, 67, 74-75]
+        shape = (self.nfoc, self.nrout, self.nt)
+        self.f1plus, self.f2, self.f1min, self.pmin = (np.empty(shape, dtype=np.float64) for _ in range(4))
+        lib().orc_init_subset(self.nfoc * self.nrout, self.nt, Gd_sub.reshape(-1), None, _opt(self.f1plus), _opt(self.f2),
+                              _opt(self.f1min), _opt(self.pmin))
         self.it = 0
 
     def step(self, N_prev_all):
@@ -195,6 +195,14 @@ class SubsetChain:
                                 self.f1min.reshape(-1), self.f2.reshape(-1), self.pmin.reshape(-1), self.klo, self.khi,
                                 _opt(out.get("G")), _opt(out.get("Gplus")), _opt(out.get("Gminus")))
         return out
+
+
+def init_field(Gd):
+    """N_{-1} = T G_d as float64 (orc_init_subset; O4)."""
+    Gd = np.ascontiguousarray(Gd, dtype=np.float32)
+    out = np.empty(Gd.shape, dtype=np.float64)
+    lib().orc_init_subset(int(np.prod(Gd.shape[:-1])), Gd.shape[-1], Gd.reshape(-1), _opt(out), None, None, None, None)
+    return out
 
 
 def image(Gminus, f1plus, dt, dx):

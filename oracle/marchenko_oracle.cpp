@@ -177,6 +177,21 @@ void orc_synthesis(int nshot, int nrout, int nt, double dt, const double* w, con
   }
 }
 
+// O4 for a set of traces (every receiver, or the chosen subset): N_{-1} = f1plus = f2 = T G_d;  f1min = pmin = 0
+// [PAPER.md:19 "N_{-1} = f^+_{1,0} = G_d(-t)", 67, 74-75].  Gd: [ntr][nt] fp32; outputs [ntr][nt] double, any may be NULL.
+void orc_init_subset(int ntr, int nt, const float* Gd, double* N_init, double* f1plus, double* f2, double* f1min,
+                     double* pmin) {
+  for (size_t i = 0; i < (size_t)ntr; ++i)
+    for (int j = 0; j < nt; ++j) {
+      const double v = (double)Gd[i * nt + wrapi((long)nt - j, nt)];
+      if (N_init) N_init[i * nt + j] = v;
+      if (f1plus) f1plus[i * nt + j] = v;
+      if (f2) f2[i * nt + j] = v;
+      if (f1min) f1min[i * nt + j] = 0.0;
+      if (pmin) pmin[i * nt + j] = 0.0;
+    }
+}
+
 // O5 for a SUBSET of output receivers (one pass of the loop body), the "single step" of
 // N_prev [nfoc][nshot][nt] is the previous iterate at EVERY source position; R [nshot][nrout][nt]
 // holds the traces of the chosen output receivers for every shot; h [nfoc][nrout] their window half-widths.
@@ -276,11 +291,8 @@ int orc_marchenko(int n, int nt, double dt, double dx, double fmin, double fmax,
   orc_window((int)ntr, nt, dt, eps, td, h.data());
 
   // O4: N_{-1} = f1plus = f2 = T G_d;  f1min = pmin = 0      [PAPER.md:19, 67, 74-75]
-  std::vector<double> N(tot), Nn(tot), f1plus(tot), f2(tot), f1min(tot, 0.0), pmin(tot, 0.0);
-  for (size_t i = 0; i < ntr; ++i)
-    for (int j = 0; j < nt; ++j) N[i * nt + j] = (double)Gd[i * nt + wrapi((long)nt - j, nt)];
-  f1plus = N;
-  f2 = N;
+  std::vector<double> N(tot), Nn(tot), f1plus(tot), f2(tot), f1min(tot), pmin(tot);
+  orc_init_subset((int)ntr, nt, Gd, N.data(), f1plus.data(), f2.data(), f1min.data(), pmin.data());
 
   // O5: niter passes, i = 0 .. niter-1                        [PAPER.md:68, 76; reading G6]
   for (int it = 0; it < niter; ++it) {

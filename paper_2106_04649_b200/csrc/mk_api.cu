@@ -161,11 +161,37 @@ int contract(mk_ctx* c, int slot, float2* Shat, int nfoc, int ldf, int ldb, int 
   else if (regime == 2) rc = launch_syn_gemm(c, slot ? c->d_Nhat2 : c->d_Nhat, Shat, ldf);
   else rc = launch_syn_tc(c, slot, slot ? c->d_Bhi2 : c->d_Bhi, slot ? c->d_Blo2 : c->d_Blo, Shat, nfoc, ldf, ldb);
   if (timed) cudaEventRecord(e1, c->stream);
-  c->regime_used = regime;
+  c->last_regime = regime;  // information only (MK_INFO_REGIME_USED); the run's regime is c->run_regime
   return rc;
 }
 
 bool is_pow2(int v) { return v > 0 && (v & (v - 1)) == 0; }
+
+// Calls that change what a run was started from (R^, eps, the operand layout) END the run in progress: the next
+// mk_step / mk_finish returns MK_ERR_STATE until mk_begin.  Between the two halves of a step they are refused.
+int end_run(mk_ctx* c, const char* who) {
+  if (c->contracted) return set_err(c, MK_ERR_STATE, std::string(who) + " between mk_step_contract and mk_step_post");
+  c->begun = false;
+  c->prepared_field = 0;
+  return MK_OK;
+}
+
+bool overlaps(const void* a, const void* b, size_t bytes) {
+  if (!a || !b) return false;
+  const char* x = static_cast<const char*>(a);
+  const char* y = static_cast<const char*>(b);
+  return x < y + bytes && y < x + bytes;
+}
+
+// outputs of the finals (and N_last) are written while the accumulators are still being read: they must not overlap
+// f1plus / f1min (the caller's fields when mk_run accumulates in them, else the library's)
+int check_output_alias(mk_ctx* c, const mk_outputs* o, const float* acc_plus, const float* acc_min, size_t bytes) {
+  const float* outs[4] = {o->N_last, o->G, o->Gplus, o->Gminus};
+  for (const float* p : outs)
+    if (overlaps(p, acc_plus, bytes) || overlaps(p, acc_min, bytes))
+      return set_err(c, MK_ERR_INVALID_ARG, "N_last / G / Gplus / Gminus must not overlap the f1plus / f1min fields");
+  return MK_OK;
+}
 
 __global__ void k_image(const float* __restrict__ Gminus, const float* __restrict__ f1plus, float* __restrict__ image, int n, int nt,
                         float w_mid, float w_end) {
@@ -195,9 +221,15 @@ __global__ void k_image(const float* __restrict__ Gminus, const float* __restric
 
 using namespace mk;
 
+// every entry point: reject a null / poisoned context and make the context's device current (the caller may have
+// switched devices between calls; kernels, allocations and IPC opens must go to the GPU the context lives on)
 #define MK_GUARD(ctx)                                          \
   if (!(ctx)) return MK_ERR_INVALID_ARG;                       \
-  if ((ctx)->sticky) return (ctx)->sticky;
+  if ((ctx)->sticky) return (ctx)->sticky;                     \
+  if (cudaSetDevice((ctx)->dev) != cudaSuccess) {              \
+    cudaGetLastError();                                        \
+    return set_err((ctx), MK_ERR_CUDA, "cudaSetDevice failed"); \
+  }
 
 extern "C" {
 
@@ -245,6 +277,7 @@ int mk_create_sharded(mk_ctx** out, int nshot, int nrec, int nt, double dt, doub
   c->ld = ((nshot + 15) / 16) * 16;
   c->plan = mkfft::make_plan(nt);
   if (int rc = check_cuda(c, cudaGetDevice(&dev), "cudaGetDevice")) return rc;
+  c->dev = dev;
   int v = 0;
   cudaDeviceGetAttribute(&v, cudaDevAttrMultiProcessorCount, dev);
   c->num_sms = v;
@@ -321,7 +354,8 @@ int mk_set_option(mk_ctx* c, int key, double value) {
   switch (key) {
     case MK_OPT_EPS_SAMPLES:
       if (value < 0 || value > c->nt) return set_err(c, MK_ERR_INVALID_ARG, "eps out of range");
-      if (c->begun) return set_err(c, MK_ERR_STATE, "eps cannot change during a run");
+      if ((int)value != c->eps)
+        if (int rc = end_run(c, "MK_OPT_EPS_SAMPLES")) return rc;  // the window table of a run in progress would be stale
       c->eps = (int)value;
       return MK_OK;
     case MK_OPT_REGIME:
@@ -371,7 +405,7 @@ int mk_get_info(mk_ctx* c, int key, double* value) {
     }
     case MK_INFO_SYN_RESET: c->ev_used = 0; *value = 0; return MK_OK;
     case MK_INFO_KERNEL_LAUNCHES: *value = (double)c->launches; return MK_OK;
-    case MK_INFO_REGIME_USED: *value = c->regime_used; return MK_OK;
+    case MK_INFO_REGIME_USED: *value = c->last_regime; return MK_OK;
     case MK_INFO_DEVICE_BYTES: *value = (double)c->device_bytes; return MK_OK;
     default: return set_err(c, MK_ERR_INVALID_ARG, "unknown info key");
   }
@@ -380,7 +414,7 @@ int mk_get_info(mk_ctx* c, int key, double* value) {
 int mk_load_R(mk_ctx* c, const float* d_R_time, int shot0, int nshots) {
   MK_GUARD(c);
   if (!d_R_time || shot0 < 0 || nshots <= 0 || shot0 + nshots > c->n) return set_err(c, MK_ERR_INVALID_ARG, "mk_load_R: bad shot range");
-  if (c->begun) return set_err(c, MK_ERR_STATE, "mk_load_R during a run");
+  if (int rc = end_run(c, "mk_load_R")) return rc;  // a run in progress was started from another R^: it is over
   if (int rc = launch_load_R(c, d_R_time, shot0, nshots)) return rc;
   for (int s = shot0; s < shot0 + nshots; ++s)
     if (!c->shot_loaded[s]) {
@@ -434,10 +468,10 @@ static int begin_impl(mk_ctx* c, const float* d_Gd, const float* d_td, int nfoc,
   c->nfoc = nfoc;
   c->ldf = ldf;
   c->ldb = ldb;
-  c->regime_used = regime;
+  c->run_regime = regime;
   c->iter = 0;
   c->contracted = false;
-  c->have_Gminus = false;
+  c->prepared_field = 0;
   if (int rc = prepare_operand(c, 0, regime, nfoc, ldf, ldb)) return rc;
   if (int rc = check_cuda(c, cudaMemsetAsync(c->d_phat, 0, nS * sizeof(float2), c->stream), "memset phat")) return rc;
   if (int rc = check_cuda(c, cudaMemsetAsync(c->acc_min, 0, ntime * sizeof(float), c->stream), "memset f1min")) return rc;
@@ -459,7 +493,7 @@ int mk_step_contract(mk_ctx* c) {
   MK_GUARD(c);
   if (!c->begun) return set_err(c, MK_ERR_STATE, "mk_step before mk_begin");
   if (c->contracted) return set_err(c, MK_ERR_STATE, "mk_step_contract twice without mk_step_post");
-  if (int rc = contract(c, 0, c->d_Shat, c->nfoc, c->ldf, c->ldb, c->regime_used)) return rc;                       // a2  [PAPER.md:69]
+  if (int rc = contract(c, 0, c->d_Shat, c->nfoc, c->ldf, c->ldb, c->run_regime)) return rc;                       // a2  [PAPER.md:69]
   c->contracted = true;
   return MK_OK;
 }
@@ -467,7 +501,7 @@ int mk_step_contract(mk_ctx* c) {
 int mk_step_post(mk_ctx* c, float* d_N_i) {
   MK_GUARD(c);
   if (!c->begun || !c->contracted) return set_err(c, MK_ERR_STATE, "mk_step_post without mk_step_contract");
-  const int regime = c->regime_used;
+  const int regime = c->run_regime;
   if (int rc = check_peers(c, 0)) return rc;
   if (int rc = launch_post(c, operand_out(c, 0, regime, c->ldf, c->ldb), (c->iter % 2) == 0, d_N_i)) return rc;     // a3..a6
   c->operand_stale[0] = c->nrow != c->n;
@@ -493,6 +527,11 @@ int mk_finish(mk_ctx* c, const mk_outputs* o) {
   if (!o) return set_err(c, MK_ERR_INVALID_ARG, "mk_finish: null outputs");
   if (o->N_last) return set_err(c, MK_ERR_INVALID_ARG, "N_last is delivered by mk_run (or by mk_step's d_N_i), not by mk_finish");
   const size_t bytes = (size_t)c->nfoc * c->n * c->nt * sizeof(float);
+  if (int rc = check_output_alias(c, o, c->acc_plus, c->acc_min, bytes)) return rc;
+  if ((o->f1plus && o->f1plus != c->acc_plus && (overlaps(o->f1plus, c->acc_plus, bytes) || overlaps(o->f1plus, c->acc_min, bytes))) ||
+      (o->f1min && o->f1min != c->acc_min && (overlaps(o->f1min, c->acc_plus, bytes) || overlaps(o->f1min, c->acc_min, bytes))) ||
+      (o->f1plus && overlaps(o->f1plus, o->f1min, bytes)))
+    return set_err(c, MK_ERR_INVALID_ARG, "mk_finish: the f1plus / f1min outputs overlap each other or the accumulators");
   if (o->f1plus && o->f1plus != c->acc_plus)  // mk_run accumulates in the caller's field directly
     if (int rc = check_cuda(c, cudaMemcpyAsync(o->f1plus, c->acc_plus, bytes, cudaMemcpyDeviceToDevice, c->stream), "copy f1plus")) return rc;
   if (o->f1min && o->f1min != c->acc_min)
@@ -502,7 +541,7 @@ int mk_finish(mk_ctx* c, const mk_outputs* o) {
   // Few focal points: the two extra syntheses of the finals ("estimating each component requires an extra
   // synthesis") are ONE pass over R^ with 2 nfoc right-hand sides — columns [0, nfoc) = spectrum of f1plus (G^-),
   // [nfoc, 2 nfoc) = spectrum of T f1min (G^+) — in the bandwidth-bound regime that costs little more than one.
-  const bool fuse = o->Gminus && o->Gplus && c->fused_finals && c->regime_used == 1 && (c->nfoc == 1 || c->nfoc == 2 || c->nfoc == 4) &&
+  const bool fuse = o->Gminus && o->Gplus && c->fused_finals && c->run_regime == 1 && (c->nfoc == 1 || c->nfoc == 2 || c->nfoc == 4) &&
                     gemv_supported(c, 2 * c->nfoc);
   if (fuse) {
     const int nf = c->nfoc, ldf2 = 2 * nf, ldb2 = ldb_for(ldf2);
@@ -533,7 +572,7 @@ int mk_finish_prepare(mk_ctx* c, int field) {
   MK_GUARD(c);
   if (!c->begun) return set_err(c, MK_ERR_STATE, "mk_finish_prepare before mk_begin");
   if (field != MK_FIELD_GMINUS && field != MK_FIELD_GPLUS) return set_err(c, MK_ERR_INVALID_ARG, "mk_finish_prepare: unknown field");
-  const int regime = c->regime_used;
+  const int regime = c->run_regime;
   if (int rc = scratch_operands(c, regime, c->nfoc, c->ldf, c->ldb)) return rc;
   // G^- = R f1plus - f1min [PAPER.md:87-88; G5]: operand = spectrum of f1plus;  G^+ = T f1plus - R (T f1min) [PAPER.md:24; G4]:
   // operand = spectrum of T f1min = conj of the spectrum of f1min
@@ -549,7 +588,7 @@ int mk_finish_complete(mk_ctx* c, int field, float* d_out) {
   MK_GUARD(c);
   if (!d_out) return set_err(c, MK_ERR_INVALID_ARG, "mk_finish_complete: null output");
   if (!c->begun || c->prepared_field != field || field == 0) return set_err(c, MK_ERR_STATE, "mk_finish_complete without the matching mk_finish_prepare");
-  const int regime = c->regime_used;
+  const int regime = c->run_regime;
   if (int rc = contract(c, 1, c->d_Shat2, c->nfoc, c->ldf, c->ldb, regime)) return rc;
   c->prepared_field = 0;
   if (field == MK_FIELD_GMINUS) return launch_inv(c, c->d_Shat2, c->nfoc, c->ldf, d_out, 1.f, c->acc_min, -1.f, nullptr, 0.f);
@@ -564,7 +603,7 @@ int mk_operand(mk_ctx* c, int slot, mk_operand_view* v) {
   v->nb = c->nb;
   v->row0 = c->r0;
   v->nrows = c->nrow;
-  if (c->regime_used == 3) {
+  if (c->run_regime == 3) {
     v->nplanes = 2;
     v->plane[0] = slot ? c->d_Bhi2 : c->d_Bhi;
     v->plane[1] = slot ? c->d_Blo2 : c->d_Blo;
@@ -625,16 +664,17 @@ int mk_ipc_close(void* d_ptr) {
 int mk_operand_reserve(mk_ctx* c, int nfoc) {
   MK_GUARD(c);
   if (nfoc <= 0) return set_err(c, MK_ERR_INVALID_ARG, "mk_operand_reserve: bad nfoc");
-  if (c->begun && nfoc != c->nfoc) c->begun = false;  // a run with another batch size is over
   int regime = 0;
   if (int rc = resolve_regime(c, nfoc, &regime)) return rc;
   const int ldf = ldf_for(regime, nfoc), ldb = ldb_for(nfoc);
+  if (c->begun && (nfoc != c->nfoc || regime != c->run_regime))  // another operand layout: the run in progress is over
+    if (int rc = end_run(c, "mk_operand_reserve")) return rc;
   if (int rc = prepare_operand(c, 0, regime, nfoc, ldf, ldb)) return rc;
   if (int rc = prepare_operand(c, 1, regime, nfoc, ldf, ldb)) return rc;
   c->nfoc = nfoc;
   c->ldf = ldf;
   c->ldb = ldb;
-  c->regime_used = regime;
+  c->run_regime = regime;
   c->reserved = true;
   return MK_OK;
 }
@@ -665,8 +705,14 @@ int mk_run(mk_ctx* c, const float* d_Gd, const float* d_td, int nfoc, int niter,
   if (c->nrow != c->n) return set_err(c, MK_ERR_STATE, "row-sharded context: drive mk_begin / mk_step / mk_finish_* with the exchanges in between");
   if (niter < 0 || !o) return set_err(c, MK_ERR_INVALID_ARG, "mk_run: bad arguments");
   if (o->N_last && niter == 0) return set_err(c, MK_ERR_INVALID_ARG, "N_last needs niter >= 1");
-  if ((o->f1plus && (o->f1plus == o->f1min || (const float*)o->f1plus == d_Gd)) || (o->f1min && (const float*)o->f1min == d_Gd))
-    return set_err(c, MK_ERR_INVALID_ARG, "mk_run: f1plus / f1min must not alias each other or G_d");
+  if (!d_Gd || nfoc <= 0) return set_err(c, MK_ERR_INVALID_ARG, "mk_run: bad arguments");
+  {
+    const size_t bytes = (size_t)nfoc * c->n * c->nt * sizeof(float);
+    if (overlaps(o->f1plus, o->f1min, bytes) || overlaps(o->f1plus, d_Gd, bytes) || overlaps(o->f1min, d_Gd, bytes))
+      return set_err(c, MK_ERR_INVALID_ARG, "mk_run: f1plus / f1min must not overlap each other or G_d");
+    // with no caller field the library's own accumulators are used; they cannot overlap caller memory
+    if (int rc = check_output_alias(c, o, o->f1plus, o->f1min, bytes)) return rc;
+  }
   if (int rc = begin_impl(c, d_Gd, d_td, nfoc, o->f1plus, o->f1min)) return rc;  // accumulate in the caller's fields
   for (int i = 0; i < niter; ++i)
     if (int rc = mk_step(c, i == niter - 1 ? o->N_last : nullptr)) return rc;

@@ -68,10 +68,10 @@ struct mk_ctx {
   float* d_Bhi2 = nullptr;
   float* d_Blo2 = nullptr;
   size_t cap_B2 = 0;
-  long long operand_key[2] = {0, 0};
+  long long operand_key[2] = {0, 0};   // layout the slot's operand was last zeroed for (0 = not zeroed)
   int npeer[2] = {0, 0};               // mk_operand_attach
   float* peer_plane[2][7][2] = {};     // [slot][peer][plane]
-  long long peer_key[2] = {0, 0};      // operand layout the peers were attached for  // layout the slot's operand was last zeroed for (0 = not zeroed)
+  long long peer_key[2] = {0, 0};      // operand layout the peers were attached for
   // regime 3: cached TMA descriptors (CUtensorMap is 128 bytes, 64-byte aligned), built by mk_syn_tc.cu
   alignas(64) unsigned char tmap_A[128];
   alignas(64) unsigned char tmap_B[2][2][128];  // [main / scratch][hi / lo]
@@ -83,13 +83,12 @@ struct mk_ctx {
   cudaStream_t copy_stream = nullptr;  // mk_run_host: device -> host copies overlapping the finals
   cudaEvent_t copy_ev = nullptr;
   size_t cap_stage = 0;
-  float* d_Gminus = nullptr;  // kept by mk_finish when G^- was requested (mk_image)
-  size_t cap_Gminus = 0;
-  bool have_Gminus = false;
 
   size_t device_bytes = 0;
   long launches = 0;
-  int regime_used = 0;
+  int run_regime = 0;   // regime of the run in progress / of the reserved operands: set by mk_begin and mk_operand_reserve only
+  int last_regime = 0;  // regime of the last contraction launch (MK_INFO_REGIME_USED; information only)
+  int dev = 0;          // CUDA device the context lives on (made current at the top of every entry point)
 
   // timing of contraction launches
   std::vector<cudaEvent_t> ev;  // pairs

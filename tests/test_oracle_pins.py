@@ -333,6 +333,31 @@ def test_subset_chain_fed_with_full_iterates_equals_the_full_chain_restricted():
         np.testing.assert_array_equal(fin[nm], full[nm][:, recs])
 
 
+def test_init_is_the_time_reversed_first_arrival():
+    """O4 (orc_init_subset; "N_{-1} = f^+_{1,0} = G_d(-t)", 67, 74-75) on a hand-written trace: t -> -t with
+    negative times stored wrapped keeps samples 0 and nt/2 in place and swaps j with nt - j; applying it twice is the
+    identity; and the spectrum of the result is the conjugate of the input's (real trace), which is what a
+    time reversal is, independent of any index formula."""
+    g = np.array([[[1.0, 2.0, 3.0, 4.0, 5.0, 6.0, 7.0, 8.0]]], np.float32)
+    np.testing.assert_array_equal(oracle.init_field(g)[0, 0], [1.0, 8.0, 7.0, 6.0, 5.0, 4.0, 3.0, 2.0])
+    x = rng.standard_normal((2, 3, 64)).astype(np.float32)
+    y = oracle.init_field(x)
+    np.testing.assert_array_equal(oracle.init_field(y.astype(np.float32)), x.astype(np.float64))
+    np.testing.assert_allclose(np.fft.fft(y), np.conj(np.fft.fft(x.astype(np.float64))), atol=1e-12)
+    # the chain starts from it: f1plus = f2 = T G_d, f1min = pmin = 0, and with niter = 0 nothing else happens
+    n, nt = 3, 64
+    R = np.zeros((n, n, nt), np.float32)
+    td = np.full((2, n), 0.1, np.float32)
+    o = oracle.marchenko(R, x, td, 0.004, 10.0, 10.0, 100.0, niter=0)
+    np.testing.assert_array_equal(o["f1plus"], y)
+    np.testing.assert_array_equal(o["f2"], y)
+    assert not o["f1min"].any() and not o["pmin"].any()
+    sub = oracle.SubsetChain(R[:, [0, 2]], td[:, [0, 2]], x[:, [0, 2]], 0.004, 10.0, 10.0, 100.0)
+    np.testing.assert_array_equal(sub.f1plus, y[:, [0, 2]])
+    np.testing.assert_array_equal(sub.f2, y[:, [0, 2]])
+    assert not sub.f1min.any() and not sub.pmin.any()
+
+
 def test_image_is_the_zero_lag_of_the_convolution():
     """image[f] = dt sum_r w[r] (G^- (*) f1plus)[0]: brute force on a tiny case and numpy's FFT convolution theorem."""
     nfoc, n, nt, dt, dx = 3, 5, 16, 0.004, 10.0
