@@ -31,6 +31,7 @@
 #include <cuda.h>
 
 #include <algorithm>
+#include <cstdlib>
 
 #include "mk_internal.cuh"
 
@@ -149,6 +150,7 @@ struct TcParams {
   int nblk, stages;     // column blocks per B' tile, stages of the ring
   int mp;               // M tiles per CTA tile (1, or 2 when ncols <= 128: accumulator m lives in columns 128 m .. of the buffer)
   size_t s_row;         // floats between consecutive receivers of S^: nb * 2 ldf
+  int dbg;              // TEMP experiment flags: 1 no TMA, 2 no split, 4 no MMA
 };
 
 __global__ void __launch_bounds__(kThreads, 1)
@@ -203,6 +205,7 @@ k_syn_gemm_tf32x3(const __grid_constant__ CUtensorMap tmA, const __grid_constant
         for (int kb = 0; kb < KB; ++kb) {
           mbar_wait(empty + s, ph ^ 1);
           uint8_t* st = smem + (size_t)s * STAGE_BYTES;
+          if (P.dbg & 1) { mbar_arrive(full + s); if (++s == STAGES) { s = 0; ph ^= 1; } continue; }
           mbar_expect_tx(full + s, TX_BYTES);
           for (int m = 0; m < MP; ++m)  // rows past the last receiver arrive as zeros (and still count their bytes)
             tma_load_3d(&tmA, full + s, st + m * A_BYTES, kb * BK, kk, (mi * MP + m) * BM);
@@ -239,6 +242,7 @@ k_syn_gemm_tf32x3(const __grid_constant__ CUtensorMap tmA, const __grid_constant
             const uint32_t b_hi = a_raw + 2 * AREG, b_lo = b_hi + B_BYTES;
 #pragma unroll
             for (int j = 0; j < BK / UK; ++j) {
+              if (P.dbg & 4) break;
               // A: K-major, 64-byte rows, SWIZZLE_64B: 8-row groups 512 B apart; a k'-chunk is 32 B further along the row
               const uint64_t da_raw = smem_desc(a_raw + j * 32, 16, 512, LAYOUT_SW64);
               const uint64_t da_lo = smem_desc(a_lo + j * 32, 16, 512, LAYOUT_SW64);
@@ -279,6 +283,7 @@ k_syn_gemm_tf32x3(const __grid_constant__ CUtensorMap tmA, const __grid_constant
       for (int kb = 0; kb < KB; ++kb, ++cnt) {
         if ((int)(cnt & 1) == sw) {
           mbar_wait(full + s, ph);
+          if (P.dbg & 2) { if (lane == 0) mbar_arrive(split + s); if (++s == STAGES) { s = 0; ph ^= 1; } continue; }
           const float4* src = reinterpret_cast<const float4*>(smem + (size_t)s * STAGE_BYTES);
           float4* dst = reinterpret_cast<float4*>(smem + (size_t)s * STAGE_BYTES + AREG);
           constexpr int kPer = (int)(A_BYTES / 16) / 32;  // 16 float4 per lane and M tile
@@ -419,6 +424,7 @@ int launch_syn_tc(mk_ctx* c, int slot, const float* d_Bhi, const float* d_Blo, f
     c->tmap_B_ldb[slot] = ldb;
   }
   TcParams P;
+  { const char* e = getenv("MK_TC_DEBUG"); P.dbg = e ? atoi(e) : 0; }
   P.n = c->nrow;  // row sharding: local rows; S^ is offset to the first one below
   P.nb = c->nb;
   P.ld = c->ld;

@@ -2,7 +2,8 @@
 test box, map each other's operand planes through CUDA IPC (mk_ipc_export / mk_ipc_open), attach them
 (mk_operand_attach) and run Algorithm 1 with shard.run_row_sharded_fused: the only thing that crosses the process
 boundary besides the peer stores of k_fwd / k_post is the host barrier (gloo).  No kernel waits on another process.
-Each rank checks its own receiver rows against a single-context run of the same problem."""
+Each rank checks its own receiver rows against the fp64 oracle (north_star tolerances) and, bit for bit, against a
+single-context run of the same problem."""
 import os
 import socket
 
@@ -55,9 +56,14 @@ def _worker(rank, world, port, regime, q):
         sl = slice(rows.start, rows.stop)
         worst = max(rel_l2(outs[nm].cpu().numpy()[:, sl], whole[nm][:, sl]) for nm in names)
         alive = float(np.linalg.norm(whole["N_last"])) > 0.0
-        q.put((rank, worst, alive, len(opened)))
+        # the parity bar proper: this rank's rows against the fp64 oracle (north_star tolerances)
+        import oracle
+        ref = oracle.marchenko(R, Gd, td, cfg.dt, cfg.dx, cfg.fmin, cfg.fmax, cfg.niter, cfg.eps)
+        e_it = rel_l2(outs["N_last"].cpu().numpy()[:, sl], ref["N_iters"][-1][:, sl])
+        e_fin = max(rel_l2(outs[nm].cpu().numpy()[:, sl], ref[nm][:, sl]) for nm in names[1:])
+        q.put((rank, worst, alive, len(opened), e_it, e_fin))
     except Exception as e:   # report instead of hanging the other rank
-        q.put((rank, repr(e), False, -1))
+        q.put((rank, repr(e), False, -1, 1.0, 1.0))
     finally:
         try:
             for p in opened:
@@ -83,7 +89,8 @@ def test_two_processes_one_gpu_fused_peer_stores(regime):
     for p in procs:
         p.join(timeout=120)
     print(res)
-    for rank, worst, alive, nopened in res:
+    for rank, worst, alive, nopened, e_it, e_fin in res:
         assert isinstance(worst, float), worst
         assert alive and worst <= 1e-6
+        assert e_it <= 2e-5 and e_fin <= 1e-4, (e_it, e_fin)
         assert nopened == (2 if regime != 3 else 4)      # one peer x two slots x planes
