@@ -58,7 +58,7 @@ enum {
   MK_OPT_EPS_SAMPLES = 1, /* window margin eps in samples (default 8; BASELINE.json config 0; G2) */
   MK_OPT_REGIME = 2,      /* contraction kernel: 0 auto (default: 1 for nfoc <= 8, else 3), 1 streaming GEMV,
                              2 FP32-FFMA GEMM, 3 tcgen05 3xTF32 GEMM with chunked fp32 accumulation (sm_100 only;
-                             MK_ERR_INVALID_ARG otherwise) */
+                             MK_ERR_INVALID_ARG otherwise).  Affects runs / syntheses started afterwards */
   MK_OPT_TIMING = 3,      /* 1: bracket every contraction launch with CUDA events on the context's stream */
   MK_OPT_FUSED_FINALS = 5, /* 1 (default): with 1, 2 or 4 focal points mk_finish / mk_run compute the extra syntheses of G^- and
                              G^+ in ONE pass over R^ (2 nfoc right-hand sides, streaming GEMV); 0: one pass each */
@@ -172,10 +172,11 @@ int mk_image(mk_ctx* ctx, const float* d_Gminus, float* d_image);
 int mk_create_sharded(mk_ctx** out, int nshot, int nrec, int nt, double dt, double dx, double fmin, double fmax,
                       int row0, int nrows);
 
-/* Where the operand of slot 0 (the run) or 1 (finals) lives.  plane[p] (p < nplanes) is a device array
- * [nb][rows_per_bin][row_floats] fp32; receiver r occupies rows rows_per_rec * r .. rows_per_rec * (r + 1) - 1 of
- * every bin.  (Regimes 1, 2: one plane, complex N^[k][s][f] as interleaved floats; regime 3: the tf32 hi / lo planes
- * of the real operand, two rows per receiver.)  Valid after mk_begin (slot 0) / mk_finish_prepare (slot 1). */
+/* Where the operand of slot 0 (the run) or 1 (finals) lives.  plane[0] is a device array [nb][rows_per_bin][row_floats]
+ * fp32: the complex operand N^[k][s][f] as interleaved (re, im) floats, one row per source position (rows_per_rec = 1,
+ * rows_per_bin = ld_shot, row_floats = 2 ldf with ldf = nfoc padded to the regime's granularity: 1 / 4 / 16 focal points
+ * for regimes 1 / 2 / 3).  Every regime reads this one plane (nplanes = 1; plane[1] is unused and NULL).
+ * Valid after mk_begin (slot 0) / mk_finish_prepare (slot 1). */
 typedef struct mk_operand_view {
   float* plane[2];
   int nplanes, nb, rows_per_bin, rows_per_rec, row_floats, row0, nrows;

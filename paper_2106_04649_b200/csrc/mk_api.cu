@@ -70,27 +70,17 @@ int resolve_regime(mk_ctx* c, int nfoc, int* regime) {
   return MK_OK;
 }
 
-inline int ldf_for(int regime, int nfoc) { return regime == 1 ? nfoc : ((nfoc + 3) / 4) * 4; }
+// columns of N^ / S^ / p^ per bin row: the GEMV reads nfoc, the FFMA GEMM 128-bit pairs, the tcgen05 GEMM 32-float TMA boxes
+inline int ldf_for(int regime, int nfoc) { return regime == 1 ? nfoc : (regime == 2 ? ((nfoc + 3) / 4) * 4 : ((nfoc + 15) / 16) * 16); }
 
-inline int ldb_for(int nfoc) { return ((2 * nfoc + 31) / 32) * 32; }
-
-// the operand of slot 0 (the run) or 1 (scratch: mk_synthesis, finals) in the layout of `regime`
-OperandOut operand_out(mk_ctx* c, int slot, int regime, int ldf, int ldb) {
+// the operand of slot 0 (the run) or 1 (scratch: mk_synthesis, finals)
+OperandOut operand_out(mk_ctx* c, int slot, int ldf) {
   OperandOut O{};
   O.ldf = ldf;
-  O.ldb = ldb;
-  if (regime == 3) {
-    O.bhi = slot ? c->d_Bhi2 : c->d_Bhi;
-    O.blo = slot ? c->d_Blo2 : c->d_Blo;
-  } else {
-    O.plain = slot ? c->d_Nhat2 : c->d_Nhat;
-  }
+  O.plain = slot ? c->d_Nhat2 : c->d_Nhat;
   if (c->npeer[slot] > 0 && c->peer_key[slot] == c->operand_key[slot] && c->operand_key[slot] != 0) {
     O.npeer = c->npeer[slot];
-    for (int p = 0; p < O.npeer; ++p) {
-      O.peer[p][0] = c->peer_plane[slot][p][0];
-      O.peer[p][1] = c->peer_plane[slot][p][1];
-    }
+    for (int p = 0; p < O.npeer; ++p) O.peer[p] = reinterpret_cast<float2*>(c->peer_plane[slot][p]);
   }
   return O;
 }
@@ -98,24 +88,8 @@ OperandOut operand_out(mk_ctx* c, int slot, int regime, int ldf, int ldb) {
 // allocate the operand of a slot; zero it when the buffer is new or its layout changed.  Pad rows / columns must be
 // zero and no kernel ever writes a non-zero there (the forward transforms store rows r < n, columns f < nfoc, and zeros
 // into the odd pad column of a pair), so an operand that keeps its layout needs no second memset.
-int prepare_operand(mk_ctx* c, int slot, int regime, int nfoc, int ldf, int ldb) {
-  const long long key = ((long long)regime << 56) ^ ((long long)nfoc << 32) ^ ((long long)ldf << 16) ^ (long long)ldb;
-  if (regime == 3) {
-    const size_t cnt = (size_t)c->nb * 2 * c->ld * ldb;
-    float** hi = slot ? &c->d_Bhi2 : &c->d_Bhi;
-    float** lo = slot ? &c->d_Blo2 : &c->d_Blo;
-    size_t* cap = slot ? &c->cap_B2 : &c->cap_B;
-    const float* before = *hi;
-    size_t cap2 = *cap;
-    if (int rc = ensure(c, hi, cap, cnt, "B' hi plane")) return rc;
-    if (int rc = ensure(c, lo, &cap2, cnt, "B' lo plane")) return rc;
-    if (*hi == before && c->operand_key[slot] == key) return MK_OK;
-    c->operand_key[slot] = 0;
-    if (int rc = check_cuda(c, cudaMemsetAsync(*hi, 0, cnt * sizeof(float), c->stream), "memset B' hi")) return rc;
-    if (int rc = check_cuda(c, cudaMemsetAsync(*lo, 0, cnt * sizeof(float), c->stream), "memset B' lo")) return rc;
-    c->operand_key[slot] = key;
-    return MK_OK;
-  }
+int prepare_operand(mk_ctx* c, int slot, int nfoc, int ldf) {
+  const long long key = ((long long)nfoc << 32) ^ (long long)ldf;
   const size_t nN = (size_t)c->nb * c->ld * ldf;
   float2** p = slot ? &c->d_Nhat2 : &c->d_Nhat;
   size_t* cap = slot ? &c->cap_Nhat2 : &c->cap_Nhat;
@@ -136,7 +110,7 @@ int check_peers(mk_ctx* c, int slot) {
   return MK_OK;
 }
 
-int contract(mk_ctx* c, int slot, float2* Shat, int nfoc, int ldf, int ldb, int regime) {
+int contract(mk_ctx* c, int slot, float2* Shat, int nfoc, int ldf, int regime) {
   if (c->operand_stale[slot])
     return set_err(c, MK_ERR_STATE, "row-sharded context: the operand rows were not exchanged (mk_operand / mk_operand_exchanged)");
   cudaEvent_t e0 = nullptr, e1 = nullptr;
@@ -159,7 +133,7 @@ int contract(mk_ctx* c, int slot, float2* Shat, int nfoc, int ldf, int ldb, int 
   int rc;
   if (regime == 1) rc = launch_syn_gemv(c, slot ? c->d_Nhat2 : c->d_Nhat, Shat, nfoc);
   else if (regime == 2) rc = launch_syn_gemm(c, slot ? c->d_Nhat2 : c->d_Nhat, Shat, ldf);
-  else rc = launch_syn_tc(c, slot, slot ? c->d_Bhi2 : c->d_Bhi, slot ? c->d_Blo2 : c->d_Blo, Shat, nfoc, ldf, ldb);
+  else rc = launch_syn_tc(c, slot, slot ? c->d_Nhat2 : c->d_Nhat, Shat, ldf);
   if (timed) cudaEventRecord(e1, c->stream);
   c->last_regime = regime;  // information only (MK_INFO_REGIME_USED); the run's regime is c->run_regime
   return rc;
@@ -330,10 +304,6 @@ int mk_destroy(mk_ctx* c) {
   cudaFree(c->d_h);
   cudaFree(c->d_Nhat2);
   cudaFree(c->d_Shat2);
-  cudaFree(c->d_Bhi);
-  cudaFree(c->d_Blo);
-  cudaFree(c->d_Bhi2);
-  cudaFree(c->d_Blo2);
   cudaFree(c->d_stage);
   if (c->copy_stream) cudaStreamDestroy(c->copy_stream);
   if (c->copy_ev) cudaEventDestroy(c->copy_ev);
@@ -449,7 +419,7 @@ static int begin_impl(mk_ctx* c, const float* d_Gd, const float* d_td, int nfoc,
   if (c->shots_loaded != c->n) return set_err(c, MK_ERR_STATE, "mk_begin before every shot of R was loaded");
   int regime = 0;
   if (int rc = resolve_regime(c, nfoc, &regime)) return rc;
-  const int ldf = ldf_for(regime, nfoc), ldb = ldb_for(nfoc);
+  const int ldf = ldf_for(regime, nfoc);
   const size_t ntime = (size_t)nfoc * c->n * c->nt;
   const size_t nS = (size_t)c->n * c->nb * ldf;
   c->begun = false;
@@ -467,12 +437,11 @@ static int begin_impl(mk_ctx* c, const float* d_Gd, const float* d_td, int nfoc,
   }
   c->nfoc = nfoc;
   c->ldf = ldf;
-  c->ldb = ldb;
   c->run_regime = regime;
   c->iter = 0;
   c->contracted = false;
   c->prepared_field = 0;
-  if (int rc = prepare_operand(c, 0, regime, nfoc, ldf, ldb)) return rc;
+  if (int rc = prepare_operand(c, 0, nfoc, ldf)) return rc;
   if (int rc = check_cuda(c, cudaMemsetAsync(c->d_phat, 0, nS * sizeof(float2), c->stream), "memset phat")) return rc;
   if (int rc = check_cuda(c, cudaMemsetAsync(c->acc_min, 0, ntime * sizeof(float), c->stream), "memset f1min")) return rc;
   if (int rc = launch_window(c, d_td, c->d_h, nfoc * c->n)) return rc;
@@ -481,7 +450,7 @@ static int begin_impl(mk_ctx* c, const float* d_Gd, const float* d_td, int nfoc,
   const bool sharded = c->nrow != c->n;
   if (sharded)  // the rows of other ranks stay zero in this rank's fields
     if (int rc = check_cuda(c, cudaMemsetAsync(c->acc_plus, 0, ntime * sizeof(float), c->stream), "memset f1plus")) return rc;
-  if (int rc = launch_fwd(c, d_Gd, operand_out(c, 0, regime, ldf, ldb), nfoc, /*conj_out=*/true, c->acc_plus)) return rc;
+  if (int rc = launch_fwd(c, d_Gd, operand_out(c, 0, ldf), nfoc, /*conj_out=*/true, c->acc_plus)) return rc;
   c->operand_stale[0] = sharded;
   c->begun = true;
   return MK_OK;
@@ -493,7 +462,7 @@ int mk_step_contract(mk_ctx* c) {
   MK_GUARD(c);
   if (!c->begun) return set_err(c, MK_ERR_STATE, "mk_step before mk_begin");
   if (c->contracted) return set_err(c, MK_ERR_STATE, "mk_step_contract twice without mk_step_post");
-  if (int rc = contract(c, 0, c->d_Shat, c->nfoc, c->ldf, c->ldb, c->run_regime)) return rc;                       // a2  [PAPER.md:69]
+  if (int rc = contract(c, 0, c->d_Shat, c->nfoc, c->ldf, c->run_regime)) return rc;                       // a2  [PAPER.md:69]
   c->contracted = true;
   return MK_OK;
 }
@@ -501,9 +470,8 @@ int mk_step_contract(mk_ctx* c) {
 int mk_step_post(mk_ctx* c, float* d_N_i) {
   MK_GUARD(c);
   if (!c->begun || !c->contracted) return set_err(c, MK_ERR_STATE, "mk_step_post without mk_step_contract");
-  const int regime = c->run_regime;
   if (int rc = check_peers(c, 0)) return rc;
-  if (int rc = launch_post(c, operand_out(c, 0, regime, c->ldf, c->ldb), (c->iter % 2) == 0, d_N_i)) return rc;     // a3..a6
+  if (int rc = launch_post(c, operand_out(c, 0, c->ldf), (c->iter % 2) == 0, d_N_i)) return rc;     // a3..a6
   c->operand_stale[0] = c->nrow != c->n;
   c->contracted = false;
   ++c->iter;
@@ -515,10 +483,10 @@ int mk_step(mk_ctx* c, float* d_N_i) {
   return mk_step_post(c, d_N_i);
 }
 
-static int scratch_operands(mk_ctx* c, int regime, int nfoc, int ldf, int ldb) {
+static int scratch_operands(mk_ctx* c, int nfoc, int ldf) {
   const size_t nS = (size_t)c->n * c->nb * ldf;
   if (int rc = ensure(c, &c->d_Shat2, &c->cap_Shat2, nS, "Shat scratch")) return rc;
-  return prepare_operand(c, 1, regime, nfoc, ldf, ldb);
+  return prepare_operand(c, 1, nfoc, ldf);
 }
 
 int mk_finish(mk_ctx* c, const mk_outputs* o) {
@@ -544,14 +512,14 @@ int mk_finish(mk_ctx* c, const mk_outputs* o) {
   const bool fuse = o->Gminus && o->Gplus && c->fused_finals && c->run_regime == 1 && (c->nfoc == 1 || c->nfoc == 2 || c->nfoc == 4) &&
                     gemv_supported(c, 2 * c->nfoc);
   if (fuse) {
-    const int nf = c->nfoc, ldf2 = 2 * nf, ldb2 = ldb_for(ldf2);
+    const int nf = c->nfoc, ldf2 = 2 * nf;
     if (int rc = ensure(c, &c->d_Shat2, &c->cap_Shat2, (size_t)c->n * c->nb * ldf2, "Shat scratch")) return rc;
-    if (int rc = prepare_operand(c, 1, 1, ldf2, ldf2, ldb2)) return rc;
-    OperandOut O = operand_out(c, 1, 1, ldf2, ldb2);
+    if (int rc = prepare_operand(c, 1, ldf2, ldf2)) return rc;
+    OperandOut O = operand_out(c, 1, ldf2);
     if (int rc = launch_fwd(c, c->acc_plus, O, nf, false, nullptr)) return rc;
     O.plain += nf;
     if (int rc = launch_fwd(c, c->acc_min, O, nf, true, nullptr)) return rc;
-    if (int rc = contract(c, 1, c->d_Shat2, ldf2, ldf2, ldb2, 1)) return rc;
+    if (int rc = contract(c, 1, c->d_Shat2, ldf2, ldf2, 1)) return rc;
     if (int rc = launch_inv(c, c->d_Shat2, nf, ldf2, o->Gminus, 1.f, c->acc_min, -1.f, nullptr, 0.f)) return rc;       // [PAPER.md:87-88]
     if (int rc = launch_inv(c, c->d_Shat2 + nf, nf, ldf2, o->Gplus, -1.f, nullptr, 0.f, c->acc_plus, 1.f)) return rc;   // [G4]
   } else if (o->Gminus) {
@@ -572,13 +540,12 @@ int mk_finish_prepare(mk_ctx* c, int field) {
   MK_GUARD(c);
   if (!c->begun) return set_err(c, MK_ERR_STATE, "mk_finish_prepare before mk_begin");
   if (field != MK_FIELD_GMINUS && field != MK_FIELD_GPLUS) return set_err(c, MK_ERR_INVALID_ARG, "mk_finish_prepare: unknown field");
-  const int regime = c->run_regime;
-  if (int rc = scratch_operands(c, regime, c->nfoc, c->ldf, c->ldb)) return rc;
+  if (int rc = scratch_operands(c, c->nfoc, c->ldf)) return rc;
   // G^- = R f1plus - f1min [PAPER.md:87-88; G5]: operand = spectrum of f1plus;  G^+ = T f1plus - R (T f1min) [PAPER.md:24; G4]:
   // operand = spectrum of T f1min = conj of the spectrum of f1min
   if (int rc = check_peers(c, 1)) return rc;
   const bool minus = field == MK_FIELD_GMINUS;
-  if (int rc = launch_fwd(c, minus ? c->acc_plus : c->acc_min, operand_out(c, 1, regime, c->ldf, c->ldb), c->nfoc, !minus, nullptr)) return rc;
+  if (int rc = launch_fwd(c, minus ? c->acc_plus : c->acc_min, operand_out(c, 1, c->ldf), c->nfoc, !minus, nullptr)) return rc;
   c->operand_stale[1] = c->nrow != c->n;
   c->prepared_field = field;
   return MK_OK;
@@ -589,7 +556,7 @@ int mk_finish_complete(mk_ctx* c, int field, float* d_out) {
   if (!d_out) return set_err(c, MK_ERR_INVALID_ARG, "mk_finish_complete: null output");
   if (!c->begun || c->prepared_field != field || field == 0) return set_err(c, MK_ERR_STATE, "mk_finish_complete without the matching mk_finish_prepare");
   const int regime = c->run_regime;
-  if (int rc = contract(c, 1, c->d_Shat2, c->nfoc, c->ldf, c->ldb, regime)) return rc;
+  if (int rc = contract(c, 1, c->d_Shat2, c->nfoc, c->ldf, regime)) return rc;
   c->prepared_field = 0;
   if (field == MK_FIELD_GMINUS) return launch_inv(c, c->d_Shat2, c->nfoc, c->ldf, d_out, 1.f, c->acc_min, -1.f, nullptr, 0.f);
   return launch_inv(c, c->d_Shat2, c->nfoc, c->ldf, d_out, -1.f, nullptr, 0.f, c->acc_plus, 1.f);
@@ -603,20 +570,11 @@ int mk_operand(mk_ctx* c, int slot, mk_operand_view* v) {
   v->nb = c->nb;
   v->row0 = c->r0;
   v->nrows = c->nrow;
-  if (c->run_regime == 3) {
-    v->nplanes = 2;
-    v->plane[0] = slot ? c->d_Bhi2 : c->d_Bhi;
-    v->plane[1] = slot ? c->d_Blo2 : c->d_Blo;
-    v->rows_per_bin = 2 * c->ld;
-    v->rows_per_rec = 2;
-    v->row_floats = c->ldb;
-  } else {
-    v->nplanes = 1;
-    v->plane[0] = reinterpret_cast<float*>(slot ? c->d_Nhat2 : c->d_Nhat);
-    v->rows_per_bin = c->ld;
-    v->rows_per_rec = 1;
-    v->row_floats = 2 * c->ldf;
-  }
+  v->nplanes = 1;  // every regime reads the one complex operand N^[k][s][f] (interleaved floats)
+  v->plane[0] = reinterpret_cast<float*>(slot ? c->d_Nhat2 : c->d_Nhat);
+  v->rows_per_bin = c->ld;
+  v->rows_per_rec = 1;
+  v->row_floats = 2 * c->ldf;
   if (!v->plane[0]) return set_err(c, MK_ERR_STATE, "mk_operand: this slot has no operand yet");
   return MK_OK;
 }
@@ -666,14 +624,13 @@ int mk_operand_reserve(mk_ctx* c, int nfoc) {
   if (nfoc <= 0) return set_err(c, MK_ERR_INVALID_ARG, "mk_operand_reserve: bad nfoc");
   int regime = 0;
   if (int rc = resolve_regime(c, nfoc, &regime)) return rc;
-  const int ldf = ldf_for(regime, nfoc), ldb = ldb_for(nfoc);
+  const int ldf = ldf_for(regime, nfoc);
   if (c->begun && (nfoc != c->nfoc || regime != c->run_regime))  // another operand layout: the run in progress is over
     if (int rc = end_run(c, "mk_operand_reserve")) return rc;
-  if (int rc = prepare_operand(c, 0, regime, nfoc, ldf, ldb)) return rc;
-  if (int rc = prepare_operand(c, 1, regime, nfoc, ldf, ldb)) return rc;
+  if (int rc = prepare_operand(c, 0, nfoc, ldf)) return rc;
+  if (int rc = prepare_operand(c, 1, nfoc, ldf)) return rc;
   c->nfoc = nfoc;
   c->ldf = ldf;
-  c->ldb = ldb;
   c->run_regime = regime;
   c->reserved = true;
   return MK_OK;
@@ -692,8 +649,7 @@ int mk_operand_attach(mk_ctx* c, int slot, int npeers, const mk_operand_view* pe
     if (v.nplanes != mine.nplanes || v.nb != mine.nb || v.rows_per_bin != mine.rows_per_bin || v.rows_per_rec != mine.rows_per_rec ||
         v.row_floats != mine.row_floats || !v.plane[0] || (v.nplanes == 2 && !v.plane[1]))
       return set_err(c, MK_ERR_INVALID_ARG, "mk_operand_attach: a peer's operand has another layout");
-    c->peer_plane[slot][p][0] = v.plane[0];
-    c->peer_plane[slot][p][1] = v.plane[1];
+    c->peer_plane[slot][p] = v.plane[0];
   }
   c->npeer[slot] = npeers;
   c->peer_key[slot] = c->operand_key[slot];
@@ -790,10 +746,10 @@ int mk_synthesis(mk_ctx* c, const float* d_N_in, float* d_S_out, int nfoc) {
   if (c->shots_loaded != c->n) return set_err(c, MK_ERR_STATE, "mk_synthesis before every shot of R was loaded");
   int regime = 0;
   if (int rc = resolve_regime(c, nfoc, &regime)) return rc;
-  const int ldf = ldf_for(regime, nfoc), ldb = ldb_for(nfoc);
-  if (int rc = scratch_operands(c, regime, nfoc, ldf, ldb)) return rc;
-  if (int rc = launch_fwd(c, d_N_in, operand_out(c, 1, regime, ldf, ldb), nfoc, false, nullptr)) return rc;   // a6
-  if (int rc = contract(c, 1, c->d_Shat2, nfoc, ldf, ldb, regime)) return rc;                                 // a2
+  const int ldf = ldf_for(regime, nfoc);
+  if (int rc = scratch_operands(c, nfoc, ldf)) return rc;
+  if (int rc = launch_fwd(c, d_N_in, operand_out(c, 1, ldf), nfoc, false, nullptr)) return rc;   // a6
+  if (int rc = contract(c, 1, c->d_Shat2, nfoc, ldf, regime)) return rc;                          // a2
   return launch_inv(c, c->d_Shat2, nfoc, ldf, d_S_out, 1.f, nullptr, 0.f, nullptr, 0.f);     // a3
 }
 

@@ -6,35 +6,11 @@
 
 namespace mk {
 
-__device__ __forceinline__ float tf32_rna(float v) {
-  unsigned u;
-  asm("cvt.rna.tf32.f32 %0, %1;" : "=r"(u) : "f"(v));
-  return __uint_as_float(u);
-}
-
-// a6 store: X = N^[k][r][f] in the layout the contraction of the active regime reads, into this rank's operand and,
-// when peers are attached (row sharding), into theirs
-__device__ __forceinline__ void store_split_rows(float* hi, float* lo, size_t row0, int ldb, float2 X) {
-  // regime 3 (mk_syn_tc.cu): real operand B' [nb][2 ld][ldb], rows (2r, 2r+1) = (X, iX) as interleaved floats,
-  // split into a tf32 "hi" plane and a tf32 "lo" plane (3xTF32).
-  const float hx = tf32_rna(X.x), hy = tf32_rna(X.y);
-  const float lx = tf32_rna(X.x - hx), ly = tf32_rna(X.y - hy);
-  *reinterpret_cast<float2*>(hi + row0) = make_float2(hx, hy);
-  *reinterpret_cast<float2*>(hi + row0 + ldb) = make_float2(-hy, hx);
-  *reinterpret_cast<float2*>(lo + row0) = make_float2(lx, ly);
-  *reinterpret_cast<float2*>(lo + row0 + ldb) = make_float2(-ly, lx);
-}
-
+// a6 store: X = N^[k][r][f], into this rank's operand and, when peers are attached (row sharding), into theirs
 __device__ __forceinline__ void store_operand(const OperandOut& O, int ld, int kk, int r, int f, float2 X) {
-  if (O.bhi == nullptr) {
-    const size_t idx = ((size_t)kk * ld + r) * O.ldf + f;
-    O.plain[idx] = X;
-    for (int p = 0; p < O.npeer; ++p) reinterpret_cast<float2*>(O.peer[p][0])[idx] = X;
-    return;
-  }
-  const size_t row0 = ((size_t)kk * 2 * ld + 2 * r) * O.ldb + 2 * f;
-  store_split_rows(O.bhi, O.blo, row0, O.ldb, X);
-  for (int p = 0; p < O.npeer; ++p) store_split_rows(O.peer[p][0], O.peer[p][1], row0, O.ldb, X);
+  const size_t idx = ((size_t)kk * ld + r) * O.ldf + f;
+  O.plain[idx] = X;
+  for (int p = 0; p < O.npeer; ++p) O.peer[p][idx] = X;
 }
 
 // mk_fft_fast.cu: true when the register-resident path handles this context's nt (and it is not switched off)

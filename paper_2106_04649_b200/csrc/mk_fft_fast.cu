@@ -345,26 +345,11 @@ __device__ __forceinline__ void band_out_pairs(const float2* smem, int nf, int l
 }
 
 // operand store of two adjacent focal points f, f + 1 (f even, ldf even): see store_operand
-__device__ __forceinline__ void store_split_rows2(float* hi, float* lo, size_t row0, int ldb, float2 X0, float2 X1) {
-  const float h0x = tf32_rna(X0.x), h0y = tf32_rna(X0.y), h1x = tf32_rna(X1.x), h1y = tf32_rna(X1.y);
-  const float l0x = tf32_rna(X0.x - h0x), l0y = tf32_rna(X0.y - h0y), l1x = tf32_rna(X1.x - h1x), l1y = tf32_rna(X1.y - h1y);
-  *reinterpret_cast<float4*>(hi + row0) = make_float4(h0x, h0y, h1x, h1y);
-  *reinterpret_cast<float4*>(hi + row0 + ldb) = make_float4(-h0y, h0x, -h1y, h1x);
-  *reinterpret_cast<float4*>(lo + row0) = make_float4(l0x, l0y, l1x, l1y);
-  *reinterpret_cast<float4*>(lo + row0 + ldb) = make_float4(-l0y, l0x, -l1y, l1x);
-}
-
 __device__ __forceinline__ void store_operand2(const OperandOut& O, int ld, int kk, int r, int f, float2 X0, float2 X1) {
-  if (O.bhi == nullptr) {
-    const size_t idx = ((size_t)kk * ld + r) * O.ldf + f;
-    const float4 v = make_float4(X0.x, X0.y, X1.x, X1.y);
-    *reinterpret_cast<float4*>(O.plain + idx) = v;
-    for (int p = 0; p < O.npeer; ++p) *reinterpret_cast<float4*>(reinterpret_cast<float2*>(O.peer[p][0]) + idx) = v;
-    return;
-  }
-  const size_t row0 = ((size_t)kk * 2 * ld + 2 * r) * O.ldb + 2 * f;
-  store_split_rows2(O.bhi, O.blo, row0, O.ldb, X0, X1);
-  for (int p = 0; p < O.npeer; ++p) store_split_rows2(O.peer[p][0], O.peer[p][1], row0, O.ldb, X0, X1);
+  const size_t idx = ((size_t)kk * ld + r) * O.ldf + f;
+  const float4 v = make_float4(X0.x, X0.y, X1.x, X1.y);
+  *reinterpret_cast<float4*>(O.plain + idx) = v;
+  for (int p = 0; p < O.npeer; ++p) *reinterpret_cast<float4*>(O.peer[p] + idx) = v;
 }
 
 // L2 prefetch of the part of a time-domain trace that meets the window (j < hh or j > nt - hh), one 128-byte line

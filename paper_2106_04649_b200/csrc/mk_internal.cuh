@@ -14,9 +14,8 @@
 // Device layouts (complex64 = float2, interleaved re/im):
 //   Rhat [n][nb][ld]      R^[r][k][s] * dt * w[s]; ld = round_up(n, 16); pad columns are zero        (a0)
 //   Nhat [nb][ld][ldf]    N^[k][s][f]; pad rows (s >= n) and pad columns (f >= nfoc) are zero        (a1, a6)
-//   regime 3 keeps N^ instead as the REAL operand B' [nb][2 ld][ldb] fp32 of the equivalent real GEMM
-//   (rows 2s, 2s+1 = N^[k][s][.] and i N^[k][s][.] as interleaved re/im floats), split into two tf32 planes
-//   hi and lo (3xTF32); ldb = round_up(2 nfoc, 32); pad rows / columns are zero
+//   (ldf = nfoc for the streaming GEMV, round_up(nfoc, 4) for the FFMA GEMM, round_up(nfoc, 16) for the tcgen05 GEMM,
+//   whose TMA boxes are 32 floats wide; every regime reads this one operand)
 //   Shat [n][nb][ldf]     S^[r][k][f]                                                                 (a2)
 //   phat [n][nb][ldf]     running p^- spectrum                                                        (a3)
 //   f1plus, f1min [nfoc][n][nt] fp32 time domain                                                      (a5)
@@ -55,29 +54,22 @@ struct mk_ctx {
   float2* d_Shat = nullptr;
   float2* d_phat = nullptr;
   size_t cap_Nhat = 0, cap_Shat = 0;  // capacities in float2
-  float* d_Bhi = nullptr;             // regime 3 operand planes (see above)
-  float* d_Blo = nullptr;
-  size_t cap_B = 0;                   // capacity (floats) of each plane
-  int ldb = 0;
   int* d_h = nullptr;
   size_t cap_h = 0;
   // scratch operands for mk_synthesis / finals (so a run in progress is not disturbed)
   float2* d_Nhat2 = nullptr;
   float2* d_Shat2 = nullptr;
   size_t cap_Nhat2 = 0, cap_Shat2 = 0;
-  float* d_Bhi2 = nullptr;
-  float* d_Blo2 = nullptr;
-  size_t cap_B2 = 0;
   long long operand_key[2] = {0, 0};   // layout the slot's operand was last zeroed for (0 = not zeroed)
   int npeer[2] = {0, 0};               // mk_operand_attach
-  float* peer_plane[2][7][2] = {};     // [slot][peer][plane]
+  float* peer_plane[2][7] = {};        // [slot][peer]: the peers' operands of the same layout
   long long peer_key[2] = {0, 0};      // operand layout the peers were attached for
   // regime 3: cached TMA descriptors (CUtensorMap is 128 bytes, 64-byte aligned), built by mk_syn_tc.cu
   alignas(64) unsigned char tmap_A[128];
-  alignas(64) unsigned char tmap_B[2][2][128];  // [main / scratch][hi / lo]
+  alignas(64) unsigned char tmap_B[2][128];  // [main / scratch operand]
   bool tmap_A_ok = false;
   const void* tmap_B_key[2] = {nullptr, nullptr};
-  int tmap_B_ldb[2] = {0, 0};
+  int tmap_B_ldf[2] = {0, 0};
   void* encode_fn = nullptr;  // cuTensorMapEncodeTiled, resolved at run time through the CUDA runtime
   float* d_stage = nullptr;  // host-call staging
   cudaStream_t copy_stream = nullptr;  // mk_run_host: device -> host copies overlapping the finals
@@ -107,19 +99,16 @@ struct FftParams {
   int r0;  // first receiver row of this context (grid row b handles receiver r0 + b; R^ is stored from row r0 on)
 };
 
-// where a forward transform stores N^ (a1, a6): the plain complex layout (regimes 1, 2) or the split real operand
-// of regime 3 (bhi != nullptr)
+// where a forward transform stores N^ (a1, a6)
 constexpr int kMaxPeers = 7;  // other ranks of a row-sharded run whose operand receives this rank's rows directly
 
 struct OperandOut {
   float2* plain;
-  float* bhi;
-  float* blo;
-  int ldf, ldb;
+  int ldf;
   // row sharding with attached peers (mk_operand_attach): every store of this rank's rows goes to the same offset of
   // each peer's operand as well — the all-gather fused into the producing kernel as peer stores over NVLink
   int npeer;
-  float* peer[kMaxPeers][2];  // [p][0] = plain (as floats) or hi plane, [p][1] = lo plane
+  float2* peer[kMaxPeers];
 };
 
 int set_err(mk_ctx* c, int code, const std::string& msg);
@@ -142,6 +131,6 @@ int launch_syn_gemv(mk_ctx* c, const float2* d_Nhat, float2* d_Shat, int nfoc);
 int launch_syn_gemm(mk_ctx* c, const float2* d_Nhat, float2* d_Shat, int ldf);
 // mk_syn_tc.cu: tcgen05 3xTF32 path.  slot: 0 = the run's operand, 1 = the scratch operand (descriptor cache)
 bool tc_supported(const mk_ctx* c);
-int launch_syn_tc(mk_ctx* c, int slot, const float* d_Bhi, const float* d_Blo, float2* d_Shat, int nfoc, int ldf, int ldb);
+int launch_syn_tc(mk_ctx* c, int slot, const float2* d_Nhat, float2* d_Shat, int ldf);
 
 }  // namespace mk

@@ -2,36 +2,54 @@
 // NEXT-2; BASELINE.json north_star (b): "a tcgen05/TMEM 3xTF32 split path only if it meets the FP32 tolerance").
 //
 // Per bin k the complex GEMM  S^_k[r][f] = sum_s R^_k[r][s] N^_k[s][f]  (eq. (1)) is run as the REAL GEMM
-//     C'[r][2f+c] = sum_{k'} A'[r][k'] B'[k'][2f+c],     k' = 2s + (0: re, 1: im),  c = (0: re, 1: im)
-//   A'  = the row R^[r][k][.] read as 2 ld interleaved floats — R^ exactly as it sits in HBM (K-major, TMA, no copy);
-//   B'  = rows (2s, 2s+1) = (N^[k][s][.], i N^[k][s][.]) as interleaved floats, written by the forward-transform
-//         kernels (mk_fft_kernels.cu store_operand) already split into two tf32 planes  B' = Bhi + Blo;
-//   C'  = S^[r][k][.] as interleaved floats — the layout k_post reads.
-// 3xTF32: A' = Ahi + Alo with Ahi = the tf32 the tensor core sees when it reads the fp32 word (the low 13 mantissa
-// bits are not used) and Alo = A' - Ahi (exact in fp32, computed on the fly by four "split" warps into a second
-// shared-memory tile); every k'-chunk issues  Alo*Bhi + Ahi*Blo + Ahi*Bhi  into one fp32 accumulator in TMEM.  The dropped
-// term Alo*Blo is O(2^-20) relative.
+//     C'[r][2f+c] = sum_s ( Re R^[r][s] * B0[s][2f+c] + Im R^[r][s] * B1[s][2f+c] ),     c = (0: re, 1: im)
+//   B0[s] = the row N^[k][s][.] read as interleaved floats (re, im)  — the operand exactly as the transform kernels
+//           store it for every regime, [nb][ld][ldf] complex64 (TMA, no copy, no second plane in HBM);
+//   B1[s] = i N^[k][s][.] = (-im, re): the same row rotated by 90 degrees, made in shared memory;
+//   A     = the row R^[r][k][.] exactly as it sits in HBM (K-major, TMA), its (re, im) pairs de-interleaved in shared
+//           memory four shots at a time, so that one K = 8 step of the tensor core reads (re s..s+3 | im s..s+3) of A
+//           against (B0 rows s..s+3 | B1 rows s..s+3) of B;
+//   C'    = S^[r][k][.] as interleaved floats — the layout k_post reads.
+// 3xTF32: x = hi + lo with hi = the tf32 the tensor core sees when it reads the fp32 word (the low 13 mantissa bits are
+// not used) and lo = x - hi (exact in fp32); every K step issues  A_lo*B_hi + A_hi*B_lo + A_hi*B_hi  into one fp32
+// accumulator in TMEM.  The dropped term A_lo*B_lo is O(2^-21) relative.  Only raw fp32 words cross HBM and L2: the lo
+// parts, the rotation and the de-interleave are computed per stage by the worker warps from the tile TMA delivered.
 //
 // Accumulation.  The tensor core adds into its fp32 accumulator with TRUNCATION, not round-to-nearest: measured on B200
 // with one accumulator over the whole K extent the relative error of S^ grows linearly with the number of MMA steps
 // (about 2e-8 per step: 6.8e-7 at n = 32, 2.9e-5 at n = 2048, against 1.2e-6 for the FFMA kernel), which breaks the
-// 2e-5 per-iteration tolerance from n ~ 600 on.  So K is cut into CHUNKS of kChunkKb k'-blocks (24 MMA steps): every
-// chunk starts a fresh TMEM accumulator, and the epilogue warps add the finished chunk into fp32 registers
-// (round-to-nearest) while the tensor core works on the next chunk in the other TMEM buffer.  The error is then that
-// of one chunk (~5e-7), independent of n.
+// 2e-5 per-iteration tolerance from n ~ 600 on.  So K is cut into CHUNKS of kChunk stages (24 MMA steps): every chunk
+// starts a fresh TMEM accumulator, and the worker warps add the finished chunk into fp32 registers (round-to-nearest)
+// while the tensor core works on the next chunk in the other TMEM buffer.  The error is then that of one chunk
+// (~5e-7), independent of n.
 //
-// Kernel: persistent, one CTA per SM, warp-specialised, 384 threads —
-//   warp 0      TMA producer: A' tile [128 rows][16 floats] (SWIZZLE_64B, K-major) and the two B' tiles
-//               [16 k'][256 floats] (SWIZZLE_128B with 32-byte atoms, MN-major) per stage, 4 stages, mbarrier full/empty ring
+// What shaped it (measured on B200, round 2):
+//   * tcgen05.mma kind::tf32 M = 128, N = 256, K = 8 from shared-memory operands runs at exactly 128 clk per instruction
+//     with nothing else going on, and is not slowed (in cycles) by LDS / STS traffic or proxy fences of other warps;
+//   * an mbarrier wait in the ISSUING thread is not free: the thread runs only ~4 MMAs ahead of the pipe and a try_wait
+//     costs 70-90 clk that the pipe then idles (2 waits per 6 MMAs: 128 -> 152 clk per MMA).  The issuing thread
+//     therefore never touches an mbarrier: readiness reaches it through plain shared-memory counters (release /
+//     acquire) that it polls with ld.shared between bursts of MMAs;
+//   * the chip is POWER-bound: every byte through L2 and every spinning warp costs SM clock (1.75 GHz with the tensor
+//     pipe alone, 1.2-1.5 GHz with the round-1 kernel's 40 KB per stage into each SM).  Hence one raw operand plane
+//     instead of four (16 KB per stage), and waits that sleep in hardware.
+//
+// Kernel: persistent, one CTA per SM, warp-specialised, 512 threads = 4 warpgroups with their own register budgets
+// (setmaxnreg: the kernel starts at 128 registers per thread; control 64, split 72, read-out 184) —
+//   warp 0      TMA producer: A tile [128 rows][16 floats] (SWIZZLE_64B, K-major) and the B tile [8 shots][<= 256 floats]
+//               (SWIZZLE_128B with 32-byte atoms, MN-major) per stage; mbarrier full / empty ring
 //   warp 1      tcgen05.mma issuer (one thread): kind::tf32, M = 128, N <= 256, K = 8; chunk accumulators double-buffered
 //               in TMEM (2 x 256 columns); tcgen05.commit releases the stage / publishes the chunk
-//   warps 2-3   split warps: Alo tile of the stage
-//   warps 4-11  epilogue: warp w owns TMEM lanes 32 (w % 4) .. +31 and the column half (w - 4) / 4; per chunk
-//               tcgen05.ld 32x32b -> += 128 running sums in registers; per tile 128-bit global stores of S^
+//   warp 2      relay: split_bar[stage] (mbarrier) -> ready[stage] (the word the MMA warp polls)
+//   warp 3      idle (completes the control warpgroup)
+//   warps 4-7   split warps (128 threads).  Per stage: A -> (A_hi de-interleaved in place, A_lo), B -> (B_lo, B1_hi, B1_lo),
+//               proxy fence, arrive on split_bar[stage]
+//   warps 8-15  read-out warps.  Per chunk: tcgen05.ld of the finished accumulator (warp w owns TMEM lanes 32 (w % 4) .. +31
+//               and the column half (w - 8) / 4) -> += 128 running sums in registers, drained += 1 per warp; per tile:
+//               128-bit global stores of S^
 #include <cuda.h>
 
 #include <algorithm>
-#include <cstdlib>
 
 #include "mk_internal.cuh"
 
@@ -39,22 +57,25 @@ namespace mk {
 
 namespace {
 
-constexpr int BM = 128;        // rows (receivers) per tile = TMEM lanes
-constexpr int BN = 256;        // real columns (2 per focal point) per tile = TMEM columns per accumulator
-constexpr int BK = 16;         // k' (floats of the interleaved shot dimension) per stage: 64-byte rows of A'
-constexpr int UK = 8;          // k' per tcgen05.mma (kind::tf32)
-constexpr int kMaxStages = 12;  // the ring has as many stages as fit (4 at N = 256, 11 for a single column block)
-constexpr int kThreads = 384;  // 12 warps
-constexpr int kChunkKb = 4;    // k'-blocks per accumulation chunk (24 MMA steps)
-constexpr int kEpiWarps = 8;
-constexpr uint32_t A_BYTES = BM * BK * 4;   // 8 KB
-constexpr uint32_t BLK_BYTES = BK * 32 * 4;  // one 32-column block of a B' tile: 2 KB
-// A stage = A raw, A lo (8 KB each), B hi, B lo (nblk column blocks each, nblk = min(8, ceil(columns / 32))): narrow
-// focal batches move and hold only the columns they have, and get a deeper ring for it (HBM-bound regime)
-// mp = M tiles (of 128 receivers) that share the stage's B' tile: 2 when the focal batch fits 128 columns, so that a
-// stage feeds as many MMA cycles as a 256-column one with 32 KB instead of 2 x 24 KB of loads (the kernel is feed-bound)
-__host__ __device__ constexpr uint32_t stage_bytes(int nblk, int mp) { return 2 * (uint32_t)mp * A_BYTES + 2 * (uint32_t)nblk * BLK_BYTES; }
-constexpr size_t kSmemExtra = 1024 /*alignment slack*/ + 512 /*barriers*/;
+constexpr int BM = 128;         // rows (receivers) per tile = TMEM lanes
+constexpr int BN = 256;         // real columns (2 per focal point) per tile = TMEM columns per accumulator
+constexpr int BKC = 8;          // shots (complex k) per stage: 64-byte rows of A
+constexpr int kMaxStages = 10;  // the ring has as many stages as fit (4 at N = 256)
+constexpr int kSplitWarps = 4, kSplitThreads = 32 * kSplitWarps;
+constexpr int kReadWarps = 8;
+constexpr int kThreads = 128 + kSplitThreads + 32 * kReadWarps;  // 16 warps = 4 warpgroups: {TMA, MMA, 2 idle}, split, read-out x 2
+// Register budget per warpgroup (setmaxnreg): launched at 128 registers per thread (4 warps per SM sub-partition); the
+// control and split warpgroups give most of their share back and the read-out warps, who hold 128 running sums each,
+// take it: 128 x 64 + 128 x 72 + 256 x 184 = 64512 <= 65536.
+constexpr int kRegsControl = 64, kRegsSplit = 72, kRegsRead = 184;
+constexpr int kChunk = 4;       // stages per accumulation chunk (24 MMA steps)
+constexpr uint32_t A_BYTES = BM * 2 * BKC * 4;  // 8 KB: one A tile
+constexpr uint32_t BLK_BYTES = BKC * 32 * 4;    // 1 KB: one 32-column block of one B region (8 rows of 128 B)
+// A stage = A_hi (the raw tile, de-interleaved in place), A_lo, then four B regions of nblk column blocks each:
+// B0_hi (raw, TMA), B0_lo, B1_hi, B1_lo; nblk = min(8, columns / 32).  The distance B0 -> B1 (two regions) is the
+// stride-byte-offset of the B descriptors: the second group of four K rows of every MMA is the rotated copy of the first.
+__host__ __device__ constexpr uint32_t stage_bytes(int nblk) { return 2 * A_BYTES + 4 * (uint32_t)nblk * BLK_BYTES; }
+constexpr size_t kSmemExtra = 1024 /*alignment slack*/ + 512 /*barriers, counters: (3 x 10 + 2) x 8 + 11 x 4 + 4 bytes*/;
 constexpr uint32_t kTmemCols = 512;
 
 // ---------------------------------------------------------------------------------------------- PTX wrappers
@@ -69,13 +90,15 @@ __device__ __forceinline__ void mbar_arrive(uint64_t* bar) {
 __device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes) {
   asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
 }
-// Bounded wait: a protocol bug traps (the launch fails with an error) instead of hanging the GPU.  The budget is a
+// Bounded waits: a protocol bug traps (the launch fails with an error) instead of hanging the GPU.  The budget is a
 // compile-time option: MK_MBAR_TIMEOUT_CYCLES (default 4e10 SM cycles, about 20 s — no stage of a healthy launch waits
 // that long, not even under a profiler's replay or on a contended GPU); -DMK_MBAR_TIMEOUT_CYCLES=0 compiles the
 // check out.
 #ifndef MK_MBAR_TIMEOUT_CYCLES
 #define MK_MBAR_TIMEOUT_CYCLES 40000000000LL
 #endif
+// try_wait sleeps in hardware until the phase completes or a time limit passes (it does not spin), so a waiting warp
+// costs next to no issue slots and power
 __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
   const uint32_t addr = smem_u32(bar);
 #if MK_MBAR_TIMEOUT_CYCLES > 0
@@ -93,6 +116,28 @@ __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
     if (done) return;
 #if MK_MBAR_TIMEOUT_CYCLES > 0
     if (clock64() - t0 > MK_MBAR_TIMEOUT_CYCLES) __trap();
+#endif
+  }
+}
+// shared-memory counters that carry readiness to the MMA-issuing thread (see the header: no mbarrier there)
+__device__ __forceinline__ void flag_add(uint32_t* p) {
+  asm volatile("red.release.cta.shared::cta.add.u32 [%0], 1;" ::"r"(smem_u32(p)) : "memory");
+}
+__device__ __forceinline__ void flag_set(uint32_t* p, uint32_t v) {
+  asm volatile("st.release.cta.shared::cta.u32 [%0], %1;" ::"r"(smem_u32(p)), "r"(v) : "memory");
+}
+__device__ __forceinline__ void flag_wait_ge(const uint32_t* p, uint32_t need) {
+  const uint32_t addr = smem_u32(p);
+#if MK_MBAR_TIMEOUT_CYCLES > 0
+  long long t0 = 0;
+#endif
+  for (;;) {
+    uint32_t v;
+    asm volatile("ld.acquire.cta.shared::cta.u32 %0, [%1];" : "=r"(v) : "r"(addr) : "memory");
+    if ((int32_t)(v - need) >= 0) return;
+#if MK_MBAR_TIMEOUT_CYCLES > 0
+    if (t0 == 0) t0 = clock64();
+    else if (clock64() - t0 > MK_MBAR_TIMEOUT_CYCLES) __trap();
 #endif
   }
 }
@@ -115,6 +160,26 @@ __device__ __forceinline__ void umma_tf32(uint32_t tmem_d, uint64_t adesc, uint6
       "tcgen05.mma.cta_group::1.kind::tf32 [%0], %1, %2, %3, p;\n\t}" ::"r"(tmem_d),
       "l"(adesc), "l"(bdesc), "r"(idesc), "r"(accumulate)
       : "memory");
+}
+// the same with the two descriptors given as 32-bit halves: the high words (SBO, version, layout) never change and the
+// low words (start address, LBO) of a stage are those of stage 0 plus a constant, so the issuing warp keeps them in
+// (uniform) registers and pays one add per descriptor and stage
+__device__ __forceinline__ void umma_tf32_w(uint32_t tmem_d, uint32_t a_lo32, uint32_t a_hi32, uint32_t b_lo32, uint32_t b_hi32, uint32_t idesc,
+                                            uint32_t accumulate) {
+  asm volatile(
+      "{\n\t.reg .pred p;\n\t.reg .b64 da, db;\n\t"
+      "mov.b64 da, {%1, %2};\n\t"
+      "mov.b64 db, {%3, %4};\n\t"
+      "setp.ne.b32 p, %6, 0;\n\t"
+      "tcgen05.mma.cta_group::1.kind::tf32 [%0], da, db, %5, p;\n\t}" ::"r"(tmem_d),
+      "r"(a_lo32), "r"(a_hi32), "r"(b_lo32), "r"(b_hi32), "r"(idesc), "r"(accumulate)
+      : "memory");
+}
+// one lane of a fully active warp (the same one every time: tcgen05.commit tracks the MMAs of the thread that runs it)
+__device__ __forceinline__ bool elect_one() {
+  uint32_t pred;
+  asm volatile("{\n\t.reg .pred p;\n\telect.sync _|p, 0xffffffff;\n\tselp.u32 %0, 1, 0, p;\n\t}" : "=r"(pred));
+  return pred != 0;
 }
 __device__ __forceinline__ void umma_commit(uint64_t* bar) {  // arrives on `bar` when every MMA issued so far is done
   asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(smem_u32(bar)) : "memory");
@@ -143,47 +208,61 @@ __device__ __forceinline__ uint32_t instr_desc(uint32_t n) {
          (1u << 16) /*B MN-major*/ | ((n >> 3) << 17) | ((uint32_t)(BM >> 4) << 24);
 }
 
+// explicit shared-space accesses with 32-bit addresses (after the alignment arithmetic on the dynamic shared-memory
+// base the compiler no longer knows the space and would emit generic 64-bit loads and stores)
+__device__ __forceinline__ float4 lds128(uint32_t addr) {
+  float4 v;
+  asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(addr));
+  return v;
+}
+__device__ __forceinline__ void sts128(uint32_t addr, float4 v) {
+  asm volatile("st.shared.v4.f32 [%0], {%1, %2, %3, %4};" ::"r"(addr), "f"(v.x), "f"(v.y), "f"(v.z), "f"(v.w) : "memory");
+}
+
+__device__ __forceinline__ float lo_part(float x) { return x - __uint_as_float(__float_as_uint(x) & 0xffffe000u); }
+__device__ __forceinline__ float4 lo4(float4 v) { return make_float4(lo_part(v.x), lo_part(v.y), lo_part(v.z), lo_part(v.w)); }
+
 struct TcParams {
-  int n, nb, ld;        // receivers, bins, padded shots
-  int ncols;            // 2 * ldf: valid real columns of S^
+  int n, nb, ld;        // receivers (rows of R^ this context owns), bins, padded shots
+  int ncols;            // 2 * ldf: real columns of S^ (a multiple of 32)
   int mt, ntl;          // tiles along M and N
-  int nblk, stages;     // column blocks per B' tile, stages of the ring
-  int mp;               // M tiles per CTA tile (1, or 2 when ncols <= 128: accumulator m lives in columns 128 m .. of the buffer)
+  int nblk, stages;     // column blocks per B region, stages of the ring
   size_t s_row;         // floats between consecutive receivers of S^: nb * 2 ldf
-  int dbg;              // TEMP experiment flags: 1 no TMA, 2 no split, 4 no MMA
 };
 
 __global__ void __launch_bounds__(kThreads, 1)
-k_syn_gemm_tf32x3(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmBhi,
-                  const __grid_constant__ CUtensorMap tmBlo, float* __restrict__ Shat, TcParams P) {
+k_syn_gemm_tf32x3(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB, float* __restrict__ Shat,
+                  TcParams P) {
   extern __shared__ uint8_t smem_raw[];
   uint8_t* smem = reinterpret_cast<uint8_t*>(((uintptr_t)smem_raw + 1023) & ~(uintptr_t)1023);
   const int STAGES = P.stages;
-  const int MP = P.mp;
-  const uint32_t STAGE_BYTES = stage_bytes(P.nblk, MP), B_BYTES = (uint32_t)P.nblk * BLK_BYTES, AREG = (uint32_t)MP * A_BYTES;
-  const uint32_t TX_BYTES = AREG + 2 * B_BYTES;
+  const uint32_t STAGE_BYTES = stage_bytes(P.nblk), REG = (uint32_t)P.nblk * BLK_BYTES;  // REG: bytes of one B region
+  const uint32_t TX_BYTES = A_BYTES + REG;
   uint64_t* bars = reinterpret_cast<uint64_t*>(smem + (size_t)STAGES * STAGE_BYTES);
-  uint64_t* full = bars;                      // [kMaxStages] TMA landed
-  uint64_t* empty = bars + kMaxStages;        // [kMaxStages] MMAs of the stage retired
-  uint64_t* split = bars + 2 * kMaxStages;    // [kMaxStages] Alo written
-  uint64_t* acc_full = bars + 3 * kMaxStages; // [2] chunk accumulator complete
-  uint64_t* acc_empty = acc_full + 2;      // [2] chunk accumulator drained
-  uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(acc_empty + 2);
+  uint64_t* full = bars;                       // [kMaxStages] TMA landed
+  uint64_t* empty = bars + kMaxStages;         // [kMaxStages] MMAs of the stage retired
+  uint64_t* split_bar = bars + 2 * kMaxStages;  // [kMaxStages] the split warps are done with the stage
+  uint64_t* acc_full = bars + 3 * kMaxStages;   // [2] chunk accumulator complete
+  uint32_t* ready = reinterpret_cast<uint32_t*>(acc_full + 2);  // [kMaxStages] uses of the stage that are ready for the MMAs (relay)
+  uint32_t* drained = ready + kMaxStages;      // [2] read-out warps done with a use of TMEM buffer b (counts up; PER BUFFER:
+                                               // one sum over both would let fast warps' arrivals for the other buffer stand in for
+                                               // a slow warp's missing one)
+  uint32_t* tmem_slot = drained + 2;
 
-  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int warp = __shfl_sync(0xffffffffu, threadIdx.x >> 5, 0), lane = threadIdx.x & 31;  // warp-uniform by construction
   const int per_bin = P.mt * P.ntl, ntiles = P.nb * per_bin;
-  const int KB = (2 * P.ld) / BK;  // k'-blocks per tile
+  const int KB = P.ld / BKC;  // stages per tile
 
   if (threadIdx.x == 0) {
     for (int s = 0; s < STAGES; ++s) {
       mbar_init(full + s, 1);
       mbar_init(empty + s, 1);
-      mbar_init(split + s, 1);
+      mbar_init(split_bar + s, kSplitWarps);
+      ready[s] = 0;
     }
-    for (int b = 0; b < 2; ++b) {
-      mbar_init(acc_full + b, 1);
-      mbar_init(acc_empty + b, kEpiWarps);
-    }
+    mbar_init(acc_full + 0, 1);
+    mbar_init(acc_full + 1, 1);
+    drained[0] = drained[1] = 0;
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   if (warp == 1) {  // TMEM: all 512 columns (one CTA per SM)
@@ -195,8 +274,10 @@ k_syn_gemm_tf32x3(const __grid_constant__ CUtensorMap tmA, const __grid_constant
   tc_fence_after();
   const uint32_t tmem_base = *tmem_slot;
 
+  // (each role's branch opens with its own setmaxnreg: ptxas budgets a branch by the setmaxnreg that dominates it)
   if (warp == 0) {
     // ------------------------------------------------------------------------------------ TMA producer
+    asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(kRegsControl));
     if (lane == 0) {
       int s = 0;
       uint32_t ph = 0;  // ring position and its phase, kept incrementally (the ring length is a run-time value)
@@ -205,12 +286,10 @@ k_syn_gemm_tf32x3(const __grid_constant__ CUtensorMap tmA, const __grid_constant
         for (int kb = 0; kb < KB; ++kb) {
           mbar_wait(empty + s, ph ^ 1);
           uint8_t* st = smem + (size_t)s * STAGE_BYTES;
-          if (P.dbg & 1) { mbar_arrive(full + s); if (++s == STAGES) { s = 0; ph ^= 1; } continue; }
           mbar_expect_tx(full + s, TX_BYTES);
-          for (int m = 0; m < MP; ++m)  // rows past the last receiver arrive as zeros (and still count their bytes)
-            tma_load_3d(&tmA, full + s, st + m * A_BYTES, kb * BK, kk, (mi * MP + m) * BM);
-          tma_load_3d(&tmBhi, full + s, st + 2 * AREG, 0, kk * 2 * P.ld + kb * BK, ni * (BN / 32));
-          tma_load_3d(&tmBlo, full + s, st + 2 * AREG + B_BYTES, 0, kk * 2 * P.ld + kb * BK, ni * (BN / 32));
+          // rows past the last receiver / column blocks past 2 ldf arrive as zeros (and still count their bytes)
+          tma_load_3d(&tmA, full + s, st, kb * 2 * BKC, kk, mi * BM);
+          tma_load_3d(&tmB, full + s, st + 2 * A_BYTES, 0, kk * P.ld + kb * BKC, ni * (BN / 32));
           if (++s == STAGES) {
             s = 0;
             ph ^= 1;
@@ -220,91 +299,128 @@ k_syn_gemm_tf32x3(const __grid_constant__ CUtensorMap tmA, const __grid_constant
     }
   } else if (warp == 1) {
     // ------------------------------------------------------------------------------------ MMA issuer
-    if (lane == 0) {
-      uint32_t chunk_it = 0, ph = 0;
-      int s = 0;
-      for (int t = blockIdx.x; t < ntiles; t += gridDim.x) {
-        const int rem = t % per_bin, ni = rem % P.ntl;
-        int nmma = P.ncols - ni * BN;
-        nmma = nmma > BN ? BN : ((nmma + 15) / 16) * 16;
-        const uint32_t idesc = instr_desc((uint32_t)nmma);
-        for (int kb0 = 0; kb0 < KB; kb0 += kChunkKb, ++chunk_it) {
-          const int b = chunk_it & 1;
-          mbar_wait(acc_empty + b, ((chunk_it >> 1) & 1) ^ 1);
+    asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(kRegsControl));
+    // The whole warp runs the loop (warp-uniform control flow and addresses: the compiler keeps them in uniform registers);
+    // one elected lane issues.  Descriptors: see smem_desc.  A: K-major, 64-byte rows, SWIZZLE_64B, 8-row groups 512 B
+    // apart; K step j = bytes 32 j .. 32 j + 31 of the row = (re of shots 4j .. 4j+3 | im of the same shots) after the
+    // split warps' de-interleave.  B: MN-major tf32 must use the 128-byte swizzle with 32-byte atoms (the only MN-major
+    // layout the tensor core takes for 32-bit operands): a region is [nblk blocks of 32 columns][8 shot rows][128 B];
+    // LBO = 1024 (next column block); the K step's first four rows are shots 4j .. 4j+3 of B0 (512 j into the block), its
+    // second four rows sit SBO = 2 regions further: the same shots of B1 = i B0.
+    const uint32_t base16 = (smem_u32(smem) & 0x3FFFF) >> 4, stage16 = STAGE_BYTES >> 4;
+    const uint32_t hiA = (512u >> 4) | (1u << 14) | (LAYOUT_SW64 << 29);
+    const uint32_t hiB = ((2 * REG) >> 4) | (1u << 14) | (LAYOUT_SW128_BASE32B << 29);
+    const uint32_t loA_hi0 = base16 | ((16u >> 4) << 16), loA_lo0 = loA_hi0 + (A_BYTES >> 4);  // A_hi / A_lo tile, K step 0 (step 1: + 2)
+    const uint32_t loB_hi0 = (base16 + ((2 * A_BYTES) >> 4)) | ((BLK_BYTES >> 4) << 16), loB_lo0 = loB_hi0 + (REG >> 4);  // (step 1: + 32)
+    uint32_t g = 0, pass = 0;  // global chunk index; completed passes over the ring
+    int s = 0;
+    for (int t = blockIdx.x; t < ntiles; t += gridDim.x) {
+      const int rem = t % per_bin, ni = rem % P.ntl;
+      int nmma = P.ncols - ni * BN;
+      nmma = nmma > BN ? BN : ((nmma + 15) / 16) * 16;
+      const uint32_t idesc = instr_desc((uint32_t)nmma);
+      for (int kb0 = 0; kb0 < KB; kb0 += kChunk, ++g) {
+        const int b = g & 1;
+        if (g >= 2) flag_wait_ge(drained + b, kReadWarps * (g >> 1));  // every earlier chunk of this buffer has been read out
+        const uint32_t d = tmem_base + (uint32_t)b * BN;
+        const int kb1 = min(kb0 + kChunk, KB);
+        for (int kb = kb0; kb < kb1; ++kb) {
+          flag_wait_ge(ready + s, pass + 1);
+          __syncwarp();  // the lanes leave the polling loop one by one: elect.sync needs them all back
           tc_fence_after();
-          const uint32_t d = tmem_base + (uint32_t)b * BN;
-          const int kb1 = min(kb0 + kChunkKb, KB);
-          for (int kb = kb0; kb < kb1; ++kb) {
-            mbar_wait(full + s, ph);
-            mbar_wait(split + s, ph);
-            tc_fence_after();
-            const uint32_t a_raw = smem_u32(smem + (size_t)s * STAGE_BYTES), a_lo = a_raw + AREG;
-            const uint32_t b_hi = a_raw + 2 * AREG, b_lo = b_hi + B_BYTES;
-#pragma unroll
-            for (int j = 0; j < BK / UK; ++j) {
-              if (P.dbg & 4) break;
-              // A: K-major, 64-byte rows, SWIZZLE_64B: 8-row groups 512 B apart; a k'-chunk is 32 B further along the row
-              const uint64_t da_raw = smem_desc(a_raw + j * 32, 16, 512, LAYOUT_SW64);
-              const uint64_t da_lo = smem_desc(a_lo + j * 32, 16, 512, LAYOUT_SW64);
-              const uint64_t da_raw1 = smem_desc(a_raw + A_BYTES + j * 32, 16, 512, LAYOUT_SW64);  // second M tile (MP = 2)
-              const uint64_t da_lo1 = smem_desc(a_lo + A_BYTES + j * 32, 16, 512, LAYOUT_SW64);
-              // B: MN-major tf32 must use the 128-byte swizzle with 32-byte atoms (the only MN-major layout the tensor
-              //    core takes for 32-bit operands): [8 blocks of 32 columns][16 k' rows][128 B]; LBO = 2048 (next column
-              //    block), SBO = 512 (next group of 4 k' rows); a k'-chunk of 8 rows is 1024 B further
-              const uint64_t db_hi = smem_desc(b_hi + j * 1024, 2048, 512, LAYOUT_SW128_BASE32B);
-              const uint64_t db_lo = smem_desc(b_lo + j * 1024, 2048, 512, LAYOUT_SW128_BASE32B);
-              umma_tf32(d, da_lo, db_hi, idesc, (kb != kb0) || (j != 0));  // small terms first; a chunk starts from zero
-              umma_tf32(d, da_raw, db_lo, idesc, 1);
-              umma_tf32(d, da_raw, db_hi, idesc, 1);
-              if (MP == 2) {
-                umma_tf32(d + BN / 2, da_lo1, db_hi, idesc, (kb != kb0) || (j != 0));
-                umma_tf32(d + BN / 2, da_raw1, db_lo, idesc, 1);
-                umma_tf32(d + BN / 2, da_raw1, db_hi, idesc, 1);
-              }
-            }
+          const uint32_t off = (uint32_t)s * stage16;
+          if (elect_one()) {
+            // small terms first; a chunk starts from zero
+            umma_tf32_w(d, loA_lo0 + off, hiA, loB_hi0 + off, hiB, idesc, kb != kb0);
+            umma_tf32_w(d, loA_hi0 + off, hiA, loB_lo0 + off, hiB, idesc, 1);
+            umma_tf32_w(d, loA_hi0 + off, hiA, loB_hi0 + off, hiB, idesc, 1);
+            umma_tf32_w(d, loA_lo0 + off + 2, hiA, loB_hi0 + off + 32, hiB, idesc, 1);
+            umma_tf32_w(d, loA_hi0 + off + 2, hiA, loB_lo0 + off + 32, hiB, idesc, 1);
+            umma_tf32_w(d, loA_hi0 + off + 2, hiA, loB_hi0 + off + 32, hiB, idesc, 1);
             umma_commit(empty + s);
-            if (++s == STAGES) {
-              s = 0;
-              ph ^= 1;
-            }
           }
-          umma_commit(acc_full + b);
+          __syncwarp();
+          if (++s == STAGES) {
+            s = 0;
+            ++pass;
+          }
         }
+        if (elect_one()) umma_commit(acc_full + b);
+        __syncwarp();
       }
     }
-  } else if (warp < 4) {
-    // ------------------------------------------------------------------------------------ split warps: Alo = A - tf32_trunc(A)
-    // The two warps take ALTERNATE stages (a whole A tile each): the generic -> async proxy fence that must follow the
-    // stores costs several hundred cycles, and this way two of them are in flight.
-    const int sw = warp - 2;  // 0, 1
-    int s = 0;
-    uint32_t ph = 0, cnt = 0;
-    for (int t = blockIdx.x; t < ntiles; t += gridDim.x) {
-      for (int kb = 0; kb < KB; ++kb, ++cnt) {
-        if ((int)(cnt & 1) == sw) {
-          mbar_wait(full + s, ph);
-          if (P.dbg & 2) { if (lane == 0) mbar_arrive(split + s); if (++s == STAGES) { s = 0; ph ^= 1; } continue; }
-          const float4* src = reinterpret_cast<const float4*>(smem + (size_t)s * STAGE_BYTES);
-          float4* dst = reinterpret_cast<float4*>(smem + (size_t)s * STAGE_BYTES + AREG);
-          constexpr int kPer = (int)(A_BYTES / 16) / 32;  // 16 float4 per lane and M tile
-          for (int h = 0; h < 2 * MP; ++h) {
-            float4 v[kPer / 2];
-#pragma unroll
-            for (int i = 0; i < kPer / 2; ++i) v[i] = src[lane + (h * (kPer / 2) + i) * 32];
-#pragma unroll
-            for (int i = 0; i < kPer / 2; ++i) {
-              float4 l;
-              l.x = v[i].x - __uint_as_float(__float_as_uint(v[i].x) & 0xffffe000u);
-              l.y = v[i].y - __uint_as_float(__float_as_uint(v[i].y) & 0xffffe000u);
-              l.z = v[i].z - __uint_as_float(__float_as_uint(v[i].z) & 0xffffe000u);
-              l.w = v[i].w - __uint_as_float(__float_as_uint(v[i].w) & 0xffffe000u);
-              dst[lane + (h * (kPer / 2) + i) * 32] = l;
-            }
+  } else if (warp == 2) {
+    // ------------------------------------------------------------------------------------ relay
+    // Readiness of a stage reaches the MMA warp through a shared-memory word, not through the mbarrier (header).  The
+    // split warps cannot write that word themselves: a plain store could become visible before their proxy fence has
+    // taken effect (measured: with a fast issuer the tensor core then read stale operands), whereas an mbarrier arrive is
+    // ordered behind the fence.  So they arrive on split_bar and this thread turns the completed phase into the word.
+    asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(kRegsControl));
+    if (lane == 0) {
+      int s = 0;
+      uint32_t pass = 0;
+      for (int t = blockIdx.x; t < ntiles; t += gridDim.x)
+        for (int kb = 0; kb < KB; ++kb) {
+          mbar_wait(split_bar + s, pass & 1);
+          flag_set(ready + s, pass + 1);
+          if (++s == STAGES) {
+            s = 0;
+            ++pass;
           }
-          asm volatile("fence.proxy.async.shared::cta;" ::: "memory");  // generic-proxy writes -> visible to the tensor core
-          __syncwarp();
-          if (lane == 0) mbar_arrive(split + s);
         }
+    }
+  } else if (warp == 3) {
+    asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(kRegsControl));  // idle: completes the control warpgroup
+  } else if (warp < 8) {
+    // ------------------------------------------------------------------------------------ split warps
+    asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(kRegsSplit));
+    const int wt = threadIdx.x - 128;  // 0 .. 127
+    const uint32_t smem_base = smem_u32(smem);
+    // A work items of this thread: 32-byte pairs p = wt and wt + 128 of the tile; pair p = row p / 2, K step p % 2.
+    // SWIZZLE_64B: the 16-byte chunk c of row r sits at chunk position c ^ ((r >> 1) & 3).
+    uint32_t a_off[2][2];
+#pragma unroll
+    for (int k = 0; k < 2; ++k) {
+      const int pr = wt + k * kSplitThreads, ar = pr >> 1, ap = pr & 1, ax = (ar >> 1) & 3;
+      a_off[k][0] = (uint32_t)ar * 64 + (uint32_t)(((2 * ap) ^ ax) << 4);
+      a_off[k][1] = (uint32_t)ar * 64 + (uint32_t)(((2 * ap + 1) ^ ax) << 4);
+    }
+    int s = 0;
+    uint32_t ph = 0;
+    for (int t = blockIdx.x; t < ntiles; t += gridDim.x) {
+      for (int kb = 0; kb < KB; ++kb) {
+        mbar_wait(full + s, ph);
+        const uint32_t st = smem_base + (uint32_t)s * STAGE_BYTES;
+        {  // A: (re0 im0 re1 im1 | re2 im2 re3 im3) -> hi (re0 re1 re2 re3 | im0 im1 im2 im3) in place, lo beside it
+          float4 c[2][2];
+#pragma unroll
+          for (int k = 0; k < 2; ++k) {
+            c[k][0] = lds128(st + a_off[k][0]);
+            c[k][1] = lds128(st + a_off[k][1]);
+          }
+#pragma unroll
+          for (int k = 0; k < 2; ++k) {
+            const float4 re = make_float4(c[k][0].x, c[k][0].z, c[k][1].x, c[k][1].z), im = make_float4(c[k][0].y, c[k][0].w, c[k][1].y, c[k][1].w);
+            sts128(st + a_off[k][0], re);
+            sts128(st + a_off[k][1], im);
+            sts128(st + A_BYTES + a_off[k][0], lo4(re));
+            sts128(st + A_BYTES + a_off[k][1], lo4(im));
+          }
+        }
+        {  // B: elementwise on the swizzled tile — lo of B0, and B1 = i B0 (every float4 holds two (re, im) pairs)
+          const uint32_t b0 = st + 2 * A_BYTES;
+#pragma unroll 2
+          for (uint32_t q = 16 * (uint32_t)wt; q < REG; q += 16 * kSplitThreads) {
+            const float4 v = lds128(b0 + q);
+            const float4 l = lo4(v);
+            sts128(b0 + q + REG, l);
+            sts128(b0 + q + 2 * REG, make_float4(-v.y, v.x, -v.w, v.z));
+            sts128(b0 + q + 3 * REG, make_float4(-l.y, l.x, -l.w, l.z));
+          }
+        }
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");  // generic-proxy writes -> visible to the tensor core
+        __syncwarp();
+        if (lane == 0) mbar_arrive(split_bar + s);
         if (++s == STAGES) {
           s = 0;
           ph ^= 1;
@@ -312,20 +428,20 @@ k_syn_gemm_tf32x3(const __grid_constant__ CUtensorMap tmA, const __grid_constant
       }
     }
   } else {
-    // ------------------------------------------------------------------------------------ epilogue: chunk sums in registers
-    const int quad = warp & 3;        // TMEM lanes 32 quad .. 32 quad + 31 are the ones this warp may read
-    const int half = (warp - 4) >> 2; // columns 128 half .. 128 half + 127 of the tile
-    uint32_t chunk_it = 0;
+    // ------------------------------------------------------------------------------------ read-out warps: chunk sums in registers
+    asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(kRegsRead));
+    const int quad = warp & 3;         // TMEM lanes 32 quad .. 32 quad + 31 are the ones this warp may read
+    const int half = (warp - 8) >> 2;  // columns 128 half .. 128 half + 127 of the tile
+    uint32_t g = 0;
     for (int t = blockIdx.x; t < ntiles; t += gridDim.x) {
       const int kk = t / per_bin, rem = t - kk * per_bin, mi = rem / P.ntl, ni = rem - mi * P.ntl;
-      // MP = 1: this warp's half of the 256 columns; MP = 2: the whole (<= 128-column) tile of M tile `half`
-      const int cols = MP == 2 ? P.ncols : P.ncols - ni * BN - half * (BN / 2);  // valid columns (may exceed BN / 2, may be <= 0)
+      const int cols = P.ncols - ni * BN - half * (BN / 2);  // valid columns of this warp's half (may exceed BN / 2, may be <= 0)
       float sum[BN / 2];
 #pragma unroll
       for (int i = 0; i < BN / 2; ++i) sum[i] = 0.f;
-      for (int kb0 = 0; kb0 < KB; kb0 += kChunkKb, ++chunk_it) {
-        const int b = chunk_it & 1;
-        mbar_wait(acc_full + b, (chunk_it >> 1) & 1);
+      for (int kb0 = 0; kb0 < KB; kb0 += kChunk, ++g) {
+        const int b = g & 1;
+        mbar_wait(acc_full + b, (g >> 1) & 1);
         tc_fence_after();
         const uint32_t ta = tmem_base + ((uint32_t)(quad * 32) << 16) + (uint32_t)(b * BN + half * (BN / 2));
 #pragma unroll
@@ -340,11 +456,11 @@ k_syn_gemm_tf32x3(const __grid_constant__ CUtensorMap tmA, const __grid_constant
         }
         tc_fence_before();
         __syncwarp();
-        if (lane == 0) mbar_arrive(acc_empty + b);
+        if (lane == 0) flag_add(drained + b);
       }
-      const int r = (MP == 2 ? mi * 2 + half : mi) * BM + quad * 32 + lane;
+      const int r = mi * BM + quad * 32 + lane;
       if (r < P.n) {
-        float* dst = Shat + (size_t)r * P.s_row + (size_t)kk * P.ncols + (MP == 2 ? 0 : ni * BN + half * (BN / 2));
+        float* dst = Shat + (size_t)r * P.s_row + (size_t)kk * P.ncols + ni * BN + half * (BN / 2);
 #pragma unroll
         for (int q = 0; q < BN / 8; ++q)
           if (q * 4 < cols)
@@ -393,59 +509,53 @@ int encode3(mk_ctx* c, EncodeTiledFn enc, void* out, const void* base, const cuu
 }  // namespace
 
 bool tc_supported(const mk_ctx* c) {
-  int dev = 0, major = 0;
-  if (cudaGetDevice(&dev) != cudaSuccess) return false;
-  cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev);
-  return major == 10 && c->smem_optin >= 2 * stage_bytes(1, 1) + kSmemExtra;
+  int major = 0;
+  cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, c->dev);
+  return major == 10 && c->smem_optin >= 2 * stage_bytes(1) + kSmemExtra;
 }
 
-int launch_syn_tc(mk_ctx* c, int slot, const float* d_Bhi, const float* d_Blo, float2* d_Shat, int nfoc, int ldf, int ldb) {
-  (void)nfoc;
+int launch_syn_tc(mk_ctx* c, int slot, const float2* d_Nhat, float2* d_Shat, int ldf) {
+  if (ldf % 16 != 0) return set_err(c, MK_ERR_INVALID_ARG, "the tcgen05 contraction needs ldf to be a multiple of 16");
   EncodeTiledFn enc = nullptr;
   if (int rc = get_encode(c, &enc)) return rc;
   if (!c->tmap_A_ok) {
-    // A' = R^ as fp32 [n][nb][2 ld]: dims (k', bin, r); box = 16 floats x 1 bin x 128 receivers; rows r >= n read as zero
+    // A = R^ as fp32 [n][nb][2 ld]: dims (float of the row, bin, r); box = 16 floats x 1 bin x 128 receivers; rows r >= n read as zero
     const cuuint64_t dims[3] = {(cuuint64_t)2 * c->ld, (cuuint64_t)c->nb, (cuuint64_t)c->nrow};  // local rows of R^
     const cuuint64_t str[2] = {(cuuint64_t)2 * c->ld * 4, (cuuint64_t)c->nb * 2 * c->ld * 4};
-    const cuuint32_t box[3] = {BK, 1, BM};
+    const cuuint32_t box[3] = {2 * BKC, 1, BM};
     if (int rc = encode3(c, enc, c->tmap_A, c->d_Rhat, dims, str, box, CU_TENSOR_MAP_SWIZZLE_64B, "A")) return rc;
     c->tmap_A_ok = true;
   }
-  const int nblk = std::min(BN / 32, (2 * ldf + 31) / 32);
-  if (c->tmap_B_key[slot] != d_Bhi || c->tmap_B_ldb[slot] != ldb) {
-    // B' plane [nb * 2 ld rows][ldb] seen as (column in block, row, column block): box = 32 x 16 x 8 lands in shared
-    // memory as [8 column blocks][16 rows][128 B], the MN-major SWIZZLE_128B_BASE32B operand layout
-    const cuuint64_t dims[3] = {32, (cuuint64_t)c->nb * 2 * c->ld, (cuuint64_t)ldb / 32};
-    const cuuint64_t str[2] = {(cuuint64_t)ldb * 4, 128};
-    const cuuint32_t box[3] = {32, BK, (cuuint32_t)nblk};  // ldb is a function of nfoc, so is nblk: one cache key
-    if (int rc = encode3(c, enc, c->tmap_B[slot][0], d_Bhi, dims, str, box, CU_TENSOR_MAP_SWIZZLE_128B_ATOM_32B, "B hi")) return rc;
-    if (int rc = encode3(c, enc, c->tmap_B[slot][1], d_Blo, dims, str, box, CU_TENSOR_MAP_SWIZZLE_128B_ATOM_32B, "B lo")) return rc;
-    c->tmap_B_key[slot] = d_Bhi;
-    c->tmap_B_ldb[slot] = ldb;
+  const int nblk = std::min(BN / 32, (2 * ldf) / 32);
+  if (c->tmap_B_key[slot] != d_Nhat || c->tmap_B_ldf[slot] != ldf) {
+    // B = N^ [nb * ld rows][2 ldf floats] seen as (float in column block, row, column block): box = 32 x 8 x nblk lands in
+    // shared memory as [nblk column blocks][8 rows][128 B], the MN-major SWIZZLE_128B_BASE32B operand layout
+    const cuuint64_t dims[3] = {32, (cuuint64_t)c->nb * c->ld, (cuuint64_t)(2 * ldf) / 32};
+    const cuuint64_t str[2] = {(cuuint64_t)2 * ldf * 4, 128};
+    const cuuint32_t box[3] = {32, BKC, (cuuint32_t)nblk};  // nblk is a function of ldf: one cache key
+    if (int rc = encode3(c, enc, c->tmap_B[slot], d_Nhat, dims, str, box, CU_TENSOR_MAP_SWIZZLE_128B_ATOM_32B, "B")) return rc;
+    c->tmap_B_key[slot] = d_Nhat;
+    c->tmap_B_ldf[slot] = ldf;
   }
   TcParams P;
-  { const char* e = getenv("MK_TC_DEBUG"); P.dbg = e ? atoi(e) : 0; }
   P.n = c->nrow;  // row sharding: local rows; S^ is offset to the first one below
   P.nb = c->nb;
   P.ld = c->ld;
   P.ncols = 2 * ldf;
-  const int mtiles = (c->nrow + BM - 1) / BM;
-  P.mp = (2 * ldf <= BN / 2 && mtiles >= 2) ? 2 : 1;
-  P.mt = (mtiles + P.mp - 1) / P.mp;
+  P.mt = (c->nrow + BM - 1) / BM;
   P.ntl = (P.ncols + BN - 1) / BN;
   P.s_row = (size_t)c->nb * 2 * ldf;
   P.nblk = nblk;
-  P.stages = (int)std::min<size_t>(kMaxStages, (c->smem_optin - kSmemExtra) / stage_bytes(nblk, P.mp));
+  P.stages = (int)std::min<size_t>(kMaxStages, (c->smem_optin - kSmemExtra) / stage_bytes(nblk));
   if (P.stages < 2) return set_err(c, MK_ERR_INVALID_ARG, "not enough shared memory for the tcgen05 contraction");
-  const size_t kSmemBytes = (size_t)P.stages * stage_bytes(nblk, P.mp) + kSmemExtra;
+  const size_t kSmemBytes = (size_t)P.stages * stage_bytes(nblk) + kSmemExtra;
   if (int rc = check_cuda(c, cudaFuncSetAttribute(k_syn_gemm_tf32x3, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemBytes),
                           "cudaFuncSetAttribute"))
     return rc;
   const int ntiles = P.nb * P.mt * P.ntl;
   const int grid = ntiles < c->num_sms ? ntiles : c->num_sms;
   k_syn_gemm_tf32x3<<<grid, kThreads, kSmemBytes, c->stream>>>(*reinterpret_cast<const CUtensorMap*>(c->tmap_A),
-                                                               *reinterpret_cast<const CUtensorMap*>(c->tmap_B[slot][0]),
-                                                               *reinterpret_cast<const CUtensorMap*>(c->tmap_B[slot][1]),
+                                                               *reinterpret_cast<const CUtensorMap*>(c->tmap_B[slot]),
                                                                reinterpret_cast<float*>(d_Shat + (size_t)c->r0 * c->nb * ldf), P);
   ++c->launches;
   return check_cuda(c, cudaGetLastError(), "k_syn_gemm_tf32x3");

@@ -93,4 +93,4 @@ def test_two_processes_one_gpu_fused_peer_stores(regime):
         assert isinstance(worst, float), worst
         assert alive and worst <= 1e-6
         assert e_it <= 2e-5 and e_fin <= 1e-4, (e_it, e_fin)
-        assert nopened == (2 if regime != 3 else 4)      # one peer x two slots x planes
+        assert nopened == 2                               # one peer x two slots x one plane
