@@ -36,12 +36,11 @@
 //
 // Kernel: persistent, one CTA per SM, warp-specialised, 512 threads = 4 warpgroups with their own register budgets
 // (setmaxnreg: the kernel starts at 128 registers per thread; control 64, split 72, read-out 184) —
-//   warp 0      TMA producer: A tile [128 rows][16 floats] (SWIZZLE_64B, K-major) and the B tile [8 shots][<= 256 floats]
-//               (SWIZZLE_128B with 32-byte atoms, MN-major) per stage; mbarrier full / empty ring
+//   warp 0      TMA producer of the A tiles [128 rows][16 floats] (SWIZZLE_64B, K-major); mbarrier full / empty ring
+//   warp 3      TMA producer of the B tiles [8 shots][<= 256 floats] (SWIZZLE_128B with 32-byte atoms, MN-major)
 //   warp 1      tcgen05.mma issuer (one thread): kind::tf32, M = 128, N <= 256, K = 8; chunk accumulators double-buffered
 //               in TMEM (2 x 256 columns); tcgen05.commit releases the stage / publishes the chunk
 //   warp 2      relay: split_bar[stage] (mbarrier) -> ready[stage] (the word the MMA warp polls)
-//   warp 3      idle (completes the control warpgroup)
 //   warps 4-7   split warps (128 threads).  Per stage: A -> (A_hi de-interleaved in place, A_lo), B -> (B_lo, B1_hi, B1_lo),
 //               proxy fence, arrive on split_bar[stage]
 //   warps 8-15  read-out warps.  Per chunk: tcgen05.ld of the finished accumulator (warp w owns TMEM lanes 32 (w % 4) .. +31
@@ -237,7 +236,6 @@ k_syn_gemm_tf32x3(const __grid_constant__ CUtensorMap tmA, const __grid_constant
   uint8_t* smem = reinterpret_cast<uint8_t*>(((uintptr_t)smem_raw + 1023) & ~(uintptr_t)1023);
   const int STAGES = P.stages;
   const uint32_t STAGE_BYTES = stage_bytes(P.nblk), REG = (uint32_t)P.nblk * BLK_BYTES;  // REG: bytes of one B region
-  const uint32_t TX_BYTES = A_BYTES + REG;
   uint64_t* bars = reinterpret_cast<uint64_t*>(smem + (size_t)STAGES * STAGE_BYTES);
   uint64_t* full = bars;                       // [kMaxStages] TMA landed
   uint64_t* empty = bars + kMaxStages;         // [kMaxStages] MMAs of the stage retired
@@ -255,7 +253,7 @@ k_syn_gemm_tf32x3(const __grid_constant__ CUtensorMap tmA, const __grid_constant
 
   if (threadIdx.x == 0) {
     for (int s = 0; s < STAGES; ++s) {
-      mbar_init(full + s, 1);
+      mbar_init(full + s, 2);  // the A producer and the B producer, each with its own byte count
       mbar_init(empty + s, 1);
       mbar_init(split_bar + s, kSplitWarps);
       ready[s] = 0;
@@ -286,10 +284,8 @@ k_syn_gemm_tf32x3(const __grid_constant__ CUtensorMap tmA, const __grid_constant
         for (int kb = 0; kb < KB; ++kb) {
           mbar_wait(empty + s, ph ^ 1);
           uint8_t* st = smem + (size_t)s * STAGE_BYTES;
-          mbar_expect_tx(full + s, TX_BYTES);
-          // rows past the last receiver / column blocks past 2 ldf arrive as zeros (and still count their bytes)
-          tma_load_3d(&tmA, full + s, st, kb * 2 * BKC, kk, mi * BM);
-          tma_load_3d(&tmB, full + s, st + 2 * A_BYTES, 0, kk * P.ld + kb * BKC, ni * (BN / 32));
+          mbar_expect_tx(full + s, A_BYTES);
+          tma_load_3d(&tmA, full + s, st, kb * 2 * BKC, kk, mi * BM);  // rows past the last receiver arrive as zeros (and still count)
           if (++s == STAGES) {
             s = 0;
             ph ^= 1;
@@ -370,7 +366,27 @@ k_syn_gemm_tf32x3(const __grid_constant__ CUtensorMap tmA, const __grid_constant
         }
     }
   } else if (warp == 3) {
-    asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(kRegsControl));  // idle: completes the control warpgroup
+    // ------------------------------------------------------------------------------------ TMA producer of the B tiles
+    // (a thread issues one TMA instruction per ~250 clk and an expect_tx per ~150, measured: with both tiles on one
+    // thread the producer alone needed ~850 clk per stage, more than the stage's MMAs)
+    asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(kRegsControl));
+    if (lane == 0) {
+      int s = 0;
+      uint32_t ph = 0;
+      for (int t = blockIdx.x; t < ntiles; t += gridDim.x) {
+        const int kk = t / per_bin, rem = t - kk * per_bin, ni = rem % P.ntl;
+        for (int kb = 0; kb < KB; ++kb) {
+          mbar_wait(empty + s, ph ^ 1);
+          mbar_expect_tx(full + s, REG);
+          // column blocks past 2 ldf arrive as zeros (and still count their bytes)
+          tma_load_3d(&tmB, full + s, smem + (size_t)s * STAGE_BYTES + 2 * A_BYTES, 0, kk * P.ld + kb * BKC, ni * (BN / 32));
+          if (++s == STAGES) {
+            s = 0;
+            ph ^= 1;
+          }
+        }
+      }
+    }
   } else if (warp < 8) {
     // ------------------------------------------------------------------------------------ split warps
     asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(kRegsSplit));
