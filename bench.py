@@ -6,8 +6,11 @@ niter + 2 = 18 syntheses) over one batch of seeded synthetic input of BASELINE.j
 one focal point, 16 iterations; the bandwidth-bound regime the metric is quoted on).  R^ (1.30 GB) is resident in
 HBM and far larger than the 126 MB L2, so no cache flush is needed between steps.
 
-  value      synthesis GB/s of R^ streamed  = syntheses * bytes(R^ unpadded) / device time   (inputs resident in HBM;
-             algorithmic bytes: with 1, 2 or 4 focal points the two final syntheses share one pass over R^)
+  value      synthesis GB/s of R^ streamed  = passes over R^ * bytes(R^ unpadded) / device time   (inputs resident in HBM;
+             with 1, 2 or 4 focal points the two final syntheses share one pass: 17 passes per step; value_algorithmic
+             counts the 18 syntheses of Algorithm 1)
+  secondary  the large-batch regimes, measured in the same invocation (N = 1): config 2 (tcgen05 3xTF32 and FP32-FFMA),
+             config 3, config 4 — each with its own ms_per_step, clocks and roofline
   e2e        same metric through mk_run_host: pinned HOST G_d / t_d in, six HOST output fields out, copies timed
   roofline   the streaming contraction kernel (k_syn_gemv): algorithmic bytes of R^ per launch / its CUDA-event time
   cpu_baseline  the fp64 oracle timed on this box's host cores on a bounded sample (one full synthesis R N_0)
@@ -189,6 +192,137 @@ def run_reference(args):
 
 
 # ------------------------------------------------------------------------------------------------ our arm
+FIELDS = ("N_last", "f1plus", "f1min", "G", "Gplus", "Gminus")
+
+
+def traffic_entry(cfg_k, regime):
+    """DRAM bytes per launch of the contraction kernel from the last committed `ncu --set full` capture (profiles/traffic.json;
+    it names the commit the captures were taken at, so a stale figure can be told from a current one)."""
+    tp = ROOT / "profiles" / "traffic.json"
+    if not tp.exists():
+        return None, None
+    d = json.loads(tp.read_text())
+    return d.get("entries", d).get(f"config{cfg_k}_regime{regime}"), d.get("source")
+
+
+def roofline_of(cfg, nb, nbytes, regime_used, syn_n, syn_ms, ms_total, clocks, share=1.0):
+    """Roofline of the dominant kernel (the contraction) from the CUDA events the library records on its own stream."""
+    peaks = measured_peaks()
+    avg_ms = syn_ms / max(syn_n, 1)
+    traffic, traffic_src = traffic_entry(cfg.k, regime_used)
+    common = {"traffic": traffic, "traffic_source": traffic_src, "launches_timed": int(syn_n), "avg_launch_ms": avg_ms,
+              "share_of_step": syn_ms / ms_total}
+    if regime_used == 1:
+        ach = share * nbytes / (avg_ms * 1e-3) / 1e9
+        return {"bound": "hbm", "kernel": "k_syn_gemv", "achieved": ach, "peak": peaks["hbm_gbs"], "unit": "GB/s",
+                "frac": ach / peaks["hbm_gbs"], "peak_source": peaks["source"] + " copy bandwidth (MEASURED_PEAKS.json)",
+                "frac_of_nominal_8TBps": ach / 8000.0, **common}
+    flops = share * 8.0 * cfg.nfoc * cfg.n * cfg.n * nb        # algorithmic: one complex MAC (8 flops) per element of R^ and focal point
+    ach = flops / (avg_ms * 1e-3) / 1e12
+    sm_max = clocks.get("sm_max_mhz") or 1965.0
+    ffma_peak = 2 * 128 * 148 * sm_max * 1e6 / 1e12            # FFMA lanes x SMs x max clock (DESIGN.md "FP32 peak")
+    if regime_used == 2:
+        return {"bound": "alu", "kernel": "k_syn_gemm_ffma", "achieved": ach, "peak": ffma_peak, "unit": "TFLOP/s",
+                "frac": ach / ffma_peak, "peak_source": "2 x 128 FFMA lanes x 148 SMs x clocks.max.sm (guide unit counts)", **common}
+    # 3xTF32: every algorithmic flop costs three tf32 tensor flops.  Peak for this dtype = measured bf16 peak (sustained
+    # figure: the kernel is timed inside a long step) x 1/2 (nominal tf32 : bf16), / 3 for the split.
+    tf32_peak = 0.5 * peaks["bf16_tflops_sustained"]
+    return {"bound": "tensor", "kernel": "k_syn_gemm_tf32x3", "achieved": ach, "peak": tf32_peak / 3.0, "unit": "TFLOP/s",
+            "frac": ach / (tf32_peak / 3.0),
+            "peak_source": peaks["source"] + " bf16 sustained x 0.5 (nominal tf32:bf16) / 3 (3xTF32 split); "
+                           "achieved counts algorithmic fp32 flops (8 per complex MAC)",
+            "tensor_tflops_issued": 3.0 * ach, "tf32_peak": tf32_peak, "frac_of_fp32_ffma_roofline": ach / ffma_peak, **common}
+
+
+def ingest_device(mk, cfg, dev):
+    """33 GB / 250 GB of time-domain R never exist at once: generated on the device in 64-shot chunks (BASELINE.json config 4)."""
+    import torch
+    gR = gen.DeviceR(cfg, dev)
+    for s0 in range(0, cfg.n, 64):
+        mk.load_R(gR.take(np.arange(s0, min(s0 + 64, cfg.n))), s0)
+    torch.cuda.synchronize()
+    del gR
+    torch.cuda.empty_cache()
+
+
+def device_fields(cfg, dev):
+    """Output fields of one run.  180 GB of HBM do not hold six distinct fields of config 4 next to R^ and the operands:
+    f1plus and f1min (the accumulators of the run) get their own, the other four outputs are written one after the
+    other into ONE shared field there (same kernels, same traffic; include/mk.h allows it)."""
+    import torch
+
+    def field():
+        return torch.empty((cfg.nfoc, cfg.n, cfg.nt), dtype=torch.float32, device=dev)
+    shared = field() if cfg.k == 4 else None
+    return {nm: (field() if (shared is None or nm in ("f1plus", "f1min")) else shared) for nm in FIELDS}
+
+
+def timed_steps(mk, run_step, steps, warmup, local, dist=None, barrier=None):
+    """W untimed warm-up steps, then exactly K steps between CUDA events (device time, max over ranks), clocks sampled
+    during the timed region, contraction launches timed by the library's own events."""
+    import torch
+    from paper_2106_04649_b200 import binding as B
+    if barrier is None:
+        barrier = torch.cuda.synchronize
+    for _ in range(warmup):
+        run_step()
+    mk.set_option(B.MK_OPT_TIMING, 1)
+    mk.get_info(B.MK_INFO_SYN_RESET)
+    l0 = mk.get_info(B.MK_INFO_KERNEL_LAUNCHES)
+    barrier()
+    sampler = ClockSampler(local)
+    sampler.start()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(steps):
+        run_step()
+    e1.record()
+    barrier()
+    clocks = sampler.stop()
+    ms_total = shard.max_over_ranks(e0.elapsed_time(e1), dist)
+    res = {"ms_total": ms_total, "clocks": clocks, "launches": int(mk.get_info(B.MK_INFO_KERNEL_LAUNCHES) - l0),
+           "syn_n": mk.get_info(B.MK_INFO_SYN_LAUNCHES), "syn_ms": mk.get_info(B.MK_INFO_SYN_MS_TOTAL),
+           "regime_used": int(mk.get_info(B.MK_INFO_REGIME_USED))}
+    mk.set_option(B.MK_OPT_TIMING, 0)
+    return res
+
+
+def secondary_entry(mk, cfg, regime, steps, warmup, local, dev, image=False):
+    """One large-batch configuration for the `secondary` list of the JSON line: same protocol as the headline (mk_run steps
+    between CUDA events, inputs resident in HBM), its own clocks and roofline."""
+    import torch
+    from paper_2106_04649_b200 import binding as B
+    nbytes, nb = rhat_bytes(cfg)
+    mk.set_option(B.MK_OPT_REGIME, regime)
+    dGd, dtd = gen.first_arrivals_torch(cfg, dev)
+    douts = device_fields(cfg, dev)
+    r = timed_steps(mk, lambda: mk.run(dGd, dtd, cfg.niter, douts), steps, warmup, local)
+    ms = r["ms_total"] / steps
+    nsyn = nsyn_per_step(cfg)
+    entry = {"workload": f"config{cfg.k}:{cfg.name}", "n": cfg.n, "nt": cfg.nt, "nfoc": cfg.nfoc, "niter": cfg.niter, "nb": nb,
+             "regime": r["regime_used"], "steps": steps, "warmup": warmup, "ms_per_step": ms,
+             "value": nsyn * nbytes / (ms * 1e-3) / 1e9, "unit": UNIT,
+             "focal_point_iterations_per_s": cfg.nfoc * cfg.niter / (ms * 1e-3),
+             "contraction_launches_per_step": r["syn_n"] / steps, "gpu_launches": r["launches"], "clocks": r["clocks"],
+             "roofline": roofline_of(cfg, nb, nbytes, r["regime_used"], r["syn_n"], r["syn_ms"], r["ms_total"], r["clocks"]),
+             "input_source": "device generator" + (", R in 64-shot chunks" if cfg.k >= 3 else " for G_d / t_d; R^ shared with config 1")}
+    if image:   # NEXT-1: the double-focusing image of the run just made, timed alone (PAPER.md:24 "about 2% of the total processing time")
+        img = torch.empty(cfg.nfoc, dtype=torch.float32, device=dev)
+        mk.image(douts["Gminus"], img)
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for _ in range(5):
+            mk.image(douts["Gminus"], img)
+        e1.record()
+        torch.cuda.synchronize()
+        entry["image_ms"] = e0.elapsed_time(e1) / 5
+        entry["image_share_of_step"] = entry["image_ms"] / ms
+    del dGd, dtd, douts
+    torch.cuda.empty_cache()
+    return entry
+
+
 def run_ours(args):
     import torch
     import torch.distributed as dist
@@ -208,7 +342,6 @@ def run_ours(args):
     my_rows = shard.row_slice(cfg.n, rank, world) if rows_mode else range(cfg.n)
     nbytes, nb = rhat_bytes(cfg)
     nfoc, niter, nsyn = cfg.nfoc, cfg.niter, nsyn_per_step(cfg)
-    fields = ("N_last", "f1plus", "f1min", "G", "Gplus", "Gminus")
     big = cfg.k >= 3            # 33 GB / 250 GB of time-domain R: generated on the device in 64-shot chunks, never on the host
 
     mk = B.Marchenko(cfg.n, cfg.n, cfg.nt, cfg.dt, cfg.dx, cfg.fmin, cfg.fmax, rows=(my_rows.start, len(my_rows)))
@@ -238,27 +371,16 @@ def run_ours(args):
         def run_step():
             mk.run(dGd, dtd, niter, douts)
     if big:
-        gR = gen.DeviceR(cfg, dev)
-        for s0 in range(0, cfg.n, 64):
-            mk.load_R(gR.take(np.arange(s0, min(s0 + 64, cfg.n))), s0)
-        torch.cuda.synchronize()
-        del gR
-        torch.cuda.empty_cache()
+        ingest_device(mk, cfg, dev)
         dGd, dtd = gen.first_arrivals_torch(cfg, dev)
         R = Gd = td = None
-        # 180 GB of HBM do not hold six distinct output fields of config 4 next to R^ and the operands: f1plus and f1min
-        # (the accumulators of the run) get their own fields, the other four outputs are written one after the other
-        # into ONE shared field there (same kernels, same traffic)
-        def field():
-            return torch.empty((nfoc, cfg.n, cfg.nt), dtype=torch.float32, device=dev)
-        shared = field() if cfg.k == 4 else None
-        douts = {nm: (field() if (shared is None or nm in ("f1plus", "f1min")) else shared) for nm in fields}
+        douts = device_fields(cfg, dev)
     else:
         R, Gd, td = workload_arrays(cfg)
         mk.load_R_host(R)
         dGd = torch.from_numpy(Gd).to(dev)
         dtd = torch.from_numpy(td).to(dev)
-        douts = {nm: torch.empty((nfoc, cfg.n, cfg.nt), dtype=torch.float32, device=dev) for nm in fields}
+        douts = {nm: torch.empty((nfoc, cfg.n, cfg.nt), dtype=torch.float32, device=dev) for nm in FIELDS}
 
     def barrier():
         if world > 1:
@@ -266,36 +388,19 @@ def run_ours(args):
         torch.cuda.synchronize()
 
     # ---- device-timed region: inputs resident in HBM
-    for _ in range(args.warmup):
-        run_step()
-    mk.set_option(B.MK_OPT_TIMING, 1)
-    mk.get_info(B.MK_INFO_SYN_RESET)
-    l0 = mk.get_info(B.MK_INFO_KERNEL_LAUNCHES)
-    barrier()
-    sampler = ClockSampler(local)
-    sampler.start()
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    e0.record()
-    for _ in range(args.steps):
-        run_step()
-    e1.record()
-    barrier()
-    clocks = sampler.stop()
-    ms_total = shard.max_over_ranks(e0.elapsed_time(e1), dist)
-    launches = int(mk.get_info(B.MK_INFO_KERNEL_LAUNCHES) - l0)
-    syn_n = mk.get_info(B.MK_INFO_SYN_LAUNCHES)
-    syn_ms = mk.get_info(B.MK_INFO_SYN_MS_TOTAL)
-    regime_used = int(mk.get_info(B.MK_INFO_REGIME_USED))
-    mk.set_option(B.MK_OPT_TIMING, 0)
+    r = timed_steps(mk, run_step, args.steps, args.warmup, local, dist, barrier)
+    ms_total, clocks, launches, syn_n, syn_ms, regime_used = (r[k] for k in ("ms_total", "clocks", "launches", "syn_n", "syn_ms", "regime_used"))
     jobs = 1 if rows_mode else world        # rows: the ranks share ONE job (strong scaling)
-    value = jobs * nsyn * nbytes * args.steps / (ms_total * 1e-3) / 1e9
+    passes = syn_n / max(args.steps, 1)     # contraction launches = passes over R^ per step (17 with the fused finals, else 18)
+    value = jobs * passes * nbytes * args.steps / (ms_total * 1e-3) / 1e9          # bytes of R^ actually streamed
+    value_alg = jobs * nsyn * nbytes * args.steps / (ms_total * 1e-3) / 1e9        # one R^ per synthesis of Algorithm 1
 
     # ---- end-to-end through the public host API: pinned host inputs, host outputs, copies inside the timed region
     e2e = None
     if not big and not rows_mode:
         hGd = torch.from_numpy(Gd).pin_memory()
         htd = torch.from_numpy(td).pin_memory()
-        houts = {nm: torch.empty((nfoc, cfg.n, cfg.nt), dtype=torch.float32).pin_memory() for nm in fields}
+        houts = {nm: torch.empty((nfoc, cfg.n, cfg.nt), dtype=torch.float32).pin_memory() for nm in FIELDS}
         e2e_steps = max(1, min(args.steps, args.e2e_steps))
         for _ in range(min(3, args.warmup)):
             mk.run_host(hGd, htd, niter, houts)
@@ -306,10 +411,12 @@ def run_ours(args):
         torch.cuda.synchronize()
         e2e_s = shard.max_over_ranks(time.perf_counter() - t0, dist)
         barrier()
-        e2e = {"value": world * nsyn * nbytes * e2e_steps / e2e_s / 1e9, "unit": UNIT,
+        e2e = {"value": world * passes * nbytes * e2e_steps / e2e_s / 1e9, "unit": UNIT,
+               "value_algorithmic": world * nsyn * nbytes * e2e_steps / e2e_s / 1e9,
                "h2d_bytes_per_step": int(hGd.numel() * 4 + htd.numel() * 4),
                "d2h_bytes_per_step": int(sum(t.numel() * 4 for t in houts.values())), "steps": e2e_steps,
                "ms_per_step": 1e3 * e2e_s / e2e_steps, "api": "mk_run_host (pinned host G_d, t_d in; 6 host fields out)"}
+        del hGd, htd, houts
 
     for ptr in ipc_ptrs:            # peers' operand mappings: closed on every rank before any context goes away
         B.ipc_close(ptr)
@@ -319,41 +426,8 @@ def run_ours(args):
             dist.destroy_process_group()
         return 0
 
-    # ---- roofline of the dominant kernel (the contraction), from CUDA events recorded by the library on its stream
-    peaks = measured_peaks()
-    avg_ms = syn_ms / max(syn_n, 1)
-    traffic = None
-    tp = ROOT / "profiles" / "traffic.json"
-    if tp.exists():
-        traffic = json.loads(tp.read_text()).get(f"config{cfg.k}_regime{regime_used}")
     share = len(my_rows) / cfg.n            # rows mode: this rank's launches contract its own rows of R^ only
-    if regime_used == 1:
-        ach = share * nbytes / (avg_ms * 1e-3) / 1e9
-        roof = {"bound": "hbm", "kernel": "k_syn_gemv", "achieved": ach, "peak": peaks["hbm_gbs"], "unit": "GB/s",
-                "frac": ach / peaks["hbm_gbs"], "traffic": traffic, "peak_source": peaks["source"] + " copy bandwidth (MEASURED_PEAKS.json)",
-                "frac_of_nominal_8TBps": ach / 8000.0, "launches_timed": int(syn_n), "avg_launch_ms": avg_ms,
-                "share_of_step": syn_ms / ms_total}
-    else:
-        flops = share * 8.0 * nfoc * cfg.n * cfg.n * nb        # algorithmic: one complex MAC (8 flops) per element of R^ and focal point
-        ach = flops / (avg_ms * 1e-3) / 1e12
-        sm_max = clocks.get("sm_max_mhz") or 1965.0
-        ffma_peak = 2 * 128 * 148 * sm_max * 1e6 / 1e12     # FFMA lanes x SMs x max clock
-        if regime_used == 2:
-            roof = {"bound": "alu", "kernel": "k_syn_gemm_ffma", "achieved": ach, "peak": ffma_peak, "unit": "TFLOP/s",
-                    "frac": ach / ffma_peak, "traffic": traffic,
-                    "peak_source": "2 x 128 FFMA lanes x 148 SMs x clocks.max.sm (guide unit counts)",
-                    "launches_timed": int(syn_n), "avg_launch_ms": avg_ms, "share_of_step": syn_ms / ms_total}
-        else:
-            # 3xTF32: every algorithmic flop costs three tf32 tensor flops.  Peak for this dtype = measured bf16 peak
-            # (sustained figure: the kernel is timed inside a long step) x 1/2 (nominal tf32 : bf16), / 3 for the split.
-            tf32_peak = 0.5 * peaks["bf16_tflops_sustained"]
-            roof = {"bound": "tensor", "kernel": "k_syn_gemm_tf32x3", "achieved": ach, "peak": tf32_peak / 3.0, "unit": "TFLOP/s",
-                    "frac": ach / (tf32_peak / 3.0), "traffic": traffic,
-                    "peak_source": peaks["source"] + " bf16 sustained x 0.5 (nominal tf32:bf16) / 3 (3xTF32 split); "
-                                   "achieved counts algorithmic fp32 flops (8 per complex MAC)",
-                    "tensor_tflops_issued": 3.0 * ach, "tf32_peak": tf32_peak,
-                    "frac_of_fp32_ffma_roofline": ach / ffma_peak,
-                    "launches_timed": int(syn_n), "avg_launch_ms": avg_ms, "share_of_step": syn_ms / ms_total}
+    roof = roofline_of(cfg, nb, nbytes, regime_used, syn_n, syn_ms, ms_total, clocks, share)
 
     # ---- the oracle as it stands, on this box's host cores, bounded sample (rank 0, N = 1 only)
     cpu = None
@@ -365,14 +439,45 @@ def run_ours(args):
                "sample": f"one oracle synthesis R N_0 (direct time-domain convolution, fp64) on {nrec_s} of {cfg.n} receivers x 1 focal "
                          f"point of config {cfg.k}: {t_s:.2f} s per synthesis, {getattr(oracle_sample, 'reps', 1)} repetitions"}
 
+    # ---- the large-batch regimes in the same invocation (N = 1, default workload only): configs 2 (tcgen05 and FFMA), 3, 4
+    secondary = []
+    if world == 1 and args.workload == 1 and not rows_mode and not args.no_secondary:
+        del dGd, dtd, douts, R, Gd, td
+        torch.cuda.empty_cache()
+        c2 = configs.get(2)          # same R as config 1 (BASELINE.json): the context and its R^ are reused
+        secondary.append(secondary_entry(mk, c2, 0, args.secondary_steps, 3, local, dev, image=True))
+        secondary.append(secondary_entry(mk, c2, 2, args.secondary_steps, 3, local, dev))
+        mk.close()
+        for k in (3, 4):
+            ck = configs.get(k)
+            free, _ = torch.cuda.mem_get_info()
+            need = 8.0 * ck.n * nb * (ck.n + 16) + 4.0 * ck.nfoc * ck.n * ck.nt * 4.2 + 8.0 * ck.n * nb * ck.nfoc * 6 + 6e9
+            if free < need:
+                secondary.append({"workload": f"config{k}:{ck.name}", "skipped": f"needs about {need / 1e9:.0f} GB of device memory, {free / 1e9:.0f} GB free"})
+                continue
+            mkk = B.Marchenko(ck.n, ck.n, ck.nt, ck.dt, ck.dx, ck.fmin, ck.fmax)
+            mkk.set_option(B.MK_OPT_EPS_SAMPLES, ck.eps)
+            t0 = time.perf_counter()
+            ingest_device(mkk, ck, dev)
+            t_ing = time.perf_counter() - t0
+            e = secondary_entry(mkk, ck, 0, args.secondary_steps, 3, local, dev)
+            e["ingest_s"] = t_ing
+            secondary.append(e)
+            mkk.close()
+            torch.cuda.empty_cache()
+    else:
+        mk.close()
+
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": ms_total / args.steps, "higher_is_better": True, "scaling": "strong" if rows_mode else "weak", "vs_baseline": None,
             "dtype": "f32", "data": "synthetic",
+            "value_algorithmic": value_alg,
             "config": {"workload": f"config{cfg.k}:{cfg.name}", "n": cfg.n, "nt": cfg.nt, "nfoc": nfoc, "niter": niter, "nb": nb,
-                       "syntheses_per_step": nsyn, "contraction_launches_per_step": syn_n / max(args.steps, 1),
-                       "note": ("value counts the niter + 2 syntheses of Algorithm 1 (algorithmic bytes: one R^ per synthesis); with "
-                                "1, 2 or 4 focal points the two syntheses of the finals share ONE pass over R^ (2 nfoc right-hand sides)"
-                                if syn_n / max(args.steps, 1) < nsyn else "one pass over R^ per synthesis"),
+                       "syntheses_per_step": nsyn, "contraction_launches_per_step": passes,
+                       "note": ("value = bytes of R^ actually streamed per second (contraction launches x bytes of R^ / time); "
+                                "value_algorithmic counts one R^ per synthesis of Algorithm 1 (niter + 2): with 1, 2 or 4 focal points the two "
+                                "syntheses of the finals share ONE pass over R^ (2 nfoc right-hand sides), so a step makes niter + 1 passes"
+                                if passes < nsyn else "one pass over R^ per synthesis"),
                        "rhat_bytes": nbytes, "regime": regime_used,
                        "l2": f"inputs_larger_than_L2 (R^ {nbytes / 1e9:.2f} GB vs 126 MB L2; no flush needed)",
                        "input_source": "device generator, 64-shot chunks (no e2e / cpu_baseline legs)" if big else "host arrays",
@@ -384,11 +489,10 @@ def run_ours(args):
             "focal_point_iterations_per_s": jobs * nfoc * niter * args.steps / (ms_total * 1e-3),
             "clocks": clocks,
             "e2e": e2e,
-            "gpu_launches": launches, "roofline": roof, "cpu_baseline": cpu}
+            "gpu_launches": launches, "roofline": roof, "cpu_baseline": cpu, "secondary": secondary}
     print(json.dumps(line), flush=True)
     if world > 1:
         dist.destroy_process_group()
-    mk.close()
     return 0
 
 
@@ -407,6 +511,8 @@ def main():
     ap.add_argument("--e2e-steps", type=int, default=50)
     ap.add_argument("--cpu-budget", type=float, default=15.0, help="seconds of oracle work for cpu_baseline")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-secondary", action="store_true", help="skip the large-batch configurations (2, 2 with --regime 2, 3, 4) of the default run")
+    ap.add_argument("--secondary-steps", type=int, default=10)
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "ours":
         args.warmup = 3

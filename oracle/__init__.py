@@ -52,6 +52,9 @@ def lib():
         L.orc_marchenko.restype = C.c_int
         L.orc_marchenko.argtypes = [C.c_int, C.c_int, C.c_double, C.c_double, C.c_double, C.c_double, C.c_int,
                                     _F32, C.c_int, _F32, _F32, C.c_int] + [C.c_void_p] * 8
+        L.orc_marchenko_geom.restype = C.c_int
+        L.orc_marchenko_geom.argtypes = [C.c_int, C.c_int, C.c_int, C.c_double, _F64, _I32, C.c_double, C.c_double, C.c_int,
+                                         _F32, C.c_int, _F32, _F32, C.c_int] + [C.c_void_p] * 8
         L.orc_init_subset.argtypes = [C.c_int, C.c_int, _F32] + [C.c_void_p] * 5
         L.orc_step_subset.argtypes = [C.c_int, C.c_int, C.c_int, C.c_double, _F64, _F32, C.c_int, _F64, _I32, C.c_int,
                                       C.c_int, C.c_int, _F64] + [C.c_void_p] * 5
@@ -144,6 +147,33 @@ def marchenko(R: np.ndarray, Gd: np.ndarray, td: np.ndarray, dt: float, dx: floa
             ptrs.append(None)
     rc = lib().orc_marchenko(n, nt, dt, dx, fmin, fmax, eps, R.reshape(-1), nfoc, Gd.reshape(-1), td.reshape(-1),
                              niter, *ptrs)
+    assert rc == 0
+    return out
+
+
+def marchenko_geom(R, Gd, td, dt, w, rec_of_shot, fmin, fmax, niter, eps=8, want=("f1plus", "f1min", "f2", "pmin", "G", "Gplus", "Gminus")):
+    """The scheme for sources and receivers that are not co-located one to one (orc_marchenko_geom; NEXT-4).
+    R: [nshot][nrec][nt]; Gd [nfoc][nrec][nt], td [nfoc][nrec] on the receiver grid; w [nshot] quadrature weights of the
+    shot grid; rec_of_shot [nshot] int (receiver co-located with each shot, or -1).  Outputs on the receiver grid."""
+    R = np.ascontiguousarray(R, dtype=np.float32)
+    Gd = np.ascontiguousarray(Gd, dtype=np.float32)
+    td = np.ascontiguousarray(td, dtype=np.float32)
+    nshot, nrec, nt = R.shape
+    nfoc = Gd.shape[0]
+    assert Gd.shape == (nfoc, nrec, nt) and td.shape == (nfoc, nrec)
+    w = np.ascontiguousarray(w, dtype=np.float64)
+    ros = np.ascontiguousarray(rec_of_shot, dtype=np.int32)
+    assert w.shape == (nshot,) and ros.shape == (nshot,)
+    out = {"N_iters": np.empty((niter, nfoc, nrec, nt), dtype=np.float64)}
+    ptrs = [out["N_iters"].ctypes.data_as(C.c_void_p)]
+    for nm in ("f1plus", "f1min", "f2", "pmin", "G", "Gplus", "Gminus"):
+        if nm in want:
+            out[nm] = np.empty((nfoc, nrec, nt), dtype=np.float64)
+            ptrs.append(out[nm].ctypes.data_as(C.c_void_p))
+        else:
+            ptrs.append(None)
+    rc = lib().orc_marchenko_geom(nshot, nrec, nt, dt, w, ros, fmin, fmax, eps, R.reshape(-1), nfoc, Gd.reshape(-1), td.reshape(-1),
+                                  niter, *ptrs)
     assert rc == 0
     return out
 

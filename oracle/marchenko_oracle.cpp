@@ -312,4 +312,51 @@ int orc_marchenko(int n, int nt, double dt, double dx, double fmin, double fmax,
   return 0;
 }
 
+// NEXT-4: the same scheme for a spread whose sources and receivers are NOT co-located one to one.
+// Eq. (1) integrates over source positions x and is evaluated at receiver positions x_R
+// ("segment size is the column size (nr receivers)") keeps the two counts apart.  R [nshot][nrec][nt] fp32; G_d
+// [nfoc][nrec][nt] and t_d [nfoc][nrec] live on the RECEIVER grid, and so does every output.  The operand of the next
+// synthesis lives on the SHOT grid: shot s carries the trace of the receiver co-located with it, rec_of_shot[s], or
+// zero when rec_of_shot[s] < 0 (no receiver there: that source position contributes nothing, the field is not known
+// at it) [DESIGN.md reading G15].  w [nshot]: quadrature weights of the shot grid (irregular spacing: the caller's).
+// Each iteration is orc_step_subset with "subset" = every receiver; the finals are orc_finals_subset.
+int orc_marchenko_geom(int nshot, int nrec, int nt, double dt, const double* w, const int* rec_of_shot, double fmin,
+                       double fmax, int eps, const float* R, int nfoc, const float* Gd, const float* td, int niter,
+                       double* N_iters, double* f1plus_out, double* f1min_out, double* f2_out, double* pmin_out, double* G_out,
+                       double* Gplus_out, double* Gminus_out) {
+  int klo, khi;
+  orc_band(nt, dt, fmin, fmax, &klo, &khi);
+  const size_t ntr = (size_t)nfoc * nrec, tot = ntr * nt, tot_s = (size_t)nfoc * nshot * nt;
+  std::vector<int> h(ntr);
+  orc_window((int)ntr, nt, dt, eps, td, h.data());
+  std::vector<double> N(tot), Nn(tot), f1plus(tot), f2(tot), f1min(tot), pmin(tot), Ns(tot_s), As(tot_s), Bs(tot_s);
+  orc_init_subset((int)ntr, nt, Gd, N.data(), f1plus.data(), f2.data(), f1min.data(), pmin.data());
+  // receiver grid -> shot grid: a copy of whole traces (index plumbing, no arithmetic)
+  auto to_shots = [&](const std::vector<double>& src, std::vector<double>& dst) {
+    for (int f = 0; f < nfoc; ++f)
+      for (int s = 0; s < nshot; ++s) {
+        double* d = dst.data() + ((size_t)f * nshot + s) * nt;
+        const int r = rec_of_shot[s];
+        if (r < 0) std::fill(d, d + nt, 0.0);
+        else std::memcpy(d, src.data() + ((size_t)f * nrec + r) * nt, nt * sizeof(double));
+      }
+  };
+  for (int it = 0; it < niter; ++it) {
+    to_shots(N, Ns);
+    orc_step_subset(nshot, nrec, nt, dt, w, R, nfoc, Ns.data(), h.data(), klo, khi, it, Nn.data(), nullptr, pmin.data(), f2.data(),
+                    f1plus.data(), f1min.data());
+    N.swap(Nn);
+    if (N_iters) std::memcpy(N_iters + (size_t)it * tot, N.data(), tot * sizeof(double));
+  }
+  to_shots(f1plus, As);
+  to_shots(f1min, Bs);
+  orc_finals_subset(nshot, nrec, nt, dt, w, R, nfoc, As.data(), Bs.data(), f1plus.data(), f1min.data(), f2.data(), pmin.data(), klo,
+                    khi, G_out, Gplus_out, Gminus_out);
+  if (f1plus_out) std::memcpy(f1plus_out, f1plus.data(), tot * sizeof(double));
+  if (f1min_out) std::memcpy(f1min_out, f1min.data(), tot * sizeof(double));
+  if (f2_out) std::memcpy(f2_out, f2.data(), tot * sizeof(double));
+  if (pmin_out) std::memcpy(pmin_out, pmin.data(), tot * sizeof(double));
+  return 0;
+}
+
 }  // extern "C"

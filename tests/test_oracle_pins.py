@@ -358,6 +358,58 @@ def test_init_is_the_time_reversed_first_arrival():
     assert not sub.f1min.any() and not sub.pmin.any()
 
 
+def test_general_geometry_is_the_square_scheme_on_the_union_grid():
+    """orc_marchenko_geom (sources and receivers not co-located one to one; eq. (1): integral over source
+    positions, evaluated at receiver positions; PAPER.md:28 keeps ns and nr apart).  Pins:
+    (i) identity geometry (nshot = nrec, shot s at receiver s, trapezoid weights) IS orc_marchenko, bit for bit;
+    (ii) any geometry equals the pinned SQUARE scheme on the union grid of positions, where a missing source or receiver
+    is a zero row / column of R and a zero first arrival with an empty window, and the shot weights are folded into R
+    (the square scheme has its own trapezoid weights) — an independent route through code that is pinned elsewhere."""
+    nt, dt, dx, eps, K = 32, 0.004, 10.0, 1, 4
+    fmin, fmax = 20.0, 100.0
+    # (i)
+    n, nfoc = 6, 2
+    R = (0.02 * rng.standard_normal((n, n, nt))).astype(np.float32)
+    Gd = rng.standard_normal((nfoc, n, nt)).astype(np.float32)
+    td = (dt * rng.uniform(5, 12, size=(nfoc, n))).astype(np.float32)
+    sq = oracle.marchenko(R, Gd, td, dt, dx, fmin, fmax, niter=K, eps=eps)
+    ge = oracle.marchenko_geom(R, Gd, td, dt, oracle.weights(n, dx), np.arange(n), fmin, fmax, K, eps)
+    for nm in ("N_iters", "f1plus", "f1min", "f2", "pmin", "G", "Gplus", "Gminus"):
+        np.testing.assert_array_equal(ge[nm], sq[nm])
+    # (ii) union grid of 9 positions; shots at S, receivers at Rc; 2 shots without a receiver, 3 receivers without a shot
+    U = 9
+    S = np.array([0, 1, 3, 4, 6, 8])            # positions of the 6 shots
+    Rc = np.array([1, 2, 3, 5, 6, 7, 8])        # positions of the 7 receivers
+    ns, nr = len(S), len(Rc)
+    rec_of_shot = np.array([int(np.nonzero(Rc == p)[0][0]) if p in Rc else -1 for p in S])
+    assert (rec_of_shot >= 0).sum() == 4
+    Rg = (0.03 * rng.standard_normal((ns, nr, nt))).astype(np.float32)
+    Gdg = rng.standard_normal((nfoc, nr, nt)).astype(np.float32)
+    tdg = (dt * rng.uniform(5, 12, size=(nfoc, nr))).astype(np.float32)
+    wU = oracle.weights(U, dx)
+    # irregular quadrature weights of the shot grid, chosen so that folding them into R is exact in fp32: powers of two times wU
+    w2 = np.array([wU[p] * 2.0 ** k for p, k in zip(S, [0, 1, -1, 0, 2, -2])])
+    RU = np.zeros((U, U, nt), np.float32)
+    for i, ps in enumerate(S):
+        for j, pr in enumerate(Rc):
+            RU[ps, pr] = Rg[i, j] * np.float32(w2[i] / wU[ps])          # exact: a power of two
+    GdU = np.zeros((nfoc, U, nt), np.float32)
+    tdU = np.zeros((nfoc, U), np.float32)                                 # t_d = 0: window half-width 0, trace stays zero
+    GdU[:, Rc] = Gdg
+    tdU[:, Rc] = tdg
+    ge = oracle.marchenko_geom(Rg, Gdg, tdg, dt, w2, rec_of_shot, fmin, fmax, K, eps)
+    sq = oracle.marchenko(RU, GdU, tdU, dt, dx, fmin, fmax, niter=K, eps=eps)
+    scale = np.abs(sq["G"]).max()
+    for nm in ("f1plus", "f1min", "f2", "pmin", "G", "Gplus", "Gminus"):
+        np.testing.assert_allclose(ge[nm], sq[nm][:, Rc], atol=1e-13 * scale, rtol=0)
+        off = np.setdiff1d(np.arange(U), Rc)
+        if nm in ("f1plus", "f1min", "f2"):
+            assert not sq[nm][:, off].any()                               # nothing lives where there is no receiver
+    for k in range(K):
+        np.testing.assert_allclose(ge["N_iters"][k], sq["N_iters"][k][:, Rc], atol=1e-13 * scale, rtol=0)
+    assert np.abs(ge["N_iters"][-1]).max() > 1e-6 * np.abs(ge["N_iters"][0]).max() > 0
+
+
 def test_image_is_the_zero_lag_of_the_convolution():
     """image[f] = dt sum_r w[r] (G^- (*) f1plus)[0]: brute force on a tiny case and numpy's FFT convolution theorem."""
     nfoc, n, nt, dt, dx = 3, 5, 16, 0.004, 10.0
