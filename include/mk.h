@@ -5,7 +5,8 @@
  * readings of the paper listed in DESIGN.md.
  *
  * What the library computes (notation of §8):
- *   n = nshot = nrec (co-located fixed spread); time index j in [0, nt), negative times stored wrapped
+ *   nshot sources, nrec receivers (n = nshot = nrec for a co-located fixed spread, as in every BASELINE.json config; see
+ *   mk_set_geometry for the general case); time index j in [0, nt), negative times stored wrapped
  *   (T f)[j] = f[(nt - j) % nt];  band B = {klo..khi} = {k : fmin <= k/(nt dt) <= fmax};  w[s] trapezoid weights
  *   synthesis  (R N)[f][r][j] = P_B { dt * sum_s w[s] * sum_j' R[s][r][(j - j') % nt] * N[f][s][j'] }      eq. (1)
  *   window     Theta[f][r][j] = ( |j+-| < h ),  h = clamp(floor(t_d/dt + 0.5) - eps, 0, nt/2)               PAPER.md:24, G2
@@ -84,8 +85,9 @@ enum {
 };
 
 /* Create a context for an nshot x nrec x nt reflection response sampled at dt (s) and dx (m), band fmin..fmax (Hz).
- * Validates nshot == nrec > 0 (G10: co-located spread; the output index of one iteration is the integration
- * index of the next), nt a power of two in [16, 32768], dt, dx > 0, 0 <= fmin <= fmax <= 1/(2 dt).
+ * Validates nshot, nrec > 0, nt a power of two in [16, 32768], dt, dx > 0, 0 <= fmin <= fmax <= 1/(2 dt).  With
+ * nshot == nrec the spread is taken as co-located (shot s at receiver s: the output index of one iteration is the
+ * integration index of the next, G10); otherwise see mk_set_geometry.
  * Allocates R^ [nrec][nb][ld_shot] complex64 on the current CUDA device (BASELINE.json north_star (a)
  * "the data layout is ordered as receivers, frequencies and shots").  *out receives the context; when a failure
  * happens after the context exists, *out is still set so that mk_last_error can be read (destroy it afterwards),
@@ -100,6 +102,17 @@ int mk_set_stream(mk_ctx* ctx, void* cuda_stream);
 
 int mk_set_option(mk_ctx* ctx, int key, double value);
 int mk_get_info(mk_ctx* ctx, int key, double* value);
+
+/* NEXT-4: sources and receivers that are not co-located one to one, irregular source spacing.
+ * Eq. (1) integrates over SOURCE positions and is evaluated at RECEIVER positions (PAPER.md:28 keeps
+ * "ns" and "nr" apart): G_d, t_d and every output field live on the receiver grid, [nfoc][nrec][nt]; the operand of the
+ * next synthesis lives on the shot grid.  h_rec_of_shot [nshot] (HOST, int): the receiver co-located with shot s, or -1
+ * when there is none — that source position then carries a zero operand, it contributes nothing to the integral because
+ * the field is not known there (reading G15); two shots may not share a receiver.  NULL = shot s at receiver
+ * s (for s < min(nshot, nrec)), which is also the state after mk_create.  h_weights [nshot] (HOST, float): quadrature
+ * weights w[s] of the shot grid in metres (finite, >= 0), folded into R^ at ingest; NULL = trapezoid rule with spacing
+ * dx.  Must be called before the first mk_load_R (MK_ERR_STATE afterwards) and not on a row-sharded context. */
+int mk_set_geometry(mk_ctx* ctx, const int* h_rec_of_shot, const float* h_weights);
 
 /* Ingest ("the whole reflection data being read, Fourier transformed and stored", 63-66; §8(a) a0).
  * d_R_time: [nshots][nrec][nt] fp32 time-domain R(x_R = rec, x = shot, t) for shots shot0 .. shot0+nshots-1.
@@ -145,12 +158,14 @@ int mk_finish(mk_ctx* ctx, const mk_outputs* d_out); /* a7; may be called more t
 int mk_step_contract(mk_ctx* ctx);
 int mk_step_post(mk_ctx* ctx, float* d_N_i);
 
-/* One bare synthesis without window (a6 + a2 + a3): d_S_out = R d_N_in, both [nfoc][nrec][nt] fp32.
- * Does not disturb a run in progress.  This is the call the GB/s metric times. */
+/* One bare synthesis without window (a6 + a2 + a3): d_S_out = R d_N_in, both [nfoc][nrec][nt] fp32 (with a geometry set
+ * by mk_set_geometry, d_N_in is on the receiver grid like every iterate: the trace of receiver r is the operand of the
+ * shot co-located with it).  Does not disturb a run in progress.  This is the call the GB/s metric times. */
 int mk_synthesis(mk_ctx* ctx, const float* d_N_in, float* d_S_out, int nfoc);
 
 /* NEXT-1 (§8(f)): double-focusing image: the zero-time sample of G^- convolved with f1plus and
- * integrated over receivers,  image[f] = dt * sum_r w[r] sum_j G^-[f][r][(nt-j)%nt] * f1plus[f][r][j].
+ * integrated over receivers (trapezoid rule with spacing dx over the nrec receivers),
+ *   image[f] = dt * sum_r w[r] sum_j G^-[f][r][(nt-j)%nt] * f1plus[f][r][j].
  * d_Gminus: [nfoc][nrec][nt] fp32 as returned by mk_run / mk_finish for the current run; d_image: [nfoc] fp32. */
 int mk_image(mk_ctx* ctx, const float* d_Gminus, float* d_image);
 
@@ -169,6 +184,7 @@ int mk_image(mk_ctx* ctx, const float* d_Gminus, float* d_image);
  * rank reads and writes only its own receiver rows of them (the other rows of its outputs are zero or untouched).
  * mk_run, mk_run_host, mk_synthesis and the G^-/G^+ fields of mk_finish need the whole operand at once and return
  * MK_ERR_STATE on a sharded context. */
+/* (row sharding exchanges operand rows by receiver index, so a sharded context needs nshot == nrec.) */
 int mk_create_sharded(mk_ctx** out, int nshot, int nrec, int nt, double dt, double dx, double fmin, double fmax,
                       int row0, int nrows);
 

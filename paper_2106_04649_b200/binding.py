@@ -23,7 +23,8 @@ REGIME_AUTO, REGIME_GEMV, REGIME_GEMM_FFMA, REGIME_GEMM_TF32X3 = 0, 1, 2, 3
 SYMBOLS = ("mk_create", "mk_destroy", "mk_set_stream", "mk_set_option", "mk_get_info", "mk_load_R", "mk_load_R_host",
            "mk_run", "mk_run_host", "mk_begin", "mk_step", "mk_finish", "mk_synthesis", "mk_image", "mk_last_error",
            "mk_version", "mk_create_sharded", "mk_operand", "mk_operand_exchanged", "mk_finish_prepare", "mk_finish_complete",
-           "mk_operand_reserve", "mk_operand_attach", "mk_step_contract", "mk_step_post", "mk_ipc_export", "mk_ipc_open", "mk_ipc_close")
+           "mk_operand_reserve", "mk_operand_attach", "mk_step_contract", "mk_step_post", "mk_ipc_export", "mk_ipc_open", "mk_ipc_close",
+           "mk_set_geometry")
 MK_FIELD_GMINUS, MK_FIELD_GPLUS = 1, 2
 
 
@@ -63,6 +64,7 @@ def load():
     L.mk_set_stream.argtypes = [vp, vp]
     L.mk_set_option.argtypes = [vp, ci, cd]
     L.mk_get_info.argtypes = [vp, ci, C.POINTER(cd)]
+    L.mk_set_geometry.argtypes = [vp, vp, vp]
     L.mk_load_R.argtypes = [vp, vp, ci, ci]
     L.mk_load_R_host.argtypes = [vp, vp, ci, ci]
     L.mk_run.argtypes = [vp, vp, vp, ci, ci, C.POINTER(mk_outputs)]
@@ -189,6 +191,19 @@ class Marchenko:
         return o
 
     # -- the calls of include/mk.h
+    def set_geometry(self, rec_of_shot=None, weights=None):
+        """rec_of_shot: int array [nshot] (receiver co-located with each shot, -1 = none) or None; weights: float array
+        [nshot] (quadrature weights of the shot grid) or None.  Before the first load_R."""
+        import numpy as np
+        ros = None if rec_of_shot is None else np.ascontiguousarray(rec_of_shot, dtype=np.int32)
+        w = None if weights is None else np.ascontiguousarray(weights, dtype=np.float32)
+        if ros is not None and ros.shape != (self.nshot,):
+            raise ValueError("rec_of_shot must have nshot entries")
+        if w is not None and w.shape != (self.nshot,):
+            raise ValueError("weights must have nshot entries")
+        self._check(self._L.mk_set_geometry(self._h, None if ros is None else C.c_void_p(ros.ctypes.data),
+                                            None if w is None else C.c_void_p(w.ctypes.data)))
+
     def load_R(self, d_R_time, shot0=0):
         import torch
         nshots = d_R_time.shape[0]

@@ -78,6 +78,7 @@ OperandOut operand_out(mk_ctx* c, int slot, int ldf) {
   OperandOut O{};
   O.ldf = ldf;
   O.plain = slot ? c->d_Nhat2 : c->d_Nhat;
+  O.shot_of_rec = c->d_shot_of_rec;
   if (c->npeer[slot] > 0 && c->peer_key[slot] == c->operand_key[slot] && c->operand_key[slot] != 0) {
     O.npeer = c->npeer[slot];
     for (int p = 0; p < O.npeer; ++p) O.peer[p] = reinterpret_cast<float2*>(c->peer_plane[slot][p]);
@@ -157,6 +158,47 @@ bool overlaps(const void* a, const void* b, size_t bytes) {
   return x < y + bytes && y < x + bytes;
 }
 
+// quadrature weights of the shot grid (folded into R^ at ingest as dt * w[s]) and the receiver -> shot map of the
+// operand rows.  h_w == nullptr: trapezoid rule with spacing dx over the ns shots; h_rec_of_shot == nullptr: shot s is
+// co-located with receiver s (for s < min(ns, n); further shots have no receiver, further receivers no shot).
+int upload_geometry(mk_ctx* c, const int* h_rec_of_shot, const float* h_w) {
+  std::vector<float> ws(c->ns);
+  for (int s = 0; s < c->ns; ++s) {
+    const double w = h_w ? (double)h_w[s] : ((c->ns > 1 && (s == 0 || s == c->ns - 1)) ? 0.5 * c->dx : c->dx);
+    if (!(w >= 0.0) || !std::isfinite(w)) return set_err(c, MK_ERR_INVALID_ARG, "mk_set_geometry: weights must be finite and >= 0");
+    ws[s] = (float)(c->dt * w);
+  }
+  std::vector<int> sor(c->n, -1);
+  bool identity = c->ns == c->n;
+  for (int s = 0; s < c->ns; ++s) {
+    const int r = h_rec_of_shot ? h_rec_of_shot[s] : (s < c->n ? s : -1);
+    if (r < -1 || r >= c->n) return set_err(c, MK_ERR_INVALID_ARG, "mk_set_geometry: rec_of_shot out of range");
+    if (r >= 0) {
+      if (sor[r] != -1) return set_err(c, MK_ERR_INVALID_ARG, "mk_set_geometry: two shots at one receiver");
+      sor[r] = s;
+    }
+    identity = identity && r == s;
+  }
+  if (!c->d_wscale) {
+    size_t cap = 0;
+    if (int rc = ensure(c, &c->d_wscale, &cap, (size_t)c->ns, "weights")) return rc;
+  }
+  if (int rc = check_cuda(c, cudaMemcpy(c->d_wscale, ws.data(), ws.size() * sizeof(float), cudaMemcpyHostToDevice), "weights upload")) return rc;
+  if (identity) {  // the kernels take the receiver index itself
+    if (c->d_shot_of_rec) {
+      cudaFree(c->d_shot_of_rec);
+      c->device_bytes -= (size_t)c->n * sizeof(int);
+      c->d_shot_of_rec = nullptr;
+    }
+    return MK_OK;
+  }
+  if (!c->d_shot_of_rec) {
+    size_t cap = 0;
+    if (int rc = ensure(c, &c->d_shot_of_rec, &cap, (size_t)c->n, "receiver -> shot map")) return rc;
+  }
+  return check_cuda(c, cudaMemcpy(c->d_shot_of_rec, sor.data(), sor.size() * sizeof(int), cudaMemcpyHostToDevice), "map upload");
+}
+
 // outputs of the finals (and N_last) are written while the accumulators are still being read: they must not overlap
 // f1plus / f1min (the caller's fields when mk_run accumulates in them, else the library's)
 int check_output_alias(mk_ctx* c, const mk_outputs* o, const float* acc_plus, const float* acc_min, size_t bytes) {
@@ -219,8 +261,9 @@ int mk_create_sharded(mk_ctx** out, int nshot, int nrec, int nt, double dt, doub
                       int nrows) {
   if (!out) return MK_ERR_INVALID_ARG;
   *out = nullptr;
-  if (nshot <= 0 || nrec <= 0 || nshot != nrec) return MK_ERR_INVALID_ARG;
+  if (nshot <= 0 || nrec <= 0) return MK_ERR_INVALID_ARG;
   if (row0 < 0 || nrows <= 0 || row0 + nrows > nrec) return MK_ERR_INVALID_ARG;
+  if (nrows != nrec && nshot != nrec) return MK_ERR_INVALID_ARG;  // row sharding exchanges operand rows by receiver index: co-located spreads only
   if (!is_pow2(nt) || nt < 16 || nt > 32768) return MK_ERR_INVALID_ARG;
   if (!(dt > 0.0) || !(dx > 0.0) || !(fmin >= 0.0) || !(fmax >= fmin) || fmax > 0.5 / dt * (1.0 + 1e-9)) return MK_ERR_INVALID_ARG;
   int dev = 0, ndev = 0;
@@ -231,7 +274,8 @@ int mk_create_sharded(mk_ctx** out, int nshot, int nrec, int nt, double dt, doub
   mk_ctx* c = new (std::nothrow) mk_ctx();
   if (!c) return MK_ERR_OOM;
   *out = c;  // returned even on failure so that mk_last_error can be read; the caller destroys it
-  c->n = nshot;
+  c->n = nrec;
+  c->ns = nshot;
   c->r0 = row0;
   c->nrow = nrows;
   c->nt = nt;
@@ -258,6 +302,7 @@ int mk_create_sharded(mk_ctx** out, int nshot, int nrec, int nt, double dt, doub
   cudaDeviceGetAttribute(&v, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
   c->smem_optin = (size_t)v;
   c->shot_loaded.assign(nshot, 0);
+  if (int rc = upload_geometry(c, nullptr, nullptr)) return rc;  // trapezoid weights; shot s at receiver s
   // twiddles e^{-2 pi i k / nt}, evaluated in double (table constants only)
   {
     std::vector<float2> tw(nt);
@@ -296,6 +341,8 @@ int mk_destroy(mk_ctx* c) {
   cudaFree(c->d_tw);
   cudaFree(c->d_tw1k);
   cudaFree(c->d_Rhat);
+  cudaFree(c->d_wscale);
+  cudaFree(c->d_shot_of_rec);
   cudaFree(c->d_f1plus);
   cudaFree(c->d_f1min);
   cudaFree(c->d_Nhat);
@@ -350,6 +397,16 @@ int mk_set_option(mk_ctx* c, int key, double value) {
   }
 }
 
+int mk_set_geometry(mk_ctx* c, const int* h_rec_of_shot, const float* h_weights) {
+  MK_GUARD(c);
+  if (c->nrow != c->n) return set_err(c, MK_ERR_STATE, "row-sharded context: mk_set_geometry is not available");
+  if (c->shots_loaded > 0) return set_err(c, MK_ERR_STATE, "mk_set_geometry after mk_load_R: the weights are folded into R^ at ingest");
+  if (int rc = end_run(c, "mk_set_geometry")) return rc;
+  c->operand_key[0] = c->operand_key[1] = 0;  // rows that had a source may lose it: the operands are zeroed again
+  c->custom_geometry = h_rec_of_shot || h_weights;
+  return upload_geometry(c, h_rec_of_shot, h_weights);
+}
+
 int mk_get_info(mk_ctx* c, int key, double* value) {
   MK_GUARD(c);
   if (!value) return MK_ERR_INVALID_ARG;
@@ -357,7 +414,7 @@ int mk_get_info(mk_ctx* c, int key, double* value) {
     case MK_INFO_NB: *value = c->nb; return MK_OK;
     case MK_INFO_KLO: *value = c->klo; return MK_OK;
     case MK_INFO_KHI: *value = c->khi; return MK_OK;
-    case MK_INFO_RHAT_BYTES: *value = 8.0 * c->nrow * (double)c->nb * c->n; return MK_OK;
+    case MK_INFO_RHAT_BYTES: *value = 8.0 * c->nrow * (double)c->nb * c->ns; return MK_OK;
     case MK_INFO_RHAT_BYTES_PADDED: *value = 8.0 * c->nrow * (double)c->nb * c->ld; return MK_OK;
     case MK_INFO_LD_SHOT: *value = c->ld; return MK_OK;
     case MK_INFO_SHOTS_LOADED: *value = c->shots_loaded; return MK_OK;
@@ -383,7 +440,7 @@ int mk_get_info(mk_ctx* c, int key, double* value) {
 
 int mk_load_R(mk_ctx* c, const float* d_R_time, int shot0, int nshots) {
   MK_GUARD(c);
-  if (!d_R_time || shot0 < 0 || nshots <= 0 || shot0 + nshots > c->n) return set_err(c, MK_ERR_INVALID_ARG, "mk_load_R: bad shot range");
+  if (!d_R_time || shot0 < 0 || nshots <= 0 || shot0 + nshots > c->ns) return set_err(c, MK_ERR_INVALID_ARG, "mk_load_R: bad shot range");
   if (int rc = end_run(c, "mk_load_R")) return rc;  // a run in progress was started from another R^: it is over
   if (int rc = launch_load_R(c, d_R_time, shot0, nshots)) return rc;
   for (int s = shot0; s < shot0 + nshots; ++s)
@@ -396,7 +453,7 @@ int mk_load_R(mk_ctx* c, const float* d_R_time, int shot0, int nshots) {
 
 int mk_load_R_host(mk_ctx* c, const float* h_R_time, int shot0, int nshots) {
   MK_GUARD(c);
-  if (!h_R_time || shot0 < 0 || nshots <= 0 || shot0 + nshots > c->n) return set_err(c, MK_ERR_INVALID_ARG, "mk_load_R_host: bad shot range");
+  if (!h_R_time || shot0 < 0 || nshots <= 0 || shot0 + nshots > c->ns) return set_err(c, MK_ERR_INVALID_ARG, "mk_load_R_host: bad shot range");
   const size_t per_shot = (size_t)c->n * c->nt;
   size_t chunk = ((size_t)1 << 28) / per_shot;  // <= 1 GiB of fp32 per staging chunk
   if (chunk < 1) chunk = 1;
@@ -416,7 +473,7 @@ int mk_load_R_host(mk_ctx* c, const float* h_R_time, int shot0, int nshots) {
 static int begin_impl(mk_ctx* c, const float* d_Gd, const float* d_td, int nfoc, float* ext_plus, float* ext_min) {
   MK_GUARD(c);
   if (!d_Gd || !d_td || nfoc <= 0) return set_err(c, MK_ERR_INVALID_ARG, "mk_begin: bad arguments");
-  if (c->shots_loaded != c->n) return set_err(c, MK_ERR_STATE, "mk_begin before every shot of R was loaded");
+  if (c->shots_loaded != c->ns) return set_err(c, MK_ERR_STATE, "mk_begin before every shot of R was loaded");
   int regime = 0;
   if (int rc = resolve_regime(c, nfoc, &regime)) return rc;
   const int ldf = ldf_for(regime, nfoc);
@@ -743,7 +800,7 @@ int mk_synthesis(mk_ctx* c, const float* d_N_in, float* d_S_out, int nfoc) {
   MK_GUARD(c);
   if (c->nrow != c->n) return set_err(c, MK_ERR_STATE, "row-sharded context: mk_synthesis is not available");
   if (!d_N_in || !d_S_out || nfoc <= 0) return set_err(c, MK_ERR_INVALID_ARG, "mk_synthesis: bad arguments");
-  if (c->shots_loaded != c->n) return set_err(c, MK_ERR_STATE, "mk_synthesis before every shot of R was loaded");
+  if (c->shots_loaded != c->ns) return set_err(c, MK_ERR_STATE, "mk_synthesis before every shot of R was loaded");
   int regime = 0;
   if (int rc = resolve_regime(c, nfoc, &regime)) return rc;
   const int ldf = ldf_for(regime, nfoc);

@@ -7,8 +7,12 @@
 namespace mk {
 
 // a6 store: X = N^[k][r][f], into this rank's operand and, when peers are attached (row sharding), into theirs
+__device__ __forceinline__ int operand_row(const OperandOut& O, int r) { return O.shot_of_rec ? __ldg(O.shot_of_rec + r) : r; }
+
 __device__ __forceinline__ void store_operand(const OperandOut& O, int ld, int kk, int r, int f, float2 X) {
-  const size_t idx = ((size_t)kk * ld + r) * O.ldf + f;
+  const int s = operand_row(O, r);
+  if (s < 0) return;
+  const size_t idx = ((size_t)kk * ld + s) * O.ldf + f;
   O.plain[idx] = X;
   for (int p = 0; p < O.npeer; ++p) O.peer[p][idx] = X;
 }

@@ -43,6 +43,7 @@ struct Geo {
 
 struct FastParams {
   const float2* tw;    // [nt]      e^{-2 pi i k / nt}
+  const float* wscale; // [ns]     dt * w[s] (k_load_R_fast)
   const float2* tw1k;  // [32][32]  e^{-2 pi i k1 t / 1024}
   int nt, n, nb, klo, ld, ldf, nfoc;
   int r0;  // first receiver row of this context (row sharding): grid row b handles receiver r0 + b
@@ -346,7 +347,9 @@ __device__ __forceinline__ void band_out_pairs(const float2* smem, int nf, int l
 
 // operand store of two adjacent focal points f, f + 1 (f even, ldf even): see store_operand
 __device__ __forceinline__ void store_operand2(const OperandOut& O, int ld, int kk, int r, int f, float2 X0, float2 X1) {
-  const size_t idx = ((size_t)kk * ld + r) * O.ldf + f;
+  const int s = operand_row(O, r);
+  if (s < 0) return;
+  const size_t idx = ((size_t)kk * ld + s) * O.ldf + f;
   const float4 v = make_float4(X0.x, X0.y, X1.x, X1.y);
   *reinterpret_cast<float4*>(O.plain + idx) = v;
   for (int p = 0; p < O.npeer; ++p) *reinterpret_cast<float4*>(O.peer[p] + idx) = v;
@@ -367,8 +370,7 @@ __device__ __forceinline__ void prefetch_window(const float* trace, int nt, int 
 // grid (ceil(nshots / ST), nrec); Rt: [nshots][nrec][nt]                                        (a0)
 template <int HF>
 __global__ void __launch_bounds__(256, 2)
-k_load_R_fast(const float* __restrict__ Rt, float2* __restrict__ Rhat, FastParams P, int shot0, int nshots, int lgST,
-              float scale_mid, float scale_end) {
+k_load_R_fast(const float* __restrict__ Rt, float2* __restrict__ Rhat, FastParams P, int shot0, int nshots, int lgST) {
   extern __shared__ float2 smem[];
   constexpr int TS = Geo<HF>::TS;
   const int ST = 1 << lgST, r = P.r0 + blockIdx.y, g0 = blockIdx.x * ST;
@@ -382,11 +384,11 @@ k_load_R_fast(const float* __restrict__ Rt, float2* __restrict__ Rhat, FastParam
     store_Z<HF>(a, zt, me.hf, me.t, P.tw);
   }
   __syncthreads();
-  auto weight = [&](int s) { return (P.n > 1 && (s == 0 || s == P.n - 1)) ? scale_end : scale_mid; };
+  auto weight = [&](int s) { return __ldg(P.wscale + s); };
   if (lgST >= 2 && ((shot0 + g0) & 1) == 0) {
     band_out_pairs<HF>(smem, ns, lgST, P, [&](int kk, int t0, float2 X0, float2 X1, bool two) {
       const int s = shot0 + g0 + t0;  // even
-      const float c0 = weight(s), c1 = weight(s + 1);
+      const float c0 = weight(s), c1 = two ? weight(s + 1) : 0.f;
       float2* dst = Rhat + ((size_t)(r - P.r0) * P.nb + kk) * P.ld + s;
       if (two) *reinterpret_cast<float4*>(dst) = make_float4(c0 * X0.x, c0 * X0.y, c1 * X1.x, c1 * X1.y);
       else *dst = make_float2(c0 * X0.x, c0 * X0.y);  // column s + 1 belongs to another chunk (or is padding)
@@ -592,6 +594,7 @@ FastParams make_fast(const mk_ctx* c, int nfoc, int ldf) {
   FastParams P;
   P.tw = c->d_tw;
   P.tw1k = c->d_tw1k;
+  P.wscale = c->d_wscale;
   P.nt = c->nt;
   P.n = c->n;
   P.nb = c->nb;
@@ -646,8 +649,7 @@ bool fast_fft_ok(const mk_ctx* c) { return (c->nt == 2048 || c->nt == 4096) && c
 int launch_load_R_fast(mk_ctx* c, const float* d_R_time, int shot0, int nshots) {
   const Shape sh = shape_for(c, nshots);
   const dim3 grid((nshots + (1 << sh.lg) - 1) >> sh.lg, c->nrow);
-  const float sm = (float)(c->dt * c->dx), se = (float)(c->dt * c->dx * 0.5);
-  MK_FAST_LAUNCH(k_load_R_fast, grid, sh, d_R_time, c->d_Rhat, make_fast(c, 0, 0), shot0, nshots, sh.lg, sm, se);
+  MK_FAST_LAUNCH(k_load_R_fast, grid, sh, d_R_time, c->d_Rhat, make_fast(c, 0, 0), shot0, nshots, sh.lg);
 }
 
 int launch_fwd_fast(mk_ctx* c, const float* d_src, const OperandOut& O, int nfoc, bool conj_out, float* d_init_Tsrc) {

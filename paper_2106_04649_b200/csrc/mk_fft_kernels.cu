@@ -192,7 +192,7 @@ __global__ void k_window(const float* __restrict__ td, int* __restrict__ h, int 
 // ------------------------------------------------------------------------------------------------ k_load_R
 // grid (ceil(nshots/ST), nrec); Rt: [nshots][nrec][nt]
 __global__ void __launch_bounds__(kThreads) k_load_R(const float* __restrict__ Rt, float2* __restrict__ Rhat, FftParams P,
-                                                     int shot0, int nshots, int lgST, float scale_mid, float scale_end) {
+                                                     int shot0, int nshots, int lgST) {
   extern __shared__ float2 smem[];
   const int MP = mkfft::padded_len(P.plan.M), ST = 1 << lgST;
   const int r = P.r0 + blockIdx.y, g0 = blockIdx.x * ST;
@@ -211,7 +211,7 @@ __global__ void __launch_bounds__(kThreads) k_load_R(const float* __restrict__ R
     const int kk = idx >> lgST, tl = idx & (ST - 1);
     if (tl >= ns) continue;
     const int s = shot0 + g0 + tl;
-    const float sc = (P.n > 1 && (s == 0 || s == P.n - 1)) ? scale_end : scale_mid;
+    const float sc = __ldg(P.wscale + s);
     const float2 X = mkfft::rfft_bin(smem + tl * MP, P.plan, P.tw, P.klo + kk);
     Rhat[((size_t)(r - P.r0) * P.nb + kk) * P.ld + s] = make_float2(sc * X.x, sc * X.y);
   }
@@ -366,6 +366,7 @@ FftParams make_params(const mk_ctx* c, int nfoc, int ldf) {
   P.plan = c->plan;
   P.tw = c->d_tw;
   P.n = c->n;
+  P.wscale = c->d_wscale;
   P.nb = c->nb;
   P.klo = c->klo;
   P.ld = c->ld;
@@ -397,8 +398,7 @@ int launch_load_R(mk_ctx* c, const float* d_R_time, int shot0, int nshots) {
   const size_t smem = trace_smem(c, lg);
   if (int rc = set_smem(c, k_load_R, smem)) return rc;
   const dim3 grid((nshots + ST - 1) / ST, c->nrow);
-  const float sm = (float)(c->dt * c->dx), se = (float)(c->dt * c->dx * 0.5);
-  k_load_R<<<grid, kThreads, smem, c->stream>>>(d_R_time, c->d_Rhat, make_params(c, 0, 0), shot0, nshots, lg, sm, se);
+  k_load_R<<<grid, kThreads, smem, c->stream>>>(d_R_time, c->d_Rhat, make_params(c, 0, 0), shot0, nshots, lg);
   ++c->launches;
   return check_cuda(c, cudaGetLastError(), "k_load_R");
 }

@@ -12,7 +12,8 @@
 #include "fft_core.cuh"
 
 // Device layouts (complex64 = float2, interleaved re/im):
-//   Rhat [n][nb][ld]      R^[r][k][s] * dt * w[s]; ld = round_up(n, 16); pad columns are zero        (a0)
+// n = receivers (rows of R^, traces per focal point), ns = shots (the integration index; ns == n for a co-located spread)
+//   Rhat [n][nb][ld]      R^[r][k][s] * dt * w[s]; ld = round_up(ns, 16); pad columns are zero       (a0)
 //   Nhat [nb][ld][ldf]    N^[k][s][f]; pad rows (s >= n) and pad columns (f >= nfoc) are zero        (a1, a6)
 //   (ldf = nfoc for the streaming GEMV, round_up(nfoc, 4) for the FFMA GEMM, round_up(nfoc, 16) for the tcgen05 GEMM,
 //   whose TMA boxes are 32 floats wide; every regime reads this one operand)
@@ -21,7 +22,7 @@
 //   f1plus, f1min [nfoc][n][nt] fp32 time domain                                                      (a5)
 //   h [nfoc][n] int32     window half-widths                                                          (a4)
 struct mk_ctx {
-  int n = 0, nt = 0, nb = 0, klo = 0, khi = 0, ld = 0;
+  int n = 0, ns = 0, nt = 0, nb = 0, klo = 0, khi = 0, ld = 0;
   int r0 = 0, nrow = 0;  // receiver rows this context owns (row sharding; nrow == n: everything)
   bool operand_stale[2] = {false, false};  // sharded: rows produced locally but not yet exchanged
   int prepared_field = 0;                  // mk_finish_prepare
@@ -37,6 +38,9 @@ struct mk_ctx {
   bool fused_finals = true;  // MK_OPT_FUSED_FINALS
   int fft_path = 0;          // MK_OPT_FFT_PATH: 0 auto, 1 generic shared-memory passes, 2 register-resident
   float2* d_Rhat = nullptr;  // [n][nb][ld]
+  float* d_wscale = nullptr;      // [ns] dt * w[s]: folded into R^ at ingest (trapezoid over the shots unless mk_set_geometry)
+  int* d_shot_of_rec = nullptr;   // [n] shot co-located with each receiver, -1 = none; nullptr = identity (co-located spread)
+  bool custom_geometry = false;
   std::vector<unsigned char> shot_loaded;
   int shots_loaded = 0;
 
@@ -95,6 +99,7 @@ namespace mk {
 struct FftParams {
   mkfft::Plan plan;
   const float2* tw;
+  const float* wscale;  // [ns] dt * w[s] (k_load_R)
   int n, nb, klo, ld, ldf, nfoc;
   int r0;  // first receiver row of this context (grid row b handles receiver r0 + b; R^ is stored from row r0 on)
 };
@@ -105,6 +110,8 @@ constexpr int kMaxPeers = 7;  // other ranks of a row-sharded run whose operand 
 struct OperandOut {
   float2* plain;
   int ldf;
+  // row of N^ that the trace of receiver r feeds: shot_of_rec[r] (-1: no source there, nothing is stored), nullptr = r
+  const int* shot_of_rec;
   // row sharding with attached peers (mk_operand_attach): every store of this rank's rows goes to the same offset of
   // each peer's operand as well — the all-gather fused into the producing kernel as peer stores over NVLink
   int npeer;

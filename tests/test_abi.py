@@ -69,7 +69,9 @@ def test_sharded_create_rejects_bad_row_ranges(lib):
 
 def test_invalid_arguments_are_rejected_before_touching_the_device(lib):
     h = C.c_void_p()
-    assert lib.mk_create(C.byref(h), 10, 11, 64, 0.004, 10.0, 5.0, 60.0) == -1      # nshot != nrec (G10)
+    assert lib.mk_create(C.byref(h), 0, 11, 64, 0.004, 10.0, 5.0, 60.0) == -1       # no shots
+    assert not h
+    assert lib.mk_create_sharded(C.byref(h), 10, 11, 64, 0.004, 10.0, 5.0, 60.0, 0, 5) == -1   # row sharding needs nshot == nrec
     assert not h
     assert lib.mk_create(C.byref(h), 10, 10, 100, 0.004, 10.0, 5.0, 60.0) == -1     # nt not a power of two
     assert lib.mk_create(C.byref(h), 10, 10, 64, -1.0, 10.0, 5.0, 60.0) == -1
