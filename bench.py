@@ -323,6 +323,83 @@ def secondary_entry(mk, cfg, regime, steps, warmup, local, dev, image=False):
     return entry
 
 
+def h2d_peak_gbs(dev, nbytes=1 << 28, reps=4):
+    """Pinned host -> device copy rate of this box, measured live: the roofline of the out-of-core contraction."""
+    import torch
+    h = torch.empty(nbytes, dtype=torch.uint8).pin_memory()
+    d = torch.empty(nbytes, dtype=torch.uint8, device=dev)
+    d.copy_(h, non_blocking=True)
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(reps):
+        d.copy_(h, non_blocking=True)
+    e1.record()
+    torch.cuda.synchronize()
+    return reps * nbytes / (e0.elapsed_time(e1) * 1e-3) / 1e9
+
+
+def variant_entry(cfg, R, Gd, td, steps, warmup, local, dev, rhat_format=0, resident_frac=None):
+    """Config 1 again on a context of its own, with (a) R^ stored as q16 block floats (MK_OPT_RHAT_FORMAT = 1: the
+    bandwidth-bound regime with 4.25 instead of 8 bytes per element; its own tolerance) or (b) R^ out
+    of core (mk_create_streamed: a fraction of the rows resident, the rest streamed from pinned host memory through two
+    windows in HBM every contraction; bit-identical results; bound by the host link)."""
+    import torch
+    from paper_2106_04649_b200 import binding as B
+    nbytes, nb = rhat_bytes(cfg)
+    streamed = None
+    if resident_frac is not None:
+        streamed = (int(round(resident_frac * cfg.n)), 0)
+    mk = B.Marchenko(cfg.n, cfg.n, cfg.nt, cfg.dt, cfg.dx, cfg.fmin, cfg.fmax, streamed=streamed)
+    mk.set_option(B.MK_OPT_EPS_SAMPLES, cfg.eps)
+    mk.set_option(B.MK_OPT_RHAT_FORMAT, rhat_format)
+    dR = torch.empty((64, cfg.n, cfg.nt), dtype=torch.float32, device=dev)
+    for s0 in range(0, cfg.n, 64):
+        s1 = min(s0 + 64, cfg.n)
+        dR[:s1 - s0].copy_(torch.from_numpy(R[s0:s1]))
+        mk.load_R(dR[:s1 - s0], s0)
+    torch.cuda.synchronize()
+    del dR
+    dGd, dtd = torch.from_numpy(Gd).to(dev), torch.from_numpy(td).to(dev)
+    douts = {nm: torch.empty((cfg.nfoc, cfg.n, cfg.nt), dtype=torch.float32, device=dev) for nm in FIELDS}
+    h0 = mk.get_info(B.MK_INFO_H2D_BYTES)
+    r = timed_steps(mk, lambda: mk.run(dGd, dtd, cfg.niter, douts), steps, warmup, local)
+    ms = r["ms_total"] / steps
+    passes = r["syn_n"] / steps
+    avg_ms = r["syn_ms"] / max(r["syn_n"], 1)
+    stored = mk.get_info(B.MK_INFO_RHAT_BYTES_STORED) * cfg.n / mk.get_info(B.MK_INFO_LD_SHOT)     # unpadded bytes as stored
+    entry = {"workload": f"config{cfg.k}:{cfg.name}", "n": cfg.n, "nt": cfg.nt, "nfoc": cfg.nfoc, "niter": cfg.niter, "nb": nb,
+             "regime": r["regime_used"], "steps": steps, "warmup": warmup, "ms_per_step": ms, "unit": UNIT,
+             "contraction_launches_per_step": passes, "gpu_launches": r["launches"], "clocks": r["clocks"],
+             "focal_point_iterations_per_s": cfg.nfoc * cfg.niter / (ms * 1e-3)}
+    peaks = measured_peaks()
+    if rhat_format == 1:
+        ach = stored / (avg_ms * 1e-3) / 1e9
+        entry.update({"variant": "R^ stored as q16 block floats (4.25 B per complex element; lossy: tolerance 5e-4 per iteration / 1e-3 finals)",
+                      "value": passes * stored / (ms * 1e-3) / 1e9, "value_fp32_equivalent": passes * nbytes / (ms * 1e-3) / 1e9,
+                      "rhat_bytes_stored": stored,
+                      "roofline": {"bound": "hbm", "kernel": "k_syn_gemv_q16", "achieved": ach, "peak": peaks["hbm_gbs"], "unit": "GB/s",
+                                   "frac": ach / peaks["hbm_gbs"], "peak_source": peaks["source"] + " copy bandwidth (MEASURED_PEAKS.json)",
+                                   "fp32_equivalent_GBps": nbytes / (avg_ms * 1e-3) / 1e9, "traffic": None,
+                                   "launches_timed": int(r["syn_n"]), "avg_launch_ms": avg_ms, "share_of_step": r["syn_ms"] / r["ms_total"]}})
+    else:
+        h2d = (mk.get_info(B.MK_INFO_H2D_BYTES) - h0) / (steps + warmup)       # bytes of R^ over the host link per step
+        link = h2d_peak_gbs(dev)
+        ach = h2d / (ms * 1e-3) / 1e9
+        entry.update({"variant": f"R^ out of core: {streamed[0]} of {cfg.n} rows resident, window {int(mk.get_info(B.MK_INFO_WINDOW_ROWS))} rows "
+                                 "(mk_create_streamed; results bit-identical to the resident context)",
+                      "value": passes * nbytes / (ms * 1e-3) / 1e9, "h2d_bytes_per_step": h2d,
+                      "roofline": {"bound": "host_link", "kernel": "H2D copies of R^ row blocks overlapped with k_syn_gemv", "achieved": ach,
+                                   "peak": link, "unit": "GB/s", "frac": ach / link,
+                                   "peak_source": "pinned host -> device cudaMemcpyAsync rate measured in this run (256 MiB copies)",
+                                   "floor_ms_per_step": h2d / link / 1e6, "traffic": None,
+                                   "launches_timed": int(r["syn_n"]), "avg_launch_ms": avg_ms, "share_of_step": r["syn_ms"] / r["ms_total"]}})
+    mk.close()
+    del dGd, dtd, douts
+    torch.cuda.empty_cache()
+    return entry
+
+
 def run_ours(args):
     import torch
     import torch.distributed as dist
@@ -442,6 +519,9 @@ def run_ours(args):
     # ---- the large-batch regimes in the same invocation (N = 1, default workload only): configs 2 (tcgen05 and FFMA), 3, 4
     secondary = []
     if world == 1 and args.workload == 1 and not rows_mode and not args.no_secondary:
+        # config 1 with compressed R^ (NEXT-4) and with R^ out of core (NEXT-3): contexts of their own
+        secondary.append(variant_entry(cfg, R, Gd, td, 100, 5, local, dev, rhat_format=1))
+        secondary.append(variant_entry(cfg, R, Gd, td, 5, 3, local, dev, resident_frac=0.25))
         del dGd, dtd, douts, R, Gd, td
         torch.cuda.empty_cache()
         c2 = configs.get(2)          # same R as config 1 (BASELINE.json): the context and its R^ are reused

@@ -63,8 +63,17 @@ enum {
   MK_OPT_TIMING = 3,      /* 1: bracket every contraction launch with CUDA events on the context's stream */
   MK_OPT_FUSED_FINALS = 5, /* 1 (default): with 1, 2 or 4 focal points mk_finish / mk_run compute the extra syntheses of G^- and
                              G^+ in ONE pass over R^ (2 nfoc right-hand sides, streaming GEMV); 0: one pass each */
-  MK_OPT_FFT_PATH = 4     /* transform kernels: 0 auto (default), 1 generic shared-memory passes (any nt),
+  MK_OPT_FFT_PATH = 4,    /* transform kernels: 0 auto (default), 1 generic shared-memory passes (any nt),
                              2 register-resident path (nt = 2048 or 4096 only; MK_ERR_INVALID_ARG otherwise) */
+  MK_OPT_RHAT_FORMAT = 6  /* NEXT-4 (compressed R "accelerates data loading"): storage of
+                             R^.  0 (default): complex64.  1: "q16" block floating point — per (receiver, bin) row, blocks of
+                             16 shots share one fp32 scale sc = max(|re|, |im|) / 32767 and every component is the int16
+                             rint(v / sc): 4.25 bytes per complex element instead of 8, error <= sc / 2 per component.  The
+                             lossy format serves the bandwidth-bound regime only (nfoc <= 8, streaming GEMV with fp32
+                             accumulation; more focal points: MK_ERR_INVALID_ARG) and is held to its own tolerance
+                             (DESIGN.md section 6c), not to north_star's.  Must be set before the first mk_load_R
+                             (MK_ERR_STATE afterwards); with it mk_load_R needs shot0 and nshots to be multiples of 16
+                             (except at the last shot).  Not available on row-sharded or streamed contexts */
 };
 
 /* mk_get_info keys (values returned as double) */
@@ -81,7 +90,11 @@ enum {
   MK_INFO_SYN_RESET = 10,    /* resets the two counters above; value returned is 0 */
   MK_INFO_KERNEL_LAUNCHES = 11, /* total kernels this context has launched since creation */
   MK_INFO_REGIME_USED = 12,  /* regime of the last contraction launch (1, 2 or 3) */
-  MK_INFO_DEVICE_BYTES = 13  /* device memory currently owned by the context */
+  MK_INFO_DEVICE_BYTES = 13, /* device memory currently owned by the context */
+  MK_INFO_RESIDENT_ROWS = 14, /* rows of R^ kept in HBM (== rows owned unless mk_create_streamed) */
+  MK_INFO_WINDOW_ROWS = 15,  /* rows per streaming window (0: R^ is resident) */
+  MK_INFO_H2D_BYTES = 16,    /* bytes of R^ the contractions have copied host -> device since mk_create_streamed */
+  MK_INFO_RHAT_BYTES_STORED = 17 /* bytes R^ occupies as stored (padded): 8 per element, 4.25 with MK_OPT_RHAT_FORMAT = 1 */
 };
 
 /* Create a context for an nshot x nrec x nt reflection response sampled at dt (s) and dx (m), band fmin..fmax (Hz).
@@ -93,6 +106,19 @@ enum {
  * happens after the context exists, *out is still set so that mk_last_error can be read (destroy it afterwards),
  * otherwise *out is NULL. */
 int mk_create(mk_ctx** out, int nshot, int nrec, int nt, double dt, double dx, double fmin, double fmax);
+
+/* NEXT-3, second half: out-of-core R^ for a reflection response whose band-limited spectrum does not
+ * fit the device.  The paper's largest experiment exists for exactly this case ("synthesis must be done in a
+ * batched fashion ... a certain batch is transferred to each GPU"; Algorithm 2's copyH2D_shot_batch loop, PAPER.md:98-112;
+ * the 249 GB set "forces pipelining").  Rows 0 .. resident_rows-1 of R^ [nrec][nb][ld_shot] stay in HBM;
+ * the other rows live in pinned host memory owned by the context (written there directly by the ingest kernel of
+ * mk_load_R), and every contraction streams them through two windows of window_rows rows in HBM (0 = choose: 1/8 of the
+ * host rows), one cudaMemcpyAsync per row block on a copy stream, overlapped with the contraction of the previous
+ * block; passes alternate direction so that the two blocks left in the windows are not transferred again.  Everything
+ * else (operands, spectra, time fields, every other call) is as with mk_create; results equal the resident context's
+ * bit for bit.  resident_rows in [0, nrec]; resident_rows == nrec is mk_create.  Not combinable with row sharding. */
+int mk_create_streamed(mk_ctx** out, int nshot, int nrec, int nt, double dt, double dx, double fmin, double fmax,
+                       int resident_rows, int window_rows);
 
 /* Frees everything the context owns.  NULL is accepted. */
 int mk_destroy(mk_ctx* ctx);

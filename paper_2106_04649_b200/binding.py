@@ -13,10 +13,10 @@ _HERE = Path(__file__).resolve().parent
 LIB_PATH = _HERE / "libmk.so"
 
 MK_OK, MK_ERR_INVALID_ARG, MK_ERR_STATE, MK_ERR_OOM, MK_ERR_CUDA = 0, -1, -2, -3, -4
-MK_OPT_EPS_SAMPLES, MK_OPT_REGIME, MK_OPT_TIMING, MK_OPT_FFT_PATH, MK_OPT_FUSED_FINALS = 1, 2, 3, 4, 5
+MK_OPT_EPS_SAMPLES, MK_OPT_REGIME, MK_OPT_TIMING, MK_OPT_FFT_PATH, MK_OPT_FUSED_FINALS, MK_OPT_RHAT_FORMAT = 1, 2, 3, 4, 5, 6
 (MK_INFO_NB, MK_INFO_KLO, MK_INFO_KHI, MK_INFO_RHAT_BYTES, MK_INFO_RHAT_BYTES_PADDED, MK_INFO_LD_SHOT,
  MK_INFO_SHOTS_LOADED, MK_INFO_SYN_LAUNCHES, MK_INFO_SYN_MS_TOTAL, MK_INFO_SYN_RESET, MK_INFO_KERNEL_LAUNCHES,
- MK_INFO_REGIME_USED, MK_INFO_DEVICE_BYTES) = range(1, 14)
+ MK_INFO_REGIME_USED, MK_INFO_DEVICE_BYTES, MK_INFO_RESIDENT_ROWS, MK_INFO_WINDOW_ROWS, MK_INFO_H2D_BYTES, MK_INFO_RHAT_BYTES_STORED) = range(1, 18)
 REGIME_AUTO, REGIME_GEMV, REGIME_GEMM_FFMA, REGIME_GEMM_TF32X3 = 0, 1, 2, 3
 
 # every symbol include/mk.h declares
@@ -24,7 +24,7 @@ SYMBOLS = ("mk_create", "mk_destroy", "mk_set_stream", "mk_set_option", "mk_get_
            "mk_run", "mk_run_host", "mk_begin", "mk_step", "mk_finish", "mk_synthesis", "mk_image", "mk_last_error",
            "mk_version", "mk_create_sharded", "mk_operand", "mk_operand_exchanged", "mk_finish_prepare", "mk_finish_complete",
            "mk_operand_reserve", "mk_operand_attach", "mk_step_contract", "mk_step_post", "mk_ipc_export", "mk_ipc_open", "mk_ipc_close",
-           "mk_set_geometry")
+           "mk_set_geometry", "mk_create_streamed")
 MK_FIELD_GMINUS, MK_FIELD_GPLUS = 1, 2
 
 
@@ -77,6 +77,7 @@ def load():
     L.mk_synthesis.argtypes = [vp, vp, vp, ci]
     L.mk_image.argtypes = [vp, vp, vp]
     L.mk_create_sharded.argtypes = [C.POINTER(vp), ci, ci, ci, cd, cd, cd, cd, ci, ci]
+    L.mk_create_streamed.argtypes = [C.POINTER(vp), ci, ci, ci, cd, cd, cd, cd, ci, ci]
     L.mk_operand.argtypes = [vp, ci, C.POINTER(mk_operand_view)]
     L.mk_operand_exchanged.argtypes = [vp, ci]
     L.mk_finish_prepare.argtypes = [vp, ci]
@@ -131,8 +132,9 @@ def _host_ptr(a, numel=None):
 class Marchenko:
     """One context = one reflection response resident in HBM (mk_create .. mk_destroy)."""
 
-    def __init__(self, nshot, nrec, nt, dt, dx, fmin, fmax, stream=None, rows=None):
-        """rows = (row0, nrows): a row-sharded context that owns these receiver rows of R^ (mk_create_sharded)."""
+    def __init__(self, nshot, nrec, nt, dt, dx, fmin, fmax, stream=None, rows=None, streamed=None):
+        """rows = (row0, nrows): a row-sharded context that owns these receiver rows of R^ (mk_create_sharded).
+        streamed = (resident_rows, window_rows): out-of-core R^, the other rows in pinned host memory (mk_create_streamed)."""
         import torch
         if not torch.cuda.is_available():
             raise RuntimeError("libmk needs a CUDA device (there is no CPU fallback)")
@@ -140,7 +142,12 @@ class Marchenko:
         self._h = C.c_void_p()
         self.nshot, self.nrec, self.nt = nshot, nrec, nt
         self.rows = (0, nrec) if rows is None else (int(rows[0]), int(rows[1]))
-        rc = self._L.mk_create_sharded(C.byref(self._h), nshot, nrec, nt, dt, dx, fmin, fmax, self.rows[0], self.rows[1])
+        if streamed is not None:
+            if rows is not None:
+                raise ValueError("row sharding and out-of-core streaming cannot be combined")
+            rc = self._L.mk_create_streamed(C.byref(self._h), nshot, nrec, nt, dt, dx, fmin, fmax, int(streamed[0]), int(streamed[1]))
+        else:
+            rc = self._L.mk_create_sharded(C.byref(self._h), nshot, nrec, nt, dt, dx, fmin, fmax, self.rows[0], self.rows[1])
         if rc != MK_OK:
             msg = self._L.mk_last_error(self._h).decode() if self._h else "mk_create failed"
             if self._h:

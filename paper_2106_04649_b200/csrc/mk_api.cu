@@ -62,6 +62,10 @@ void release(mk_ctx* c, T** p, size_t* cap) {
 
 int resolve_regime(mk_ctx* c, int nfoc, int* regime) {
   int r = c->regime;
+  if (c->rhat_format == 1) {  // compressed R^ serves the bandwidth-bound regime only
+    if (!gemv_supported(c, nfoc) || r > 1) return set_err(c, MK_ERR_INVALID_ARG, "compressed R^ (MK_OPT_RHAT_FORMAT = 1) needs the streaming regime: nfoc <= 8");
+    r = 1;
+  }
   if (r == 0) r = gemv_supported(c, nfoc) ? 1 : (tc_supported(c) ? 3 : 2);
   if (r == 1 && !gemv_supported(c, nfoc)) return set_err(c, MK_ERR_INVALID_ARG, "GEMV regime needs nfoc <= 8 and ld*nfoc*8 <= 96 KiB");
   if (r < 1 || r > 3) return set_err(c, MK_ERR_INVALID_ARG, "unknown regime");
@@ -103,6 +107,54 @@ int prepare_operand(mk_ctx* c, int slot, int nfoc, int ldf) {
   return MK_OK;
 }
 
+// Out-of-core R^ (mk_create_streamed; "synthesis must be done in a batched fashion ... a certain batch is
+// transferred to each GPU", Algorithm 2's copyH2D_shot_batch loop PAPER.md:98-112, the 249 GB case PAPER.md:42): the rows
+// of R^ that do not fit are kept in pinned host memory and every contraction pulls them through two windows in HBM, one
+// cudaMemcpyAsync per row block on a copy stream, the contraction of block b overlapping the transfer of block b + 1.
+// Row blocks are independent (every output trace depends on one row of R^), so the result is that of the
+// resident contraction bit for bit.  Consecutive passes walk the blocks in opposite directions: the two blocks left in
+// the windows by one pass are the first two of the next and are not transferred again.
+template <typename Launch>
+int stream_host_rows(mk_ctx* c, Launch&& launch, const RowBlock& resident) {
+  const int nhost = c->nrow - c->nres, W = c->win_rows, B = (nhost + W - 1) / W;
+  // the copy stream starts behind everything enqueued so far (ingest into the host rows, earlier uses of the windows)
+  if (int rc = check_cuda(c, cudaEventRecord(c->win_main, c->stream), "cudaEventRecord")) return rc;
+  if (int rc = check_cuda(c, cudaStreamWaitEvent(c->h2d_stream, c->win_main, 0), "cudaStreamWaitEvent")) return rc;
+  const size_t row_elems = (size_t)c->nb * c->ld;
+  auto fetch = [&](int b) -> int {  // enqueue the transfer of block b unless its window already holds it
+    const int buf = b & 1;
+    if (c->win_block[buf] == b) return MK_OK;
+    const int rows = std::min(W, nhost - b * W);
+    if (c->win_block[buf] >= 0)  // the contraction that last read this window (this pass or an earlier one)
+      if (int rc = check_cuda(c, cudaStreamWaitEvent(c->h2d_stream, c->win_free[buf], 0), "cudaStreamWaitEvent")) return rc;
+    c->win_block[buf] = -1;
+    const size_t bytes = (size_t)rows * row_elems * sizeof(float2);
+    if (int rc = check_cuda(c, cudaMemcpyAsync(c->d_win[buf], c->h_Rhat + (size_t)b * W * row_elems, bytes, cudaMemcpyHostToDevice, c->h2d_stream),
+                            "H2D row block of R^"))
+      return rc;
+    if (int rc = check_cuda(c, cudaEventRecord(c->win_ready[buf], c->h2d_stream), "cudaEventRecord")) return rc;
+    c->win_block[buf] = b;
+    c->h2d_bytes += (double)bytes;
+    return MK_OK;
+  };
+  auto block_at = [&](int i) { return c->win_reverse ? B - 1 - i : i; };
+  if (int rc = fetch(block_at(0))) return rc;
+  if (B > 1)
+    if (int rc = fetch(block_at(1))) return rc;
+  if (resident.nrow > 0)  // runs while the first blocks arrive
+    if (int rc = launch(resident)) return rc;
+  for (int i = 0; i < B; ++i) {
+    const int b = block_at(i), buf = b & 1, rows = std::min(W, nhost - b * W);
+    if (int rc = check_cuda(c, cudaStreamWaitEvent(c->stream, c->win_ready[buf], 0), "cudaStreamWaitEvent")) return rc;
+    if (int rc = launch(RowBlock{c->d_win[buf], c->nres + b * W, rows})) return rc;
+    if (int rc = check_cuda(c, cudaEventRecord(c->win_free[buf], c->stream), "cudaEventRecord")) return rc;
+    if (i + 2 < B)
+      if (int rc = fetch(block_at(i + 2))) return rc;
+  }
+  c->win_reverse = !c->win_reverse;
+  return MK_OK;
+}
+
 // a2: S^ = R^ x N^ per bin, on the context's stream; optionally bracketed by events
 // peers attached for another operand layout would silently receive nothing: refuse to produce rows then
 int check_peers(mk_ctx* c, int slot) {
@@ -131,10 +183,16 @@ int contract(mk_ctx* c, int slot, float2* Shat, int nfoc, int ldf, int regime) {
     c->ev_used += 2;
     cudaEventRecord(e0, c->stream);
   }
-  int rc;
-  if (regime == 1) rc = launch_syn_gemv(c, slot ? c->d_Nhat2 : c->d_Nhat, Shat, nfoc);
-  else if (regime == 2) rc = launch_syn_gemm(c, slot ? c->d_Nhat2 : c->d_Nhat, Shat, ldf);
-  else rc = launch_syn_tc(c, slot, slot ? c->d_Nhat2 : c->d_Nhat, Shat, ldf);
+  const float2* Nhat = slot ? c->d_Nhat2 : c->d_Nhat;
+  auto launch = [&](const RowBlock& rb) -> int {
+    if (c->rhat_format == 1) return launch_syn_gemv_q16(c, Nhat, Shat, nfoc);
+    if (regime == 1) return launch_syn_gemv(c, rb, Nhat, Shat, nfoc);
+    if (regime == 2) return launch_syn_gemm(c, rb, Nhat, Shat, ldf);
+    return launch_syn_tc(c, rb, slot, Nhat, Shat, ldf);
+  };
+  int rc = MK_OK;
+  if (c->nres < c->nrow) rc = stream_host_rows(c, launch, /*before the first block arrives:*/ RowBlock{c->d_Rhat, c->r0, c->nres});
+  else rc = launch(RowBlock{c->d_Rhat, c->r0, c->nrow});
   if (timed) cudaEventRecord(e1, c->stream);
   c->last_regime = regime;  // information only (MK_INFO_REGIME_USED); the run's regime is c->run_regime
   return rc;
@@ -253,12 +311,28 @@ const char* mk_version(void) { return "libmk 0.1 (sm_100a)"; }
 
 const char* mk_last_error(mk_ctx* ctx) { return ctx ? ctx->err.c_str() : "null context"; }
 
+static int create_impl(mk_ctx** out, int nshot, int nrec, int nt, double dt, double dx, double fmin, double fmax, int row0,
+                       int nrows, int resident_rows, int window_rows);
+
 int mk_create(mk_ctx** out, int nshot, int nrec, int nt, double dt, double dx, double fmin, double fmax) {
-  return mk_create_sharded(out, nshot, nrec, nt, dt, dx, fmin, fmax, 0, nrec);
+  return create_impl(out, nshot, nrec, nt, dt, dx, fmin, fmax, 0, nrec, nrec, 0);
 }
 
 int mk_create_sharded(mk_ctx** out, int nshot, int nrec, int nt, double dt, double dx, double fmin, double fmax, int row0,
                       int nrows) {
+  return create_impl(out, nshot, nrec, nt, dt, dx, fmin, fmax, row0, nrows, nrows, 0);
+}
+
+int mk_create_streamed(mk_ctx** out, int nshot, int nrec, int nt, double dt, double dx, double fmin, double fmax,
+                       int resident_rows, int window_rows) {
+  if (!out) return MK_ERR_INVALID_ARG;
+  *out = nullptr;
+  if (resident_rows < 0 || resident_rows > nrec || window_rows < 0) return MK_ERR_INVALID_ARG;
+  return create_impl(out, nshot, nrec, nt, dt, dx, fmin, fmax, 0, nrec, resident_rows, window_rows);
+}
+
+static int create_impl(mk_ctx** out, int nshot, int nrec, int nt, double dt, double dx, double fmin, double fmax, int row0,
+                       int nrows, int resident_rows, int window_rows) {
   if (!out) return MK_ERR_INVALID_ARG;
   *out = nullptr;
   if (nshot <= 0 || nrec <= 0) return MK_ERR_INVALID_ARG;
@@ -327,11 +401,38 @@ int mk_create_sharded(mk_ctx** out, int nshot, int nrec, int nt, double dt, doub
     if (int rc = ensure(c, &c->d_tw1k, &cap, (size_t)1024, "twiddles 1k")) return rc;
     if (int rc = check_cuda(c, cudaMemcpy(c->d_tw1k, tw.data(), 1024 * sizeof(float2), cudaMemcpyHostToDevice), "twiddle upload")) return rc;
   }
-  {
+  c->nres = resident_rows;
+  if (c->nres > 0) {
     size_t cap = 0;
-    const size_t cnt = (size_t)nrows * c->nb * c->ld;  // the rows this context owns
+    const size_t cnt = (size_t)c->nres * c->nb * c->ld;  // the rows this context owns and keeps in HBM
     if (int rc = ensure(c, &c->d_Rhat, &cap, cnt, "Rhat")) return rc;
     if (int rc = check_cuda(c, cudaMemset(c->d_Rhat, 0, cnt * sizeof(float2)), "Rhat memset")) return rc;
+  }
+  if (c->nres < nrows) {  // out-of-core: the other rows in pinned, device-mapped host memory + two windows in HBM
+    const int nhost = nrows - c->nres;
+    c->win_rows = window_rows > 0 ? std::min(window_rows, nhost) : std::max(1, (nhost + 7) / 8);
+    const size_t row_elems = (size_t)c->nb * c->ld, host_bytes = (size_t)nhost * row_elems * sizeof(float2);
+    void* hp = nullptr;
+    if (cudaHostAlloc(&hp, host_bytes, cudaHostAllocMapped) != cudaSuccess) {
+      cudaGetLastError();
+      return set_err(c, MK_ERR_OOM, "cudaHostAlloc of the host-resident rows of R^ failed");
+    }
+    c->h_Rhat = static_cast<float2*>(hp);
+    std::memset(hp, 0, host_bytes);  // pad columns stay zero
+    void* dp = nullptr;
+    if (int rc = check_cuda(c, cudaHostGetDevicePointer(&dp, hp, 0), "cudaHostGetDevicePointer")) return rc;
+    c->h_Rhat_dev = static_cast<float2*>(dp);
+    const int nwin = nhost > c->win_rows ? 2 : 1;
+    for (int i = 0; i < nwin; ++i) {
+      size_t cap = 0;
+      if (int rc = ensure(c, &c->d_win[i], &cap, (size_t)c->win_rows * row_elems, "R^ window")) return rc;
+    }
+    if (int rc = check_cuda(c, cudaStreamCreateWithFlags(&c->h2d_stream, cudaStreamNonBlocking), "cudaStreamCreate")) return rc;
+    for (int i = 0; i < 2; ++i) {
+      if (int rc = check_cuda(c, cudaEventCreateWithFlags(&c->win_ready[i], cudaEventDisableTiming), "cudaEventCreate")) return rc;
+      if (int rc = check_cuda(c, cudaEventCreateWithFlags(&c->win_free[i], cudaEventDisableTiming), "cudaEventCreate")) return rc;
+    }
+    if (int rc = check_cuda(c, cudaEventCreateWithFlags(&c->win_main, cudaEventDisableTiming), "cudaEventCreate")) return rc;
   }
   return MK_OK;
 }
@@ -352,6 +453,21 @@ int mk_destroy(mk_ctx* c) {
   cudaFree(c->d_Nhat2);
   cudaFree(c->d_Shat2);
   cudaFree(c->d_stage);
+  cudaFree(c->d_Rq);
+  cudaFree(c->d_Rscale);
+  cudaFree(c->d_qstage);
+  cudaFree(c->d_win[0]);
+  cudaFree(c->d_win[1]);
+  if (c->h2d_stream) {
+    cudaStreamSynchronize(c->h2d_stream);
+    cudaStreamDestroy(c->h2d_stream);
+  }
+  for (int i = 0; i < 2; ++i) {
+    if (c->win_ready[i]) cudaEventDestroy(c->win_ready[i]);
+    if (c->win_free[i]) cudaEventDestroy(c->win_free[i]);
+  }
+  if (c->win_main) cudaEventDestroy(c->win_main);
+  if (c->h_Rhat) cudaFreeHost(c->h_Rhat);
   if (c->copy_stream) cudaStreamDestroy(c->copy_stream);
   if (c->copy_ev) cudaEventDestroy(c->copy_ev);
   for (cudaEvent_t e : c->ev) cudaEventDestroy(e);
@@ -386,6 +502,32 @@ int mk_set_option(mk_ctx* c, int key, double value) {
     case MK_OPT_FUSED_FINALS:
       c->fused_finals = value != 0.0;
       return MK_OK;
+    case MK_OPT_RHAT_FORMAT: {
+      if (value != 0.0 && value != 1.0) return set_err(c, MK_ERR_INVALID_ARG, "R^ format must be 0 (complex64) or 1 (q16 block float)");
+      if ((int)value == c->rhat_format) return MK_OK;
+      if (c->shots_loaded > 0) return set_err(c, MK_ERR_STATE, "MK_OPT_RHAT_FORMAT after mk_load_R: R^ is converted at ingest");
+      if (c->nrow != c->n || c->nres != c->nrow) return set_err(c, MK_ERR_STATE, "compressed R^ is not available on row-sharded or streamed contexts");
+      if (int rc = end_run(c, "MK_OPT_RHAT_FORMAT")) return rc;
+      const size_t cnt = (size_t)c->n * c->nb * c->ld;
+      if ((int)value == 1) {
+        size_t cap = cnt;
+        release(c, &c->d_Rhat, &cap);
+        size_t cq = 0, cs = 0;
+        if (int rc = ensure(c, &c->d_Rq, &cq, cnt, "Rhat q16")) return rc;
+        if (int rc = ensure(c, &c->d_Rscale, &cs, cnt / 16, "Rhat scales")) return rc;
+        if (int rc = check_cuda(c, cudaMemset(c->d_Rq, 0, cnt * sizeof(uint32_t)), "memset")) return rc;
+        if (int rc = check_cuda(c, cudaMemset(c->d_Rscale, 0, cnt / 16 * sizeof(float)), "memset")) return rc;
+      } else {
+        size_t cq = cnt, cs = cnt / 16, cap = 0;
+        release(c, &c->d_Rq, &cq);
+        release(c, &c->d_Rscale, &cs);
+        release(c, &c->d_qstage, &c->cap_qstage);
+        if (int rc = ensure(c, &c->d_Rhat, &cap, cnt, "Rhat")) return rc;
+        if (int rc = check_cuda(c, cudaMemset(c->d_Rhat, 0, cnt * sizeof(float2)), "memset")) return rc;
+      }
+      c->rhat_format = (int)value;
+      return MK_OK;
+    }
     case MK_OPT_FFT_PATH:
       if (value < 0 || value > 2 || value != std::floor(value)) return set_err(c, MK_ERR_INVALID_ARG, "fft path must be 0..2");
       if ((int)value == 2 && c->nt != 2048 && c->nt != 4096)
@@ -416,6 +558,7 @@ int mk_get_info(mk_ctx* c, int key, double* value) {
     case MK_INFO_KHI: *value = c->khi; return MK_OK;
     case MK_INFO_RHAT_BYTES: *value = 8.0 * c->nrow * (double)c->nb * c->ns; return MK_OK;
     case MK_INFO_RHAT_BYTES_PADDED: *value = 8.0 * c->nrow * (double)c->nb * c->ld; return MK_OK;
+    case MK_INFO_RHAT_BYTES_STORED: *value = (c->rhat_format == 1 ? 4.25 : 8.0) * c->nrow * (double)c->nb * c->ld; return MK_OK;
     case MK_INFO_LD_SHOT: *value = c->ld; return MK_OK;
     case MK_INFO_SHOTS_LOADED: *value = c->shots_loaded; return MK_OK;
     case MK_INFO_SYN_LAUNCHES: *value = (double)(c->ev_used / 2); return MK_OK;
@@ -434,6 +577,9 @@ int mk_get_info(mk_ctx* c, int key, double* value) {
     case MK_INFO_KERNEL_LAUNCHES: *value = (double)c->launches; return MK_OK;
     case MK_INFO_REGIME_USED: *value = c->last_regime; return MK_OK;
     case MK_INFO_DEVICE_BYTES: *value = (double)c->device_bytes; return MK_OK;
+    case MK_INFO_RESIDENT_ROWS: *value = c->nres; return MK_OK;
+    case MK_INFO_WINDOW_ROWS: *value = c->win_rows; return MK_OK;
+    case MK_INFO_H2D_BYTES: *value = c->h2d_bytes; return MK_OK;
     default: return set_err(c, MK_ERR_INVALID_ARG, "unknown info key");
   }
 }
@@ -442,7 +588,27 @@ int mk_load_R(mk_ctx* c, const float* d_R_time, int shot0, int nshots) {
   MK_GUARD(c);
   if (!d_R_time || shot0 < 0 || nshots <= 0 || shot0 + nshots > c->ns) return set_err(c, MK_ERR_INVALID_ARG, "mk_load_R: bad shot range");
   if (int rc = end_run(c, "mk_load_R")) return rc;  // a run in progress was started from another R^: it is over
-  if (int rc = launch_load_R(c, d_R_time, shot0, nshots)) return rc;
+  if (c->rhat_format == 1) {
+    // compressed R^: whole 16-shot blocks only (a block's scale needs all of its shots); sub-chunks of <= 64 shots go
+    // through an fp32 stage [n * nb][<= 64] and the quantiser
+    if (shot0 % 16 != 0 || (nshots % 16 != 0 && shot0 + nshots != c->ns))
+      return set_err(c, MK_ERR_INVALID_ARG, "mk_load_R with compressed R^: shot0 and nshots must be multiples of 16 (except at the last shot)");
+    const size_t rows = (size_t)c->n * c->nb;
+    if (int rc = ensure(c, &c->d_qstage, &c->cap_qstage, rows * 64, "q16 stage")) return rc;
+    for (int s0 = 0; s0 < nshots; s0 += 64) {
+      const int m = std::min(64, nshots - s0), ldc = ((m + 15) / 16) * 16;
+      if (m != ldc)
+        if (int rc = check_cuda(c, cudaMemsetAsync(c->d_qstage, 0, rows * ldc * sizeof(float2), c->stream), "memset q16 stage")) return rc;
+      RowBlock rb{c->d_qstage - (shot0 + s0), 0, c->n, ldc};  // the ingest kernel addresses columns by global shot index
+      if (int rc = launch_load_R(c, rb, d_R_time + (size_t)s0 * c->n * c->nt, shot0 + s0, m)) return rc;
+      if (int rc = launch_quantize_q16(c, c->d_qstage, ldc, shot0 + s0)) return rc;
+    }
+  } else if (c->nres > 0)
+    if (int rc = launch_load_R(c, RowBlock{c->d_Rhat, c->r0, c->nres}, d_R_time, shot0, nshots)) return rc;
+  if (c->nres < c->nrow) {  // out-of-core rows: the ingest kernel writes them to the mapped host memory directly
+    if (int rc = launch_load_R(c, RowBlock{c->h_Rhat_dev, c->nres, c->nrow - c->nres}, d_R_time, shot0, nshots)) return rc;
+    c->win_block[0] = c->win_block[1] = -1;  // what the windows hold is stale
+  }
   for (int s = shot0; s < shot0 + nshots; ++s)
     if (!c->shot_loaded[s]) {
       c->shot_loaded[s] = 1;

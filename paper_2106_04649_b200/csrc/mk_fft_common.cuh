@@ -19,7 +19,7 @@ __device__ __forceinline__ void store_operand(const OperandOut& O, int ld, int k
 
 // mk_fft_fast.cu: true when the register-resident path handles this context's nt (and it is not switched off)
 bool fast_fft_ok(const mk_ctx* c);
-int launch_load_R_fast(mk_ctx* c, const float* d_R_time, int shot0, int nshots);
+int launch_load_R_fast(mk_ctx* c, const RowBlock& rb, const float* d_R_time, int shot0, int nshots);
 int launch_fwd_fast(mk_ctx* c, const float* d_src, const OperandOut& O, int nfoc, bool conj_out, float* d_init_Tsrc);
 int launch_inv_fast(mk_ctx* c, const float2* d_spec, int nfoc, int ldf, float* d_out, float sS, const float* d_A, float sA,
                     const float* d_B, float sB);

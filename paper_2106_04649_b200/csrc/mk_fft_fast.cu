@@ -646,10 +646,13 @@ bool fast_fft_ok(const mk_ctx* c) { return (c->nt == 2048 || c->nt == 4096) && c
     return check_cuda(c, cudaGetLastError(), #KERN);                                 \
   } while (0)
 
-int launch_load_R_fast(mk_ctx* c, const float* d_R_time, int shot0, int nshots) {
+int launch_load_R_fast(mk_ctx* c, const RowBlock& rb, const float* d_R_time, int shot0, int nshots) {
   const Shape sh = shape_for(c, nshots);
-  const dim3 grid((nshots + (1 << sh.lg) - 1) >> sh.lg, c->nrow);
-  MK_FAST_LAUNCH(k_load_R_fast, grid, sh, d_R_time, c->d_Rhat, make_fast(c, 0, 0), shot0, nshots, sh.lg);
+  const dim3 grid((nshots + (1 << sh.lg) - 1) >> sh.lg, rb.nrow);
+  FastParams P = make_fast(c, 0, 0);
+  P.r0 = rb.r0;
+  if (rb.ld) P.ld = rb.ld;
+  MK_FAST_LAUNCH(k_load_R_fast, grid, sh, d_R_time, rb.Rhat, P, shot0, nshots, sh.lg);
 }
 
 int launch_fwd_fast(mk_ctx* c, const float* d_src, const OperandOut& O, int nfoc, bool conj_out, float* d_init_Tsrc) {

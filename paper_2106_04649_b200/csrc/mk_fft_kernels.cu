@@ -392,13 +392,16 @@ int launch_window(mk_ctx* c, const float* d_td, int* d_h, int ntr) {
   return check_cuda(c, cudaGetLastError(), "k_window");
 }
 
-int launch_load_R(mk_ctx* c, const float* d_R_time, int shot0, int nshots) {
-  if (fast_fft_ok(c)) return launch_load_R_fast(c, d_R_time, shot0, nshots);
+int launch_load_R(mk_ctx* c, const RowBlock& rb, const float* d_R_time, int shot0, int nshots) {
+  if (fast_fft_ok(c)) return launch_load_R_fast(c, rb, d_R_time, shot0, nshots);
   const int lg = pick_lgft(c, nshots), ST = 1 << lg;
   const size_t smem = trace_smem(c, lg);
   if (int rc = set_smem(c, k_load_R, smem)) return rc;
-  const dim3 grid((nshots + ST - 1) / ST, c->nrow);
-  k_load_R<<<grid, kThreads, smem, c->stream>>>(d_R_time, c->d_Rhat, make_params(c, 0, 0), shot0, nshots, lg);
+  const dim3 grid((nshots + ST - 1) / ST, rb.nrow);
+  FftParams P = make_params(c, 0, 0);
+  P.r0 = rb.r0;
+  if (rb.ld) P.ld = rb.ld;
+  k_load_R<<<grid, kThreads, smem, c->stream>>>(d_R_time, rb.Rhat, P, shot0, nshots, lg);
   ++c->launches;
   return check_cuda(c, cudaGetLastError(), "k_load_R");
 }

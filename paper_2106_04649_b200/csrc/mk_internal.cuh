@@ -43,6 +43,24 @@ struct mk_ctx {
   bool custom_geometry = false;
   std::vector<unsigned char> shot_loaded;
   int shots_loaded = 0;
+  // out-of-core R^ (mk_create_streamed): rows [0, nres) of R^ live in d_Rhat, rows [nres, nrow) in
+  // pinned, device-mapped host memory and pass through two windows of win_rows rows in HBM during every contraction
+  int nres = 0;                   // rows of R^ resident in HBM (== nrow unless streamed)
+  float2* h_Rhat = nullptr;       // [(nrow - nres)][nb][ld], pinned + mapped (host address)
+  float2* h_Rhat_dev = nullptr;   // the same memory as the ingest kernels address it
+  int win_rows = 0;
+  float2* d_win[2] = {nullptr, nullptr};
+  int win_block[2] = {-1, -1};    // row block each window holds (-1: none)
+  bool win_reverse = false;       // passes alternate direction, so the two blocks left in the windows are reused
+  cudaStream_t h2d_stream = nullptr;
+  cudaEvent_t win_ready[2] = {nullptr, nullptr}, win_free[2] = {nullptr, nullptr}, win_main = nullptr;
+  double h2d_bytes = 0;           // bytes of R^ copied host -> device by contractions since creation
+  // compressed R^ (MK_OPT_RHAT_FORMAT = 1, mk_syn_gemv_q16.cu): block floating point, int16 mantissas, one scale per 16 shots
+  int rhat_format = 0;
+  uint32_t* d_Rq = nullptr;       // [n][nb][ld] packed (re, im) int16
+  float* d_Rscale = nullptr;      // [n][nb][ld / 16]
+  float2* d_qstage = nullptr;     // fp32 spectra of one sub-chunk of shots on their way to the quantiser
+  size_t cap_qstage = 0;
 
   // run state
   int nfoc = 0, ldf = 0, iter = 0;
@@ -69,9 +87,10 @@ struct mk_ctx {
   float* peer_plane[2][7] = {};        // [slot][peer]: the peers' operands of the same layout
   long long peer_key[2] = {0, 0};      // operand layout the peers were attached for
   // regime 3: cached TMA descriptors (CUtensorMap is 128 bytes, 64-byte aligned), built by mk_syn_tc.cu
-  alignas(64) unsigned char tmap_A[128];
+  alignas(64) unsigned char tmap_A[3][128];  // [resident rows / window 0 / window 1]
   alignas(64) unsigned char tmap_B[2][128];  // [main / scratch operand]
-  bool tmap_A_ok = false;
+  const void* tmap_A_key[3] = {nullptr, nullptr, nullptr};
+  int tmap_A_rows[3] = {0, 0, 0};
   const void* tmap_B_key[2] = {nullptr, nullptr};
   int tmap_B_ldf[2] = {0, 0};
   void* encode_fn = nullptr;  // cuTensorMapEncodeTiled, resolved at run time through the CUDA runtime
@@ -104,6 +123,14 @@ struct FftParams {
   int r0;  // first receiver row of this context (grid row b handles receiver r0 + b; R^ is stored from row r0 on)
 };
 
+// a block of consecutive receiver rows of R^ as one launch sees it: Rhat points at row r0 (its [nrow][nb][ld] block may be
+// the resident part, a streaming window, or the mapped host part during ingest); S^ is indexed by the global receiver
+struct RowBlock {
+  float2* Rhat;
+  int r0, nrow;
+  int ld = 0;  // ingest only: elements between consecutive (receiver, bin) rows of the target (0 = the context's ld)
+};
+
 // where a forward transform stores N^ (a1, a6)
 constexpr int kMaxPeers = 7;  // other ranks of a row-sharded run whose operand receives this rank's rows directly
 
@@ -123,7 +150,7 @@ int check_cuda(mk_ctx* c, cudaError_t e, const char* what);
 
 // mk_fft_kernels.cu
 int launch_window(mk_ctx* c, const float* d_td, int* d_h, int ntr);
-int launch_load_R(mk_ctx* c, const float* d_R_time, int shot0, int nshots);
+int launch_load_R(mk_ctx* c, const RowBlock& rb, const float* d_R_time, int shot0, int nshots);
 // time [nfoc][n][nt] -> Nhat band;  conj_out: spectrum of T(src);  d_init_Tsrc: optional, receives T src
 int launch_fwd(mk_ctx* c, const float* d_src, const OperandOut& O, int nfoc, bool conj_out, float* d_init_Tsrc);
 // spectrum [n][nb][ldf] -> out[j] = sS*S[j] + sA*A[j] + sB*B[(nt-j)%nt]
@@ -134,10 +161,13 @@ int launch_post(mk_ctx* c, const OperandOut& O, int parity_even, float* d_Ni_out
 
 // mk_syn_gemv.cu / mk_syn_gemm.cu:  Shat = Rhat x Nhat per bin
 bool gemv_supported(const mk_ctx* c, int nfoc);
-int launch_syn_gemv(mk_ctx* c, const float2* d_Nhat, float2* d_Shat, int nfoc);
-int launch_syn_gemm(mk_ctx* c, const float2* d_Nhat, float2* d_Shat, int ldf);
+int launch_syn_gemv(mk_ctx* c, const RowBlock& rb, const float2* d_Nhat, float2* d_Shat, int nfoc);
+int launch_syn_gemm(mk_ctx* c, const RowBlock& rb, const float2* d_Nhat, float2* d_Shat, int ldf);
+// mk_syn_gemv_q16.cu: the streaming GEMV on block-float R^, and the quantiser of the ingest
+int launch_syn_gemv_q16(mk_ctx* c, const float2* d_Nhat, float2* d_Shat, int nfoc);
+int launch_quantize_q16(mk_ctx* c, const float2* d_stage, int ldc, int shot0);
 // mk_syn_tc.cu: tcgen05 3xTF32 path.  slot: 0 = the run's operand, 1 = the scratch operand (descriptor cache)
 bool tc_supported(const mk_ctx* c);
-int launch_syn_tc(mk_ctx* c, int slot, const float2* d_Nhat, float2* d_Shat, int ldf);
+int launch_syn_tc(mk_ctx* c, const RowBlock& rb, int slot, const float2* d_Nhat, float2* d_Shat, int ldf);
 
 }  // namespace mk

@@ -139,14 +139,14 @@ __global__ void __launch_bounds__(kThreads, 2) k_syn_gemm_ffma(const float2* __r
 
 }  // namespace
 
-int launch_syn_gemm(mk_ctx* c, const float2* d_Nhat, float2* d_Shat, int ldf) {
+int launch_syn_gemm(mk_ctx* c, const RowBlock& rb, const float2* d_Nhat, float2* d_Shat, int ldf) {
   const size_t smem = kSmemA + kSmemB;
   if (int rc = check_cuda(c, cudaFuncSetAttribute(k_syn_gemm_ffma, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem),
                           "cudaFuncSetAttribute"))
     return rc;
-  // row sharding: R^ holds the rows r0 .. r0 + nrow - 1; S^ is indexed by the global receiver
-  const dim3 grid((ldf + BN - 1) / BN, (c->nrow + BM - 1) / BM, c->nb);
-  k_syn_gemm_ffma<<<grid, kThreads, smem, c->stream>>>(c->d_Rhat, d_Nhat, d_Shat + (size_t)c->r0 * c->nb * ldf, c->nrow, c->nb, c->ld, ldf);
+  // the block holds the rows r0 .. r0 + nrow - 1 of R^; S^ is indexed by the global receiver
+  const dim3 grid((ldf + BN - 1) / BN, (rb.nrow + BM - 1) / BM, c->nb);
+  k_syn_gemm_ffma<<<grid, kThreads, smem, c->stream>>>(rb.Rhat, d_Nhat, d_Shat + (size_t)rb.r0 * c->nb * ldf, rb.nrow, c->nb, c->ld, ldf);
   ++c->launches;
   return check_cuda(c, cudaGetLastError(), "k_syn_gemm_ffma");
 }

@@ -115,14 +115,14 @@ __global__ void __launch_bounds__(kThreads, Tune<NFOC>::kMinBlocks) k_syn_gemv(c
 }
 
 template <int NFOC>
-int launch_t(mk_ctx* c, const float2* d_Nhat, float2* d_Shat) {
+int launch_t(mk_ctx* c, const RowBlock& rb, const float2* d_Nhat, float2* d_Shat) {
   const size_t smem = (size_t)c->ld * NFOC * sizeof(float2);
   auto kern = k_syn_gemv<NFOC>;
   if (int rc = check_cuda(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem), "cudaFuncSetAttribute"))
     return rc;
-  // row sharding: R^ holds the rows r0 .. r0 + nrow - 1; S^ is indexed by the global receiver
-  const dim3 grid(c->nb, (c->nrow + kRowsPerCta - 1) / kRowsPerCta);
-  kern<<<grid, kThreads, smem, c->stream>>>(c->d_Rhat, d_Nhat, d_Shat + (size_t)c->r0 * c->nb * NFOC, c->nrow, c->nb, c->ld);
+  // the block holds the rows r0 .. r0 + nrow - 1 of R^; S^ is indexed by the global receiver
+  const dim3 grid(c->nb, (rb.nrow + kRowsPerCta - 1) / kRowsPerCta);
+  kern<<<grid, kThreads, smem, c->stream>>>(rb.Rhat, d_Nhat, d_Shat + (size_t)rb.r0 * c->nb * NFOC, rb.nrow, c->nb, c->ld);
   ++c->launches;
   return check_cuda(c, cudaGetLastError(), "k_syn_gemv");
 }
@@ -133,16 +133,16 @@ bool gemv_supported(const mk_ctx* c, int nfoc) {
   return nfoc >= 1 && nfoc <= 8 && (size_t)c->ld * nfoc * sizeof(float2) <= 96 * 1024;
 }
 
-int launch_syn_gemv(mk_ctx* c, const float2* d_Nhat, float2* d_Shat, int nfoc) {
+int launch_syn_gemv(mk_ctx* c, const RowBlock& rb, const float2* d_Nhat, float2* d_Shat, int nfoc) {
   switch (nfoc) {
-    case 1: return launch_t<1>(c, d_Nhat, d_Shat);
-    case 2: return launch_t<2>(c, d_Nhat, d_Shat);
-    case 3: return launch_t<3>(c, d_Nhat, d_Shat);
-    case 4: return launch_t<4>(c, d_Nhat, d_Shat);
-    case 5: return launch_t<5>(c, d_Nhat, d_Shat);
-    case 6: return launch_t<6>(c, d_Nhat, d_Shat);
-    case 7: return launch_t<7>(c, d_Nhat, d_Shat);
-    case 8: return launch_t<8>(c, d_Nhat, d_Shat);
+    case 1: return launch_t<1>(c, rb, d_Nhat, d_Shat);
+    case 2: return launch_t<2>(c, rb, d_Nhat, d_Shat);
+    case 3: return launch_t<3>(c, rb, d_Nhat, d_Shat);
+    case 4: return launch_t<4>(c, rb, d_Nhat, d_Shat);
+    case 5: return launch_t<5>(c, rb, d_Nhat, d_Shat);
+    case 6: return launch_t<6>(c, rb, d_Nhat, d_Shat);
+    case 7: return launch_t<7>(c, rb, d_Nhat, d_Shat);
+    case 8: return launch_t<8>(c, rb, d_Nhat, d_Shat);
     default: return set_err(c, MK_ERR_INVALID_ARG, "gemv regime needs 1 <= nfoc <= 8");
   }
 }

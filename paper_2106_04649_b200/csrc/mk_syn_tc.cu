@@ -539,17 +539,20 @@ bool tc_supported(const mk_ctx* c) {
   return major == 10 && c->smem_optin >= 2 * stage_bytes(1) + kSmemExtra;
 }
 
-int launch_syn_tc(mk_ctx* c, int slot, const float2* d_Nhat, float2* d_Shat, int ldf) {
+int launch_syn_tc(mk_ctx* c, const RowBlock& rb, int slot, const float2* d_Nhat, float2* d_Shat, int ldf) {
   if (ldf % 16 != 0) return set_err(c, MK_ERR_INVALID_ARG, "the tcgen05 contraction needs ldf to be a multiple of 16");
   EncodeTiledFn enc = nullptr;
   if (int rc = get_encode(c, &enc)) return rc;
-  if (!c->tmap_A_ok) {
+  // descriptor cache: the resident rows, or one of the two streaming windows (mk_create_streamed)
+  const int ia = rb.Rhat == c->d_win[0] && c->d_win[0] ? 1 : (rb.Rhat == c->d_win[1] && c->d_win[1] ? 2 : 0);
+  if (c->tmap_A_key[ia] != rb.Rhat || c->tmap_A_rows[ia] != rb.nrow) {
     // A = R^ as fp32 [n][nb][2 ld]: dims (float of the row, bin, r); box = 16 floats x 1 bin x 128 receivers; rows r >= n read as zero
-    const cuuint64_t dims[3] = {(cuuint64_t)2 * c->ld, (cuuint64_t)c->nb, (cuuint64_t)c->nrow};  // local rows of R^
+    const cuuint64_t dims[3] = {(cuuint64_t)2 * c->ld, (cuuint64_t)c->nb, (cuuint64_t)rb.nrow};  // rows of this block
     const cuuint64_t str[2] = {(cuuint64_t)2 * c->ld * 4, (cuuint64_t)c->nb * 2 * c->ld * 4};
     const cuuint32_t box[3] = {2 * BKC, 1, BM};
-    if (int rc = encode3(c, enc, c->tmap_A, c->d_Rhat, dims, str, box, CU_TENSOR_MAP_SWIZZLE_64B, "A")) return rc;
-    c->tmap_A_ok = true;
+    if (int rc = encode3(c, enc, c->tmap_A[ia], rb.Rhat, dims, str, box, CU_TENSOR_MAP_SWIZZLE_64B, "A")) return rc;
+    c->tmap_A_key[ia] = rb.Rhat;
+    c->tmap_A_rows[ia] = rb.nrow;
   }
   const int nblk = std::min(BN / 32, (2 * ldf) / 32);
   if (c->tmap_B_key[slot] != d_Nhat || c->tmap_B_ldf[slot] != ldf) {
@@ -563,11 +566,11 @@ int launch_syn_tc(mk_ctx* c, int slot, const float2* d_Nhat, float2* d_Shat, int
     c->tmap_B_ldf[slot] = ldf;
   }
   TcParams P;
-  P.n = c->nrow;  // row sharding: local rows; S^ is offset to the first one below
+  P.n = rb.nrow;  // rows of this block; S^ is offset to the first one below
   P.nb = c->nb;
   P.ld = c->ld;
   P.ncols = 2 * ldf;
-  P.mt = (c->nrow + BM - 1) / BM;
+  P.mt = (rb.nrow + BM - 1) / BM;
   P.ntl = (P.ncols + BN - 1) / BN;
   P.s_row = (size_t)c->nb * 2 * ldf;
   P.nblk = nblk;
@@ -579,9 +582,9 @@ int launch_syn_tc(mk_ctx* c, int slot, const float2* d_Nhat, float2* d_Shat, int
     return rc;
   const int ntiles = P.nb * P.mt * P.ntl;
   const int grid = ntiles < c->num_sms ? ntiles : c->num_sms;
-  k_syn_gemm_tf32x3<<<grid, kThreads, kSmemBytes, c->stream>>>(*reinterpret_cast<const CUtensorMap*>(c->tmap_A),
+  k_syn_gemm_tf32x3<<<grid, kThreads, kSmemBytes, c->stream>>>(*reinterpret_cast<const CUtensorMap*>(c->tmap_A[ia]),
                                                                *reinterpret_cast<const CUtensorMap*>(c->tmap_B[slot]),
-                                                               reinterpret_cast<float*>(d_Shat + (size_t)c->r0 * c->nb * ldf), P);
+                                                               reinterpret_cast<float*>(d_Shat + (size_t)rb.r0 * c->nb * ldf), P);
   ++c->launches;
   return check_cuda(c, cudaGetLastError(), "k_syn_gemm_tf32x3");
 }

@@ -22,18 +22,20 @@ def problem(cfg, focs=None):
 
 
 def gpu_chain(cfg, R, Gd, td, niter=None, regime=0, keep_iters=True, host_api=False, outputs=("f1plus", "f1min", "G", "Gplus", "Gminus"),
-              fft_path=0):
-    """Runs the CUDA path through the C ABI; returns numpy arrays like oracle.marchenko does."""
+              fft_path=0, streamed=None, rhat_format=0):
+    """Runs the CUDA path through the C ABI; returns numpy arrays like oracle.marchenko does.
+    streamed = (resident_rows, window_rows): out-of-core R^ (mk_create_streamed); rhat_format: MK_OPT_RHAT_FORMAT."""
     import torch
     from paper_2106_04649_b200 import binding as B
     niter = cfg.niter if niter is None else niter
     nfoc = Gd.shape[0]
     dev = torch.device("cuda:0")
     out = {}
-    with B.Marchenko(cfg.n, cfg.n, cfg.nt, cfg.dt, cfg.dx, cfg.fmin, cfg.fmax) as mk:
+    with B.Marchenko(cfg.n, cfg.n, cfg.nt, cfg.dt, cfg.dx, cfg.fmin, cfg.fmax, streamed=streamed) as mk:
         mk.set_option(B.MK_OPT_EPS_SAMPLES, cfg.eps)
         mk.set_option(B.MK_OPT_REGIME, regime)
         mk.set_option(B.MK_OPT_FFT_PATH, fft_path)
+        mk.set_option(B.MK_OPT_RHAT_FORMAT, rhat_format)
         if host_api:
             mk.load_R_host(np.ascontiguousarray(R))
             houts = {nm: np.empty((nfoc, cfg.n, cfg.nt), np.float32) for nm in outputs + ("N_last",)}
@@ -43,6 +45,8 @@ def gpu_chain(cfg, R, Gd, td, niter=None, regime=0, keep_iters=True, host_api=Fa
             return out
         # ingest in two uneven chunks to exercise shot0 / nshots
         cut = max(1, (2 * cfg.n) // 3)
+        if rhat_format:   # compressed R^ is ingested in whole 16-shot blocks
+            cut = max(16, cut // 16 * 16) if cfg.n > 16 else cfg.n
         mk.load_R(torch.from_numpy(np.ascontiguousarray(R[:cut])).to(dev), 0)
         if cut < cfg.n:
             mk.load_R(torch.from_numpy(np.ascontiguousarray(R[cut:])).to(dev), cut)
@@ -65,6 +69,8 @@ def gpu_chain(cfg, R, Gd, td, niter=None, regime=0, keep_iters=True, host_api=Fa
         for nm, t in douts.items():
             out[nm] = t.cpu().numpy()
         out["regime_used"] = int(mk.get_info(B.MK_INFO_REGIME_USED))
+        out["h2d_bytes"] = mk.get_info(B.MK_INFO_H2D_BYTES)
+        out["rhat_bytes_padded"] = mk.get_info(B.MK_INFO_RHAT_BYTES_PADDED)
     return out
 
 

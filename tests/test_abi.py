@@ -67,6 +67,13 @@ def test_sharded_create_rejects_bad_row_ranges(lib):
         assert not h
 
 
+def test_streamed_create_rejects_bad_row_counts(lib):
+    h = C.c_void_p()
+    for resident, window in ((-1, 0), (11, 0), (4, -2)):
+        assert lib.mk_create_streamed(C.byref(h), 10, 10, 64, 0.004, 10.0, 5.0, 60.0, resident, window) == -1
+        assert not h
+
+
 def test_invalid_arguments_are_rejected_before_touching_the_device(lib):
     h = C.c_void_p()
     assert lib.mk_create(C.byref(h), 0, 11, 64, 0.004, 10.0, 5.0, 60.0) == -1       # no shots
