@@ -65,7 +65,7 @@ enum {
                              G^+ in ONE pass over R^ (2 nfoc right-hand sides, streaming GEMV); 0: one pass each */
   MK_OPT_FFT_PATH = 4,    /* transform kernels: 0 auto (default), 1 generic shared-memory passes (any nt),
                              2 register-resident path (nt = 2048 or 4096 only; MK_ERR_INVALID_ARG otherwise) */
-  MK_OPT_RHAT_FORMAT = 6  /* NEXT-4 (compressed R "accelerates data loading"): storage of
+  MK_OPT_RHAT_FORMAT = 6, /* NEXT-4 (compressed R "accelerates data loading"): storage of
                              R^.  0 (default): complex64.  1: "q16" block floating point — per (receiver, bin) row, blocks of
                              16 shots share one fp32 scale sc = max(|re|, |im|) / 32767 and every component is the int16
                              rint(v / sc): 4.25 bytes per complex element instead of 8, error <= sc / 2 per component.  The
@@ -74,6 +74,10 @@ enum {
                              (DESIGN.md section 6c), not to north_star's.  Must be set before the first mk_load_R
                              (MK_ERR_STATE afterwards); with it mk_load_R needs shot0 and nshots to be multiples of 16
                              (except at the last shot).  Not available on row-sharded or streamed contexts */
+  MK_OPT_TUNE = 7         /* measurement switches, a bit mask (default 0 = the product path; results are the same for
+                             every value, only the speed differs).  bit 0: k_post_fast does not prefetch the next tile's
+                             spectra to L2; bit 1: the split warps of the tcgen05 contraction work as two groups on
+                             alternate stages instead of all eight on every stage */
 };
 
 /* mk_get_info keys (values returned as double) */

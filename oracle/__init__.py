@@ -15,14 +15,19 @@ import numpy as np
 
 _HERE = Path(__file__).resolve().parent
 _SRC = _HERE / "marchenko_oracle.cpp"
-_LIB = _HERE / "libmarchenko_oracle.so"
+# ORACLE_SANITIZE=1 builds and loads an AddressSanitizer + UBSan copy instead (run the pins under
+# LD_PRELOAD=$(gcc -print-file-name=libasan.so) ASAN_OPTIONS=detect_leaks=0; profiles/sanitizers_r2.md)
+_SAN = os.environ.get("ORACLE_SANITIZE", "0") not in ("", "0")
+_LIB = _HERE / ("libmarchenko_oracle_san.so" if _SAN else "libmarchenko_oracle.so")
 _lib = None
 
 
 def build(force: bool = False) -> Path:
     """g++ -O2 -fopenmp; no fast-math, no FFT library, nothing but libstdc++/libgomp."""
     if force or not _LIB.exists() or _LIB.stat().st_mtime < _SRC.stat().st_mtime:
-        cmd = ["g++", "-O3", "-mavx2", "-fopenmp", "-std=c++17", "-shared", "-fPIC",
+        opt = ["-O1", "-g", "-fsanitize=address,undefined", "-fno-sanitize-recover=undefined", "-fno-omit-frame-pointer"] if _SAN \
+            else ["-O3", "-mavx2"]
+        cmd = ["g++", *opt, "-fopenmp", "-std=c++17", "-shared", "-fPIC",
                "-ffp-contract=off", str(_SRC), "-o", str(_LIB)]
         subprocess.check_call(cmd)
     return _LIB

@@ -267,27 +267,56 @@ int check_output_alias(mk_ctx* c, const mk_outputs* o, const float* acc_plus, co
   return MK_OK;
 }
 
-__global__ void k_image(const float* __restrict__ Gminus, const float* __restrict__ f1plus, float* __restrict__ image, int n, int nt,
-                        float w_mid, float w_end) {
-  // image[f] = dt * sum_r w[r] sum_j G^-[f][r][(nt-j)%nt] f1plus[f][r][j]: zero-time sample of the convolution  [PAPER.md:24, 89]
-  const int f = blockIdx.x;
+// NEXT-1 imaging: image[f] = dt * sum_r w[r] sum_j G^-[f][r][(nt-j)%nt] f1plus[f][r][j], the zero-time sample of the
+// convolution of G^- with f1plus summed over the receivers [PAPER.md:24, 89].  Neither field is band-limited (the window
+// Theta is applied in time), so the sum is taken over the time samples; it is a plain dot product of two fields and
+// HBM-bound: grid (focal point, receiver chunk), coalesced forward reads of f1plus and coalesced backward reads of G^-,
+// 8 independent loads per thread in flight, fp32 per (thread, receiver), double across receivers, fixed-order two-stage
+// reduction (bit-reproducible).
+constexpr int kImgThreads = 256;
+
+__global__ void __launch_bounds__(kImgThreads)
+k_image_partial(const float* __restrict__ Gminus, const float* __restrict__ f1plus, double* __restrict__ part, int n, int nt,
+                int rows_per_cta, float w_mid, float w_end) {
+  const int f = blockIdx.x, r0 = blockIdx.y * rows_per_cta, r1 = min(n, r0 + rows_per_cta);
+  const int tid = threadIdx.x, mask = nt - 1;
   double acc = 0.0;
-  for (int r = 0; r < n; ++r) {
+  for (int r = r0; r < r1; ++r) {
     const float* g = Gminus + ((size_t)f * n + r) * nt;
     const float* p = f1plus + ((size_t)f * n + r) * nt;
-    float part = 0.f;
-    for (int j = threadIdx.x; j < nt; j += blockDim.x) part = fmaf(g[(nt - j) & (nt - 1)], p[j], part);
+    float s[4] = {0.f, 0.f, 0.f, 0.f};
+    int j = tid;
+    for (; j + 3 * kImgThreads < nt; j += 4 * kImgThreads) {
+      float gv[4], pv[4];
+#pragma unroll
+      for (int u = 0; u < 4; ++u) {
+        pv[u] = __ldg(p + j + u * kImgThreads);
+        gv[u] = __ldg(g + ((nt - j - u * kImgThreads) & mask));
+      }
+#pragma unroll
+      for (int u = 0; u < 4; ++u) s[u] = fmaf(gv[u], pv[u], s[u]);
+    }
+    for (; j < nt; j += kImgThreads) s[0] = fmaf(__ldg(g + ((nt - j) & mask)), __ldg(p + j), s[0]);
     const float w = (n > 1 && (r == 0 || r == n - 1)) ? w_end : w_mid;
-    acc += (double)(w * part);
+    acc += (double)(w * ((s[0] + s[1]) + (s[2] + s[3])));
   }
-  __shared__ double red[256];
-  red[threadIdx.x] = acc;
+  for (int o = 16; o > 0; o >>= 1) acc += __shfl_down_sync(0xffffffffu, acc, o);
+  __shared__ double red[kImgThreads / 32];
+  if ((tid & 31) == 0) red[tid >> 5] = acc;
   __syncthreads();
-  for (int s = 128; s > 0; s >>= 1) {
-    if ((int)threadIdx.x < s) red[threadIdx.x] += red[threadIdx.x + s];
-    __syncthreads();
+  if (tid == 0) {
+    double t = 0.0;
+    for (int i = 0; i < kImgThreads / 32; ++i) t += red[i];
+    part[(size_t)f * gridDim.y + blockIdx.y] = t;
   }
-  if (threadIdx.x == 0) image[f] = (float)red[0];
+}
+
+__global__ void k_image_final(const double* __restrict__ part, float* __restrict__ image, int nfoc, int nchunk) {
+  const int f = blockIdx.x * blockDim.x + threadIdx.x;
+  if (f >= nfoc) return;
+  double t = 0.0;
+  for (int i = 0; i < nchunk; ++i) t += part[(size_t)f * nchunk + i];
+  image[f] = (float)t;
 }
 
 }  // namespace
@@ -375,6 +404,8 @@ static int create_impl(mk_ctx** out, int nshot, int nrec, int nt, double dt, dou
   c->num_sms = v;
   cudaDeviceGetAttribute(&v, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
   c->smem_optin = (size_t)v;
+  cudaDeviceGetAttribute(&v, cudaDevAttrMaxSharedMemoryPerMultiprocessor, dev);
+  c->smem_sm = (size_t)v;
   c->shot_loaded.assign(nshot, 0);
   if (int rc = upload_geometry(c, nullptr, nullptr)) return rc;  // trapezoid weights; shot s at receiver s
   // twiddles e^{-2 pi i k / nt}, evaluated in double (table constants only)
@@ -456,6 +487,7 @@ int mk_destroy(mk_ctx* c) {
   cudaFree(c->d_Rq);
   cudaFree(c->d_Rscale);
   cudaFree(c->d_qstage);
+  cudaFree(c->d_img_part);
   cudaFree(c->d_win[0]);
   cudaFree(c->d_win[1]);
   if (c->h2d_stream) {
@@ -528,6 +560,10 @@ int mk_set_option(mk_ctx* c, int key, double value) {
       c->rhat_format = (int)value;
       return MK_OK;
     }
+    case MK_OPT_TUNE:
+      if (value < 0 || value != std::floor(value) || value > 65535) return set_err(c, MK_ERR_INVALID_ARG, "tune mask out of range");
+      c->tune = (int)value;
+      return MK_OK;
     case MK_OPT_FFT_PATH:
       if (value < 0 || value > 2 || value != std::floor(value)) return set_err(c, MK_ERR_INVALID_ARG, "fft path must be 0..2");
       if ((int)value == 2 && c->nt != 2048 && c->nt != 4096)
@@ -981,7 +1017,16 @@ int mk_image(mk_ctx* c, const float* d_Gminus, float* d_image) {
   if (!d_Gminus || !d_image) return set_err(c, MK_ERR_INVALID_ARG, "mk_image: bad arguments");
   if (!c->begun) return set_err(c, MK_ERR_STATE, "mk_image before a run");
   const float wm = (float)(c->dt * c->dx), we = (float)(c->dt * c->dx * 0.5);
-  k_image<<<c->nfoc, 256, 0, c->stream>>>(d_Gminus, c->acc_plus, d_image, c->n, c->nt, wm, we);
+  // enough CTAs to fill the machine several times over, whole receivers per CTA
+  const long long traces = (long long)c->nfoc * c->n;
+  int rows_per_cta = (int)std::max<long long>(1, traces / ((long long)c->num_sms * 16));
+  rows_per_cta = std::min(rows_per_cta, c->n);
+  const int nchunk = (c->n + rows_per_cta - 1) / rows_per_cta;
+  if (int rc = ensure(c, &c->d_img_part, &c->cap_img_part, (size_t)c->nfoc * nchunk, "image partial sums")) return rc;
+  k_image_partial<<<dim3(c->nfoc, nchunk), kImgThreads, 0, c->stream>>>(d_Gminus, c->acc_plus, c->d_img_part, c->n, c->nt, rows_per_cta, wm, we);
+  ++c->launches;
+  if (int rc = check_cuda(c, cudaGetLastError(), "k_image_partial")) return rc;
+  k_image_final<<<(c->nfoc + 127) / 128, 128, 0, c->stream>>>(c->d_img_part, d_image, c->nfoc, nchunk);
   ++c->launches;
   return check_cuda(c, cudaGetLastError(), "k_image");
 }

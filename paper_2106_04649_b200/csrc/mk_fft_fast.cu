@@ -35,6 +35,16 @@ using mkfft::csub;
 
 constexpr int SUB = 32 * 33;  // float2 per 1024-point block: 32 rows of 32 + 1 pad
 
+// Accumulations into global memory (p^ += S^, f1min += w, f1plus -= w) are reductions performed by the L2: every address is
+// touched once per launch, so the result is the same round-to-nearest sum a load / add / store would give (subnormals are
+// flushed), but no thread ever waits for the old value — the pass has ONE exposed global round trip left (the S^ loads)
+__device__ __forceinline__ void red_add2(float* p, float a, float b) {
+  asm volatile("red.global.add.v2.f32 [%0], {%1, %2};" ::"l"(p), "f"(a), "f"(b) : "memory");
+}
+__device__ __forceinline__ void red_add4(float2* p, float4 v) {
+  asm volatile("red.global.add.v4.f32 [%0], {%1, %2, %3, %4};" ::"l"(p), "f"(v.x), "f"(v.y), "f"(v.z), "f"(v.w) : "memory");
+}
+
 template <int HF>
 struct Geo {
   static constexpr int M = 1024 * HF;      // complex length of a trace
@@ -251,14 +261,13 @@ __device__ __forceinline__ void spectrum_in_pairs(float2* smem, int nf, int lgFT
   const int lgP = lgFT - 1, pm = (1 << lgP) - 1;  // focal-point pairs per bin
   const int total = P.nb << lgP;
   for (int i0 = threadIdx.x; i0 < total; i0 += kBatch * nthr) {
-    float4 sv[kBatch], pv[kBatch];
+    float4 sv[kBatch];
 #pragma unroll
     for (int u = 0; u < kBatch; ++u) {
       const int idx = i0 + u * nthr;
       if (idx < total && 2 * (idx & pm) < nf) {
         const size_t o = (size_t)(idx >> lgP) * P.ldf + 2 * (idx & pm);
         sv[u] = __ldg(reinterpret_cast<const float4*>(Srow + o));
-        if (RMW) pv[u] = *reinterpret_cast<const float4*>(prow + o);
       }
     }
 #pragma unroll
@@ -267,10 +276,7 @@ __device__ __forceinline__ void spectrum_in_pairs(float2* smem, int nf, int lgFT
       if (idx >= total) continue;
       const int kk = idx >> lgP, t0 = 2 * (idx & pm), k = klo + kk;
       if (t0 >= nf) continue;
-      if (RMW) {
-        const size_t o = (size_t)kk * P.ldf + t0;
-        *reinterpret_cast<float4*>(prow + o) = make_float4(pv[u].x + sv[u].x, pv[u].y + sv[u].y, pv[u].z + sv[u].z, pv[u].w + sv[u].w);
-      }
+      if (RMW) red_add4(prow + (size_t)kk * P.ldf + t0, sv[u]);
       const float2 tw = __ldg(P.tw + k);
       const int a0 = zaddr(k), a1 = zaddr(M - k);
 #pragma unroll
@@ -305,14 +311,13 @@ __device__ __forceinline__ void spectrum_in_singles(float2* smem, int nf, int lg
   }
   const int total = P.nb << lgFT;
   for (int i0 = threadIdx.x; i0 < total; i0 += kBatch * nthr) {
-    float2 sv[kBatch], pv[kBatch], tw[kBatch];
+    float2 sv[kBatch], tw[kBatch];
 #pragma unroll
     for (int u = 0; u < kBatch; ++u) {
       const int idx = i0 + u * nthr;
       if (idx < total && (idx & fm) < nf) {
         const size_t o = (size_t)(idx >> lgFT) * P.ldf + (idx & fm);
         sv[u] = __ldg(Srow + o);
-        if (RMW) pv[u] = prow[o];
         tw[u] = __ldg(P.tw + klo + (idx >> lgFT));
       }
     }
@@ -321,7 +326,7 @@ __device__ __forceinline__ void spectrum_in_singles(float2* smem, int nf, int lg
       const int idx = i0 + u * nthr;
       if (idx >= total || (idx & fm) >= nf) continue;
       const int kk = idx >> lgFT, tl = idx & fm, k = klo + kk;
-      if (RMW) prow[(size_t)kk * P.ldf + tl] = make_float2(pv[u].x + sv[u].x, pv[u].y + sv[u].y);
+      if (RMW) red_add2(reinterpret_cast<float*>(prow + (size_t)kk * P.ldf + tl), sv[u].x, sv[u].y);
       const float xr = sv[u].x, xi = conj_in ? -sv[u].y : sv[u].y;
       const float o_r = xr * tw[u].x + xi * tw[u].y, o_i = xi * tw[u].x - xr * tw[u].y;
       float2* zt = smem + tl * TS;
@@ -353,17 +358,6 @@ __device__ __forceinline__ void store_operand2(const OperandOut& O, int ld, int 
   const float4 v = make_float4(X0.x, X0.y, X1.x, X1.y);
   *reinterpret_cast<float4*>(O.plain + idx) = v;
   for (int p = 0; p < O.npeer; ++p) *reinterpret_cast<float4*>(O.peer[p] + idx) = v;
-}
-
-// L2 prefetch of the part of a time-domain trace that meets the window (j < hh or j > nt - hh), one 128-byte line
-// per lane and step; issued at kernel start so that P3 finds the rows in L2
-template <int HF>
-__device__ __forceinline__ void prefetch_window(const float* trace, int nt, int hh, const Who& me) {
-#pragma unroll
-  for (int i = 0; i < 2; ++i) {
-    const int line = me.hf * 64 + me.t + 32 * i, j0 = 32 * line;
-    if (j0 < hh || j0 + 31 > nt - hh) asm volatile("prefetch.global.L2 [%0];" ::"l"(trace + j0));
-  }
 }
 
 // ------------------------------------------------------------------------------------------------ k_load_R_fast
@@ -497,7 +491,7 @@ template <int HF>
 __global__ void __launch_bounds__(256, 2)
 k_post_fast(const float2* __restrict__ Shat, float2* __restrict__ phat, OperandOut O, const int* __restrict__ h,
             float* __restrict__ f1plus, float* __restrict__ f1min, FastParams P, int lgFT, int parity_even,
-            float* __restrict__ Ni_out) {
+            float* __restrict__ Ni_out, int pf_dist) {
   extern __shared__ float2 smem[];
   constexpr int TS = Geo<HF>::TS;
   const int FT = 1 << lgFT, r = P.r0 + blockIdx.y, f0 = blockIdx.x * FT;
@@ -505,11 +499,17 @@ k_post_fast(const float2* __restrict__ Shat, float2* __restrict__ phat, OperandO
   const size_t rowoff = (size_t)r * P.nb * P.ldf + f0;
   const Who me = who<HF>();
   const bool pairs = lgFT >= 2 && (P.ldf & 1) == 0;
-  int hh = 0;
-  if (me.tl < nf) {  // the accumulator rows that P3 will touch: on their way to L2 while P1 / P2 run
-    hh = __ldg(h + (size_t)(f0 + me.tl) * P.n + r);
-    prefetch_window<HF>((parity_even ? f1min : f1plus) + ((size_t)(f0 + me.tl) * P.n + r) * nt, nt, hh, me);
+  if (pf_dist > 0) {
+    // The S^ rows of the tile that takes this CTA's place on the SM (pf_dist = CTAs resident at once) start their way
+    // from HBM to L2 now: its P1 then pays an L2 hit per round trip instead of a DRAM access behind everyone else's
+    const long long L = (long long)blockIdx.y * gridDim.x + blockIdx.x + pf_dist;
+    const int by = (int)(L / gridDim.x), bx = (int)(L - (long long)by * gridDim.x);
+    if (by < (int)gridDim.y) {
+      const size_t o = (size_t)(P.r0 + by) * P.nb * P.ldf + (size_t)bx * FT;
+      for (int kk = threadIdx.x; kk < P.nb; kk += blockDim.x) asm volatile("prefetch.global.L2 [%0];" ::"l"(Shat + o + (size_t)kk * P.ldf));
+    }
   }
+  const int hh = me.tl < nf ? __ldg(h + (size_t)(f0 + me.tl) * P.n + r) : 0;
   // a3: p^ += S^   [PAPER.md:79]
   if (pairs && simple_band(P, Geo<HF>::M)) {
     spectrum_in_pairs<HF, true>(smem, nf, lgFT, parity_even == 0, P, Shat + rowoff, phat + rowoff);
@@ -535,32 +535,15 @@ k_post_fast(const float2* __restrict__ Shat, float2* __restrict__ phat, OperandO
     const size_t base = ((size_t)(f0 + me.tl) * P.n + r) * nt;
     float* acc = (parity_even ? f1min : f1plus) + base;
     const float sg = parity_even ? 1.f : -1.f;
-    // a4 + a5.  Theta[j] = 1 iff j < h or j > nt - h (hard 0/1 window, strict inequality; G2).  A register row q of
-    // the warp covers samples [jlo, jlo + 64 HF - 2 HF + 1]; rows that miss the window touch no memory.
+    // a4 + a5.  Theta[j] = 1 iff j < h or j > nt - h (hard 0/1 window, strict inequality; G2).  Sample pairs that miss the
+    // window touch no memory; the others are added to the accumulator by the L2 (red_add2: nothing is loaded).
 #pragma unroll
-    for (int q0 = 0; q0 < 32; q0 += 8) {
-      float2 c[8];
-#pragma unroll
-      for (int u = 0; u < 8; ++u) {
-        const int q = q0 + u;
-        const int jlo = sample_j<HF>(q, 0, me.hf), jhi = sample_j<HF>(q, 31, me.hf) + 1;
-        c[u] = make_float2(0.f, 0.f);
-        if (jlo < hh || jhi > nt - hh) c[u] = *reinterpret_cast<const float2*>(acc + sample_j<HF>(q, me.t, me.hf));
-      }
-#pragma unroll
-      for (int u = 0; u < 8; ++u) {
-        const int q = q0 + u;
-        const int jlo = sample_j<HF>(q, 0, me.hf), jhi = sample_j<HF>(q, 31, me.hf) + 1;
-        if (jlo < hh || jhi > nt - hh) {
-          const int j = sample_j<HF>(q, me.t, me.hf);
-          const float wx = (j < hh || j > nt - hh) ? a[q].x : 0.f;
-          const float wy = (j + 1 < hh || j + 1 > nt - hh) ? a[q].y : 0.f;
-          a[q] = make_float2(wx, wy);
-          *reinterpret_cast<float2*>(acc + j) = make_float2(c[u].x + sg * wx, c[u].y + sg * wy);
-        } else {
-          a[q] = make_float2(0.f, 0.f);
-        }
-      }
+    for (int q = 0; q < 32; ++q) {
+      const int j = sample_j<HF>(q, me.t, me.hf);
+      const bool in0 = j < hh || j > nt - hh, in1 = j + 1 < hh || j + 1 > nt - hh;
+      const float wx = in0 ? a[q].x : 0.f, wy = in1 ? a[q].y : 0.f;
+      a[q] = make_float2(wx, wy);
+      if (in0 || in1) red_add2(acc + j, sg * wx, sg * wy);
     }
     if (Ni_out) {  // test / N_last copy of the new iterate
       float* ni = Ni_out + base;
@@ -671,8 +654,12 @@ int launch_inv_fast(mk_ctx* c, const float2* d_spec, int nfoc, int ldf, float* d
 int launch_post_fast(mk_ctx* c, const OperandOut& O, int parity_even, float* d_Ni_out) {
   const Shape sh = shape_for(c, c->nfoc);
   const dim3 grid((c->nfoc + (1 << sh.lg) - 1) >> sh.lg, c->nrow);
+  // CTAs resident at once (registers: 128 per thread; shared memory): the distance of the L2 prefetch of the next tile's spectra
+  const int per_sm = std::max<int>(1, std::min<size_t>(std::min<size_t>(65536 / (128 * sh.threads), (c->smem_sm ? c->smem_sm : 233472) / (sh.smem + 1024)), 32));
+  const long long total = (long long)grid.x * grid.y;
+  const int pf_dist = !(c->tune & 1) && total > (long long)per_sm * c->num_sms ? per_sm * c->num_sms : 0;
   MK_FAST_LAUNCH(k_post_fast, grid, sh, c->d_Shat, c->d_phat, O, c->d_h, c->acc_plus, c->acc_min, make_fast(c, c->nfoc, c->ldf),
-                 sh.lg, parity_even, d_Ni_out);
+                 sh.lg, parity_even, d_Ni_out, pf_dist);
 }
 
 }  // namespace mk

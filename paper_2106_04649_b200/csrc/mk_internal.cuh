@@ -95,6 +95,8 @@ struct mk_ctx {
   int tmap_B_ldf[2] = {0, 0};
   void* encode_fn = nullptr;  // cuTensorMapEncodeTiled, resolved at run time through the CUDA runtime
   float* d_stage = nullptr;  // host-call staging
+  double* d_img_part = nullptr;  // mk_image: per (focal point, receiver chunk) partial sums
+  size_t cap_img_part = 0;
   cudaStream_t copy_stream = nullptr;  // mk_run_host: device -> host copies overlapping the finals
   cudaEvent_t copy_ev = nullptr;
   size_t cap_stage = 0;
@@ -103,6 +105,8 @@ struct mk_ctx {
   long launches = 0;
   int run_regime = 0;   // regime of the run in progress / of the reserved operands: set by mk_begin and mk_operand_reserve only
   int last_regime = 0;  // regime of the last contraction launch (MK_INFO_REGIME_USED; information only)
+  size_t smem_sm = 0;   // shared memory per SM
+  int tune = 0;         // MK_OPT_TUNE: measurement switches (bit mask, include/mk.h)
   int dev = 0;          // CUDA device the context lives on (made current at the top of every entry point)
 
   // timing of contraction launches

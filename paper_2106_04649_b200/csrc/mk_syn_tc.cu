@@ -34,17 +34,21 @@
 //     pipe alone, 1.2-1.5 GHz with the round-1 kernel's 40 KB per stage into each SM).  Hence one raw operand plane
 //     instead of four (16 KB per stage), and waits that sleep in hardware.
 //
-// Kernel: persistent, one CTA per SM, warp-specialised, 512 threads = 4 warpgroups with their own register budgets
-// (setmaxnreg: the kernel starts at 128 registers per thread; control 64, split 72, read-out 184) —
+//   * the SPLIT is what paces the kernel once the feed is lean (ncu, round 2, config 2: tensor pipe 55 % active, the four
+//     split warps busy 94 % of the time at ~390 instructions per stage and warp, 1400 clk per stage against the 768 of
+//     its six MMAs).  Hence two split groups on alternate stages and a three-instruction lo part.
+//
+// Kernel: persistent, one CTA per SM, warp-specialised, 640 threads = 5 warpgroups with their own register budgets
+// (setmaxnreg: the kernel starts at 96 registers per thread; control 32, split 64, read-out 160) —
 //   warp 0      TMA producer of the A tiles [128 rows][16 floats] (SWIZZLE_64B, K-major); mbarrier full / empty ring
 //   warp 3      TMA producer of the B tiles [8 shots][<= 256 floats] (SWIZZLE_128B with 32-byte atoms, MN-major)
 //   warp 1      tcgen05.mma issuer (one thread): kind::tf32, M = 128, N <= 256, K = 8; chunk accumulators double-buffered
 //               in TMEM (2 x 256 columns); tcgen05.commit releases the stage / publishes the chunk
 //   warp 2      relay: split_bar[stage] (mbarrier) -> ready[stage] (the word the MMA warp polls)
-//   warps 4-7   split warps (128 threads).  Per stage: A -> (A_hi de-interleaved in place, A_lo), B -> (B_lo, B1_hi, B1_lo),
-//               proxy fence, arrive on split_bar[stage]
-//   warps 8-15  read-out warps.  Per chunk: tcgen05.ld of the finished accumulator (warp w owns TMEM lanes 32 (w % 4) .. +31
-//               and the column half (w - 8) / 4) -> += 128 running sums in registers, drained += 1 per warp; per tile:
+//   warps 4-11  split warps, two groups of 128 threads on alternate stages.  Per stage: A -> (A_hi de-interleaved in place,
+//               A_lo), B -> (B_lo, B1_hi, B1_lo), proxy fence, arrive on split_bar[stage]
+//   warps 12-19 read-out warps.  Per chunk: tcgen05.ld of the finished accumulator (warp w owns TMEM lanes 32 (w % 4) .. +31
+//               and the column half (w - 12) / 4) -> += 128 running sums in registers, drained += 1 per warp; per tile:
 //               128-bit global stores of S^
 #include <cuda.h>
 
@@ -60,13 +64,15 @@ constexpr int BM = 128;         // rows (receivers) per tile = TMEM lanes
 constexpr int BN = 256;         // real columns (2 per focal point) per tile = TMEM columns per accumulator
 constexpr int BKC = 8;          // shots (complex k) per stage: 64-byte rows of A
 constexpr int kMaxStages = 10;  // the ring has as many stages as fit (4 at N = 256)
-constexpr int kSplitWarps = 4, kSplitThreads = 32 * kSplitWarps;
+constexpr int kSplitWarps = 4, kSplitThreads = 32 * kSplitWarps;  // per split group
+constexpr int kSplitGroups = 2;  // the groups take alternate stages
 constexpr int kReadWarps = 8;
-constexpr int kThreads = 128 + kSplitThreads + 32 * kReadWarps;  // 16 warps = 4 warpgroups: {TMA, MMA, 2 idle}, split, read-out x 2
-// Register budget per warpgroup (setmaxnreg): launched at 128 registers per thread (4 warps per SM sub-partition); the
+constexpr int kFirstReadWarp = 4 + kSplitGroups * kSplitWarps;
+constexpr int kThreads = 128 + kSplitGroups * kSplitThreads + 32 * kReadWarps;  // 20 warps = 5 warpgroups: {TMA A, MMA, relay, TMA B}, split x 2, read-out x 2
+// Register budget per warpgroup (setmaxnreg): launched at 96 registers per thread (640 x 96 = 61440 is the CTA's pool); the
 // control and split warpgroups give most of their share back and the read-out warps, who hold 128 running sums each,
-// take it: 128 x 64 + 128 x 72 + 256 x 184 = 64512 <= 65536.
-constexpr int kRegsControl = 64, kRegsSplit = 72, kRegsRead = 184;
+// take it: 128 x 32 + 256 x 64 + 256 x 160 = 61440.
+constexpr int kRegsControl = 32, kRegsSplit = 64, kRegsRead = 160;
 constexpr int kChunk = 4;       // stages per accumulation chunk (24 MMA steps)
 constexpr uint32_t A_BYTES = BM * 2 * BKC * 4;  // 8 KB: one A tile
 constexpr uint32_t BLK_BYTES = BKC * 32 * 4;    // 1 KB: one 32-column block of one B region (8 rows of 128 B)
@@ -184,14 +190,12 @@ __device__ __forceinline__ void umma_commit(uint64_t* bar) {  // arrives on `bar
   asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(smem_u32(bar)) : "memory");
 }
 
-__device__ __forceinline__ void tmem_ld16(uint32_t taddr, uint32_t* v) {
-  asm volatile(
-      "tcgen05.ld.sync.aligned.32x32b.x16.b32 "
-      "{%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15}, [%16];"
-      : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]), "=r"(v[8]), "=r"(v[9]),
-        "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15])
-      : "r"(taddr)
-      : "memory");
+// eight columns at a time: the read-out warps hold 128 running sums each and have 160 registers
+__device__ __forceinline__ void tmem_ld8(uint32_t taddr, uint32_t* v) {
+  asm volatile("tcgen05.ld.sync.aligned.32x32b.x8.b32 {%0, %1, %2, %3, %4, %5, %6, %7}, [%8];"
+               : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7])
+               : "r"(taddr)
+               : "memory");
 }
 
 // shared-memory matrix descriptor (tcgen05): start >> 4 | LBO >> 4 << 16 | SBO >> 4 << 32 | version 1 << 46 | layout << 61
@@ -218,15 +222,15 @@ __device__ __forceinline__ void sts128(uint32_t addr, float4 v) {
   asm volatile("st.shared.v4.f32 [%0], {%1, %2, %3, %4};" ::"r"(addr), "f"(v.x), "f"(v.y), "f"(v.z), "f"(v.w) : "memory");
 }
 
-// lo = x - hi is exact in fp32 and can have 13 significant bits; the tensor core would TRUNCATE it to the 11 of tf32, a bias
-// of ~2^-23 |x| with the sign of x on every operand, i.e. a coherent relative shrink of every product that adds up over
-// the Neumann iterations (measured: 8e-6 after 8 iterations against 1e-6 for the FFMA kernel).  Rounding lo to nearest
-// tf32 here makes the tensor core's truncation a no-op and the remaining error unbiased.
+// lo = x - hi is exact in fp32 and can have 13 significant bits; the tensor core TRUNCATES it to the 11 of tf32 (it does not
+// use the low 13 bits of the word), a bias of ~2^-23 |x| with the sign of x on every operand, i.e. a coherent relative
+// shrink of every product that adds up over the Neumann iterations (measured: 8e-6 after 8 iterations against 1e-6 for
+// the FFMA kernel).  Adding half a tf32 ulp to the magnitude here (one integer add on the sign-magnitude word) turns the
+// tensor core's truncation into round-to-nearest and the remaining error is unbiased.  Three instructions per element:
+// the split warps' instruction stream is what paces the kernel (ncu, round 2: they were busy 94 % of the time).
 __device__ __forceinline__ float lo_part(float x) {
   const float l = x - __uint_as_float(__float_as_uint(x) & 0xffffe000u);
-  uint32_t r;
-  asm("cvt.rna.tf32.f32 %0, %1;" : "=r"(r) : "f"(l));
-  return __uint_as_float(r);
+  return __uint_as_float(__float_as_uint(l) + 0x1000u);
 }
 __device__ __forceinline__ float4 lo4(float4 v) { return make_float4(lo_part(v.x), lo_part(v.y), lo_part(v.z), lo_part(v.w)); }
 
@@ -238,6 +242,7 @@ struct TcParams {
   size_t s_row;         // floats between consecutive receivers of S^: nb * 2 ldf
 };
 
+template <int JOINT>  // split warps: 0 = two groups on alternate stages, 1 = all eight warps on every stage
 __global__ void __launch_bounds__(kThreads, 1)
 k_syn_gemm_tf32x3(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB, float* __restrict__ Shat,
                   TcParams P) {
@@ -264,7 +269,7 @@ k_syn_gemm_tf32x3(const __grid_constant__ CUtensorMap tmA, const __grid_constant
     for (int s = 0; s < STAGES; ++s) {
       mbar_init(full + s, 2);  // the A producer and the B producer, each with its own byte count
       mbar_init(empty + s, 1);
-      mbar_init(split_bar + s, kSplitWarps);
+      mbar_init(split_bar + s, JOINT ? kSplitGroups * kSplitWarps : kSplitWarps);  // the warps that take the stage
       ready[s] = 0;
     }
     mbar_init(acc_full + 0, 1);
@@ -396,67 +401,72 @@ k_syn_gemm_tf32x3(const __grid_constant__ CUtensorMap tmA, const __grid_constant
         }
       }
     }
-  } else if (warp < 8) {
+  } else if (warp < kFirstReadWarp) {
     // ------------------------------------------------------------------------------------ split warps
+    // Two groups of four warps; group g takes the stages g, g + 2, g + 4, ... of this CTA's stage sequence, so the
+    // latency chain of one stage (wait, LDS -> ALU -> STS, proxy fence, arrive) overlaps the other group's
     asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(kRegsSplit));
-    const int wt = threadIdx.x - 128;  // 0 .. 127
+    const int grp = JOINT ? 0 : (warp - 4) / kSplitWarps;
+    constexpr int NT = JOINT ? kSplitGroups * kSplitThreads : kSplitThreads;  // threads that share a stage
+    constexpr int STEP = JOINT ? 1 : kSplitGroups;
+    const int wt = threadIdx.x - 128 - grp * kSplitThreads;  // 0 .. NT - 1
     const uint32_t smem_base = smem_u32(smem);
-    // A work items of this thread: 32-byte pairs p = wt and wt + 128 of the tile; pair p = row p / 2, K step p % 2.
+    // A work items of this thread: 32-byte pairs p = wt (and wt + 128) of the tile; pair p = row p / 2, K step p % 2.
     // SWIZZLE_64B: the 16-byte chunk c of row r sits at chunk position c ^ ((r >> 1) & 3).
-    uint32_t a_off[2][2];
+    constexpr int NA = 256 / NT;
+    uint32_t a_off[NA][2];
 #pragma unroll
-    for (int k = 0; k < 2; ++k) {
-      const int pr = wt + k * kSplitThreads, ar = pr >> 1, ap = pr & 1, ax = (ar >> 1) & 3;
+    for (int k = 0; k < NA; ++k) {
+      const int pr = wt + k * NT, ar = pr >> 1, ap = pr & 1, ax = (ar >> 1) & 3;
       a_off[k][0] = (uint32_t)ar * 64 + (uint32_t)(((2 * ap) ^ ax) << 4);
       a_off[k][1] = (uint32_t)ar * 64 + (uint32_t)(((2 * ap + 1) ^ ax) << 4);
     }
-    int s = 0;
-    uint32_t ph = 0;
-    for (int t = blockIdx.x; t < ntiles; t += gridDim.x) {
-      for (int kb = 0; kb < KB; ++kb) {
-        mbar_wait(full + s, ph);
-        const uint32_t st = smem_base + (uint32_t)s * STAGE_BYTES;
-        {  // A: (re0 im0 re1 im1 | re2 im2 re3 im3) -> hi (re0 re1 re2 re3 | im0 im1 im2 im3) in place, lo beside it
-          float4 c[2][2];
+    const int my_tiles = blockIdx.x < ntiles ? (ntiles - blockIdx.x + gridDim.x - 1) / gridDim.x : 0;
+    const long long total = (long long)my_tiles * KB;  // stages this CTA runs through
+    int s = grp % STAGES;
+    uint32_t ph = (grp / STAGES) & 1;
+    for (long long it = grp; it < total; it += STEP) {
+      mbar_wait(full + s, ph);
+      const uint32_t st = smem_base + (uint32_t)s * STAGE_BYTES, b0 = st + 2 * A_BYTES;
+      {  // A: (re0 im0 re1 im1 | re2 im2 re3 im3) -> hi (re0 re1 re2 re3 | im0 im1 im2 im3) in place, lo beside it
+        float4 c[NA][2];
 #pragma unroll
-          for (int k = 0; k < 2; ++k) {
-            c[k][0] = lds128(st + a_off[k][0]);
-            c[k][1] = lds128(st + a_off[k][1]);
-          }
-#pragma unroll
-          for (int k = 0; k < 2; ++k) {
-            const float4 re = make_float4(c[k][0].x, c[k][0].z, c[k][1].x, c[k][1].z), im = make_float4(c[k][0].y, c[k][0].w, c[k][1].y, c[k][1].w);
-            sts128(st + a_off[k][0], re);
-            sts128(st + a_off[k][1], im);
-            sts128(st + A_BYTES + a_off[k][0], lo4(re));
-            sts128(st + A_BYTES + a_off[k][1], lo4(im));
-          }
+        for (int k = 0; k < NA; ++k) {
+          c[k][0] = lds128(st + a_off[k][0]);
+          c[k][1] = lds128(st + a_off[k][1]);
         }
-        {  // B: elementwise on the swizzled tile — lo of B0, and B1 = i B0 (every float4 holds two (re, im) pairs)
-          const uint32_t b0 = st + 2 * A_BYTES;
+#pragma unroll
+        for (int k = 0; k < NA; ++k) {
+          const float4 re = make_float4(c[k][0].x, c[k][0].z, c[k][1].x, c[k][1].z), im = make_float4(c[k][0].y, c[k][0].w, c[k][1].y, c[k][1].w);
+          sts128(st + a_off[k][0], re);
+          sts128(st + a_off[k][1], im);
+          sts128(st + A_BYTES + a_off[k][0], lo4(re));
+          sts128(st + A_BYTES + a_off[k][1], lo4(im));
+        }
+      }
+      // B: elementwise on the swizzled tile — lo of B0, and B1 = i B0 (every float4 holds two (re, im) pairs)
 #pragma unroll 2
-          for (uint32_t q = 16 * (uint32_t)wt; q < REG; q += 16 * kSplitThreads) {
-            const float4 v = lds128(b0 + q);
-            const float4 l = lo4(v);
-            sts128(b0 + q + REG, l);
-            sts128(b0 + q + 2 * REG, make_float4(-v.y, v.x, -v.w, v.z));
-            sts128(b0 + q + 3 * REG, make_float4(-l.y, l.x, -l.w, l.z));
-          }
-        }
-        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");  // generic-proxy writes -> visible to the tensor core
-        __syncwarp();
-        if (lane == 0) mbar_arrive(split_bar + s);
-        if (++s == STAGES) {
-          s = 0;
-          ph ^= 1;
-        }
+      for (uint32_t q = 16 * (uint32_t)wt; q < REG; q += 16 * NT) {
+        const float4 v = lds128(b0 + q);
+        const float4 l = lo4(v);
+        sts128(b0 + q + REG, l);
+        sts128(b0 + q + 2 * REG, make_float4(-v.y, v.x, -v.w, v.z));
+        sts128(b0 + q + 3 * REG, make_float4(-l.y, l.x, -l.w, l.z));
+      }
+      asm volatile("fence.proxy.async.shared::cta;" ::: "memory");  // generic-proxy writes -> visible to the tensor core
+      __syncwarp();
+      if (lane == 0) mbar_arrive(split_bar + s);
+      s += STEP;
+      if (s >= STAGES) {  // STAGES >= 2: at most one wrap
+        s -= STAGES;
+        ph ^= 1;
       }
     }
   } else {
     // ------------------------------------------------------------------------------------ read-out warps: chunk sums in registers
     asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(kRegsRead));
     const int quad = warp & 3;         // TMEM lanes 32 quad .. 32 quad + 31 are the ones this warp may read
-    const int half = (warp - 8) >> 2;  // columns 128 half .. 128 half + 127 of the tile
+    const int half = (warp - kFirstReadWarp) >> 2;  // columns 128 half .. 128 half + 127 of the tile
     uint32_t g = 0;
     for (int t = blockIdx.x; t < ntiles; t += gridDim.x) {
       const int kk = t / per_bin, rem = t - kk * per_bin, mi = rem / P.ntl, ni = rem - mi * P.ntl;
@@ -470,13 +480,13 @@ k_syn_gemm_tf32x3(const __grid_constant__ CUtensorMap tmA, const __grid_constant
         tc_fence_after();
         const uint32_t ta = tmem_base + ((uint32_t)(quad * 32) << 16) + (uint32_t)(b * BN + half * (BN / 2));
 #pragma unroll
-        for (int c = 0; c < BN / 32; ++c) {
-          if (c * 16 < cols) {  // warp-uniform; columns past the MMA's N hold stale data
-            uint32_t v[16];
-            tmem_ld16(ta + (uint32_t)(c * 16), v);
+        for (int c = 0; c < BN / 16; ++c) {
+          if (c * 8 < cols) {  // warp-uniform; columns past the MMA's N hold stale data
+            uint32_t v[8];
+            tmem_ld8(ta + (uint32_t)(c * 8), v);
             asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
 #pragma unroll
-            for (int q = 0; q < 16; ++q) sum[c * 16 + q] += __uint_as_float(v[q]);
+            for (int q = 0; q < 8; ++q) sum[c * 8 + q] += __uint_as_float(v[q]);
           }
         }
         tc_fence_before();
@@ -577,14 +587,20 @@ int launch_syn_tc(mk_ctx* c, const RowBlock& rb, int slot, const float2* d_Nhat,
   P.stages = (int)std::min<size_t>(kMaxStages, (c->smem_optin - kSmemExtra) / stage_bytes(nblk));
   if (P.stages < 2) return set_err(c, MK_ERR_INVALID_ARG, "not enough shared memory for the tcgen05 contraction");
   const size_t kSmemBytes = (size_t)P.stages * stage_bytes(nblk) + kSmemExtra;
-  if (int rc = check_cuda(c, cudaFuncSetAttribute(k_syn_gemm_tf32x3, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemBytes),
-                          "cudaFuncSetAttribute"))
-    return rc;
   const int ntiles = P.nb * P.mt * P.ntl;
   const int grid = ntiles < c->num_sms ? ntiles : c->num_sms;
-  k_syn_gemm_tf32x3<<<grid, kThreads, kSmemBytes, c->stream>>>(*reinterpret_cast<const CUtensorMap*>(c->tmap_A[ia]),
-                                                               *reinterpret_cast<const CUtensorMap*>(c->tmap_B[slot]),
-                                                               reinterpret_cast<float*>(d_Shat + (size_t)rb.r0 * c->nb * ldf), P);
+  float* S0 = reinterpret_cast<float*>(d_Shat + (size_t)rb.r0 * c->nb * ldf);
+  const CUtensorMap& mA = *reinterpret_cast<const CUtensorMap*>(c->tmap_A[ia]);
+  const CUtensorMap& mB = *reinterpret_cast<const CUtensorMap*>(c->tmap_B[slot]);
+  if (c->tune & 2) {
+    if (int rc = check_cuda(c, cudaFuncSetAttribute(k_syn_gemm_tf32x3<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemBytes), "cudaFuncSetAttribute"))
+      return rc;
+    k_syn_gemm_tf32x3<0><<<grid, kThreads, kSmemBytes, c->stream>>>(mA, mB, S0, P);
+  } else {
+    if (int rc = check_cuda(c, cudaFuncSetAttribute(k_syn_gemm_tf32x3<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemBytes), "cudaFuncSetAttribute"))
+      return rc;
+    k_syn_gemm_tf32x3<1><<<grid, kThreads, kSmemBytes, c->stream>>>(mA, mB, S0, P);
+  }
   ++c->launches;
   return check_cuda(c, cudaGetLastError(), "k_syn_gemm_tf32x3");
 }
