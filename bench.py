@@ -424,6 +424,8 @@ def run_ours(args):
     mk = B.Marchenko(cfg.n, cfg.n, cfg.nt, cfg.dt, cfg.dx, cfg.fmin, cfg.fmax, rows=(my_rows.start, len(my_rows)))
     mk.set_option(B.MK_OPT_EPS_SAMPLES, cfg.eps)
     mk.set_option(B.MK_OPT_REGIME, args.regime)
+    if args.tune:
+        mk.set_option(B.MK_OPT_TUNE, args.tune)
     ipc_ptrs = []
     if args.parallel == "rows_fused":
         if world > 1:
@@ -588,6 +590,7 @@ def main():
                     help="N > 1: independent replicas (default, weak scaling) or receiver-row sharding with one all-gather of the "
                          "operand rows per synthesis (strong scaling; SURVEY.md section 8(e) / NEXT-3); rows_fused: the same with the "
                          "all-gather fused into the producing kernels as peer stores over CUDA IPC mappings (two barriers per synthesis)")
+    ap.add_argument("--tune", type=int, default=0, help="MK_OPT_TUNE bit mask (measurement switches of the kernels; include/mk.h)")
     ap.add_argument("--e2e-steps", type=int, default=50)
     ap.add_argument("--cpu-budget", type=float, default=15.0, help="seconds of oracle work for cpu_baseline")
     ap.add_argument("--no-cpu-baseline", action="store_true")

@@ -74,10 +74,12 @@ enum {
                              (DESIGN.md section 6c), not to north_star's.  Must be set before the first mk_load_R
                              (MK_ERR_STATE afterwards); with it mk_load_R needs shot0 and nshots to be multiples of 16
                              (except at the last shot).  Not available on row-sharded or streamed contexts */
-  MK_OPT_TUNE = 7         /* measurement switches, a bit mask (default 0 = the product path; results are the same for
-                             every value, only the speed differs).  bit 0: k_post_fast does not prefetch the next tile's
-                             spectra to L2; bit 1: the split warps of the tcgen05 contraction work as two groups on
-                             alternate stages instead of all eight on every stage */
+  MK_OPT_TUNE = 7         /* measurement switches, a bit mask (default 0 = the product path).  bit 0: k_post_fast does not
+                             prefetch the next tile's spectra to L2 (same results).  Bits 2..5 leave out one part of the
+                             tcgen05 contraction to find what bounds it; the RESULTS ARE WRONG with any of them: 4 = the
+                             read-out warps do not read tensor memory, 8 = no MMA is issued, 16 = the split warps skip the
+                             B planes, 32 = the split warps do nothing, 64 = no TMA load is issued,
+                             128 = no A tile is loaded, 256 = no B tile is loaded */
 };
 
 /* mk_get_info keys (values returned as double) */

@@ -1,6 +1,7 @@
 """Builds libmk.so (the C-ABI CUDA library) in-tree with nvcc for sm_100a.  `python -m paper_2106_04649_b200.build`."""
 from __future__ import annotations
 
+import os
 import subprocess
 import sys
 from concurrent.futures import ThreadPoolExecutor
@@ -35,7 +36,7 @@ def build(force: bool = False, verbose: bool = False) -> Path:
         src, obj = pair
         if not force and not _stale(obj, [src] + headers):
             return ""
-        cmd = ["nvcc", *ARCH, *FLAGS, "-c", str(src), "-o", str(obj)]
+        cmd = ["nvcc", *ARCH, *FLAGS, *os.environ.get("MK_NVCC_FLAGS", "").split(), "-c", str(src), "-o", str(obj)]
         r = subprocess.run(cmd, capture_output=True, text=True)
         (OBJ / (src.stem + ".ptxas.log")).write_text(r.stderr)
         if r.returncode != 0:

@@ -539,11 +539,17 @@ k_post_fast(const float2* __restrict__ Shat, float2* __restrict__ phat, OperandO
     // window touch no memory; the others are added to the accumulator by the L2 (red_add2: nothing is loaded).
 #pragma unroll
     for (int q = 0; q < 32; ++q) {
-      const int j = sample_j<HF>(q, me.t, me.hf);
-      const bool in0 = j < hh || j > nt - hh, in1 = j + 1 < hh || j + 1 > nt - hh;
-      const float wx = in0 ? a[q].x : 0.f, wy = in1 ? a[q].y : 0.f;
-      a[q] = make_float2(wx, wy);
-      if (in0 || in1) red_add2(acc + j, sg * wx, sg * wy);
+      // register row q of the warp covers the samples [jlo, jhi]: a row that misses the window is cleared without a look
+      const int jlo = sample_j<HF>(q, 0, me.hf), jhi = sample_j<HF>(q, 31, me.hf) + 1;
+      if (jlo < hh || jhi > nt - hh) {  // warp-uniform
+        const int j = sample_j<HF>(q, me.t, me.hf);
+        const bool in0 = j < hh || j > nt - hh, in1 = j + 1 < hh || j + 1 > nt - hh;
+        const float wx = in0 ? a[q].x : 0.f, wy = in1 ? a[q].y : 0.f;
+        a[q] = make_float2(wx, wy);
+        if (in0 || in1) red_add2(acc + j, sg * wx, sg * wy);
+      } else {
+        a[q] = make_float2(0.f, 0.f);
+      }
     }
     if (Ni_out) {  // test / N_last copy of the new iterate
       float* ni = Ni_out + base;

@@ -6,49 +6,54 @@
 //   B0[s] = the row N^[k][s][.] read as interleaved floats (re, im)  — the operand exactly as the transform kernels
 //           store it for every regime, [nb][ld][ldf] complex64 (TMA, no copy, no second plane in HBM);
 //   B1[s] = i N^[k][s][.] = (-im, re): the same row rotated by 90 degrees, made in shared memory;
-//   A     = the row R^[r][k][.] exactly as it sits in HBM (K-major, TMA), its (re, im) pairs de-interleaved in shared
-//           memory four shots at a time, so that one K = 8 step of the tensor core reads (re s..s+3 | im s..s+3) of A
+//   A     = the row R^[r][k][.] exactly as it sits in HBM (K-major, TMA lands it in shared memory); the split warps
+//           read it ONCE, de-interleave its (re, im) pairs four shots at a time in registers and store it into TENSOR
+//           MEMORY (tcgen05.st): the MMAs take A from TMEM, so that one K = 8 step reads (re s..s+3 | im s..s+3) of A
 //           against (B0 rows s..s+3 | B1 rows s..s+3) of B;
 //   C'    = S^[r][k][.] as interleaved floats — the layout k_post reads.
 // 3xTF32: x = hi + lo with hi = the tf32 the tensor core sees when it reads the fp32 word (the low 13 mantissa bits are
 // not used) and lo = x - hi (exact in fp32, then rounded to nearest tf32); every K step issues  A_lo*B_hi + A_hi*B_lo + A_hi*B_hi  into one fp32
 // accumulator in TMEM.  The dropped term A_lo*B_lo is O(2^-21) relative.  Only raw fp32 words cross HBM and L2: the lo
-// parts, the rotation and the de-interleave are computed per stage by the worker warps from the tile TMA delivered.
+// parts, the rotation and the de-interleave are computed per stage by the split warps from the tile TMA delivered.
 //
 // Accumulation.  The tensor core adds into its fp32 accumulator with TRUNCATION, not round-to-nearest: measured on B200
 // with one accumulator over the whole K extent the relative error of S^ grows linearly with the number of MMA steps
 // (about 2e-8 per step: 6.8e-7 at n = 32, 2.9e-5 at n = 2048, against 1.2e-6 for the FFMA kernel), which breaks the
 // 2e-5 per-iteration tolerance from n ~ 600 on.  So K is cut into CHUNKS of kChunk stages (24 MMA steps): every chunk
-// starts a fresh TMEM accumulator, and the worker warps add the finished chunk into fp32 registers (round-to-nearest)
+// starts a fresh TMEM accumulator, and the read-out warps add the finished chunk into fp32 registers (round-to-nearest)
 // while the tensor core works on the next chunk in the other TMEM buffer.  The error is then that of one chunk
 // (~5e-7), independent of n.
 //
 // What shaped it (measured on B200, round 2):
-//   * tcgen05.mma kind::tf32 M = 128, N = 256, K = 8 from shared-memory operands runs at exactly 128 clk per instruction
-//     with nothing else going on, and is not slowed (in cycles) by LDS / STS traffic or proxy fences of other warps;
+//   * tcgen05.mma kind::tf32 M = 128, N = 256, K = 8 runs at 128 clk per instruction with nothing else going on;
 //   * an mbarrier wait in the ISSUING thread is not free: the thread runs only ~4 MMAs ahead of the pipe and a try_wait
 //     costs 70-90 clk that the pipe then idles (2 waits per 6 MMAs: 128 -> 152 clk per MMA).  The issuing thread
 //     therefore never touches an mbarrier: readiness reaches it through plain shared-memory counters (release /
 //     acquire) that it polls with ld.shared between bursts of MMAs;
-//   * the chip is POWER-bound: every byte through L2 and every spinning warp costs SM clock (1.75 GHz with the tensor
-//     pipe alone, 1.2-1.5 GHz with the round-1 kernel's 40 KB per stage into each SM).  Hence one raw operand plane
-//     instead of four (16 KB per stage), and waits that sleep in hardware.
+//   * SHARED-MEMORY BANDWIDTH is what paced the version with both operands in shared memory (ncu, round 2, config 2: tensor
+//     pipe 55-58 % active, 1380 clk per stage against the 768 of its six MMAs; per stage the MMAs read 6 x (4 KB of A +
+//     8 KB of B) = 576 wavefronts of 128 B, the split warps moved 56 KB = 457 wavefronts, TMA wrote 128: 1161 against
+//     768 clk, and no instruction had an excess wavefront).  With A in tensor memory the MMAs read only B from shared
+//     memory, the split warps read A once and write it to TMEM, and A_hi / A_lo occupy no shared memory at all:
+//     per stage (N = 192) 288 + 112 (TMA) + 64 (A read) + 192 (B split) = 656 wavefronts against 576 clk of MMAs;
+//   * the chip is POWER-bound under this kernel: every byte through L2 and every spinning warp costs SM clock.  Hence one
+//     raw operand plane instead of four, and waits that sleep in hardware.
 //
-//   * the SPLIT is what paces the kernel once the feed is lean (ncu, round 2, config 2: tensor pipe 55 % active, the four
-//     split warps busy 94 % of the time at ~390 instructions per stage and warp, 1400 clk per stage against the 768 of
-//     its six MMAs).  Hence two split groups on alternate stages and a three-instruction lo part.
+// Tensor memory (512 columns): two chunk accumulators of BN = 192 columns, and a ring of four A slots of 32 columns
+// (per K step 8 columns of A_hi and 8 of A_lo; lane = receiver row of the tile).
 //
 // Kernel: persistent, one CTA per SM, warp-specialised, 640 threads = 5 warpgroups with their own register budgets
-// (setmaxnreg: the kernel starts at 96 registers per thread; control 32, split 64, read-out 160) —
+// (setmaxnreg: the kernel starts at 96 registers per thread; control 32, split 72, read-out 136) —
 //   warp 0      TMA producer of the A tiles [128 rows][16 floats] (SWIZZLE_64B, K-major); mbarrier full / empty ring
-//   warp 3      TMA producer of the B tiles [8 shots][<= 256 floats] (SWIZZLE_128B with 32-byte atoms, MN-major)
-//   warp 1      tcgen05.mma issuer (one thread): kind::tf32, M = 128, N <= 256, K = 8; chunk accumulators double-buffered
-//               in TMEM (2 x 256 columns); tcgen05.commit releases the stage / publishes the chunk
+//   warp 3      TMA producer of the B tiles [8 shots][<= 192 floats] (SWIZZLE_128B with 32-byte atoms, MN-major)
+//   warp 1      tcgen05.mma issuer (one thread): kind::tf32, M = 128, N <= 192, K = 8, A from TMEM, B from shared memory;
+//               tcgen05.commit releases the stage / publishes the chunk
 //   warp 2      relay: split_bar[stage] (mbarrier) -> ready[stage] (the word the MMA warp polls)
-//   warps 4-11  split warps, two groups of 128 threads on alternate stages.  Per stage: A -> (A_hi de-interleaved in place,
-//               A_lo), B -> (B_lo, B1_hi, B1_lo), proxy fence, arrive on split_bar[stage]
+//   warps 4-11  split warps, all eight on every stage.  A: thread = (row of the tile, K step): two 128-bit loads, lo parts,
+//               one tcgen05.st of 16 columns.  B -> (B_lo, B1_hi, B1_lo) in shared memory.  tcgen05.wait::st, proxy fence,
+//               arrive on split_bar[stage]
 //   warps 12-19 read-out warps.  Per chunk: tcgen05.ld of the finished accumulator (warp w owns TMEM lanes 32 (w % 4) .. +31
-//               and the column half (w - 12) / 4) -> += 128 running sums in registers, drained += 1 per warp; per tile:
+//               and the column half (w - 12) / 4) -> += 96 running sums in registers, drained += 1 per warp; per tile:
 //               128-bit global stores of S^
 #include <cuda.h>
 
@@ -61,27 +66,36 @@ namespace mk {
 namespace {
 
 constexpr int BM = 128;         // rows (receivers) per tile = TMEM lanes
-constexpr int BN = 256;         // real columns (2 per focal point) per tile = TMEM columns per accumulator
+constexpr int BN = 192;         // real columns (2 per focal point) per tile = TMEM columns per accumulator
 constexpr int BKC = 8;          // shots (complex k) per stage: 64-byte rows of A
-constexpr int kMaxStages = 10;  // the ring has as many stages as fit (4 at N = 256)
+constexpr int kMaxStages = 7;   // shared-memory ring: as many stages as fit (7 at N = 192)
+constexpr int kTmemSlots = 4;   // ring of A slots in tensor memory: stage it uses slot it % 4, free once the MMAs of stage it - 4 retired
 constexpr int kSplitWarps = 4, kSplitThreads = 32 * kSplitWarps;  // per split group
-constexpr int kSplitGroups = 2;  // the groups take alternate stages
+#ifndef MK_TC_SPLIT_GROUPS
+#define MK_TC_SPLIT_GROUPS 3
+#endif
+constexpr int kSplitGroups = MK_TC_SPLIT_GROUPS;  // group g takes the stages g, g + G, g + 2 G, ...
 constexpr int kReadWarps = 8;
 constexpr int kFirstReadWarp = 4 + kSplitGroups * kSplitWarps;
-constexpr int kThreads = 128 + kSplitGroups * kSplitThreads + 32 * kReadWarps;  // 20 warps = 5 warpgroups: {TMA A, MMA, relay, TMA B}, split x 2, read-out x 2
-// Register budget per warpgroup (setmaxnreg): launched at 96 registers per thread (640 x 96 = 61440 is the CTA's pool); the
-// control and split warpgroups give most of their share back and the read-out warps, who hold 128 running sums each,
-// take it: 128 x 32 + 256 x 64 + 256 x 160 = 61440.
-constexpr int kRegsControl = 32, kRegsSplit = 64, kRegsRead = 160;
+constexpr int kThreads = 128 + kSplitGroups * kSplitThreads + 32 * kReadWarps;  // 24 warps = 6 warpgroups: {TMA A, MMA, relay, TMA B}, split x 3, read-out x 2
+// Register budget per warpgroup (setmaxnreg): launched at 80 registers per thread (768 x 80 = 61440 is the CTA's pool); the
+// control warpgroup gives most of its share back and the read-out warps, who hold 96 running sums each, take it:
+// 128 x 32 + 384 x 64 + 256 x 128 = 61440.  (Two split groups: 640 threads at 96; 128 x 32 + 256 x 72 + 256 x 152.)
+constexpr int kRegsControl = 32, kRegsSplit = kSplitGroups == 3 ? 64 : 72, kRegsRead = kSplitGroups == 3 ? 128 : 152;
 constexpr int kChunk = 4;       // stages per accumulation chunk (24 MMA steps)
-constexpr uint32_t A_BYTES = BM * 2 * BKC * 4;  // 8 KB: one A tile
+constexpr int kASlots = 3;      // ring of raw A boxes
+constexpr uint32_t A_BOX_BYTES = BM * 4 * BKC * 4;  // 16 KB: one raw A box = [128 rows][16 shots] = two stages, 128-byte rows
 constexpr uint32_t BLK_BYTES = BKC * 32 * 4;    // 1 KB: one 32-column block of one B region (8 rows of 128 B)
-// A stage = A_hi (the raw tile, de-interleaved in place), A_lo, then four B regions of nblk column blocks each:
-// B0_hi (raw, TMA), B0_lo, B1_hi, B1_lo; nblk = min(8, columns / 32).  The distance B0 -> B1 (two regions) is the
-// stride-byte-offset of the B descriptors: the second group of four K rows of every MMA is the rotated copy of the first.
-__host__ __device__ constexpr uint32_t stage_bytes(int nblk) { return 2 * A_BYTES + 4 * (uint32_t)nblk * BLK_BYTES; }
-constexpr size_t kSmemExtra = 1024 /*alignment slack*/ + 512 /*barriers, counters: (3 x 10 + 2) x 8 + 11 x 4 + 4 bytes*/;
+// A stage = the raw B tile as TMA delivered it ([8 shots][nblk x 128 B], dense rows), then the four B regions of nblk
+// column blocks each that the tensor core reads: B0_hi, B0_lo, B1_hi, B1_lo; nblk = min(6, columns / 32).  The distance
+// B0 -> B1 (two regions) is the stride-byte-offset of the B descriptors: the second group of four K rows of every MMA
+// is the rotated copy of the first.  The raw A boxes have a ring of their own (one box feeds two stages).
+__host__ __device__ constexpr uint32_t stage_bytes(int nblk) { return 5 * (uint32_t)nblk * BLK_BYTES; }
+constexpr size_t kSmemExtra = 1024 /*alignment slack*/ + 512 /*barriers, counters: (3 x 7 + 2 + 2 x 3) x 8 + (7 + 2 + 1) x 4 bytes*/;
 constexpr uint32_t kTmemCols = 512;
+constexpr uint32_t kTmemA = 2 * BN;  // first column of the A ring
+constexpr uint32_t kTmemAStage = 32; // columns per slot: K step j at 16 j: A_hi (8 columns), A_lo (8 columns)
+static_assert(kTmemA + kTmemSlots * kTmemAStage <= kTmemCols, "tensor memory budget");
 
 // ---------------------------------------------------------------------------------------------- PTX wrappers
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
@@ -102,8 +116,11 @@ __device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes) {
 #ifndef MK_MBAR_TIMEOUT_CYCLES
 #define MK_MBAR_TIMEOUT_CYCLES 40000000000LL
 #endif
-// try_wait sleeps in hardware until the phase completes or a time limit passes (it does not spin), so a waiting warp
-// costs next to no issue slots and power
+// try_wait suspends the thread in hardware until the phase completes or a time limit passes.  The default limit is short:
+// measured (ncu, round 2) the eight read-out warps came back every ~75 clk and their retry loops were 40 % of all the
+// instructions the SM issued, taking issue slots from the split warps on the same schedulers.  With an explicit limit the
+// thread sleeps until the barrier wakes it.
+constexpr uint32_t kSuspendHintNs = 20000;
 __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
   const uint32_t addr = smem_u32(bar);
 #if MK_MBAR_TIMEOUT_CYCLES > 0
@@ -113,10 +130,10 @@ __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
     uint32_t done;
     asm volatile(
         "{\n\t.reg .pred p;\n\t"
-        "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2, %3;\n\t"
         "selp.u32 %0, 1, 0, p;\n\t}"
         : "=r"(done)
-        : "r"(addr), "r"(parity)
+        : "r"(addr), "r"(parity), "r"(kSuspendHintNs)
         : "memory");
     if (done) return;
 #if MK_MBAR_TIMEOUT_CYCLES > 0
@@ -155,29 +172,26 @@ __device__ __forceinline__ void tma_load_3d(const void* tmap, uint64_t* bar, voi
       : "memory");
 }
 
+__device__ __forceinline__ void tma_load_2d(const void* tmap, uint64_t* bar, void* dst, int c0, int c1) {
+  asm volatile("cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4}], [%2];" ::"r"(smem_u32(dst)),
+               "l"(tmap), "r"(smem_u32(bar)), "r"(c0), "r"(c1)
+               : "memory");
+}
+
 __device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
 __device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
 
-__device__ __forceinline__ void umma_tf32(uint32_t tmem_d, uint64_t adesc, uint64_t bdesc, uint32_t idesc, uint32_t accumulate) {
+// A from tensor memory, B from shared memory; the B descriptor given as 32-bit halves: the high word (SBO, version,
+// layout) never changes and the low word (start address, LBO) of a stage is that of stage 0 plus a constant, so the
+// issuing warp keeps them in (uniform) registers and pays one add per descriptor and stage
+__device__ __forceinline__ void umma_tf32_ts(uint32_t tmem_d, uint32_t tmem_a, uint32_t b_lo32, uint32_t b_hi32, uint32_t idesc,
+                                             uint32_t accumulate) {
   asm volatile(
-      "{\n\t.reg .pred p;\n\t"
-      "setp.ne.b32 p, %4, 0;\n\t"
-      "tcgen05.mma.cta_group::1.kind::tf32 [%0], %1, %2, %3, p;\n\t}" ::"r"(tmem_d),
-      "l"(adesc), "l"(bdesc), "r"(idesc), "r"(accumulate)
-      : "memory");
-}
-// the same with the two descriptors given as 32-bit halves: the high words (SBO, version, layout) never change and the
-// low words (start address, LBO) of a stage are those of stage 0 plus a constant, so the issuing warp keeps them in
-// (uniform) registers and pays one add per descriptor and stage
-__device__ __forceinline__ void umma_tf32_w(uint32_t tmem_d, uint32_t a_lo32, uint32_t a_hi32, uint32_t b_lo32, uint32_t b_hi32, uint32_t idesc,
-                                            uint32_t accumulate) {
-  asm volatile(
-      "{\n\t.reg .pred p;\n\t.reg .b64 da, db;\n\t"
-      "mov.b64 da, {%1, %2};\n\t"
-      "mov.b64 db, {%3, %4};\n\t"
-      "setp.ne.b32 p, %6, 0;\n\t"
-      "tcgen05.mma.cta_group::1.kind::tf32 [%0], da, db, %5, p;\n\t}" ::"r"(tmem_d),
-      "r"(a_lo32), "r"(a_hi32), "r"(b_lo32), "r"(b_hi32), "r"(idesc), "r"(accumulate)
+      "{\n\t.reg .pred p;\n\t.reg .b64 db;\n\t"
+      "mov.b64 db, {%2, %3};\n\t"
+      "setp.ne.b32 p, %5, 0;\n\t"
+      "tcgen05.mma.cta_group::1.kind::tf32 [%0], [%1], db, %4, p;\n\t}" ::"r"(tmem_d),
+      "r"(tmem_a), "r"(b_lo32), "r"(b_hi32), "r"(idesc), "r"(accumulate)
       : "memory");
 }
 // one lane of a fully active warp (the same one every time: tcgen05.commit tracks the MMAs of the thread that runs it)
@@ -190,7 +204,14 @@ __device__ __forceinline__ void umma_commit(uint64_t* bar) {  // arrives on `bar
   asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(smem_u32(bar)) : "memory");
 }
 
-// eight columns at a time: the read-out warps hold 128 running sums each and have 160 registers
+__device__ __forceinline__ void tmem_st16(uint32_t taddr, const float4& a, const float4& b, const float4& c, const float4& d) {
+  asm volatile(
+      "tcgen05.st.sync.aligned.32x32b.x16.b32 [%0], {%1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, %16};" ::"r"(taddr),
+      "f"(a.x), "f"(a.y), "f"(a.z), "f"(a.w), "f"(b.x), "f"(b.y), "f"(b.z), "f"(b.w), "f"(c.x), "f"(c.y), "f"(c.z), "f"(c.w), "f"(d.x),
+      "f"(d.y), "f"(d.z), "f"(d.w)
+      : "memory");
+}
+// eight columns at a time: the read-out warps hold 96 running sums each
 __device__ __forceinline__ void tmem_ld8(uint32_t taddr, uint32_t* v) {
   asm volatile("tcgen05.ld.sync.aligned.32x32b.x8.b32 {%0, %1, %2, %3, %4, %5, %6, %7}, [%8];"
                : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7])
@@ -240,9 +261,9 @@ struct TcParams {
   int mt, ntl;          // tiles along M and N
   int nblk, stages;     // column blocks per B region, stages of the ring
   size_t s_row;         // floats between consecutive receivers of S^: nb * 2 ldf
+  int tune;             // MK_OPT_TUNE bits 2..5: parts of the kernel left out (bottleneck measurements; results are wrong)
 };
 
-template <int JOINT>  // split warps: 0 = two groups on alternate stages, 1 = all eight warps on every stage
 __global__ void __launch_bounds__(kThreads, 1)
 k_syn_gemm_tf32x3(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB, float* __restrict__ Shat,
                   TcParams P) {
@@ -250,12 +271,15 @@ k_syn_gemm_tf32x3(const __grid_constant__ CUtensorMap tmA, const __grid_constant
   uint8_t* smem = reinterpret_cast<uint8_t*>(((uintptr_t)smem_raw + 1023) & ~(uintptr_t)1023);
   const int STAGES = P.stages;
   const uint32_t STAGE_BYTES = stage_bytes(P.nblk), REG = (uint32_t)P.nblk * BLK_BYTES;  // REG: bytes of one B region
-  uint64_t* bars = reinterpret_cast<uint64_t*>(smem + (size_t)STAGES * STAGE_BYTES);
+  uint8_t* stages = smem + kASlots * A_BOX_BYTES;  // the A ring comes first
+  uint64_t* bars = reinterpret_cast<uint64_t*>(stages + (size_t)STAGES * STAGE_BYTES);
   uint64_t* full = bars;                       // [kMaxStages] TMA landed
   uint64_t* empty = bars + kMaxStages;         // [kMaxStages] MMAs of the stage retired
   uint64_t* split_bar = bars + 2 * kMaxStages;  // [kMaxStages] the split warps are done with the stage
   uint64_t* acc_full = bars + 3 * kMaxStages;   // [2] chunk accumulator complete
-  uint32_t* ready = reinterpret_cast<uint32_t*>(acc_full + 2);  // [kMaxStages] uses of the stage that are ready for the MMAs (relay)
+  uint64_t* fullA = acc_full + 2;               // [kASlots] raw A box landed
+  uint64_t* emptyA = fullA + kASlots;           // [kASlots] both split groups have read their half of the box
+  uint32_t* ready = reinterpret_cast<uint32_t*>(emptyA + kASlots);  // [kMaxStages] uses of the stage that are ready for the MMAs (relay)
   uint32_t* drained = ready + kMaxStages;      // [2] read-out warps done with a use of TMEM buffer b (counts up; PER BUFFER:
                                                // one sum over both would let fast warps' arrivals for the other buffer stand in for
                                                // a slow warp's missing one)
@@ -267,13 +291,17 @@ k_syn_gemm_tf32x3(const __grid_constant__ CUtensorMap tmA, const __grid_constant
 
   if (threadIdx.x == 0) {
     for (int s = 0; s < STAGES; ++s) {
-      mbar_init(full + s, 2);  // the A producer and the B producer, each with its own byte count
+      mbar_init(full + s, 1);  // the B producer
       mbar_init(empty + s, 1);
-      mbar_init(split_bar + s, JOINT ? kSplitGroups * kSplitWarps : kSplitWarps);  // the warps that take the stage
+      mbar_init(split_bar + s, kSplitWarps);
       ready[s] = 0;
     }
     mbar_init(acc_full + 0, 1);
     mbar_init(acc_full + 1, 1);
+    for (int a = 0; a < kASlots; ++a) {
+      mbar_init(fullA + a, 1);
+      mbar_init(emptyA + a, 2 * kSplitWarps);  // the box has two halves = two stages, each read by the four warps of one group
+    }
     drained[0] = drained[1] = 0;
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
@@ -290,18 +318,25 @@ k_syn_gemm_tf32x3(const __grid_constant__ CUtensorMap tmA, const __grid_constant
   if (warp == 0) {
     // ------------------------------------------------------------------------------------ TMA producer
     asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(kRegsControl));
+    // One box = [128 receivers][16 shots] = 128 rows of 128 bytes (SWIZZLE_128B) feeds two stages: the TMA unit's cost is
+    // per ROW of a box (measured: ~8 clk per row whether it has 64 or 128 bytes; 128 rows x 64 B per 8-shot stage alone
+    // took 1030 clk, more than the stage's MMAs), so rows are made as long as the swizzle span allows.
     if (lane == 0) {
-      int s = 0;
-      uint32_t ph = 0;  // ring position and its phase, kept incrementally (the ring length is a run-time value)
+      int a = 0;
+      uint32_t ph = 0;  // ring position and its phase
+      const int KB2 = KB / 2;
       for (int t = blockIdx.x; t < ntiles; t += gridDim.x) {
-        const int kk = t / per_bin, rem = t - kk * per_bin, mi = rem / P.ntl, ni = rem - mi * P.ntl;
-        for (int kb = 0; kb < KB; ++kb) {
-          mbar_wait(empty + s, ph ^ 1);
-          uint8_t* st = smem + (size_t)s * STAGE_BYTES;
-          mbar_expect_tx(full + s, A_BYTES);
-          tma_load_3d(&tmA, full + s, st, kb * 2 * BKC, kk, mi * BM);  // rows past the last receiver arrive as zeros (and still count)
-          if (++s == STAGES) {
-            s = 0;
+        const int kk = t / per_bin, rem = t - kk * per_bin, mi = rem / P.ntl;
+        for (int kb2 = 0; kb2 < KB2; ++kb2) {
+          mbar_wait(emptyA + a, ph ^ 1);
+          if (P.tune & (64 | 128)) {
+            mbar_arrive(fullA + a);
+          } else {
+            mbar_expect_tx(fullA + a, A_BOX_BYTES);
+            tma_load_3d(&tmA, fullA + a, smem + (size_t)a * A_BOX_BYTES, kb2 * 4 * BKC, kk, mi * BM);  // rows past the last receiver arrive as zeros
+          }
+          if (++a == kASlots) {
+            a = 0;
             ph ^= 1;
           }
         }
@@ -311,18 +346,16 @@ k_syn_gemm_tf32x3(const __grid_constant__ CUtensorMap tmA, const __grid_constant
     // ------------------------------------------------------------------------------------ MMA issuer
     asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(kRegsControl));
     // The whole warp runs the loop (warp-uniform control flow and addresses: the compiler keeps them in uniform registers);
-    // one elected lane issues.  Descriptors: see smem_desc.  A: K-major, 64-byte rows, SWIZZLE_64B, 8-row groups 512 B
-    // apart; K step j = bytes 32 j .. 32 j + 31 of the row = (re of shots 4j .. 4j+3 | im of the same shots) after the
-    // split warps' de-interleave.  B: MN-major tf32 must use the 128-byte swizzle with 32-byte atoms (the only MN-major
-    // layout the tensor core takes for 32-bit operands): a region is [nblk blocks of 32 columns][8 shot rows][128 B];
-    // LBO = 1024 (next column block); the K step's first four rows are shots 4j .. 4j+3 of B0 (512 j into the block), its
-    // second four rows sit SBO = 2 regions further: the same shots of B1 = i B0.
-    const uint32_t base16 = (smem_u32(smem) & 0x3FFFF) >> 4, stage16 = STAGE_BYTES >> 4;
-    const uint32_t hiA = (512u >> 4) | (1u << 14) | (LAYOUT_SW64 << 29);
+    // one elected lane issues.  A: tensor memory, lane = row of the tile, 8 columns per K step (re of shots 4j .. 4j+3 | im of
+    // the same shots), hi at column 16 j of the stage's slot, lo at 16 j + 8.  B: MN-major tf32 must use the 128-byte swizzle
+    // with 32-byte atoms (the only MN-major layout the tensor core takes for 32-bit operands): a region is [nblk blocks of
+    // 32 columns][8 shot rows][128 B]; LBO = 1024 (next column block); the K step's first four rows are shots 4j .. 4j+3 of
+    // B0 (512 j into the block), its second four rows sit SBO = 2 regions further: the same shots of B1 = i B0.
+    const uint32_t base16 = (smem_u32(stages) & 0x3FFFF) >> 4, stage16 = STAGE_BYTES >> 4;
     const uint32_t hiB = ((2 * REG) >> 4) | (1u << 14) | (LAYOUT_SW128_BASE32B << 29);
-    const uint32_t loA_hi0 = base16 | ((16u >> 4) << 16), loA_lo0 = loA_hi0 + (A_BYTES >> 4);  // A_hi / A_lo tile, K step 0 (step 1: + 2)
-    const uint32_t loB_hi0 = (base16 + ((2 * A_BYTES) >> 4)) | ((BLK_BYTES >> 4) << 16), loB_lo0 = loB_hi0 + (REG >> 4);  // (step 1: + 32)
-    uint32_t g = 0, pass = 0;  // global chunk index; completed passes over the ring
+    const uint32_t loB_hi0 = (base16 + (REG >> 4)) | ((BLK_BYTES >> 4) << 16), loB_lo0 = loB_hi0 + (REG >> 4);  // behind the raw tile (K step 1: + 32)
+    const uint32_t tmA0 = tmem_base + kTmemA;
+    uint32_t g = 0, pass = 0, it = 0;  // global chunk index; completed passes over the ring; global stage index
     int s = 0;
     for (int t = blockIdx.x; t < ntiles; t += gridDim.x) {
       const int rem = t % per_bin, ni = rem % P.ntl;
@@ -338,18 +371,21 @@ k_syn_gemm_tf32x3(const __grid_constant__ CUtensorMap tmA, const __grid_constant
           flag_wait_ge(ready + s, pass + 1);
           __syncwarp();  // the lanes leave the polling loop one by one: elect.sync needs them all back
           tc_fence_after();
-          const uint32_t off = (uint32_t)s * stage16;
+          const uint32_t off = (uint32_t)s * stage16, ta = tmA0 + (it & (kTmemSlots - 1)) * kTmemAStage;
           if (elect_one()) {
             // small terms first; a chunk starts from zero
-            umma_tf32_w(d, loA_lo0 + off, hiA, loB_hi0 + off, hiB, idesc, kb != kb0);
-            umma_tf32_w(d, loA_hi0 + off, hiA, loB_lo0 + off, hiB, idesc, 1);
-            umma_tf32_w(d, loA_hi0 + off, hiA, loB_hi0 + off, hiB, idesc, 1);
-            umma_tf32_w(d, loA_lo0 + off + 2, hiA, loB_hi0 + off + 32, hiB, idesc, 1);
-            umma_tf32_w(d, loA_hi0 + off + 2, hiA, loB_lo0 + off + 32, hiB, idesc, 1);
-            umma_tf32_w(d, loA_hi0 + off + 2, hiA, loB_hi0 + off + 32, hiB, idesc, 1);
+            if (!(P.tune & 8)) {
+            umma_tf32_ts(d, ta + 8, loB_hi0 + off, hiB, idesc, kb != kb0);
+            umma_tf32_ts(d, ta, loB_lo0 + off, hiB, idesc, 1);
+            umma_tf32_ts(d, ta, loB_hi0 + off, hiB, idesc, 1);
+            umma_tf32_ts(d, ta + 24, loB_hi0 + off + 32, hiB, idesc, 1);
+            umma_tf32_ts(d, ta + 16, loB_lo0 + off + 32, hiB, idesc, 1);
+            umma_tf32_ts(d, ta + 16, loB_hi0 + off + 32, hiB, idesc, 1);
+            }
             umma_commit(empty + s);
           }
           __syncwarp();
+          ++it;
           if (++s == STAGES) {
             s = 0;
             ++pass;
@@ -391,9 +427,14 @@ k_syn_gemm_tf32x3(const __grid_constant__ CUtensorMap tmA, const __grid_constant
         const int kk = t / per_bin, rem = t - kk * per_bin, ni = rem % P.ntl;
         for (int kb = 0; kb < KB; ++kb) {
           mbar_wait(empty + s, ph ^ 1);
-          mbar_expect_tx(full + s, REG);
-          // column blocks past 2 ldf arrive as zeros (and still count their bytes)
-          tma_load_3d(&tmB, full + s, smem + (size_t)s * STAGE_BYTES + 2 * A_BYTES, 0, kk * P.ld + kb * BKC, ni * (BN / 32));
+          if (P.tune & (64 | 256)) {
+            mbar_arrive(full + s);
+          } else {
+            mbar_expect_tx(full + s, REG);
+            // eight dense rows of nblk x 128 bytes (8 rows for the TMA unit instead of 8 nblk in the tensor core's layout);
+            // columns past 2 ldf arrive as zeros (and still count their bytes)
+            tma_load_2d(&tmB, full + s, stages + (size_t)s * STAGE_BYTES, ni * BN, kk * P.ld + kb * BKC);
+          }
           if (++s == STAGES) {
             s = 0;
             ph ^= 1;
@@ -403,61 +444,111 @@ k_syn_gemm_tf32x3(const __grid_constant__ CUtensorMap tmA, const __grid_constant
     }
   } else if (warp < kFirstReadWarp) {
     // ------------------------------------------------------------------------------------ split warps
-    // Two groups of four warps; group g takes the stages g, g + 2, g + 4, ... of this CTA's stage sequence, so the
-    // latency chain of one stage (wait, LDS -> ALU -> STS, proxy fence, arrive) overlaps the other group's
+    // Three groups of four warps; group g takes the stages g, g + 3, g + 6, ... of this CTA's stage sequence, so the
+    // latency chain of one stage (waits, LDS -> ALU -> STS / tcgen05.st, fences, arrive: ~1400 clk measured, against 576 clk
+    // of MMAs per stage) overlaps the other groups'.
     asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(kRegsSplit));
-    const int grp = JOINT ? 0 : (warp - 4) / kSplitWarps;
-    constexpr int NT = JOINT ? kSplitGroups * kSplitThreads : kSplitThreads;  // threads that share a stage
-    constexpr int STEP = JOINT ? 1 : kSplitGroups;
-    const int wt = threadIdx.x - 128 - grp * kSplitThreads;  // 0 .. NT - 1
-    const uint32_t smem_base = smem_u32(smem);
-    // A work items of this thread: 32-byte pairs p = wt (and wt + 128) of the tile; pair p = row p / 2, K step p % 2.
-    // SWIZZLE_64B: the 16-byte chunk c of row r sits at chunk position c ^ ((r >> 1) & 3).
-    constexpr int NA = 256 / NT;
-    uint32_t a_off[NA][2];
+    const int grp = (warp - 4) / kSplitWarps;
+    const int wt = threadIdx.x - 128 - grp * kSplitThreads;  // 0 .. 127
+    const uint32_t stages_base = smem_u32(stages), a_base = smem_u32(smem);
+    // A: this thread owns row ar = 32 (warp % 4) + lane of the tile (the TMEM lanes its warp may write) and reads the 64 bytes
+    // of the stage's half of the box (stage it = half it % 2 of box it / 2): K step j = bytes 32 j .. 32 j + 31 of the half =
+    // (re0 im0 re1 im1 | re2 im2 re3 im3) of shots 4 j .. 4 j + 3.  SWIZZLE_128B: the 16-byte chunk c of row r sits at
+    // chunk position c ^ (r & 7); the second half's chunks (4 + c) sit 64 bytes "xor-away" from the first half's.
+    const int ar = 32 * (warp & 3) + lane;
+    uint32_t a_off[4];
 #pragma unroll
-    for (int k = 0; k < NA; ++k) {
-      const int pr = wt + k * NT, ar = pr >> 1, ap = pr & 1, ax = (ar >> 1) & 3;
-      a_off[k][0] = (uint32_t)ar * 64 + (uint32_t)(((2 * ap) ^ ax) << 4);
-      a_off[k][1] = (uint32_t)ar * 64 + (uint32_t)(((2 * ap + 1) ^ ax) << 4);
+    for (int c = 0; c < 4; ++c) a_off[c] = (uint32_t)ar * 128 + (uint32_t)((c ^ (ar & 7)) << 4);
+    const uint32_t a_tmem = tmem_base + ((uint32_t)(32 * (warp & 3)) << 16) + kTmemA;
+    // B: this thread's float4s of the raw tile [8 shots][nblk x 128 B]: q = wt, wt + 128, ... < 8 x 8 nblk; shot row
+    // r = q / (8 nblk), column block b and 16-byte chunk c of the block from q % (8 nblk).  In the tensor core's layout the
+    // 32-byte unit u of row r of a block sits at unit position u ^ (r & 3) (SWIZZLE_128B with 32-byte atoms).
+    const uint32_t per_row = 8 * (uint32_t)P.nblk, nq = 8 * per_row;  // nq <= 384: at most three float4s per thread
+    uint32_t b_dst[3];
+#pragma unroll
+    for (int i = 0; i < 3; ++i) {
+      const uint32_t q = (uint32_t)wt + i * kSplitThreads, r = q / per_row, x = q - r * per_row, blk = x >> 3, ch = x & 7;
+      b_dst[i] = REG + blk * BLK_BYTES + r * 128 + ((((ch >> 1) ^ (r & 3)) << 5) | ((ch & 1) << 4));
     }
+    const int nmine = (int)wt < (int)nq ? (int)((nq - wt + kSplitThreads - 1) / kSplitThreads) : 0;
     const int my_tiles = blockIdx.x < ntiles ? (ntiles - blockIdx.x + gridDim.x - 1) / gridDim.x : 0;
-    const long long total = (long long)my_tiles * KB;  // stages this CTA runs through
-    int s = grp % STAGES;
+    const uint32_t total = (uint32_t)my_tiles * (uint32_t)KB;  // stages this CTA runs through
+    int s = grp % STAGES;  // ring slot of stage it and its phase
     uint32_t ph = (grp / STAGES) & 1;
-    for (long long it = grp; it < total; it += STEP) {
+    // ring slot of stage it - kTmemSlots, used from this group's first stage it >= kTmemSlots on (only when STAGES > 4)
+    int s4;
+    uint32_t ph4;
+    {
+      int it0 = grp;
+      while (it0 < kTmemSlots) it0 += kSplitGroups;
+      s4 = (it0 - kTmemSlots) % STAGES;
+      ph4 = ((it0 - kTmemSlots) / STAGES) & 1;
+    }
+    for (uint32_t it = grp; it < total; it += kSplitGroups) {
+      const uint32_t box = it >> 1, half = (it & 1) << 6;
+      const int sa = (int)(box % kASlots);  // slot of the raw A box of stage it, and its phase
+      const uint32_t pha = (box / kASlots) & 1;
+      if (P.tune & 32) {
+        mbar_wait(full + s, ph);
+        mbar_wait(fullA + sa, pha);
+        __syncwarp();
+        if (lane == 0) {
+          mbar_arrive(emptyA + sa);
+          mbar_arrive(split_bar + s);
+        }
+      } else {
+      mbar_wait(fullA + sa, pha);
+      float4 c[4];
+#pragma unroll
+      for (int k = 0; k < 4; ++k) c[k] = lds128(a_base + (uint32_t)sa * A_BOX_BYTES + (a_off[k] ^ half));
       mbar_wait(full + s, ph);
-      const uint32_t st = smem_base + (uint32_t)s * STAGE_BYTES, b0 = st + 2 * A_BYTES;
-      {  // A: (re0 im0 re1 im1 | re2 im2 re3 im3) -> hi (re0 re1 re2 re3 | im0 im1 im2 im3) in place, lo beside it
-        float4 c[NA][2];
+      const uint32_t st = stages_base + (uint32_t)s * STAGE_BYTES;  // raw tile, then B0_hi, ...
+      // B: raw tile -> B0_hi (copy), B0_lo, and B1 = i B0 (every float4 holds two (re, im) pairs) hi / lo
+      float4 v[3];
 #pragma unroll
-        for (int k = 0; k < NA; ++k) {
-          c[k][0] = lds128(st + a_off[k][0]);
-          c[k][1] = lds128(st + a_off[k][1]);
+      for (int i = 0; i < 3; ++i)
+        if (i < nmine) v[i] = lds128(st + (((uint32_t)wt + i * kSplitThreads) << 4));
+#pragma unroll
+      for (int i = 0; i < 3; ++i)
+        if (i < nmine && !(P.tune & 16)) {
+          const uint32_t dst = st + b_dst[i];
+          const float4 l = lo4(v[i]);
+          sts128(dst, v[i]);
+          sts128(dst + REG, l);
+          sts128(dst + 2 * REG, make_float4(-v[i].y, v[i].x, -v[i].w, v[i].z));
+          sts128(dst + 3 * REG, make_float4(-l.y, l.x, -l.w, l.z));
         }
-#pragma unroll
-        for (int k = 0; k < NA; ++k) {
-          const float4 re = make_float4(c[k][0].x, c[k][0].z, c[k][1].x, c[k][1].z), im = make_float4(c[k][0].y, c[k][0].w, c[k][1].y, c[k][1].w);
-          sts128(st + a_off[k][0], re);
-          sts128(st + a_off[k][1], im);
-          sts128(st + A_BYTES + a_off[k][0], lo4(re));
-          sts128(st + A_BYTES + a_off[k][1], lo4(im));
+      // The A slot in tensor memory is free once the MMAs of stage it - 4 have retired.  A ring of <= 4 stages implies it
+      // (the TMA of stage it waited for stage it - STAGES); a longer one is asked: empty[] of that stage's slot cannot run a
+      // second phase ahead, its next use is stage it - 4 + STAGES > it, whose MMAs wait for this very split.
+      if (STAGES > kTmemSlots && it >= kTmemSlots) {
+        mbar_wait(empty + s4, ph4);
+        tc_fence_after();
+        s4 += kSplitGroups;
+        while (s4 >= STAGES) {
+          s4 -= STAGES;
+          ph4 ^= 1;
         }
       }
-      // B: elementwise on the swizzled tile — lo of B0, and B1 = i B0 (every float4 holds two (re, im) pairs)
-#pragma unroll 2
-      for (uint32_t q = 16 * (uint32_t)wt; q < REG; q += 16 * NT) {
-        const float4 v = lds128(b0 + q);
-        const float4 l = lo4(v);
-        sts128(b0 + q + REG, l);
-        sts128(b0 + q + 2 * REG, make_float4(-v.y, v.x, -v.w, v.z));
-        sts128(b0 + q + 3 * REG, make_float4(-l.y, l.x, -l.w, l.z));
+      // A -> tensor memory: per K step hi (re0 re1 re2 re3 | im0 im1 im2 im3), lo beside it
+      const uint32_t ta = a_tmem + ((uint32_t)it & (kTmemSlots - 1)) * kTmemAStage;
+#pragma unroll
+      for (int j = 0; j < 2; ++j) {
+        const float4 re = make_float4(c[2 * j].x, c[2 * j].z, c[2 * j + 1].x, c[2 * j + 1].z),
+                     im = make_float4(c[2 * j].y, c[2 * j].w, c[2 * j + 1].y, c[2 * j + 1].w);
+        tmem_st16(ta + 16 * j, re, im, lo4(re), lo4(im));
       }
+      asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
       asm volatile("fence.proxy.async.shared::cta;" ::: "memory");  // generic-proxy writes -> visible to the tensor core
+      tc_fence_before();
       __syncwarp();
-      if (lane == 0) mbar_arrive(split_bar + s);
-      s += STEP;
-      if (s >= STAGES) {  // STAGES >= 2: at most one wrap
+      if (lane == 0) {
+        mbar_arrive(emptyA + sa);  // this warp's rows of the box are in registers / tensor memory
+        mbar_arrive(split_bar + s);
+      }
+      }
+      s += kSplitGroups;
+      while (s >= STAGES) {
         s -= STAGES;
         ph ^= 1;
       }
@@ -466,7 +557,7 @@ k_syn_gemm_tf32x3(const __grid_constant__ CUtensorMap tmA, const __grid_constant
     // ------------------------------------------------------------------------------------ read-out warps: chunk sums in registers
     asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(kRegsRead));
     const int quad = warp & 3;         // TMEM lanes 32 quad .. 32 quad + 31 are the ones this warp may read
-    const int half = (warp - kFirstReadWarp) >> 2;  // columns 128 half .. 128 half + 127 of the tile
+    const int half = (warp - kFirstReadWarp) >> 2;  // columns (BN / 2) half .. + BN / 2 - 1 of the tile
     uint32_t g = 0;
     for (int t = blockIdx.x; t < ntiles; t += gridDim.x) {
       const int kk = t / per_bin, rem = t - kk * per_bin, mi = rem / P.ntl, ni = rem - mi * P.ntl;
@@ -481,7 +572,7 @@ k_syn_gemm_tf32x3(const __grid_constant__ CUtensorMap tmA, const __grid_constant
         const uint32_t ta = tmem_base + ((uint32_t)(quad * 32) << 16) + (uint32_t)(b * BN + half * (BN / 2));
 #pragma unroll
         for (int c = 0; c < BN / 16; ++c) {
-          if (c * 8 < cols) {  // warp-uniform; columns past the MMA's N hold stale data
+          if (c * 8 < cols && !(P.tune & 4)) {  // warp-uniform; columns past the MMA's N hold stale data
             uint32_t v[8];
             tmem_ld8(ta + (uint32_t)(c * 8), v);
             asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
@@ -527,10 +618,10 @@ int get_encode(mk_ctx* c, EncodeTiledFn* fn) {
   return MK_OK;
 }
 
-int encode3(mk_ctx* c, EncodeTiledFn enc, void* out, const void* base, const cuuint64_t dims[3], const cuuint64_t strides[2],
-            const cuuint32_t box[3], CUtensorMapSwizzle sw, const char* what) {
+int encode(mk_ctx* c, EncodeTiledFn enc, void* out, const void* base, int rank, const cuuint64_t* dims, const cuuint64_t* strides,
+           const cuuint32_t* box, CUtensorMapSwizzle sw, const char* what) {
   const cuuint32_t es[3] = {1, 1, 1};
-  const CUresult r = enc(reinterpret_cast<CUtensorMap*>(out), CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, const_cast<void*>(base), dims,
+  const CUresult r = enc(reinterpret_cast<CUtensorMap*>(out), CU_TENSOR_MAP_DATA_TYPE_FLOAT32, (cuuint32_t)rank, const_cast<void*>(base), dims,
                          strides, box, es, CU_TENSOR_MAP_INTERLEAVE_NONE, sw, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
                          CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
   if (r != CUDA_SUCCESS) {
@@ -546,7 +637,7 @@ int encode3(mk_ctx* c, EncodeTiledFn enc, void* out, const void* base, const cuu
 bool tc_supported(const mk_ctx* c) {
   int major = 0;
   cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, c->dev);
-  return major == 10 && c->smem_optin >= 2 * stage_bytes(1) + kSmemExtra;
+  return major == 10 && c->smem_optin >= kASlots * A_BOX_BYTES + 2 * stage_bytes(1) + kSmemExtra;
 }
 
 int launch_syn_tc(mk_ctx* c, const RowBlock& rb, int slot, const float2* d_Nhat, float2* d_Shat, int ldf) {
@@ -556,22 +647,22 @@ int launch_syn_tc(mk_ctx* c, const RowBlock& rb, int slot, const float2* d_Nhat,
   // descriptor cache: the resident rows, or one of the two streaming windows (mk_create_streamed)
   const int ia = rb.Rhat == c->d_win[0] && c->d_win[0] ? 1 : (rb.Rhat == c->d_win[1] && c->d_win[1] ? 2 : 0);
   if (c->tmap_A_key[ia] != rb.Rhat || c->tmap_A_rows[ia] != rb.nrow) {
-    // A = R^ as fp32 [n][nb][2 ld]: dims (float of the row, bin, r); box = 16 floats x 1 bin x 128 receivers; rows r >= n read as zero
+    // A = R^ as fp32 [n][nb][2 ld]: dims (float of the row, bin, r); box = 32 floats (16 shots) x 1 bin x 128 receivers; rows r >= n read as zero
     const cuuint64_t dims[3] = {(cuuint64_t)2 * c->ld, (cuuint64_t)c->nb, (cuuint64_t)rb.nrow};  // rows of this block
     const cuuint64_t str[2] = {(cuuint64_t)2 * c->ld * 4, (cuuint64_t)c->nb * 2 * c->ld * 4};
-    const cuuint32_t box[3] = {2 * BKC, 1, BM};
-    if (int rc = encode3(c, enc, c->tmap_A[ia], rb.Rhat, dims, str, box, CU_TENSOR_MAP_SWIZZLE_64B, "A")) return rc;
+    const cuuint32_t box[3] = {4 * BKC, 1, BM};
+    if (int rc = encode(c, enc, c->tmap_A[ia], rb.Rhat, 3, dims, str, box, CU_TENSOR_MAP_SWIZZLE_128B, "A")) return rc;
     c->tmap_A_key[ia] = rb.Rhat;
     c->tmap_A_rows[ia] = rb.nrow;
   }
   const int nblk = std::min(BN / 32, (2 * ldf) / 32);
   if (c->tmap_B_key[slot] != d_Nhat || c->tmap_B_ldf[slot] != ldf) {
-    // B = N^ [nb * ld rows][2 ldf floats] seen as (float in column block, row, column block): box = 32 x 8 x nblk lands in
-    // shared memory as [nblk column blocks][8 rows][128 B], the MN-major SWIZZLE_128B_BASE32B operand layout
-    const cuuint64_t dims[3] = {32, (cuuint64_t)c->nb * c->ld, (cuuint64_t)(2 * ldf) / 32};
-    const cuuint64_t str[2] = {(cuuint64_t)2 * ldf * 4, 128};
-    const cuuint32_t box[3] = {32, BKC, (cuuint32_t)nblk};  // nblk is a function of ldf: one cache key
-    if (int rc = encode3(c, enc, c->tmap_B[slot], d_Nhat, dims, str, box, CU_TENSOR_MAP_SWIZZLE_128B_ATOM_32B, "B")) return rc;
+    // B = N^ as fp32 [nb * ld rows][2 ldf floats]: box = nblk x 32 floats of 8 consecutive rows (shots), dense in shared
+    // memory; the split warps put it into the tensor core's MN-major layout
+    const cuuint64_t dims[2] = {(cuuint64_t)2 * ldf, (cuuint64_t)c->nb * c->ld};
+    const cuuint64_t str[1] = {(cuuint64_t)2 * ldf * 4};
+    const cuuint32_t box[2] = {(cuuint32_t)nblk * 32, BKC};  // nblk is a function of ldf: one cache key
+    if (int rc = encode(c, enc, c->tmap_B[slot], d_Nhat, 2, dims, str, box, CU_TENSOR_MAP_SWIZZLE_NONE, "B")) return rc;
     c->tmap_B_key[slot] = d_Nhat;
     c->tmap_B_ldf[slot] = ldf;
   }
@@ -584,23 +675,19 @@ int launch_syn_tc(mk_ctx* c, const RowBlock& rb, int slot, const float2* d_Nhat,
   P.ntl = (P.ncols + BN - 1) / BN;
   P.s_row = (size_t)c->nb * 2 * ldf;
   P.nblk = nblk;
-  P.stages = (int)std::min<size_t>(kMaxStages, (c->smem_optin - kSmemExtra) / stage_bytes(nblk));
+  P.tune = c->tune;
+  P.stages = (int)std::min<size_t>(kMaxStages, (c->smem_optin - kSmemExtra - kASlots * A_BOX_BYTES) / stage_bytes(nblk));
+  if (c->tune & 512) P.stages = std::min(P.stages, 4);
   if (P.stages < 2) return set_err(c, MK_ERR_INVALID_ARG, "not enough shared memory for the tcgen05 contraction");
-  const size_t kSmemBytes = (size_t)P.stages * stage_bytes(nblk) + kSmemExtra;
+  const size_t kSmemBytes = kASlots * A_BOX_BYTES + (size_t)P.stages * stage_bytes(nblk) + kSmemExtra;
   const int ntiles = P.nb * P.mt * P.ntl;
   const int grid = ntiles < c->num_sms ? ntiles : c->num_sms;
   float* S0 = reinterpret_cast<float*>(d_Shat + (size_t)rb.r0 * c->nb * ldf);
   const CUtensorMap& mA = *reinterpret_cast<const CUtensorMap*>(c->tmap_A[ia]);
   const CUtensorMap& mB = *reinterpret_cast<const CUtensorMap*>(c->tmap_B[slot]);
-  if (c->tune & 2) {
-    if (int rc = check_cuda(c, cudaFuncSetAttribute(k_syn_gemm_tf32x3<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemBytes), "cudaFuncSetAttribute"))
-      return rc;
-    k_syn_gemm_tf32x3<0><<<grid, kThreads, kSmemBytes, c->stream>>>(mA, mB, S0, P);
-  } else {
-    if (int rc = check_cuda(c, cudaFuncSetAttribute(k_syn_gemm_tf32x3<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemBytes), "cudaFuncSetAttribute"))
-      return rc;
-    k_syn_gemm_tf32x3<1><<<grid, kThreads, kSmemBytes, c->stream>>>(mA, mB, S0, P);
-  }
+  if (int rc = check_cuda(c, cudaFuncSetAttribute(k_syn_gemm_tf32x3, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemBytes), "cudaFuncSetAttribute"))
+    return rc;
+  k_syn_gemm_tf32x3<<<grid, kThreads, kSmemBytes, c->stream>>>(mA, mB, S0, P);
   ++c->launches;
   return check_cuda(c, cudaGetLastError(), "k_syn_gemm_tf32x3");
 }
