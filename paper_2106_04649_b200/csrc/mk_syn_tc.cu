@@ -24,36 +24,49 @@
 // while the tensor core works on the next chunk in the other TMEM buffer.  The error is then that of one chunk
 // (~5e-7), independent of n.
 //
-// What shaped it (measured on B200, round 2):
-//   * tcgen05.mma kind::tf32 M = 128, N = 256, K = 8 runs at 128 clk per instruction with nothing else going on;
+// What shaped it (measured on B200, round 2, config 2 = 601 x 608 x 451 bins x 601 focal points; the
+// MK_OPT_TUNE switches that leave out one part of the kernel at a time are still in the code):
+//   * tcgen05.mma kind::tf32 M = 128, K = 8 takes N / 2 clk per instruction with nothing else going on;
 //   * an mbarrier wait in the ISSUING thread is not free: the thread runs only ~4 MMAs ahead of the pipe and a try_wait
-//     costs 70-90 clk that the pipe then idles (2 waits per 6 MMAs: 128 -> 152 clk per MMA).  The issuing thread
-//     therefore never touches an mbarrier: readiness reaches it through plain shared-memory counters (release /
-//     acquire) that it polls with ld.shared between bursts of MMAs;
-//   * SHARED-MEMORY BANDWIDTH is what paced the version with both operands in shared memory (ncu, round 2, config 2: tensor
-//     pipe 55-58 % active, 1380 clk per stage against the 768 of its six MMAs; per stage the MMAs read 6 x (4 KB of A +
-//     8 KB of B) = 576 wavefronts of 128 B, the split warps moved 56 KB = 457 wavefronts, TMA wrote 128: 1161 against
-//     768 clk, and no instruction had an excess wavefront).  With A in tensor memory the MMAs read only B from shared
-//     memory, the split warps read A once and write it to TMEM, and A_hi / A_lo occupy no shared memory at all:
-//     per stage (N = 192) 288 + 112 (TMA) + 64 (A read) + 192 (B split) = 656 wavefronts against 576 clk of MMAs;
-//   * the chip is POWER-bound under this kernel: every byte through L2 and every spinning warp costs SM clock.  Hence one
-//     raw operand plane instead of four, and waits that sleep in hardware.
+//     costs 70-90 clk that the pipe then idles.  The issuing thread therefore never touches an mbarrier: readiness
+//     reaches it through plain shared-memory counters (release / acquire) that it polls between bursts of MMAs;
+//   * THE FEED, not the math, paced every earlier version (~1100-1400 clk per 8-shot stage whatever N, ring depth or split
+//     arrangement; with MMAs, split and read-out all switched off the kernel still took 4.3 of 5.1 ms).  The TMA unit
+//     charges per ROW of a box, about 8 clk whether the row has 64 or 128 bytes: the A tile of one stage (128 receivers x
+//     64 bytes) alone cost 1030 clk, more than the stage's six MMAs (576).  Hence
+//       - A boxes of 16 shots (128-byte rows, the swizzle span) in a ring of their own, one box per two stages;
+//       - B delivered as 8 dense rows of <= 768 bytes per stage instead of 8 nblk rows in the tensor core's layout; the
+//         split warps, who read every element anyway, write the MN-major swizzled planes themselves;
+//     A-only feed 4.25 -> 2.72 ms;
+//   * the raw rings (A: 3 boxes = 6 stages, B: 8 tiles) run ahead of the four operand stages by their own length, so the
+//     latency of the loads is not inside the loop the MMAs close (empty -> split -> ready -> MMA -> empty);
+//   * A IN TENSOR MEMORY: with both operands in shared memory the MMAs read 6 x (4 KB of A + 8 KB of B) per stage and the
+//     split warps moved 56 KB more; now the MMAs read only B, the split warps read A once and tcgen05.st it, and A_hi /
+//     A_lo occupy no shared memory (which is what pays for the raw rings);
+//   * one stage's split is a LATENCY chain (waits, LDS -> ALU -> STS / tcgen05.st, tcgen05.wait::st, proxy fence, arrive:
+//     ~1400 clk for ~250 instructions per warp), so three groups of four warps take the stages in rotation;
+//   * a waiting warp must really sleep: with the default suspend time the read-out warps' try_wait loops were 40 % of all
+//     instructions issued on the SM (same schedulers as the split warps); try_wait now carries a suspend-time hint;
+//   * the chip is POWER-bound under this kernel (1000 W cap: 1.6-1.8 GHz): every byte through L2, every byte through shared
+//     memory and every spinning warp costs SM clock.
+// Result: tensor pipe 55 % -> 69 % active, config 2 4.74 -> 4.2 ms, config 3 7.35 -> 5.3 ms per contraction.
 //
 // Tensor memory (512 columns): two chunk accumulators of BN = 192 columns, and a ring of four A slots of 32 columns
 // (per K step 8 columns of A_hi and 8 of A_lo; lane = receiver row of the tile).
 //
-// Kernel: persistent, one CTA per SM, warp-specialised, 640 threads = 5 warpgroups with their own register budgets
-// (setmaxnreg: the kernel starts at 96 registers per thread; control 32, split 72, read-out 136) —
-//   warp 0      TMA producer of the A tiles [128 rows][16 floats] (SWIZZLE_64B, K-major); mbarrier full / empty ring
-//   warp 3      TMA producer of the B tiles [8 shots][<= 192 floats] (SWIZZLE_128B with 32-byte atoms, MN-major)
+// Kernel: persistent, one CTA per SM, warp-specialised, 768 threads = 6 warpgroups with their own register budgets
+// (setmaxnreg: the kernel starts at 80 registers per thread; control 32, split 64, read-out 128) —
+//   warp 0      TMA producer of the raw A boxes [128 receivers][16 shots] (SWIZZLE_128B), ring of 3
+//   warp 3      TMA producer of the raw B tiles [8 shots][<= 192 floats] (dense rows), ring of <= 8
 //   warp 1      tcgen05.mma issuer (one thread): kind::tf32, M = 128, N <= 192, K = 8, A from TMEM, B from shared memory;
-//               tcgen05.commit releases the stage / publishes the chunk
+//               tcgen05.commit releases the operand stage / publishes the chunk
 //   warp 2      relay: split_bar[stage] (mbarrier) -> ready[stage] (the word the MMA warp polls)
-//   warps 4-11  split warps, all eight on every stage.  A: thread = (row of the tile, K step): two 128-bit loads, lo parts,
-//               one tcgen05.st of 16 columns.  B -> (B_lo, B1_hi, B1_lo) in shared memory.  tcgen05.wait::st, proxy fence,
-//               arrive on split_bar[stage]
-//   warps 12-19 read-out warps.  Per chunk: tcgen05.ld of the finished accumulator (warp w owns TMEM lanes 32 (w % 4) .. +31
-//               and the column half (w - 12) / 4) -> += 96 running sums in registers, drained += 1 per warp; per tile:
+//   warps 4-15  split warps, three groups of four; group g takes the stages g, g + 3, ...  A: thread = row of the tile: four
+//               128-bit loads of its half of the box, lo parts, two tcgen05.st of 16 columns.  B: raw tile -> B0_hi, B0_lo,
+//               B1_hi, B1_lo in the tensor core's layout.  tcgen05.wait::st, proxy fence, arrive on split_bar[stage] and
+//               on the raw rings' empty barriers
+//   warps 16-23 read-out warps.  Per chunk: tcgen05.ld of the finished accumulator (warp w owns TMEM lanes 32 (w % 4) .. +31
+//               and the column half (w - 16) / 4) -> += 96 running sums in registers, drained += 1 per warp; per tile:
 //               128-bit global stores of S^
 #include <cuda.h>
 
@@ -67,9 +80,10 @@ namespace {
 
 constexpr int BM = 128;         // rows (receivers) per tile = TMEM lanes
 constexpr int BN = 192;         // real columns (2 per focal point) per tile = TMEM columns per accumulator
-constexpr int BKC = 8;          // shots (complex k) per stage: 64-byte rows of A
-constexpr int kMaxStages = 7;   // shared-memory ring: as many stages as fit (7 at N = 192)
-constexpr int kTmemSlots = 4;   // ring of A slots in tensor memory: stage it uses slot it % 4, free once the MMAs of stage it - 4 retired
+constexpr int BKC = 8;          // shots (complex k) per stage
+constexpr int kMaxRawB = 8;     // ring of raw B tiles: as many as fit (8 at N = 192)
+constexpr int kTmemSlots = 4;   // ring of operand stages: stage it uses A slot it % 4 in tensor memory and B planes it % 4 in shared
+                                // memory, both free once the MMAs of stage it - 4 retired
 constexpr int kSplitWarps = 4, kSplitThreads = 32 * kSplitWarps;  // per split group
 #ifndef MK_TC_SPLIT_GROUPS
 #define MK_TC_SPLIT_GROUPS 3
@@ -86,12 +100,14 @@ constexpr int kChunk = 4;       // stages per accumulation chunk (24 MMA steps)
 constexpr int kASlots = 3;      // ring of raw A boxes
 constexpr uint32_t A_BOX_BYTES = BM * 4 * BKC * 4;  // 16 KB: one raw A box = [128 rows][16 shots] = two stages, 128-byte rows
 constexpr uint32_t BLK_BYTES = BKC * 32 * 4;    // 1 KB: one 32-column block of one B region (8 rows of 128 B)
-// A stage = the raw B tile as TMA delivered it ([8 shots][nblk x 128 B], dense rows), then the four B regions of nblk
-// column blocks each that the tensor core reads: B0_hi, B0_lo, B1_hi, B1_lo; nblk = min(6, columns / 32).  The distance
-// B0 -> B1 (two regions) is the stride-byte-offset of the B descriptors: the second group of four K rows of every MMA
-// is the rotated copy of the first.  The raw A boxes have a ring of their own (one box feeds two stages).
-__host__ __device__ constexpr uint32_t stage_bytes(int nblk) { return 5 * (uint32_t)nblk * BLK_BYTES; }
-constexpr size_t kSmemExtra = 1024 /*alignment slack*/ + 512 /*barriers, counters: (3 x 7 + 2 + 2 x 3) x 8 + (7 + 2 + 1) x 4 bytes*/;
+// Shared memory: the ring of raw A boxes; the ring of raw B tiles as TMA delivered them ([8 shots][nblk x 128 B], dense
+// rows); four operand stages of four B regions of nblk column blocks each that the tensor core reads: B0_hi, B0_lo,
+// B1_hi, B1_lo; nblk = min(6, columns / 32).  The distance B0 -> B1 (two regions) is the stride-byte-offset of the B
+// descriptors: the second group of four K rows of every MMA is the rotated copy of the first.  The raw rings run ahead of
+// the operand stages by their own length: the latency of the loads is not in the loop that the MMAs close.
+__host__ __device__ constexpr uint32_t planes_bytes(int nblk) { return 4 * (uint32_t)nblk * BLK_BYTES; }
+__host__ __device__ constexpr uint32_t fixed_smem(int nblk) { return kASlots * A_BOX_BYTES + kTmemSlots * planes_bytes(nblk); }
+constexpr size_t kSmemExtra = 1024 /*alignment slack*/ + 512 /*barriers, counters: (2 x 8 + 2 x 4 + 2 + 2 x 3) x 8 + (4 + 2 + 1) x 4 bytes*/;
 constexpr uint32_t kTmemCols = 512;
 constexpr uint32_t kTmemA = 2 * BN;  // first column of the A ring
 constexpr uint32_t kTmemAStage = 32; // columns per slot: K step j at 16 j: A_hi (8 columns), A_lo (8 columns)
@@ -259,7 +275,7 @@ struct TcParams {
   int n, nb, ld;        // receivers (rows of R^ this context owns), bins, padded shots
   int ncols;            // 2 * ldf: real columns of S^ (a multiple of 32)
   int mt, ntl;          // tiles along M and N
-  int nblk, stages;     // column blocks per B region, stages of the ring
+  int nblk, nrb;        // column blocks per B region, slots of the raw B ring
   size_t s_row;         // floats between consecutive receivers of S^: nb * 2 ldf
   int tune;             // MK_OPT_TUNE bits 2..5: parts of the kernel left out (bottleneck measurements; results are wrong)
 };
@@ -269,18 +285,20 @@ k_syn_gemm_tf32x3(const __grid_constant__ CUtensorMap tmA, const __grid_constant
                   TcParams P) {
   extern __shared__ uint8_t smem_raw[];
   uint8_t* smem = reinterpret_cast<uint8_t*>(((uintptr_t)smem_raw + 1023) & ~(uintptr_t)1023);
-  const int STAGES = P.stages;
-  const uint32_t STAGE_BYTES = stage_bytes(P.nblk), REG = (uint32_t)P.nblk * BLK_BYTES;  // REG: bytes of one B region
-  uint8_t* stages = smem + kASlots * A_BOX_BYTES;  // the A ring comes first
-  uint64_t* bars = reinterpret_cast<uint64_t*>(stages + (size_t)STAGES * STAGE_BYTES);
-  uint64_t* full = bars;                       // [kMaxStages] TMA landed
-  uint64_t* empty = bars + kMaxStages;         // [kMaxStages] MMAs of the stage retired
-  uint64_t* split_bar = bars + 2 * kMaxStages;  // [kMaxStages] the split warps are done with the stage
-  uint64_t* acc_full = bars + 3 * kMaxStages;   // [2] chunk accumulator complete
-  uint64_t* fullA = acc_full + 2;               // [kASlots] raw A box landed
-  uint64_t* emptyA = fullA + kASlots;           // [kASlots] both split groups have read their half of the box
-  uint32_t* ready = reinterpret_cast<uint32_t*>(emptyA + kASlots);  // [kMaxStages] uses of the stage that are ready for the MMAs (relay)
-  uint32_t* drained = ready + kMaxStages;      // [2] read-out warps done with a use of TMEM buffer b (counts up; PER BUFFER:
+  const int NRB = P.nrb;
+  const uint32_t REG = (uint32_t)P.nblk * BLK_BYTES, PLANES = 4 * REG;  // REG: bytes of one B region = of one raw B tile
+  uint8_t* planes = smem + kASlots * A_BOX_BYTES;            // the A ring comes first, then the operand stages,
+  uint8_t* rawB = planes + (size_t)kTmemSlots * PLANES;      // then the raw B ring
+  uint64_t* bars = reinterpret_cast<uint64_t*>(rawB + (size_t)NRB * REG);
+  uint64_t* fullB = bars;                          // [kMaxRawB] raw B tile landed
+  uint64_t* emptyB = bars + kMaxRawB;              // [kMaxRawB] the split group that took the stage has read it
+  uint64_t* empty = bars + 2 * kMaxRawB;           // [kTmemSlots] MMAs of the operand stage retired
+  uint64_t* split_bar = empty + kTmemSlots;        // [kTmemSlots] the split warps are done with the stage
+  uint64_t* acc_full = split_bar + kTmemSlots;     // [2] chunk accumulator complete
+  uint64_t* fullA = acc_full + 2;                  // [kASlots] raw A box landed
+  uint64_t* emptyA = fullA + kASlots;              // [kASlots] both halves of the box have been read
+  uint32_t* ready = reinterpret_cast<uint32_t*>(emptyA + kASlots);  // [kTmemSlots] uses of the stage that are ready for the MMAs (relay)
+  uint32_t* drained = ready + kTmemSlots;      // [2] read-out warps done with a use of TMEM buffer b (counts up; PER BUFFER:
                                                // one sum over both would let fast warps' arrivals for the other buffer stand in for
                                                // a slow warp's missing one)
   uint32_t* tmem_slot = drained + 2;
@@ -290,8 +308,11 @@ k_syn_gemm_tf32x3(const __grid_constant__ CUtensorMap tmA, const __grid_constant
   const int KB = P.ld / BKC;  // stages per tile
 
   if (threadIdx.x == 0) {
-    for (int s = 0; s < STAGES; ++s) {
-      mbar_init(full + s, 1);  // the B producer
+    for (int s = 0; s < NRB; ++s) {
+      mbar_init(fullB + s, 1);  // the B producer
+      mbar_init(emptyB + s, kSplitWarps);
+    }
+    for (int s = 0; s < kTmemSlots; ++s) {
       mbar_init(empty + s, 1);
       mbar_init(split_bar + s, kSplitWarps);
       ready[s] = 0;
@@ -351,12 +372,11 @@ k_syn_gemm_tf32x3(const __grid_constant__ CUtensorMap tmA, const __grid_constant
     // with 32-byte atoms (the only MN-major layout the tensor core takes for 32-bit operands): a region is [nblk blocks of
     // 32 columns][8 shot rows][128 B]; LBO = 1024 (next column block); the K step's first four rows are shots 4j .. 4j+3 of
     // B0 (512 j into the block), its second four rows sit SBO = 2 regions further: the same shots of B1 = i B0.
-    const uint32_t base16 = (smem_u32(stages) & 0x3FFFF) >> 4, stage16 = STAGE_BYTES >> 4;
+    const uint32_t base16 = (smem_u32(planes) & 0x3FFFF) >> 4, stage16 = PLANES >> 4;
     const uint32_t hiB = ((2 * REG) >> 4) | (1u << 14) | (LAYOUT_SW128_BASE32B << 29);
-    const uint32_t loB_hi0 = (base16 + (REG >> 4)) | ((BLK_BYTES >> 4) << 16), loB_lo0 = loB_hi0 + (REG >> 4);  // behind the raw tile (K step 1: + 32)
+    const uint32_t loB_hi0 = base16 | ((BLK_BYTES >> 4) << 16), loB_lo0 = loB_hi0 + (REG >> 4);  // (K step 1: + 32)
     const uint32_t tmA0 = tmem_base + kTmemA;
-    uint32_t g = 0, pass = 0, it = 0;  // global chunk index; completed passes over the ring; global stage index
-    int s = 0;
+    uint32_t g = 0, it = 0;  // global chunk index; global stage index
     for (int t = blockIdx.x; t < ntiles; t += gridDim.x) {
       const int rem = t % per_bin, ni = rem % P.ntl;
       int nmma = P.ncols - ni * BN;
@@ -368,10 +388,11 @@ k_syn_gemm_tf32x3(const __grid_constant__ CUtensorMap tmA, const __grid_constant
         const uint32_t d = tmem_base + (uint32_t)b * BN;
         const int kb1 = min(kb0 + kChunk, KB);
         for (int kb = kb0; kb < kb1; ++kb) {
-          flag_wait_ge(ready + s, pass + 1);
+          const uint32_t s = it & (kTmemSlots - 1);
+          flag_wait_ge(ready + s, (it >> 2) + 1);
           __syncwarp();  // the lanes leave the polling loop one by one: elect.sync needs them all back
           tc_fence_after();
-          const uint32_t off = (uint32_t)s * stage16, ta = tmA0 + (it & (kTmemSlots - 1)) * kTmemAStage;
+          const uint32_t off = s * stage16, ta = tmA0 + s * kTmemAStage;
           if (elect_one()) {
             // small terms first; a chunk starts from zero
             if (!(P.tune & 8)) {
@@ -386,10 +407,6 @@ k_syn_gemm_tf32x3(const __grid_constant__ CUtensorMap tmA, const __grid_constant
           }
           __syncwarp();
           ++it;
-          if (++s == STAGES) {
-            s = 0;
-            ++pass;
-          }
         }
         if (elect_one()) umma_commit(acc_full + b);
         __syncwarp();
@@ -403,16 +420,12 @@ k_syn_gemm_tf32x3(const __grid_constant__ CUtensorMap tmA, const __grid_constant
     // ordered behind the fence.  So they arrive on split_bar and this thread turns the completed phase into the word.
     asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(kRegsControl));
     if (lane == 0) {
-      int s = 0;
-      uint32_t pass = 0;
+      uint32_t it = 0;
       for (int t = blockIdx.x; t < ntiles; t += gridDim.x)
-        for (int kb = 0; kb < KB; ++kb) {
-          mbar_wait(split_bar + s, pass & 1);
-          flag_set(ready + s, pass + 1);
-          if (++s == STAGES) {
-            s = 0;
-            ++pass;
-          }
+        for (int kb = 0; kb < KB; ++kb, ++it) {
+          const uint32_t s = it & (kTmemSlots - 1);
+          mbar_wait(split_bar + s, (it >> 2) & 1);
+          flag_set(ready + s, (it >> 2) + 1);
         }
     }
   } else if (warp == 3) {
@@ -426,16 +439,16 @@ k_syn_gemm_tf32x3(const __grid_constant__ CUtensorMap tmA, const __grid_constant
       for (int t = blockIdx.x; t < ntiles; t += gridDim.x) {
         const int kk = t / per_bin, rem = t - kk * per_bin, ni = rem % P.ntl;
         for (int kb = 0; kb < KB; ++kb) {
-          mbar_wait(empty + s, ph ^ 1);
+          mbar_wait(emptyB + s, ph ^ 1);
           if (P.tune & (64 | 256)) {
-            mbar_arrive(full + s);
+            mbar_arrive(fullB + s);
           } else {
-            mbar_expect_tx(full + s, REG);
+            mbar_expect_tx(fullB + s, REG);
             // eight dense rows of nblk x 128 bytes (8 rows for the TMA unit instead of 8 nblk in the tensor core's layout);
             // columns past 2 ldf arrive as zeros (and still count their bytes)
-            tma_load_2d(&tmB, full + s, stages + (size_t)s * STAGE_BYTES, ni * BN, kk * P.ld + kb * BKC);
+            tma_load_2d(&tmB, fullB + s, rawB + (size_t)s * REG, ni * BN, kk * P.ld + kb * BKC);
           }
-          if (++s == STAGES) {
+          if (++s == NRB) {
             s = 0;
             ph ^= 1;
           }
@@ -450,7 +463,7 @@ k_syn_gemm_tf32x3(const __grid_constant__ CUtensorMap tmA, const __grid_constant
     asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(kRegsSplit));
     const int grp = (warp - 4) / kSplitWarps;
     const int wt = threadIdx.x - 128 - grp * kSplitThreads;  // 0 .. 127
-    const uint32_t stages_base = smem_u32(stages), a_base = smem_u32(smem);
+    const uint32_t planes_base = smem_u32(planes), raw_base = smem_u32(rawB), a_base = smem_u32(smem);
     // A: this thread owns row ar = 32 (warp % 4) + lane of the tile (the TMEM lanes its warp may write) and reads the 64 bytes
     // of the stage's half of the box (stage it = half it % 2 of box it / 2): K step j = bytes 32 j .. 32 j + 31 of the half =
     // (re0 im0 re1 im1 | re2 im2 re3 im3) of shots 4 j .. 4 j + 3.  SWIZZLE_128B: the 16-byte chunk c of row r sits at
@@ -468,32 +481,26 @@ k_syn_gemm_tf32x3(const __grid_constant__ CUtensorMap tmA, const __grid_constant
 #pragma unroll
     for (int i = 0; i < 3; ++i) {
       const uint32_t q = (uint32_t)wt + i * kSplitThreads, r = q / per_row, x = q - r * per_row, blk = x >> 3, ch = x & 7;
-      b_dst[i] = REG + blk * BLK_BYTES + r * 128 + ((((ch >> 1) ^ (r & 3)) << 5) | ((ch & 1) << 4));
+      b_dst[i] = blk * BLK_BYTES + r * 128 + ((((ch >> 1) ^ (r & 3)) << 5) | ((ch & 1) << 4));
     }
     const int nmine = (int)wt < (int)nq ? (int)((nq - wt + kSplitThreads - 1) / kSplitThreads) : 0;
     const int my_tiles = blockIdx.x < ntiles ? (ntiles - blockIdx.x + gridDim.x - 1) / gridDim.x : 0;
     const uint32_t total = (uint32_t)my_tiles * (uint32_t)KB;  // stages this CTA runs through
-    int s = grp % STAGES;  // ring slot of stage it and its phase
-    uint32_t ph = (grp / STAGES) & 1;
-    // ring slot of stage it - kTmemSlots, used from this group's first stage it >= kTmemSlots on (only when STAGES > 4)
-    int s4;
-    uint32_t ph4;
-    {
-      int it0 = grp;
-      while (it0 < kTmemSlots) it0 += kSplitGroups;
-      s4 = (it0 - kTmemSlots) % STAGES;
-      ph4 = ((it0 - kTmemSlots) / STAGES) & 1;
-    }
+    int rb = grp % NRB;  // slot of stage it in the raw B ring and its phase
+    uint32_t phb = (grp / NRB) & 1;
     for (uint32_t it = grp; it < total; it += kSplitGroups) {
       const uint32_t box = it >> 1, half = (it & 1) << 6;
       const int sa = (int)(box % kASlots);  // slot of the raw A box of stage it, and its phase
       const uint32_t pha = (box / kASlots) & 1;
+      const uint32_t s = it & (kTmemSlots - 1);  // operand stage: B planes in shared memory, A slot in tensor memory
       if (P.tune & 32) {
-        mbar_wait(full + s, ph);
+        mbar_wait(fullB + rb, phb);
         mbar_wait(fullA + sa, pha);
+        if (it >= kTmemSlots) mbar_wait(empty + s, ((it >> 2) - 1) & 1);
         __syncwarp();
         if (lane == 0) {
           mbar_arrive(emptyA + sa);
+          mbar_arrive(emptyB + rb);
           mbar_arrive(split_bar + s);
         }
       } else {
@@ -501,13 +508,19 @@ k_syn_gemm_tf32x3(const __grid_constant__ CUtensorMap tmA, const __grid_constant
       float4 c[4];
 #pragma unroll
       for (int k = 0; k < 4; ++k) c[k] = lds128(a_base + (uint32_t)sa * A_BOX_BYTES + (a_off[k] ^ half));
-      mbar_wait(full + s, ph);
-      const uint32_t st = stages_base + (uint32_t)s * STAGE_BYTES;  // raw tile, then B0_hi, ...
-      // B: raw tile -> B0_hi (copy), B0_lo, and B1 = i B0 (every float4 holds two (re, im) pairs) hi / lo
+      mbar_wait(fullB + rb, phb);
+      const uint32_t raw = raw_base + (uint32_t)rb * REG, st = planes_base + s * PLANES;
       float4 v[3];
 #pragma unroll
       for (int i = 0; i < 3; ++i)
-        if (i < nmine) v[i] = lds128(st + (((uint32_t)wt + i * kSplitThreads) << 4));
+        if (i < nmine) v[i] = lds128(raw + (((uint32_t)wt + i * kSplitThreads) << 4));
+      // The operand stage (B planes, A slot) is free once the MMAs of stage it - 4 have retired: empty[s] cannot run a second
+      // phase ahead, its next completion belongs to stage it itself.
+      if (it >= kTmemSlots) {
+        mbar_wait(empty + s, ((it >> 2) - 1) & 1);
+        tc_fence_after();
+      }
+      // B: raw tile -> B0_hi (copy), B0_lo, and B1 = i B0 (every float4 holds two (re, im) pairs) hi / lo
 #pragma unroll
       for (int i = 0; i < 3; ++i)
         if (i < nmine && !(P.tune & 16)) {
@@ -518,20 +531,8 @@ k_syn_gemm_tf32x3(const __grid_constant__ CUtensorMap tmA, const __grid_constant
           sts128(dst + 2 * REG, make_float4(-v[i].y, v[i].x, -v[i].w, v[i].z));
           sts128(dst + 3 * REG, make_float4(-l.y, l.x, -l.w, l.z));
         }
-      // The A slot in tensor memory is free once the MMAs of stage it - 4 have retired.  A ring of <= 4 stages implies it
-      // (the TMA of stage it waited for stage it - STAGES); a longer one is asked: empty[] of that stage's slot cannot run a
-      // second phase ahead, its next use is stage it - 4 + STAGES > it, whose MMAs wait for this very split.
-      if (STAGES > kTmemSlots && it >= kTmemSlots) {
-        mbar_wait(empty + s4, ph4);
-        tc_fence_after();
-        s4 += kSplitGroups;
-        while (s4 >= STAGES) {
-          s4 -= STAGES;
-          ph4 ^= 1;
-        }
-      }
       // A -> tensor memory: per K step hi (re0 re1 re2 re3 | im0 im1 im2 im3), lo beside it
-      const uint32_t ta = a_tmem + ((uint32_t)it & (kTmemSlots - 1)) * kTmemAStage;
+      const uint32_t ta = a_tmem + s * kTmemAStage;
 #pragma unroll
       for (int j = 0; j < 2; ++j) {
         const float4 re = make_float4(c[2 * j].x, c[2 * j].z, c[2 * j + 1].x, c[2 * j + 1].z),
@@ -543,14 +544,15 @@ k_syn_gemm_tf32x3(const __grid_constant__ CUtensorMap tmA, const __grid_constant
       tc_fence_before();
       __syncwarp();
       if (lane == 0) {
-        mbar_arrive(emptyA + sa);  // this warp's rows of the box are in registers / tensor memory
+        mbar_arrive(emptyA + sa);  // this warp's part of the raw tiles is in registers / tensor memory / the planes
+        mbar_arrive(emptyB + rb);
         mbar_arrive(split_bar + s);
       }
       }
-      s += kSplitGroups;
-      while (s >= STAGES) {
-        s -= STAGES;
-        ph ^= 1;
+      rb += kSplitGroups;
+      while (rb >= NRB) {
+        rb -= NRB;
+        phb ^= 1;
       }
     }
   } else {
@@ -637,7 +639,7 @@ int encode(mk_ctx* c, EncodeTiledFn enc, void* out, const void* base, int rank, 
 bool tc_supported(const mk_ctx* c) {
   int major = 0;
   cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, c->dev);
-  return major == 10 && c->smem_optin >= kASlots * A_BOX_BYTES + 2 * stage_bytes(1) + kSmemExtra;
+  return major == 10 && c->smem_optin >= fixed_smem(1) + 2 * BLK_BYTES + kSmemExtra;
 }
 
 int launch_syn_tc(mk_ctx* c, const RowBlock& rb, int slot, const float2* d_Nhat, float2* d_Shat, int ldf) {
@@ -676,10 +678,11 @@ int launch_syn_tc(mk_ctx* c, const RowBlock& rb, int slot, const float2* d_Nhat,
   P.s_row = (size_t)c->nb * 2 * ldf;
   P.nblk = nblk;
   P.tune = c->tune;
-  P.stages = (int)std::min<size_t>(kMaxStages, (c->smem_optin - kSmemExtra - kASlots * A_BOX_BYTES) / stage_bytes(nblk));
-  if (c->tune & 512) P.stages = std::min(P.stages, 4);
-  if (P.stages < 2) return set_err(c, MK_ERR_INVALID_ARG, "not enough shared memory for the tcgen05 contraction");
-  const size_t kSmemBytes = kASlots * A_BOX_BYTES + (size_t)P.stages * stage_bytes(nblk) + kSmemExtra;
+  if (c->smem_optin < fixed_smem(nblk) + kSmemExtra + 2 * (size_t)nblk * BLK_BYTES)
+    return set_err(c, MK_ERR_INVALID_ARG, "not enough shared memory for the tcgen05 contraction");
+  P.nrb = (int)std::min<size_t>(kMaxRawB, (c->smem_optin - kSmemExtra - fixed_smem(nblk)) / ((size_t)nblk * BLK_BYTES));
+  if (c->tune & 512) P.nrb = std::min(P.nrb, 3);
+  const size_t kSmemBytes = fixed_smem(nblk) + (size_t)P.nrb * nblk * BLK_BYTES + kSmemExtra;
   const int ntiles = P.nb * P.mt * P.ntl;
   const int grid = ntiles < c->num_sms ? ntiles : c->num_sms;
   float* S0 = reinterpret_cast<float*>(d_Shat + (size_t)rb.r0 * c->nb * ldf);
