@@ -47,6 +47,11 @@
 //     ~1400 clk for ~250 instructions per warp), so three groups of four warps take the stages in rotation;
 //   * a waiting warp must really sleep: with the default suspend time the read-out warps' try_wait loops were 40 % of all
 //     instructions issued on the SM (same schedulers as the split warps); try_wait now carries a suspend-time hint;
+//   * NOT the depth of the operand ring: with every load, MMA, split and read-out switched off the barrier chain alone
+//     (empty[s] -> split -> split_bar -> relay -> ready -> MMA issue -> tcgen05.commit) takes 1.83 ms = 443 clk per stage,
+//     but N tiles of 128 columns with EIGHT operand stages (-DMK_TC_BN=128) are slower on every config (config 2 4.94 ms,
+//     config 3 5.33, config 4 70.1 against 4.21 / 5.20 / 66.7), and waking the waiters without a suspend hint changes
+//     nothing.  What holds config 3 at ~650 clk per stage against 384 clk of MMAs is not identified;
 //   * the chip is POWER-bound under this kernel (1000 W cap: 1.6-1.8 GHz): every byte through L2, every byte through shared
 //     memory and every spinning warp costs SM clock.
 // Result: tensor pipe 55 % -> 69 % active, config 2 4.74 -> 4.2 ms, config 3 7.35 -> 5.3 ms per contraction.
@@ -78,11 +83,14 @@ namespace mk {
 
 namespace {
 
+#ifndef MK_TC_BN
+#define MK_TC_BN 192
+#endif
 constexpr int BM = 128;         // rows (receivers) per tile = TMEM lanes
-constexpr int BN = 192;         // real columns (2 per focal point) per tile = TMEM columns per accumulator
+constexpr int BN = MK_TC_BN;    // real columns (2 per focal point) per tile = TMEM columns per accumulator (128 or 192)
 constexpr int BKC = 8;          // shots (complex k) per stage
 constexpr int kMaxRawB = 8;     // ring of raw B tiles: as many as fit (8 at N = 192)
-constexpr int kTmemSlots = 4;   // ring of operand stages: stage it uses A slot it % 4 in tensor memory and B planes it % 4 in shared
+constexpr int kTmemSlots = MK_TC_BN == 128 ? 8 : 4, kLgSlots = MK_TC_BN == 128 ? 3 : 2;  // ring of operand stages: stage it uses A slot it % 4 in tensor memory and B planes it % 4 in shared
                                 // memory, both free once the MMAs of stage it - 4 retired
 constexpr int kSplitWarps = 4, kSplitThreads = 32 * kSplitWarps;  // per split group
 #ifndef MK_TC_SPLIT_GROUPS
@@ -389,7 +397,7 @@ k_syn_gemm_tf32x3(const __grid_constant__ CUtensorMap tmA, const __grid_constant
         const int kb1 = min(kb0 + kChunk, KB);
         for (int kb = kb0; kb < kb1; ++kb) {
           const uint32_t s = it & (kTmemSlots - 1);
-          flag_wait_ge(ready + s, (it >> 2) + 1);
+          flag_wait_ge(ready + s, (it >> kLgSlots) + 1);
           __syncwarp();  // the lanes leave the polling loop one by one: elect.sync needs them all back
           tc_fence_after();
           const uint32_t off = s * stage16, ta = tmA0 + s * kTmemAStage;
@@ -424,8 +432,8 @@ k_syn_gemm_tf32x3(const __grid_constant__ CUtensorMap tmA, const __grid_constant
       for (int t = blockIdx.x; t < ntiles; t += gridDim.x)
         for (int kb = 0; kb < KB; ++kb, ++it) {
           const uint32_t s = it & (kTmemSlots - 1);
-          mbar_wait(split_bar + s, (it >> 2) & 1);
-          flag_set(ready + s, (it >> 2) + 1);
+          mbar_wait(split_bar + s, (it >> kLgSlots) & 1);
+          flag_set(ready + s, (it >> kLgSlots) + 1);
         }
     }
   } else if (warp == 3) {
@@ -496,7 +504,7 @@ k_syn_gemm_tf32x3(const __grid_constant__ CUtensorMap tmA, const __grid_constant
       if (P.tune & 32) {
         mbar_wait(fullB + rb, phb);
         mbar_wait(fullA + sa, pha);
-        if (it >= kTmemSlots) mbar_wait(empty + s, ((it >> 2) - 1) & 1);
+        if (it >= kTmemSlots) mbar_wait(empty + s, ((it >> kLgSlots) - 1) & 1);
         __syncwarp();
         if (lane == 0) {
           mbar_arrive(emptyA + sa);
@@ -517,7 +525,7 @@ k_syn_gemm_tf32x3(const __grid_constant__ CUtensorMap tmA, const __grid_constant
       // The operand stage (B planes, A slot) is free once the MMAs of stage it - 4 have retired: empty[s] cannot run a second
       // phase ahead, its next completion belongs to stage it itself.
       if (it >= kTmemSlots) {
-        mbar_wait(empty + s, ((it >> 2) - 1) & 1);
+        mbar_wait(empty + s, ((it >> kLgSlots) - 1) & 1);
         tc_fence_after();
       }
       // B: raw tile -> B0_hi (copy), B0_lo, and B1 = i B0 (every float4 holds two (re, im) pairs) hi / lo
