@@ -79,7 +79,8 @@ enum {
                              tcgen05 contraction to find what bounds it; the RESULTS ARE WRONG with any of them: 4 = the
                              read-out warps do not read tensor memory, 8 = no MMA is issued, 16 = the split warps skip the
                              B planes, 32 = the split warps do nothing, 64 = no TMA load is issued,
-                             128 = no A tile is loaded, 256 = no B tile is loaded */
+                             128 = no A tile is loaded, 256 = no B tile is loaded.  512: the raw B ring has 3 slots; 1024: the CTAs
+                             that share an A tile keep in step through global progress counters (same results, slower) */
 };
 
 /* mk_get_info keys (values returned as double) */

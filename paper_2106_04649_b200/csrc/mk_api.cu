@@ -488,6 +488,7 @@ int mk_destroy(mk_ctx* c) {
   cudaFree(c->d_Rscale);
   cudaFree(c->d_qstage);
   cudaFree(c->d_img_part);
+  cudaFree(c->d_tc_progress);
   cudaFree(c->d_win[0]);
   cudaFree(c->d_win[1]);
   if (c->h2d_stream) {

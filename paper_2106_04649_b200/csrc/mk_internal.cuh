@@ -93,6 +93,7 @@ struct mk_ctx {
   int tmap_A_rows[3] = {0, 0, 0};
   const void* tmap_B_key[2] = {nullptr, nullptr};
   int tmap_B_ldf[2] = {0, 0};
+  uint32_t* d_tc_progress = nullptr;  // tcgen05 contraction: A boxes asked for, per CTA (sibling CTAs keep in step)
   void* encode_fn = nullptr;  // cuTensorMapEncodeTiled, resolved at run time through the CUDA runtime
   float* d_stage = nullptr;  // host-call staging
   double* d_img_part = nullptr;  // mk_image: per (focal point, receiver chunk) partial sums

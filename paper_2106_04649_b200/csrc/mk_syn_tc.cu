@@ -282,11 +282,16 @@ __device__ __forceinline__ float4 lo4(float4 v) { return make_float4(lo_part(v.x
 struct TcParams {
   int n, nb, ld;        // receivers (rows of R^ this context owns), bins, padded shots
   int ncols;            // 2 * ldf: real columns of S^ (a multiple of 32)
-  int mt, ntl;          // tiles along M and N
+  int mt, ntl;          // tiles along M and N; N tile ni covers the 32-column blocks [ni nblocks / ntl, (ni + 1) nblocks / ntl):
+                        // widths differ by at most one block, so the CTAs that share an A tile run in step and meet in L2
+  int nblocks;          // ncols / 32
   int nblk, nrb;        // column blocks per B region, slots of the raw B ring
   size_t s_row;         // floats between consecutive receivers of S^: nb * 2 ldf
+  uint32_t* progress;   // [grid] raw A boxes each CTA has asked for (zeroed before the launch); NULL when ntl == 1
   int tune;             // MK_OPT_TUNE bits 2..5: parts of the kernel left out (bottleneck measurements; results are wrong)
 };
+
+__device__ __forceinline__ int tile_col0(const TcParams& P, int ni) { return 32 * ((ni * P.nblocks) / P.ntl); }
 
 __global__ void __launch_bounds__(kThreads, 1)
 k_syn_gemm_tf32x3(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB, float* __restrict__ Shat,
@@ -350,13 +355,39 @@ k_syn_gemm_tf32x3(const __grid_constant__ CUtensorMap tmA, const __grid_constant
     // One box = [128 receivers][16 shots] = 128 rows of 128 bytes (SWIZZLE_128B) feeds two stages: the TMA unit's cost is
     // per ROW of a box (measured: ~8 clk per row whether it has 64 or 128 bytes; 128 rows x 64 B per 8-shot stage alone
     // took 1030 clk, more than the stage's MMAs), so rows are made as long as the swizzle span allows.
+    // The ntl CTAs that work on the N tiles of one (bin, receiver tile) read the SAME A boxes.  Left alone they drift apart
+    // by more than the L2 holds (measured on config 4: 155 GB from DRAM per launch for 62 GB of operands: every N tile
+    // reads R^ from HBM again).  MK_OPT_TUNE bit 10 keeps them in step — the grid is a multiple of ntl, CTA b's siblings
+    // are the ntl-aligned group around it (same tiles, other ni), every CTA publishes how many boxes it has asked for and
+    // nobody runs more than kLead boxes ahead of its slowest sibling — and DRAM reads do drop (155 -> 104 GB), but every
+    // CTA then moves at the pace of the momentarily slowest of its group: config 4 66 -> 82 ms, config 2 4.2 -> 5.3 ms.
+    // Off by default; the remedy that does not couple the CTAs' pace is a cluster with the A box multicast (not built).
     if (lane == 0) {
       int a = 0;
       uint32_t ph = 0;  // ring position and its phase
       const int KB2 = KB / 2;
+      uint32_t q = 0;   // boxes asked for so far
+      const int sib0 = (int)blockIdx.x - (int)blockIdx.x % P.ntl;
+      constexpr uint32_t kLead = 16, kEvery = 8;  // looked at every 8th box only: a look is ntl - 1 round trips to L2
       for (int t = blockIdx.x; t < ntiles; t += gridDim.x) {
         const int kk = t / per_bin, rem = t - kk * per_bin, mi = rem / P.ntl;
-        for (int kb2 = 0; kb2 < KB2; ++kb2) {
+        for (int kb2 = 0; kb2 < KB2; ++kb2, ++q) {
+          if (P.progress && q >= kLead && q % kEvery == 0) {
+#if MK_MBAR_TIMEOUT_CYCLES > 0
+            const long long t0 = clock64();
+#endif
+            for (int j = 0; j < P.ntl; ++j) {
+              if (sib0 + j == (int)blockIdx.x) continue;
+              for (;;) {
+                uint32_t v;
+                asm volatile("ld.relaxed.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(P.progress + sib0 + j) : "memory");
+                if (v + kLead > q) break;
+#if MK_MBAR_TIMEOUT_CYCLES > 0
+                if (clock64() - t0 > MK_MBAR_TIMEOUT_CYCLES) __trap();
+#endif
+              }
+            }
+          }
           mbar_wait(emptyA + a, ph ^ 1);
           if (P.tune & (64 | 128)) {
             mbar_arrive(fullA + a);
@@ -364,6 +395,8 @@ k_syn_gemm_tf32x3(const __grid_constant__ CUtensorMap tmA, const __grid_constant
             mbar_expect_tx(fullA + a, A_BOX_BYTES);
             tma_load_3d(&tmA, fullA + a, smem + (size_t)a * A_BOX_BYTES, kb2 * 4 * BKC, kk, mi * BM);  // rows past the last receiver arrive as zeros
           }
+          if (P.progress && (q + 1) % kEvery == 0)
+            asm volatile("st.relaxed.gpu.global.u32 [%0], %1;" ::"l"(P.progress + blockIdx.x), "r"(q + 1) : "memory");
           if (++a == kASlots) {
             a = 0;
             ph ^= 1;
@@ -387,9 +420,7 @@ k_syn_gemm_tf32x3(const __grid_constant__ CUtensorMap tmA, const __grid_constant
     uint32_t g = 0, it = 0;  // global chunk index; global stage index
     for (int t = blockIdx.x; t < ntiles; t += gridDim.x) {
       const int rem = t % per_bin, ni = rem % P.ntl;
-      int nmma = P.ncols - ni * BN;
-      nmma = nmma > BN ? BN : ((nmma + 15) / 16) * 16;
-      const uint32_t idesc = instr_desc((uint32_t)nmma);
+      const uint32_t idesc = instr_desc((uint32_t)(tile_col0(P, ni + 1) - tile_col0(P, ni)));  // a multiple of 32, <= BN
       for (int kb0 = 0; kb0 < KB; kb0 += kChunk, ++g) {
         const int b = g & 1;
         if (g >= 2) flag_wait_ge(drained + b, kReadWarps * (g >> 1));  // every earlier chunk of this buffer has been read out
@@ -454,7 +485,7 @@ k_syn_gemm_tf32x3(const __grid_constant__ CUtensorMap tmA, const __grid_constant
             mbar_expect_tx(fullB + s, REG);
             // eight dense rows of nblk x 128 bytes (8 rows for the TMA unit instead of 8 nblk in the tensor core's layout);
             // columns past 2 ldf arrive as zeros (and still count their bytes)
-            tma_load_2d(&tmB, fullB + s, rawB + (size_t)s * REG, ni * BN, kk * P.ld + kb * BKC);
+            tma_load_2d(&tmB, fullB + s, rawB + (size_t)s * REG, tile_col0(P, ni), kk * P.ld + kb * BKC);
           }
           if (++s == NRB) {
             s = 0;
@@ -571,7 +602,8 @@ k_syn_gemm_tf32x3(const __grid_constant__ CUtensorMap tmA, const __grid_constant
     uint32_t g = 0;
     for (int t = blockIdx.x; t < ntiles; t += gridDim.x) {
       const int kk = t / per_bin, rem = t - kk * per_bin, mi = rem / P.ntl, ni = rem - mi * P.ntl;
-      const int cols = P.ncols - ni * BN - half * (BN / 2);  // valid columns of this warp's half (may exceed BN / 2, may be <= 0)
+      const int col0 = tile_col0(P, ni);
+      const int cols = tile_col0(P, ni + 1) - col0 - half * (BN / 2);  // valid columns of this warp's half (may exceed BN / 2, may be <= 0)
       float sum[BN / 2];
 #pragma unroll
       for (int i = 0; i < BN / 2; ++i) sum[i] = 0.f;
@@ -596,7 +628,7 @@ k_syn_gemm_tf32x3(const __grid_constant__ CUtensorMap tmA, const __grid_constant
       }
       const int r = mi * BM + quad * 32 + lane;
       if (r < P.n) {
-        float* dst = Shat + (size_t)r * P.s_row + (size_t)kk * P.ncols + ni * BN + half * (BN / 2);
+        float* dst = Shat + (size_t)r * P.s_row + (size_t)kk * P.ncols + col0 + half * (BN / 2);
 #pragma unroll
         for (int q = 0; q < BN / 8; ++q)
           if (q * 4 < cols)
@@ -683,6 +715,7 @@ int launch_syn_tc(mk_ctx* c, const RowBlock& rb, int slot, const float2* d_Nhat,
   P.ncols = 2 * ldf;
   P.mt = (rb.nrow + BM - 1) / BM;
   P.ntl = (P.ncols + BN - 1) / BN;
+  P.nblocks = P.ncols / 32;
   P.s_row = (size_t)c->nb * 2 * ldf;
   P.nblk = nblk;
   P.tune = c->tune;
@@ -692,7 +725,15 @@ int launch_syn_tc(mk_ctx* c, const RowBlock& rb, int slot, const float2* d_Nhat,
   if (c->tune & 512) P.nrb = std::min(P.nrb, 3);
   const size_t kSmemBytes = fixed_smem(nblk) + (size_t)P.nrb * nblk * BLK_BYTES + kSmemExtra;
   const int ntiles = P.nb * P.mt * P.ntl;
-  const int grid = ntiles < c->num_sms ? ntiles : c->num_sms;
+  // a multiple of ntl, so that every CTA keeps its N tile and its siblings (see the A producer)
+  const int grid = ntiles < c->num_sms ? ntiles : (P.ntl <= c->num_sms ? (c->num_sms / P.ntl) * P.ntl : c->num_sms);
+  P.progress = nullptr;
+  if (P.ntl > 1 && grid % P.ntl == 0 && grid <= 1024 && (c->tune & 1024)) {  // measurement switch, off: it costs more than it saves
+    if (!c->d_tc_progress)
+      if (int rc = check_cuda(c, cudaMalloc(&c->d_tc_progress, 1024 * sizeof(uint32_t)), "cudaMalloc progress")) return rc;
+    if (int rc = check_cuda(c, cudaMemsetAsync(c->d_tc_progress, 0, 1024 * sizeof(uint32_t), c->stream), "memset progress")) return rc;
+    P.progress = c->d_tc_progress;
+  }
   float* S0 = reinterpret_cast<float*>(d_Shat + (size_t)rb.r0 * c->nb * ldf);
   const CUtensorMap& mA = *reinterpret_cast<const CUtensorMap*>(c->tmap_A[ia]);
   const CUtensorMap& mB = *reinterpret_cast<const CUtensorMap*>(c->tmap_B[slot]);
