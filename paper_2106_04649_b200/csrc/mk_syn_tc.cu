@@ -725,10 +725,11 @@ int launch_syn_tc(mk_ctx* c, const RowBlock& rb, int slot, const float2* d_Nhat,
   if (c->tune & 512) P.nrb = std::min(P.nrb, 3);
   const size_t kSmemBytes = fixed_smem(nblk) + (size_t)P.nrb * nblk * BLK_BYTES + kSmemExtra;
   const int ntiles = P.nb * P.mt * P.ntl;
-  // a multiple of ntl, so that every CTA keeps its N tile and its siblings (see the A producer)
-  const int grid = ntiles < c->num_sms ? ntiles : (P.ntl <= c->num_sms ? (c->num_sms / P.ntl) * P.ntl : c->num_sms);
+  // (in step: a multiple of ntl, so that every CTA keeps its N tile and its siblings, see the A producer)
+  const bool in_step = (c->tune & 1024) && P.ntl > 1 && P.ntl <= c->num_sms;  // measurement switch, off: it costs more than it saves
+  const int grid = ntiles < c->num_sms ? ntiles : (in_step ? (c->num_sms / P.ntl) * P.ntl : c->num_sms);
   P.progress = nullptr;
-  if (P.ntl > 1 && grid % P.ntl == 0 && grid <= 1024 && (c->tune & 1024)) {  // measurement switch, off: it costs more than it saves
+  if (in_step && grid % P.ntl == 0 && grid <= 1024) {
     if (!c->d_tc_progress)
       if (int rc = check_cuda(c, cudaMalloc(&c->d_tc_progress, 1024 * sizeof(uint32_t)), "cudaMalloc progress")) return rc;
     if (int rc = check_cuda(c, cudaMemsetAsync(c->d_tc_progress, 0, 1024 * sizeof(uint32_t), c->stream), "memset progress")) return rc;
