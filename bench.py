@@ -430,14 +430,14 @@ def run_ours(args):
     if args.parallel == "rows_fused":
         if world > 1:
             ipc_ptrs = shard.attach_ipc(mk, cfg.nfoc, dist)
-
-        def fused_barrier():
+            ipc_ptrs += shard.sync_attach_ipc(mk, dist)
             torch.cuda.synchronize()
-            if world > 1:
-                dist.barrier()
+            dist.barrier()              # every rank's flags exist before anyone writes
+        else:
+            mk.sync_create(0, 1)
 
-        def run_step():
-            shard.run_row_sharded_fused(mk, dGd, dtd, niter, douts, fused_barrier)
+        def run_step():                 # the barriers between the ranks are stream-ordered flag writes / waits (mk_sync_barrier)
+            shard.run_row_sharded_fused(mk, dGd, dtd, niter, douts, mk.sync_barrier)
     elif rows_mode:
         if world > 1:
             exchange = shard.distributed_exchange(mk, dist)
@@ -589,7 +589,8 @@ def main():
     ap.add_argument("--parallel", default="replicas", choices=["replicas", "rows", "rows_fused"],
                     help="N > 1: independent replicas (default, weak scaling) or receiver-row sharding with one all-gather of the "
                          "operand rows per synthesis (strong scaling; SURVEY.md section 8(e) / NEXT-3); rows_fused: the same with the "
-                         "all-gather fused into the producing kernels as peer stores over CUDA IPC mappings (two barriers per synthesis)")
+                         "all-gather fused into the producing kernels as peer stores over CUDA IPC mappings; the two barriers per synthesis are "
+                         "stream memory operations (mk_sync_barrier), no host synchronisation inside a step")
     ap.add_argument("--tune", type=int, default=0, help="MK_OPT_TUNE bit mask (measurement switches of the kernels; include/mk.h)")
     ap.add_argument("--e2e-steps", type=int, default=50)
     ap.add_argument("--cpu-budget", type=float, default=15.0, help="seconds of oracle work for cpu_baseline")

@@ -252,6 +252,22 @@ int mk_ipc_export(const void* d_ptr, unsigned char handle[64]);
 int mk_ipc_open(const unsigned char handle[64], void** d_ptr);
 int mk_ipc_close(void* d_ptr);
 
+/* Stream-ordered barrier between the ranks of a row-sharded run (NEXT-3; the ordering the fused exchange needs, without
+ * the host: no cudaStreamSynchronize, no host barrier inside the iteration loop).  Every rank owns a small array of
+ * world 32-bit flags in device memory (mk_sync_create allocates and zeroes it; mk_sync_flags returns it so that it can
+ * be exported with mk_ipc_export and opened by the other ranks, or handed to other contexts of the same process).
+ * mk_sync_attach gives the context the flag arrays of ALL ranks as device pointers valid in this process
+ * (d_flags_of_rank[rank] may be NULL: the context's own).  mk_sync_barrier then ENQUEUES on the context's stream: one
+ * 32-bit write of the next epoch number into flags[rank] of every other rank (ordered behind all work enqueued so far,
+ * peer stores of operand rows included), followed by one wait per other rank until that rank's epoch has arrived in the
+ * own array (cuStreamWriteValue32 / cuStreamWaitValue32: the GPU's front end waits, no SM is held, the host does not
+ * block).  Work enqueued after it on the stream starts only when every rank has reached the same barrier.  All ranks
+ * must call it the same number of times.  MK_ERR_CUDA if the driver has no stream memory operations. */
+int mk_sync_create(mk_ctx* ctx, int rank, int world);
+int mk_sync_flags(mk_ctx* ctx, void** d_flags);
+int mk_sync_attach(mk_ctx* ctx, void* const* d_flags_of_rank);
+int mk_sync_barrier(mk_ctx* ctx);
+
 enum { MK_FIELD_GMINUS = 1, MK_FIELD_GPLUS = 2 };
 int mk_finish_prepare(mk_ctx* ctx, int field);                   /* forward transform of f1plus / T f1min -> slot 1 */
 int mk_finish_complete(mk_ctx* ctx, int field, float* d_out);    /* contraction + inverse transform + epilogue      */

@@ -24,7 +24,7 @@ SYMBOLS = ("mk_create", "mk_destroy", "mk_set_stream", "mk_set_option", "mk_get_
            "mk_run", "mk_run_host", "mk_begin", "mk_step", "mk_finish", "mk_synthesis", "mk_image", "mk_last_error",
            "mk_version", "mk_create_sharded", "mk_operand", "mk_operand_exchanged", "mk_finish_prepare", "mk_finish_complete",
            "mk_operand_reserve", "mk_operand_attach", "mk_step_contract", "mk_step_post", "mk_ipc_export", "mk_ipc_open", "mk_ipc_close",
-           "mk_set_geometry", "mk_create_streamed")
+           "mk_set_geometry", "mk_create_streamed", "mk_sync_create", "mk_sync_flags", "mk_sync_attach", "mk_sync_barrier")
 MK_FIELD_GMINUS, MK_FIELD_GPLUS = 1, 2
 
 
@@ -86,6 +86,10 @@ def load():
     L.mk_ipc_export.argtypes = [vp, C.c_char_p]
     L.mk_ipc_open.argtypes = [C.c_char_p, C.POINTER(vp)]
     L.mk_ipc_close.argtypes = [vp]
+    L.mk_sync_create.argtypes = [vp, ci, ci]
+    L.mk_sync_flags.argtypes = [vp, C.POINTER(vp)]
+    L.mk_sync_attach.argtypes = [vp, C.POINTER(vp)]
+    L.mk_sync_barrier.argtypes = [vp]
     L.mk_finish_complete.argtypes = [vp, ci, vp]
     L.mk_last_error.argtypes = [vp]
     L.mk_last_error.restype = C.c_char_p
@@ -296,6 +300,23 @@ class Marchenko:
 
     def operand_exchanged(self, slot):
         self._check(self._L.mk_operand_exchanged(self._h, slot))
+
+    # ---- stream-ordered barrier between the ranks of a row-sharded run (include/mk.h mk_sync_*)
+    def sync_create(self, rank, world):
+        self._check(self._L.mk_sync_create(self._h, rank, world))
+
+    def sync_flags(self) -> int:
+        p = C.c_void_p()
+        self._check(self._L.mk_sync_flags(self._h, C.byref(p)))
+        return int(p.value)
+
+    def sync_attach(self, flags_of_rank):
+        """flags_of_rank: one device pointer (int) per rank, valid in this process; the own rank's entry may be None."""
+        arr = (C.c_void_p * len(flags_of_rank))(*[C.c_void_p(p) if p else C.c_void_p() for p in flags_of_rank])
+        self._check(self._L.mk_sync_attach(self._h, arr))
+
+    def sync_barrier(self):
+        self._check(self._L.mk_sync_barrier(self._h))
 
     def finish_prepare(self, field):
         self._check(self._L.mk_finish_prepare(self._h, field))

@@ -1,6 +1,8 @@
 // mk_api.cu — the C ABI of include/mk.h: argument checks, device buffers, and the order of kernel launches.
 // No arithmetic of the method happens on the host: every step of SURVEY.md §8(a) is a kernel in
 // mk_fft_kernels.cu / mk_syn_gemv.cu / mk_syn_gemm.cu.  There is no CPU fallback.
+#include <cuda.h>
+
 #include <algorithm>
 #include <cmath>
 #include <cstdio>
@@ -489,6 +491,7 @@ int mk_destroy(mk_ctx* c) {
   cudaFree(c->d_qstage);
   cudaFree(c->d_img_part);
   cudaFree(c->d_tc_progress);
+  cudaFree(c->d_sync_flags);
   cudaFree(c->d_win[0]);
   cudaFree(c->d_win[1]);
   if (c->h2d_stream) {
@@ -875,6 +878,76 @@ int mk_ipc_close(void* d_ptr) {
   if (cudaIpcCloseMemHandle(d_ptr) != cudaSuccess) {
     cudaGetLastError();
     return MK_ERR_CUDA;
+  }
+  return MK_OK;
+}
+
+int mk_sync_create(mk_ctx* c, int rank, int world) {
+  MK_GUARD(c);
+  if (world < 1 || world > 8 || rank < 0 || rank >= world) return set_err(c, MK_ERR_INVALID_ARG, "mk_sync_create: need 0 <= rank < world <= 8");
+  if (!c->write32_fn) {
+    cudaDriverEntryPointQueryResult q;
+    void* w = nullptr;
+    void* t = nullptr;
+    if (cudaGetDriverEntryPoint("cuStreamWriteValue32", &w, cudaEnableDefault, &q) != cudaSuccess || q != cudaDriverEntryPointSuccess || !w ||
+        cudaGetDriverEntryPoint("cuStreamWaitValue32", &t, cudaEnableDefault, &q) != cudaSuccess || q != cudaDriverEntryPointSuccess || !t) {
+      cudaGetLastError();
+      return set_err(c, MK_ERR_CUDA, "stream memory operations (cuStreamWriteValue32 / cuStreamWaitValue32) are not available");
+    }
+    c->write32_fn = w;
+    c->wait32_fn = t;
+  }
+  if (!c->d_sync_flags)
+    if (int rc = check_cuda(c, cudaMalloc(&c->d_sync_flags, 8 * sizeof(uint32_t)), "cudaMalloc sync flags")) return rc;
+  if (int rc = check_cuda(c, cudaMemset(c->d_sync_flags, 0, 8 * sizeof(uint32_t)), "memset sync flags")) return rc;
+  c->sync_rank = rank;
+  c->sync_world = world;
+  c->sync_epoch = 0;
+  c->sync_attached = world == 1;
+  for (auto& p : c->sync_peer) p = nullptr;
+  c->sync_peer[rank] = c->d_sync_flags;
+  return MK_OK;
+}
+
+int mk_sync_flags(mk_ctx* c, void** d_flags) {
+  MK_GUARD(c);
+  if (!d_flags) return MK_ERR_INVALID_ARG;
+  if (!c->d_sync_flags) return set_err(c, MK_ERR_STATE, "mk_sync_flags before mk_sync_create");
+  *d_flags = c->d_sync_flags;
+  return MK_OK;
+}
+
+int mk_sync_attach(mk_ctx* c, void* const* d_flags_of_rank) {
+  MK_GUARD(c);
+  if (!c->d_sync_flags) return set_err(c, MK_ERR_STATE, "mk_sync_attach before mk_sync_create");
+  if (!d_flags_of_rank) return MK_ERR_INVALID_ARG;
+  for (int g = 0; g < c->sync_world; ++g) {
+    if (g == c->sync_rank) continue;
+    if (!d_flags_of_rank[g]) return set_err(c, MK_ERR_INVALID_ARG, "mk_sync_attach: a peer's flag array is NULL");
+    c->sync_peer[g] = static_cast<uint32_t*>(d_flags_of_rank[g]);
+  }
+  c->sync_attached = true;
+  return MK_OK;
+}
+
+int mk_sync_barrier(mk_ctx* c) {
+  MK_GUARD(c);
+  if (!c->sync_attached) return set_err(c, MK_ERR_STATE, "mk_sync_barrier before mk_sync_create / mk_sync_attach");
+  typedef CUresult (*Write32)(CUstream, CUdeviceptr, cuuint32_t, unsigned int);
+  typedef CUresult (*Wait32)(CUstream, CUdeviceptr, cuuint32_t, unsigned int);
+  const Write32 wr = reinterpret_cast<Write32>(c->write32_fn);
+  const Wait32 wt = reinterpret_cast<Wait32>(c->wait32_fn);
+  const uint32_t e = ++c->sync_epoch;
+  CUstream st = reinterpret_cast<CUstream>(c->stream);
+  for (int g = 0; g < c->sync_world; ++g) {
+    if (g == c->sync_rank) continue;
+    if (wr(st, reinterpret_cast<CUdeviceptr>(c->sync_peer[g] + c->sync_rank), e, CU_STREAM_WRITE_VALUE_DEFAULT) != CUDA_SUCCESS)
+      return set_err(c, MK_ERR_CUDA, "cuStreamWriteValue32 failed");
+  }
+  for (int g = 0; g < c->sync_world; ++g) {
+    if (g == c->sync_rank) continue;
+    if (wt(st, reinterpret_cast<CUdeviceptr>(c->d_sync_flags + g), e, CU_STREAM_WAIT_VALUE_GEQ) != CUDA_SUCCESS)
+      return set_err(c, MK_ERR_CUDA, "cuStreamWaitValue32 failed");
   }
   return MK_OK;
 }

@@ -94,6 +94,14 @@ struct mk_ctx {
   const void* tmap_B_key[2] = {nullptr, nullptr};
   int tmap_B_ldf[2] = {0, 0};
   uint32_t* d_tc_progress = nullptr;  // tcgen05 contraction: A boxes asked for, per CTA (sibling CTAs keep in step)
+  // mk_sync_*: stream-ordered barrier between ranks
+  uint32_t* d_sync_flags = nullptr;   // [sync_world] epochs the other ranks have written here
+  uint32_t* sync_peer[8] = {};        // every rank's flag array as mapped in this process ([sync_rank] = own)
+  int sync_rank = -1, sync_world = 0;
+  uint32_t sync_epoch = 0;
+  bool sync_attached = false;
+  void* write32_fn = nullptr;         // cuStreamWriteValue32 / cuStreamWaitValue32, resolved through the runtime
+  void* wait32_fn = nullptr;
   void* encode_fn = nullptr;  // cuTensorMapEncodeTiled, resolved at run time through the CUDA runtime
   float* d_stage = nullptr;  // host-call staging
   double* d_img_part = nullptr;  // mk_image: per (focal point, receiver chunk) partial sums

@@ -175,9 +175,11 @@ def attach_ipc(mk, nfoc: int, dist):
 
 def run_row_sharded_fused(mk, d_Gd, d_td, niter: int, outs: dict, barrier, on_iterate=None) -> None:
     """Algorithm 1 on a row-sharded context whose peers are attached: no copies, two barriers per synthesis.
-    `barrier()` must return only when every rank's stream has finished the work enqueued so far (e.g.
-    torch.cuda.synchronize(); dist.barrier()): once before a rank may overwrite operand rows that others read
-    (contractions done), once before anyone reads the new rows (stores done)."""
+    `barrier()` must order this rank's LATER work behind every rank's EARLIER work: either on the stream —
+    mk.sync_barrier after sync_attach_in_process / sync_attach_ipc: flag writes and waits enqueued on the context's
+    stream, the host never blocks — or on the host (torch.cuda.synchronize(); dist.barrier()).  It is needed once before
+    a rank may overwrite operand rows that others read (contractions done) and once before anyone reads the new rows
+    (stores done)."""
     from . import binding as B
     barrier()                                      # nobody still reads the operands of a previous run
     mk.begin(d_Gd, d_td)
@@ -201,3 +203,38 @@ def run_row_sharded_fused(mk, d_Gd, d_td, niter: int, outs: dict, barrier, on_it
             barrier()
             mk.operand_exchanged(1)
             mk.finish_complete(field, outs[name])
+
+
+# ---- the barriers of run_row_sharded_fused on the device: stream-ordered flags instead of host synchronisation ----------
+def sync_attach_in_process(mks) -> None:
+    """Row-sharded contexts of ONE process: every context learns every other context's flag array."""
+    for g, mk in enumerate(mks):
+        mk.sync_create(g, len(mks))
+    flags = [mk.sync_flags() for mk in mks]
+    for mk in mks:
+        mk.sync_attach(flags)
+
+
+def sync_attach_ipc(mk, dist):
+    """One process per GPU (or several on one GPU): the flag arrays travel as CUDA IPC handles through torch.distributed.
+    Returns the opened pointers (close them with binding.ipc_close before the contexts are destroyed)."""
+    from . import binding as B
+    rank, world = dist.get_rank(), dist.get_world_size()
+    mk.sync_create(rank, world)
+    everyone = [None] * world
+    dist.all_gather_object(everyone, B.ipc_export(mk.sync_flags()))
+    flags, opened = [], []
+    for g in range(world):
+        if g == rank:
+            flags.append(None)
+        else:
+            p = B.ipc_open(everyone[g])
+            opened.append(p)
+            flags.append(p)
+    mk.sync_attach(flags)
+    return opened
+
+
+def device_barrier(mk):
+    """barrier() for run_row_sharded_fused that never blocks the host: mk_sync_barrier enqueued on the context's stream."""
+    return mk.sync_barrier

@@ -347,6 +347,92 @@ def test_row_sharded_with_fused_peer_stores(k, n, nt, nfoc, regime, world):
             mk.close()
 
 
+@pytest.mark.parametrize("k,n,nt,nfoc,regime,world", [(1, 37, 512, 3, 1, 2), (3, 150, 2048, 19, 3, 3)])
+def test_row_sharded_fused_with_stream_ordered_barriers(k, n, nt, nfoc, regime, world):
+    """mk_sync_barrier: the two barriers per synthesis of the fused exchange as stream-ordered flag writes / waits.  Every
+    rank runs on a stream of its OWN; the host enqueues the whole run without ever synchronising (one synchronize at the
+    very end); the results must equal the single context's bit for bit and meet the oracle."""
+    import torch
+    from paper_2106_04649_b200 import binding as B, shard
+    cfg = calibrated(configs.scaled(k, n=n, nt=nt, nfoc=nfoc, focal="fan:250", niter=5))
+    R, Gd, td = problem(cfg)
+    whole = gpu_chain(cfg, R, Gd, td, regime=regime)
+    ref = _oracle_chain(cfg, R, Gd, td)
+    dev = torch.device("cuda:0")
+    dR, dGd, dtd = (torch.from_numpy(np.ascontiguousarray(a)).to(dev) for a in (R, Gd, td))
+    streams = [torch.cuda.Stream(device=dev) for _ in range(world)]
+    mks = []
+    try:
+        for g in range(world):
+            rows = shard.row_slice(n, g, world)
+            mk = B.Marchenko(n, n, nt, cfg.dt, cfg.dx, cfg.fmin, cfg.fmax, rows=(rows.start, len(rows)))
+            mk.set_option(B.MK_OPT_EPS_SAMPLES, cfg.eps)
+            mk.set_option(B.MK_OPT_REGIME, regime)
+            mk.load_R(dR)
+            mks.append(mk)
+        shard.attach_in_process(mks, nfoc)
+        shard.sync_attach_in_process(mks)
+        its = [[torch.zeros((nfoc, n, nt), dtype=torch.float32, device=dev) for _ in range(cfg.niter)] for _ in mks]
+        outs = [{nm: torch.zeros((nfoc, n, nt), dtype=torch.float32, device=dev) for nm in FINALS} for _ in mks]
+
+        def all_ranks(call):
+            for g, mk in enumerate(mks):
+                call(g, mk)
+
+        # one lock-step pass on the default stream first, so that every buffer the run needs exists: an allocation in
+        # the middle of the real run could make the host wait for a stream that waits for a rank not yet enqueued
+        all_ranks(lambda g, mk: mk.begin(dGd, dtd))
+        all_ranks(lambda g, mk: mk.operand_exchanged(0))
+        all_ranks(lambda g, mk: mk.step_contract())
+        all_ranks(lambda g, mk: mk.step_post(None))
+        all_ranks(lambda g, mk: mk.operand_exchanged(0))
+        for field in (B.MK_FIELD_GMINUS, B.MK_FIELD_GPLUS):
+            all_ranks(lambda g, mk: mk.finish_prepare(field))
+            all_ranks(lambda g, mk: mk.operand_exchanged(1))
+            all_ranks(lambda g, mk: mk.finish_complete(field, outs[g]["G"]))
+        torch.cuda.synchronize()                    # inputs, ingest, operands and workspaces are in place
+        for g, mk in enumerate(mks):
+            mk.set_stream(streams[g].cuda_stream)
+
+        # shard.run_row_sharded_fused, rank by rank in one host thread: only ENQUEUES, the ordering is the streams'
+        all_ranks(lambda g, mk: mk.sync_barrier())
+        all_ranks(lambda g, mk: mk.begin(dGd, dtd))
+        all_ranks(lambda g, mk: mk.sync_barrier())
+        all_ranks(lambda g, mk: mk.operand_exchanged(0))
+        for i in range(cfg.niter):
+            all_ranks(lambda g, mk: mk.step_contract())
+            all_ranks(lambda g, mk: mk.sync_barrier())          # every rank has read the operand
+            all_ranks(lambda g, mk: mk.step_post(its[g][i]))
+            all_ranks(lambda g, mk: mk.sync_barrier())          # every rank's rows have landed everywhere
+            all_ranks(lambda g, mk: mk.operand_exchanged(0))
+        all_ranks(lambda g, mk: mk.finish({nm: outs[g][nm] for nm in ("f1plus", "f1min", "G")}))
+        for name, field in (("Gminus", B.MK_FIELD_GMINUS), ("Gplus", B.MK_FIELD_GPLUS)):
+            all_ranks(lambda g, mk: mk.sync_barrier())
+            all_ranks(lambda g, mk: mk.finish_prepare(field))
+            all_ranks(lambda g, mk: mk.sync_barrier())
+            all_ranks(lambda g, mk: mk.operand_exchanged(1))
+            all_ranks(lambda g, mk: mk.finish_complete(field, outs[g][name]))
+        torch.cuda.synchronize()                    # the only host synchronisation of the run
+        worst = 0.0
+        np_its = [[t.cpu().numpy() for t in its[g]] for g in range(world)]
+        for g in range(world):
+            rows = shard.row_slice(n, g, world)
+            sl = slice(rows.start, rows.stop)
+            for i in range(cfg.niter):
+                worst = max(worst, rel_l2(np_its[g][i][:, sl], whole["N_iters"][i][:, sl]))
+            for nm in FINALS:
+                worst = max(worst, rel_l2(outs[g][nm].cpu().numpy()[:, sl], whole[nm][:, sl]))
+        worst_it, worst_fin = _sharded_vs_oracle(ref, world, n, np_its, outs, cfg.niter)
+        print(f"\n[stream-ordered barriers, {world} ranks on {world} streams, n={n} nt={nt} nfoc={nfoc} regime={regime}] worst deviation from "
+              f"the single context {worst:.1e}; against the oracle: per-iteration {worst_it:.2e}, finals {worst_fin:.2e}")
+        assert worst <= 1e-6
+        assert worst_it <= TOL_ITER and worst_fin <= TOL_FINAL
+    finally:
+        torch.cuda.synchronize()
+        for mk in mks:
+            mk.close()
+
+
 @pytest.mark.parametrize("nfoc", [1, 2, 4])
 def test_fused_finals_match_separate_finals(nfoc):
     """MK_OPT_FUSED_FINALS: with 1, 2 or 4 focal points G^- and G^+ come from ONE pass over R^ (2 nfoc right-hand sides);

@@ -21,7 +21,7 @@ def _free_port():
     return p
 
 
-def _worker(rank, world, port, regime, q):
+def _worker(rank, world, port, regime, q, device_barrier=False):
     import sys
     from pathlib import Path
     sys.path.insert(0, str(Path(__file__).resolve().parent))
@@ -45,14 +45,21 @@ def _worker(rank, world, port, regime, q):
         mk.load_R(torch.from_numpy(R).to(dev))
         opened = shard.attach_ipc(mk, cfg.nfoc, dist)
 
-        def barrier():
+        def host_barrier():
             torch.cuda.synchronize()
             dist.barrier()
+
+        if device_barrier:      # mk_sync_barrier: flag writes / waits on the stream, the host never blocks inside the run
+            opened += shard.sync_attach_ipc(mk, dist)
+            host_barrier()      # every rank's flags exist and are zero before anyone writes
+            barrier = mk.sync_barrier
+        else:
+            barrier = host_barrier
 
         names = ("N_last", "f1plus", "f1min", "G", "Gplus", "Gminus")
         outs = {nm: torch.zeros((cfg.nfoc, cfg.n, cfg.nt), dtype=torch.float32, device=dev) for nm in names}
         shard.run_row_sharded_fused(mk, torch.from_numpy(Gd).to(dev), torch.from_numpy(td).to(dev), cfg.niter, outs, barrier)
-        barrier()
+        host_barrier()
         sl = slice(rows.start, rows.stop)
         worst = max(rel_l2(outs[nm].cpu().numpy()[:, sl], whole[nm][:, sl]) for nm in names)
         alive = float(np.linalg.norm(whole["N_last"])) > 0.0
@@ -61,7 +68,7 @@ def _worker(rank, world, port, regime, q):
         ref = oracle.marchenko(R, Gd, td, cfg.dt, cfg.dx, cfg.fmin, cfg.fmax, cfg.niter, cfg.eps)
         e_it = rel_l2(outs["N_last"].cpu().numpy()[:, sl], ref["N_iters"][-1][:, sl])
         e_fin = max(rel_l2(outs[nm].cpu().numpy()[:, sl], ref[nm][:, sl]) for nm in names[1:])
-        q.put((rank, worst, alive, len(opened), e_it, e_fin))
+        q.put((rank, worst, alive, len(opened) - (world - 1 if device_barrier else 0), e_it, e_fin))
     except Exception as e:   # report instead of hanging the other rank
         q.put((rank, repr(e), False, -1, 1.0, 1.0))
     finally:
@@ -94,3 +101,29 @@ def test_two_processes_one_gpu_fused_peer_stores(regime):
         assert alive and worst <= 1e-6
         assert e_it <= 2e-5 and e_fin <= 1e-4, (e_it, e_fin)
         assert nopened == 2                               # one peer x two slots x one plane
+
+
+@pytest.mark.timeout(300)
+def test_two_processes_one_gpu_stream_ordered_barriers():
+    """The same run with mk_sync_barrier in place of the host barriers: the flag arrays travel as CUDA
+    IPC handles, every barrier of shard.run_row_sharded_fused is two stream memory operations per peer, and the host of
+    either process enqueues its whole run without waiting for the other."""
+    import torch.multiprocessing as mp
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    port, world = _free_port(), 2
+    procs = [ctx.Process(target=_worker, args=(r, world, port, 3, q, True)) for r in range(world)]
+    for p in procs:
+        p.start()
+    try:
+        res = sorted(q.get(timeout=240) for _ in range(world))
+    finally:
+        for p in procs:
+            p.join(timeout=30)
+            if p.is_alive():
+                p.kill()
+    print(res)
+    for rank, worst, alive, nopened, e_it, e_fin in res:
+        assert isinstance(worst, float), worst
+        assert alive and worst <= 1e-6
+        assert e_it <= 2e-5 and e_fin <= 1e-4, (e_it, e_fin)
