@@ -154,7 +154,12 @@ int mk_set_geometry(mk_ctx* ctx, const int* h_rec_of_shot, const float* h_weight
  * May be called repeatedly with disjoint shot ranges (config 4: 61 calls of 64 shots), and again later to replace
  * shots (it ends a run in progress, see "run state" above). */
 int mk_load_R(mk_ctx* ctx, const float* d_R_time, int shot0, int nshots);
-/* Same from a HOST buffer: staged through an internal device buffer in bounded chunks; returns when done. */
+/* The same for a source that holds only the receiver rows this context owns: d_R_rows is [nshots][nrows][nt] with
+ * nrows = the context's rows (row0 .. row0+nrows-1 of mk_create_sharded; all nrec rows otherwise, where the call equals
+ * mk_load_R).  With it the G ranks of a row-sharded run read 1/G of R each instead of all of it (config 4: 250 GB of
+ * time-domain R would otherwise be produced G times).  Not available with compressed or out-of-core R^. */
+int mk_load_R_rows(mk_ctx* ctx, const float* d_R_rows, int shot0, int nshots);
+/* Same as mk_load_R from a HOST buffer: staged through an internal device buffer in bounded chunks; returns when done. */
 int mk_load_R_host(mk_ctx* ctx, const float* h_R_time, int shot0, int nshots);
 
 /* Outputs of a run; each pointer is [nfoc][nrec][nt] fp32 or NULL to skip that field.  G^- and G^+ cost one
@@ -208,7 +213,8 @@ int mk_image(mk_ctx* ctx, const float* d_Gminus, float* d_image);
  * never moves) and computes a2..a6 for those rows; the ONE exchange step per synthesis is an all-gather of the rows
  * of the operand N^ the ranks have just produced.  The library computes; the caller moves the rows (NCCL all-gather
  * or peer copies) between the calls, in this order:
- *   mk_create_sharded; mk_load_R (same full chunks on every rank: the library keeps its rows only);
+ *   mk_create_sharded; mk_load_R (same full chunks on every rank: the library keeps its rows only) or mk_load_R_rows
+ *   (each rank passes its own receiver rows only);
  *   mk_begin; [exchange slot 0]; niter x { mk_step; [exchange slot 0] };
  *   for G^-, G^+: mk_finish_prepare(field); [exchange slot 1]; mk_finish_complete(field, out);  mk_finish for f1+-, G.
  * "[exchange slot s]" = read mk_operand(ctx, s, &v), make every rank's rows of every plane identical on all ranks,

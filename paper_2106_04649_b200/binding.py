@@ -24,7 +24,7 @@ SYMBOLS = ("mk_create", "mk_destroy", "mk_set_stream", "mk_set_option", "mk_get_
            "mk_run", "mk_run_host", "mk_begin", "mk_step", "mk_finish", "mk_synthesis", "mk_image", "mk_last_error",
            "mk_version", "mk_create_sharded", "mk_operand", "mk_operand_exchanged", "mk_finish_prepare", "mk_finish_complete",
            "mk_operand_reserve", "mk_operand_attach", "mk_step_contract", "mk_step_post", "mk_ipc_export", "mk_ipc_open", "mk_ipc_close",
-           "mk_set_geometry", "mk_create_streamed", "mk_sync_create", "mk_sync_flags", "mk_sync_attach", "mk_sync_barrier")
+           "mk_set_geometry", "mk_create_streamed", "mk_sync_create", "mk_sync_flags", "mk_sync_attach", "mk_sync_barrier", "mk_load_R_rows")
 MK_FIELD_GMINUS, MK_FIELD_GPLUS = 1, 2
 
 
@@ -67,6 +67,7 @@ def load():
     L.mk_set_geometry.argtypes = [vp, vp, vp]
     L.mk_load_R.argtypes = [vp, vp, ci, ci]
     L.mk_load_R_host.argtypes = [vp, vp, ci, ci]
+    L.mk_load_R_rows.argtypes = [vp, vp, ci, ci]
     L.mk_run.argtypes = [vp, vp, vp, ci, ci, C.POINTER(mk_outputs)]
     L.mk_run_host.argtypes = [vp, vp, vp, ci, ci, C.POINTER(mk_outputs)]
     L.mk_begin.argtypes = [vp, vp, vp, ci]
@@ -219,6 +220,12 @@ class Marchenko:
         import torch
         nshots = d_R_time.shape[0]
         self._check(self._L.mk_load_R(self._h, _dev_ptr(d_R_time, torch.float32, nshots * self.nrec * self.nt), shot0, nshots))
+
+    def load_R_rows(self, d_R_rows, shot0=0):
+        """d_R_rows: [nshots][rows of this context][nt] (the receiver rows a row-sharded context owns, nothing else)."""
+        import torch
+        nshots, nrows = d_R_rows.shape[0], d_R_rows.shape[1]
+        self._check(self._L.mk_load_R_rows(self._h, _dev_ptr(d_R_rows, torch.float32, nshots * nrows * self.nt), shot0, nshots))
 
     def load_R_host(self, h_R_time, shot0=0):
         nshots = h_R_time.shape[0]

@@ -657,6 +657,23 @@ int mk_load_R(mk_ctx* c, const float* d_R_time, int shot0, int nshots) {
   return MK_OK;
 }
 
+int mk_load_R_rows(mk_ctx* c, const float* d_R_rows, int shot0, int nshots) {
+  MK_GUARD(c);
+  if (!d_R_rows || shot0 < 0 || nshots <= 0 || shot0 + nshots > c->ns) return set_err(c, MK_ERR_INVALID_ARG, "mk_load_R_rows: bad shot range");
+  if (c->rhat_format == 1 || c->nres < c->nrow) return set_err(c, MK_ERR_STATE, "mk_load_R_rows: not available with compressed or out-of-core R^");
+  if (int rc = end_run(c, "mk_load_R_rows")) return rc;
+  // the kernels address the source by the global receiver index: shift the base so that row r0 is the array's first
+  RowBlock rb{c->d_Rhat, c->r0, c->nrow};
+  rb.src_n = c->nrow;
+  if (int rc = launch_load_R(c, rb, d_R_rows - (ptrdiff_t)c->r0 * c->nt, shot0, nshots)) return rc;
+  for (int s = shot0; s < shot0 + nshots; ++s)
+    if (!c->shot_loaded[s]) {
+      c->shot_loaded[s] = 1;
+      ++c->shots_loaded;
+    }
+  return MK_OK;
+}
+
 int mk_load_R_host(mk_ctx* c, const float* h_R_time, int shot0, int nshots) {
   MK_GUARD(c);
   if (!h_R_time || shot0 < 0 || nshots <= 0 || shot0 + nshots > c->ns) return set_err(c, MK_ERR_INVALID_ARG, "mk_load_R_host: bad shot range");

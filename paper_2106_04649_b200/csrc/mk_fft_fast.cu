@@ -641,6 +641,7 @@ int launch_load_R_fast(mk_ctx* c, const RowBlock& rb, const float* d_R_time, int
   FastParams P = make_fast(c, 0, 0);
   P.r0 = rb.r0;
   if (rb.ld) P.ld = rb.ld;
+  if (rb.src_n) P.n = rb.src_n;
   MK_FAST_LAUNCH(k_load_R_fast, grid, sh, d_R_time, rb.Rhat, P, shot0, nshots, sh.lg);
 }
 

@@ -401,6 +401,7 @@ int launch_load_R(mk_ctx* c, const RowBlock& rb, const float* d_R_time, int shot
   FftParams P = make_params(c, 0, 0);
   P.r0 = rb.r0;
   if (rb.ld) P.ld = rb.ld;
+  if (rb.src_n) P.n = rb.src_n;
   k_load_R<<<grid, kThreads, smem, c->stream>>>(d_R_time, rb.Rhat, P, shot0, nshots, lg);
   ++c->launches;
   return check_cuda(c, cudaGetLastError(), "k_load_R");

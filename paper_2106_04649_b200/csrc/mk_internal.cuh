@@ -142,6 +142,7 @@ struct RowBlock {
   float2* Rhat;
   int r0, nrow;
   int ld = 0;  // ingest only: elements between consecutive (receiver, bin) rows of the target (0 = the context's ld)
+  int src_n = 0;  // ingest only: receivers per shot in the SOURCE array (0 = the context's nrec; mk_load_R_rows: its own rows)
 };
 
 // where a forward transform stores N^ (a1, a6)

@@ -123,10 +123,31 @@ def run_row_sharded(mk, d_Gd, d_td, niter: int, outs: dict, exchange, on_iterate
 
 
 def distributed_exchange(mk, dist):
-    """exchange(slot) for run_row_sharded under torch.distributed (one process per GPU, backend nccl)."""
+    """exchange(slot) for run_row_sharded under torch.distributed (one process per GPU, backend nccl): one
+    all_gather_into_tensor per plane on buffers allocated ONCE (no allocation, no Python-side list of receive tensors and
+    one strided copy in / one per peer out on the data path)."""
+    import torch
+    rank, world, n = dist.get_rank(), dist.get_world_size(), mk.nrec
+    nmax = max(len(row_slice(n, g, world)) for g in range(world))
+    mine = row_slice(n, rank, world)
+    bufs = {}
+
     def exchange(slot):
         planes, v = mk.operand(slot)
-        allgather_operand_rows(planes, v.rows_per_rec, mk.nrec, dist.get_rank(), dist.get_world_size(), dist)
+        rpr = v.rows_per_rec
+        for pi, plane in enumerate(planes):
+            nb, _, rf = plane.shape
+            key = (slot, pi, nb, rf, plane.dtype, plane.device)
+            if key not in bufs:
+                bufs[key] = (torch.zeros((nb, nmax * rpr, rf), dtype=plane.dtype, device=plane.device),
+                             torch.empty((world, nb, nmax * rpr, rf), dtype=plane.dtype, device=plane.device))
+            send, recv = bufs[key]
+            send[:, :rpr * len(mine)].copy_(plane[:, rpr * mine.start:rpr * mine.stop])
+            dist.all_gather_into_tensor(recv.view(-1), send.view(-1))
+            for g in range(world):
+                if g != rank:
+                    rg = row_slice(n, g, world)
+                    plane[:, rpr * rg.start:rpr * rg.stop].copy_(recv[g, :, :rpr * len(rg)])
         mk.operand_exchanged(slot)
     return exchange
 

@@ -368,7 +368,11 @@ def test_row_sharded_fused_with_stream_ordered_barriers(k, n, nt, nfoc, regime, 
             mk = B.Marchenko(n, n, nt, cfg.dt, cfg.dx, cfg.fmin, cfg.fmax, rows=(rows.start, len(rows)))
             mk.set_option(B.MK_OPT_EPS_SAMPLES, cfg.eps)
             mk.set_option(B.MK_OPT_REGIME, regime)
-            mk.load_R(dR)
+            # every rank ingests ONLY its own receiver rows (mk_load_R_rows), in two uneven shot chunks
+            mine = dR[:, rows.start:rows.stop].contiguous()
+            cut = max(1, n // 3)
+            mk.load_R_rows(mine[:cut], 0)
+            mk.load_R_rows(mine[cut:], cut)
             mks.append(mk)
         shard.attach_in_process(mks, nfoc)
         shard.sync_attach_in_process(mks)

@@ -92,7 +92,32 @@ def _row_worker(rank, world, port, q, n, nb, rpr, rf, nplanes):
             t[:, rpr * n:] = 0.0                      # pad rows are zero and must stay zero
             planes.append(t)
         shard.allgather_operand_rows(planes, rpr, n, rank, world, dist)
-        ok = all(bool(torch.equal(planes[p][:, :rpr * n], full[p][:, :rpr * n])) and float(planes[p][:, rpr * n:].abs().max()) == 0.0
+        # the exchange that bench.py --parallel rows uses (buffers allocated once, all_gather_into_tensor), driven twice on
+        # a stand-in for the context: it must give the same planes
+        again = []
+        for p in range(nplanes):
+            t = torch.full((nb, rpr * ld, rf), -1.0)
+            t[:, rpr * mine.start:rpr * mine.stop] = full[p][:, rpr * mine.start:rpr * mine.stop]
+            t[:, rpr * n:] = 0.0
+            again.append(t)
+
+        class FakeContext:
+            nrec = n
+            acked = 0
+
+            def operand(self, slot):
+                class V:
+                    rows_per_rec = rpr
+                return again, V
+
+            def operand_exchanged(self, slot):
+                self.acked += 1
+        fake = FakeContext()
+        exchange = shard.distributed_exchange(fake, dist)
+        exchange(0)
+        exchange(0)
+        same = fake.acked == 2 and all(bool(torch.equal(a, b)) for a, b in zip(again, planes))
+        ok = same and all(bool(torch.equal(planes[p][:, :rpr * n], full[p][:, :rpr * n])) and float(planes[p][:, rpr * n:].abs().max()) == 0.0
                  for p in range(nplanes))
         q.put((rank, ok))
     finally:
