@@ -14,7 +14,11 @@ __device__ __forceinline__ void store_operand(const OperandOut& O, int ld, int k
   if (s < 0) return;
   const size_t idx = ((size_t)kk * ld + s) * O.ldf + f;
   O.plain[idx] = X;
-  for (int p = 0; p < O.npeer; ++p) O.peer[p][idx] = X;
+  // compile-time indices: a run-time index into peer[] would make the compiler copy the whole struct to local memory
+  // (measured: 155 local loads and generic-space stores in k_post_fast)
+#pragma unroll
+  for (int p = 0; p < kMaxPeers; ++p)
+    if (p < O.npeer) O.peer[p][idx] = X;
 }
 
 // mk_fft_fast.cu: true when the register-resident path handles this context's nt (and it is not switched off)

@@ -357,7 +357,9 @@ __device__ __forceinline__ void store_operand2(const OperandOut& O, int ld, int 
   const size_t idx = ((size_t)kk * ld + s) * O.ldf + f;
   const float4 v = make_float4(X0.x, X0.y, X1.x, X1.y);
   *reinterpret_cast<float4*>(O.plain + idx) = v;
-  for (int p = 0; p < O.npeer; ++p) *reinterpret_cast<float4*>(O.peer[p] + idx) = v;
+#pragma unroll
+  for (int p = 0; p < kMaxPeers; ++p)
+    if (p < O.npeer) *reinterpret_cast<float4*>(O.peer[p] + idx) = v;
 }
 
 // ------------------------------------------------------------------------------------------------ k_load_R_fast
@@ -400,7 +402,7 @@ k_load_R_fast(const float* __restrict__ Rt, float2* __restrict__ Rhat, FastParam
 // grid (ceil(nfoc / FT), n); src: [nfoc][n][nt]                                                        (a1, a6)
 template <int HF>
 __global__ void __launch_bounds__(256, 2)
-k_fwd_fast(const float* __restrict__ src, OperandOut O, FastParams P, int lgFT, int conj_out, float* __restrict__ init_Tsrc) {
+k_fwd_fast(const float* __restrict__ src, const __grid_constant__ OperandOut O, FastParams P, int lgFT, int conj_out, float* __restrict__ init_Tsrc) {
   extern __shared__ float2 smem[];
   constexpr int TS = Geo<HF>::TS;
   const int FT = 1 << lgFT, r = P.r0 + blockIdx.y, f0 = blockIdx.x * FT;
@@ -489,7 +491,7 @@ k_inv_fast(const float2* __restrict__ spec, FastParams P, int lgFT, float* __res
 // the time fields is a natural-order float2 row; only the optional N_i copy of an even step is written reversed.
 template <int HF>
 __global__ void __launch_bounds__(256, 2)
-k_post_fast(const float2* __restrict__ Shat, float2* __restrict__ phat, OperandOut O, const int* __restrict__ h,
+k_post_fast(const float2* __restrict__ Shat, float2* __restrict__ phat, const __grid_constant__ OperandOut O, const int* __restrict__ h,
             float* __restrict__ f1plus, float* __restrict__ f1min, FastParams P, int lgFT, int parity_even,
             float* __restrict__ Ni_out, int pf_dist) {
   extern __shared__ float2 smem[];

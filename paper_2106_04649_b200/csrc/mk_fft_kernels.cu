@@ -219,7 +219,7 @@ __global__ void __launch_bounds__(kThreads) k_load_R(const float* __restrict__ R
 
 // ------------------------------------------------------------------------------------------------ k_fwd
 // grid (ceil(nfoc/FT), n); src: [nfoc][n][nt]
-__global__ void __launch_bounds__(kThreads) k_fwd(const float* __restrict__ src, OperandOut O, FftParams P, int lgFT,
+__global__ void __launch_bounds__(kThreads) k_fwd(const float* __restrict__ src, const __grid_constant__ OperandOut O, FftParams P, int lgFT,
                                                   int conj_out, float* __restrict__ init_Tsrc) {
   extern __shared__ float2 smem[];
   const int MP = mkfft::padded_len(P.plan.M), FT = 1 << lgFT;
@@ -289,7 +289,7 @@ __global__ void __launch_bounds__(kThreads) k_inv(const float2* __restrict__ spe
 // ------------------------------------------------------------------------------------------------ k_post
 // grid (ceil(nfoc/FT), n).  Shat, phat: [n][nb][ldf]; operand out: see store_operand; h: [nfoc][n];
 // f1plus / f1min: [nfoc][n][nt]
-__global__ void __launch_bounds__(kThreads) k_post(const float2* __restrict__ Shat, float2* __restrict__ phat, OperandOut O,
+__global__ void __launch_bounds__(kThreads) k_post(const float2* __restrict__ Shat, float2* __restrict__ phat, const __grid_constant__ OperandOut O,
                                                    const int* __restrict__ h, float* __restrict__ f1plus, float* __restrict__ f1min,
                                                    FftParams P, int lgFT, int parity_even, float* __restrict__ Ni_out) {
   extern __shared__ float2 smem[];
