@@ -12,7 +12,7 @@ import sys
 from .build import OBJ
 
 ALWAYS = re.compile(r"UTC|LDTM|STTM|UTMA|SYNCS|RED|ATOM|LDG|STG|LDS|STS|LDGSTS|SETMAXREG|FENCE|NANOSLEEP|HMMA|ELECT|FFMA|MUFU")
-INSTR = re.compile(r"^\s+/\*[0-9a-f]+\*/\s+(?:@!?U?P\d+\s+)?([A-Z][A-Z0-9_.]*)")
+INSTR = re.compile(r"^\s+/\*[0-9a-f]+\*/\s+(?:@!?U?P\d+\s+)?([A-Z][A-Za-z0-9_.]*)")
 
 
 def histogram(obj):
