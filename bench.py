@@ -527,6 +527,9 @@ def run_ours(args):
         del dGd, dtd, douts, R, Gd, td
         torch.cuda.empty_cache()
         c2 = configs.get(2)          # same R as config 1 (BASELINE.json): the context and its R^ are reused
+        # the paper's middle case, 29 focal points, on config 1's R^: the narrow end of the tensor regime
+        c29 = configs.scaled(2, nfoc=29, focal="fan:600", name="3GB_29foc")
+        secondary.append(secondary_entry(mk, c29, 0, 20, 3, local, dev))
         secondary.append(secondary_entry(mk, c2, 0, args.secondary_steps, 3, local, dev, image=True))
         secondary.append(secondary_entry(mk, c2, 2, args.secondary_steps, 3, local, dev))
         mk.close()

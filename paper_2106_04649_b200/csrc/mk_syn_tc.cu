@@ -105,7 +105,18 @@ constexpr int kThreads = 128 + kSplitGroups * kSplitThreads + 32 * kReadWarps;  
 // 128 x 32 + 384 x 64 + 256 x 128 = 61440.  (Two split groups: 640 threads at 96; 128 x 32 + 256 x 72 + 256 x 152.)
 constexpr int kRegsControl = 32, kRegsSplit = kSplitGroups == 3 ? 64 : 72, kRegsRead = kSplitGroups == 3 ? 128 : 152;
 constexpr int kChunk = 4;       // stages per accumulation chunk (24 MMA steps)
-constexpr int kASlots = 3;      // ring of raw A boxes
+#ifndef MK_TC_A_LDG
+#define MK_TC_A_LDG 0
+#endif
+// How the A tile reaches the split warps: 0 = TMA boxes of 16 shots into a shared-memory ring (the TMA unit's per-row cost
+// makes this the slowest part of the feed, 128 rows per box ~ 1000-1300 clk, but it runs 3 boxes ahead); 1 = every split
+// thread loads the 64 bytes of its receiver row straight from global memory (four 128-bit ld.global.nc issued before the
+// stage's other waits; no TMA, no shared memory for A).  Measured: 1 is far slower (config 2 5.7 ms, config 3 21.3 ms,
+// config 4 286 ms against 4.2 / 5.3 / 66): with one stage per split group in flight the ~1.5 us of a load from HBM sits in
+// the chain of every stage; the register budget of the split warps has no room for the 4-6 stages of prefetch that TMA
+// gives for free.
+constexpr bool kALdg = MK_TC_A_LDG != 0;
+constexpr int kASlots = kALdg ? 0 : 3;      // ring of raw A boxes
 constexpr uint32_t A_BOX_BYTES = BM * 4 * BKC * 4;  // 16 KB: one raw A box = [128 rows][16 shots] = two stages, 128-byte rows
 constexpr uint32_t BLK_BYTES = BKC * 32 * 4;    // 1 KB: one 32-column block of one B region (8 rows of 128 B)
 // Shared memory: the ring of raw A boxes; the ring of raw B tiles as TMA delivered them ([8 shots][nblk x 128 B], dense
@@ -258,6 +269,11 @@ __device__ __forceinline__ uint32_t instr_desc(uint32_t n) {
 
 // explicit shared-space accesses with 32-bit addresses (after the alignment arithmetic on the dynamic shared-memory
 // base the compiler no longer knows the space and would emit generic 64-bit loads and stores)
+__device__ __forceinline__ float4 ldg128_stream(const float4* p) {
+  float4 v;
+  asm volatile("ld.global.nc.L1::no_allocate.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "l"(p));
+  return v;
+}
 __device__ __forceinline__ float4 lds128(uint32_t addr) {
   float4 v;
   asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(addr));
@@ -287,6 +303,9 @@ struct TcParams {
   int nblocks;          // ncols / 32
   int nblk, nrb;        // column blocks per B region, slots of the raw B ring
   size_t s_row;         // floats between consecutive receivers of S^: nb * 2 ldf
+  const float4* Rhat4;  // kALdg: the row block of R^ as float4; receiver row r, bin kk, shots 8 kb .. 8 kb + 7 = 4 float4 at
+  size_t a_row4;        //   Rhat4 + r a_row4 + kk ld4 + 4 kb   (a_row4 = nb ld / 2, ld4 = ld / 2)
+  int ld4;
   uint32_t* progress;   // [grid] raw A boxes each CTA has asked for (zeroed before the launch); NULL when ntl == 1
   int tune;             // MK_OPT_TUNE bits 2..5: parts of the kernel left out (bottleneck measurements; results are wrong)
 };
@@ -362,7 +381,7 @@ k_syn_gemm_tf32x3(const __grid_constant__ CUtensorMap tmA, const __grid_constant
     // nobody runs more than kLead boxes ahead of its slowest sibling — and DRAM reads do drop (155 -> 104 GB), but every
     // CTA then moves at the pace of the momentarily slowest of its group: config 4 66 -> 82 ms, config 2 4.2 -> 5.3 ms.
     // Off by default; the remedy that does not couple the CTAs' pace is a cluster with the A box multicast (not built).
-    if (lane == 0) {
+    if (lane == 0 && !kALdg) {
       int a = 0;
       uint32_t ph = 0;  // ring position and its phase
       const int KB2 = KB / 2;
@@ -397,7 +416,7 @@ k_syn_gemm_tf32x3(const __grid_constant__ CUtensorMap tmA, const __grid_constant
           }
           if (P.progress && (q + 1) % kEvery == 0)
             asm volatile("st.relaxed.gpu.global.u32 [%0], %1;" ::"l"(P.progress + blockIdx.x), "r"(q + 1) : "memory");
-          if (++a == kASlots) {
+          if (++a >= kASlots) {
             a = 0;
             ph ^= 1;
           }
@@ -527,26 +546,50 @@ k_syn_gemm_tf32x3(const __grid_constant__ CUtensorMap tmA, const __grid_constant
     const uint32_t total = (uint32_t)my_tiles * (uint32_t)KB;  // stages this CTA runs through
     int rb = grp % NRB;  // slot of stage it in the raw B ring and its phase
     uint32_t phb = (grp / NRB) & 1;
+    // kALdg: this thread's receiver row of the current tile, and the stage's position in the tile
+    int tile_i = grp / KB, kb = grp % KB, tile_seen = -1;
+    const float4* a_row = nullptr;
     for (uint32_t it = grp; it < total; it += kSplitGroups) {
       const uint32_t box = it >> 1, half = (it & 1) << 6;
-      const int sa = (int)(box % kASlots);  // slot of the raw A box of stage it, and its phase
-      const uint32_t pha = (box / kASlots) & 1;
+      const int sa = kALdg ? 0 : (int)(box % (kASlots ? kASlots : 1));  // slot of the raw A box of stage it, and its phase
+      const uint32_t pha = kALdg ? 0 : (box / (kASlots ? kASlots : 1)) & 1;
+      float4 c[4];
+      if (kALdg) {
+        if (tile_i != tile_seen) {
+          tile_seen = tile_i;
+          const int t = blockIdx.x + tile_i * gridDim.x, kk = t / per_bin, mi = (t - kk * per_bin) / P.ntl, r = mi * BM + ar;
+          a_row = r < P.n ? P.Rhat4 + (size_t)r * P.a_row4 + (size_t)kk * P.ld4 : nullptr;  // rows past the last receiver are zeros
+        }
+        if (a_row) {
+#pragma unroll
+          for (int k = 0; k < 4; ++k) c[k] = ldg128_stream(a_row + 4 * kb + k);
+        } else {
+#pragma unroll
+          for (int k = 0; k < 4; ++k) c[k] = make_float4(0.f, 0.f, 0.f, 0.f);
+        }
+        kb += kSplitGroups;
+        while (kb >= KB) {
+          kb -= KB;
+          ++tile_i;
+        }
+      }
       const uint32_t s = it & (kTmemSlots - 1);  // operand stage: B planes in shared memory, A slot in tensor memory
       if (P.tune & 32) {
         mbar_wait(fullB + rb, phb);
-        mbar_wait(fullA + sa, pha);
+        if (!kALdg) mbar_wait(fullA + sa, pha);
         if (it >= kTmemSlots) mbar_wait(empty + s, ((it >> kLgSlots) - 1) & 1);
         __syncwarp();
         if (lane == 0) {
-          mbar_arrive(emptyA + sa);
+          if (!kALdg) mbar_arrive(emptyA + sa);
           mbar_arrive(emptyB + rb);
           mbar_arrive(split_bar + s);
         }
       } else {
-      mbar_wait(fullA + sa, pha);
-      float4 c[4];
+      if (!kALdg) {
+        mbar_wait(fullA + sa, pha);
 #pragma unroll
-      for (int k = 0; k < 4; ++k) c[k] = lds128(a_base + (uint32_t)sa * A_BOX_BYTES + (a_off[k] ^ half));
+        for (int k = 0; k < 4; ++k) c[k] = lds128(a_base + (uint32_t)sa * A_BOX_BYTES + (a_off[k] ^ half));
+      }
       mbar_wait(fullB + rb, phb);
       const uint32_t raw = raw_base + (uint32_t)rb * REG, st = planes_base + s * PLANES;
       float4 v[3];
@@ -583,7 +626,7 @@ k_syn_gemm_tf32x3(const __grid_constant__ CUtensorMap tmA, const __grid_constant
       tc_fence_before();
       __syncwarp();
       if (lane == 0) {
-        mbar_arrive(emptyA + sa);  // this warp's part of the raw tiles is in registers / tensor memory / the planes
+        if (!kALdg) mbar_arrive(emptyA + sa);  // this warp's part of the raw tiles is in registers / tensor memory / the planes
         mbar_arrive(emptyB + rb);
         mbar_arrive(split_bar + s);
       }
@@ -716,6 +759,9 @@ int launch_syn_tc(mk_ctx* c, const RowBlock& rb, int slot, const float2* d_Nhat,
   P.mt = (rb.nrow + BM - 1) / BM;
   P.ntl = (P.ncols + BN - 1) / BN;
   P.nblocks = P.ncols / 32;
+  P.Rhat4 = reinterpret_cast<const float4*>(rb.Rhat);
+  P.a_row4 = (size_t)c->nb * c->ld / 2;
+  P.ld4 = c->ld / 2;
   P.s_row = (size_t)c->nb * 2 * ldf;
   P.nblk = nblk;
   P.tune = c->tune;
