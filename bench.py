@@ -305,7 +305,8 @@ def secondary_entry(mk, cfg, regime, steps, warmup, local, dev, image=False):
              "focal_point_iterations_per_s": cfg.nfoc * cfg.niter / (ms * 1e-3),
              "contraction_launches_per_step": r["syn_n"] / steps, "gpu_launches": r["launches"], "clocks": r["clocks"],
              "roofline": roofline_of(cfg, nb, nbytes, r["regime_used"], r["syn_n"], r["syn_ms"], r["ms_total"], r["clocks"]),
-             "input_source": "device generator" + (", R in 64-shot chunks" if cfg.k >= 3 else " for G_d / t_d; R^ shared with config 1")}
+             "rhat_layout": "tiled (16 KB boxes of 128 receivers x 16 shots)" if mk.get_info(B.MK_INFO_RHAT_LAYOUT) else "row-major [rec][bin][shot]",
+             "input_source": "device generator" + (", R in 64-shot chunks" if cfg.k >= 3 else " for G_d / t_d; R from the host generator")}
     if image:   # NEXT-1: the double-focusing image of the run just made, timed alone ("about 2% of the total processing time")
         img = torch.empty(cfg.nfoc, dtype=torch.float32, device=dev)
         mk.image(douts["Gminus"], img)
@@ -424,6 +425,8 @@ def run_ours(args):
     mk = B.Marchenko(cfg.n, cfg.n, cfg.nt, cfg.dt, cfg.dx, cfg.fmin, cfg.fmax, rows=(my_rows.start, len(my_rows)))
     mk.set_option(B.MK_OPT_EPS_SAMPLES, cfg.eps)
     mk.set_option(B.MK_OPT_REGIME, args.regime)
+    if args.rhat_layout and cfg.nfoc > 8 and not rows_mode and args.regime in (0, 3):
+        mk.set_option(B.MK_OPT_RHAT_LAYOUT, 1)
     if args.tune:
         mk.set_option(B.MK_OPT_TUNE, args.tune)
     ipc_ptrs = []
@@ -526,11 +529,21 @@ def run_ours(args):
         secondary.append(variant_entry(cfg, R, Gd, td, 5, 3, local, dev, resident_frac=0.25))
         del dGd, dtd, douts, R, Gd, td
         torch.cuda.empty_cache()
-        c2 = configs.get(2)          # same R as config 1 (BASELINE.json): the context and its R^ are reused
+        mk.close()
+        c2 = configs.get(2)          # same R as config 1 (BASELINE.json), ingested again in the layout of the tensor regime
+        mk = B.Marchenko(c2.n, c2.n, c2.nt, c2.dt, c2.dx, c2.fmin, c2.fmax)
+        mk.set_option(B.MK_OPT_EPS_SAMPLES, c2.eps)
+        mk.set_option(B.MK_OPT_RHAT_LAYOUT, args.rhat_layout)
+        mk.load_R_host(gen.R_full(c2))
         # the paper's middle case, 29 focal points, on config 1's R^: the narrow end of the tensor regime
         c29 = configs.scaled(2, nfoc=29, focal="fan:600", name="3GB_29foc")
         secondary.append(secondary_entry(mk, c29, 0, 20, 3, local, dev))
         secondary.append(secondary_entry(mk, c2, 0, args.secondary_steps, 3, local, dev, image=True))
+        mk.close()
+        if args.rhat_layout:         # the FFMA kernel reads the row-major layout
+            mk = B.Marchenko(c2.n, c2.n, c2.nt, c2.dt, c2.dx, c2.fmin, c2.fmax)
+            mk.set_option(B.MK_OPT_EPS_SAMPLES, c2.eps)
+            mk.load_R_host(gen.R_full(c2))
         secondary.append(secondary_entry(mk, c2, 2, args.secondary_steps, 3, local, dev))
         mk.close()
         for k in (3, 4):
@@ -542,6 +555,7 @@ def run_ours(args):
                 continue
             mkk = B.Marchenko(ck.n, ck.n, ck.nt, ck.dt, ck.dx, ck.fmin, ck.fmax)
             mkk.set_option(B.MK_OPT_EPS_SAMPLES, ck.eps)
+            mkk.set_option(B.MK_OPT_RHAT_LAYOUT, args.rhat_layout)
             t0 = time.perf_counter()
             ingest_device(mkk, ck, dev)
             t_ing = time.perf_counter() - t0
@@ -594,6 +608,8 @@ def main():
                          "operand rows per synthesis (strong scaling; SURVEY.md section 8(e) / NEXT-3); rows_fused: the same with the "
                          "all-gather fused into the producing kernels as peer stores over CUDA IPC mappings; the two barriers per synthesis are "
                          "stream memory operations (mk_sync_barrier), no host synchronisation inside a step")
+    ap.add_argument("--rhat-layout", type=int, default=1, help="layout of R^ for the tensor-regime workloads (MK_OPT_RHAT_LAYOUT): "
+                    "1 tiled in 16 KB boxes (default), 0 row-major")
     ap.add_argument("--tune", type=int, default=0, help="MK_OPT_TUNE bit mask (measurement switches of the kernels; include/mk.h)")
     ap.add_argument("--e2e-steps", type=int, default=50)
     ap.add_argument("--cpu-budget", type=float, default=15.0, help="seconds of oracle work for cpu_baseline")

@@ -74,6 +74,13 @@ enum {
                              (DESIGN.md section 6c), not to north_star's.  Must be set before the first mk_load_R
                              (MK_ERR_STATE afterwards); with it mk_load_R needs shot0 and nshots to be multiples of 16
                              (except at the last shot).  Not available on row-sharded or streamed contexts */
+  MK_OPT_RHAT_LAYOUT = 8, /* memory layout of R^ in HBM.  0 (default): [rec][bin][shot], one (receiver, bin) row contiguous —
+                             what the streaming GEMV reads; every regime works on it.  1: TILED for the tensor regime:
+                             [rec / 128][bin][shot / 16] boxes of [128 receivers][16 shots] = 16 KB contiguous (receiver rows
+                             padded to a multiple of 128), the unit the tcgen05 contraction consumes per two stages, fetched
+                             with ONE bulk copy instead of 128 rows 2 MB apart.  Only the tcgen05 regime reads it (every nfoc
+                             then takes regime 3; MK_OPT_REGIME 1 / 2: MK_ERR_INVALID_ARG).  Must be set before the first
+                             mk_load_R (MK_ERR_STATE afterwards); plain contexts only (not sharded / streamed / compressed) */
   MK_OPT_TUNE = 7         /* measurement switches, a bit mask (default 0 = the product path).  bit 0: k_post_fast does not
                              prefetch the next tile's spectra to L2 (same results).  Bits 2..5 leave out one part of the
                              tcgen05 contraction to find what bounds it; the RESULTS ARE WRONG with any of them: 4 = the
@@ -101,7 +108,8 @@ enum {
   MK_INFO_RESIDENT_ROWS = 14, /* rows of R^ kept in HBM (== rows owned unless mk_create_streamed) */
   MK_INFO_WINDOW_ROWS = 15,  /* rows per streaming window (0: R^ is resident) */
   MK_INFO_H2D_BYTES = 16,    /* bytes of R^ the contractions have copied host -> device since mk_create_streamed */
-  MK_INFO_RHAT_BYTES_STORED = 17 /* bytes R^ occupies as stored (padded): 8 per element, 4.25 with MK_OPT_RHAT_FORMAT = 1 */
+  MK_INFO_RHAT_BYTES_STORED = 17, /* bytes R^ occupies as stored (padded): 8 per element, 4.25 with MK_OPT_RHAT_FORMAT = 1 */
+  MK_INFO_RHAT_LAYOUT = 18   /* MK_OPT_RHAT_LAYOUT as set */
 };
 
 /* Create a context for an nshot x nrec x nt reflection response sampled at dt (s) and dx (m), band fmin..fmax (Hz).

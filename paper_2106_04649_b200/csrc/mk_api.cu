@@ -68,6 +68,10 @@ int resolve_regime(mk_ctx* c, int nfoc, int* regime) {
     if (!gemv_supported(c, nfoc) || r > 1) return set_err(c, MK_ERR_INVALID_ARG, "compressed R^ (MK_OPT_RHAT_FORMAT = 1) needs the streaming regime: nfoc <= 8");
     r = 1;
   }
+  if (c->rhat_layout == 1) {  // tiled R^ is read by the tcgen05 contraction only
+    if (r != 0 && r != 3) return set_err(c, MK_ERR_INVALID_ARG, "tiled R^ (MK_OPT_RHAT_LAYOUT = 1) is read by the tcgen05 regime only");
+    r = 3;
+  }
   if (r == 0) r = gemv_supported(c, nfoc) ? 1 : (tc_supported(c) ? 3 : 2);
   if (r == 1 && !gemv_supported(c, nfoc)) return set_err(c, MK_ERR_INVALID_ARG, "GEMV regime needs nfoc <= 8 and ld*nfoc*8 <= 96 KiB");
   if (r < 1 || r > 3) return set_err(c, MK_ERR_INVALID_ARG, "unknown regime");
@@ -437,6 +441,7 @@ static int create_impl(mk_ctx** out, int nshot, int nrec, int nt, double dt, dou
   c->nres = resident_rows;
   if (c->nres > 0) {
     size_t cap = 0;
+    c->rhat_rows_alloc = c->nres;
     const size_t cnt = (size_t)c->nres * c->nb * c->ld;  // the rows this context owns and keeps in HBM
     if (int rc = ensure(c, &c->d_Rhat, &cap, cnt, "Rhat")) return rc;
     if (int rc = check_cuda(c, cudaMemset(c->d_Rhat, 0, cnt * sizeof(float2)), "Rhat memset")) return rc;
@@ -542,7 +547,7 @@ int mk_set_option(mk_ctx* c, int key, double value) {
       if (value != 0.0 && value != 1.0) return set_err(c, MK_ERR_INVALID_ARG, "R^ format must be 0 (complex64) or 1 (q16 block float)");
       if ((int)value == c->rhat_format) return MK_OK;
       if (c->shots_loaded > 0) return set_err(c, MK_ERR_STATE, "MK_OPT_RHAT_FORMAT after mk_load_R: R^ is converted at ingest");
-      if (c->nrow != c->n || c->nres != c->nrow) return set_err(c, MK_ERR_STATE, "compressed R^ is not available on row-sharded or streamed contexts");
+      if (c->nrow != c->n || c->nres != c->nrow || c->rhat_layout != 0) return set_err(c, MK_ERR_STATE, "compressed R^ is not available on row-sharded, streamed or tiled contexts");
       if (int rc = end_run(c, "MK_OPT_RHAT_FORMAT")) return rc;
       const size_t cnt = (size_t)c->n * c->nb * c->ld;
       if ((int)value == 1) {
@@ -562,6 +567,25 @@ int mk_set_option(mk_ctx* c, int key, double value) {
         if (int rc = check_cuda(c, cudaMemset(c->d_Rhat, 0, cnt * sizeof(float2)), "memset")) return rc;
       }
       c->rhat_format = (int)value;
+      return MK_OK;
+    }
+    case MK_OPT_RHAT_LAYOUT: {
+      if (value != 0.0 && value != 1.0) return set_err(c, MK_ERR_INVALID_ARG, "R^ layout must be 0 (row-major) or 1 (tiled)");
+      if ((int)value == c->rhat_layout) return MK_OK;
+      if (c->shots_loaded > 0) return set_err(c, MK_ERR_STATE, "MK_OPT_RHAT_LAYOUT after mk_load_R: R^ is laid out at ingest");
+      if (c->nrow != c->n || c->nres != c->nrow || c->rhat_format != 0)
+        return set_err(c, MK_ERR_STATE, "tiled R^ is not available on row-sharded, streamed or compressed contexts");
+      if ((int)value == 1 && !tc_supported(c)) return set_err(c, MK_ERR_INVALID_ARG, "tiled R^ needs the tcgen05 regime (an sm_100 device)");
+      if (int rc = end_run(c, "MK_OPT_RHAT_LAYOUT")) return rc;
+      const size_t rows = (int)value == 1 ? (size_t)((c->n + 127) / 128) * 128 : (size_t)c->n;  // receiver rows padded to whole tiles
+      const size_t cnt = rows * c->nb * c->ld;
+      size_t cap = 0;
+      release(c, &c->d_Rhat, &cap);
+      c->device_bytes -= (size_t)c->rhat_rows_alloc * c->nb * c->ld * sizeof(float2);
+      if (int rc = ensure(c, &c->d_Rhat, &cap, cnt, "Rhat")) return rc;
+      if (int rc = check_cuda(c, cudaMemset(c->d_Rhat, 0, cnt * sizeof(float2)), "memset")) return rc;
+      c->rhat_rows_alloc = (int)rows;
+      c->rhat_layout = (int)value;
       return MK_OK;
     }
     case MK_OPT_TUNE:
@@ -620,6 +644,7 @@ int mk_get_info(mk_ctx* c, int key, double* value) {
     case MK_INFO_RESIDENT_ROWS: *value = c->nres; return MK_OK;
     case MK_INFO_WINDOW_ROWS: *value = c->win_rows; return MK_OK;
     case MK_INFO_H2D_BYTES: *value = c->h2d_bytes; return MK_OK;
+    case MK_INFO_RHAT_LAYOUT: *value = c->rhat_layout; return MK_OK;
     default: return set_err(c, MK_ERR_INVALID_ARG, "unknown info key");
   }
 }

@@ -56,6 +56,7 @@ struct FastParams {
   const float* wscale; // [ns]     dt * w[s] (k_load_R_fast)
   const float2* tw1k;  // [32][32]  e^{-2 pi i k1 t / 1024}
   int nt, n, nb, klo, ld, ldf, nfoc;
+  int tiled;  // k_load_R_fast: layout of R^ (rhat_index)
   int r0;  // first receiver row of this context (row sharding): grid row b handles receiver r0 + b
 };
 
@@ -385,7 +386,7 @@ k_load_R_fast(const float* __restrict__ Rt, float2* __restrict__ Rhat, FastParam
     band_out_pairs<HF>(smem, ns, lgST, P, [&](int kk, int t0, float2 X0, float2 X1, bool two) {
       const int s = shot0 + g0 + t0;  // even
       const float c0 = weight(s), c1 = two ? weight(s + 1) : 0.f;
-      float2* dst = Rhat + ((size_t)(r - P.r0) * P.nb + kk) * P.ld + s;
+      float2* dst = Rhat + rhat_index(P.tiled, r - P.r0, kk, s, P.nb, P.ld);  // s even: (s, s + 1) share one 16-byte chunk in either layout
       if (two) *reinterpret_cast<float4*>(dst) = make_float4(c0 * X0.x, c0 * X0.y, c1 * X1.x, c1 * X1.y);
       else *dst = make_float2(c0 * X0.x, c0 * X0.y);  // column s + 1 belongs to another chunk (or is padding)
     });
@@ -393,7 +394,7 @@ k_load_R_fast(const float* __restrict__ Rt, float2* __restrict__ Rhat, FastParam
     band_out<HF>(smem, ns, lgST, P, [&](int tl, int kk, float2 X) {
       const int s = shot0 + g0 + tl;
       const float sc = weight(s);
-      Rhat[((size_t)(r - P.r0) * P.nb + kk) * P.ld + s] = make_float2(sc * X.x, sc * X.y);
+      Rhat[rhat_index(P.tiled, r - P.r0, kk, s, P.nb, P.ld)] = make_float2(sc * X.x, sc * X.y);
     });
   }
 }
@@ -593,6 +594,7 @@ FastParams make_fast(const mk_ctx* c, int nfoc, int ldf) {
   P.ld = c->ld;
   P.ldf = ldf;
   P.nfoc = nfoc;
+  P.tiled = c->rhat_layout;
   P.r0 = c->r0;
   return P;
 }

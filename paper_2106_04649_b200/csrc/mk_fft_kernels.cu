@@ -213,7 +213,7 @@ __global__ void __launch_bounds__(kThreads) k_load_R(const float* __restrict__ R
     const int s = shot0 + g0 + tl;
     const float sc = __ldg(P.wscale + s);
     const float2 X = mkfft::rfft_bin(smem + tl * MP, P.plan, P.tw, P.klo + kk);
-    Rhat[((size_t)(r - P.r0) * P.nb + kk) * P.ld + s] = make_float2(sc * X.x, sc * X.y);
+    Rhat[rhat_index(P.tiled, r - P.r0, kk, s, P.nb, P.ld)] = make_float2(sc * X.x, sc * X.y);
   }
 }
 
@@ -372,6 +372,7 @@ FftParams make_params(const mk_ctx* c, int nfoc, int ldf) {
   P.ld = c->ld;
   P.ldf = ldf;
   P.nfoc = nfoc;
+  P.tiled = c->rhat_layout;
   P.r0 = c->r0;
   return P;
 }

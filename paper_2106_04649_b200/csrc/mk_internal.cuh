@@ -115,6 +115,8 @@ struct mk_ctx {
   int run_regime = 0;   // regime of the run in progress / of the reserved operands: set by mk_begin and mk_operand_reserve only
   int last_regime = 0;  // regime of the last contraction launch (MK_INFO_REGIME_USED; information only)
   size_t smem_sm = 0;   // shared memory per SM
+  int rhat_rows_alloc = 0;  // receiver rows d_Rhat was allocated for (tiled: padded to a multiple of 128)
+  int rhat_layout = 0;  // MK_OPT_RHAT_LAYOUT: 0 row-major [rec][bin][shot], 1 tiled for the tensor regime
   int tune = 0;         // MK_OPT_TUNE: measurement switches (bit mask, include/mk.h)
   int dev = 0;          // CUDA device the context lives on (made current at the top of every entry point)
 
@@ -133,8 +135,19 @@ struct FftParams {
   const float2* tw;
   const float* wscale;  // [ns] dt * w[s] (k_load_R)
   int n, nb, klo, ld, ldf, nfoc;
+  int tiled;  // k_load_R: layout of R^ (rhat_index)
   int r0;  // first receiver row of this context (grid row b handles receiver r0 + b; R^ is stored from row r0 on)
 };
+
+// R^ element (receiver row rr of the block, bin kk, shot s) -> offset in float2.  Row-major (the default, what the streaming
+// GEMV wants): [row][bin][ld].  Tiled (MK_OPT_RHAT_LAYOUT = 1, for the tensor regime): [row / 128][bin][shot / 16] boxes of
+// [128 rows][16 shots] = 16 KB contiguous, the unit the tcgen05 contraction feeds on, stored already in the shared-memory
+// layout its split warps read (the 16-byte chunk c = (s % 16) / 2 of row r sits at chunk position c ^ (r & 7)).
+__host__ __device__ __forceinline__ size_t rhat_index(int tiled, int rr, int kk, int s, int nb, int ld) {
+  if (!tiled) return ((size_t)rr * nb + kk) * ld + s;
+  const int row = rr & 127, c = (s & 15) >> 1;
+  return ((((size_t)(rr >> 7) * nb + kk) * (ld >> 4) + (s >> 4)) * 128 + row) * 16 + (size_t)(((c ^ (row & 7)) << 1) | (s & 1));
+}
 
 // a block of consecutive receiver rows of R^ as one launch sees it: Rhat points at row r0 (its [nrow][nb][ld] block may be
 // the resident part, a streaming window, or the mapped host part during ingest); S^ is indexed by the global receiver

@@ -115,7 +115,11 @@ constexpr int kChunk = 4;       // stages per accumulation chunk (24 MMA steps)
 // config 4 286 ms against 4.2 / 5.3 / 66): with one stage per split group in flight the ~1.5 us of a load from HBM sits in
 // the chain of every stage; the register budget of the split warps has no room for the 4-6 stages of prefetch that TMA
 // gives for free.
-constexpr bool kALdg = MK_TC_A_LDG != 0;
+constexpr bool kALdg = MK_TC_A_LDG == 1;
+// MK_TC_A_LDG = 2: the A ring is filled by cp.async (LDGSTS) of the whole producer warp instead of one TMA instruction:
+// per box 32 instructions of 32 lanes x 16 bytes (8 lanes = one 128-byte row, 4 rows per instruction), written in the same
+// swizzled layout, completion through cp.async.mbarrier.arrive on the box's full barrier.
+constexpr bool kACpAsync = MK_TC_A_LDG == 2;
 constexpr int kASlots = kALdg ? 0 : 3;      // ring of raw A boxes
 constexpr uint32_t A_BOX_BYTES = BM * 4 * BKC * 4;  // 16 KB: one raw A box = [128 rows][16 shots] = two stages, 128-byte rows
 constexpr uint32_t BLK_BYTES = BKC * 32 * 4;    // 1 KB: one 32-column block of one B region (8 rows of 128 B)
@@ -213,6 +217,12 @@ __device__ __forceinline__ void tma_load_2d(const void* tmap, uint64_t* bar, voi
                : "memory");
 }
 
+__device__ __forceinline__ void bulk_load(uint64_t* bar, void* dst, const void* src, uint32_t bytes) {
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(smem_u32(dst)), "l"(src), "r"(bytes),
+               "r"(smem_u32(bar))
+               : "memory");
+}
+
 __device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
 __device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
 
@@ -306,6 +316,7 @@ struct TcParams {
   const float4* Rhat4;  // kALdg: the row block of R^ as float4; receiver row r, bin kk, shots 8 kb .. 8 kb + 7 = 4 float4 at
   size_t a_row4;        //   Rhat4 + r a_row4 + kk ld4 + 4 kb   (a_row4 = nb ld / 2, ld4 = ld / 2)
   int ld4;
+  int a_tiled;          // R^ is stored in 16 KB boxes (MK_OPT_RHAT_LAYOUT = 1): one bulk copy per box
   uint32_t* progress;   // [grid] raw A boxes each CTA has asked for (zeroed before the launch); NULL when ntl == 1
   int tune;             // MK_OPT_TUNE bits 2..5: parts of the kernel left out (bottleneck measurements; results are wrong)
 };
@@ -352,7 +363,7 @@ k_syn_gemm_tf32x3(const __grid_constant__ CUtensorMap tmA, const __grid_constant
     mbar_init(acc_full + 0, 1);
     mbar_init(acc_full + 1, 1);
     for (int a = 0; a < kASlots; ++a) {
-      mbar_init(fullA + a, 1);
+      mbar_init(fullA + a, kACpAsync ? 32 : 1);
       mbar_init(emptyA + a, 2 * kSplitWarps);  // the box has two halves = two stages, each read by the four warps of one group
     }
     drained[0] = drained[1] = 0;
@@ -381,7 +392,33 @@ k_syn_gemm_tf32x3(const __grid_constant__ CUtensorMap tmA, const __grid_constant
     // nobody runs more than kLead boxes ahead of its slowest sibling — and DRAM reads do drop (155 -> 104 GB), but every
     // CTA then moves at the pace of the momentarily slowest of its group: config 4 66 -> 82 ms, config 2 4.2 -> 5.3 ms.
     // Off by default; the remedy that does not couple the CTAs' pace is a cluster with the A box multicast (not built).
-    if (lane == 0 && !kALdg) {
+    if (kACpAsync) {
+      int a = 0;
+      uint32_t ph = 0;
+      const int KB2 = KB / 2;
+      const int sub = lane >> 3, ch = lane & 7;  // this lane: rows sub, sub + 4, ..., 16-byte chunk ch of the 128-byte row
+      const uint32_t a_smem = smem_u32(smem);
+      for (int t = blockIdx.x; t < ntiles; t += gridDim.x) {
+        const int kk = t / per_bin, rem = t - kk * per_bin, mi = rem / P.ntl;
+        for (int kb2 = 0; kb2 < KB2; ++kb2) {
+          mbar_wait(emptyA + a, ph ^ 1);
+          const uint32_t dst0 = a_smem + (uint32_t)a * A_BOX_BYTES;
+#pragma unroll 8
+          for (int i = 0; i < BM / 4; ++i) {
+            const int row = 4 * i + sub, r = mi * BM + row;
+            const bool in = r < P.n;
+            const float4* src = P.Rhat4 + (size_t)(in ? r : 0) * P.a_row4 + (size_t)kk * P.ld4 + 8 * kb2 + ch;
+            const uint32_t dst = dst0 + (uint32_t)row * 128 + (uint32_t)((ch ^ (row & 7)) << 4);
+            asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(dst), "l"(src), "r"(in ? 16 : 0) : "memory");  // rows past the last receiver: zeros
+          }
+          asm volatile("cp.async.mbarrier.arrive.noinc.shared::cta.b64 [%0];" ::"r"(smem_u32(fullA + a)) : "memory");
+          if (++a >= kASlots) {
+            a = 0;
+            ph ^= 1;
+          }
+        }
+      }
+    } else if (lane == 0 && !kALdg) {
       int a = 0;
       uint32_t ph = 0;  // ring position and its phase
       const int KB2 = KB / 2;
@@ -412,7 +449,11 @@ k_syn_gemm_tf32x3(const __grid_constant__ CUtensorMap tmA, const __grid_constant
             mbar_arrive(fullA + a);
           } else {
             mbar_expect_tx(fullA + a, A_BOX_BYTES);
-            tma_load_3d(&tmA, fullA + a, smem + (size_t)a * A_BOX_BYTES, kb2 * 4 * BKC, kk, mi * BM);  // rows past the last receiver arrive as zeros
+            if (P.a_tiled)  // the box is 16 KB contiguous in HBM, already in the swizzled layout (rows past the last receiver are stored zeros)
+              bulk_load(fullA + a, smem + (size_t)a * A_BOX_BYTES,
+                        reinterpret_cast<const uint8_t*>(P.Rhat4) + (((size_t)mi * P.nb + kk) * KB2 + kb2) * A_BOX_BYTES, A_BOX_BYTES);
+            else
+              tma_load_3d(&tmA, fullA + a, smem + (size_t)a * A_BOX_BYTES, kb2 * 4 * BKC, kk, mi * BM);  // rows past the last receiver arrive as zeros
           }
           if (P.progress && (q + 1) % kEvery == 0)
             asm volatile("st.relaxed.gpu.global.u32 [%0], %1;" ::"l"(P.progress + blockIdx.x), "r"(q + 1) : "memory");
@@ -762,6 +803,7 @@ int launch_syn_tc(mk_ctx* c, const RowBlock& rb, int slot, const float2* d_Nhat,
   P.Rhat4 = reinterpret_cast<const float4*>(rb.Rhat);
   P.a_row4 = (size_t)c->nb * c->ld / 2;
   P.ld4 = c->ld / 2;
+  P.a_tiled = c->rhat_layout == 1;
   P.s_row = (size_t)c->nb * 2 * ldf;
   P.nblk = nblk;
   P.tune = c->tune;

@@ -22,9 +22,9 @@ def problem(cfg, focs=None):
 
 
 def gpu_chain(cfg, R, Gd, td, niter=None, regime=0, keep_iters=True, host_api=False, outputs=("f1plus", "f1min", "G", "Gplus", "Gminus"),
-              fft_path=0, streamed=None, rhat_format=0):
+              fft_path=0, streamed=None, rhat_format=0, rhat_layout=0):
     """Runs the CUDA path through the C ABI; returns numpy arrays like oracle.marchenko does.
-    streamed = (resident_rows, window_rows): out-of-core R^ (mk_create_streamed); rhat_format: MK_OPT_RHAT_FORMAT."""
+    streamed = (resident_rows, window_rows): out-of-core R^ (mk_create_streamed); rhat_format: MK_OPT_RHAT_FORMAT; rhat_layout: MK_OPT_RHAT_LAYOUT."""
     import torch
     from paper_2106_04649_b200 import binding as B
     niter = cfg.niter if niter is None else niter
@@ -36,6 +36,7 @@ def gpu_chain(cfg, R, Gd, td, niter=None, regime=0, keep_iters=True, host_api=Fa
         mk.set_option(B.MK_OPT_REGIME, regime)
         mk.set_option(B.MK_OPT_FFT_PATH, fft_path)
         mk.set_option(B.MK_OPT_RHAT_FORMAT, rhat_format)
+        mk.set_option(B.MK_OPT_RHAT_LAYOUT, rhat_layout)
         if host_api:
             mk.load_R_host(np.ascontiguousarray(R))
             houts = {nm: np.empty((nfoc, cfg.n, cfg.nt), np.float32) for nm in outputs + ("N_last",)}

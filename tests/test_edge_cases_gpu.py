@@ -7,7 +7,8 @@ import numpy as np
 import pytest
 
 import oracle
-from _util import rel_l2
+from _util import calibrated, gpu_chain, problem, rel_l2
+from paper_2106_04649_b200 import configs
 
 pytestmark = pytest.mark.gpu
 
@@ -261,3 +262,45 @@ def test_overlapping_outputs_are_refused():
         torch.cuda.synchronize()
         ref = oracle.marchenko(R, Gd.cpu().numpy(), td.cpu().numpy(), dt, dx, 10.0, 100.0, 1, 2)
         assert rel_l2(lib_plus.cpu().numpy(), ref["f1plus"]) <= TOL_FINAL
+
+
+@pytest.mark.parametrize("k,n,nt,nfoc", [(2, 70, 512, 70), (3, 150, 2048, 19), (4, 60, 1024, 33), (1, 300, 256, 5), (1, 129, 64, 1)])
+def test_tiled_rhat_layout_equals_the_row_major_one(k, n, nt, nfoc):
+    """MK_OPT_RHAT_LAYOUT = 1: R^ stored in 16 KB boxes of [128 receivers][16 shots] for the tcgen05 contraction (one bulk
+    copy per box instead of a TMA box of 128 rows 2 MB apart).  Same kernel, same arithmetic, another address map: the
+    whole chain must equal the row-major regime-3 run BIT FOR BIT and meet the oracle; receiver counts that are no
+    multiple of 128 (padded tile rows), ragged focal batches, one focal point (which takes regime 3 here as well)."""
+    import oracle
+    cfg = calibrated(configs.scaled(k, n=n, nt=nt, nfoc=nfoc, focal="single:400" if nfoc == 1 else "fan:250", niter=5))
+    R, Gd, td = problem(cfg)
+    a = gpu_chain(cfg, R, Gd, td, regime=3, rhat_layout=0)
+    b = gpu_chain(cfg, R, Gd, td, regime=0, rhat_layout=1)
+    assert b["regime_used"] == 3
+    for nm in ("N_iters", "f1plus", "f1min", "G", "Gplus", "Gminus"):
+        assert np.array_equal(a[nm], b[nm]), nm
+    ref = oracle.marchenko(R, Gd, td, cfg.dt, cfg.dx, cfg.fmin, cfg.fmax, cfg.niter, cfg.eps)
+    errs = [rel_l2(b["N_iters"][i], ref["N_iters"][i]) for i in range(cfg.niter)]
+    fin = max(rel_l2(b[nm], ref[nm]) for nm in ("f1plus", "f1min", "G", "Gplus", "Gminus"))
+    print(f"\n[tiled R^ n={n} nt={nt} nfoc={nfoc}] bit-identical to the row-major layout; per-iteration max {max(errs):.2e}, finals {fin:.2e}")
+    assert max(errs) <= 2e-5 and fin <= 1e-4
+
+
+def test_tiled_rhat_layout_rules():
+    import torch
+    from paper_2106_04649_b200 import binding as B
+    cfg = configs.scaled(1, n=40, nt=64, nfoc=2, focal="fan:250", niter=1)
+    R, Gd, td = problem(cfg)
+    dev = torch.device("cuda:0")
+    with B.Marchenko(cfg.n, cfg.n, cfg.nt, cfg.dt, cfg.dx, cfg.fmin, cfg.fmax) as mk:
+        mk.set_option(B.MK_OPT_RHAT_LAYOUT, 1)
+        mk.set_option(B.MK_OPT_REGIME, 1)
+        mk.load_R(torch.from_numpy(R).to(dev))
+        with pytest.raises(B.MkError):                      # the streaming GEMV cannot read the tiled layout
+            mk.begin(torch.from_numpy(Gd).to(dev), torch.from_numpy(td).to(dev))
+        with pytest.raises(B.MkError):                      # laid out at ingest
+            mk.set_option(B.MK_OPT_RHAT_LAYOUT, 0)
+        with pytest.raises(B.MkError):
+            mk.set_option(B.MK_OPT_RHAT_FORMAT, 1)
+    with B.Marchenko(cfg.n, cfg.n, cfg.nt, cfg.dt, cfg.dx, cfg.fmin, cfg.fmax, rows=(0, 20)) as mk:
+        with pytest.raises(B.MkError):                      # plain contexts only
+            mk.set_option(B.MK_OPT_RHAT_LAYOUT, 1)
