@@ -83,14 +83,22 @@ namespace mk {
 
 namespace {
 
+// MK_TC_K16 = 1: a stage is 16 shots (one whole A box, two 8-shot sub-stages of B planes, 12 MMAs) and the N tile 128 columns
+// (tensor memory: 2 x 128 accumulator columns + 4 x 64 columns of A); 0: 8-shot stages, N tile MK_TC_BN.  Measured: half as
+// many, fatter stages change nothing (config 2 4.46 ms, config 3 5.18, config 4 67.1, narrow batches 367 us against 4.02 /
+// 5.21 / 64.0 / 354): the cost is not per stage.
+#ifndef MK_TC_K16
+#define MK_TC_K16 0
+#endif
 #ifndef MK_TC_BN
-#define MK_TC_BN 192
+#define MK_TC_BN (MK_TC_K16 ? 128 : 192)
 #endif
 constexpr int BM = 128;         // rows (receivers) per tile = TMEM lanes
 constexpr int BN = MK_TC_BN;    // real columns (2 per focal point) per tile = TMEM columns per accumulator (128 or 192)
 constexpr int BKC = 8;          // shots (complex k) per stage
 constexpr int kMaxRawB = 8;     // ring of raw B tiles: as many as fit (8 at N = 192)
-constexpr int kTmemSlots = MK_TC_BN == 128 ? 8 : 4, kLgSlots = MK_TC_BN == 128 ? 3 : 2;  // ring of operand stages: stage it uses A slot it % 4 in tensor memory and B planes it % 4 in shared
+constexpr int kSub = MK_TC_K16 ? 2 : 1;  // 8-shot sub-stages per stage
+constexpr int kTmemSlots = (MK_TC_BN == 128 && !MK_TC_K16) ? 8 : 4, kLgSlots = (MK_TC_BN == 128 && !MK_TC_K16) ? 3 : 2;  // ring of operand stages: stage it uses A slot it % 4 in tensor memory and B planes it % 4 in shared
                                 // memory, both free once the MMAs of stage it - 4 retired
 constexpr int kSplitWarps = 4, kSplitThreads = 32 * kSplitWarps;  // per split group
 #ifndef MK_TC_SPLIT_GROUPS
@@ -104,7 +112,7 @@ constexpr int kThreads = 128 + kSplitGroups * kSplitThreads + 32 * kReadWarps;  
 // control warpgroup gives most of its share back and the read-out warps, who hold 96 running sums each, take it:
 // 128 x 32 + 384 x 64 + 256 x 128 = 61440.  (Two split groups: 640 threads at 96; 128 x 32 + 256 x 72 + 256 x 152.)
 constexpr int kRegsControl = 32, kRegsSplit = kSplitGroups == 3 ? 64 : 72, kRegsRead = kSplitGroups == 3 ? 128 : 152;
-constexpr int kChunk = 4;       // stages per accumulation chunk (24 MMA steps)
+constexpr int kChunk = 4 / kSub;  // stages per accumulation chunk (24 MMA steps)
 #ifndef MK_TC_A_LDG
 #define MK_TC_A_LDG 0
 #endif
@@ -120,7 +128,8 @@ constexpr bool kALdg = MK_TC_A_LDG == 1;
 // per box 32 instructions of 32 lanes x 16 bytes (8 lanes = one 128-byte row, 4 rows per instruction), written in the same
 // swizzled layout, completion through cp.async.mbarrier.arrive on the box's full barrier.
 constexpr bool kACpAsync = MK_TC_A_LDG == 2;
-constexpr int kASlots = kALdg ? 0 : 3;      // ring of raw A boxes
+constexpr int kMinASlots = kALdg ? 0 : 3, kMaxASlots = kALdg ? 0 : 12;  // ring of raw A boxes: as many as fit (bytes in flight per SM are
+                                                                          // what the rate of R^ from HBM follows: 3 boxes = 48 KB gave 3.5 TB/s)
 constexpr uint32_t A_BOX_BYTES = BM * 4 * BKC * 4;  // 16 KB: one raw A box = [128 rows][16 shots] = two stages, 128-byte rows
 constexpr uint32_t BLK_BYTES = BKC * 32 * 4;    // 1 KB: one 32-column block of one B region (8 rows of 128 B)
 // Shared memory: the ring of raw A boxes; the ring of raw B tiles as TMA delivered them ([8 shots][nblk x 128 B], dense
@@ -128,12 +137,12 @@ constexpr uint32_t BLK_BYTES = BKC * 32 * 4;    // 1 KB: one 32-column block of 
 // B1_hi, B1_lo; nblk = min(6, columns / 32).  The distance B0 -> B1 (two regions) is the stride-byte-offset of the B
 // descriptors: the second group of four K rows of every MMA is the rotated copy of the first.  The raw rings run ahead of
 // the operand stages by their own length: the latency of the loads is not in the loop that the MMAs close.
-__host__ __device__ constexpr uint32_t planes_bytes(int nblk) { return 4 * (uint32_t)nblk * BLK_BYTES; }
-__host__ __device__ constexpr uint32_t fixed_smem(int nblk) { return kASlots * A_BOX_BYTES + kTmemSlots * planes_bytes(nblk); }
-constexpr size_t kSmemExtra = 1024 /*alignment slack*/ + 512 /*barriers, counters: (2 x 8 + 2 x 4 + 2 + 2 x 3) x 8 + (4 + 2 + 1) x 4 bytes*/;
+__host__ __device__ constexpr uint32_t planes_bytes(int nblk) { return kSub * 4 * (uint32_t)nblk * BLK_BYTES; }
+__host__ __device__ constexpr uint32_t fixed_smem(int nblk) { return kMinASlots * A_BOX_BYTES + kTmemSlots * planes_bytes(nblk); }
+constexpr size_t kSmemExtra = 1024 /*alignment slack*/ + 512 /*barriers, counters: (2 x 8 + 2 x 8 + 2 + 2 x 12) x 8 + (8 + 2 + 1) x 4 bytes*/;
 constexpr uint32_t kTmemCols = 512;
 constexpr uint32_t kTmemA = 2 * BN;  // first column of the A ring
-constexpr uint32_t kTmemAStage = 32; // columns per slot: K step j at 16 j: A_hi (8 columns), A_lo (8 columns)
+constexpr uint32_t kTmemAStage = 32 * kSub; // columns per slot: K step j at 16 j: A_hi (8 columns), A_lo (8 columns)
 static_assert(kTmemA + kTmemSlots * kTmemAStage <= kTmemCols, "tensor memory budget");
 
 // ---------------------------------------------------------------------------------------------- PTX wrappers
@@ -311,7 +320,7 @@ struct TcParams {
   int mt, ntl;          // tiles along M and N; N tile ni covers the 32-column blocks [ni nblocks / ntl, (ni + 1) nblocks / ntl):
                         // widths differ by at most one block, so the CTAs that share an A tile run in step and meet in L2
   int nblocks;          // ncols / 32
-  int nblk, nrb;        // column blocks per B region, slots of the raw B ring
+  int nblk, nrb, na;    // column blocks per B region, slots of the raw B ring, slots of the raw A ring
   size_t s_row;         // floats between consecutive receivers of S^: nb * 2 ldf
   const float4* Rhat4;  // kALdg: the row block of R^ as float4; receiver row r, bin kk, shots 8 kb .. 8 kb + 7 = 4 float4 at
   size_t a_row4;        //   Rhat4 + r a_row4 + kk ld4 + 4 kb   (a_row4 = nb ld / 2, ld4 = ld / 2)
@@ -329,18 +338,19 @@ k_syn_gemm_tf32x3(const __grid_constant__ CUtensorMap tmA, const __grid_constant
   extern __shared__ uint8_t smem_raw[];
   uint8_t* smem = reinterpret_cast<uint8_t*>(((uintptr_t)smem_raw + 1023) & ~(uintptr_t)1023);
   const int NRB = P.nrb;
-  const uint32_t REG = (uint32_t)P.nblk * BLK_BYTES, PLANES = 4 * REG;  // REG: bytes of one B region = of one raw B tile
-  uint8_t* planes = smem + kASlots * A_BOX_BYTES;            // the A ring comes first, then the operand stages,
+  const uint32_t REG = (uint32_t)P.nblk * BLK_BYTES, SUBPL = 4 * REG, PLANES = kSub * SUBPL, RAW = kSub * REG;  // REG: bytes of one B region of 8 shots
+  const int kASlots = P.na;
+  uint8_t* planes = smem + (size_t)kASlots * A_BOX_BYTES;            // the A ring comes first, then the operand stages,
   uint8_t* rawB = planes + (size_t)kTmemSlots * PLANES;      // then the raw B ring
-  uint64_t* bars = reinterpret_cast<uint64_t*>(rawB + (size_t)NRB * REG);
+  uint64_t* bars = reinterpret_cast<uint64_t*>(rawB + (size_t)NRB * RAW);
   uint64_t* fullB = bars;                          // [kMaxRawB] raw B tile landed
   uint64_t* emptyB = bars + kMaxRawB;              // [kMaxRawB] the split group that took the stage has read it
   uint64_t* empty = bars + 2 * kMaxRawB;           // [kTmemSlots] MMAs of the operand stage retired
   uint64_t* split_bar = empty + kTmemSlots;        // [kTmemSlots] the split warps are done with the stage
   uint64_t* acc_full = split_bar + kTmemSlots;     // [2] chunk accumulator complete
   uint64_t* fullA = acc_full + 2;                  // [kASlots] raw A box landed
-  uint64_t* emptyA = fullA + kASlots;              // [kASlots] both halves of the box have been read
-  uint32_t* ready = reinterpret_cast<uint32_t*>(emptyA + kASlots);  // [kTmemSlots] uses of the stage that are ready for the MMAs (relay)
+  uint64_t* emptyA = fullA + kMaxASlots;           // [kASlots] both halves of the box have been read
+  uint32_t* ready = reinterpret_cast<uint32_t*>(emptyA + kMaxASlots);  // [kTmemSlots] uses of the stage that are ready for the MMAs (relay)
   uint32_t* drained = ready + kTmemSlots;      // [2] read-out warps done with a use of TMEM buffer b (counts up; PER BUFFER:
                                                // one sum over both would let fast warps' arrivals for the other buffer stand in for
                                                // a slow warp's missing one)
@@ -348,7 +358,7 @@ k_syn_gemm_tf32x3(const __grid_constant__ CUtensorMap tmA, const __grid_constant
 
   const int warp = __shfl_sync(0xffffffffu, threadIdx.x >> 5, 0), lane = threadIdx.x & 31;  // warp-uniform by construction
   const int per_bin = P.mt * P.ntl, ntiles = P.nb * per_bin;
-  const int KB = P.ld / BKC;  // stages per tile
+  const int KB = P.ld / (BKC * kSub);  // stages per tile
 
   if (threadIdx.x == 0) {
     for (int s = 0; s < NRB; ++s) {
@@ -364,7 +374,7 @@ k_syn_gemm_tf32x3(const __grid_constant__ CUtensorMap tmA, const __grid_constant
     mbar_init(acc_full + 1, 1);
     for (int a = 0; a < kASlots; ++a) {
       mbar_init(fullA + a, kACpAsync ? 32 : 1);
-      mbar_init(emptyA + a, 2 * kSplitWarps);  // the box has two halves = two stages, each read by the four warps of one group
+      mbar_init(emptyA + a, (2 / kSub) * kSplitWarps);  // 8-shot stages: the box has two halves = two stages, each read by the four warps of one group
     }
     drained[0] = drained[1] = 0;
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
@@ -395,7 +405,7 @@ k_syn_gemm_tf32x3(const __grid_constant__ CUtensorMap tmA, const __grid_constant
     if (kACpAsync) {
       int a = 0;
       uint32_t ph = 0;
-      const int KB2 = KB / 2;
+      const int KB2 = KB * kSub / 2;  // A boxes per tile
       const int sub = lane >> 3, ch = lane & 7;  // this lane: rows sub, sub + 4, ..., 16-byte chunk ch of the 128-byte row
       const uint32_t a_smem = smem_u32(smem);
       for (int t = blockIdx.x; t < ntiles; t += gridDim.x) {
@@ -421,7 +431,7 @@ k_syn_gemm_tf32x3(const __grid_constant__ CUtensorMap tmA, const __grid_constant
     } else if (lane == 0 && !kALdg) {
       int a = 0;
       uint32_t ph = 0;  // ring position and its phase
-      const int KB2 = KB / 2;
+      const int KB2 = KB * kSub / 2;  // A boxes per tile
       uint32_t q = 0;   // boxes asked for so far
       const int sib0 = (int)blockIdx.x - (int)blockIdx.x % P.ntl;
       constexpr uint32_t kLead = 16, kEvery = 8;  // looked at every 8th box only: a look is ntl - 1 round trips to L2
@@ -495,12 +505,16 @@ k_syn_gemm_tf32x3(const __grid_constant__ CUtensorMap tmA, const __grid_constant
           if (elect_one()) {
             // small terms first; a chunk starts from zero
             if (!(P.tune & 8)) {
-            umma_tf32_ts(d, ta + 8, loB_hi0 + off, hiB, idesc, kb != kb0);
-            umma_tf32_ts(d, ta, loB_lo0 + off, hiB, idesc, 1);
-            umma_tf32_ts(d, ta, loB_hi0 + off, hiB, idesc, 1);
-            umma_tf32_ts(d, ta + 24, loB_hi0 + off + 32, hiB, idesc, 1);
-            umma_tf32_ts(d, ta + 16, loB_lo0 + off + 32, hiB, idesc, 1);
-            umma_tf32_ts(d, ta + 16, loB_hi0 + off + 32, hiB, idesc, 1);
+#pragma unroll
+              for (int h = 0; h < kSub; ++h) {
+                const uint32_t o = off + h * (SUBPL >> 4), a = ta + 32 * h;
+                umma_tf32_ts(d, a + 8, loB_hi0 + o, hiB, idesc, kb != kb0 || h != 0);
+                umma_tf32_ts(d, a, loB_lo0 + o, hiB, idesc, 1);
+                umma_tf32_ts(d, a, loB_hi0 + o, hiB, idesc, 1);
+                umma_tf32_ts(d, a + 24, loB_hi0 + o + 32, hiB, idesc, 1);
+                umma_tf32_ts(d, a + 16, loB_lo0 + o + 32, hiB, idesc, 1);
+                umma_tf32_ts(d, a + 16, loB_hi0 + o + 32, hiB, idesc, 1);
+              }
             }
             umma_commit(empty + s);
           }
@@ -542,10 +556,10 @@ k_syn_gemm_tf32x3(const __grid_constant__ CUtensorMap tmA, const __grid_constant
           if (P.tune & (64 | 256)) {
             mbar_arrive(fullB + s);
           } else {
-            mbar_expect_tx(fullB + s, REG);
+            mbar_expect_tx(fullB + s, RAW);
             // eight dense rows of nblk x 128 bytes (8 rows for the TMA unit instead of 8 nblk in the tensor core's layout);
             // columns past 2 ldf arrive as zeros (and still count their bytes)
-            tma_load_2d(&tmB, fullB + s, rawB + (size_t)s * REG, tile_col0(P, ni), kk * P.ld + kb * BKC);
+            tma_load_2d(&tmB, fullB + s, rawB + (size_t)s * RAW, tile_col0(P, ni), kk * P.ld + kb * BKC * kSub);
           }
           if (++s == NRB) {
             s = 0;
@@ -590,8 +604,10 @@ k_syn_gemm_tf32x3(const __grid_constant__ CUtensorMap tmA, const __grid_constant
     // kALdg: this thread's receiver row of the current tile, and the stage's position in the tile
     int tile_i = grp / KB, kb = grp % KB, tile_seen = -1;
     const float4* a_row = nullptr;
+    static_assert(!(kALdg && kSub == 2), "direct global loads of A exist for 8-shot stages only");
     for (uint32_t it = grp; it < total; it += kSplitGroups) {
-      const uint32_t box = it >> 1, half = (it & 1) << 6;
+      // 8-shot stages: stage it is half it % 2 of box it / 2; 16-shot stages: stage it is box it
+      const uint32_t box = kSub == 2 ? it : it >> 1, half0 = kSub == 2 ? 0u : (it & 1) << 6;
       const int sa = kALdg ? 0 : (int)(box % (kASlots ? kASlots : 1));  // slot of the raw A box of stage it, and its phase
       const uint32_t pha = kALdg ? 0 : (box / (kASlots ? kASlots : 1)) & 1;
       float4 c[4];
@@ -626,41 +642,43 @@ k_syn_gemm_tf32x3(const __grid_constant__ CUtensorMap tmA, const __grid_constant
           mbar_arrive(split_bar + s);
         }
       } else {
-      if (!kALdg) {
-        mbar_wait(fullA + sa, pha);
-#pragma unroll
-        for (int k = 0; k < 4; ++k) c[k] = lds128(a_base + (uint32_t)sa * A_BOX_BYTES + (a_off[k] ^ half));
-      }
+      if (!kALdg) mbar_wait(fullA + sa, pha);
       mbar_wait(fullB + rb, phb);
-      const uint32_t raw = raw_base + (uint32_t)rb * REG, st = planes_base + s * PLANES;
-      float4 v[3];
+      const uint32_t raw = raw_base + (uint32_t)rb * RAW, st = planes_base + s * PLANES, ta = a_tmem + s * kTmemAStage;
 #pragma unroll
-      for (int i = 0; i < 3; ++i)
-        if (i < nmine) v[i] = lds128(raw + (((uint32_t)wt + i * kSplitThreads) << 4));
-      // The operand stage (B planes, A slot) is free once the MMAs of stage it - 4 have retired: empty[s] cannot run a second
-      // phase ahead, its next completion belongs to stage it itself.
-      if (it >= kTmemSlots) {
-        mbar_wait(empty + s, ((it >> kLgSlots) - 1) & 1);
-        tc_fence_after();
-      }
-      // B: raw tile -> B0_hi (copy), B0_lo, and B1 = i B0 (every float4 holds two (re, im) pairs) hi / lo
+      for (int h = 0; h < kSub; ++h) {  // the 8-shot sub-stages of the stage
+        if (!kALdg) {
 #pragma unroll
-      for (int i = 0; i < 3; ++i)
-        if (i < nmine && !(P.tune & 16)) {
-          const uint32_t dst = st + b_dst[i];
-          const float4 l = lo4(v[i]);
-          sts128(dst, v[i]);
-          sts128(dst + REG, l);
-          sts128(dst + 2 * REG, make_float4(-v[i].y, v[i].x, -v[i].w, v[i].z));
-          sts128(dst + 3 * REG, make_float4(-l.y, l.x, -l.w, l.z));
+          for (int k = 0; k < 4; ++k) c[k] = lds128(a_base + (uint32_t)sa * A_BOX_BYTES + (a_off[k] ^ (half0 | ((uint32_t)h << 6))));
         }
-      // A -> tensor memory: per K step hi (re0 re1 re2 re3 | im0 im1 im2 im3), lo beside it
-      const uint32_t ta = a_tmem + s * kTmemAStage;
+        float4 v[3];
 #pragma unroll
-      for (int j = 0; j < 2; ++j) {
-        const float4 re = make_float4(c[2 * j].x, c[2 * j].z, c[2 * j + 1].x, c[2 * j + 1].z),
-                     im = make_float4(c[2 * j].y, c[2 * j].w, c[2 * j + 1].y, c[2 * j + 1].w);
-        tmem_st16(ta + 16 * j, re, im, lo4(re), lo4(im));
+        for (int i = 0; i < 3; ++i)
+          if (i < nmine) v[i] = lds128(raw + h * REG + (((uint32_t)wt + i * kSplitThreads) << 4));
+        // The operand stage (B planes, A slot) is free once the MMAs of stage it - 4 have retired: empty[s] cannot run a
+        // second phase ahead, its next completion belongs to stage it itself.
+        if (h == 0 && it >= kTmemSlots) {
+          mbar_wait(empty + s, ((it >> kLgSlots) - 1) & 1);
+          tc_fence_after();
+        }
+        // B: raw tile -> B0_hi (copy), B0_lo, and B1 = i B0 (every float4 holds two (re, im) pairs) hi / lo
+#pragma unroll
+        for (int i = 0; i < 3; ++i)
+          if (i < nmine && !(P.tune & 16)) {
+            const uint32_t dst = st + h * SUBPL + b_dst[i];
+            const float4 l = lo4(v[i]);
+            sts128(dst, v[i]);
+            sts128(dst + REG, l);
+            sts128(dst + 2 * REG, make_float4(-v[i].y, v[i].x, -v[i].w, v[i].z));
+            sts128(dst + 3 * REG, make_float4(-l.y, l.x, -l.w, l.z));
+          }
+        // A -> tensor memory: per K step hi (re0 re1 re2 re3 | im0 im1 im2 im3), lo beside it
+#pragma unroll
+        for (int j = 0; j < 2; ++j) {
+          const float4 re = make_float4(c[2 * j].x, c[2 * j].z, c[2 * j + 1].x, c[2 * j + 1].z),
+                       im = make_float4(c[2 * j].y, c[2 * j].w, c[2 * j + 1].y, c[2 * j + 1].w);
+          tmem_st16(ta + 32 * h + 16 * j, re, im, lo4(re), lo4(im));
+        }
       }
       asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
       asm volatile("fence.proxy.async.shared::cta;" ::: "memory");  // generic-proxy writes -> visible to the tensor core
@@ -763,7 +781,7 @@ int encode(mk_ctx* c, EncodeTiledFn enc, void* out, const void* base, int rank, 
 bool tc_supported(const mk_ctx* c) {
   int major = 0;
   cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, c->dev);
-  return major == 10 && c->smem_optin >= fixed_smem(1) + 2 * BLK_BYTES + kSmemExtra;
+  return major == 10 && c->smem_optin >= fixed_smem(1) + 2 * kSub * BLK_BYTES + kSmemExtra;
 }
 
 int launch_syn_tc(mk_ctx* c, const RowBlock& rb, int slot, const float2* d_Nhat, float2* d_Shat, int ldf) {
@@ -787,7 +805,7 @@ int launch_syn_tc(mk_ctx* c, const RowBlock& rb, int slot, const float2* d_Nhat,
     // memory; the split warps put it into the tensor core's MN-major layout
     const cuuint64_t dims[2] = {(cuuint64_t)2 * ldf, (cuuint64_t)c->nb * c->ld};
     const cuuint64_t str[1] = {(cuuint64_t)2 * ldf * 4};
-    const cuuint32_t box[2] = {(cuuint32_t)nblk * 32, BKC};  // nblk is a function of ldf: one cache key
+    const cuuint32_t box[2] = {(cuuint32_t)nblk * 32, BKC * kSub};  // nblk is a function of ldf: one cache key
     if (int rc = encode(c, enc, c->tmap_B[slot], d_Nhat, 2, dims, str, box, CU_TENSOR_MAP_SWIZZLE_NONE, "B")) return rc;
     c->tmap_B_key[slot] = d_Nhat;
     c->tmap_B_ldf[slot] = ldf;
@@ -807,11 +825,22 @@ int launch_syn_tc(mk_ctx* c, const RowBlock& rb, int slot, const float2* d_Nhat,
   P.s_row = (size_t)c->nb * 2 * ldf;
   P.nblk = nblk;
   P.tune = c->tune;
-  if (c->smem_optin < fixed_smem(nblk) + kSmemExtra + 2 * (size_t)nblk * BLK_BYTES)
+  const size_t raw_b = (size_t)kSub * nblk * BLK_BYTES;
+  if (c->smem_optin < fixed_smem(nblk) + kSmemExtra + 2 * raw_b)
     return set_err(c, MK_ERR_INVALID_ARG, "not enough shared memory for the tcgen05 contraction");
-  P.nrb = (int)std::min<size_t>(kMaxRawB, (c->smem_optin - kSmemExtra - fixed_smem(nblk)) / ((size_t)nblk * BLK_BYTES));
-  if (c->tune & 512) P.nrb = std::min(P.nrb, 3);
-  const size_t kSmemBytes = fixed_smem(nblk) + (size_t)P.nrb * nblk * BLK_BYTES + kSmemExtra;
+  // what is left after the operand stages goes to the raw rings: 6 B tiles first, then A boxes (the deeper ring: R^ comes
+  // from HBM or L2 at the rate the bytes in flight allow), then up to 8 B tiles
+  size_t left = c->smem_optin - kSmemExtra - fixed_smem(nblk);
+  P.nrb = (int)std::min<size_t>(6, left / raw_b);
+  left -= P.nrb * raw_b;
+  P.na = kMinASlots + (kALdg ? 0 : (int)std::min<size_t>(kMaxASlots - kMinASlots, left / A_BOX_BYTES));
+  left -= (size_t)(P.na - kMinASlots) * A_BOX_BYTES;
+  P.nrb += (int)std::min<size_t>(kMaxRawB - P.nrb, left / raw_b);
+  if (c->tune & 512) {
+    P.nrb = std::min(P.nrb, 3);
+    P.na = kMinASlots;
+  }
+  const size_t kSmemBytes = (size_t)P.na * A_BOX_BYTES + kTmemSlots * (size_t)planes_bytes(nblk) + (size_t)P.nrb * raw_b + kSmemExtra;
   const int ntiles = P.nb * P.mt * P.ntl;
   // (in step: a multiple of ntl, so that every CTA keeps its N tile and its siblings, see the A producer)
   const bool in_step = (c->tune & 1024) && P.ntl > 1 && P.ntl <= c->num_sms;  // measurement switch, off: it costs more than it saves
