@@ -264,7 +264,7 @@ def test_overlapping_outputs_are_refused():
         assert rel_l2(lib_plus.cpu().numpy(), ref["f1plus"]) <= TOL_FINAL
 
 
-@pytest.mark.parametrize("k,n,nt,nfoc", [(2, 70, 512, 70), (3, 150, 2048, 19), (4, 60, 1024, 33), (1, 300, 256, 5), (1, 129, 64, 1)])
+@pytest.mark.parametrize("k,n,nt,nfoc", [(2, 70, 512, 70), (3, 150, 2048, 19), (4, 60, 1024, 33), (1, 300, 256, 5), (1, 129, 512, 1)])
 def test_tiled_rhat_layout_equals_the_row_major_one(k, n, nt, nfoc):
     """MK_OPT_RHAT_LAYOUT = 1: R^ stored in 16 KB boxes of [128 receivers][16 shots] for the tcgen05 contraction (one bulk
     copy per box instead of a TMA box of 128 rows 2 MB apart).  Same kernel, same arithmetic, another address map: the
@@ -282,6 +282,7 @@ def test_tiled_rhat_layout_equals_the_row_major_one(k, n, nt, nfoc):
     errs = [rel_l2(b["N_iters"][i], ref["N_iters"][i]) for i in range(cfg.niter)]
     fin = max(rel_l2(b[nm], ref[nm]) for nm in ("f1plus", "f1min", "G", "Gplus", "Gminus"))
     print(f"\n[tiled R^ n={n} nt={nt} nfoc={nfoc}] bit-identical to the row-major layout; per-iteration max {max(errs):.2e}, finals {fin:.2e}")
+    assert np.linalg.norm(ref["N_iters"][-1]) > 0          # the series is alive: the bounds are not vacuous
     assert max(errs) <= 2e-5 and fin <= 1e-4
 
 

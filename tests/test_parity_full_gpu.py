@@ -69,7 +69,12 @@ def test_full_size_single_steps_on_seeded_subset(k):
     _single_steps(k, _subset_shape(k))
 
 
-def _single_steps(k, subset_shape):
+def test_full_size_config2_with_tiled_rhat():
+    """The launch configuration bench.py times for the tensor-regime entries: R^ in the tiled layout (MK_OPT_RHAT_LAYOUT = 1)."""
+    _single_steps(2, _subset_shape(2), rhat_layout=1)
+
+
+def _single_steps(k, subset_shape, rhat_layout=0):
     if k in SKIP:
         pytest.skip("MK_PARITY_SKIP")
     import torch
@@ -96,6 +101,7 @@ def _single_steps(k, subset_shape):
     with B.Marchenko(n, n, nt, cfg.dt, cfg.dx, cfg.fmin, cfg.fmax) as mk:
         mk.set_option(B.MK_OPT_EPS_SAMPLES, cfg.eps)
         mk.set_option(B.MK_OPT_REGIME, REGIME)
+        mk.set_option(B.MK_OPT_RHAT_LAYOUT, rhat_layout)
         for s0 in range(0, n, 64):                                    # BASELINE.json config 4: 64-shot chunks
             s1 = min(s0 + 64, n)
             chunk = gR.take(np.arange(s0, s1))
@@ -137,7 +143,7 @@ def _single_steps(k, subset_shape):
         for nm in ("G", "Gplus", "Gminus"):
             mk.finish({nm: buf})
             fin_err[nm] = rel_l2(buf[focs_t][:, recs_t].cpu().numpy(), fin[nm])
-    print(f"\n[config {k} full size n={n} nt={nt} nfoc={nfoc} regime={regime}; subset {len(recs)} rec x {len(focs)} foc; "
+    print(f"\n[config {k} full size n={n} nt={nt} nfoc={nfoc} regime={regime}{' tiled R^' if rhat_layout else ''}; subset {len(recs)} rec x {len(focs)} foc; "
           f"ingest {t_load:.0f} s, oracle {t_or:.0f} s on {oracle.num_threads()} threads] per-iteration max {max(errs):.2e}; "
           + " ".join(f"{a}={b:.1e}" for a, b in fin_err.items()))
     assert norms[-1] > 1e-7 * norms[0] > 0, norms                    # the series is alive: the bound is not vacuous
