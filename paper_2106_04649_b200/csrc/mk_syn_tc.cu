@@ -38,8 +38,12 @@
 //       - B delivered as 8 dense rows of <= 768 bytes per stage instead of 8 nblk rows in the tensor core's layout; the
 //         split warps, who read every element anyway, write the MN-major swizzled planes themselves;
 //     A-only feed 4.25 -> 2.72 ms;
-//   * the raw rings (A: 3 boxes = 6 stages, B: 8 tiles) run ahead of the four operand stages by their own length, so the
-//     latency of the loads is not inside the loop the MMAs close (empty -> split -> ready -> MMA -> empty);
+//   * the raw rings (A: 3 .. 12 boxes of two stages each, as many as shared memory allows; B: <= 8 tiles) run ahead of the
+//     four operand stages by their own length, so the latency of the loads is not inside the loop the MMAs close
+//     (empty -> split -> ready -> MMA -> empty);
+//   * with R^ in its TILED layout (MK_OPT_RHAT_LAYOUT = 1: the box is 16 KB contiguous in HBM, stored pre-swizzled) the
+//     producer issues one cp.async.bulk per box instead of a TMA box of 128 rows that lie 2 MB apart: config 2 4.23 -> 4.12 ms
+//     per contraction, DRAM traffic 6.1 -> 4.3 GB (3.9 algorithmic), config 4 146 -> 105 GB;
 //   * A IN TENSOR MEMORY: with both operands in shared memory the MMAs read 6 x (4 KB of A + 8 KB of B) per stage and the
 //     split warps moved 56 KB more; now the MMAs read only B, the split warps read A once and tcgen05.st it, and A_hi /
 //     A_lo occupy no shared memory (which is what pays for the raw rings);
@@ -54,14 +58,15 @@
 //     nothing.  What holds config 3 at ~650 clk per stage against 384 clk of MMAs is not identified;
 //   * the chip is POWER-bound under this kernel (1000 W cap: 1.6-1.8 GHz): every byte through L2, every byte through shared
 //     memory and every spinning warp costs SM clock.
-// Result: tensor pipe 55 % -> 69 % active, config 2 4.74 -> 4.2 ms, config 3 7.35 -> 5.3 ms per contraction.
+// Result: tensor pipe 55 % -> 68-69 % active (config 4: 78-81 %), config 2 4.74 -> 4.12 ms, config 3 7.35 -> 5.28 ms per contraction.
 //
 // Tensor memory (512 columns): two chunk accumulators of BN = 192 columns, and a ring of four A slots of 32 columns
 // (per K step 8 columns of A_hi and 8 of A_lo; lane = receiver row of the tile).
 //
 // Kernel: persistent, one CTA per SM, warp-specialised, 768 threads = 6 warpgroups with their own register budgets
 // (setmaxnreg: the kernel starts at 80 registers per thread; control 32, split 64, read-out 128) —
-//   warp 0      TMA producer of the raw A boxes [128 receivers][16 shots] (SWIZZLE_128B), ring of 3
+//   warp 0      producer of the raw A boxes [128 receivers][16 shots]: TMA (SWIZZLE_128B) from the row-major R^, one bulk copy from
+//               the tiled R^; ring of 3 .. 12
 //   warp 3      TMA producer of the raw B tiles [8 shots][<= 192 floats] (dense rows), ring of <= 8
 //   warp 1      tcgen05.mma issuer (one thread): kind::tf32, M = 128, N <= 192, K = 8, A from TMEM, B from shared memory;
 //               tcgen05.commit releases the operand stage / publishes the chunk
