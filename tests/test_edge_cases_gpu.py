@@ -305,3 +305,39 @@ def test_tiled_rhat_layout_rules():
     with B.Marchenko(cfg.n, cfg.n, cfg.nt, cfg.dt, cfg.dx, cfg.fmin, cfg.fmax, rows=(0, 20)) as mk:
         with pytest.raises(B.MkError):                      # plain contexts only
             mk.set_option(B.MK_OPT_RHAT_LAYOUT, 1)
+
+
+def test_sync_and_row_ingest_argument_rules():
+    """mk_sync_* and mk_load_R_rows refuse what they cannot do (MK_ERR_*), and a one-rank barrier is a no-op."""
+    import torch
+    from paper_2106_04649_b200 import binding as B
+    cfg = configs.scaled(1, n=40, nt=64, nfoc=2, focal="fan:250", niter=1)
+    R, Gd, td = problem(cfg)
+    dev = torch.device("cuda:0")
+    with B.Marchenko(cfg.n, cfg.n, cfg.nt, cfg.dt, cfg.dx, cfg.fmin, cfg.fmax) as mk:
+        with pytest.raises(B.MkError):
+            mk.sync_barrier()                                # before mk_sync_create
+        with pytest.raises(B.MkError):
+            mk.sync_flags()
+        with pytest.raises(B.MkError):
+            mk.sync_create(2, 2)                             # rank out of range
+        with pytest.raises(B.MkError):
+            mk.sync_create(0, 9)                             # more ranks than flag slots
+        mk.sync_create(0, 1)
+        mk.sync_barrier()                                    # one rank: nothing to wait for
+        mk.sync_create(0, 2)
+        assert mk.sync_flags() != 0
+        with pytest.raises(B.MkError):
+            mk.sync_barrier()                                # two ranks, peers not attached
+        with pytest.raises(B.MkError):
+            mk.sync_attach([None, None])                     # the peer's flag array is missing
+        # mk_load_R_rows on an unsharded context is mk_load_R
+        mk.load_R_rows(torch.from_numpy(R).to(dev))
+        a = torch.empty((cfg.nfoc, cfg.n, cfg.nt), dtype=torch.float32, device=dev)
+        mk.run(torch.from_numpy(Gd).to(dev), torch.from_numpy(td).to(dev), 1, {"G": a})
+        torch.cuda.synchronize()
+    ref = gpu_chain(cfg, R, Gd, td, niter=1, keep_iters=False, outputs=("G",))
+    assert np.array_equal(a.cpu().numpy(), ref["G"])
+    with B.Marchenko(cfg.n, cfg.n, cfg.nt, cfg.dt, cfg.dx, cfg.fmin, cfg.fmax, streamed=(10, 10)) as mk:
+        with pytest.raises(B.MkError):                       # out-of-core R^: rows do not all live on the device
+            mk.load_R_rows(torch.from_numpy(R).to(dev))
