@@ -87,7 +87,9 @@ enum {
                              read-out warps do not read tensor memory, 8 = no MMA is issued, 16 = the split warps skip the
                              B planes, 32 = the split warps do nothing, 64 = no TMA load is issued,
                              128 = no A tile is loaded, 256 = no B tile is loaded.  512: the raw B ring has 3 slots; 1024: the CTAs
-                             that share an A tile keep in step through global progress counters (same results, slower) */
+                             that share an A tile keep in step through global progress counters (same results, slower); 2048: the
+                             fused pass of nt = 4096 takes eight traces per CTA (512 threads, one CTA per SM) instead of four
+                             (same results, same speed) */
 };
 
 /* mk_get_info keys (values returned as double) */

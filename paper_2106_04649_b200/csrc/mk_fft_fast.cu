@@ -68,12 +68,16 @@ template <int HF>
 __device__ __forceinline__ void trace_sync(int tl) {
   if (HF == 1) {
     __syncwarp();
-  } else {  // named barriers 1..4 (immediate ids, so that only these are reserved); FT <= 4 when HF = 2
+  } else {  // named barriers 1..8 (immediate ids, so that only these are reserved); FT <= 8
     switch (tl) {
       case 0: asm volatile("bar.sync 1, %0;" ::"n"(32 * HF) : "memory"); break;
       case 1: asm volatile("bar.sync 2, %0;" ::"n"(32 * HF) : "memory"); break;
       case 2: asm volatile("bar.sync 3, %0;" ::"n"(32 * HF) : "memory"); break;
-      default: asm volatile("bar.sync 4, %0;" ::"n"(32 * HF) : "memory"); break;
+      case 3: asm volatile("bar.sync 4, %0;" ::"n"(32 * HF) : "memory"); break;
+      case 4: asm volatile("bar.sync 5, %0;" ::"n"(32 * HF) : "memory"); break;
+      case 5: asm volatile("bar.sync 6, %0;" ::"n"(32 * HF) : "memory"); break;
+      case 6: asm volatile("bar.sync 7, %0;" ::"n"(32 * HF) : "memory"); break;
+      default: asm volatile("bar.sync 8, %0;" ::"n"(32 * HF) : "memory"); break;
     }
   }
 }
@@ -366,7 +370,7 @@ __device__ __forceinline__ void store_operand2(const OperandOut& O, int ld, int 
 // ------------------------------------------------------------------------------------------------ k_load_R_fast
 // grid (ceil(nshots / ST), nrec); Rt: [nshots][nrec][nt]                                        (a0)
 template <int HF>
-__global__ void __launch_bounds__(256, 2)
+__global__ void __launch_bounds__(256 * HF, 3 - HF)
 k_load_R_fast(const float* __restrict__ Rt, float2* __restrict__ Rhat, FastParams P, int shot0, int nshots, int lgST) {
   extern __shared__ float2 smem[];
   constexpr int TS = Geo<HF>::TS;
@@ -402,7 +406,7 @@ k_load_R_fast(const float* __restrict__ Rt, float2* __restrict__ Rhat, FastParam
 // ------------------------------------------------------------------------------------------------ k_fwd_fast
 // grid (ceil(nfoc / FT), n); src: [nfoc][n][nt]                                                        (a1, a6)
 template <int HF>
-__global__ void __launch_bounds__(256, 2)
+__global__ void __launch_bounds__(256 * HF, 3 - HF)
 k_fwd_fast(const float* __restrict__ src, const __grid_constant__ OperandOut O, FastParams P, int lgFT, int conj_out, float* __restrict__ init_Tsrc) {
   extern __shared__ float2 smem[];
   constexpr int TS = Geo<HF>::TS;
@@ -440,7 +444,7 @@ k_fwd_fast(const float* __restrict__ src, const __grid_constant__ OperandOut O, 
 // ------------------------------------------------------------------------------------------------ k_inv_fast
 // grid (ceil(nfoc / FT), n); spec: [n][nb][ldf]; out[j] = sS*S[j] + sA*A[j] + sB*B[(nt-j)%nt]              (a3, a7)
 template <int HF>
-__global__ void __launch_bounds__(256, 2)
+__global__ void __launch_bounds__(256 * HF, 3 - HF)
 k_inv_fast(const float2* __restrict__ spec, FastParams P, int lgFT, float* __restrict__ out, float sS,
            const float* __restrict__ A, float sA, const float* __restrict__ B, float sB) {
   extern __shared__ float2 smem[];
@@ -491,7 +495,7 @@ k_inv_fast(const float2* __restrict__ spec, FastParams P, int lgFT, float* __res
 // (Theta is symmetric in +-t, so Theta T = T Theta; w is real, so FFT(T w) = conj FFT(w).)  Every global access of
 // the time fields is a natural-order float2 row; only the optional N_i copy of an even step is written reversed.
 template <int HF>
-__global__ void __launch_bounds__(256, 2)
+__global__ void __launch_bounds__(256 * HF, 3 - HF)
 k_post_fast(const float2* __restrict__ Shat, float2* __restrict__ phat, const __grid_constant__ OperandOut O, const int* __restrict__ h,
             float* __restrict__ f1plus, float* __restrict__ f1min, FastParams P, int lgFT, int parity_even,
             float* __restrict__ Ni_out, int pf_dist) {
@@ -608,7 +612,8 @@ struct Shape {
 // the CTA-wide phases P1 / P5.  Measured on config 1 (601 traces per launch): 256 threads 29 us (3 waves), 32 threads 40 us
 Shape shape_for(const mk_ctx* c, int count) {
   const int HF = c->nt / 2048;
-  int lg = HF == 1 ? 3 : 2;  // 256 threads and <= 68 KB of traces per CTA: two CTAs per SM overlap each other's memory phases
+  int lg = HF == 1 || (c->tune & 2048) ? 3 : 2;  // 256 threads and <= 68 KB of traces per CTA: two CTAs per SM overlap each other's memory phases
+                                                 // (MK_OPT_TUNE bit 11: nt = 4096 with eight traces = 512 threads, one CTA per SM)
   while (lg > 0 && (1 << (lg - 1)) >= count) --lg;
   Shape s;
   s.lg = lg;
