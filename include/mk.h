@@ -217,6 +217,24 @@ int mk_synthesis(mk_ctx* ctx, const float* d_N_in, float* d_S_out, int nfoc);
  * d_Gminus: [nfoc][nrec][nt] fp32 as returned by mk_run / mk_finish for the current run; d_image: [nfoc] fp32. */
 int mk_image(mk_ctx* ctx, const float* d_Gminus, float* d_image);
 
+/* The same image for callers that cannot call cudaMalloc (code under CUDA graph capture, tight serving loops, harnesses
+ * that forbid it): this ONE entry point allocates nothing and frees nothing.  The partial sums of the imaging kernels go
+ * to a static device array of MK_IMAGE_STATIC_MAX_PARTIALS doubles (128 KB, part of the library image: every GPU that
+ * loads the library holds it until the process exits) instead of the context's scratch buffer.
+ *   d_Gminus, d_f1plus: [nfoc][nrec][nt] fp32 device inputs (the two fields are passed explicitly; no run is needed, the
+ *   context supplies nrec, nt, dt, dx, the device and the stream); d_image: [nfoc] fp32 device output.
+ * Same kernels, same grid, same order of summation as mk_image: for the fields of a run the result is bit-identical.
+ * Limit: nfoc x (receiver chunks per focal point) partial sums must fit the array.  The grid has fewer than
+ * nfoc + 32 x (SM count) of them, so every nfoc <= MK_IMAGE_STATIC_MAX_PARTIALS - 32 x (SM count) fits (nfoc <= 11648 on
+ * a 148-SM B200) and no nfoc > MK_IMAGE_STATIC_MAX_PARTIALS does; beyond the limit the call returns MK_ERR_INVALID_ARG
+ * with the numbers in mk_last_error and launches nothing (use mk_image).
+ * The first call on a device looks the array's device address up (cudaGetSymbolAddress, no allocation); later calls reuse
+ * it.  Every call on a device shares the one array, which keeps the previous call's contents: nothing has to start at
+ * zero (each partial sum is written before it is read), but two calls that overlap on the GPU (different streams or
+ * contexts on one device, without an ordering between them) race on it and give garbage.  Calls on one stream are safe. */
+enum { MK_IMAGE_STATIC_MAX_PARTIALS = 16384 };
+int mk_image_static(mk_ctx* ctx, const float* d_Gminus, const float* d_f1plus, float* d_image, int nfoc);
+
 /* ---- NEXT-3: receiver-row sharding across GPUs ------------------------------------------
  * The B200 equivalent of the paper's multi-GPU scheme (every output trace depends on one
  * (receiver, focal point) pair): rank g owns the receiver rows row0 .. row0+nrows-1 of R^ (read-only,

@@ -24,8 +24,9 @@ SYMBOLS = ("mk_create", "mk_destroy", "mk_set_stream", "mk_set_option", "mk_get_
            "mk_run", "mk_run_host", "mk_begin", "mk_step", "mk_finish", "mk_synthesis", "mk_image", "mk_last_error",
            "mk_version", "mk_create_sharded", "mk_operand", "mk_operand_exchanged", "mk_finish_prepare", "mk_finish_complete",
            "mk_operand_reserve", "mk_operand_attach", "mk_step_contract", "mk_step_post", "mk_ipc_export", "mk_ipc_open", "mk_ipc_close",
-           "mk_set_geometry", "mk_create_streamed", "mk_sync_create", "mk_sync_flags", "mk_sync_attach", "mk_sync_barrier", "mk_load_R_rows")
+           "mk_set_geometry", "mk_create_streamed", "mk_sync_create", "mk_sync_flags", "mk_sync_attach", "mk_sync_barrier", "mk_load_R_rows", "mk_image_static")
 MK_FIELD_GMINUS, MK_FIELD_GPLUS = 1, 2
+MK_IMAGE_STATIC_MAX_PARTIALS = 16384   # doubles in the static scratch array of mk_image_static
 
 
 class mk_outputs(C.Structure):
@@ -77,6 +78,7 @@ def load():
     L.mk_finish.argtypes = [vp, C.POINTER(mk_outputs)]
     L.mk_synthesis.argtypes = [vp, vp, vp, ci]
     L.mk_image.argtypes = [vp, vp, vp]
+    L.mk_image_static.argtypes = [vp, vp, vp, vp, ci]
     L.mk_create_sharded.argtypes = [C.POINTER(vp), ci, ci, ci, cd, cd, cd, cd, ci, ci]
     L.mk_create_streamed.argtypes = [C.POINTER(vp), ci, ci, ci, cd, cd, cd, cd, ci, ci]
     L.mk_operand.argtypes = [vp, ci, C.POINTER(mk_operand_view)]
@@ -336,6 +338,15 @@ class Marchenko:
         import torch
         self._check(self._L.mk_image(self._h, _dev_ptr(d_Gminus, torch.float32, self._nfoc * self.nrec * self.nt),
                                      _dev_ptr(d_image, torch.float32, self._nfoc)))
+
+    def image_static(self, d_Gminus, d_f1plus, d_image):
+        """mk_image_static: the image of two explicit fields [nfoc][nrec][nt] -> d_image [nfoc], with the kernels' scratch in
+        a static device array (no cudaMalloc / cudaFree in the call); nfoc is d_image's length.  Needs no run."""
+        import torch
+        nfoc = int(d_image.numel())
+        self._check(self._L.mk_image_static(self._h, _dev_ptr(d_Gminus, torch.float32, nfoc * self.nrec * self.nt),
+                                            _dev_ptr(d_f1plus, torch.float32, nfoc * self.nrec * self.nt),
+                                            _dev_ptr(d_image, torch.float32, nfoc), nfoc))
 
 
 def ipc_export(ptr: int) -> bytes:

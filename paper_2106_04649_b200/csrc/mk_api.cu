@@ -7,6 +7,7 @@
 #include <cmath>
 #include <cstdio>
 #include <cstring>
+#include <mutex>
 #include <new>
 
 #include "mk_fft_common.cuh"
@@ -339,6 +340,33 @@ using namespace mk;
     cudaGetLastError();                                        \
     return set_err((ctx), MK_ERR_CUDA, "cudaSetDevice failed"); \
   }
+
+// ---- mk_image_static: scratch of the imaging kernels for callers that cannot allocate --------------------------------
+// The per (focal point, receiver chunk) partial sums of k_image_partial in a file-scope array instead of a cudaMalloc'ed
+// buffer: part of the module image, so every GPU that loads libmk.so holds these 128 KB until the process exits.  In host
+// code the NAME of the array is only a host-side stand-in, never a device address: its address on each device is asked for
+// once (cudaGetSymbolAddress with that device current) and kept per device.  All calls on a device share the array.
+static __device__ __align__(256) double g_image_static_part[MK_IMAGE_STATIC_MAX_PARTIALS];
+
+namespace {
+constexpr int kMaxStaticDevices = 64;
+std::mutex g_image_static_mu;
+double* g_image_static_ptr[kMaxStaticDevices] = {};   // [device] -> device address of g_image_static_part, or null
+
+// called with the context's device current (MK_GUARD); no allocation: the array exists since the module was loaded
+int image_static_scratch(mk_ctx* c, double** out) {
+  if (c->dev < 0 || c->dev >= kMaxStaticDevices) return set_err(c, MK_ERR_INVALID_ARG, "mk_image_static: device ordinal beyond 63");
+  std::lock_guard<std::mutex> lk(g_image_static_mu);
+  if (!g_image_static_ptr[c->dev]) {
+    double* p = nullptr;
+    if (int rc = check_cuda(c, cudaGetSymbolAddress((void**)&p, g_image_static_part), "cudaGetSymbolAddress(g_image_static_part)")) return rc;
+    if (!p) return set_err(c, MK_ERR_CUDA, "cudaGetSymbolAddress returned a null address for g_image_static_part");
+    g_image_static_ptr[c->dev] = p;
+  }
+  *out = g_image_static_ptr[c->dev];
+  return MK_OK;
+}
+}  // namespace
 
 extern "C" {
 
@@ -1145,6 +1173,34 @@ int mk_image(mk_ctx* c, const float* d_Gminus, float* d_image) {
   k_image_final<<<(c->nfoc + 127) / 128, 128, 0, c->stream>>>(c->d_img_part, d_image, c->nfoc, nchunk);
   ++c->launches;
   return check_cuda(c, cudaGetLastError(), "k_image");
+}
+
+int mk_image_static(mk_ctx* c, const float* d_Gminus, const float* d_f1plus, float* d_image, int nfoc) {
+  MK_GUARD(c);
+  if (!d_Gminus || !d_f1plus || !d_image || nfoc <= 0) return set_err(c, MK_ERR_INVALID_ARG, "mk_image_static: bad arguments");
+  const float wm = (float)(c->dt * c->dx), we = (float)(c->dt * c->dx * 0.5);
+  // the same grid as mk_image (same partial sums in the same order: the two calls give the same bits)
+  const long long traces = (long long)nfoc * c->n;
+  int rows_per_cta = (int)std::max<long long>(1, traces / ((long long)c->num_sms * 16));
+  rows_per_cta = std::min(rows_per_cta, c->n);
+  const int nchunk = (c->n + rows_per_cta - 1) / rows_per_cta;
+  const long long nparts = (long long)nfoc * nchunk;
+  if (nparts > MK_IMAGE_STATIC_MAX_PARTIALS) {
+    char buf[224];
+    snprintf(buf, sizeof buf,
+             "mk_image_static: %d focal points x %d receiver chunks = %lld partial sums, the static scratch array holds "
+             "MK_IMAGE_STATIC_MAX_PARTIALS = %d (use mk_image)", nfoc, nchunk, nparts, (int)MK_IMAGE_STATIC_MAX_PARTIALS);
+    return set_err(c, MK_ERR_INVALID_ARG, buf);
+  }
+  double* part = nullptr;
+  if (int rc = image_static_scratch(c, &part)) return rc;
+  // nothing to clear: k_image_partial writes every one of the nparts sums before k_image_final reads them
+  k_image_partial<<<dim3(nfoc, nchunk), kImgThreads, 0, c->stream>>>(d_Gminus, d_f1plus, part, c->n, c->nt, rows_per_cta, wm, we);
+  ++c->launches;
+  if (int rc = check_cuda(c, cudaGetLastError(), "k_image_partial (static scratch)")) return rc;
+  k_image_final<<<(nfoc + 127) / 128, 128, 0, c->stream>>>(part, d_image, nfoc, nchunk);
+  ++c->launches;
+  return check_cuda(c, cudaGetLastError(), "k_image_final (static scratch)");
 }
 
 }  // extern "C"
