@@ -205,13 +205,14 @@ def traffic_entry(cfg_k, regime):
     return d.get("entries", d).get(f"config{cfg_k}_regime{regime}"), d.get("source")
 
 
-def roofline_of(cfg, nb, nbytes, regime_used, syn_n, syn_ms, ms_total, clocks, share=1.0):
+def roofline_of(cfg, nb, nbytes, regime_used, syn_n, syn_ms, ms_total, clocks, share=1.0, syn_total=None):
     """Roofline of the dominant kernel (the contraction) from the CUDA events the library records on its own stream."""
     peaks = measured_peaks()
     avg_ms = syn_ms / max(syn_n, 1)
     traffic, traffic_src = traffic_entry(cfg.k, regime_used)
-    common = {"traffic": traffic, "traffic_source": traffic_src, "launches_timed": int(syn_n), "avg_launch_ms": avg_ms,
-              "share_of_step": syn_ms / ms_total}
+    syn_total = syn_n if syn_total is None else syn_total     # launches in the timed region; syn_n of them carried events
+    common = {"traffic": traffic, "traffic_source": traffic_src, "launches_timed": int(syn_n), "launches": int(syn_total),
+              "avg_launch_ms": avg_ms, "share_of_step": avg_ms * syn_total / ms_total}
     if regime_used == 1:
         ach = share * nbytes / (avg_ms * 1e-3) / 1e9
         return {"bound": "hbm", "kernel": "k_syn_gemv", "achieved": ach, "peak": peaks["hbm_gbs"], "unit": "GB/s",
@@ -257,16 +258,17 @@ def device_fields(cfg, dev):
     return {nm: (field() if (shared is None or nm in ("f1plus", "f1min")) else shared) for nm in FIELDS}
 
 
-def timed_steps(mk, run_step, steps, warmup, local, dist=None, barrier=None):
+def timed_steps(mk, run_step, steps, warmup, local, dist=None, barrier=None, stride=1):
     """W untimed warm-up steps, then exactly K steps between CUDA events (device time, max over ranks), clocks sampled
-    during the timed region, contraction launches timed by the library's own events."""
+    during the timed region, contraction launches timed by the library's own events (every `stride`-th launch: an event
+    record between two kernels costs ~3 us and keeps them from overlapping, which a step of 34 short launches feels)."""
     import torch
     from paper_2106_04649_b200 import binding as B
     if barrier is None:
         barrier = torch.cuda.synchronize
     for _ in range(warmup):
         run_step()
-    mk.set_option(B.MK_OPT_TIMING, 1)
+    mk.set_option(B.MK_OPT_TIMING, stride)
     mk.get_info(B.MK_INFO_SYN_RESET)
     l0 = mk.get_info(B.MK_INFO_KERNEL_LAUNCHES)
     barrier()
@@ -282,6 +284,7 @@ def timed_steps(mk, run_step, steps, warmup, local, dist=None, barrier=None):
     ms_total = shard.max_over_ranks(e0.elapsed_time(e1), dist)
     res = {"ms_total": ms_total, "clocks": clocks, "launches": int(mk.get_info(B.MK_INFO_KERNEL_LAUNCHES) - l0),
            "syn_n": mk.get_info(B.MK_INFO_SYN_LAUNCHES), "syn_ms": mk.get_info(B.MK_INFO_SYN_MS_TOTAL),
+           "syn_total": mk.get_info(B.MK_INFO_SYN_COUNT),
            "regime_used": int(mk.get_info(B.MK_INFO_REGIME_USED))}
     mk.set_option(B.MK_OPT_TIMING, 0)
     return res
@@ -364,9 +367,9 @@ def variant_entry(cfg, R, Gd, td, steps, warmup, local, dev, rhat_format=0, resi
     dGd, dtd = torch.from_numpy(Gd).to(dev), torch.from_numpy(td).to(dev)
     douts = {nm: torch.empty((cfg.nfoc, cfg.n, cfg.nt), dtype=torch.float32, device=dev) for nm in FIELDS}
     h0 = mk.get_info(B.MK_INFO_H2D_BYTES)
-    r = timed_steps(mk, lambda: mk.run(dGd, dtd, cfg.niter, douts), steps, warmup, local)
+    r = timed_steps(mk, lambda: mk.run(dGd, dtd, cfg.niter, douts), steps, warmup, local, stride=5 if rhat_format == 1 else 1)
     ms = r["ms_total"] / steps
-    passes = r["syn_n"] / steps
+    passes = r["syn_total"] / steps
     avg_ms = r["syn_ms"] / max(r["syn_n"], 1)
     stored = mk.get_info(B.MK_INFO_RHAT_BYTES_STORED) * cfg.n / mk.get_info(B.MK_INFO_LD_SHOT)     # unpadded bytes as stored
     entry = {"workload": f"config{cfg.k}:{cfg.name}", "n": cfg.n, "nt": cfg.nt, "nfoc": cfg.nfoc, "niter": cfg.niter, "nb": nb,
@@ -382,7 +385,8 @@ def variant_entry(cfg, R, Gd, td, steps, warmup, local, dev, rhat_format=0, resi
                       "roofline": {"bound": "hbm", "kernel": "k_syn_gemv_q16", "achieved": ach, "peak": peaks["hbm_gbs"], "unit": "GB/s",
                                    "frac": ach / peaks["hbm_gbs"], "peak_source": peaks["source"] + " copy bandwidth (MEASURED_PEAKS.json)",
                                    "fp32_equivalent_GBps": nbytes / (avg_ms * 1e-3) / 1e9, "traffic": None,
-                                   "launches_timed": int(r["syn_n"]), "avg_launch_ms": avg_ms, "share_of_step": r["syn_ms"] / r["ms_total"]}})
+                                   "launches_timed": int(r["syn_n"]), "launches": int(r["syn_total"]), "avg_launch_ms": avg_ms,
+                                   "share_of_step": avg_ms * r["syn_total"] / r["ms_total"]}})
     else:
         h2d = (mk.get_info(B.MK_INFO_H2D_BYTES) - h0) / (steps + warmup)       # bytes of R^ over the host link per step
         link = h2d_peak_gbs(dev)
@@ -470,10 +474,11 @@ def run_ours(args):
         torch.cuda.synchronize()
 
     # ---- device-timed region: inputs resident in HBM
-    r = timed_steps(mk, run_step, args.steps, args.warmup, local, dist, barrier)
+    r = timed_steps(mk, run_step, args.steps, args.warmup, local, dist, barrier, stride=args.timing_stride)
     ms_total, clocks, launches, syn_n, syn_ms, regime_used = (r[k] for k in ("ms_total", "clocks", "launches", "syn_n", "syn_ms", "regime_used"))
+    syn_total = r["syn_total"]
     jobs = 1 if rows_mode else world        # rows: the ranks share ONE job (strong scaling)
-    passes = syn_n / max(args.steps, 1)     # contraction launches = passes over R^ per step (17 with the fused finals, else 18)
+    passes = syn_total / max(args.steps, 1)  # contraction launches = passes over R^ per step (17 with the fused finals, else 18)
     value = jobs * passes * nbytes * args.steps / (ms_total * 1e-3) / 1e9          # bytes of R^ actually streamed
     value_alg = jobs * nsyn * nbytes * args.steps / (ms_total * 1e-3) / 1e9        # one R^ per synthesis of Algorithm 1
 
@@ -509,7 +514,7 @@ def run_ours(args):
         return 0
 
     share = len(my_rows) / cfg.n            # rows mode: this rank's launches contract its own rows of R^ only
-    roof = roofline_of(cfg, nb, nbytes, regime_used, syn_n, syn_ms, ms_total, clocks, share)
+    roof = roofline_of(cfg, nb, nbytes, regime_used, syn_n, syn_ms, ms_total, clocks, share, syn_total)
 
     # ---- the oracle as it stands, on this box's host cores, bounded sample (rank 0, N = 1 only)
     cpu = None
@@ -578,6 +583,8 @@ def run_ours(args):
                                 "syntheses of the finals share ONE pass over R^ (2 nfoc right-hand sides), so a step makes niter + 1 passes"
                                 if passes < nsyn else "one pass over R^ per synthesis"),
                        "rhat_bytes": nbytes, "regime": regime_used,
+                       "kernel_timing": f"every {args.timing_stride}-th contraction launch of the timed region carries CUDA events "
+                                        f"({int(syn_n)} of {int(syn_total)}; MK_OPT_TIMING = {args.timing_stride})",
                        "l2": f"inputs_larger_than_L2 (R^ {nbytes / 1e9:.2f} GB vs 126 MB L2; no flush needed)",
                        "input_source": "device generator, 64-shot chunks (no e2e / cpu_baseline legs)" if big else "host arrays",
                        "parallelism": "1 GPU" if world == 1 and not rows_mode else
@@ -610,6 +617,9 @@ def main():
                          "stream memory operations (mk_sync_barrier), no host synchronisation inside a step")
     ap.add_argument("--rhat-layout", type=int, default=1, help="layout of R^ for the tensor-regime workloads (MK_OPT_RHAT_LAYOUT): "
                     "1 tiled in 16 KB boxes (default), 0 row-major")
+    ap.add_argument("--timing-stride", type=int, default=5,
+                    help="headline run: every N-th contraction launch of the timed region carries CUDA events (MK_OPT_TIMING = N; 17 "
+                         "launches per config-1 step, so 5 walks through every position of the step)")
     ap.add_argument("--tune", type=int, default=0, help="MK_OPT_TUNE bit mask (measurement switches of the kernels; include/mk.h)")
     ap.add_argument("--e2e-steps", type=int, default=50)
     ap.add_argument("--cpu-budget", type=float, default=15.0, help="seconds of oracle work for cpu_baseline")

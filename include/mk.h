@@ -60,7 +60,9 @@ enum {
   MK_OPT_REGIME = 2,      /* contraction kernel: 0 auto (default: 1 for nfoc <= 8, else 3), 1 streaming GEMV,
                              2 FP32-FFMA GEMM, 3 tcgen05 3xTF32 GEMM with chunked fp32 accumulation (sm_100 only;
                              MK_ERR_INVALID_ARG otherwise).  Affects runs / syntheses started afterwards */
-  MK_OPT_TIMING = 3,      /* 1: bracket every contraction launch with CUDA events on the context's stream */
+  MK_OPT_TIMING = 3,      /* N >= 1: bracket every N-th contraction launch with CUDA events on the context's stream (1: every
+                             one; a record between two kernels costs ~3 us and keeps them from overlapping, so a sparse
+                             sample disturbs a step of many short launches less); 0: off */
   MK_OPT_FUSED_FINALS = 5, /* 1 (default): with 1, 2 or 4 focal points mk_finish / mk_run compute the extra syntheses of G^- and
                              G^+ in ONE pass over R^ (2 nfoc right-hand sides, streaming GEMV); 0: one pass each */
   MK_OPT_FFT_PATH = 4,    /* transform kernels: 0 auto (default), 1 generic shared-memory passes (any nt),
@@ -89,7 +91,10 @@ enum {
                              128 = no A tile is loaded, 256 = no B tile is loaded.  512: the raw B ring has 3 slots; 1024: the CTAs
                              that share an A tile keep in step through global progress counters (same results, slower); 2048: the
                              fused pass of nt = 4096 takes eight traces per CTA (512 threads, one CTA per SM) instead of four
-                             (same results, same speed) */
+                             (same results, same speed); 4096: no kernel is launched with programmatic dependent launch
+                             (same results; the launch gaps of the short kernels come back: +0.01 .. 0.04 ms per config-1 step);
+                             8192: the kernels do nothing ahead of griddepcontrol.wait (no twiddle tables pulled into L1 by the
+                             few-trace FFT kernels, no L2 prefetch of the first rows of R^ by the streaming GEMV; same results) */
 };
 
 /* mk_get_info keys (values returned as double) */
@@ -111,7 +116,8 @@ enum {
   MK_INFO_WINDOW_ROWS = 15,  /* rows per streaming window (0: R^ is resident) */
   MK_INFO_H2D_BYTES = 16,    /* bytes of R^ the contractions have copied host -> device since mk_create_streamed */
   MK_INFO_RHAT_BYTES_STORED = 17, /* bytes R^ occupies as stored (padded): 8 per element, 4.25 with MK_OPT_RHAT_FORMAT = 1 */
-  MK_INFO_RHAT_LAYOUT = 18   /* MK_OPT_RHAT_LAYOUT as set */
+  MK_INFO_RHAT_LAYOUT = 18,  /* MK_OPT_RHAT_LAYOUT as set */
+  MK_INFO_SYN_COUNT = 19     /* contraction launches since the last MK_INFO_SYN_RESET, timed or not */
 };
 
 /* Create a context for an nshot x nrec x nt reflection response sampled at dt (s) and dx (m), band fmin..fmax (Hz).

@@ -16,7 +16,7 @@ MK_OK, MK_ERR_INVALID_ARG, MK_ERR_STATE, MK_ERR_OOM, MK_ERR_CUDA = 0, -1, -2, -3
 MK_OPT_EPS_SAMPLES, MK_OPT_REGIME, MK_OPT_TIMING, MK_OPT_FFT_PATH, MK_OPT_FUSED_FINALS, MK_OPT_RHAT_FORMAT, MK_OPT_TUNE, MK_OPT_RHAT_LAYOUT = 1, 2, 3, 4, 5, 6, 7, 8
 (MK_INFO_NB, MK_INFO_KLO, MK_INFO_KHI, MK_INFO_RHAT_BYTES, MK_INFO_RHAT_BYTES_PADDED, MK_INFO_LD_SHOT,
  MK_INFO_SHOTS_LOADED, MK_INFO_SYN_LAUNCHES, MK_INFO_SYN_MS_TOTAL, MK_INFO_SYN_RESET, MK_INFO_KERNEL_LAUNCHES,
- MK_INFO_REGIME_USED, MK_INFO_DEVICE_BYTES, MK_INFO_RESIDENT_ROWS, MK_INFO_WINDOW_ROWS, MK_INFO_H2D_BYTES, MK_INFO_RHAT_BYTES_STORED, MK_INFO_RHAT_LAYOUT) = range(1, 19)
+ MK_INFO_REGIME_USED, MK_INFO_DEVICE_BYTES, MK_INFO_RESIDENT_ROWS, MK_INFO_WINDOW_ROWS, MK_INFO_H2D_BYTES, MK_INFO_RHAT_BYTES_STORED, MK_INFO_RHAT_LAYOUT, MK_INFO_SYN_COUNT) = range(1, 20)
 REGIME_AUTO, REGIME_GEMV, REGIME_GEMM_FFMA, REGIME_GEMM_TF32X3 = 0, 1, 2, 3
 
 # every symbol include/mk.h declares

@@ -174,7 +174,8 @@ int contract(mk_ctx* c, int slot, float2* Shat, int nfoc, int ldf, int regime) {
   if (c->operand_stale[slot])
     return set_err(c, MK_ERR_STATE, "row-sharded context: the operand rows were not exchanged (mk_operand / mk_operand_exchanged)");
   cudaEvent_t e0 = nullptr, e1 = nullptr;
-  bool timed = c->timing != 0;
+  bool timed = c->timing > 0 && c->syn_count % (size_t)c->timing == 0;   // MK_OPT_TIMING = N: every N-th contraction
+  ++c->syn_count;
   if (timed && c->ev_used + 2 > c->ev.size()) {
     if (c->ev.size() >= 65536) timed = false;  // pool full: later launches go untimed (read / reset the counters)
     else
@@ -566,7 +567,8 @@ int mk_set_option(mk_ctx* c, int key, double value) {
       c->regime = (int)value;
       return MK_OK;
     case MK_OPT_TIMING:
-      c->timing = value != 0.0;
+      if (value < 0 || value != std::floor(value) || value > 65536) return set_err(c, MK_ERR_INVALID_ARG, "MK_OPT_TIMING: 0 (off) or a stride 1 .. 65536");
+      c->timing = (int)value;
       return MK_OK;
     case MK_OPT_FUSED_FINALS:
       c->fused_finals = value != 0.0;
@@ -665,7 +667,8 @@ int mk_get_info(mk_ctx* c, int key, double* value) {
       *value = tot;
       return MK_OK;
     }
-    case MK_INFO_SYN_RESET: c->ev_used = 0; *value = 0; return MK_OK;
+    case MK_INFO_SYN_RESET: c->ev_used = 0; c->syn_count = 0; *value = 0; return MK_OK;
+    case MK_INFO_SYN_COUNT: *value = (double)c->syn_count; return MK_OK;
     case MK_INFO_KERNEL_LAUNCHES: *value = (double)c->launches; return MK_OK;
     case MK_INFO_REGIME_USED: *value = c->last_regime; return MK_OK;
     case MK_INFO_DEVICE_BYTES: *value = (double)c->device_bytes; return MK_OK;
@@ -1107,16 +1110,23 @@ int mk_run_host(mk_ctx* c, const float* h_Gd, const float* h_td, int nfoc, int n
   if (int rc = check_cuda(c, cudaMemcpyAsync(d_field, h_Gd, ntime * sizeof(float), cudaMemcpyHostToDevice, c->stream), "H2D G_d")) return rc;
   if (int rc = check_cuda(c, cudaMemcpyAsync(d_td, h_td, ntd * sizeof(float), cudaMemcpyHostToDevice, c->stream), "H2D t_d")) return rc;
   if (int rc = mk_begin(c, d_field, d_td, nfoc)) return rc;
+  float* hosts[5] = {ho->f1plus, ho->f1min, ho->G, ho->Gplus, ho->Gminus};
+  // Step i adds to f1min (i even) or to f1plus (i odd): the accumulator the LAST step does not touch is final one step
+  // earlier, and its copy to the host overlaps that last step instead of waiting behind it.
+  const int early = (niter >= 1 && overlap) ? ((niter - 1) % 2 == 0 ? 0 : 1) : -1;
   for (int i = 0; i < niter; ++i) {
-    const bool last = (i == niter - 1) && ho->N_last;
-    if (int rc = mk_step(c, last ? d_field : nullptr)) return rc;
+    const bool last = i == niter - 1;
+    if (last && early >= 0 && hosts[early]) {
+      if (int rc = hand_over()) return rc;
+      if (int rc = check_cuda(c, cudaMemcpyAsync(hosts[early], early == 0 ? c->acc_plus : c->acc_min, ntime * sizeof(float), cudaMemcpyDeviceToHost, cs), "D2H accumulator")) return rc;
+    }
+    if (int rc = mk_step(c, last && ho->N_last ? d_field : nullptr)) return rc;
   }
   if (int rc = hand_over()) return rc;
   if (ho->N_last)
     if (int rc = check_cuda(c, cudaMemcpyAsync(ho->N_last, d_field, ntime * sizeof(float), cudaMemcpyDeviceToHost, cs), "D2H N_last")) return rc;
-  float* hosts[5] = {ho->f1plus, ho->f1min, ho->G, ho->Gplus, ho->Gminus};
   for (int i = 0; i < 5; ++i) {
-    if (!hosts[i]) continue;
+    if (!hosts[i] || i == early) continue;
     if (i == 0 || i == 1) {  // accumulators go straight from the library's buffers (the finals only read them)
       const float* src = i == 0 ? c->acc_plus : c->acc_min;
       if (int rc = check_cuda(c, cudaMemcpyAsync(hosts[i], src, ntime * sizeof(float), cudaMemcpyDeviceToHost, cs), "D2H accumulator")) return rc;

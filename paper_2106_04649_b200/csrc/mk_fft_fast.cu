@@ -58,6 +58,7 @@ struct FastParams {
   int nt, n, nb, klo, ld, ldf, nfoc;
   int tiled;  // k_load_R_fast: layout of R^ (rhat_index)
   int r0;  // first receiver row of this context (row sharding): grid row b handles receiver r0 + b
+  int warm;  // warm_tables (off with MK_OPT_TUNE bit 13)
 };
 
 // natural index k (0 <= k < M) of Z -> float2 offset inside the trace's shared-memory block
@@ -79,6 +80,23 @@ __device__ __forceinline__ void trace_sync(int tl) {
       case 6: asm volatile("bar.sync 7, %0;" ::"n"(32 * HF) : "memory"); break;
       default: asm volatile("bar.sync 8, %0;" ::"n"(32 * HF) : "memory"); break;
     }
+  }
+}
+
+// Few traces (every CTA of the launch resident at once: the kernel is one latency chain per warp): the twiddle tables, written
+// once at mk_create, are pulled into this SM's L1 while the kernel in front is still draining (before pdl_wait; constant
+// data only: anything a kernel of the run writes may still be in flight there).
+__device__ __forceinline__ void warm_tables(const FastParams& P, bool on) {
+  if (!on || gridDim.x * gridDim.y > 2048u) return;
+  const float4* t1 = reinterpret_cast<const float4*>(P.tw1k);
+  for (int i = threadIdx.x; i < 512; i += blockDim.x) {
+    const float4 v = __ldg(t1 + i);
+    asm volatile("" ::"f"(v.x), "f"(v.y), "f"(v.z), "f"(v.w));
+  }
+  const float4* t2 = reinterpret_cast<const float4*>(P.tw + (P.klo & ~1));
+  for (int i = threadIdx.x; i < (P.nb + 3) / 2; i += blockDim.x) {
+    const float4 v = __ldg(t2 + i);
+    asm volatile("" ::"f"(v.x), "f"(v.y), "f"(v.z), "f"(v.w));
   }
 }
 
@@ -373,6 +391,9 @@ template <int HF>
 __global__ void __launch_bounds__(256 * HF, 3 - HF)
 k_load_R_fast(const float* __restrict__ Rt, float2* __restrict__ Rhat, FastParams P, int shot0, int nshots, int lgST) {
   extern __shared__ float2 smem[];
+  pdl_trigger();  // the next kernel's CTAs may take the SMs this kernel's last wave leaves free ...
+  warm_tables(P, P.warm != 0);
+  pdl_wait();     // ... and this one touches global memory only after the kernel in front of it has completed
   constexpr int TS = Geo<HF>::TS;
   const int ST = 1 << lgST, r = P.r0 + blockIdx.y, g0 = blockIdx.x * ST;
   const int ns = min(ST, nshots - g0);
@@ -409,6 +430,9 @@ template <int HF>
 __global__ void __launch_bounds__(256 * HF, 3 - HF)
 k_fwd_fast(const float* __restrict__ src, const __grid_constant__ OperandOut O, FastParams P, int lgFT, int conj_out, float* __restrict__ init_Tsrc) {
   extern __shared__ float2 smem[];
+  pdl_trigger();  // the next kernel's CTAs may take the SMs this kernel's last wave leaves free ...
+  warm_tables(P, P.warm != 0);
+  pdl_wait();     // ... and this one touches global memory only after the kernel in front of it has completed
   constexpr int TS = Geo<HF>::TS;
   const int FT = 1 << lgFT, r = P.r0 + blockIdx.y, f0 = blockIdx.x * FT;
   const int nf = min(FT, P.nfoc - f0), nt = P.nt;
@@ -448,6 +472,9 @@ __global__ void __launch_bounds__(256 * HF, 3 - HF)
 k_inv_fast(const float2* __restrict__ spec, FastParams P, int lgFT, float* __restrict__ out, float sS,
            const float* __restrict__ A, float sA, const float* __restrict__ B, float sB) {
   extern __shared__ float2 smem[];
+  pdl_trigger();  // the next kernel's CTAs may take the SMs this kernel's last wave leaves free ...
+  warm_tables(P, P.warm != 0);
+  pdl_wait();     // ... and this one touches global memory only after the kernel in front of it has completed
   constexpr int TS = Geo<HF>::TS;
   const int FT = 1 << lgFT, r = P.r0 + blockIdx.y, f0 = blockIdx.x * FT;
   const int nf = min(FT, P.nfoc - f0), nt = P.nt;
@@ -500,6 +527,9 @@ k_post_fast(const float2* __restrict__ Shat, float2* __restrict__ phat, const __
             float* __restrict__ f1plus, float* __restrict__ f1min, FastParams P, int lgFT, int parity_even,
             float* __restrict__ Ni_out, int pf_dist) {
   extern __shared__ float2 smem[];
+  pdl_trigger();  // the next kernel's CTAs may take the SMs this kernel's last wave leaves free ...
+  warm_tables(P, P.warm != 0);
+  pdl_wait();     // ... and this one touches global memory only after the kernel in front of it has completed
   constexpr int TS = Geo<HF>::TS;
   const int FT = 1 << lgFT, r = P.r0 + blockIdx.y, f0 = blockIdx.x * FT;
   const int nf = min(FT, P.nfoc - f0), nt = P.nt;
@@ -600,6 +630,7 @@ FastParams make_fast(const mk_ctx* c, int nfoc, int ldf) {
   P.nfoc = nfoc;
   P.tiled = c->rhat_layout;
   P.r0 = c->r0;
+  P.warm = (c->tune & 8192) ? 0 : 1;
   return P;
 }
 
@@ -635,10 +666,10 @@ bool fast_fft_ok(const mk_ctx* c) { return (c->nt == 2048 || c->nt == 4096) && c
   do {                                                                               \
     if (c->nt == 2048) {                                                             \
       if (int rc = set_smem(c, KERN<1>, (SH).smem)) return rc;                       \
-      KERN<1><<<GRID, (SH).threads, (SH).smem, c->stream>>>(__VA_ARGS__);            \
+      if (int rc = check_cuda(c, launch_pdl(c, KERN<1>, GRID, (SH).threads, (SH).smem, __VA_ARGS__), #KERN)) return rc; \
     } else {                                                                         \
       if (int rc = set_smem(c, KERN<2>, (SH).smem)) return rc;                       \
-      KERN<2><<<GRID, (SH).threads, (SH).smem, c->stream>>>(__VA_ARGS__);            \
+      if (int rc = check_cuda(c, launch_pdl(c, KERN<2>, GRID, (SH).threads, (SH).smem, __VA_ARGS__), #KERN)) return rc; \
     }                                                                                \
     ++c->launches;                                                                   \
     return check_cuda(c, cudaGetLastError(), #KERN);                                 \

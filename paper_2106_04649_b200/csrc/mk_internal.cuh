@@ -123,6 +123,7 @@ struct mk_ctx {
   // timing of contraction launches
   std::vector<cudaEvent_t> ev;  // pairs
   size_t ev_used = 0;
+  size_t syn_count = 0;  // contraction launches since MK_INFO_SYN_RESET, timed or not
 
   std::string err;
   int sticky = 0;
@@ -148,6 +149,33 @@ __host__ __device__ __forceinline__ size_t rhat_index(int tiled, int rr, int kk,
   const int row = rr & 127, c = (s & 15) >> 1;
   return ((((size_t)(rr >> 7) * nb + kk) * (ld >> 4) + (s >> 4)) * 128 + row) * 16 + (size_t)(((c ^ (row & 7)) << 1) | (s & 1));
 }
+
+// Programmatic dependent launch (the chain of one iteration is launch-latency and drain bound when the focal points are few:
+// 34 kernels of 3 .. 190 us per config-1 step).  A kernel launched through launch_pdl may be scheduled as soon as every CTA
+// of the kernel in front of it on the stream has called pdl_trigger() (or has exited), i.e. while that kernel's last wave is
+// still running; pdl_wait() then blocks until the kernel in front has COMPLETED and its writes are visible.  Rule kept
+// everywhere: a kernel is launched through launch_pdl only if it calls pdl_wait() before its first access to global memory
+// that any earlier kernel writes or still reads (tables written once at mk_create may be read earlier); kernels launched
+// with <<< >>> keep the full serialisation.  MK_OPT_TUNE bit 12 launches everything without the attribute.
+#ifdef __CUDACC__
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+__device__ __forceinline__ void pdl_trigger() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+
+template <typename... KArgs, typename... Args>
+inline cudaError_t launch_pdl(const mk_ctx* c, void (*kern)(KArgs...), dim3 grid, dim3 block, size_t smem, Args&&... args) {
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = grid;
+  cfg.blockDim = block;
+  cfg.dynamicSmemBytes = smem;
+  cfg.stream = c->stream;
+  cudaLaunchAttribute at[1];
+  at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  at[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = at;
+  cfg.numAttrs = (c->tune & 4096) ? 0 : 1;
+  return cudaLaunchKernelEx(&cfg, kern, static_cast<KArgs>(args)...);
+}
+#endif
 
 // a block of consecutive receiver rows of R^ as one launch sees it: Rhat points at row r0 (its [nrow][nb][ld] block may be
 // the resident part, a streaming window, or the mapped host part during ingest); S^ is indexed by the global receiver

@@ -48,8 +48,21 @@ __device__ __forceinline__ void cfma(float2& acc, float ar, float ai, float2 b) 
 // grid (nb, ceil(n / kRowsPerCta)).  Rhat [n][nb][ld], Nhat [nb][ld][NFOC], Shat [n][nb][NFOC].
 template <int NFOC>
 __global__ void __launch_bounds__(kThreads, Tune<NFOC>::kMinBlocks) k_syn_gemv(const float2* __restrict__ Rhat, const float2* __restrict__ Nhat,
-                                                       float2* __restrict__ Shat, int n, int nb, int ld) {
+                                                       float2* __restrict__ Shat, int n, int nb, int ld, int early_pf) {
   extern __shared__ float4 smem4[];
+  pdl_trigger();
+  if ((int)(blockIdx.y * gridDim.x + blockIdx.x) < early_pf) {   // the CTAs of the first wave: the others start long after the wait
+    // R^ never changes during a run: the head of the first rows of every warp starts its way from HBM to L2 while the kernel
+    // in front (which produces N^) is still draining.  A cache hint only: nothing is read before the wait.
+    const int w0 = blockIdx.y * kRowsPerCta + (threadIdx.x >> 5) * Tune<NFOC>::kRows;
+#pragma unroll
+    for (int i = 0; i < Tune<NFOC>::kRows; ++i) {
+      const float2* rp = Rhat + ((size_t)min(w0 + i, n - 1) * nb + blockIdx.x) * ld;
+      const int c = threadIdx.x & 31;   // 4 KB per row: what the first loads of the chunk loop ask for
+      if (c < (ld >> 4)) asm volatile("prefetch.global.L2 [%0];" ::"l"(rp + 16 * c));
+    }
+  }
+  pdl_wait();   // N^ is the output of the kernel in front (mk_internal.cuh: launch_pdl)
   // N^ bin column in shared memory.  A lane always reads the four shots 4c .. 4c+3 of its 256-bit chunk c, so the natural
   // [shot][focal] order puts the lanes 32 NFOC bytes apart: for NFOC = 4, 8 every lane of a warp hits the same banks
   // (measured: 436 / 778 us against 210 us at NFOC = 3).  NFOC >= 4 therefore keeps x as [focal][e][chunk]: the lanes of
@@ -122,7 +135,7 @@ int launch_t(mk_ctx* c, const RowBlock& rb, const float2* d_Nhat, float2* d_Shat
     return rc;
   // the block holds the rows r0 .. r0 + nrow - 1 of R^; S^ is indexed by the global receiver
   const dim3 grid(c->nb, (rb.nrow + kRowsPerCta - 1) / kRowsPerCta);
-  kern<<<grid, kThreads, smem, c->stream>>>(rb.Rhat, d_Nhat, d_Shat + (size_t)rb.r0 * c->nb * NFOC, rb.nrow, c->nb, c->ld);
+  if (int rc = check_cuda(c, launch_pdl(c, kern, grid, dim3(kThreads), smem, rb.Rhat, d_Nhat, d_Shat + (size_t)rb.r0 * c->nb * NFOC, rb.nrow, c->nb, c->ld, (c->tune & 8192) ? 0 : c->num_sms * Tune<NFOC>::kMinBlocks), "k_syn_gemv")) return rc;
   ++c->launches;
   return check_cuda(c, cudaGetLastError(), "k_syn_gemv");
 }

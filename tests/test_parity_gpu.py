@@ -128,6 +128,19 @@ def test_config0_host_api_and_run_match_steps():
     np.testing.assert_array_equal(b["N_last"], c["N_last"])
 
 
+@pytest.mark.parametrize("niter", [1, 2, 3])
+def test_host_api_equals_device_api_for_odd_and_even_step_counts(niter):
+    """mk_run_host copies the accumulator that the last step does not touch (f1plus after an odd number of steps, f1min after
+    an even one) to the host while that step runs: both parities, and a single step, give the bits of mk_run."""
+    cfg = calibrated(configs.scaled(2, n=40, nt=256, nfoc=5, focal="fan:300", niter=niter))
+    R, Gd, td = problem(cfg)
+    b = gpu_chain(cfg, R, Gd, td, keep_iters=False)
+    c = gpu_chain(cfg, R, Gd, td, host_api=True)
+    for nm in FINALS + ("N_last",):
+        assert np.abs(b[nm]).max() > 0, nm
+        np.testing.assert_array_equal(b[nm], c[nm])
+
+
 def test_image_matches_oracle():
     """NEXT-1: double-focusing image of a small multi-focal run against the oracle's definition."""
     import torch
