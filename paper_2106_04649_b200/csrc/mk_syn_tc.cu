@@ -116,8 +116,17 @@ constexpr int kThreads = 128 + kSplitGroups * kSplitThreads + 32 * kReadWarps;  
 // Register budget per warpgroup (setmaxnreg): launched at 80 registers per thread (768 x 80 = 61440 is the CTA's pool); the
 // control warpgroup gives most of its share back and the read-out warps, who hold 96 running sums each, take it:
 // 128 x 32 + 384 x 64 + 256 x 128 = 61440.  (Two split groups: 640 threads at 96; 128 x 32 + 256 x 72 + 256 x 152.)
-constexpr int kRegsControl = 32, kRegsSplit = kSplitGroups == 3 ? 64 : 72, kRegsRead = kSplitGroups == 3 ? 128 : 152;
-constexpr int kChunk = 4 / kSub;  // stages per accumulation chunk (24 MMA steps)
+// (Four split groups, -DMK_TC_SPLIT_GROUPS=4: 896 threads at 72 = 64512; 128 x 32 + 512 x 56 + 256 x 120 = 63488.  Measured: no
+// gain - narrow batches 347 us against 340, config 2 4.25 ms per contraction against 4.12: three groups already keep up.)
+constexpr int kRegsControl = 32, kRegsSplit = kSplitGroups == 3 ? 64 : (kSplitGroups == 4 ? 56 : 72),
+              kRegsRead = kSplitGroups == 3 ? 128 : (kSplitGroups == 4 ? 120 : 152);
+#ifndef MK_TC_READ16
+#define MK_TC_READ16 1
+#endif
+#ifndef MK_TC_CHUNK
+#define MK_TC_CHUNK (4 / kSub)
+#endif
+constexpr int kChunk = MK_TC_CHUNK;  // stages per accumulation chunk (24 MMA steps)
 #ifndef MK_TC_A_LDG
 #define MK_TC_A_LDG 0
 #endif
@@ -193,6 +202,40 @@ __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
     if (clock64() - t0 > MK_MBAR_TIMEOUT_CYCLES) __trap();
 #endif
   }
+}
+// MK_TC_PROBE = 1 (diagnosis only): every role of CTA 0 sums the clocks it spends in each of its waits and prints them.
+// Round 2, config 2 (8106 stages on CTA 0, 835 clk per stage): the producers wait 73 %, the relay 85 %, the read-out
+// warps 49 %, the MMA issuer 42 % (35 % for a stage to become ready, 7 % for a drained accumulator); the split groups wait
+// 28 % (6 % + 6 % for raw tiles that are long there, 16 % for the operand stage to come free) and WORK the rest: ~1800 clk
+// per stage and group (narrow batches: ~1040), i.e. 600 clk per stage over three groups against 576 clk of MMAs.  The
+// split warps pace the kernel; a fourth group does not help (the groups share the schedulers and the shared-memory pipe,
+// 61 % and 70 % busy in ncu), so the next step is less split work per stage, not more warps.
+#ifndef MK_TC_PROBE
+#define MK_TC_PROBE 0
+#endif
+#if MK_TC_PROBE
+#define PROBE_DECL long long pw_[3] = {0, 0, 0}; const long long pt0_ = clock64()
+#define PROBE_WAIT(i, ...) do { const long long a_ = clock64(); __VA_ARGS__; pw_[i] += clock64() - a_; } while (0)
+#define PROBE_PRINT(name) do { if (blockIdx.x == 0) printf("%-12s total %9lld  wait0 %9lld  wait1 %9lld  wait2 %9lld\n", name, clock64() - pt0_, pw_[0], pw_[1], pw_[2]); } while (0)
+#else
+#define PROBE_DECL
+#define PROBE_WAIT(i, ...) do { __VA_ARGS__; } while (0)
+#define PROBE_PRINT(name)
+#endif
+// A whole warp waiting on one barrier costs ~150 clk even when the phase is long complete (measured with MK_TC_PROBE: the
+// three waits of a split group are ~450 of the ~2500 clk it spends per stage).  MK_TC_WARP_WAIT = 1 lets one lane wait and
+// the others join it at a __syncwarp: SLOWER (CTA 0 of config 2: 7.60 M clk against 6.77 M; narrow batches 812 k against
+// 680 k), the divergence costs more than the 31 redundant try_waits.  Off.
+#ifndef MK_TC_WARP_WAIT
+#define MK_TC_WARP_WAIT 0
+#endif
+__device__ __forceinline__ void mbar_wait_warp(uint64_t* bar, uint32_t parity) {
+#if MK_TC_WARP_WAIT
+  if ((threadIdx.x & 31) == 0) mbar_wait(bar, parity);
+  __syncwarp();
+#else
+  mbar_wait(bar, parity);
+#endif
 }
 // shared-memory counters that carry readiness to the MMA-issuing thread (see the header: no mbarrier there)
 __device__ __forceinline__ void flag_add(uint32_t* p) {
@@ -276,6 +319,18 @@ __device__ __forceinline__ void tmem_ld8(uint32_t taddr, uint32_t* v) {
                : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7])
                : "r"(taddr)
                : "memory");
+}
+
+// sixteen columns with one instruction (MK_TC_READ16 = 1, the default: the read-out of a chunk is a chain of load -> wait ->
+// add round trips and the issuer waits for it two chunks later; half as many round trips: narrow batches 340 -> 327 us,
+// 128 / 256 focal points on config 1's R^ 987 -> 973 / 1642 -> 1624 us; same sums in the same order)
+__device__ __forceinline__ void tmem_ld16(uint32_t taddr, uint32_t* v) {
+  asm volatile(
+      "tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15}, [%16];"
+      : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]), "=r"(v[8]), "=r"(v[9]),
+        "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15])
+      : "r"(taddr)
+      : "memory");
 }
 
 // shared-memory matrix descriptor (tcgen05): start >> 4 | LBO >> 4 << 16 | SBO >> 4 << 32 | version 1 << 46 | layout << 61
@@ -438,6 +493,7 @@ k_syn_gemm_tf32x3(const __grid_constant__ CUtensorMap tmA, const __grid_constant
       uint32_t ph = 0;  // ring position and its phase
       const int KB2 = KB * kSub / 2;  // A boxes per tile
       uint32_t q = 0;   // boxes asked for so far
+      PROBE_DECL;
       const int sib0 = (int)blockIdx.x - (int)blockIdx.x % P.ntl;
       constexpr uint32_t kLead = 16, kEvery = 8;  // looked at every 8th box only: a look is ntl - 1 round trips to L2
       for (int t = blockIdx.x; t < ntiles; t += gridDim.x) {
@@ -459,7 +515,7 @@ k_syn_gemm_tf32x3(const __grid_constant__ CUtensorMap tmA, const __grid_constant
               }
             }
           }
-          mbar_wait(emptyA + a, ph ^ 1);
+          PROBE_WAIT(0, mbar_wait(emptyA + a, ph ^ 1));
           if (P.tune & (64 | 128)) {
             mbar_arrive(fullA + a);
           } else {
@@ -478,6 +534,7 @@ k_syn_gemm_tf32x3(const __grid_constant__ CUtensorMap tmA, const __grid_constant
           }
         }
       }
+      PROBE_PRINT("A producer");
     }
   } else if (warp == 1) {
     // ------------------------------------------------------------------------------------ MMA issuer
@@ -493,17 +550,18 @@ k_syn_gemm_tf32x3(const __grid_constant__ CUtensorMap tmA, const __grid_constant
     const uint32_t loB_hi0 = base16 | ((BLK_BYTES >> 4) << 16), loB_lo0 = loB_hi0 + (REG >> 4);  // (K step 1: + 32)
     const uint32_t tmA0 = tmem_base + kTmemA;
     uint32_t g = 0, it = 0;  // global chunk index; global stage index
+    PROBE_DECL;
     for (int t = blockIdx.x; t < ntiles; t += gridDim.x) {
       const int rem = t % per_bin, ni = rem % P.ntl;
       const uint32_t idesc = instr_desc((uint32_t)(tile_col0(P, ni + 1) - tile_col0(P, ni)));  // a multiple of 32, <= BN
       for (int kb0 = 0; kb0 < KB; kb0 += kChunk, ++g) {
         const int b = g & 1;
-        if (g >= 2) flag_wait_ge(drained + b, kReadWarps * (g >> 1));  // every earlier chunk of this buffer has been read out
+        if (g >= 2) PROBE_WAIT(0, flag_wait_ge(drained + b, kReadWarps * (g >> 1)));  // every earlier chunk of this buffer has been read out
         const uint32_t d = tmem_base + (uint32_t)b * BN;
         const int kb1 = min(kb0 + kChunk, KB);
         for (int kb = kb0; kb < kb1; ++kb) {
           const uint32_t s = it & (kTmemSlots - 1);
-          flag_wait_ge(ready + s, (it >> kLgSlots) + 1);
+          PROBE_WAIT(1, flag_wait_ge(ready + s, (it >> kLgSlots) + 1));
           __syncwarp();  // the lanes leave the polling loop one by one: elect.sync needs them all back
           tc_fence_after();
           const uint32_t off = s * stage16, ta = tmA0 + s * kTmemAStage;
@@ -530,6 +588,7 @@ k_syn_gemm_tf32x3(const __grid_constant__ CUtensorMap tmA, const __grid_constant
         __syncwarp();
       }
     }
+    if (lane == 0) PROBE_PRINT("MMA issuer");
   } else if (warp == 2) {
     // ------------------------------------------------------------------------------------ relay
     // Readiness of a stage reaches the MMA warp through a shared-memory word, not through the mbarrier (header).  The
@@ -539,12 +598,14 @@ k_syn_gemm_tf32x3(const __grid_constant__ CUtensorMap tmA, const __grid_constant
     asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(kRegsControl));
     if (lane == 0) {
       uint32_t it = 0;
+      PROBE_DECL;
       for (int t = blockIdx.x; t < ntiles; t += gridDim.x)
         for (int kb = 0; kb < KB; ++kb, ++it) {
           const uint32_t s = it & (kTmemSlots - 1);
-          mbar_wait(split_bar + s, (it >> kLgSlots) & 1);
+          PROBE_WAIT(0, mbar_wait(split_bar + s, (it >> kLgSlots) & 1));
           flag_set(ready + s, (it >> kLgSlots) + 1);
         }
+      PROBE_PRINT("relay");
     }
   } else if (warp == 3) {
     // ------------------------------------------------------------------------------------ TMA producer of the B tiles
@@ -554,10 +615,11 @@ k_syn_gemm_tf32x3(const __grid_constant__ CUtensorMap tmA, const __grid_constant
     if (lane == 0) {
       int s = 0;
       uint32_t ph = 0;
+      PROBE_DECL;
       for (int t = blockIdx.x; t < ntiles; t += gridDim.x) {
         const int kk = t / per_bin, rem = t - kk * per_bin, ni = rem % P.ntl;
         for (int kb = 0; kb < KB; ++kb) {
-          mbar_wait(emptyB + s, ph ^ 1);
+          PROBE_WAIT(0, mbar_wait(emptyB + s, ph ^ 1));
           if (P.tune & (64 | 256)) {
             mbar_arrive(fullB + s);
           } else {
@@ -572,6 +634,7 @@ k_syn_gemm_tf32x3(const __grid_constant__ CUtensorMap tmA, const __grid_constant
           }
         }
       }
+      PROBE_PRINT("B producer");
     }
   } else if (warp < kFirstReadWarp) {
     // ------------------------------------------------------------------------------------ split warps
@@ -610,6 +673,7 @@ k_syn_gemm_tf32x3(const __grid_constant__ CUtensorMap tmA, const __grid_constant
     int tile_i = grp / KB, kb = grp % KB, tile_seen = -1;
     const float4* a_row = nullptr;
     static_assert(!(kALdg && kSub == 2), "direct global loads of A exist for 8-shot stages only");
+    PROBE_DECL;
     for (uint32_t it = grp; it < total; it += kSplitGroups) {
       // 8-shot stages: stage it is half it % 2 of box it / 2; 16-shot stages: stage it is box it
       const uint32_t box = kSub == 2 ? it : it >> 1, half0 = kSub == 2 ? 0u : (it & 1) << 6;
@@ -647,8 +711,8 @@ k_syn_gemm_tf32x3(const __grid_constant__ CUtensorMap tmA, const __grid_constant
           mbar_arrive(split_bar + s);
         }
       } else {
-      if (!kALdg) mbar_wait(fullA + sa, pha);
-      mbar_wait(fullB + rb, phb);
+      if (!kALdg) PROBE_WAIT(0, mbar_wait_warp(fullA + sa, pha));
+      PROBE_WAIT(1, mbar_wait_warp(fullB + rb, phb));
       const uint32_t raw = raw_base + (uint32_t)rb * RAW, st = planes_base + s * PLANES, ta = a_tmem + s * kTmemAStage;
 #pragma unroll
       for (int h = 0; h < kSub; ++h) {  // the 8-shot sub-stages of the stage
@@ -663,7 +727,7 @@ k_syn_gemm_tf32x3(const __grid_constant__ CUtensorMap tmA, const __grid_constant
         // The operand stage (B planes, A slot) is free once the MMAs of stage it - 4 have retired: empty[s] cannot run a
         // second phase ahead, its next completion belongs to stage it itself.
         if (h == 0 && it >= kTmemSlots) {
-          mbar_wait(empty + s, ((it >> kLgSlots) - 1) & 1);
+          PROBE_WAIT(2, mbar_wait_warp(empty + s, ((it >> kLgSlots) - 1) & 1));
           tc_fence_after();
         }
         // B: raw tile -> B0_hi (copy), B0_lo, and B1 = i B0 (every float4 holds two (re, im) pairs) hi / lo
@@ -701,12 +765,14 @@ k_syn_gemm_tf32x3(const __grid_constant__ CUtensorMap tmA, const __grid_constant
         phb ^= 1;
       }
     }
+    if (wt == 0) PROBE_PRINT(grp == 0 ? "split g0" : (grp == 1 ? "split g1" : "split g2+"));
   } else {
     // ------------------------------------------------------------------------------------ read-out warps: chunk sums in registers
     asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(kRegsRead));
     const int quad = warp & 3;         // TMEM lanes 32 quad .. 32 quad + 31 are the ones this warp may read
     const int half = (warp - kFirstReadWarp) >> 2;  // columns (BN / 2) half .. + BN / 2 - 1 of the tile
     uint32_t g = 0;
+    PROBE_DECL;
     for (int t = blockIdx.x; t < ntiles; t += gridDim.x) {
       const int kk = t / per_bin, rem = t - kk * per_bin, mi = rem / P.ntl, ni = rem - mi * P.ntl;
       const int col0 = tile_col0(P, ni);
@@ -716,9 +782,21 @@ k_syn_gemm_tf32x3(const __grid_constant__ CUtensorMap tmA, const __grid_constant
       for (int i = 0; i < BN / 2; ++i) sum[i] = 0.f;
       for (int kb0 = 0; kb0 < KB; kb0 += kChunk, ++g) {
         const int b = g & 1;
-        mbar_wait(acc_full + b, (g >> 1) & 1);
+        PROBE_WAIT(0, mbar_wait_warp(acc_full + b, (g >> 1) & 1));
         tc_fence_after();
         const uint32_t ta = tmem_base + ((uint32_t)(quad * 32) << 16) + (uint32_t)(b * BN + half * (BN / 2));
+#if MK_TC_READ16   // (two such loads in flight per wait spill in the 128-register budget: 331 us / 1684 us, slower)
+#pragma unroll
+        for (int c = 0; c < BN / 32; ++c) {
+          if (c * 16 < cols && !(P.tune & 4)) {  // warp-uniform (the MMA's N is a multiple of 32); columns past it hold stale data
+            uint32_t v[16];
+            tmem_ld16(ta + (uint32_t)(c * 16), v);
+            asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+#pragma unroll
+            for (int q = 0; q < 16; ++q) sum[c * 16 + q] += __uint_as_float(v[q]);
+          }
+        }
+#else
 #pragma unroll
         for (int c = 0; c < BN / 16; ++c) {
           if (c * 8 < cols && !(P.tune & 4)) {  // warp-uniform; columns past the MMA's N hold stale data
@@ -729,6 +807,7 @@ k_syn_gemm_tf32x3(const __grid_constant__ CUtensorMap tmA, const __grid_constant
             for (int q = 0; q < 8; ++q) sum[c * 8 + q] += __uint_as_float(v[q]);
           }
         }
+#endif
         tc_fence_before();
         __syncwarp();
         if (lane == 0) flag_add(drained + b);
@@ -742,6 +821,7 @@ k_syn_gemm_tf32x3(const __grid_constant__ CUtensorMap tmA, const __grid_constant
             *reinterpret_cast<float4*>(dst + q * 4) = make_float4(sum[4 * q], sum[4 * q + 1], sum[4 * q + 2], sum[4 * q + 3]);
       }
     }
+    if (warp == kFirstReadWarp && lane == 0) PROBE_PRINT("read-out w0");
   }
 
   tc_fence_before();
