@@ -222,6 +222,23 @@ __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
 #define PROBE_WAIT(i, ...) do { __VA_ARGS__; } while (0)
 #define PROBE_PRINT(name)
 #endif
+// non-blocking look at a barrier's phase (the two raw-tile barriers of a stage are asked together, see the split warps)
+__device__ __forceinline__ uint32_t mbar_test(uint64_t* bar, uint32_t parity) {
+  uint32_t done;
+  asm volatile(
+      "{\n\t.reg .pred p;\n\t"
+      "mbarrier.test_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+      "selp.u32 %0, 1, 0, p;\n\t}"
+      : "=r"(done)
+      : "r"(smem_u32(bar)), "r"(parity)
+      : "memory");
+  return done;
+}
+// (MK_TC_TEST2 = 1.  Measured: neutral - narrow batches 327.6 us against 327, 128 focal points 955 against 973, config 2
+// 4.09 ms per contraction against 4.12, inside the run-to-run spread; off.)
+#ifndef MK_TC_TEST2
+#define MK_TC_TEST2 0
+#endif
 // A whole warp waiting on one barrier costs ~150 clk even when the phase is long complete (measured with MK_TC_PROBE: the
 // three waits of a split group are ~450 of the ~2500 clk it spends per stage).  MK_TC_WARP_WAIT = 1 lets one lane wait and
 // the others join it at a __syncwarp: SLOWER (CTA 0 of config 2: 7.60 M clk against 6.77 M; narrow batches 812 k against
@@ -711,8 +728,18 @@ k_syn_gemm_tf32x3(const __grid_constant__ CUtensorMap tmA, const __grid_constant
           mbar_arrive(split_bar + s);
         }
       } else {
+#if MK_TC_TEST2
+      // The raw rings run stages ahead, so both tiles are normally long there - but a wait costs ~150 clk even then: the two
+      // are asked in one go (independent instructions, their latencies overlap); only a tile that is really missing is waited for.
+      {
+        const uint32_t okA = kALdg ? 1u : mbar_test(fullA + sa, pha), okB = mbar_test(fullB + rb, phb);
+        if (!okA) PROBE_WAIT(0, mbar_wait_warp(fullA + sa, pha));
+        if (!okB) PROBE_WAIT(1, mbar_wait_warp(fullB + rb, phb));
+      }
+#else
       if (!kALdg) PROBE_WAIT(0, mbar_wait_warp(fullA + sa, pha));
       PROBE_WAIT(1, mbar_wait_warp(fullB + rb, phb));
+#endif
       const uint32_t raw = raw_base + (uint32_t)rb * RAW, st = planes_base + s * PLANES, ta = a_tmem + s * kTmemAStage;
 #pragma unroll
       for (int h = 0; h < kSub; ++h) {  // the 8-shot sub-stages of the stage

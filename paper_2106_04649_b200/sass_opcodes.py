@@ -11,7 +11,7 @@ import sys
 
 from .build import OBJ
 
-ALWAYS = re.compile(r"UTC|LDTM|STTM|UTMA|SYNCS|RED|ATOM|LDG|STG|LDS|STS|LDGSTS|SETMAXREG|FENCE|NANOSLEEP|HMMA|ELECT|FFMA|MUFU")
+ALWAYS = re.compile(r"UTC|LDTM|STTM|UTMA|SYNCS|RED|ATOM|LDG|STG|LDS|STS|LDGSTS|SETMAXREG|FENCE|NANOSLEEP|HMMA|ELECT|FFMA|MUFU|PREEXIT|ACQBULK|CCTL")
 INSTR = re.compile(r"^\s+/\*[0-9a-f]+\*/\s+(?:@!?U?P\d+\s+)?([A-Z][A-Za-z0-9_.]*)")
 
 
