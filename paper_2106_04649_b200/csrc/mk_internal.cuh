@@ -151,7 +151,7 @@ __host__ __device__ __forceinline__ size_t rhat_index(int tiled, int rr, int kk,
 }
 
 // Programmatic dependent launch (the chain of one iteration is launch-latency and drain bound when the focal points are few:
-// 34 kernels of 3 .. 190 us per config-1 step).  A kernel launched through launch_pdl may be scheduled as soon as every CTA
+// 40 kernels of 3 .. 190 us per config-1 step).  A kernel launched through launch_pdl may be scheduled as soon as every CTA
 // of the kernel in front of it on the stream has called pdl_trigger() (or has exited), i.e. while that kernel's last wave is
 // still running; pdl_wait() then blocks until the kernel in front has COMPLETED and its writes are visible.  Rule kept
 // everywhere: a kernel is launched through launch_pdl only if it calls pdl_wait() before its first access to global memory
