@@ -13,7 +13,12 @@ namespace {
 
 constexpr int kThreads = 256;
 constexpr int kWarps = kThreads / 32;
-constexpr int kRowsPerCta = 64;  // receivers per CTA
+// receivers per CTA (measured, config-1 step over three 40-step runs: 32 rows 3.440 / 3.465 / 3.486 ms, 64 rows 3.429 / 3.455 /
+// 3.476, 128 rows 3.460 / 3.485 / 3.509)
+#ifndef MK_GEMV_ROWS_PER_CTA
+#define MK_GEMV_ROWS_PER_CTA 64
+#endif
+constexpr int kRowsPerCta = MK_GEMV_ROWS_PER_CTA;  // receivers per CTA
 // Rows of R^ a warp streams at once (x reuse, independent load streams), unroll of the chunk loop (loads in flight per
 // stream) and CTAs per SM.  Measured on B200, config 1 (nfoc = 1, 1.30 GB of R^): (4, 2, 3) 6.81 TB/s, (4, 1, 4) 7.00,
 // (2, 4, 4) 7.03; a pure read of the same bytes peaks at 7.70 TB/s.  Larger NFOC: registers decide (accumulators =
